@@ -1,0 +1,159 @@
+/* include/vr.h — C ABI of libvr: ray-casting volume rendering of float32 spectral cubes on one
+ * B200 (sm_100a).  The boundary of BASELINE.json `north_star` item (1): "a small C-ABI library
+ * (upload_cube, set_view, set_transfer_function, render_mip, render_ea, composite_bricks) whose
+ * calls follow the paper's statement of the problem" - data file + orientation + colour map +
+ * output size -> image (section 2 "colour map"; lines 37-45 section 3 "a static
+ * image of the current data file with the same orientation information but with a different
+ * output size (defined by the user)"; line 13 abstract "using the ray-casting algorithm";
+ * line 57 footnote 4, float32 voxels).  SURVEY.md section 8(b) lists the calls; DESIGN.md states
+ * every reading (O-1 ... O-12) the arithmetic follows.
+ *
+ * Conventions
+ *  - Every function returns an int status: 0 = VR_OK, negative = error.  No exceptions, no
+ *    aborts.  `vr_last_error(ctx)` returns the text of the last error of that context.
+ *  - "d_" arguments are DEVICE pointers, "h_" arguments are HOST pointers.  Large buffers (cube,
+ *    meta, frames, partial images) are CALLER-OWNED device memory (e.g. torch tensors); the
+ *    library never allocates O(cube) or O(frame) memory.  It owns only small device scratch:
+ *    the transfer-function tables (8 KiB), counters, the source lists of the generator, the
+ *    descriptors of partial images (<= ~100 B per brick) and, for host uploads, one staging slab.
+ *  - `stream` is a cudaStream_t passed as void* (torch.cuda.current_stream().cuda_stream); work
+ *    is enqueued on it and no call synchronises the device unless stated.  Outputs are valid
+ *    after the caller synchronises the stream.
+ *  - One context per host thread; a context is bound to one device.
+ *  - Voxel (i,j,k) = (RA, Dec, frequency) sits at integer position (i,j,k); the rendered domain
+ *    is the closed box [0,nx-1] x [0,ny-1] x [0,nz-1] (O-1).  Linear cubes are x-fastest.
+ *  - Dimensions need not be multiples of the brick size (1721 x 1721 x 1025);
+ *    edge bricks are partial.  Voxels must be finite.
+ */
+#ifndef VR_H
+#define VR_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vr_ctx vr_ctx;
+
+enum {
+    VR_OK = 0,
+    VR_ERR_INVALID_ARG = -1, /* null pointer, non-positive size, vmax <= vmin, step <= 0, singular matrix */
+    VR_ERR_BUFFER = -2,      /* a caller buffer is too small */
+    VR_ERR_CUDA = -3,        /* a CUDA call failed; text kept in vr_last_error */
+    VR_ERR_STATE = -4,       /* render before cube / view / transfer function were set */
+    VR_ERR_UNSUPPORTED = -5
+};
+enum { VR_MODE_MIP = 0, VR_MODE_EA = 1 };
+
+/* ---- lifetime ------------------------------------------------------------------------------ */
+int vr_create(vr_ctx** out, int device);
+int vr_destroy(vr_ctx* ctx);
+const char* vr_last_error(const vr_ctx* ctx);
+const char* vr_status_string(int status);
+
+/* ---- S0: cube residency (BASELINE.json north_star (2),(4)) -------------- */
+/* Bytes the caller must allocate for the brick-major cube (bricks of bx*by*bz voxels stored with
+ * a one-sided +1 halo, x pitch padded to a multiple of 4 floats) and for its metadata (per-brick
+ * and per-8^3-cell (min,max) over the halo-inclusive voxel set, plus activity bits). */
+int vr_cube_layout(int nx, int ny, int nz, int bx, int by, int bz, size_t* cube_bytes,
+                   size_t* meta_bytes);
+
+/* Rebrick a linear x-fastest float32 cube (host if src_is_device == 0, else device) into d_cube
+ * and compute d_meta.  Host sources are streamed slab by slab through a library staging buffer;
+ * the call returns after the last slab was enqueued (it synchronises `stream` between slabs). */
+int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int ny, int nz,
+                   int bx, int by, int bz, void* d_cube, void* d_meta, void* stream);
+
+/* Device-side generator of the synthetic cubes (north_star (4); recipe SURVEY.md 8(d)):
+ * value(x,y,z) = N(0,1) noise from a counter-based hash of (seed, x + nx (y + ny z))
+ *              + continuum * z / (nz - 1) + sum of the sources whose integer box holds (x,y,z),
+ * zero inside the zero boxes; written brick-major in place, then d_meta is computed. */
+typedef struct {
+    const double* h_sources; /* n_sources x 16 doubles: x0 y0 z0 amp sigma_a sigma_b sigma_z
+                                cos sin gradient xlo xhi ylo yhi zlo zhi (boxes inclusive) */
+    int n_sources;
+    const int* h_zero_boxes; /* n_zero_boxes x 6 ints: xlo xhi ylo yhi zlo zhi (inclusive) */
+    int n_zero_boxes;
+    double continuum;
+} vr_gen_params;
+int vr_generate_cube(vr_ctx* ctx, const vr_gen_params* params, uint64_t seed, int nx, int ny,
+                     int nz, int bx, int by, int bz, void* d_cube, void* d_meta, void* stream);
+
+/* Attach an already resident brick-major cube + meta (e.g. after a context was re-created). */
+int vr_attach_cube(vr_ctx* ctx, int nx, int ny, int nz, int bx, int by, int bz, const void* d_cube,
+                   void* d_meta);
+
+/* Copy brick `brick_id` (= bx_i + gx (by_i + gy bz_i)) without halo, clipped to the cube, x
+ * fastest, into d_dst (device, >= ex*ey*ez floats).  Used to hand cube bytes to a checker. */
+int vr_download_brick(vr_ctx* ctx, int brick_id, float* d_dst, void* stream);
+
+/* ---- S1: per-view / per-TF state (O-2, O-6, O-9) ------------------------ */
+/* mvp: row-major 4x4, clip = M (x,y,z,1)^T in voxel coordinates, GL clip space.  width/height:
+ * the image this matrix maps to.  step_voxels: sampling step Delta.  Resets the viewport to
+ * (0, 0, pitch = width). */
+int vr_set_view(vr_ctx* ctx, const float mvp[16], int width, int height, float step_voxels);
+/* Place the width x height image at pixel (x0, y0) of a larger frame whose rows are pitch_px
+ * pixels apart (5 x 5 panels of 1920 x 1080 in one 9600 x 5400 frame). */
+int vr_set_viewport(vr_ctx* ctx, int x0, int y0, size_t pitch_px);
+/* rgba: 256 entries (r,g,b,a) in [0,1], a = opacity per unit voxel length; values map linearly
+ * from [vmin, vmax] onto entries 0..255, clamped, linear between entries (O-6). */
+int vr_set_transfer_function(vr_ctx* ctx, const float rgba[256 * 4], float vmin, float vmax);
+
+/* ---- S2-S4: the ray marcher, whole frame, one accumulator per ray (O-8 GLOBAL) ------------- */
+/* MIP (O-5): d_out_scalar[(y0+j)*pitch + x0+i] = max over taken samples, or miss_value.  If
+ * d_out_rgba_or_null != NULL it receives the raw transfer function evaluated at that maximum
+ * ((0,0,0,0) for a miss). */
+int vr_render_mip(vr_ctx* ctx, float* d_out_scalar, float* d_out_rgba_or_null, float miss_value,
+                  void* stream);
+/* Emission-absorption (O-7): front-to-back, early ray termination once alpha >= ert_tau
+ * (> 1 disables), result = premultiplied colour over bg, 4 floats per pixel. */
+int vr_render_ea(vr_ctx* ctx, float* d_out_rgba, const float bg[4], float ert_tau, void* stream);
+
+/* ---- S5: sort-last path (north_star: "per-brick partial images are then composited sort-last
+ *      in visibility order"; O-8 SORT-LAST, O-9) ------------------------------------------- */
+typedef struct {
+    int brick;        /* brick id */
+    int x0, y0, w, h; /* screen rectangle in view pixels (inside [0,width) x [0,height)) */
+    void* d_data;     /* device: w*h pixels, row pitch `pitch_px`; EA float4, MIP float */
+    size_t pitch_px;
+} vr_partial;
+
+/* Front-to-back order of the bricks that can contribute under the current view (inside the
+ * frustum; for VR_MODE_EA also active against the transfer function, O-10).  h_order_or_null
+ * receives *n_active brick ids (room for all bricks). */
+int vr_sort_bricks(vr_ctx* ctx, int mode, int* h_order_or_null, int* n_active);
+/* Screen rectangles of n bricks and a packing of their partial images into one arena: fills
+ * h_partials[i] (brick, rect, pitch; d_data = byte OFFSET into the arena) and *arena_bytes. */
+int vr_partial_layout(vr_ctx* ctx, int mode, const int* h_brick_ids, int n, vr_partial* h_partials,
+                      size_t* arena_bytes);
+/* Render the partial image of each listed brick: premultiplied (C_b, A_b) with ERT local to the
+ * brick (EA) or the brick's maximum, -inf where no sample falls in it (MIP). */
+int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* h_partials, int n, float ert_tau,
+                     void* stream);
+/* Fold n partial images in the given order (h_partials[0] in front): over-operator then bg (EA),
+ * max then miss value bg[0] (MIP), into the viewport of d_out. */
+int vr_composite_bricks(vr_ctx* ctx, int mode, const vr_partial* h_partials, int n, float* d_out,
+                        const float bg[4], void* stream);
+
+/* ---- counters (SURVEY.md section 5 "metrics") ---------------------------------------------- */
+typedef struct {
+    int64_t rays;             /* rays that had at least one lattice sample inside the cube */
+    int64_t nominal_samples;  /* lattice samples inside the cube (O-3) */
+    int64_t taken_samples;    /* samples actually interpolated (after skipping and ERT) */
+    int64_t bricks_visited;   /* (ray, brick) or (ray, cell) runs marched */
+    int64_t bricks_skipped;   /* runs skipped by min/max (O-10) */
+    int64_t rays_terminated;  /* rays stopped by ERT */
+    int64_t kernel_launches;  /* kernels launched by this context since the last reset */
+} vr_counters;
+/* Synchronises `stream`, then copies the device counters. */
+int vr_get_counters(vr_ctx* ctx, vr_counters* out, void* stream);
+int vr_reset_counters(vr_ctx* ctx, void* stream);
+/* Options: VR_OPT_SKIP (default 1) turns min/max empty-space skipping on/off (tests assert that
+ * it never changes a frame). */
+enum { VR_OPT_SKIP = 1 };
+int vr_set_option(vr_ctx* ctx, int option, int value);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

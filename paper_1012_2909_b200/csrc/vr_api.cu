@@ -1,0 +1,632 @@
+// Host side of libvr: the C ABI of include/vr.h.  Per-view / per-transfer-function setup
+// (matrix inverse in fp64, opacity-corrected table, brick classification
+// against the table, visibility keys + sort) and the launch plumbing.  No torch types.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+#include "vr_internal.cuh"
+
+using namespace vr;
+
+struct vr_ctx {
+    int device = 0;
+    std::string err;
+    // cube
+    bool has_cube = false;
+    CubeDesc cube{};
+    std::vector<float2> h_brick_mm;
+    // view
+    bool has_view = false;
+    double M[16], Minv[16];
+    ViewDesc view{};
+    // transfer function
+    bool has_tf = false;
+    float tf_raw[1024], tf_baked[1024];
+    float vmin = 0, vmax = 1, scale = 1;
+    float baked_step = -1;
+    bool tables_dirty = true, activity_dirty = true;
+    std::vector<int> h_brick_active;
+    // small device scratch owned by the library
+    float4* d_tf_baked = nullptr;
+    float4* d_tf_raw = nullptr;
+    unsigned long long* d_counters = nullptr;
+    PartialDev* d_partials = nullptr;
+    size_t partials_cap = 0;
+    float* d_stage = nullptr;
+    size_t stage_bytes = 0;
+    int64_t launches = 0;
+    int opt_skip = 1;
+};
+
+namespace {
+
+int fail(vr_ctx* ctx, int code, const std::string& msg) {
+    if (ctx) ctx->err = msg;
+    return code;
+}
+
+int cuda_fail(vr_ctx* ctx, cudaError_t e, const char* where) {
+    return fail(ctx, VR_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+#define VR_CUDA(ctx, call)                                             \
+    do {                                                               \
+        cudaError_t e__ = (call);                                      \
+        if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call);     \
+    } while (0)
+
+// 4x4 inverse by cofactors (adjugate / determinant), fp64.
+bool invert4(const double m[16], double inv[16]) {
+    double a[16];
+    a[0] = m[5] * m[10] * m[15] - m[5] * m[11] * m[14] - m[9] * m[6] * m[15] + m[9] * m[7] * m[14] + m[13] * m[6] * m[11] - m[13] * m[7] * m[10];
+    a[4] = -m[4] * m[10] * m[15] + m[4] * m[11] * m[14] + m[8] * m[6] * m[15] - m[8] * m[7] * m[14] - m[12] * m[6] * m[11] + m[12] * m[7] * m[10];
+    a[8] = m[4] * m[9] * m[15] - m[4] * m[11] * m[13] - m[8] * m[5] * m[15] + m[8] * m[7] * m[13] + m[12] * m[5] * m[11] - m[12] * m[7] * m[9];
+    a[12] = -m[4] * m[9] * m[14] + m[4] * m[10] * m[13] + m[8] * m[5] * m[14] - m[8] * m[6] * m[13] - m[12] * m[5] * m[10] + m[12] * m[6] * m[9];
+    a[1] = -m[1] * m[10] * m[15] + m[1] * m[11] * m[14] + m[9] * m[2] * m[15] - m[9] * m[3] * m[14] - m[13] * m[2] * m[11] + m[13] * m[3] * m[10];
+    a[5] = m[0] * m[10] * m[15] - m[0] * m[11] * m[14] - m[8] * m[2] * m[15] + m[8] * m[3] * m[14] + m[12] * m[2] * m[11] - m[12] * m[3] * m[10];
+    a[9] = -m[0] * m[9] * m[15] + m[0] * m[11] * m[13] + m[8] * m[1] * m[15] - m[8] * m[3] * m[13] - m[12] * m[1] * m[11] + m[12] * m[3] * m[9];
+    a[13] = m[0] * m[9] * m[14] - m[0] * m[10] * m[13] - m[8] * m[1] * m[14] + m[8] * m[2] * m[13] + m[12] * m[1] * m[10] - m[12] * m[2] * m[9];
+    a[2] = m[1] * m[6] * m[15] - m[1] * m[7] * m[14] - m[5] * m[2] * m[15] + m[5] * m[3] * m[14] + m[13] * m[2] * m[7] - m[13] * m[3] * m[6];
+    a[6] = -m[0] * m[6] * m[15] + m[0] * m[7] * m[14] + m[4] * m[2] * m[15] - m[4] * m[3] * m[14] - m[12] * m[2] * m[7] + m[12] * m[3] * m[6];
+    a[10] = m[0] * m[5] * m[15] - m[0] * m[7] * m[13] - m[4] * m[1] * m[15] + m[4] * m[3] * m[13] + m[12] * m[1] * m[7] - m[12] * m[3] * m[5];
+    a[14] = -m[0] * m[5] * m[14] + m[0] * m[6] * m[13] + m[4] * m[1] * m[14] - m[4] * m[2] * m[13] - m[12] * m[1] * m[6] + m[12] * m[2] * m[5];
+    a[3] = -m[1] * m[6] * m[11] + m[1] * m[7] * m[10] + m[5] * m[2] * m[11] - m[5] * m[3] * m[10] - m[9] * m[2] * m[7] + m[9] * m[3] * m[6];
+    a[7] = m[0] * m[6] * m[11] - m[0] * m[7] * m[10] - m[4] * m[2] * m[11] + m[4] * m[3] * m[10] + m[8] * m[2] * m[7] - m[8] * m[3] * m[6];
+    a[11] = -m[0] * m[5] * m[11] + m[0] * m[7] * m[9] + m[4] * m[1] * m[11] - m[4] * m[3] * m[9] - m[8] * m[1] * m[7] + m[8] * m[3] * m[5];
+    a[15] = m[0] * m[5] * m[10] - m[0] * m[6] * m[9] - m[4] * m[1] * m[10] + m[4] * m[2] * m[9] + m[8] * m[1] * m[6] - m[8] * m[2] * m[5];
+    double det = m[0] * a[0] + m[1] * a[4] + m[2] * a[8] + m[3] * a[12];
+    if (det == 0.0 || !std::isfinite(det)) return false;
+    for (int i = 0; i < 16; ++i) {
+        inv[i] = a[i] / det;
+        if (!std::isfinite(inv[i])) return false;
+    }
+    return true;
+}
+
+bool valid_dims(int nx, int ny, int nz, int bx, int by, int bz) {
+    return nx > 0 && ny > 0 && nz > 0 && bx > 0 && by > 0 && bz > 0 &&
+           (long long)nx < (1 << 22) && (long long)ny < (1 << 22) && (long long)nz < (1 << 22);
+}
+
+void bind_meta(CubeDesc& c, const void* d_cube, void* d_meta) {
+    MetaLayout ml = meta_layout(c);
+    char* m = (char*)d_meta;
+    c.cube = (const float*)d_cube;
+    c.brick_mm = (float2*)(m + ml.brick_mm);
+    c.cell_mm = (float2*)(m + ml.cell_mm);
+    c.cell_bits = (unsigned*)(m + ml.cell_bits);
+    c.brick_active = (int*)(m + ml.brick_active);
+}
+
+int finish_cube(vr_ctx* ctx, cudaStream_t s) {
+    CubeDesc& c = ctx->cube;
+    VR_CUDA(ctx, launch_minmax(c, s));
+    ctx->launches += 2;
+    ctx->h_brick_mm.resize(c.nbricks);
+    VR_CUDA(ctx, cudaMemcpyAsync(ctx->h_brick_mm.data(), c.brick_mm, sizeof(float2) * c.nbricks, cudaMemcpyDeviceToHost, s));
+    VR_CUDA(ctx, cudaStreamSynchronize(s));
+    ctx->has_cube = true;
+    ctx->activity_dirty = true;
+    return VR_OK;
+}
+
+// O-6: a'_i = 1 - (1 - a_i)^Delta in fp64, rounded to float32; colours unchanged.
+void bake_tf(vr_ctx* ctx) {
+    const double step = (double)ctx->view.step;
+    for (int i = 0; i < 256; ++i) {
+        for (int ch = 0; ch < 3; ++ch) ctx->tf_baked[4 * i + ch] = ctx->tf_raw[4 * i + ch];
+        ctx->tf_baked[4 * i + 3] = (float)(1.0 - std::pow(1.0 - (double)ctx->tf_raw[4 * i + 3], step));
+    }
+    ctx->baked_step = ctx->view.step;
+}
+
+// O-10: a brick is inactive iff a'_j = 0 for every table index the values of [min, max] can
+// touch, j in [floor(x(min)), ceil(x(max))], x evaluated exactly as the kernel evaluates it.
+bool range_active(const vr_ctx* ctx, float mn, float mx) {
+    if (!(mn <= mx)) return false;                           // empty brick (no voxel of the cube)
+    auto xof = [&](float v) {
+        float x = (v - ctx->vmin) * ctx->scale;
+        return std::fmin(std::fmax(x, 0.f), 255.f);
+    };
+    int lo = (int)std::floor(xof(mn)), hi = (int)std::ceil(xof(mx));
+    lo = std::max(0, std::min(lo, 255)); hi = std::max(0, std::min(hi, 255));
+    for (int j = lo; j <= hi; ++j) if (ctx->tf_baked[4 * j + 3] != 0.f) return true;
+    return false;
+}
+
+int ensure_tables(vr_ctx* ctx, cudaStream_t s) {
+    if (!ctx->has_tf) return VR_OK;
+    if (ctx->tables_dirty || ctx->baked_step != ctx->view.step) {
+        bake_tf(ctx);
+        VR_CUDA(ctx, launch_upload_table(ctx->d_tf_baked, ctx->tf_baked, s));
+        VR_CUDA(ctx, launch_upload_table(ctx->d_tf_raw, ctx->tf_raw, s));
+        ctx->launches += 4;
+        ctx->tables_dirty = false;
+        ctx->activity_dirty = true;
+    }
+    if (ctx->activity_dirty && ctx->has_cube) {
+        const int nb = ctx->cube.nbricks;
+        ctx->h_brick_active.resize(nb);
+        for (int b = 0; b < nb; ++b)
+            ctx->h_brick_active[b] = range_active(ctx, ctx->h_brick_mm[b].x, ctx->h_brick_mm[b].y) ? 1 : 0;
+        // pageable source: cudaMemcpyAsync stages it before returning, so the vector may change later
+        VR_CUDA(ctx, cudaMemcpyAsync(ctx->cube.brick_active, ctx->h_brick_active.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, s));
+        ctx->activity_dirty = false;
+    }
+    return VR_OK;
+}
+
+TFDesc tf_desc(const vr_ctx* ctx) {
+    TFDesc t;
+    t.baked = ctx->d_tf_baked; t.raw = ctx->d_tf_raw; t.vmin = ctx->vmin; t.scale = ctx->scale;
+    return t;
+}
+
+// Screen rectangle (view pixels, clipped) that holds every pixel whose ray can meet brick b.
+// Returns false if the brick is outside the frustum.
+bool brick_rect(const vr_ctx* ctx, int bid, int rect[4]) {
+    const CubeDesc& c = ctx->cube;
+    const int W = ctx->view.W, H = ctx->view.H;
+    int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
+    double lo[3], hi[3];
+    for (int a = 0; a < 3; ++a) {
+        lo[a] = (double)b[a] * c.B[a];
+        hi[a] = std::min((double)(b[a] + 1) * c.B[a], (double)(c.N[a] - 1));
+        if (hi[a] < lo[a]) return false;
+    }
+    double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300, zmin = 1e300, zmax = -1e300;
+    bool behind = false;
+    for (int k = 0; k < 8; ++k) {
+        double p[3] = {(k & 1) ? hi[0] : lo[0], (k & 2) ? hi[1] : lo[1], (k & 4) ? hi[2] : lo[2]};
+        const double* M = ctx->M;
+        double X = M[0] * p[0] + M[1] * p[1] + M[2] * p[2] + M[3];
+        double Y = M[4] * p[0] + M[5] * p[1] + M[6] * p[2] + M[7];
+        double Z = M[8] * p[0] + M[9] * p[1] + M[10] * p[2] + M[11];
+        double Wc = M[12] * p[0] + M[13] * p[1] + M[14] * p[2] + M[15];
+        if (!(Wc > 1e-9)) { behind = true; continue; }
+        double xn = X / Wc, yn = Y / Wc, zn = Z / Wc;
+        xmin = std::min(xmin, xn); xmax = std::max(xmax, xn);
+        ymin = std::min(ymin, yn); ymax = std::max(ymax, yn);
+        zmin = std::min(zmin, zn); zmax = std::max(zmax, zn);
+    }
+    int x0 = 0, x1 = W - 1, y0 = 0, y1 = H - 1;
+    if (!behind) {
+        if (zmin > 1.0 + 1e-6 || zmax < -1.0 - 1e-6) return false;      // beyond far / before near
+        // pixel centre i has xn = 2 (i + 1/2) / W - 1 ; row j has yn = 1 - 2 (j + 1/2) / H
+        x0 = std::max(0, (int)std::floor((xmin + 1.0) * 0.5 * W - 0.5) - 1);
+        x1 = std::min(W - 1, (int)std::ceil((xmax + 1.0) * 0.5 * W - 0.5) + 1);
+        y0 = std::max(0, (int)std::floor((1.0 - ymax) * 0.5 * H - 0.5) - 1);
+        y1 = std::min(H - 1, (int)std::ceil((1.0 - ymin) * 0.5 * H - 0.5) + 1);
+    }
+    if (x1 < x0 || y1 < y0) return false;
+    rect[0] = x0; rect[1] = y0; rect[2] = x1 - x0 + 1; rect[3] = y1 - y0 + 1;
+    return true;
+}
+
+int check_render_state(vr_ctx* ctx, bool need_tf) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (!ctx->has_cube) return fail(ctx, VR_ERR_STATE, "no cube: call vr_upload_cube / vr_generate_cube first");
+    if (!ctx->has_view) return fail(ctx, VR_ERR_STATE, "no view: call vr_set_view first");
+    if (need_tf && !ctx->has_tf) return fail(ctx, VR_ERR_STATE, "no transfer function: call vr_set_transfer_function first");
+    return VR_OK;
+}
+
+int upload_partials(vr_ctx* ctx, int mode, const vr_partial* hp, int n, bool with_tiles, int* total_tiles, cudaStream_t s) {
+    if (n > (int)ctx->partials_cap) {
+        if (ctx->d_partials) cudaFree(ctx->d_partials);
+        ctx->d_partials = nullptr;
+        size_t cap = std::max<size_t>(256, (size_t)n * 2);
+        VR_CUDA(ctx, cudaMalloc(&ctx->d_partials, cap * sizeof(PartialDev)));
+        ctx->partials_cap = cap;
+    }
+    std::vector<PartialDev> v(n);
+    int tiles = 0;
+    const int W = ctx->view.W, H = ctx->view.H;
+    for (int i = 0; i < n; ++i) {
+        const vr_partial& p = hp[i];
+        if (p.brick < 0 || p.brick >= ctx->cube.nbricks || p.w <= 0 || p.h <= 0 || p.x0 < 0 || p.y0 < 0 ||
+            p.x0 + p.w > W || p.y0 + p.h > H || !p.d_data || p.pitch_px < (size_t)p.w)
+            return fail(ctx, VR_ERR_INVALID_ARG, "bad vr_partial entry");
+        if (((uintptr_t)p.d_data & (mode == VR_MODE_EA ? 15 : 3)) != 0)
+            return fail(ctx, VR_ERR_INVALID_ARG, "vr_partial.d_data misaligned");
+        v[i].brick = p.brick; v[i].x0 = p.x0; v[i].y0 = p.y0; v[i].w = p.w; v[i].h = p.h;
+        v[i].pitch = (long long)p.pitch_px; v[i].data = p.d_data; v[i].tile0 = tiles;
+        if (with_tiles) tiles += ((p.w + kTileW - 1) / kTileW) * ((p.h + kTileH - 1) / kTileH);
+    }
+    if (total_tiles) *total_tiles = tiles;
+    if (n > 0) VR_CUDA(ctx, cudaMemcpyAsync(ctx->d_partials, v.data(), sizeof(PartialDev) * n, cudaMemcpyHostToDevice, s));
+    return VR_OK;
+}
+
+}  // namespace
+
+namespace vr {
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz) {
+    std::memset(&c, 0, sizeof(c));
+    int N[3] = {nx, ny, nz}, B[3] = {bx, by, bz};
+    for (int a = 0; a < 3; ++a) {
+        c.N[a] = N[a]; c.B[a] = std::min(B[a], N[a]);
+        c.G[a] = (c.N[a] + c.B[a] - 1) / c.B[a];
+        c.P[a] = c.B[a] + 1;
+        c.sh[a] = -1;
+        for (int s = 0; s < 30; ++s) if ((1 << s) == c.B[a]) c.sh[a] = s;
+        c.C[a] = (c.B[a] + kCell - 1) / kCell;
+    }
+    c.P[0] = (c.P[0] + 3) / 4 * 4;
+    c.nbricks = c.G[0] * c.G[1] * c.G[2];
+    c.cells_per_brick = c.C[0] * c.C[1] * c.C[2];
+    c.cell_words_per_brick = (c.cells_per_brick + 31) / 32;
+    c.stride = (long long)align_up((size_t)c.P[0] * c.P[1] * c.P[2], 32);
+}
+
+size_t cube_bytes(const CubeDesc& c) { return (size_t)c.nbricks * (size_t)c.stride * sizeof(float); }
+
+MetaLayout meta_layout(const CubeDesc& c) {
+    MetaLayout m;
+    size_t off = 0;
+    m.brick_mm = off; off = align_up(off + sizeof(float2) * c.nbricks, 256);
+    m.cell_mm = off; off = align_up(off + sizeof(float2) * (size_t)c.nbricks * c.cells_per_brick, 256);
+    m.cell_bits = off; off = align_up(off + sizeof(unsigned) * (size_t)c.nbricks * c.cell_words_per_brick, 256);
+    m.brick_active = off; off = align_up(off + sizeof(int) * c.nbricks, 256);
+    m.total = off;
+    return m;
+}
+
+}  // namespace vr
+
+extern "C" {
+
+const char* vr_status_string(int status) {
+    switch (status) {
+        case VR_OK: return "VR_OK";
+        case VR_ERR_INVALID_ARG: return "VR_ERR_INVALID_ARG";
+        case VR_ERR_BUFFER: return "VR_ERR_BUFFER";
+        case VR_ERR_CUDA: return "VR_ERR_CUDA";
+        case VR_ERR_STATE: return "VR_ERR_STATE";
+        case VR_ERR_UNSUPPORTED: return "VR_ERR_UNSUPPORTED";
+        default: return "VR_ERR_UNKNOWN";
+    }
+}
+
+const char* vr_last_error(const vr_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int vr_create(vr_ctx** out, int device) {
+    if (!out) return VR_ERR_INVALID_ARG;
+    *out = nullptr;
+    int n = 0;
+    if (cudaGetDeviceCount(&n) != cudaSuccess || device < 0 || device >= n) return VR_ERR_CUDA;
+    vr_ctx* ctx = new vr_ctx();
+    ctx->device = device;
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_tf_baked, 256 * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_tf_raw, 256 * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, kNumCounters * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(ctx->d_counters, 0, kNumCounters * sizeof(unsigned long long));
+    if (e != cudaSuccess) { vr_destroy(ctx); return VR_ERR_CUDA; }
+    *out = ctx;
+    return VR_OK;
+}
+
+int vr_destroy(vr_ctx* ctx) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    cudaSetDevice(ctx->device);
+    if (ctx->d_tf_baked) cudaFree(ctx->d_tf_baked);
+    if (ctx->d_tf_raw) cudaFree(ctx->d_tf_raw);
+    if (ctx->d_counters) cudaFree(ctx->d_counters);
+    if (ctx->d_partials) cudaFree(ctx->d_partials);
+    if (ctx->d_stage) cudaFree(ctx->d_stage);
+    delete ctx;
+    return VR_OK;
+}
+
+int vr_cube_layout(int nx, int ny, int nz, int bx, int by, int bz, size_t* cube_bytes_out, size_t* meta_bytes_out) {
+    if (!valid_dims(nx, ny, nz, bx, by, bz) || !cube_bytes_out || !meta_bytes_out) return VR_ERR_INVALID_ARG;
+    CubeDesc c;
+    fill_cube_desc(c, nx, ny, nz, bx, by, bz);
+    *cube_bytes_out = cube_bytes(c);
+    *meta_bytes_out = meta_layout(c).total;
+    return VR_OK;
+}
+
+int vr_attach_cube(vr_ctx* ctx, int nx, int ny, int nz, int bx, int by, int bz, const void* d_cube, void* d_meta) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (!valid_dims(nx, ny, nz, bx, by, bz) || !d_cube || !d_meta) return fail(ctx, VR_ERR_INVALID_ARG, "vr_attach_cube: bad argument");
+    fill_cube_desc(ctx->cube, nx, ny, nz, bx, by, bz);
+    bind_meta(ctx->cube, d_cube, d_meta);
+    ctx->h_brick_mm.resize(ctx->cube.nbricks);
+    VR_CUDA(ctx, cudaMemcpy(ctx->h_brick_mm.data(), ctx->cube.brick_mm, sizeof(float2) * ctx->cube.nbricks, cudaMemcpyDeviceToHost));
+    ctx->has_cube = true;
+    ctx->activity_dirty = true;
+    return VR_OK;
+}
+
+int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int ny, int nz, int bx, int by,
+                   int bz, void* d_cube, void* d_meta, void* stream) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (!valid_dims(nx, ny, nz, bx, by, bz) || !src || !d_cube || !d_meta) return fail(ctx, VR_ERR_INVALID_ARG, "vr_upload_cube: bad argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    ctx->has_cube = false;
+    CubeDesc& c = ctx->cube;
+    fill_cube_desc(c, nx, ny, nz, bx, by, bz);
+    bind_meta(c, d_cube, d_meta);
+    VR_CUDA(ctx, cudaMemsetAsync(d_cube, 0, cube_bytes(c), s));
+    if (src_is_device) {
+        VR_CUDA(ctx, launch_rebrick(c, (float*)d_cube, src, 0, nz, s));
+        ctx->launches += 1;
+    } else {
+        const size_t plane = (size_t)nx * ny * sizeof(float);
+        size_t want = std::max(plane * (size_t)std::min(nz, c.B[2]), std::min(plane * nz, (size_t)256 << 20));
+        int planes = (int)std::max<size_t>(1, std::min<size_t>((size_t)nz, want / plane));
+        if (ctx->stage_bytes < plane * planes) {
+            if (ctx->d_stage) cudaFree(ctx->d_stage);
+            ctx->d_stage = nullptr; ctx->stage_bytes = 0;
+            VR_CUDA(ctx, cudaMalloc(&ctx->d_stage, plane * planes));
+            ctx->stage_bytes = plane * planes;
+        }
+        for (int z0 = 0; z0 < nz; z0 += planes) {
+            int z1 = std::min(nz, z0 + planes);
+            VR_CUDA(ctx, cudaMemcpyAsync(ctx->d_stage, src + (size_t)z0 * nx * ny, plane * (z1 - z0), cudaMemcpyHostToDevice, s));
+            VR_CUDA(ctx, launch_rebrick(c, (float*)d_cube, ctx->d_stage, z0, z1, s));
+            ctx->launches += 1;
+            VR_CUDA(ctx, cudaStreamSynchronize(s));          // the staging slab is reused
+        }
+    }
+    return finish_cube(ctx, s);
+}
+
+int vr_generate_cube(vr_ctx* ctx, const vr_gen_params* prm, uint64_t seed, int nx, int ny, int nz, int bx,
+                     int by, int bz, void* d_cube, void* d_meta, void* stream) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (!valid_dims(nx, ny, nz, bx, by, bz) || !prm || !d_cube || !d_meta) return fail(ctx, VR_ERR_INVALID_ARG, "vr_generate_cube: bad argument");
+    if (prm->n_sources < 0 || prm->n_zero_boxes < 0 || (prm->n_sources > 0 && !prm->h_sources) ||
+        (prm->n_zero_boxes > 0 && !prm->h_zero_boxes))
+        return fail(ctx, VR_ERR_INVALID_ARG, "vr_generate_cube: bad source / zero-box list");
+    cudaStream_t s = (cudaStream_t)stream;
+    ctx->has_cube = false;
+    CubeDesc& c = ctx->cube;
+    fill_cube_desc(c, nx, ny, nz, bx, by, bz);
+    bind_meta(c, d_cube, d_meta);
+    // bin the sources (ascending id) and the zero boxes over 32^3 tiles of the cube
+    const int T[3] = {(nx + 31) / 32, (ny + 31) / 32, (nz + 31) / 32};
+    const size_t ntile = (size_t)T[0] * T[1] * T[2];
+    std::vector<int> cnt(ntile + 1, 0);
+    std::vector<char> zflag(ntile, 0);
+    auto for_tiles = [&](const double* box, auto&& fn) {
+        int lo[3], hi[3];
+        const int N[3] = {nx, ny, nz};
+        for (int a = 0; a < 3; ++a) {
+            lo[a] = std::max(0, (int)box[2 * a]) >> 5;
+            hi[a] = std::min(N[a] - 1, (int)box[2 * a + 1]) >> 5;
+        }
+        for (int z = lo[2]; z <= hi[2]; ++z) for (int y = lo[1]; y <= hi[1]; ++y) for (int x = lo[0]; x <= hi[0]; ++x)
+            fn((size_t)x + T[0] * ((size_t)y + (size_t)T[1] * z));
+    };
+    for (int i = 0; i < prm->n_sources; ++i) for_tiles(prm->h_sources + 16 * (size_t)i + 10, [&](size_t t) { cnt[t + 1]++; });
+    for (size_t t = 0; t < ntile; ++t) cnt[t + 1] += cnt[t];
+    std::vector<int> ids((size_t)cnt[ntile] + 1), fillp(cnt.begin(), cnt.end() - 1);
+    for (int i = 0; i < prm->n_sources; ++i) for_tiles(prm->h_sources + 16 * (size_t)i + 10, [&](size_t t) { ids[fillp[t]++] = i; });
+    for (int i = 0; i < prm->n_zero_boxes; ++i) {
+        double box[6];
+        for (int k = 0; k < 6; ++k) box[k] = prm->h_zero_boxes[6 * i + k];
+        for_tiles(box, [&](size_t t) { zflag[t] = 1; });
+    }
+    std::vector<int> offs(cnt);
+    for (size_t t = 0; t < ntile; ++t) if (zflag[t]) offs[t] = ~offs[t];
+    double* d_src = nullptr; int* d_offs = nullptr; int* d_ids = nullptr; int* d_zb = nullptr;
+    auto cleanup = [&]() { cudaFree(d_src); cudaFree(d_offs); cudaFree(d_ids); cudaFree(d_zb); };
+    cudaError_t e = cudaMalloc(&d_src, sizeof(double) * 16 * std::max(1, prm->n_sources));
+    if (e == cudaSuccess) e = cudaMalloc(&d_offs, sizeof(int) * offs.size());
+    if (e == cudaSuccess) e = cudaMalloc(&d_ids, sizeof(int) * ids.size());
+    if (e == cudaSuccess) e = cudaMalloc(&d_zb, sizeof(int) * 6 * std::max(1, prm->n_zero_boxes));
+    if (e == cudaSuccess && prm->n_sources) e = cudaMemcpyAsync(d_src, prm->h_sources, sizeof(double) * 16 * prm->n_sources, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_offs, offs.data(), sizeof(int) * offs.size(), cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_ids, ids.data(), sizeof(int) * ids.size(), cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess && prm->n_zero_boxes) e = cudaMemcpyAsync(d_zb, prm->h_zero_boxes, sizeof(int) * 6 * prm->n_zero_boxes, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) {
+        GenDev g;
+        g.sources = d_src; g.tile_offsets = d_offs; g.tile_ids = d_ids;
+        g.tiles[0] = T[0]; g.tiles[1] = T[1]; g.tiles[2] = T[2];
+        g.zero_boxes = d_zb; g.n_zero = prm->n_zero_boxes; g.continuum = prm->continuum; g.seed = seed;
+        e = launch_generate(c, (float*)d_cube, g, s);
+        ctx->launches += 1;
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cleanup();
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "vr_generate_cube");
+    return finish_cube(ctx, s);
+}
+
+int vr_download_brick(vr_ctx* ctx, int brick_id, float* d_dst, void* stream) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (!ctx->has_cube) return fail(ctx, VR_ERR_STATE, "no cube");
+    if (brick_id < 0 || brick_id >= ctx->cube.nbricks || !d_dst) return fail(ctx, VR_ERR_INVALID_ARG, "vr_download_brick: bad argument");
+    VR_CUDA(ctx, launch_unbrick(ctx->cube, brick_id, d_dst, (cudaStream_t)stream));
+    ctx->launches += 1;
+    return VR_OK;
+}
+
+int vr_set_view(vr_ctx* ctx, const float mvp[16], int width, int height, float step) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (!mvp || width <= 0 || height <= 0 || !(step > 0.f) || !std::isfinite(step)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_view: bad argument");
+    double M[16], Minv[16];
+    for (int i = 0; i < 16; ++i) { M[i] = (double)mvp[i]; if (!std::isfinite(M[i])) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_view: non-finite matrix"); }
+    if (!invert4(M, Minv)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_view: singular matrix");
+    std::memcpy(ctx->M, M, sizeof(M)); std::memcpy(ctx->Minv, Minv, sizeof(Minv));
+    std::memcpy(ctx->view.Minv, Minv, sizeof(Minv));
+    ctx->view.W = width; ctx->view.H = height; ctx->view.step = step;
+    ctx->view.vx0 = 0; ctx->view.vy0 = 0; ctx->view.pitch = width;
+    ctx->has_view = true;
+    return VR_OK;
+}
+
+int vr_set_viewport(vr_ctx* ctx, int x0, int y0, size_t pitch_px) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (!ctx->has_view) return fail(ctx, VR_ERR_STATE, "vr_set_viewport before vr_set_view");
+    if (x0 < 0 || y0 < 0 || pitch_px < (size_t)(x0 + ctx->view.W)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_viewport: bad argument");
+    ctx->view.vx0 = x0; ctx->view.vy0 = y0; ctx->view.pitch = (long long)pitch_px;
+    return VR_OK;
+}
+
+int vr_set_transfer_function(vr_ctx* ctx, const float rgba[1024], float vmin, float vmax) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (!rgba || !(vmax > vmin) || !std::isfinite(vmin) || !std::isfinite(vmax)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_transfer_function: bad argument");
+    for (int i = 0; i < 1024; ++i) if (!(rgba[i] >= 0.f && rgba[i] <= 1.f)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_transfer_function: entries must lie in [0,1]");
+    std::memcpy(ctx->tf_raw, rgba, sizeof(ctx->tf_raw));
+    ctx->vmin = vmin; ctx->vmax = vmax;
+    ctx->scale = (float)(255.0 / ((double)vmax - (double)vmin));
+    ctx->has_tf = true; ctx->tables_dirty = true;
+    return VR_OK;
+}
+
+int vr_render_mip(vr_ctx* ctx, float* d_out, float* d_out_rgba, float miss, void* stream) {
+    int rc = check_render_state(ctx, d_out_rgba != nullptr);
+    if (rc) return rc;
+    if (!d_out) return fail(ctx, VR_ERR_INVALID_ARG, "vr_render_mip: null output");
+    cudaStream_t s = (cudaStream_t)stream;
+    if ((rc = ensure_tables(ctx, s))) return rc;
+    RenderArgs a{};
+    a.mode = VR_MODE_MIP; a.tau = 2.f; a.miss = miss; a.skip = ctx->opt_skip;
+    a.out = d_out; a.out_rgba = d_out_rgba; a.counters = ctx->d_counters;
+    VR_CUDA(ctx, launch_render_global(ctx->cube, ctx->view, tf_desc(ctx), a, s));
+    ctx->launches += 1;
+    return VR_OK;
+}
+
+int vr_render_ea(vr_ctx* ctx, float* d_out, const float bg[4], float tau, void* stream) {
+    int rc = check_render_state(ctx, true);
+    if (rc) return rc;
+    if (!d_out || !bg || !(tau > 0.f)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_render_ea: bad argument");
+    if (((uintptr_t)d_out & 15) != 0) return fail(ctx, VR_ERR_INVALID_ARG, "vr_render_ea: output must be 16-byte aligned");
+    cudaStream_t s = (cudaStream_t)stream;
+    if ((rc = ensure_tables(ctx, s))) return rc;
+    RenderArgs a{};
+    a.mode = VR_MODE_EA; a.tau = tau; a.skip = ctx->opt_skip;
+    for (int i = 0; i < 4; ++i) a.bg[i] = bg[i];
+    a.out = d_out; a.counters = ctx->d_counters;
+    VR_CUDA(ctx, launch_render_global(ctx->cube, ctx->view, tf_desc(ctx), a, s));
+    ctx->launches += 1;
+    return VR_OK;
+}
+
+int vr_sort_bricks(vr_ctx* ctx, int mode, int* h_order, int* n_active) {
+    int rc = check_render_state(ctx, mode == VR_MODE_EA);
+    if (rc) return rc;
+    if (!n_active || (mode != VR_MODE_MIP && mode != VR_MODE_EA)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_sort_bricks: bad argument");
+    const CubeDesc& c = ctx->cube;
+    if (mode == VR_MODE_EA && (ctx->tables_dirty || ctx->baked_step != ctx->view.step)) { bake_tf(ctx); ctx->tables_dirty = true; }
+    // O-9: h = Minv (0,0,1,0)^T; perspective eye = h.xyz / h.w, else common direction sign(d)
+    const double* Mi = ctx->Minv;
+    double h[4] = {Mi[2], Mi[6], Mi[10], Mi[14]};
+    double nrm = std::fabs(h[0]) + std::fabs(h[1]) + std::fabs(h[2]);
+    double nmax = (double)std::max(c.N[0], std::max(c.N[1], c.N[2]));
+    bool persp = std::fabs(h[3]) * nmax * 1e9 > nrm;
+    int E[3] = {0, 0, 0}, sg[3] = {0, 0, 0};
+    if (persp) {
+        for (int a = 0; a < 3; ++a) E[a] = (int)std::floor((h[a] / h[3]) / (double)c.B[a]);
+    } else {
+        // direction of the central ray: far point minus near point
+        double pn[4], pf[4];
+        for (int r = 0; r < 4; ++r) { pn[r] = -Mi[4 * r + 2] + Mi[4 * r + 3]; pf[r] = Mi[4 * r + 2] + Mi[4 * r + 3]; }
+        double L = 0, d[3];
+        for (int a = 0; a < 3; ++a) { d[a] = pf[a] / pf[3] - pn[a] / pn[3]; L += d[a] * d[a]; }
+        L = std::sqrt(L);
+        for (int a = 0; a < 3; ++a) sg[a] = d[a] / L > 1e-12 ? 1 : (d[a] / L < -1e-12 ? -1 : 0);
+    }
+    std::vector<std::pair<int, int>> keyed;
+    keyed.reserve(c.nbricks);
+    for (int bid = 0; bid < c.nbricks; ++bid) {
+        int rect[4];
+        if (!brick_rect(ctx, bid, rect)) continue;
+        if (mode == VR_MODE_EA && ctx->opt_skip && !range_active(ctx, ctx->h_brick_mm[bid].x, ctx->h_brick_mm[bid].y)) continue;
+        int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
+        int key = 0;
+        for (int a = 0; a < 3; ++a)
+            key += persp ? std::abs(b[a] - E[a]) : (sg[a] > 0 ? b[a] : (sg[a] < 0 ? c.G[a] - 1 - b[a] : 0));
+        keyed.emplace_back(key, bid);
+    }
+    std::stable_sort(keyed.begin(), keyed.end());
+    *n_active = (int)keyed.size();
+    if (h_order) for (size_t i = 0; i < keyed.size(); ++i) h_order[i] = keyed[i].second;
+    return VR_OK;
+}
+
+int vr_partial_layout(vr_ctx* ctx, int mode, const int* ids, int n, vr_partial* hp, size_t* arena_bytes) {
+    int rc = check_render_state(ctx, false);
+    if (rc) return rc;
+    if (n < 0 || (n > 0 && (!ids || !hp)) || !arena_bytes || (mode != VR_MODE_MIP && mode != VR_MODE_EA))
+        return fail(ctx, VR_ERR_INVALID_ARG, "vr_partial_layout: bad argument");
+    const size_t px_bytes = mode == VR_MODE_EA ? 16 : 4;
+    size_t off = 0;
+    for (int i = 0; i < n; ++i) {
+        if (ids[i] < 0 || ids[i] >= ctx->cube.nbricks) return fail(ctx, VR_ERR_INVALID_ARG, "vr_partial_layout: bad brick id");
+        int rect[4];
+        if (!brick_rect(ctx, ids[i], rect)) { rect[0] = rect[1] = 0; rect[2] = rect[3] = 1; }   // off-screen: 1 px
+        hp[i].brick = ids[i];
+        hp[i].x0 = rect[0]; hp[i].y0 = rect[1]; hp[i].w = rect[2]; hp[i].h = rect[3];
+        hp[i].pitch_px = (size_t)rect[2];
+        hp[i].d_data = (void*)off;
+        off = align_up(off + px_bytes * (size_t)rect[2] * rect[3], 256);
+    }
+    *arena_bytes = off;
+    return VR_OK;
+}
+
+int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float tau, void* stream) {
+    int rc = check_render_state(ctx, mode == VR_MODE_EA);
+    if (rc) return rc;
+    if (n < 0 || (n > 0 && !hp) || (mode != VR_MODE_MIP && mode != VR_MODE_EA) || !(tau > 0.f))
+        return fail(ctx, VR_ERR_INVALID_ARG, "vr_render_bricks: bad argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    if ((rc = ensure_tables(ctx, s))) return rc;
+    int tiles = 0;
+    if ((rc = upload_partials(ctx, mode, hp, n, true, &tiles, s))) return rc;
+    RenderArgs a{};
+    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = ctx->opt_skip; a.counters = ctx->d_counters;
+    VR_CUDA(ctx, launch_render_bricks(ctx->cube, ctx->view, tf_desc(ctx), a, ctx->d_partials, n, tiles, s));
+    ctx->launches += (n > 0 && tiles > 0) ? 1 : 0;
+    return VR_OK;
+}
+
+int vr_composite_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float* d_out, const float bg[4], void* stream) {
+    int rc = check_render_state(ctx, false);
+    if (rc) return rc;
+    if (n < 0 || (n > 0 && !hp) || !d_out || !bg || (mode != VR_MODE_MIP && mode != VR_MODE_EA))
+        return fail(ctx, VR_ERR_INVALID_ARG, "vr_composite_bricks: bad argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    if ((rc = upload_partials(ctx, mode, hp, n, false, nullptr, s))) return rc;
+    VR_CUDA(ctx, launch_composite(ctx->view, mode, ctx->d_partials, n, d_out, bg, s));
+    ctx->launches += 1;
+    return VR_OK;
+}
+
+int vr_get_counters(vr_ctx* ctx, vr_counters* out, void* stream) {
+    if (!ctx || !out) return VR_ERR_INVALID_ARG;
+    unsigned long long h[kNumCounters];
+    cudaStream_t s = (cudaStream_t)stream;
+    VR_CUDA(ctx, cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s));
+    VR_CUDA(ctx, cudaStreamSynchronize(s));
+    out->rays = (int64_t)h[kRays]; out->nominal_samples = (int64_t)h[kNominal]; out->taken_samples = (int64_t)h[kTaken];
+    out->bricks_visited = (int64_t)h[kVisited]; out->bricks_skipped = (int64_t)h[kSkipped];
+    out->rays_terminated = (int64_t)h[kTerminated]; out->kernel_launches = ctx->launches;
+    return VR_OK;
+}
+
+int vr_reset_counters(vr_ctx* ctx, void* stream) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    VR_CUDA(ctx, cudaMemsetAsync(ctx->d_counters, 0, kNumCounters * sizeof(unsigned long long), (cudaStream_t)stream));
+    ctx->launches = 0;
+    return VR_OK;
+}
+
+int vr_set_option(vr_ctx* ctx, int option, int value) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (option == VR_OPT_SKIP) { ctx->opt_skip = value ? 1 : 0; return VR_OK; }
+    return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown option");
+}
+
+}  // extern "C"

@@ -1,0 +1,86 @@
+// Internal declarations shared by the libvr translation units (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/vr.h"
+
+namespace vr {
+
+constexpr int kCell = 8;            // edge of the min/max macro-cells under the configured bricks
+constexpr int kTileW = 16, kTileH = 8, kThreads = 128;   // pixel tile of one CTA: 4 warps of 8x4
+
+// Brick-major cube in HBM.  Brick b = bx + G0 (by + G1 bz) occupies
+// `stride` floats; voxel (lx,ly,lz) of it, 0 <= l <= B (the +1 is the one-sided halo), sits at
+// lx + P0 (ly + P1 lz).  Halo voxels beyond the cube are zero.
+struct CubeDesc {
+    int N[3];        // voxels
+    int B[3];        // configured brick size
+    int G[3];        // brick grid
+    int P[3];        // padded brick extents: P0 = roundup4(B0 + 1), P1 = B1 + 1, P2 = B2 + 1
+    int sh[3];       // log2(B) if B is a power of two, else -1
+    int C[3];        // macro-cells per brick axis = ceil(B / kCell)
+    int nbricks;
+    int cells_per_brick;
+    long long stride;            // floats per brick (multiple of 32)
+    const float* cube;
+    float2* brick_mm;            // (min,max) per brick, halo-inclusive
+    float2* cell_mm;             // (min,max) per macro-cell, halo-inclusive, brick-major
+    unsigned* cell_bits;         // EA activity of macro-cells vs the transfer function, 1 bit each
+    int* brick_active;           // EA activity of bricks vs the transfer function
+    int cell_words_per_brick;
+};
+
+struct ViewDesc {
+    double Minv[16];
+    int W, H;
+    float step;
+    int vx0, vy0;
+    long long pitch;
+};
+
+struct TFDesc {
+    const float4* baked;   // device: opacity-corrected table (O-6)
+    const float4* raw;     // device: raw table
+    float vmin, scale;     // scale = (float)(255 / (vmax - vmin))
+};
+
+struct PartialDev {        // device descriptor of one partial image
+    int brick, x0, y0, w, h, tile0;   // tile0: first CTA tile of this partial in the launch
+    long long pitch;
+    void* data;
+};
+
+enum Counter { kRays = 0, kNominal, kTaken, kVisited, kSkipped, kTerminated, kNumCounters };
+
+size_t align_up(size_t v, size_t a);
+void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz);
+size_t cube_bytes(const CubeDesc& c);
+struct MetaLayout { size_t brick_mm, cell_mm, cell_bits, brick_active, total; };
+MetaLayout meta_layout(const CubeDesc& c);
+
+// kernels' host launchers (vr_cube.cu / vr_march.cu / vr_composite.cu)
+cudaError_t launch_rebrick(const CubeDesc& c, float* d_cube, const float* d_src, int z0, int z1, cudaStream_t s);
+cudaError_t launch_unbrick(const CubeDesc& c, int brick, float* d_dst, cudaStream_t s);
+cudaError_t launch_minmax(const CubeDesc& c, cudaStream_t s);
+struct GenDev {
+    const double* sources; const int* tile_offsets; const int* tile_ids; int tiles[3];
+    const int* zero_boxes; int n_zero; double continuum; uint64_t seed;
+};
+cudaError_t launch_generate(const CubeDesc& c, float* d_cube, const GenDev& g, cudaStream_t s);
+
+struct RenderArgs {
+    int mode; float tau; float bg[4]; float miss; int skip;
+    float* out; float* out_rgba; unsigned long long* counters;
+};
+cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s);
+cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a,
+                                 const PartialDev* d_partials, int n, int total_tiles, cudaStream_t s);
+cudaError_t launch_composite(const ViewDesc& v, int mode, const PartialDev* d_partials, int n, float* out,
+                             const float bg[4], cudaStream_t s);
+cudaError_t launch_upload_table(float4* d_dst, const float* h_src_1024, cudaStream_t s);
+
+}  // namespace vr

@@ -1,0 +1,308 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle
+on the same seeded inputs, element by element.  Tolerances are BASELINE.json's: max-abs <= 1e-4 and
+RMS <= 1e-5 per RGBA channel in [0,1] against the fp64 oracle (MIP after normalising by
+(m - vmin) / (vmax - vmin)), bit-exact for MIP under axis-aligned orthographic views.  Beyond
+that, the kernels implement the canonical float32 arithmetic of SURVEY.md 8(c) O-11, so frames
+are also compared bit-for-bit with the float32 instantiation of the oracle.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1012_2909_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+BG = (0.25, 0.5, 0.125, 0.75)
+
+
+@pytest.fixture(scope="module")
+def H():
+    import helpers
+    helpers.torch_cuda()
+    return helpers
+
+
+def noise_cube(shape, seed=0, scale=1.0):
+    return (np.random.default_rng(seed).normal(size=shape) * scale).astype(np.float32)
+
+
+def bit_fraction(a, b):
+    return float(np.mean(a.view(np.uint32) == b.view(np.uint32)))
+
+
+# ------------------------------------------------------------------------------ S0
+@pytest.mark.parametrize("dims,brick", [((37, 29, 41), (16, 16, 16)), ((64, 64, 64), (64, 64, 64)),
+                                        ((50, 33, 20), (24, 20, 32)), ((8, 8, 8), (16, 16, 16))])
+def test_upload_roundtrip_ragged_bricks(H, dims, brick):
+    cube = noise_cube(dims[::-1], 1)
+    sc = H.Scene(dims, brick, cube=cube)
+    assert np.array_equal(sc.host_cube(), cube)
+    # device-resident source gives the same bricks
+    import torch
+    sc2 = H.Scene.__new__(H.Scene)
+    sc2.__dict__.update(sc.__dict__)
+    d_src = torch.from_numpy(cube).cuda()
+    cb, mb = sc.vr.cube_layout(dims, brick)
+    sc2.d_cube = torch.empty(cb // 4, dtype=torch.float32, device="cuda")
+    sc2.d_meta = torch.empty(mb, dtype=torch.uint8, device="cuda")
+    sc2.ctx = sc.vr.Context(0)
+    sc2.ctx.upload_cube(d_src, dims, brick, sc2.d_cube, sc2.d_meta)
+    sc2._host = None
+    assert np.array_equal(sc2.host_cube(), cube)
+
+
+def test_generator_matches_oracle_and_ignores_brick_size(H):
+    w = wl.scaled(wl.C3, "gen", (96, 80, 128), (32, 32, 32), (64, 64), n_sources=7)
+    S = wl.make_sources(w)
+    zb = np.array([[32, 63, 0, 31, 64, 95], [5, 9, 70, 79, 0, 3]], dtype=np.int32)
+    gen = {"seed": w.seed, "sources": S, "zero_boxes": zb, "continuum": w.continuum}
+    a = H.Scene(w.dims, (32, 32, 32), gen=gen).host_cube()
+    b = H.Scene(w.dims, (24, 16, 40), gen=gen).host_cube()
+    assert np.array_equal(a, b)                     # bytes independent of the brick size
+    from oracle import ovr
+    ref = ovr.generate(w.seed, w.dims, sources=S, zero_boxes=zb, continuum=w.continuum)
+    # both sides evaluate the same fp64 expression and round once to float32; the only freedom
+    # left is the last bit of log / cos / exp in fp64, which can move a float32 rounding
+    ulp = np.spacing(np.abs(ref).astype(np.float32))
+    assert (np.abs(a - ref) <= ulp).all()
+    assert np.mean(a == ref) > 0.9999
+    assert (a[64:96, 0:32, 32:64] == 0).all() and (a[0:4, 70:80, 5:10] == 0).all()
+
+
+# ------------------------------------------------------------------------------ closed forms on the GPU
+def test_mip_axis_aligned_bit_exact(H):
+    # BASELINE.json: "bit-exact for MIP under axis-aligned orthographic views"
+    for dims, brick in [((64, 64, 64), (64, 64, 64)), ((40, 24, 56), (16, 16, 16)), ((33, 20, 17), (8, 12, 8))]:
+        cube = noise_cube(dims[::-1], 3)
+        cube[-1, -1, -1] = 40.0
+        sc = H.Scene(dims, brick, cube=cube)
+        vol = sc.oracle_volume()
+        for axis in range(3):
+            for sign in (1, -1):
+                M, (W, Hh) = wl.axis_ortho_camera(dims, axis, sign)
+                got = sc.render_mip(M, W, Hh, 0.5, miss=-1.0)
+                ua, va = [(1, 2), (0, 2), (0, 1)][axis]
+                assert np.array_equal(got[:dims[va], :dims[ua]], cube.max(axis=2 - axis))
+                assert (got[dims[va]:] == -1.0).all() and (got[:, dims[ua]:] == -1.0).all()
+                ref, _, _ = sc.ovr.render(vol, M, W, Hh, 0.5, sc.ovr.MIP, sc.ovr.F32, miss=-1.0)
+                assert np.array_equal(got, ref)
+
+
+def test_beer_lambert_and_ert_on_gpu(H):
+    dims, step, a = (16, 16, 64), 0.5, 0.15
+    rgb = np.array([0.2, 0.7, 0.5], dtype=np.float32)
+    sc = H.Scene(dims, (16, 16, 16), cube=np.full(dims[::-1], 0.5, dtype=np.float32))
+    t = np.zeros((256, 4), dtype=np.float32); t[:, :3] = rgb; t[:, 3] = a
+    tf = (t, 0.0, 1.0)
+    M, (W, Hh) = wl.axis_ortho_camera(dims, 2, 1)
+    n = math.floor((dims[2] - 1) / step) + 1
+    ap = 1.0 - (1.0 - a) ** step
+    out = sc.render_ea(M, W, Hh, step, tf, tau=2.0)
+    A = 1.0 - (1.0 - ap) ** n
+    assert np.allclose(out[..., 3], A, atol=1e-5) and np.allclose(out[..., :3], rgb * A, atol=1e-5)
+    sc.ctx.reset_counters()
+    out = sc.render_ea(M, W, Hh, step, tf, tau=0.9)
+    nstar = math.ceil(math.log(1.0 - 0.9) / math.log(1.0 - ap))
+    c = sc.ctx.get_counters()
+    assert c["taken_samples"] == nstar * W * Hh and c["rays_terminated"] == W * Hh
+    assert c["nominal_samples"] == n * W * Hh
+    assert (out[..., 3] >= 0.9).all() and (out[..., 3] <= 0.9 + 0.1 * ap + 1e-6).all()
+
+
+def test_empty_cube_renders_background_bit_exact(H):
+    dims = (40, 40, 40)
+    sc = H.Scene(dims, (16, 16, 16), cube=np.zeros(dims[::-1], dtype=np.float32))
+    M = wl.perspective_camera(dims, (70, 50))
+    out = sc.render_ea(M, 70, 50, 0.5, wl.tf_src(), bg=BG, tau=0.99)
+    assert np.array_equal(out, np.broadcast_to(np.array(BG, dtype=np.float32), out.shape))
+    mip = sc.render_mip(M, 70, 50, 0.5, miss=-7.0)
+    assert set(np.unique(mip)) == {0.0, -7.0}
+
+
+# ------------------------------------------------------------------------------ BASELINE.json configs[0] (C1)
+def test_config_c1_parity(H):
+    w = wl.C1
+    sc = H.Scene(w.dims, w.brick, gen={"seed": w.seed, "sources": wl.make_sources(w)})
+    vol, ovr = sc.oracle_volume(), sc.ovr
+    tf = wl.tf_ramp()
+    W, Hh = w.frame
+    for view in range(3):
+        M = wl.config_camera(w, view)
+        got = sc.render_ea(M, W, Hh, w.step, tf, bg=BG, tau=w.tau)
+        o64, fl, _ = ovr.render(vol, M, W, Hh, w.step, ovr.EA, ovr.F64, tf=tf, bg=BG, tau=w.tau)
+        o32, _, _ = ovr.render(vol, M, W, Hh, w.step, ovr.EA, ovr.F32, tf=tf, bg=BG, tau=w.tau)
+        H.compare(got, o64, fl, o32, what=f"C1 EA view {view}")
+        assert bit_fraction(got, o32) == 1.0
+        mip, rgba = sc.render_mip(M, W, Hh, w.step, miss=0.0, tf=tf)
+        m64, fl, _ = ovr.render(vol, M, W, Hh, w.step, ovr.MIP, ovr.F64, miss=0.0)
+        m32, _, _ = ovr.render(vol, M, W, Hh, w.step, ovr.MIP, ovr.F32, miss=0.0)
+        H.compare(mip, m64, fl, m32, mode_mip=True, vmin=tf[1], vmax=tf[2], miss=0.0, what=f"C1 MIP view {view}")
+        assert bit_fraction(mip, m32) == 1.0
+        # MIP colour = raw transfer function at the maximum
+        j, i = np.unravel_index(np.argmax(mip), mip.shape)
+        assert np.allclose(rgba[j, i], ovr.tf_lookup(tf, w.step, float(mip[j, i]), baked=False), atol=1e-6)
+        assert (rgba[mip == 0.0] == 0).all() or (m64 != 0.0).all()
+
+
+# ------------------------------------------------------------------------------ bricked, perspective (C2-like)
+CASES = [
+    ("c2-like", (96, 80, 128), (32, 32, 32), (160, 90), 0.5),
+    ("ragged", (70, 45, 83), (24, 20, 32), (97, 61), 0.5),
+    ("fine-step", (48, 48, 64), (16, 16, 16), (80, 64), 0.25),
+    ("odd-step", (48, 40, 56), (16, 16, 16), (64, 48), 0.3),
+]
+
+
+@pytest.mark.parametrize("name,dims,brick,frame,step", CASES)
+def test_bricked_perspective_parity(H, name, dims, brick, frame, step):
+    w = wl.scaled(wl.C2, name, dims, brick, frame, n_sources=8)
+    sc = H.Scene(dims, brick, gen={"seed": w.seed, "sources": wl.make_sources(w)})
+    vol, ovr = sc.oracle_volume(), sc.ovr
+    W, Hh = frame
+    for az in (30.0, 200.0):
+        M = wl.perspective_camera(dims, frame, azimuth_deg=az)
+        for tfname, tau in (("src", 0.99), ("fog", 0.99), ("fog", 2.0)):
+            tf = wl.TFS[tfname]()
+            got = sc.render_ea(M, W, Hh, step, tf, bg=BG, tau=tau)
+            o64, fl, c64 = ovr.render(vol, M, W, Hh, step, ovr.EA, ovr.F64, tf=tf, bg=BG, tau=tau)
+            o32, _, _ = ovr.render(vol, M, W, Hh, step, ovr.EA, ovr.F32, tf=tf, bg=BG, tau=tau)
+            H.compare(got, o64, fl, o32, what=f"{name} EA {tfname} tau={tau} az={az}")
+            assert bit_fraction(got, o32) == 1.0, f"{name} EA {tfname}: not bit-identical to the float32 oracle"
+        sc.ctx.reset_counters()
+        mip = sc.render_mip(M, W, Hh, step, miss=-3.0)
+        c = sc.ctx.get_counters()
+        m64, fl, c64 = ovr.render(vol, M, W, Hh, step, ovr.MIP, ovr.F64, miss=-3.0)
+        m32, _, c32 = ovr.render(vol, M, W, Hh, step, ovr.MIP, ovr.F32, miss=-3.0)
+        H.compare(mip, m64, fl, m32, mode_mip=True, vmin=0.0, vmax=32.0, miss=-3.0, what=f"{name} MIP az={az}")
+        assert bit_fraction(mip, m32) == 1.0
+        assert c["nominal_samples"] == c32["nominal"]        # integer lattice invariant (O-3)
+
+
+def test_skipping_never_changes_a_frame(H):
+    dims, brick, frame = (96, 96, 96), (16, 16, 16), (120, 90)
+    w = wl.scaled(wl.C2, "skip", dims, brick, frame, n_sources=4)
+    sc = H.Scene(dims, brick, gen={"seed": w.seed, "sources": wl.make_sources(w)})
+    M = wl.perspective_camera(dims, frame)
+    tf = wl.tf_src()
+    res = {}
+    for skip in (1, 0):
+        sc.ctx.set_option(sc.vr.OPT_SKIP, skip)
+        sc.ctx.reset_counters()
+        ea = sc.render_ea(M, *frame, 0.5, tf, bg=BG, tau=0.99)
+        c_ea = sc.ctx.get_counters()
+        sc.ctx.reset_counters()
+        mip = sc.render_mip(M, *frame, 0.5)
+        c_mip = sc.ctx.get_counters()
+        fr, _, ids = sc.render_sortlast(M, *frame, 0.5, sc.vr.MODE_EA, tf=tf, bg=BG, tau=2.0)
+        res[skip] = (ea, mip, c_ea, c_mip, fr, len(ids))
+    assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
+    assert np.array_equal(res[0][4], res[1][4])
+    assert res[1][2]["bricks_skipped"] > 0 and res[0][2]["bricks_skipped"] == 0
+    assert res[1][2]["taken_samples"] < res[0][2]["taken_samples"]
+    assert res[1][3]["taken_samples"] < res[0][3]["taken_samples"]
+    assert res[1][5] < res[0][5]                       # inactive bricks drop out of the sort-last list
+    assert res[1][2]["nominal_samples"] == res[0][2]["nominal_samples"]
+
+
+# ------------------------------------------------------------------------------ S5 sort-last
+@pytest.mark.parametrize("persp", [True, False])
+def test_sort_last_partials_and_composite(H, persp):
+    dims, brick, frame, step = (64, 48, 80), (32, 16, 32), (100, 70), 0.5
+    cube = np.abs(noise_cube(dims[::-1], 5)) * 3.0
+    sc = H.Scene(dims, brick, cube=cube)
+    vol, ovr, vr = sc.oracle_volume(), sc.ovr, sc.vr
+    tf = wl.tf_fog()
+    M = wl.perspective_camera(dims, frame, azimuth_deg=130.0) if persp else \
+        wl.ortho_camera(dims, frame, wl.seeded_directions(3, 1)[0])
+    W, Hh = frame
+    g = sc.grid()
+    for mode, omode in ((vr.MODE_EA, ovr.EA), (vr.MODE_MIP, ovr.MIP)):
+        for tau in ((0.9, 2.0) if mode == vr.MODE_EA else (2.0,)):
+            fr, imgs, ids = sc.render_sortlast(M, W, Hh, step, mode, tf=tf, bg=BG, tau=tau)
+            # visibility order: oracle keys non-decreasing along the library's order (O-9)
+            keys, _ = ovr.visibility_keys(M, W, Hh, step, brick, g)
+            assert (np.diff(keys[ids]) >= 0).all() and len(set(ids)) == len(ids)
+            # a few partial images, bit for bit against the float32 oracle
+            for q in (0, len(imgs) // 2, len(imgs) - 1):
+                p = imgs[q]
+                ref = ovr.render_brick(vol, M, W, Hh, step, omode, p["brick"], p["rect"], brick, ovr.F32, tf=tf, tau=tau)
+                assert np.array_equal(p["image"], ref), (mode, tau, p["brick"])
+            # every pixel outside a brick's rectangle must get nothing from that brick
+            for p in imgs[:3]:
+                full = ovr.render_brick(vol, M, W, Hh, step, omode, p["brick"], (0, 0, W, Hh), brick, ovr.F32, tf=tf, tau=tau)
+                x0, y0, ww, hh = p["rect"]
+                mask = np.ones((Hh, W), bool); mask[y0:y0 + hh, x0:x0 + ww] = False
+                empty = (full[mask] == 0).all() if mode == vr.MODE_EA else np.isneginf(full[mask]).all()
+                assert empty
+            # the composited frame against the oracle's sort-last render (same mode, partition, tau)
+            o32, _, _ = ovr.render(vol, M, W, Hh, step, omode, ovr.F32, tf=tf, bg=BG, tau=tau, miss=BG[0],
+                                   split=ovr.SPLIT_SORTLAST, partition=brick)
+            o64, fl, _ = ovr.render(vol, M, W, Hh, step, omode, ovr.F64, tf=tf, bg=BG, tau=tau, miss=BG[0],
+                                    split=ovr.SPLIT_SORTLAST, partition=brick)
+            assert np.array_equal(fr, o32)
+            if mode == vr.MODE_EA:
+                H.compare(fr, o64, fl, o32, what=f"sort-last EA tau={tau}")
+            # split == unsplit (north_star closed form): MIP bit-exact, EA (ERT off) to 1e-6
+            if mode == vr.MODE_MIP:
+                assert np.array_equal(fr, sc.render_mip(M, W, Hh, step, miss=BG[0]))
+            elif tau > 1.0:
+                assert np.abs(fr - sc.render_ea(M, W, Hh, step, tf, bg=BG, tau=2.0)).max() < 1e-6
+    # negative test: reversing the order of a near-opaque scene changes the frame
+    fr_fwd, _, ids = sc.render_sortlast(M, W, Hh, step, vr.MODE_EA, tf=tf, bg=BG, tau=2.0)
+    fr_rev, _, _ = sc.render_sortlast(M, W, Hh, step, vr.MODE_EA, tf=tf, bg=BG, tau=2.0, order=ids[::-1])
+    assert np.abs(fr_fwd - fr_rev).max() > 1e-3
+
+
+# ------------------------------------------------------------------------------ S6 tiled frame
+def test_tiled_panels_into_one_pitched_frame(H):
+    import torch
+    dims, brick = (64, 64, 96), (32, 32, 32)
+    w = wl.scaled(wl.C4, "tiles", dims, brick, (160, 90), n_sources=5)
+    sc = H.Scene(dims, brick, gen={"seed": w.seed, "sources": wl.make_sources(w)})
+    tf = wl.tf_fog()
+    cols, rows, pw, ph = 5, 5, 32, 18
+    W, Hh = cols * pw, rows * ph
+    M = wl.perspective_camera(dims, (W, Hh))
+    single = sc.render_ea(M, W, Hh, 0.25, tf, bg=BG, tau=0.99)
+    frame = torch.full((Hh, W, 4), -7.0, dtype=torch.float32, device="cuda")
+    sc.ctx.set_transfer_function(*tf)
+    for r in range(rows):
+        for c in range(cols):
+            Mp = wl.panel_matrix(M, cols, rows, c, r)
+            sc.ctx.set_view(Mp, pw, ph, 0.25)
+            sc.ctx.set_viewport(c * pw, r * ph, W)
+            sc.ctx.render_ea(frame, BG, 0.99)
+    torch.cuda.synchronize()
+    tiled = frame.cpu().numpy()
+    assert (tiled != -7.0).all()
+    assert np.abs(tiled - single).max() < 1e-4
+    # one panel against the oracle with that panel's own matrix
+    Mp = wl.panel_matrix(M, cols, rows, 2, 2)
+    o32, _, _ = sc.ovr.render(sc.oracle_volume(), Mp, pw, ph, 0.25, sc.ovr.EA, sc.ovr.F32, tf=tf, bg=BG, tau=0.99)
+    assert np.array_equal(tiled[2 * ph:3 * ph, 2 * pw:3 * pw], o32)
+
+
+# ------------------------------------------------------------------------------ errors
+def test_error_codes(H):
+    import torch
+    from paper_1012_2909_b200 import vr
+    ctx = vr.Context(0)
+    out = torch.zeros(16, 16, 4, device="cuda")
+    with pytest.raises(vr.VRError) as e:
+        ctx.render_ea(out)
+    assert e.value.status == vr.ERR_STATE
+    with pytest.raises(vr.VRError) as e:
+        ctx.set_view(np.zeros(16, dtype=np.float32), 16, 16, 0.5)      # singular
+    assert e.value.status == vr.ERR_INVALID_ARG
+    with pytest.raises(vr.VRError) as e:
+        ctx.set_view(np.eye(4, dtype=np.float32), 16, 16, 0.0)         # step <= 0
+    assert e.value.status == vr.ERR_INVALID_ARG
+    with pytest.raises(vr.VRError) as e:
+        ctx.set_transfer_function(np.zeros((256, 4), dtype=np.float32), 1.0, 1.0)   # vmax <= vmin
+    assert e.value.status == vr.ERR_INVALID_ARG
+    ctx.set_view(np.eye(4, dtype=np.float32), 16, 16, 0.5)
+    with pytest.raises(vr.VRError) as e:
+        ctx.render_mip(out)                                            # still no cube
+    assert e.value.status == vr.ERR_STATE
