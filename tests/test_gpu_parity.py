@@ -306,3 +306,67 @@ def test_error_codes(H):
     with pytest.raises(vr.VRError) as e:
         ctx.render_mip(out)                                            # still no cube
     assert e.value.status == vr.ERR_STATE
+
+
+# ------------------------------------------------------------------------------ BASELINE.json full sizes
+def _fullsize_check(H, w, block, n_random, frame_index):
+    """Parity at a config's full size, in the launch configuration bench.py times (sort-last EA,
+    plus whole-frame MIP): sampled pixels against the oracle (cube bytes fetched back brick by
+    brick), and whole-frame properties that hold at any size."""
+    import torch
+    from oracle import ovr
+    sc = H.Scene(w.dims, w.brick, gen={"seed": w.seed, "sources": wl.make_sources(w),
+                                       "zero_boxes": wl.make_zero_boxes(w), "continuum": w.continuum})
+    vr = sc.vr
+    W, Hh = w.frame
+    M = wl.config_camera(w, frame_index)
+    tf = wl.TFS[w.tf]()
+    frame, imgs, ids = sc.render_sortlast(M, W, Hh, w.step, vr.MODE_EA, tf=tf, bg=BG, tau=w.tau)
+    mip = sc.render_mip(M, W, Hh, w.step, miss=0.0)
+    # sampled pixels: a block at the frame centre + seeded random pixels that hit the cube
+    rng = np.random.default_rng(w.view_seed)
+    cx, cy = W // 2, Hh // 2
+    xs, ys = np.arange(cx - block // 2, cx + block // 2), np.arange(cy - block // 2, cy + block // 2)
+    pix = np.stack(np.meshgrid(xs, ys), axis=-1).reshape(-1, 2)
+    if n_random:
+        hit = np.argwhere(mip != 0.0)
+        pick = hit[rng.choice(len(hit), size=min(n_random, len(hit)), replace=False)]
+        pix = np.concatenate([pix, pick[:, ::-1]])
+    pix = pix.astype(np.int32)
+    brick = tuple(min(b, n) for b, n in zip(w.brick, w.dims))
+    touched = ovr.bricks_touched(M, W, Hh, w.step, w.dims, brick, pix)
+    vol = ovr.Volume(w.dims, brick, {int(b): sc.download_brick(int(b)) for b in touched})
+    kw = dict(tf=tf, bg=BG, tau=w.tau, pixels=pix)
+    o64, fl, _ = ovr.render(vol, M, W, Hh, w.step, ovr.EA, ovr.F64, split=ovr.SPLIT_SORTLAST, partition=brick, **kw)
+    o32, _, _ = ovr.render(vol, M, W, Hh, w.step, ovr.EA, ovr.F32, split=ovr.SPLIT_SORTLAST, partition=brick, **kw)
+    got = frame[pix[:, 1], pix[:, 0]]
+    H.compare(got, o64, fl, o32, what=f"{w.name} full-size EA sort-last")
+    assert np.array_equal(got, o32)
+    m64, flm, _ = ovr.render(vol, M, W, Hh, w.step, ovr.MIP, ovr.F64, miss=0.0, pixels=pix)
+    m32, _, _ = ovr.render(vol, M, W, Hh, w.step, ovr.MIP, ovr.F32, miss=0.0, pixels=pix)
+    gm = mip[pix[:, 1], pix[:, 0]]
+    H.compare(gm, m64, flm, m32, mode_mip=True, vmin=tf[1], vmax=tf[2], miss=0.0, what=f"{w.name} full-size MIP")
+    assert np.array_equal(gm, m32)
+    # whole-frame properties: MIP split == unsplit bit-exact; EA sort-last (ERT off) == global to 1e-6;
+    # ERT bound |frame_tau - frame_inf| <= (1 - tau) / tau; alpha within [0, 1]
+    mip_sl, _, _ = sc.render_sortlast(M, W, Hh, w.step, vr.MODE_MIP, bg=(0.0, 0, 0, 0))
+    assert np.array_equal(mip_sl, mip)
+    sl_inf, _, _ = sc.render_sortlast(M, W, Hh, w.step, vr.MODE_EA, tf=tf, bg=BG, tau=2.0)
+    gl_inf = sc.render_ea(M, W, Hh, w.step, tf, bg=BG, tau=2.0)
+    assert np.abs(sl_inf - gl_inf).max() < 2e-6
+    assert np.abs(frame - sl_inf).max() <= (1 - w.tau) / w.tau + 1e-6
+    assert frame[..., 3].min() >= 0.0 and frame[..., 3].max() <= 1.0 + 1e-6
+    del sc
+    torch.cuda.empty_cache()
+
+
+def test_config_c2_full_size(H):
+    _fullsize_check(H, wl.C2, block=16, n_random=200, frame_index=0)
+
+
+def test_config_c3_full_size_64gib(H):
+    import torch
+    free, total = torch.cuda.mem_get_info()
+    if free < 80e9:
+        pytest.skip("needs ~70 GB of free HBM")
+    _fullsize_check(H, wl.C3, block=12, n_random=0, frame_index=37)
