@@ -148,9 +148,13 @@ typedef struct {
 /* Synchronises `stream`, then copies the device counters. */
 int vr_get_counters(vr_ctx* ctx, vr_counters* out, void* stream);
 int vr_reset_counters(vr_ctx* ctx, void* stream);
-/* Options: VR_OPT_SKIP (default 1) turns min/max empty-space skipping on/off (tests assert that
- * it never changes a frame). */
-enum { VR_OPT_SKIP = 1 };
+/* Options.  None of them changes a frame (tests assert it); they exist for A/B measurements.
+ *  VR_OPT_SKIP (default 1): min/max empty-space skipping (O-10) on/off, all levels.
+ *  VR_OPT_VARIANT (default 1): 0 = the marcher reads the 8 voxels of every sample; 1 = it keeps
+ *    the current trilinear cell in registers and fetches only the face that changed.
+ *  VR_OPT_CELL_SKIP (default 1): the 8^3 macro-cell level of the skipping under the configured
+ *    bricks on/off (needs VR_OPT_SKIP). */
+enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETCH = 4 };
 int vr_set_option(vr_ctx* ctx, int option, int value);
 
 #ifdef __cplusplus

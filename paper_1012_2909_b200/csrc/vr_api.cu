@@ -37,7 +37,8 @@ struct vr_ctx {
     float* d_stage = nullptr;
     size_t stage_bytes = 0;
     int64_t launches = 0;
-    int opt_skip = 1;
+    int opt_skip = 1, opt_cell_skip = 1, opt_variant = 1;
+    float x_clear = -INFINITY;
 };
 
 namespace {
@@ -153,14 +154,27 @@ int ensure_tables(vr_ctx* ctx, cudaStream_t s) {
             ctx->h_brick_active[b] = range_active(ctx, ctx->h_brick_mm[b].x, ctx->h_brick_mm[b].y) ? 1 : 0;
         // pageable source: cudaMemcpyAsync stages it before returning, so the vector may change later
         VR_CUDA(ctx, cudaMemcpyAsync(ctx->cube.brick_active, ctx->h_brick_active.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, s));
+        // the same test per 8^3 macro-cell, on the device (one bit per cell)
+        int nz[257];
+        nz[0] = 0;
+        for (int j = 0; j < 256; ++j) nz[j + 1] = nz[j] + (ctx->tf_baked[4 * j + 3] != 0.f ? 1 : 0);
+        VR_CUDA(ctx, launch_classify_cells(ctx->cube, nz, ctx->vmin, ctx->scale, s));
+        ctx->launches += 1;
+        // samples with table coordinate x < x_clear interpolate two entries of zero opacity
+        int i0 = -1;
+        while (i0 + 1 < 256 && ctx->tf_baked[4 * (i0 + 1) + 3] == 0.f) ++i0;
+        ctx->x_clear = i0 >= 1 ? (float)i0 : -INFINITY;
         ctx->activity_dirty = false;
     }
     return VR_OK;
 }
 
+int skip_level(const vr_ctx* ctx) { return ctx->opt_skip ? (ctx->opt_cell_skip ? 2 : 1) : 0; }
+
 TFDesc tf_desc(const vr_ctx* ctx) {
     TFDesc t;
     t.baked = ctx->d_tf_baked; t.raw = ctx->d_tf_raw; t.vmin = ctx->vmin; t.scale = ctx->scale;
+    t.x_clear = ctx->x_clear;
     return t;
 }
 
@@ -490,7 +504,7 @@ int vr_render_mip(vr_ctx* ctx, float* d_out, float* d_out_rgba, float miss, void
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
-    a.mode = VR_MODE_MIP; a.tau = 2.f; a.miss = miss; a.skip = ctx->opt_skip;
+    a.mode = VR_MODE_MIP; a.tau = 2.f; a.miss = miss; a.skip = skip_level(ctx); a.variant = ctx->opt_variant;
     a.out = d_out; a.out_rgba = d_out_rgba; a.counters = ctx->d_counters;
     VR_CUDA(ctx, launch_render_global(ctx->cube, ctx->view, tf_desc(ctx), a, s));
     ctx->launches += 1;
@@ -505,7 +519,7 @@ int vr_render_ea(vr_ctx* ctx, float* d_out, const float bg[4], float tau, void* 
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
-    a.mode = VR_MODE_EA; a.tau = tau; a.skip = ctx->opt_skip;
+    a.mode = VR_MODE_EA; a.tau = tau; a.skip = skip_level(ctx); a.variant = ctx->opt_variant;
     for (int i = 0; i < 4; ++i) a.bg[i] = bg[i];
     a.out = d_out; a.counters = ctx->d_counters;
     VR_CUDA(ctx, launch_render_global(ctx->cube, ctx->view, tf_desc(ctx), a, s));
@@ -586,7 +600,8 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
     int tiles = 0;
     if ((rc = upload_partials(ctx, mode, hp, n, true, &tiles, s))) return rc;
     RenderArgs a{};
-    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = ctx->opt_skip; a.counters = ctx->d_counters;
+    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx); a.variant = ctx->opt_variant;
+    a.counters = ctx->d_counters;
     VR_CUDA(ctx, launch_render_bricks(ctx->cube, ctx->view, tf_desc(ctx), a, ctx->d_partials, n, tiles, s));
     ctx->launches += (n > 0 && tiles > 0) ? 1 : 0;
     return VR_OK;
@@ -626,6 +641,16 @@ int vr_reset_counters(vr_ctx* ctx, void* stream) {
 int vr_set_option(vr_ctx* ctx, int option, int value) {
     if (!ctx) return VR_ERR_INVALID_ARG;
     if (option == VR_OPT_SKIP) { ctx->opt_skip = value ? 1 : 0; return VR_OK; }
+    if (option == VR_OPT_CELL_SKIP) { ctx->opt_cell_skip = value ? 1 : 0; return VR_OK; }
+    if (option == VR_OPT_L2_FETCH) {
+        if (value != 32 && value != 64 && value != 128) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: L2 fetch granularity must be 32, 64 or 128");
+        VR_CUDA(ctx, cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)value));
+        return VR_OK;
+    }
+    if (option == VR_OPT_VARIANT) {
+        if (value < 0 || value > 2) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");
+        ctx->opt_variant = value; return VR_OK;
+    }
     return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown option");
 }
 

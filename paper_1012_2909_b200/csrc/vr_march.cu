@@ -95,44 +95,117 @@ __device__ __forceinline__ int floor_pos(float p, float& fl) {
 
 __device__ __forceinline__ float lerp(float a, float b, float w) { return __fmaf_rn(w, __fsub_rn(b, a), a); }   // O-4
 
-// O-4 trilinear through a brick's storage; `base` is pre-offset so that global voxel indices
-// address it directly (valid only while floor(p) stays inside that brick).
-__device__ __forceinline__ float sample(const float* __restrict__ base, int P0, int P01, const float p[3]) {
-    float fx, fy, fz;
-    int ix = floor_pos(p[0], fx), iy = floor_pos(p[1], fy), iz = floor_pos(p[2], fz);
-    float wx = __fsub_rn(p[0], fx), wy = __fsub_rn(p[1], fy), wz = __fsub_rn(p[2], fz);
-    const float* q = base + (ix + P0 * iy + P01 * iz);
-    float c000 = __ldg(q), c100 = __ldg(q + 1);
-    float c010 = __ldg(q + P0), c110 = __ldg(q + P0 + 1);
-    float c001 = __ldg(q + P01), c101 = __ldg(q + P01 + 1);
-    float c011 = __ldg(q + P01 + P0), c111 = __ldg(q + P01 + P0 + 1);
-    float c00 = lerp(c000, c100, wx), c10 = lerp(c010, c110, wx);
-    float c01 = lerp(c001, c101, wx), c11 = lerp(c011, c111, wx);
-    float c0 = lerp(c00, c10, wy), c1 = lerp(c01, c11, wy);
-    return lerp(c0, c1, wz);
+// The 8 corner voxels of the trilinear cell a ray is in, kept in registers between samples
+// (DESIGN.md "Cell cache").  With a step of half a voxel consecutive samples mostly fall in the
+// same cell or in a face neighbour, so a sample needs 0 or 4 new voxels instead of 8.  The values
+// are the voxels themselves, so the interpolated result does not depend on the cache.
+struct Cell {
+    float c000, c100, c010, c110, c001, c101, c011, c111;
+    int ix, iy, iz;                       // cell index (global voxel coordinates); ix < 0: invalid
+};
+constexpr int kNoCell = -(1 << 30);
+
+struct BrickRef {
+    const float* base;     // first float of the brick
+    unsigned off0;         // lo0 + P0 lo1 + P01 lo2 (mod 2^32): subtracting it makes offsets brick-local
+    unsigned P0, P01;
+};
+
+__device__ __forceinline__ unsigned voxel_offset(const BrickRef& b, int ix, int iy, int iz) {
+    return (unsigned)ix + b.P0 * (unsigned)iy + b.P01 * (unsigned)iz - b.off0;
 }
 
-// O-6 lookup through a table in shared memory.
-__device__ __forceinline__ float4 tf_lookup(const float4* __restrict__ tab, float vmin, float scale, float v) {
-    float x = __fmul_rn(__fsub_rn(v, vmin), scale);
-    x = fminf(fmaxf(x, 0.f), 255.f);
-    float fl;
-    int i = min(floor_pos(x, fl), 254);
-    float f = __fsub_rn(x, (float)i);
-    float4 a = tab[i], b = tab[i + 1];
-    return make_float4(lerp(a.x, b.x, f), lerp(a.y, b.y, f), lerp(a.z, b.z, f), lerp(a.w, b.w, f));
+__device__ __forceinline__ void cell_load_all(const BrickRef& b, int ix, int iy, int iz, Cell& cc) {
+    const float* q = b.base + voxel_offset(b, ix, iy, iz);
+    cc.c000 = __ldg(q);                 cc.c100 = __ldg(q + 1);
+    cc.c010 = __ldg(q + b.P0);          cc.c110 = __ldg(q + b.P0 + 1);
+    cc.c001 = __ldg(q + b.P01);         cc.c101 = __ldg(q + b.P01 + 1);
+    cc.c011 = __ldg(q + b.P01 + b.P0);  cc.c111 = __ldg(q + b.P01 + b.P0 + 1);
+}
+
+// Move the cached cell to (ix, iy, iz): one face shift (4 new voxels) per axis that moved by one,
+// through the intermediate cells (ix, cy, cz) -> (ix, iy, cz) -> (ix, iy, iz), all of which lie in
+// the brick because the old and the new cell do.  Anything else reloads the 8 voxels.
+__device__ __forceinline__ void cell_move(const BrickRef& b, int ix, int iy, int iz, Cell& cc) {
+    const int ddx = ix - cc.ix, ddy = iy - cc.iy, ddz = iz - cc.iz;
+    if ((unsigned)(ddx + 1) <= 2u && (unsigned)(ddy + 1) <= 2u && (unsigned)(ddz + 1) <= 2u) {
+        if (ddx != 0) {
+            const float* q = b.base + voxel_offset(b, ix, cc.iy, cc.iz);
+            if (ddx > 0) {
+                cc.c000 = cc.c100; cc.c010 = cc.c110; cc.c001 = cc.c101; cc.c011 = cc.c111;
+                cc.c100 = __ldg(q + 1);         cc.c110 = __ldg(q + b.P0 + 1);
+                cc.c101 = __ldg(q + b.P01 + 1); cc.c111 = __ldg(q + b.P01 + b.P0 + 1);
+            } else {
+                cc.c100 = cc.c000; cc.c110 = cc.c010; cc.c101 = cc.c001; cc.c111 = cc.c011;
+                cc.c000 = __ldg(q);             cc.c010 = __ldg(q + b.P0);
+                cc.c001 = __ldg(q + b.P01);     cc.c011 = __ldg(q + b.P01 + b.P0);
+            }
+        }
+        if (ddy != 0) {
+            const float* q = b.base + voxel_offset(b, ix, iy, cc.iz);
+            if (ddy > 0) {
+                cc.c000 = cc.c010; cc.c100 = cc.c110; cc.c001 = cc.c011; cc.c101 = cc.c111;
+                cc.c010 = __ldg(q + b.P0);          cc.c110 = __ldg(q + b.P0 + 1);
+                cc.c011 = __ldg(q + b.P01 + b.P0);  cc.c111 = __ldg(q + b.P01 + b.P0 + 1);
+            } else {
+                cc.c010 = cc.c000; cc.c110 = cc.c100; cc.c011 = cc.c001; cc.c111 = cc.c101;
+                cc.c000 = __ldg(q);                 cc.c100 = __ldg(q + 1);
+                cc.c001 = __ldg(q + b.P01);         cc.c101 = __ldg(q + b.P01 + 1);
+            }
+        }
+        if (ddz != 0) {
+            const float* q = b.base + voxel_offset(b, ix, iy, iz);
+            if (ddz > 0) {
+                cc.c000 = cc.c001; cc.c100 = cc.c101; cc.c010 = cc.c011; cc.c110 = cc.c111;
+                cc.c001 = __ldg(q + b.P01);         cc.c101 = __ldg(q + b.P01 + 1);
+                cc.c011 = __ldg(q + b.P01 + b.P0);  cc.c111 = __ldg(q + b.P01 + b.P0 + 1);
+            } else {
+                cc.c001 = cc.c000; cc.c101 = cc.c100; cc.c011 = cc.c010; cc.c111 = cc.c110;
+                cc.c000 = __ldg(q);                 cc.c100 = __ldg(q + 1);
+                cc.c010 = __ldg(q + b.P0);          cc.c110 = __ldg(q + b.P0 + 1);
+            }
+        }
+    } else {
+        cell_load_all(b, ix, iy, iz, cc);
+    }
+    cc.ix = ix; cc.iy = iy; cc.iz = iz;
+}
+
+// O-4 trilinear at p (floor(p) inside brick b).  VAR 0 reads the 8 voxels of every sample, VAR 1
+// goes through the cell cache.
+template <int VAR>
+__device__ __forceinline__ float sample(const BrickRef& b, const float p[3], Cell& cc) {
+    float fx, fy, fz;
+    const int ix = floor_pos(p[0], fx), iy = floor_pos(p[1], fy), iz = floor_pos(p[2], fz);
+    const float wx = __fsub_rn(p[0], fx), wy = __fsub_rn(p[1], fy), wz = __fsub_rn(p[2], fz);
+    if (VAR == 0) cell_load_all(b, ix, iy, iz, cc);
+    else if (ix != cc.ix || iy != cc.iy || iz != cc.iz) cell_move(b, ix, iy, iz, cc);
+    const float c00 = lerp(cc.c000, cc.c100, wx), c10 = lerp(cc.c010, cc.c110, wx);
+    const float c01 = lerp(cc.c001, cc.c101, wx), c11 = lerp(cc.c011, cc.c111, wx);
+    const float c0 = lerp(c00, c10, wy), c1 = lerp(c01, c11, wy);
+    return lerp(c0, c1, wz);
 }
 
 struct Accum { float C[3]; float A; float m; };
 
+// O-5 / O-6 / O-7: fold one sample value into the ray's accumulator.  A sample whose table
+// coordinate x lies below T.x_clear falls between two entries of zero opacity: its weight
+// w = (1 - A) * 0 is exactly zero and leaves C and A unchanged, so the lookup is not done.
 template <int MODE>
 __device__ __forceinline__ bool fold(Accum& acc, float v, const float4* tab, const TFDesc& T, float tau) {
     if (MODE == VR_MODE_MIP) { acc.m = fmaxf(acc.m, v); return false; }
-    float4 q = tf_lookup(tab, T.vmin, T.scale, v);
-    float w = __fmul_rn(__fsub_rn(1.f, acc.A), q.w);        // O-7
-    acc.C[0] = __fmaf_rn(w, q.x, acc.C[0]);
-    acc.C[1] = __fmaf_rn(w, q.y, acc.C[1]);
-    acc.C[2] = __fmaf_rn(w, q.z, acc.C[2]);
+    float x = __fmul_rn(__fsub_rn(v, T.vmin), T.scale);
+    if (x < T.x_clear) return false;
+    x = fminf(fmaxf(x, 0.f), 255.f);
+    float fl;
+    const int i = min(floor_pos(x, fl), 254);
+    const float f = __fsub_rn(x, fminf(fl, 254.f));
+    const float4 a = tab[i], b = tab[i + 1];
+    const float qa = lerp(a.w, b.w, f);
+    const float w = __fmul_rn(__fsub_rn(1.f, acc.A), qa);        // O-7
+    acc.C[0] = __fmaf_rn(w, lerp(a.x, b.x, f), acc.C[0]);
+    acc.C[1] = __fmaf_rn(w, lerp(a.y, b.y, f), acc.C[1]);
+    acc.C[2] = __fmaf_rn(w, lerp(a.z, b.z, f), acc.C[2]);
     acc.A = __fadd_rn(acc.A, w);
     return acc.A >= tau;
 }
@@ -171,8 +244,94 @@ __device__ __forceinline__ void tile_pixel(int& tx, int& ty) {     // warp = 8 x
     ty = (warp >> 1) * 4 + (lane >> 3);
 }
 
+// Shrink the taken interval [ka, kb] of ray r to its members of brick b (O-3): conservative float32
+// bracket of the brick's slab interval, then exact shrink with the membership predicate
+// floor(p_a) / B_a == b_a, which is monotone per axis.
+__device__ __forceinline__ void brick_interval(const CubeDesc& c, const Ray& r, const int b[3], const int lo[3], int& ka, int& kb) {
+    if (ka > kb) return;
+    float t0 = 0.f, t1 = 3.0e38f;
+    bool empty = false;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        float flo = (float)lo[a] - r.margin, fhi = (float)(lo[a] + c.B[a]) + r.margin;
+        if (r.d[a] == 0.f) { if (r.o[a] < flo || r.o[a] > fhi) empty = true; continue; }
+        float ta = (flo - r.o[a]) / r.d[a], tb = (fhi - r.o[a]) / r.d[a];
+        t0 = fmaxf(t0, fminf(ta, tb)); t1 = fminf(t1, fmaxf(ta, tb));
+    }
+    if (empty || !(t0 <= t1)) { ka = 0; kb = -1; return; }
+    float qa = floorf(t0 / r.step) - 2.f, qb = ceilf(t1 / r.step) + 2.f;
+    ka = max(ka, (int)fminf(fmaxf(qa, 0.f), 1.0e9f));
+    kb = min(kb, (int)fminf(fmaxf(qb, -1.f), 1.0e9f));
+    float p[3], fl;
+    while (ka <= kb) {
+        position(r, (float)ka, p);
+        int iv[3] = {floor_pos(p[0], fl), floor_pos(p[1], fl), floor_pos(p[2], fl)};
+        int bb[3]; brick_of(c, iv, bb);
+        if (bb[0] == b[0] && bb[1] == b[1] && bb[2] == b[2]) break;
+        ++ka;
+    }
+    while (kb >= ka) {
+        position(r, (float)kb, p);
+        int iv[3] = {floor_pos(p[0], fl), floor_pos(p[1], fl), floor_pos(p[2], fl)};
+        int bb[3]; brick_of(c, iv, bb);
+        if (bb[0] == b[0] && bb[1] == b[1] && bb[2] == b[2]) break;
+        --kb;
+    }
+}
+
+struct Stats { unsigned long long taken, visit, skip; };
+
+__device__ __forceinline__ BrickRef brick_ref(const CubeDesc& c, int bid, const int lo[3]) {
+    BrickRef b;
+    b.base = c.cube + (long long)bid * c.stride;
+    b.P0 = (unsigned)c.P[0]; b.P01 = (unsigned)(c.P[0] * c.P[1]);
+    b.off0 = (unsigned)lo[0] + b.P0 * (unsigned)lo[1] + b.P01 * (unsigned)lo[2];
+    return b;
+}
+
+// March the lattice samples k .. ke (all of them members of brick `bid`, O-3) into `acc`.  With
+// A.skip >= 2 the interval is cut into runs inside 8^3 macro-cells and a run is skipped when its
+// cell cannot contribute (O-10, exact): EA - every table entry its value range can touch has zero
+// opacity (bit precomputed per transfer function); MIP - the cell's maximum cannot raise m.
+// Returns true if early ray termination fired.
+template <int MODE, int VAR>
+__device__ __forceinline__ bool march_interval(const CubeDesc& c, const Ray& r, const TFDesc& T, const RenderArgs& A,
+                                               const float4* tab, int bid, const int lo[3], int k, int ke,
+                                               Accum& acc, Stats& st) {
+    const BrickRef b = brick_ref(c, bid, lo);
+    const int S8[3] = {kCell, kCell, kCell};
+    Cell cc;
+    cc.ix = cc.iy = cc.iz = kNoCell;
+    float kf = (float)k;                                    // exact: k < 2^24
+    while (k <= ke) {
+        int n = ke - k + 1;
+        if (A.skip >= 2) {
+            float p[3], fl;
+            position(r, kf, p);
+            const int cl[3] = {(floor_pos(p[0], fl) - lo[0]) >> 3, (floor_pos(p[1], fl) - lo[1]) >> 3,
+                               (floor_pos(p[2], fl) - lo[2]) >> 3};
+            const int clo[3] = {lo[0] + (cl[0] << 3), lo[1] + (cl[1] << 3), lo[2] + (cl[2] << 3)};
+            n = min(n, run_length(r, p, clo, S8));
+            const int cidx = cl[0] + c.C[0] * (cl[1] + c.C[1] * cl[2]);
+            bool skip;
+            if (MODE == VR_MODE_MIP) skip = __ldg(&c.cell_mm[(long long)bid * c.cells_per_brick + cidx]).y <= acc.m;
+            else skip = ((__ldg(&c.cell_bits[(long long)bid * c.cell_words_per_brick + (cidx >> 5)]) >> (cidx & 31)) & 1u) == 0u;
+            if (skip) { k += n; kf = __fadd_rn(kf, (float)n); ++st.skip; continue; }
+        }
+        ++st.visit;
+        for (const int e = k + n; k < e; ++k, kf = __fadd_rn(kf, 1.f)) {
+            float p[3];
+            position(r, kf, p);
+            const float v = sample<VAR>(b, p, cc);
+            ++st.taken;
+            if (fold<MODE>(acc, v, tab, T, A.tau)) return true;
+        }
+    }
+    return false;
+}
+
 // ---------------------------------------------------------------- whole frame, O-8 GLOBAL
-template <int MODE>
+template <int MODE, int VAR>
 __global__ void __launch_bounds__(kThreads)
 render_global_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                      const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A) {
@@ -184,9 +343,8 @@ render_global_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
     Ray r; r.k0 = 0; r.k1 = -1;
     if (live) setup_ray(V, c, i, j, r);
     Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-    unsigned long long n_taken = 0, n_visit = 0, n_skip = 0;
+    Stats st = {0, 0, 0};
     bool stopped = false;
-    const int P0 = c.P[0], P01 = c.P[0] * c.P[1];
     int k = r.k0;
     while (k <= r.k1) {
         float p[3];
@@ -202,16 +360,9 @@ render_global_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
             if (MODE == VR_MODE_MIP) skip = c.brick_mm[bid].y <= acc.m;       // O-10 (exact)
             else skip = c.brick_active[bid] == 0;
         }
-        if (skip) { k += n; ++n_skip; continue; }
-        ++n_visit;
-        const float* base = c.cube + ((long long)bid * c.stride - (lo[0] + P0 * lo[1] + (long long)P01 * lo[2]));
-        for (int e = k + n; k < e; ++k) {
-            position(r, (float)k, p);
-            float v = sample(base, P0, P01, p);
-            ++n_taken;
-            if (fold<MODE>(acc, v, tab, T, A.tau)) { stopped = true; break; }
-        }
-        if (stopped) break;
+        if (skip) { k += n; ++st.skip; continue; }
+        if (march_interval<MODE, VAR>(c, r, T, A, tab, bid, lo, k, k + n - 1, acc, st)) { stopped = true; break; }
+        k += n;
     }
     if (live) {
         const long long px = (long long)(V.vy0 + j) * V.pitch + (V.vx0 + i);
@@ -241,15 +392,15 @@ render_global_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
         const unsigned long long nom = r.k1 >= r.k0 ? (unsigned long long)(r.k1 - r.k0 + 1) : 0ULL;
         count(A.counters, kRays, nom ? 1 : 0);
         count(A.counters, kNominal, nom);
-        count(A.counters, kTaken, n_taken);
-        count(A.counters, kVisited, n_visit);
-        count(A.counters, kSkipped, n_skip);
+        count(A.counters, kTaken, st.taken);
+        count(A.counters, kVisited, st.visit);
+        count(A.counters, kSkipped, st.skip);
         count(A.counters, kTerminated, stopped ? 1 : 0);
     }
 }
 
 // ---------------------------------------------------------------- per-brick partial images (O-8 SORT-LAST)
-template <int MODE>
+template <int MODE, int VAR>
 __global__ void __launch_bounds__(kThreads)
 render_bricks_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                      const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
@@ -274,52 +425,10 @@ render_bricks_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
     const int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
     const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
     int ka = r.k0, kb = r.k1;
-    if (ka <= kb) {
-        // conservative float32 bracket of the brick's slab interval, then exact shrink with the
-        // membership predicate of O-3 (floor(p_a) / B_a == b_a), monotone per axis
-        float t0 = 0.f, t1 = 3.0e38f;
-        bool empty = false;
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            float flo = (float)lo[a] - r.margin, fhi = (float)(lo[a] + c.B[a]) + r.margin;
-            if (r.d[a] == 0.f) { if (r.o[a] < flo || r.o[a] > fhi) empty = true; continue; }
-            float ta = (flo - r.o[a]) / r.d[a], tb = (fhi - r.o[a]) / r.d[a];
-            t0 = fmaxf(t0, fminf(ta, tb)); t1 = fminf(t1, fmaxf(ta, tb));
-        }
-        if (empty || !(t0 <= t1)) { ka = 0; kb = -1; }
-        else {
-            float qa = floorf(t0 / r.step) - 2.f, qb = ceilf(t1 / r.step) + 2.f;
-            ka = max(ka, (int)fminf(fmaxf(qa, 0.f), 1.0e9f));
-            kb = min(kb, (int)fminf(fmaxf(qb, -1.f), 1.0e9f));
-            float p[3], fl;
-            while (ka <= kb) {
-                position(r, (float)ka, p);
-                int iv[3] = {floor_pos(p[0], fl), floor_pos(p[1], fl), floor_pos(p[2], fl)};
-                int bb[3]; brick_of(c, iv, bb);
-                if (bb[0] == b[0] && bb[1] == b[1] && bb[2] == b[2]) break;
-                ++ka;
-            }
-            while (kb >= ka) {
-                position(r, (float)kb, p);
-                int iv[3] = {floor_pos(p[0], fl), floor_pos(p[1], fl), floor_pos(p[2], fl)};
-                int bb[3]; brick_of(c, iv, bb);
-                if (bb[0] == b[0] && bb[1] == b[1] && bb[2] == b[2]) break;
-                --kb;
-            }
-        }
-    }
+    brick_interval(c, r, b, lo, ka, kb);
     Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-    const int P0 = c.P[0], P01 = c.P[0] * c.P[1];
-    const float* base = c.cube + ((long long)bid * c.stride - (lo[0] + P0 * lo[1] + (long long)P01 * lo[2]));
-    unsigned long long n_taken = 0;
-    bool stopped = false;
-    for (int k = ka; k <= kb; ++k) {
-        float p[3];
-        position(r, (float)k, p);
-        float v = sample(base, P0, P01, p);
-        ++n_taken;
-        if (fold<MODE>(acc, v, tab, T, A.tau)) { stopped = true; break; }
-    }
+    Stats st = {0, 0, 0};
+    const bool stopped = march_interval<MODE, VAR>(c, r, T, A, tab, bid, lo, ka, kb, acc, st);
     if (live) {
         const long long px = (long long)ly * part.pitch + lx;
         if (MODE == VR_MODE_MIP) reinterpret_cast<float*>(part.data)[px] = acc.m;
@@ -327,9 +436,148 @@ render_bricks_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
     }
     if (A.counters) {
         count(A.counters, kNominal, kb >= ka ? (unsigned long long)(kb - ka + 1) : 0ULL);
-        count(A.counters, kTaken, n_taken);
-        count(A.counters, kVisited, kb >= ka ? 1 : 0);
+        count(A.counters, kTaken, st.taken);
+        count(A.counters, kVisited, st.visit);
+        count(A.counters, kSkipped, st.skip);
         count(A.counters, kTerminated, stopped ? 1 : 0);
+    }
+}
+
+// ---------------------------------------------------------------- sort-last, one ray per warp
+// Variant 2 ("sample-parallel").  The 128 threads of a CTA first set up
+// the 128 rays of their pixel tile exactly as above (one ray per thread).  Then every warp walks
+// through its own 32 rays one after the other, and the 32 lanes take 32 CONSECUTIVE lattice
+// samples k .. k+31 of that one ray: positions, voxel gathers and trilinear interpolation run in
+// parallel, and the lanes' addresses follow the ray, so every 32-byte sector the ray needs is
+// fetched once and used at once - nothing has to survive in L1/L2 between iterations, whatever
+// the view direction.  The front-to-back fold stays sequential in k (O-7): opaque samples are
+// picked out with a ballot and folded in ascending order through shuffles, all lanes keeping the
+// same accumulator; transparent samples (x < x_clear) contribute exact zeros and are not folded.
+// MIP folds with a warp maximum (exact in any order).
+template <int MODE>
+__global__ void __launch_bounds__(kThreads)
+render_bricks_sp_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
+                        const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
+                        const PartialDev* __restrict__ parts, int n_parts) {
+    __shared__ float4 tab[256];
+    __shared__ PartialDev part;
+    if (threadIdx.x == 0) {
+        int lo = 0, hi = n_parts - 1;
+        const int tile = blockIdx.x;
+        while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (parts[mid].tile0 <= tile) lo = mid; else hi = mid - 1; }
+        part = parts[lo];
+    }
+    if (MODE == VR_MODE_EA) load_tf(tab, T.baked); else __syncthreads();
+    int tx, ty; tile_pixel(tx, ty);
+    const int tiles_x = (part.w + kTileW - 1) / kTileW;
+    const int tile = blockIdx.x - part.tile0;
+    const int lx = (tile % tiles_x) * kTileW + tx, ly = (tile / tiles_x) * kTileH + ty;
+    const bool live = lx < part.w && ly < part.h;
+    Ray r; r.k0 = 0; r.k1 = -1;
+    r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
+    if (live) setup_ray(V, c, part.x0 + lx, part.y0 + ly, r);
+    const int bid = part.brick;
+    const int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
+    const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
+    int ka = r.k0, kb = r.k1;
+    brick_interval(c, r, b, lo, ka, kb);
+    const BrickRef br = brick_ref(c, bid, lo);
+    const int lane = threadIdx.x & 31;
+    Accum mine = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
+    unsigned long long n_taken = 0, n_term = 0, n_visit = 0;
+    const unsigned todo = __ballot_sync(0xffffffffu, ka <= kb);
+    for (unsigned rays = todo; rays; rays &= rays - 1) {
+        const int src = __ffs(rays) - 1;
+        Ray q;
+        q.step = r.step;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { q.o[a] = __shfl_sync(0xffffffffu, r.o[a], src); q.d[a] = __shfl_sync(0xffffffffu, r.d[a], src); }
+        const int qa = __shfl_sync(0xffffffffu, ka, src), qb = __shfl_sync(0xffffffffu, kb, src);
+        Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
+        bool stopped = false;
+        for (int k0 = qa; k0 <= qb && !stopped; k0 += 32) {
+            const int k = k0 + lane;
+            const bool act = k <= qb;
+            float p[3];
+            position(q, (float)min(k, qb), p);               // idle lanes repeat the last sample
+            Cell cc;
+            const float v = sample<0>(br, p, cc);
+            if (MODE == VR_MODE_MIP) {
+                float m = act ? v : -INFINITY;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+                acc.m = fmaxf(acc.m, m);
+                if (lane == 0) n_taken += (unsigned long long)(min(qb - k0, 31) + 1);
+            } else {
+                float x = __fmul_rn(__fsub_rn(v, T.vmin), T.scale);
+                const bool opaque = act && !(x < T.x_clear);
+                unsigned bits = __ballot_sync(0xffffffffu, opaque);
+                int n_here = min(qb - k0, 31) + 1;
+                if (bits) {
+                    float4 col = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (opaque) {                           // O-6 lookup, one sample per lane
+                        x = fminf(fmaxf(x, 0.f), 255.f);
+                        float fl;
+                        const int i = min(floor_pos(x, fl), 254);
+                        const float f = __fsub_rn(x, fminf(fl, 254.f));
+                        const float4 ta = tab[i], tb = tab[i + 1];
+                        col = make_float4(lerp(ta.x, tb.x, f), lerp(ta.y, tb.y, f), lerp(ta.z, tb.z, f), lerp(ta.w, tb.w, f));
+                    }
+                    while (bits) {                          // O-7, ascending k
+                        const int j = __ffs(bits) - 1;
+                        bits &= bits - 1;
+                        const float cr = __shfl_sync(0xffffffffu, col.x, j), cg = __shfl_sync(0xffffffffu, col.y, j);
+                        const float cb = __shfl_sync(0xffffffffu, col.z, j), ca = __shfl_sync(0xffffffffu, col.w, j);
+                        const float w = __fmul_rn(__fsub_rn(1.f, acc.A), ca);
+                        acc.C[0] = __fmaf_rn(w, cr, acc.C[0]);
+                        acc.C[1] = __fmaf_rn(w, cg, acc.C[1]);
+                        acc.C[2] = __fmaf_rn(w, cb, acc.C[2]);
+                        acc.A = __fadd_rn(acc.A, w);
+                        if (acc.A >= A.tau) { stopped = true; n_here = j + 1; break; }
+                    }
+                }
+                if (lane == 0) n_taken += (unsigned long long)n_here;
+            }
+        }
+        if (lane == 0) { ++n_visit; n_term += stopped ? 1 : 0; }
+        if (lane == src) mine = acc;
+    }
+    if (live) {
+        const long long px = (long long)ly * part.pitch + lx;
+        if (MODE == VR_MODE_MIP) reinterpret_cast<float*>(part.data)[px] = mine.m;
+        else reinterpret_cast<float4*>(part.data)[px] = make_float4(mine.C[0], mine.C[1], mine.C[2], mine.A);
+    }
+    if (A.counters) {
+        count(A.counters, kNominal, kb >= ka ? (unsigned long long)(kb - ka + 1) : 0ULL);
+        count(A.counters, kTaken, n_taken);
+        count(A.counters, kVisited, n_visit);
+        count(A.counters, kTerminated, n_term);
+    }
+}
+
+// O-10 per transfer function: one bit per 8^3 macro-cell, set iff a table entry that the cell's
+// value range [min, max] (halo-inclusive) can touch has non-zero opacity.  `nz` is the running
+// count of entries with non-zero baked opacity, so the range test is one subtraction.
+struct NzPrefix { int v[257]; };
+__global__ void classify_cells_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ NzPrefix nz,
+                                      float vmin, float scale, long long n_slots) {
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n_slots;
+         e += (long long)gridDim.x * blockDim.x) {
+        const long long word = e >> 5;
+        const int brick = (int)(word / c.cell_words_per_brick);
+        const int cidx = (int)(word % c.cell_words_per_brick) * 32 + (int)(e & 31);
+        bool active = false;
+        if (cidx < c.cells_per_brick) {
+            const float2 mm = c.cell_mm[(long long)brick * c.cells_per_brick + cidx];
+            if (mm.x <= mm.y) {
+                float xa = fminf(fmaxf(__fmul_rn(__fsub_rn(mm.x, vmin), scale), 0.f), 255.f);
+                float xb = fminf(fmaxf(__fmul_rn(__fsub_rn(mm.y, vmin), scale), 0.f), 255.f);
+                const int lo = max(0, min((int)floorf(xa), 255)), hi = max(0, min((int)ceilf(xb), 255));
+                active = nz.v[hi + 1] - nz.v[lo] > 0;
+            }
+        }
+        const unsigned bits = __ballot_sync(0xffffffffu, active);
+        if ((e & 31) == 0) c.cell_bits[word] = bits;
     }
 }
 
@@ -342,16 +590,41 @@ __global__ void upload_half_kernel(float4* dst, const __grid_constant__ HalfTabl
 
 cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s) {
     dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
-    if (a.mode == VR_MODE_MIP) render_global_kernel<VR_MODE_MIP><<<grid, kThreads, 0, s>>>(c, v, t, a);
-    else render_global_kernel<VR_MODE_EA><<<grid, kThreads, 0, s>>>(c, v, t, a);
+    const bool mip = a.mode == VR_MODE_MIP;
+    if (a.variant == 0) {
+        if (mip) render_global_kernel<VR_MODE_MIP, 0><<<grid, kThreads, 0, s>>>(c, v, t, a);
+        else render_global_kernel<VR_MODE_EA, 0><<<grid, kThreads, 0, s>>>(c, v, t, a);
+    } else {
+        if (mip) render_global_kernel<VR_MODE_MIP, 1><<<grid, kThreads, 0, s>>>(c, v, t, a);
+        else render_global_kernel<VR_MODE_EA, 1><<<grid, kThreads, 0, s>>>(c, v, t, a);
+    }
     return cudaGetLastError();
 }
 
 cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a,
                                  const PartialDev* d_partials, int n, int total_tiles, cudaStream_t s) {
     if (n == 0 || total_tiles == 0) return cudaSuccess;
-    if (a.mode == VR_MODE_MIP) render_bricks_kernel<VR_MODE_MIP><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-    else render_bricks_kernel<VR_MODE_EA><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
+    const bool mip = a.mode == VR_MODE_MIP;
+    if (a.variant == 2) {
+        if (mip) render_bricks_sp_kernel<VR_MODE_MIP><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
+        else render_bricks_sp_kernel<VR_MODE_EA><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
+    } else if (a.variant == 0) {
+        if (mip) render_bricks_kernel<VR_MODE_MIP, 0><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
+        else render_bricks_kernel<VR_MODE_EA, 0><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
+    } else {
+        if (mip) render_bricks_kernel<VR_MODE_MIP, 1><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
+        else render_bricks_kernel<VR_MODE_EA, 1><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_classify_cells(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale, cudaStream_t s) {
+    NzPrefix nz;
+    for (int i = 0; i < 257; ++i) nz.v[i] = nz_prefix[i];
+    const long long n_slots = (long long)c.nbricks * c.cell_words_per_brick * 32;
+    long long blocks = (n_slots + 255) / 256;
+    if (blocks > 148LL * 32) blocks = 148LL * 32;
+    classify_cells_kernel<<<(int)blocks, 256, 0, s>>>(c, nz, vmin, scale, n_slots);
     return cudaGetLastError();
 }
 
