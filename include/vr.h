@@ -150,11 +150,14 @@ int vr_get_counters(vr_ctx* ctx, vr_counters* out, void* stream);
 int vr_reset_counters(vr_ctx* ctx, void* stream);
 /* Options.  None of them changes a frame (tests assert it); they exist for A/B measurements.
  *  VR_OPT_SKIP (default 1): min/max empty-space skipping (O-10) on/off, all levels.
- *  VR_OPT_VARIANT (default 1): 0 = the marcher reads the 8 voxels of every sample; 1 = it keeps
- *    the current trilinear cell in registers and fetches only the face that changed.
- *  VR_OPT_CELL_SKIP (default 1): the 8^3 macro-cell level of the skipping under the configured
- *    bricks on/off (needs VR_OPT_SKIP). */
-enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETCH = 4 };
+ *  VR_OPT_VARIANT (default 2): 0 = one ray per thread, the 32 lanes of a warp take 8 x 4 pixels;
+ *    2 = one ray per warp, the 32 lanes take 32 consecutive samples of it.
+ *  VR_OPT_CELL_SKIP (default 0): the 8^3 macro-cell level of the skipping under the configured
+ *    bricks on/off (needs VR_OPT_SKIP).
+ *  VR_OPT_LAYOUT (default 1): voxel order inside a brick, 0 = rows (x fastest), 1 = 4 x 4 x 2
+ *    micro-blocks of one 128-byte line each; read by the next upload / generate / attach call.
+ *  VR_OPT_L2_FETCH: cudaLimitMaxL2FetchGranularity of the device (32, 64 or 128 bytes). */
+enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETCH = 4, VR_OPT_LAYOUT = 5 };
 int vr_set_option(vr_ctx* ctx, int option, int value);
 
 #ifdef __cplusplus

@@ -37,7 +37,7 @@ struct vr_ctx {
     float* d_stage = nullptr;
     size_t stage_bytes = 0;
     int64_t launches = 0;
-    int opt_skip = 1, opt_cell_skip = 1, opt_variant = 1;
+    int opt_skip = 1, opt_cell_skip = 0, opt_variant = 2, opt_layout = 1;
     float x_clear = -INFINITY;
 };
 
@@ -260,8 +260,9 @@ namespace vr {
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz) {
+void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz, int layout) {
     std::memset(&c, 0, sizeof(c));
+    c.layout = layout;
     int N[3] = {nx, ny, nz}, B[3] = {bx, by, bz};
     for (int a = 0; a < 3; ++a) {
         c.N[a] = N[a]; c.B[a] = std::min(B[a], N[a]);
@@ -271,11 +272,13 @@ void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz)
         for (int s = 0; s < 30; ++s) if ((1 << s) == c.B[a]) c.sh[a] = s;
         c.C[a] = (c.B[a] + kCell - 1) / kCell;
     }
-    c.P[0] = (c.P[0] + 3) / 4 * 4;
+    if (layout == 0) c.P[0] = (c.P[0] + 3) / 4 * 4;
+    c.T[0] = (c.P[0] + 3) / 4; c.T[1] = (c.P[1] + 3) / 4; c.T[2] = (c.P[2] + 1) / 2;
     c.nbricks = c.G[0] * c.G[1] * c.G[2];
     c.cells_per_brick = c.C[0] * c.C[1] * c.C[2];
     c.cell_words_per_brick = (c.cells_per_brick + 31) / 32;
-    c.stride = (long long)align_up((size_t)c.P[0] * c.P[1] * c.P[2], 32);
+    c.stride = layout == 0 ? (long long)align_up((size_t)c.P[0] * c.P[1] * c.P[2], 32)
+                           : 32LL * c.T[0] * c.T[1] * c.T[2];
 }
 
 size_t cube_bytes(const CubeDesc& c) { return (size_t)c.nbricks * (size_t)c.stride * sizeof(float); }
@@ -340,17 +343,18 @@ int vr_destroy(vr_ctx* ctx) {
 
 int vr_cube_layout(int nx, int ny, int nz, int bx, int by, int bz, size_t* cube_bytes_out, size_t* meta_bytes_out) {
     if (!valid_dims(nx, ny, nz, bx, by, bz) || !cube_bytes_out || !meta_bytes_out) return VR_ERR_INVALID_ARG;
-    CubeDesc c;
-    fill_cube_desc(c, nx, ny, nz, bx, by, bz);
-    *cube_bytes_out = cube_bytes(c);
-    *meta_bytes_out = meta_layout(c).total;
+    CubeDesc c0, c1;                       // enough for either in-brick layout (VR_OPT_LAYOUT)
+    fill_cube_desc(c0, nx, ny, nz, bx, by, bz, 0);
+    fill_cube_desc(c1, nx, ny, nz, bx, by, bz, 1);
+    *cube_bytes_out = std::max(cube_bytes(c0), cube_bytes(c1));
+    *meta_bytes_out = meta_layout(c0).total;
     return VR_OK;
 }
 
 int vr_attach_cube(vr_ctx* ctx, int nx, int ny, int nz, int bx, int by, int bz, const void* d_cube, void* d_meta) {
     if (!ctx) return VR_ERR_INVALID_ARG;
     if (!valid_dims(nx, ny, nz, bx, by, bz) || !d_cube || !d_meta) return fail(ctx, VR_ERR_INVALID_ARG, "vr_attach_cube: bad argument");
-    fill_cube_desc(ctx->cube, nx, ny, nz, bx, by, bz);
+    fill_cube_desc(ctx->cube, nx, ny, nz, bx, by, bz, ctx->opt_layout);
     bind_meta(ctx->cube, d_cube, d_meta);
     ctx->h_brick_mm.resize(ctx->cube.nbricks);
     VR_CUDA(ctx, cudaMemcpy(ctx->h_brick_mm.data(), ctx->cube.brick_mm, sizeof(float2) * ctx->cube.nbricks, cudaMemcpyDeviceToHost));
@@ -366,7 +370,7 @@ int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int
     cudaStream_t s = (cudaStream_t)stream;
     ctx->has_cube = false;
     CubeDesc& c = ctx->cube;
-    fill_cube_desc(c, nx, ny, nz, bx, by, bz);
+    fill_cube_desc(c, nx, ny, nz, bx, by, bz, ctx->opt_layout);
     bind_meta(c, d_cube, d_meta);
     VR_CUDA(ctx, cudaMemsetAsync(d_cube, 0, cube_bytes(c), s));
     if (src_is_device) {
@@ -403,7 +407,7 @@ int vr_generate_cube(vr_ctx* ctx, const vr_gen_params* prm, uint64_t seed, int n
     cudaStream_t s = (cudaStream_t)stream;
     ctx->has_cube = false;
     CubeDesc& c = ctx->cube;
-    fill_cube_desc(c, nx, ny, nz, bx, by, bz);
+    fill_cube_desc(c, nx, ny, nz, bx, by, bz, ctx->opt_layout);
     bind_meta(c, d_cube, d_meta);
     // bin the sources (ascending id) and the zero boxes over 32^3 tiles of the cube
     const int T[3] = {(nx + 31) / 32, (ny + 31) / 32, (nz + 31) / 32};
@@ -642,13 +646,17 @@ int vr_set_option(vr_ctx* ctx, int option, int value) {
     if (!ctx) return VR_ERR_INVALID_ARG;
     if (option == VR_OPT_SKIP) { ctx->opt_skip = value ? 1 : 0; return VR_OK; }
     if (option == VR_OPT_CELL_SKIP) { ctx->opt_cell_skip = value ? 1 : 0; return VR_OK; }
+    if (option == VR_OPT_LAYOUT) {
+        if (value != 0 && value != 1) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: layout must be 0 (rows) or 1 (4x4x2 blocks)");
+        ctx->opt_layout = value; return VR_OK;                  // takes effect at the next upload / generate / attach
+    }
     if (option == VR_OPT_L2_FETCH) {
         if (value != 32 && value != 64 && value != 128) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: L2 fetch granularity must be 32, 64 or 128");
         VR_CUDA(ctx, cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)value));
         return VR_OK;
     }
     if (option == VR_OPT_VARIANT) {
-        if (value < 0 || value > 2) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");
+        if (value != 0 && value != 2) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");
         ctx->opt_variant = value; return VR_OK;
     }
     return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown option");

@@ -9,14 +9,23 @@ namespace {
 
 struct Elem { int b[3]; int l[3]; int g[3]; bool stored; bool in_cube; };
 
-// Decompose a flat element index of the brick-major cube.
+// Decompose a storage slot (brick, offset inside the brick) of the brick-major cube.
 __device__ __forceinline__ Elem decode(const CubeDesc& c, long long brick, long long rem) {
     Elem e;
     int bi = (int)brick;
     e.b[0] = bi % c.G[0]; e.b[1] = (bi / c.G[0]) % c.G[1]; e.b[2] = bi / (c.G[0] * c.G[1]);
-    e.l[0] = (int)(rem % c.P[0]); long long r2 = rem / c.P[0];
-    e.l[1] = (int)(r2 % c.P[1]); e.l[2] = (int)(r2 / c.P[1]);
-    e.stored = e.l[2] < c.P[2];
+    if (c.layout == 0) {
+        e.l[0] = (int)(rem % c.P[0]); long long r2 = rem / c.P[0];
+        e.l[1] = (int)(r2 % c.P[1]); e.l[2] = (int)(r2 / c.P[1]);
+        e.stored = e.l[2] < c.P[2];
+    } else {
+        const int w = (int)(rem & 31);
+        long long blk = rem >> 5;
+        const int tx = (int)(blk % c.T[0]); blk /= c.T[0];
+        const int ty = (int)(blk % c.T[1]), tz = (int)(blk / c.T[1]);
+        e.l[0] = 4 * tx + (w & 3); e.l[1] = 4 * ty + ((w >> 2) & 3); e.l[2] = 2 * tz + (w >> 4);
+        e.stored = tz < c.T[2];                       // padding slots are stored too (as zeros)
+    }
     e.in_cube = e.stored;
     for (int a = 0; a < 3; ++a) {
         e.g[a] = e.b[a] * c.B[a] + e.l[a];
@@ -25,9 +34,14 @@ __device__ __forceinline__ Elem decode(const CubeDesc& c, long long brick, long 
     return e;
 }
 
+// slots iterated per brick by the kernels below
+__host__ __device__ inline long long slots_per_brick(const CubeDesc& c) {
+    return c.layout == 0 ? (long long)c.P[0] * c.P[1] * c.P[2] : c.stride;
+}
+
 __global__ void rebrick_kernel(CubeDesc c, float* __restrict__ cube, const float* __restrict__ src,
                                int z0, int z1, int brick_lo, long long n_elems) {
-    const long long per = (long long)c.P[0] * c.P[1] * c.P[2];
+    const long long per = slots_per_brick(c);
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n_elems;
          e += (long long)gridDim.x * blockDim.x) {
         long long brick = brick_lo + e / per, rem = e % per;
@@ -44,7 +58,7 @@ __global__ void unbrick_kernel(CubeDesc c, int brick, float* __restrict__ dst, i
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n;
          e += (long long)gridDim.x * blockDim.x) {
         int x = (int)(e % ex), y = (int)((e / ex) % ey), z = (int)(e / ((long long)ex * ey));
-        dst[e] = B[x + (long long)c.P[0] * (y + (long long)c.P[1] * z)];
+        dst[e] = B[voxel_slot(c, x, y, z)];
     }
 }
 
@@ -69,10 +83,10 @@ __global__ void cell_minmax_kernel(CubeDesc c) {
         if (!empty) {
             const float* B = c.cube + (long long)brick * c.stride;
             for (int z = lo[2]; z <= hi[2]; ++z)
-                for (int y = lo[1]; y <= hi[1]; ++y) {
-                    const float* row = B + (long long)c.P[0] * (y + (long long)c.P[1] * z);
-                    for (int x = lo[0]; x <= hi[0]; ++x) { float v = __ldg(row + x); mn = fminf(mn, v); mx = fmaxf(mx, v); }
-                }
+                for (int y = lo[1]; y <= hi[1]; ++y)
+                    for (int x = lo[0]; x <= hi[0]; ++x) {
+                        float v = __ldg(B + voxel_slot(c, x, y, z)); mn = fminf(mn, v); mx = fmaxf(mx, v);
+                    }
         }
         c.cell_mm[e] = make_float2(mn, mx);
     }
@@ -115,7 +129,7 @@ __device__ __forceinline__ double gauss_noise(uint64_t seed, uint64_t idx) {
 }
 
 __global__ void generate_kernel(CubeDesc c, float* __restrict__ cube, GenDev g, long long n_elems) {
-    const long long per = (long long)c.P[0] * c.P[1] * c.P[2];
+    const long long per = slots_per_brick(c);
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n_elems;
          e += (long long)gridDim.x * blockDim.x) {
         long long brick = e / per, rem = e % per;
@@ -168,7 +182,7 @@ cudaError_t launch_rebrick(const CubeDesc& c, float* d_cube, const float* d_src,
     int bz_hi = (z1 - 1) / c.B[2];
     if (bz_hi > c.G[2] - 1) bz_hi = c.G[2] - 1;
     long long layer = (long long)c.G[0] * c.G[1];
-    long long per = (long long)c.P[0] * c.P[1] * c.P[2];
+    long long per = slots_per_brick(c);
     long long n = layer * (bz_hi - bz_lo + 1) * per;
     rebrick_kernel<<<grid_for(n, 256), 256, 0, s>>>(c, d_cube, d_src, z0, z1, (int)(layer * bz_lo), n);
     return cudaGetLastError();
@@ -193,7 +207,7 @@ cudaError_t launch_minmax(const CubeDesc& c, cudaStream_t s) {
 }
 
 cudaError_t launch_generate(const CubeDesc& c, float* d_cube, const GenDev& g, cudaStream_t s) {
-    long long n = (long long)c.nbricks * c.P[0] * c.P[1] * c.P[2];
+    long long n = (long long)c.nbricks * slots_per_brick(c);
     generate_kernel<<<grid_for(n, 256), 256, 0, s>>>(c, d_cube, g, n);
     return cudaGetLastError();
 }

@@ -14,13 +14,20 @@ constexpr int kCell = 8;            // edge of the min/max macro-cells under the
 constexpr int kTileW = 16, kTileH = 8, kThreads = 128;   // pixel tile of one CTA: 4 warps of 8x4
 
 // Brick-major cube in HBM.  Brick b = bx + G0 (by + G1 bz) occupies
-// `stride` floats; voxel (lx,ly,lz) of it, 0 <= l <= B (the +1 is the one-sided halo), sits at
-// lx + P0 (ly + P1 lz).  Halo voxels beyond the cube are zero.
+// `stride` floats; it stores voxels (lx,ly,lz), 0 <= l <= B (the +1 is the one-sided halo).
+// Halo voxels beyond the cube and padding slots are zero.  Two layouts inside a brick:
+//  layout 0 (rows):   offset = lx + P0 (ly + P1 lz), P0 = roundup4(B0 + 1);
+//  layout 1 (blocks): 4 x 4 x 2 micro-blocks of 32 voxels = one 128-byte line each,
+//                     offset = 32 ((lx>>2) + T0 ((ly>>2) + T1 (lz>>1))) + 16 (lz&1) + 4 (ly&3) + (lx&3),
+//                     so that a ray's 2 x 2 x 2 footprints meet about the same number of lines
+//                     whatever its direction.
 struct CubeDesc {
     int N[3];        // voxels
     int B[3];        // configured brick size
     int G[3];        // brick grid
-    int P[3];        // padded brick extents: P0 = roundup4(B0 + 1), P1 = B1 + 1, P2 = B2 + 1
+    int P[3];        // stored brick extents: B + 1 (layout 0: P0 rounded up to a multiple of 4)
+    int layout;      // 0: rows, 1: 4x4x2 micro-blocks
+    int T[3];        // layout 1: micro-blocks per axis = ceil(P0/4), ceil(P1/4), ceil(P2/2)
     int sh[3];       // log2(B) if B is a power of two, else -1
     int C[3];        // macro-cells per brick axis = ceil(B / kCell)
     int nbricks;
@@ -57,8 +64,15 @@ struct PartialDev {        // device descriptor of one partial image
 
 enum Counter { kRays = 0, kNominal, kTaken, kVisited, kSkipped, kTerminated, kNumCounters };
 
+// offset (floats) of stored voxel (lx, ly, lz) inside its brick
+__host__ __device__ inline long long voxel_slot(const CubeDesc& c, int lx, int ly, int lz) {
+    if (c.layout == 0) return lx + (long long)c.P[0] * (ly + (long long)c.P[1] * lz);
+    return 32LL * ((lx >> 2) + (long long)c.T[0] * ((ly >> 2) + (long long)c.T[1] * (lz >> 1))) +
+           16 * (lz & 1) + 4 * (ly & 3) + (lx & 3);
+}
+
 size_t align_up(size_t v, size_t a);
-void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz);
+void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz, int layout);
 size_t cube_bytes(const CubeDesc& c);
 struct MetaLayout { size_t brick_mm, cell_mm, cell_bits, brick_active, total; };
 MetaLayout meta_layout(const CubeDesc& c);

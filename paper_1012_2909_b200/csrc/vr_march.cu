@@ -95,98 +95,80 @@ __device__ __forceinline__ int floor_pos(float p, float& fl) {
 
 __device__ __forceinline__ float lerp(float a, float b, float w) { return __fmaf_rn(w, __fsub_rn(b, a), a); }   // O-4
 
-// The 8 corner voxels of the trilinear cell a ray is in, kept in registers between samples
-// (DESIGN.md "Cell cache").  With a step of half a voxel consecutive samples mostly fall in the
-// same cell or in a face neighbour, so a sample needs 0 or 4 new voxels instead of 8.  The values
-// are the voxels themselves, so the interpolated result does not depend on the cache.
-struct Cell {
-    float c000, c100, c010, c110, c001, c101, c011, c111;
-    int ix, iy, iz;                       // cell index (global voxel coordinates); ix < 0: invalid
-};
-constexpr int kNoCell = -(1 << 30);
-
+// One brick as the sampler sees it.  s0 / s1: layout 0 - row pitch P0 and plane pitch P0 P1;
+// layout 1 - floats per row of micro-blocks (32 T0) and per plane of micro-blocks (32 T0 T1).
 struct BrickRef {
-    const float* base;     // first float of the brick
-    unsigned off0;         // lo0 + P0 lo1 + P01 lo2 (mod 2^32): subtracting it makes offsets brick-local
-    unsigned P0, P01;
+    const float* base;
+    int lo[3];
+    unsigned s0, s1;
 };
 
-__device__ __forceinline__ unsigned voxel_offset(const BrickRef& b, int ix, int iy, int iz) {
-    return (unsigned)ix + b.P0 * (unsigned)iy + b.P01 * (unsigned)iz - b.off0;
+template <int LAYOUT>
+__device__ __forceinline__ BrickRef brick_ref(const CubeDesc& c, int bid, const int lo[3]) {
+    BrickRef b;
+    b.base = c.cube + (long long)bid * c.stride;
+    b.lo[0] = lo[0]; b.lo[1] = lo[1]; b.lo[2] = lo[2];
+    if (LAYOUT == 0) { b.s0 = (unsigned)c.P[0]; b.s1 = (unsigned)(c.P[0] * c.P[1]); }
+    else { b.s0 = 32u * (unsigned)c.T[0]; b.s1 = 32u * (unsigned)(c.T[0] * c.T[1]); }
+    return b;
 }
 
-__device__ __forceinline__ void cell_load_all(const BrickRef& b, int ix, int iy, int iz, Cell& cc) {
-    const float* q = b.base + voxel_offset(b, ix, iy, iz);
-    cc.c000 = __ldg(q);                 cc.c100 = __ldg(q + 1);
-    cc.c010 = __ldg(q + b.P0);          cc.c110 = __ldg(q + b.P0 + 1);
-    cc.c001 = __ldg(q + b.P01);         cc.c101 = __ldg(q + b.P01 + 1);
-    cc.c011 = __ldg(q + b.P01 + b.P0);  cc.c111 = __ldg(q + b.P01 + b.P0 + 1);
-}
-
-// Move the cached cell to (ix, iy, iz): one face shift (4 new voxels) per axis that moved by one,
-// through the intermediate cells (ix, cy, cz) -> (ix, iy, cz) -> (ix, iy, iz), all of which lie in
-// the brick because the old and the new cell do.  Anything else reloads the 8 voxels.
-__device__ __forceinline__ void cell_move(const BrickRef& b, int ix, int iy, int iz, Cell& cc) {
-    const int ddx = ix - cc.ix, ddy = iy - cc.iy, ddz = iz - cc.iz;
-    if ((unsigned)(ddx + 1) <= 2u && (unsigned)(ddy + 1) <= 2u && (unsigned)(ddz + 1) <= 2u) {
-        if (ddx != 0) {
-            const float* q = b.base + voxel_offset(b, ix, cc.iy, cc.iz);
-            if (ddx > 0) {
-                cc.c000 = cc.c100; cc.c010 = cc.c110; cc.c001 = cc.c101; cc.c011 = cc.c111;
-                cc.c100 = __ldg(q + 1);         cc.c110 = __ldg(q + b.P0 + 1);
-                cc.c101 = __ldg(q + b.P01 + 1); cc.c111 = __ldg(q + b.P01 + b.P0 + 1);
-            } else {
-                cc.c100 = cc.c000; cc.c110 = cc.c010; cc.c101 = cc.c001; cc.c111 = cc.c011;
-                cc.c000 = __ldg(q);             cc.c010 = __ldg(q + b.P0);
-                cc.c001 = __ldg(q + b.P01);     cc.c011 = __ldg(q + b.P01 + b.P0);
-            }
-        }
-        if (ddy != 0) {
-            const float* q = b.base + voxel_offset(b, ix, iy, cc.iz);
-            if (ddy > 0) {
-                cc.c000 = cc.c010; cc.c100 = cc.c110; cc.c001 = cc.c011; cc.c101 = cc.c111;
-                cc.c010 = __ldg(q + b.P0);          cc.c110 = __ldg(q + b.P0 + 1);
-                cc.c011 = __ldg(q + b.P01 + b.P0);  cc.c111 = __ldg(q + b.P01 + b.P0 + 1);
-            } else {
-                cc.c010 = cc.c000; cc.c110 = cc.c100; cc.c011 = cc.c001; cc.c111 = cc.c101;
-                cc.c000 = __ldg(q);                 cc.c100 = __ldg(q + 1);
-                cc.c001 = __ldg(q + b.P01);         cc.c101 = __ldg(q + b.P01 + 1);
-            }
-        }
-        if (ddz != 0) {
-            const float* q = b.base + voxel_offset(b, ix, iy, iz);
-            if (ddz > 0) {
-                cc.c000 = cc.c001; cc.c100 = cc.c101; cc.c010 = cc.c011; cc.c110 = cc.c111;
-                cc.c001 = __ldg(q + b.P01);         cc.c101 = __ldg(q + b.P01 + 1);
-                cc.c011 = __ldg(q + b.P01 + b.P0);  cc.c111 = __ldg(q + b.P01 + b.P0 + 1);
-            } else {
-                cc.c001 = cc.c000; cc.c101 = cc.c100; cc.c011 = cc.c010; cc.c111 = cc.c110;
-                cc.c000 = __ldg(q);                 cc.c100 = __ldg(q + 1);
-                cc.c010 = __ldg(q + b.P0);          cc.c110 = __ldg(q + b.P0 + 1);
-            }
-        }
-    } else {
-        cell_load_all(b, ix, iy, iz, cc);
+// The 8 voxels of the trilinear cell whose lower corner is (ix, iy, iz) (global voxel indices,
+// inside brick b or on its halo), in the order 000 100 010 110 001 101 011 111.
+template <int LAYOUT>
+__device__ __forceinline__ void gather8(const BrickRef& b, int ix, int iy, int iz, float v[8]) {
+    const unsigned lx = (unsigned)(ix - b.lo[0]), ly = (unsigned)(iy - b.lo[1]), lz = (unsigned)(iz - b.lo[2]);
+    unsigned q, dx, dy, dz;
+    if (LAYOUT == 0) {
+        q = lx + b.s0 * ly + b.s1 * lz;
+        dx = 1u; dy = b.s0; dz = b.s1;
+    } else {                              // step to the +1 neighbour: inside the micro-block or into the next one
+        q = ((lx >> 2) << 5) + (lx & 3u) + (ly >> 2) * b.s0 + ((ly & 3u) << 2) + (lz >> 1) * b.s1 + ((lz & 1u) << 4);
+        dx = (lx & 3u) == 3u ? 29u : 1u;
+        dy = (ly & 3u) == 3u ? b.s0 - 12u : 4u;
+        dz = (lz & 1u) ? b.s1 - 16u : 16u;
     }
-    cc.ix = ix; cc.iy = iy; cc.iz = iz;
+    const float* p = b.base + q;
+    v[0] = __ldg(p);           v[1] = __ldg(p + dx);
+    v[2] = __ldg(p + dy);      v[3] = __ldg(p + dy + dx);
+    v[4] = __ldg(p + dz);      v[5] = __ldg(p + dz + dx);
+    v[6] = __ldg(p + dz + dy); v[7] = __ldg(p + dz + dy + dx);
 }
 
-// O-4 trilinear at p (floor(p) inside brick b).  VAR 0 reads the 8 voxels of every sample, VAR 1
-// goes through the cell cache.
-template <int VAR>
-__device__ __forceinline__ float sample(const BrickRef& b, const float p[3], Cell& cc) {
-    float fx, fy, fz;
+__device__ __forceinline__ float trilinear(const float v[8], float wx, float wy, float wz) {   // O-4: x, then y, then z
+    const float c00 = lerp(v[0], v[1], wx), c10 = lerp(v[2], v[3], wx);
+    const float c01 = lerp(v[4], v[5], wx), c11 = lerp(v[6], v[7], wx);
+    return lerp(lerp(c00, c10, wy), lerp(c01, c11, wy), wz);
+}
+
+template <int LAYOUT>
+__device__ __forceinline__ float sample(const BrickRef& b, const float p[3]) {
+    float fx, fy, fz, v[8];
     const int ix = floor_pos(p[0], fx), iy = floor_pos(p[1], fy), iz = floor_pos(p[2], fz);
-    const float wx = __fsub_rn(p[0], fx), wy = __fsub_rn(p[1], fy), wz = __fsub_rn(p[2], fz);
-    if (VAR == 0) cell_load_all(b, ix, iy, iz, cc);
-    else if (ix != cc.ix || iy != cc.iy || iz != cc.iz) cell_move(b, ix, iy, iz, cc);
-    const float c00 = lerp(cc.c000, cc.c100, wx), c10 = lerp(cc.c010, cc.c110, wx);
-    const float c01 = lerp(cc.c001, cc.c101, wx), c11 = lerp(cc.c011, cc.c111, wx);
-    const float c0 = lerp(c00, c10, wy), c1 = lerp(c01, c11, wy);
-    return lerp(c0, c1, wz);
+    gather8<LAYOUT>(b, ix, iy, iz, v);
+    return trilinear(v, __fsub_rn(p[0], fx), __fsub_rn(p[1], fy), __fsub_rn(p[2], fz));
 }
 
 struct Accum { float C[3]; float A; float m; };
+
+// O-6 lookup of table coordinate x (already scaled, not yet clamped) in the baked table.
+__device__ __forceinline__ float4 tf_at(const float4* __restrict__ tab, float x) {
+    x = fminf(fmaxf(x, 0.f), 255.f);
+    float fl;
+    const int i = min(floor_pos(x, fl), 254);
+    const float f = __fsub_rn(x, fminf(fl, 254.f));
+    const float4 a = tab[i], b = tab[i + 1];
+    return make_float4(lerp(a.x, b.x, f), lerp(a.y, b.y, f), lerp(a.z, b.z, f), lerp(a.w, b.w, f));
+}
+
+__device__ __forceinline__ bool over(Accum& acc, float cr, float cg, float cb, float ca, float tau) {   // O-7
+    const float w = __fmul_rn(__fsub_rn(1.f, acc.A), ca);
+    acc.C[0] = __fmaf_rn(w, cr, acc.C[0]);
+    acc.C[1] = __fmaf_rn(w, cg, acc.C[1]);
+    acc.C[2] = __fmaf_rn(w, cb, acc.C[2]);
+    acc.A = __fadd_rn(acc.A, w);
+    return acc.A >= tau;
+}
 
 // O-5 / O-6 / O-7: fold one sample value into the ray's accumulator.  A sample whose table
 // coordinate x lies below T.x_clear falls between two entries of zero opacity: its weight
@@ -194,20 +176,10 @@ struct Accum { float C[3]; float A; float m; };
 template <int MODE>
 __device__ __forceinline__ bool fold(Accum& acc, float v, const float4* tab, const TFDesc& T, float tau) {
     if (MODE == VR_MODE_MIP) { acc.m = fmaxf(acc.m, v); return false; }
-    float x = __fmul_rn(__fsub_rn(v, T.vmin), T.scale);
+    const float x = __fmul_rn(__fsub_rn(v, T.vmin), T.scale);
     if (x < T.x_clear) return false;
-    x = fminf(fmaxf(x, 0.f), 255.f);
-    float fl;
-    const int i = min(floor_pos(x, fl), 254);
-    const float f = __fsub_rn(x, fminf(fl, 254.f));
-    const float4 a = tab[i], b = tab[i + 1];
-    const float qa = lerp(a.w, b.w, f);
-    const float w = __fmul_rn(__fsub_rn(1.f, acc.A), qa);        // O-7
-    acc.C[0] = __fmaf_rn(w, lerp(a.x, b.x, f), acc.C[0]);
-    acc.C[1] = __fmaf_rn(w, lerp(a.y, b.y, f), acc.C[1]);
-    acc.C[2] = __fmaf_rn(w, lerp(a.z, b.z, f), acc.C[2]);
-    acc.A = __fadd_rn(acc.A, w);
-    return acc.A >= tau;
+    const float4 q = tf_at(tab, x);
+    return over(acc, q.x, q.y, q.z, q.w, tau);
 }
 
 // Conservative number (>= 1) of samples, starting at the one at p, whose floor(position) stays in
@@ -279,50 +251,62 @@ __device__ __forceinline__ void brick_interval(const CubeDesc& c, const Ray& r, 
     }
 }
 
-struct Stats { unsigned long long taken, visit, skip; };
-
-__device__ __forceinline__ BrickRef brick_ref(const CubeDesc& c, int bid, const int lo[3]) {
-    BrickRef b;
-    b.base = c.cube + (long long)bid * c.stride;
-    b.P0 = (unsigned)c.P[0]; b.P01 = (unsigned)(c.P[0] * c.P[1]);
-    b.off0 = (unsigned)lo[0] + b.P0 * (unsigned)lo[1] + b.P01 * (unsigned)lo[2];
-    return b;
+// Which partial does this CTA's tile belong to, and which pixel of it is this thread's.
+__device__ __forceinline__ bool locate_tile(const PartialDev* __restrict__ parts, int n_parts, PartialDev& part, int& lx, int& ly) {
+    if (threadIdx.x == 0) {
+        int lo = 0, hi = n_parts - 1;
+        const int tile = blockIdx.x;
+        while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (parts[mid].tile0 <= tile) lo = mid; else hi = mid - 1; }
+        part = parts[lo];
+    }
+    __syncthreads();
+    int tx, ty; tile_pixel(tx, ty);
+    const int tiles_x = (part.w + kTileW - 1) / kTileW;
+    const int tile = blockIdx.x - part.tile0;
+    lx = (tile % tiles_x) * kTileW + tx; ly = (tile / tiles_x) * kTileH + ty;
+    return lx < part.w && ly < part.h;
 }
 
+// O-10 at the 8^3 macro-cell level for the sample whose cell has lower corner (ix, iy, iz) in
+// brick bid: true if the sample cannot contribute.  EA: every table entry the cell's value range
+// can touch has zero opacity (one bit per cell, classify_cells_kernel); MIP: the cell's maximum
+// cannot raise m.
+template <int MODE>
+__device__ __forceinline__ bool cell_idle(const CubeDesc& c, int bid, const int lo[3], int ix, int iy, int iz, float m) {
+    const int cidx = ((ix - lo[0]) >> 3) + c.C[0] * (((iy - lo[1]) >> 3) + c.C[1] * ((iz - lo[2]) >> 3));
+    if (MODE == VR_MODE_MIP) return __ldg(&c.cell_mm[(long long)bid * c.cells_per_brick + cidx]).y <= m;
+    return ((__ldg(&c.cell_bits[(long long)bid * c.cell_words_per_brick + (cidx >> 5)]) >> (cidx & 31)) & 1u) == 0u;
+}
+
+struct Stats { unsigned long long taken, visit, skip; };
+
+// ================================================================== variant 0: one ray per thread
 // March the lattice samples k .. ke (all of them members of brick `bid`, O-3) into `acc`.  With
-// A.skip >= 2 the interval is cut into runs inside 8^3 macro-cells and a run is skipped when its
-// cell cannot contribute (O-10, exact): EA - every table entry its value range can touch has zero
-// opacity (bit precomputed per transfer function); MIP - the cell's maximum cannot raise m.
+// A.skip >= 2 the interval is cut into runs inside 8^3 macro-cells and idle runs are jumped.
 // Returns true if early ray termination fired.
-template <int MODE, int VAR>
+template <int MODE, int LAYOUT>
 __device__ __forceinline__ bool march_interval(const CubeDesc& c, const Ray& r, const TFDesc& T, const RenderArgs& A,
                                                const float4* tab, int bid, const int lo[3], int k, int ke,
                                                Accum& acc, Stats& st) {
-    const BrickRef b = brick_ref(c, bid, lo);
+    const BrickRef b = brick_ref<LAYOUT>(c, bid, lo);
     const int S8[3] = {kCell, kCell, kCell};
-    Cell cc;
-    cc.ix = cc.iy = cc.iz = kNoCell;
     float kf = (float)k;                                    // exact: k < 2^24
     while (k <= ke) {
         int n = ke - k + 1;
         if (A.skip >= 2) {
             float p[3], fl;
             position(r, kf, p);
-            const int cl[3] = {(floor_pos(p[0], fl) - lo[0]) >> 3, (floor_pos(p[1], fl) - lo[1]) >> 3,
-                               (floor_pos(p[2], fl) - lo[2]) >> 3};
-            const int clo[3] = {lo[0] + (cl[0] << 3), lo[1] + (cl[1] << 3), lo[2] + (cl[2] << 3)};
+            const int iv[3] = {floor_pos(p[0], fl), floor_pos(p[1], fl), floor_pos(p[2], fl)};
+            const int clo[3] = {lo[0] + (((iv[0] - lo[0]) >> 3) << 3), lo[1] + (((iv[1] - lo[1]) >> 3) << 3),
+                                lo[2] + (((iv[2] - lo[2]) >> 3) << 3)};
             n = min(n, run_length(r, p, clo, S8));
-            const int cidx = cl[0] + c.C[0] * (cl[1] + c.C[1] * cl[2]);
-            bool skip;
-            if (MODE == VR_MODE_MIP) skip = __ldg(&c.cell_mm[(long long)bid * c.cells_per_brick + cidx]).y <= acc.m;
-            else skip = ((__ldg(&c.cell_bits[(long long)bid * c.cell_words_per_brick + (cidx >> 5)]) >> (cidx & 31)) & 1u) == 0u;
-            if (skip) { k += n; kf = __fadd_rn(kf, (float)n); ++st.skip; continue; }
+            if (cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], acc.m)) { k += n; kf = __fadd_rn(kf, (float)n); ++st.skip; continue; }
         }
         ++st.visit;
         for (const int e = k + n; k < e; ++k, kf = __fadd_rn(kf, 1.f)) {
             float p[3];
             position(r, kf, p);
-            const float v = sample<VAR>(b, p, cc);
+            const float v = sample<LAYOUT>(b, p);
             ++st.taken;
             if (fold<MODE>(acc, v, tab, T, A.tau)) return true;
         }
@@ -330,8 +314,28 @@ __device__ __forceinline__ bool march_interval(const CubeDesc& c, const Ray& r, 
     return false;
 }
 
+__device__ __forceinline__ float4 raw_tf_at(const TFDesc& T, float m) {
+    float x = __fmul_rn(__fsub_rn(m, T.vmin), T.scale);
+    return tf_at(T.raw, x);
+}
+
+template <int MODE>
+__device__ __forceinline__ void write_frame_pixel(const ViewDesc& V, const TFDesc& T, const RenderArgs& A, int i, int j,
+                                                  const Accum& acc, bool any) {
+    const long long px = (long long)(V.vy0 + j) * V.pitch + (V.vx0 + i);
+    if (MODE == VR_MODE_MIP) {
+        A.out[px] = any ? acc.m : A.miss;
+        if (A.out_rgba)
+            reinterpret_cast<float4*>(A.out_rgba)[px] = any ? raw_tf_at(T, acc.m) : make_float4(0.f, 0.f, 0.f, 0.f);
+    } else {                                               // O-7: premultiplied colour over bg
+        const float t = __fsub_rn(1.f, acc.A);
+        reinterpret_cast<float4*>(A.out)[px] = make_float4(__fmaf_rn(t, A.bg[0], acc.C[0]), __fmaf_rn(t, A.bg[1], acc.C[1]),
+                                                           __fmaf_rn(t, A.bg[2], acc.C[2]), __fmaf_rn(t, A.bg[3], acc.A));
+    }
+}
+
 // ---------------------------------------------------------------- whole frame, O-8 GLOBAL
-template <int MODE, int VAR>
+template <int MODE, int LAYOUT>
 __global__ void __launch_bounds__(kThreads)
 render_global_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                      const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A) {
@@ -361,33 +365,10 @@ render_global_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
             else skip = c.brick_active[bid] == 0;
         }
         if (skip) { k += n; ++st.skip; continue; }
-        if (march_interval<MODE, VAR>(c, r, T, A, tab, bid, lo, k, k + n - 1, acc, st)) { stopped = true; break; }
+        if (march_interval<MODE, LAYOUT>(c, r, T, A, tab, bid, lo, k, k + n - 1, acc, st)) { stopped = true; break; }
         k += n;
     }
-    if (live) {
-        const long long px = (long long)(V.vy0 + j) * V.pitch + (V.vx0 + i);
-        if (MODE == VR_MODE_MIP) {
-            const bool any = r.k1 >= r.k0;
-            A.out[px] = any ? acc.m : A.miss;
-            if (A.out_rgba) {
-                float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (any) {
-                    float x = __fmul_rn(__fsub_rn(acc.m, T.vmin), T.scale);
-                    x = fminf(fmaxf(x, 0.f), 255.f);
-                    float fl; int ii = min(floor_pos(x, fl), 254);
-                    float f = __fsub_rn(x, (float)ii);
-                    float4 a = T.raw[ii], bb = T.raw[ii + 1];
-                    q = make_float4(lerp(a.x, bb.x, f), lerp(a.y, bb.y, f), lerp(a.z, bb.z, f), lerp(a.w, bb.w, f));
-                }
-                reinterpret_cast<float4*>(A.out_rgba)[px] = q;
-            }
-        } else {                                           // O-7: premultiplied colour over bg
-            float t = __fsub_rn(1.f, acc.A);
-            float4 o = make_float4(__fmaf_rn(t, A.bg[0], acc.C[0]), __fmaf_rn(t, A.bg[1], acc.C[1]),
-                                   __fmaf_rn(t, A.bg[2], acc.C[2]), __fmaf_rn(t, A.bg[3], acc.A));
-            reinterpret_cast<float4*>(A.out)[px] = o;
-        }
-    }
+    if (live) write_frame_pixel<MODE>(V, T, A, i, j, acc, r.k1 >= r.k0);
     if (A.counters) {
         const unsigned long long nom = r.k1 >= r.k0 ? (unsigned long long)(r.k1 - r.k0 + 1) : 0ULL;
         count(A.counters, kRays, nom ? 1 : 0);
@@ -400,25 +381,16 @@ render_global_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
 }
 
 // ---------------------------------------------------------------- per-brick partial images (O-8 SORT-LAST)
-template <int MODE, int VAR>
+template <int MODE, int LAYOUT>
 __global__ void __launch_bounds__(kThreads)
 render_bricks_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                      const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
                      const PartialDev* __restrict__ parts, int n_parts) {
     __shared__ float4 tab[256];
     __shared__ PartialDev part;
-    if (threadIdx.x == 0) {           // which partial does this CTA's tile belong to?
-        int lo = 0, hi = n_parts - 1;
-        const int tile = blockIdx.x;
-        while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (parts[mid].tile0 <= tile) lo = mid; else hi = mid - 1; }
-        part = parts[lo];
-    }
-    if (MODE == VR_MODE_EA) load_tf(tab, T.baked); else __syncthreads();
-    int tx, ty; tile_pixel(tx, ty);
-    const int tiles_x = (part.w + kTileW - 1) / kTileW;
-    const int tile = blockIdx.x - part.tile0;
-    const int lx = (tile % tiles_x) * kTileW + tx, ly = (tile / tiles_x) * kTileH + ty;
-    const bool live = lx < part.w && ly < part.h;
+    int lx, ly;
+    const bool live = locate_tile(parts, n_parts, part, lx, ly);
+    if (MODE == VR_MODE_EA) load_tf(tab, T.baked);
     Ray r; r.k0 = 0; r.k1 = -1;
     if (live) setup_ray(V, c, part.x0 + lx, part.y0 + ly, r);
     const int bid = part.brick;
@@ -428,7 +400,7 @@ render_bricks_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
     brick_interval(c, r, b, lo, ka, kb);
     Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
     Stats st = {0, 0, 0};
-    const bool stopped = march_interval<MODE, VAR>(c, r, T, A, tab, bid, lo, ka, kb, acc, st);
+    const bool stopped = march_interval<MODE, LAYOUT>(c, r, T, A, tab, bid, lo, ka, kb, acc, st);
     if (live) {
         const long long px = (long long)ly * part.pitch + lx;
         if (MODE == VR_MODE_MIP) reinterpret_cast<float*>(part.data)[px] = acc.m;
@@ -443,36 +415,58 @@ render_bricks_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
     }
 }
 
-// ---------------------------------------------------------------- sort-last, one ray per warp
-// Variant 2 ("sample-parallel").  The 128 threads of a CTA first set up
-// the 128 rays of their pixel tile exactly as above (one ray per thread).  Then every warp walks
-// through its own 32 rays one after the other, and the 32 lanes take 32 CONSECUTIVE lattice
-// samples k .. k+31 of that one ray: positions, voxel gathers and trilinear interpolation run in
-// parallel, and the lanes' addresses follow the ray, so every 32-byte sector the ray needs is
-// fetched once and used at once - nothing has to survive in L1/L2 between iterations, whatever
-// the view direction.  The front-to-back fold stays sequential in k (O-7): opaque samples are
-// picked out with a ballot and folded in ascending order through shuffles, all lanes keeping the
-// same accumulator; transparent samples (x < x_clear) contribute exact zeros and are not folded.
-// MIP folds with a warp maximum (exact in any order).
+// ================================================================== variant 2: one ray per warp
+// ("sample-parallel").  The 128 threads of a CTA first set up the 128
+// rays of their pixel tile exactly as above (one ray per thread).  Then every warp walks through
+// its own 32 rays one after the other, and the 32 lanes take 32 CONSECUTIVE lattice samples
+// k .. k+31 of that one ray: positions, voxel gathers and trilinear interpolation run in parallel,
+// and the lanes' addresses follow the ray, so the lines the ray needs are fetched once and used at
+// once - nothing has to survive in L1/L2 between iterations, whatever the view direction.  The
+// gathers of the next 32 samples are issued before the current ones are folded.  The
+// front-to-back fold stays sequential in k (O-7): opaque samples are picked out with a ballot
+// and folded in ascending order through shuffles, all lanes keeping the same accumulator;
+// transparent samples (x < x_clear) contribute exact zeros and are not folded.  MIP folds with a
+// warp maximum (exact in any order).
+struct Lane8 { float v[8]; float w[3]; bool idle; };
+
+// Fold the 32 values `val` (lane = sample, `act` = the lane holds a taken, non-skipped sample) of
+// one ray into acc (identical in all lanes).  Returns the number of samples consumed if ERT
+// fired (>= 1), else 0.
 template <int MODE>
+__device__ __forceinline__ int fold32(Accum& acc, float val, bool act, const float4* tab, const TFDesc& T, float tau) {
+    if (MODE == VR_MODE_MIP) {
+        float m = act ? val : -INFINITY;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+        acc.m = fmaxf(acc.m, m);
+        return 0;
+    }
+    const float x = __fmul_rn(__fsub_rn(val, T.vmin), T.scale);
+    const bool opaque = act && !(x < T.x_clear);
+    unsigned bits = __ballot_sync(0xffffffffu, opaque);
+    if (!bits) return 0;
+    float4 col = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (opaque) col = tf_at(tab, x);                        // O-6, one sample per lane
+    while (bits) {                                          // O-7, ascending k
+        const int j = __ffs(bits) - 1;
+        bits &= bits - 1;
+        const float cr = __shfl_sync(0xffffffffu, col.x, j), cg = __shfl_sync(0xffffffffu, col.y, j);
+        const float cb = __shfl_sync(0xffffffffu, col.z, j), ca = __shfl_sync(0xffffffffu, col.w, j);
+        if (over(acc, cr, cg, cb, ca, tau)) return j + 1;
+    }
+    return 0;
+}
+
+template <int MODE, int LAYOUT>
 __global__ void __launch_bounds__(kThreads)
 render_bricks_sp_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                         const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
                         const PartialDev* __restrict__ parts, int n_parts) {
     __shared__ float4 tab[256];
     __shared__ PartialDev part;
-    if (threadIdx.x == 0) {
-        int lo = 0, hi = n_parts - 1;
-        const int tile = blockIdx.x;
-        while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (parts[mid].tile0 <= tile) lo = mid; else hi = mid - 1; }
-        part = parts[lo];
-    }
-    if (MODE == VR_MODE_EA) load_tf(tab, T.baked); else __syncthreads();
-    int tx, ty; tile_pixel(tx, ty);
-    const int tiles_x = (part.w + kTileW - 1) / kTileW;
-    const int tile = blockIdx.x - part.tile0;
-    const int lx = (tile % tiles_x) * kTileW + tx, ly = (tile / tiles_x) * kTileH + ty;
-    const bool live = lx < part.w && ly < part.h;
+    int lx, ly;
+    const bool live = locate_tile(parts, n_parts, part, lx, ly);
+    if (MODE == VR_MODE_EA) load_tf(tab, T.baked);
     Ray r; r.k0 = 0; r.k1 = -1;
     r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
     if (live) setup_ray(V, c, part.x0 + lx, part.y0 + ly, r);
@@ -481,12 +475,12 @@ render_bricks_sp_kernel(const __grid_constant__ CubeDesc c, const __grid_constan
     const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
     int ka = r.k0, kb = r.k1;
     brick_interval(c, r, b, lo, ka, kb);
-    const BrickRef br = brick_ref(c, bid, lo);
+    const BrickRef br = brick_ref<LAYOUT>(c, bid, lo);
     const int lane = threadIdx.x & 31;
+    const bool cells = A.skip >= 2;
     Accum mine = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-    unsigned long long n_taken = 0, n_term = 0, n_visit = 0;
-    const unsigned todo = __ballot_sync(0xffffffffu, ka <= kb);
-    for (unsigned rays = todo; rays; rays &= rays - 1) {
+    unsigned long long n_taken = 0, n_term = 0, n_visit = 0, n_skip = 0;
+    for (unsigned rays = __ballot_sync(0xffffffffu, ka <= kb); rays; rays &= rays - 1) {
         const int src = __ffs(rays) - 1;
         Ray q;
         q.step = r.step;
@@ -494,50 +488,38 @@ render_bricks_sp_kernel(const __grid_constant__ CubeDesc c, const __grid_constan
         for (int a = 0; a < 3; ++a) { q.o[a] = __shfl_sync(0xffffffffu, r.o[a], src); q.d[a] = __shfl_sync(0xffffffffu, r.d[a], src); }
         const int qa = __shfl_sync(0xffffffffu, ka, src), qb = __shfl_sync(0xffffffffu, kb, src);
         Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-        bool stopped = false;
-        for (int k0 = qa; k0 <= qb && !stopped; k0 += 32) {
-            const int k = k0 + lane;
-            const bool act = k <= qb;
-            float p[3];
-            position(q, (float)min(k, qb), p);               // idle lanes repeat the last sample
-            Cell cc;
-            const float v = sample<0>(br, p, cc);
-            if (MODE == VR_MODE_MIP) {
-                float m = act ? v : -INFINITY;
+        // issue the gathers of samples k0 + lane (idle lanes repeat the ray's last sample)
+        auto issue = [&](int k0, Lane8& L) {
+            float p[3], fx, fy, fz;
+            position(q, (float)min(k0 + lane, qb), p);
+            const int ix = floor_pos(p[0], fx), iy = floor_pos(p[1], fy), iz = floor_pos(p[2], fz);
+            L.w[0] = __fsub_rn(p[0], fx); L.w[1] = __fsub_rn(p[1], fy); L.w[2] = __fsub_rn(p[2], fz);
+            L.idle = cells && cell_idle<MODE>(c, bid, lo, ix, iy, iz, acc.m);
+            if (!L.idle) gather8<LAYOUT>(br, ix, iy, iz, L.v);
+            else {
 #pragma unroll
-                for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-                acc.m = fmaxf(acc.m, m);
-                if (lane == 0) n_taken += (unsigned long long)(min(qb - k0, 31) + 1);
-            } else {
-                float x = __fmul_rn(__fsub_rn(v, T.vmin), T.scale);
-                const bool opaque = act && !(x < T.x_clear);
-                unsigned bits = __ballot_sync(0xffffffffu, opaque);
-                int n_here = min(qb - k0, 31) + 1;
-                if (bits) {
-                    float4 col = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (opaque) {                           // O-6 lookup, one sample per lane
-                        x = fminf(fmaxf(x, 0.f), 255.f);
-                        float fl;
-                        const int i = min(floor_pos(x, fl), 254);
-                        const float f = __fsub_rn(x, fminf(fl, 254.f));
-                        const float4 ta = tab[i], tb = tab[i + 1];
-                        col = make_float4(lerp(ta.x, tb.x, f), lerp(ta.y, tb.y, f), lerp(ta.z, tb.z, f), lerp(ta.w, tb.w, f));
-                    }
-                    while (bits) {                          // O-7, ascending k
-                        const int j = __ffs(bits) - 1;
-                        bits &= bits - 1;
-                        const float cr = __shfl_sync(0xffffffffu, col.x, j), cg = __shfl_sync(0xffffffffu, col.y, j);
-                        const float cb = __shfl_sync(0xffffffffu, col.z, j), ca = __shfl_sync(0xffffffffu, col.w, j);
-                        const float w = __fmul_rn(__fsub_rn(1.f, acc.A), ca);
-                        acc.C[0] = __fmaf_rn(w, cr, acc.C[0]);
-                        acc.C[1] = __fmaf_rn(w, cg, acc.C[1]);
-                        acc.C[2] = __fmaf_rn(w, cb, acc.C[2]);
-                        acc.A = __fadd_rn(acc.A, w);
-                        if (acc.A >= A.tau) { stopped = true; n_here = j + 1; break; }
-                    }
-                }
-                if (lane == 0) n_taken += (unsigned long long)n_here;
+                for (int e = 0; e < 8; ++e) L.v[e] = 0.f;
             }
+        };
+        Lane8 cur, nxt;
+        issue(qa, cur);
+        bool stopped = false;
+        for (int k0 = qa; k0 <= qb; k0 += 32) {
+            const bool more = k0 + 32 <= qb;
+            if (more) issue(k0 + 32, nxt);
+            const bool act = k0 + lane <= qb && !cur.idle;
+            const float val = trilinear(cur.v, cur.w[0], cur.w[1], cur.w[2]);
+            const int n_in = min(qb - k0, 31) + 1;
+            const int hit = fold32<MODE>(acc, val, act, tab, T, A.tau);
+            const unsigned idle_bits = __ballot_sync(0xffffffffu, cur.idle && k0 + lane <= qb);
+            if (lane == 0) {
+                const unsigned upto = hit ? (hit >= 32 ? 0xffffffffu : ((1u << hit) - 1u)) : 0xffffffffu;
+                const int idle_n = __popc(idle_bits & upto);
+                n_taken += (unsigned long long)((hit ? hit : n_in) - idle_n);
+                n_skip += (unsigned long long)idle_n;
+            }
+            if (hit) { stopped = true; break; }
+            cur = nxt;
         }
         if (lane == 0) { ++n_visit; n_term += stopped ? 1 : 0; }
         if (lane == src) mine = acc;
@@ -551,6 +533,88 @@ render_bricks_sp_kernel(const __grid_constant__ CubeDesc c, const __grid_constan
         count(A.counters, kNominal, kb >= ka ? (unsigned long long)(kb - ka + 1) : 0ULL);
         count(A.counters, kTaken, n_taken);
         count(A.counters, kVisited, n_visit);
+        count(A.counters, kSkipped, n_skip);
+        count(A.counters, kTerminated, n_term);
+    }
+}
+
+// Whole frame, O-8 GLOBAL, one ray per warp: the lanes' 32 consecutive samples may lie in
+// different bricks, so every lane finds its own brick (O-3 membership from its own position); the
+// accumulator is carried along the ray, so ERT and the sample order are those of the unsplit march.
+template <int MODE, int LAYOUT>
+__global__ void __launch_bounds__(kThreads)
+render_global_sp_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
+                        const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A) {
+    __shared__ float4 tab[256];
+    if (MODE == VR_MODE_EA) load_tf(tab, T.baked);
+    int tx, ty; tile_pixel(tx, ty);
+    const int i = blockIdx.x * kTileW + tx, j = blockIdx.y * kTileH + ty;
+    const bool live = i < V.W && j < V.H;
+    Ray r; r.k0 = 0; r.k1 = -1;
+    r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
+    if (live) setup_ray(V, c, i, j, r);
+    const int lane = threadIdx.x & 31;
+    Accum mine = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
+    unsigned long long n_taken = 0, n_term = 0, n_visit = 0, n_skip = 0;
+    for (unsigned rays = __ballot_sync(0xffffffffu, r.k0 <= r.k1); rays; rays &= rays - 1) {
+        const int src = __ffs(rays) - 1;
+        Ray q;
+        q.step = r.step;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { q.o[a] = __shfl_sync(0xffffffffu, r.o[a], src); q.d[a] = __shfl_sync(0xffffffffu, r.d[a], src); }
+        const int qa = __shfl_sync(0xffffffffu, r.k0, src), qb = __shfl_sync(0xffffffffu, r.k1, src);
+        Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
+        auto issue = [&](int k0, Lane8& L) {
+            float p[3], fx, fy, fz;
+            position(q, (float)min(k0 + lane, qb), p);
+            const int iv[3] = {floor_pos(p[0], fx), floor_pos(p[1], fy), floor_pos(p[2], fz)};
+            L.w[0] = __fsub_rn(p[0], fx); L.w[1] = __fsub_rn(p[1], fy); L.w[2] = __fsub_rn(p[2], fz);
+            int b[3]; brick_of(c, iv, b);
+            const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
+            const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
+            L.idle = false;
+            if (A.skip) {                                   // O-10 (exact), per sample
+                if (MODE == VR_MODE_MIP) L.idle = __ldg(&c.brick_mm[bid]).y <= acc.m;
+                else L.idle = __ldg(&c.brick_active[bid]) == 0;
+                if (A.skip >= 2 && !L.idle) L.idle = cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], acc.m);
+            }
+            if (!L.idle) { const BrickRef br = brick_ref<LAYOUT>(c, bid, lo); gather8<LAYOUT>(br, iv[0], iv[1], iv[2], L.v); }
+            else {
+#pragma unroll
+                for (int e = 0; e < 8; ++e) L.v[e] = 0.f;
+            }
+        };
+        Lane8 cur, nxt;
+        issue(qa, cur);
+        bool stopped = false;
+        for (int k0 = qa; k0 <= qb; k0 += 32) {
+            const bool more = k0 + 32 <= qb;
+            if (more) issue(k0 + 32, nxt);
+            const bool act = k0 + lane <= qb && !cur.idle;
+            const float val = trilinear(cur.v, cur.w[0], cur.w[1], cur.w[2]);
+            const int n_in = min(qb - k0, 31) + 1;
+            const int hit = fold32<MODE>(acc, val, act, tab, T, A.tau);
+            const unsigned idle_bits = __ballot_sync(0xffffffffu, cur.idle && k0 + lane <= qb);
+            if (lane == 0) {
+                const unsigned upto = hit ? (hit >= 32 ? 0xffffffffu : ((1u << hit) - 1u)) : 0xffffffffu;
+                const int idle_n = __popc(idle_bits & upto);
+                n_taken += (unsigned long long)((hit ? hit : n_in) - idle_n);
+                n_skip += (unsigned long long)idle_n;
+            }
+            if (hit) { stopped = true; break; }
+            cur = nxt;
+        }
+        if (lane == 0) { ++n_visit; n_term += stopped ? 1 : 0; }
+        if (lane == src) mine = acc;
+    }
+    if (live) write_frame_pixel<MODE>(V, T, A, i, j, mine, r.k1 >= r.k0);
+    if (A.counters) {
+        const unsigned long long nom = r.k1 >= r.k0 ? (unsigned long long)(r.k1 - r.k0 + 1) : 0ULL;
+        count(A.counters, kRays, nom ? 1 : 0);
+        count(A.counters, kNominal, nom);
+        count(A.counters, kTaken, n_taken);
+        count(A.counters, kVisited, n_visit);
+        count(A.counters, kSkipped, n_skip);
         count(A.counters, kTerminated, n_term);
     }
 }
@@ -588,33 +652,29 @@ __global__ void upload_half_kernel(float4* dst, const __grid_constant__ HalfTabl
 
 }  // namespace
 
+#define VR_DISPATCH(KERNEL, GRID, ...)                                                                   \
+    do {                                                                                                 \
+        if (a.mode == VR_MODE_MIP) {                                                                     \
+            if (c.layout == 0) KERNEL<VR_MODE_MIP, 0><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);            \
+            else KERNEL<VR_MODE_MIP, 1><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);                          \
+        } else {                                                                                         \
+            if (c.layout == 0) KERNEL<VR_MODE_EA, 0><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);             \
+            else KERNEL<VR_MODE_EA, 1><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);                           \
+        }                                                                                                \
+    } while (0)
+
 cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s) {
     dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
-    const bool mip = a.mode == VR_MODE_MIP;
-    if (a.variant == 0) {
-        if (mip) render_global_kernel<VR_MODE_MIP, 0><<<grid, kThreads, 0, s>>>(c, v, t, a);
-        else render_global_kernel<VR_MODE_EA, 0><<<grid, kThreads, 0, s>>>(c, v, t, a);
-    } else {
-        if (mip) render_global_kernel<VR_MODE_MIP, 1><<<grid, kThreads, 0, s>>>(c, v, t, a);
-        else render_global_kernel<VR_MODE_EA, 1><<<grid, kThreads, 0, s>>>(c, v, t, a);
-    }
+    if (a.variant == 2) VR_DISPATCH(render_global_sp_kernel, grid, c, v, t, a);
+    else VR_DISPATCH(render_global_kernel, grid, c, v, t, a);
     return cudaGetLastError();
 }
 
 cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a,
                                  const PartialDev* d_partials, int n, int total_tiles, cudaStream_t s) {
     if (n == 0 || total_tiles == 0) return cudaSuccess;
-    const bool mip = a.mode == VR_MODE_MIP;
-    if (a.variant == 2) {
-        if (mip) render_bricks_sp_kernel<VR_MODE_MIP><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-        else render_bricks_sp_kernel<VR_MODE_EA><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-    } else if (a.variant == 0) {
-        if (mip) render_bricks_kernel<VR_MODE_MIP, 0><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-        else render_bricks_kernel<VR_MODE_EA, 0><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-    } else {
-        if (mip) render_bricks_kernel<VR_MODE_MIP, 1><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-        else render_bricks_kernel<VR_MODE_EA, 1><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-    }
+    if (a.variant == 2) VR_DISPATCH(render_bricks_sp_kernel, total_tiles, c, v, t, a, d_partials, n);
+    else VR_DISPATCH(render_bricks_kernel, total_tiles, c, v, t, a, d_partials, n);
     return cudaGetLastError();
 }
 

@@ -29,8 +29,9 @@ def test_layout_and_status_strings_need_no_gpu():
     lib = vr.load()
     assert lib.vr_status_string(0) == b"VR_OK" and lib.vr_status_string(-4) == b"VR_ERR_STATE"
     cb, mb = vr.cube_layout((512, 512, 1024), (64, 64, 64))
-    # 1024 bricks of 68 x 65 x 65 floats (one-sided halo, x pitch padded to 4)
-    assert cb == 1024 * ((68 * 65 * 65 + 31) // 32 * 32) * 4
+    # 1024 bricks with a one-sided halo: rows layout 68 x 65 x 65 floats (x pitch padded to 4), blocks
+    # layout 17 x 17 x 33 micro-blocks of 32 floats; the caller's buffer must hold either (VR_OPT_LAYOUT)
+    assert cb == 1024 * max((68 * 65 * 65 + 31) // 32 * 32, 32 * 17 * 17 * 33) * 4
     assert mb > 1024 * 8
     # C5: 128 GiB cube with halos must fit the 180 GB of one B200 (hard part 4)
     cb5, mb5 = vr.cube_layout((4096, 4096, 2048), (256, 256, 256))
