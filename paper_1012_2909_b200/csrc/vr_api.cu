@@ -37,11 +37,16 @@ struct vr_ctx {
     float* d_stage = nullptr;
     size_t stage_bytes = 0;
     int64_t launches = 0;
-    int opt_skip = 1, opt_cell_skip = 0, opt_variant = 2, opt_layout = 1;
+    int opt_skip = 1, opt_cell_skip = -1, opt_variant = -1, opt_layout = 1;   // -1: chosen per view / TF
     float x_clear = -INFINITY;
+    double active_cell_fraction = 1.0;   // macro-cells active against the current table (EA)
+    unsigned long long* d_scratch = nullptr;
 };
 
 namespace {
+
+constexpr double kSparseRaySpacing = 2.0;     // voxels between neighbouring rays: variant 3 at or above
+constexpr double kCellSkipMaxActive = 0.75;   // macro-cell skipping only if fewer cells than this are active
 
 int fail(vr_ctx* ctx, int code, const std::string& msg) {
     if (ctx) ctx->err = msg;
@@ -158,8 +163,13 @@ int ensure_tables(vr_ctx* ctx, cudaStream_t s) {
         int nz[257];
         nz[0] = 0;
         for (int j = 0; j < 256; ++j) nz[j + 1] = nz[j] + (ctx->tf_baked[4 * j + 3] != 0.f ? 1 : 0);
-        VR_CUDA(ctx, launch_classify_cells(ctx->cube, nz, ctx->vmin, ctx->scale, s));
+        VR_CUDA(ctx, cudaMemsetAsync(ctx->d_scratch, 0, sizeof(unsigned long long), s));
+        VR_CUDA(ctx, launch_classify_cells(ctx->cube, nz, ctx->vmin, ctx->scale, ctx->d_scratch, s));
         ctx->launches += 1;
+        unsigned long long n_active = 0;
+        VR_CUDA(ctx, cudaMemcpyAsync(&n_active, ctx->d_scratch, sizeof(n_active), cudaMemcpyDeviceToHost, s));
+        VR_CUDA(ctx, cudaStreamSynchronize(s));
+        ctx->active_cell_fraction = (double)n_active / std::max(1.0, (double)ctx->cube.nbricks * ctx->cube.cells_per_brick);
         // samples with table coordinate x < x_clear interpolate two entries of zero opacity
         int i0 = -1;
         while (i0 + 1 < 256 && ctx->tf_baked[4 * (i0 + 1) + 3] == 0.f) ++i0;
@@ -169,7 +179,43 @@ int ensure_tables(vr_ctx* ctx, cudaStream_t s) {
     return VR_OK;
 }
 
-int skip_level(const vr_ctx* ctx) { return ctx->opt_skip ? (ctx->opt_cell_skip ? 2 : 1) : 0; }
+// Distance in voxels between the rays of neighbouring pixels where they pass the cube centre.
+double ray_spacing(const vr_ctx* ctx) {
+    const CubeDesc& c = ctx->cube;
+    const double* M = ctx->M; const double* Mi = ctx->Minv;
+    const double ctr[3] = {0.5 * (c.N[0] - 1), 0.5 * (c.N[1] - 1), 0.5 * (c.N[2] - 1)};
+    const double Z = M[8] * ctr[0] + M[9] * ctr[1] + M[10] * ctr[2] + M[11];
+    const double Wc = M[12] * ctr[0] + M[13] * ctr[1] + M[14] * ctr[2] + M[15];
+    const double zn = Wc > 1e-12 ? std::min(1.0, std::max(-1.0, Z / Wc)) : 0.0;
+    auto unproj = [&](double xn, double yn, double out[3]) {
+        double v[4];
+        for (int r = 0; r < 4; ++r) v[r] = Mi[4 * r] * xn + Mi[4 * r + 1] * yn + Mi[4 * r + 2] * zn + Mi[4 * r + 3];
+        for (int a = 0; a < 3; ++a) out[a] = v[a] / v[3];
+    };
+    double p0[3], p1[3], p2[3];
+    unproj(0.0, 0.0, p0); unproj(2.0 / ctx->view.W, 0.0, p1); unproj(0.0, 2.0 / ctx->view.H, p2);
+    double sx = 0, sy = 0;
+    for (int a = 0; a < 3; ++a) { sx += (p1[a] - p0[a]) * (p1[a] - p0[a]); sy += (p2[a] - p0[a]) * (p2[a] - p0[a]); }
+    const double s = std::sqrt(std::sqrt(sx) * std::sqrt(sy));
+    return std::isfinite(s) ? s : 1.0;
+}
+
+// Marcher variant.  Rays of neighbouring pixels less than about two voxels
+// apart share their cache lines inside a warp of 8 x 4 pixels: one ray per thread (variant 0).
+// Sparser rays share nothing: the lanes of a warp take consecutive samples of one ray (variant 3).
+int resolve_variant(const vr_ctx* ctx) {
+    if (ctx->opt_variant >= 0) return ctx->opt_variant;
+    return ray_spacing(ctx) >= kSparseRaySpacing ? 3 : 0;
+}
+
+// Skipping level: 0 none, 1 configured bricks, 2 bricks and 8^3 macro-cells.  The macro-cell level
+// costs a lookup per run / sample, so by default it is used only for emission-absorption and only
+// if the current table leaves a fair share of the cells idle.
+int skip_level(const vr_ctx* ctx, int mode) {
+    if (!ctx->opt_skip) return 0;
+    if (ctx->opt_cell_skip >= 0) return ctx->opt_cell_skip ? 2 : 1;
+    return (mode == VR_MODE_EA && ctx->active_cell_fraction < kCellSkipMaxActive) ? 2 : 1;
+}
 
 TFDesc tf_desc(const vr_ctx* ctx) {
     TFDesc t;
@@ -324,6 +370,7 @@ int vr_create(vr_ctx** out, int device) {
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_tf_raw, 256 * sizeof(float4));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, kNumCounters * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(ctx->d_counters, 0, kNumCounters * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_scratch, sizeof(unsigned long long));
     if (e != cudaSuccess) { vr_destroy(ctx); return VR_ERR_CUDA; }
     *out = ctx;
     return VR_OK;
@@ -335,6 +382,7 @@ int vr_destroy(vr_ctx* ctx) {
     if (ctx->d_tf_baked) cudaFree(ctx->d_tf_baked);
     if (ctx->d_tf_raw) cudaFree(ctx->d_tf_raw);
     if (ctx->d_counters) cudaFree(ctx->d_counters);
+    if (ctx->d_scratch) cudaFree(ctx->d_scratch);
     if (ctx->d_partials) cudaFree(ctx->d_partials);
     if (ctx->d_stage) cudaFree(ctx->d_stage);
     delete ctx;
@@ -508,7 +556,7 @@ int vr_render_mip(vr_ctx* ctx, float* d_out, float* d_out_rgba, float miss, void
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
-    a.mode = VR_MODE_MIP; a.tau = 2.f; a.miss = miss; a.skip = skip_level(ctx); a.variant = ctx->opt_variant;
+    a.mode = VR_MODE_MIP; a.tau = 2.f; a.miss = miss; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx);
     a.out = d_out; a.out_rgba = d_out_rgba; a.counters = ctx->d_counters;
     VR_CUDA(ctx, launch_render_global(ctx->cube, ctx->view, tf_desc(ctx), a, s));
     ctx->launches += 1;
@@ -523,7 +571,7 @@ int vr_render_ea(vr_ctx* ctx, float* d_out, const float bg[4], float tau, void* 
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
-    a.mode = VR_MODE_EA; a.tau = tau; a.skip = skip_level(ctx); a.variant = ctx->opt_variant;
+    a.mode = VR_MODE_EA; a.tau = tau; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx);
     for (int i = 0; i < 4; ++i) a.bg[i] = bg[i];
     a.out = d_out; a.counters = ctx->d_counters;
     VR_CUDA(ctx, launch_render_global(ctx->cube, ctx->view, tf_desc(ctx), a, s));
@@ -604,7 +652,7 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
     int tiles = 0;
     if ((rc = upload_partials(ctx, mode, hp, n, true, &tiles, s))) return rc;
     RenderArgs a{};
-    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx); a.variant = ctx->opt_variant;
+    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx);
     a.counters = ctx->d_counters;
     VR_CUDA(ctx, launch_render_bricks(ctx->cube, ctx->view, tf_desc(ctx), a, ctx->d_partials, n, tiles, s));
     ctx->launches += (n > 0 && tiles > 0) ? 1 : 0;
@@ -645,7 +693,7 @@ int vr_reset_counters(vr_ctx* ctx, void* stream) {
 int vr_set_option(vr_ctx* ctx, int option, int value) {
     if (!ctx) return VR_ERR_INVALID_ARG;
     if (option == VR_OPT_SKIP) { ctx->opt_skip = value ? 1 : 0; return VR_OK; }
-    if (option == VR_OPT_CELL_SKIP) { ctx->opt_cell_skip = value ? 1 : 0; return VR_OK; }
+    if (option == VR_OPT_CELL_SKIP) { ctx->opt_cell_skip = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_LAYOUT) {
         if (value != 0 && value != 1) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: layout must be 0 (rows) or 1 (4x4x2 blocks)");
         ctx->opt_layout = value; return VR_OK;                  // takes effect at the next upload / generate / attach
@@ -656,7 +704,7 @@ int vr_set_option(vr_ctx* ctx, int option, int value) {
         return VR_OK;
     }
     if (option == VR_OPT_VARIANT) {
-        if (value != 0 && value != 2) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");
+        if (value != -1 && value != 0 && value != 2 && value != 3) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");
         ctx->opt_variant = value; return VR_OK;
     }
     return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown option");

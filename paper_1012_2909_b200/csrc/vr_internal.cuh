@@ -90,7 +90,7 @@ cudaError_t launch_generate(const CubeDesc& c, float* d_cube, const GenDev& g, c
 struct RenderArgs {
     int mode; float tau; float bg[4]; float miss;
     int skip;              // 0: none; 1: configured bricks; 2: bricks and 8^3 macro-cells (O-10)
-    int variant;           // 0: 8 voxel loads per sample; 1: register cell cache
+    int variant;           // 0: one ray per thread; 2: one ray per warp; 3: lockstep, two phases
     float* out; float* out_rgba; unsigned long long* counters;
 };
 cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s);
@@ -98,7 +98,8 @@ cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFD
                                  const PartialDev* d_partials, int n, int total_tiles, cudaStream_t s);
 cudaError_t launch_composite(const ViewDesc& v, int mode, const PartialDev* d_partials, int n, float* out,
                              const float bg[4], cudaStream_t s);
-cudaError_t launch_classify_cells(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale, cudaStream_t s);
+cudaError_t launch_classify_cells(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale,
+                                  unsigned long long* d_active_count, cudaStream_t s);
 cudaError_t launch_upload_table(float4* d_dst, const float* h_src_1024, cudaStream_t s);
 
 }  // namespace vr

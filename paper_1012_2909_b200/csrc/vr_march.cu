@@ -619,12 +619,161 @@ render_global_sp_kernel(const __grid_constant__ CubeDesc c, const __grid_constan
     }
 }
 
+// ================================================================== variant 3: lockstep, two phases
+// A warp owns the 32 rays of its 8 x 4 pixel tile and walks them TOGETHER through chunks of 32
+// lattice indices [kbase, kbase + 31] (k counts from the near plane, so a chunk is a thin shell
+// that all 32 rays cross at about the same place: lines shared by neighbouring rays are fetched
+// once and hit in L1 / L2, not re-read from HBM).  Each chunk has two phases:
+//   phase 1, sample-parallel: for every ray of the warp in turn the 32 lanes take the 32 samples
+//     of that ray in the chunk (positions, gathers, trilinear, O-3 / O-4); the lanes' addresses
+//     follow the ray, and the gathers of the next ray are issued before the current ones are
+//     used.  Interpolated values go to shared memory, vals[ray][sample].
+//   phase 2, ray-parallel: lane r folds the 32 values of ITS ray front to back (O-5 / O-7), the
+//     accumulator never leaves the lane, so dense opaque transfer functions cost the same as
+//     sparse ones and ERT (O-7) is exact per ray.
+// Skipped samples (O-10) are stored as -inf and never folded.
+constexpr int kValPitch = 33;
+
+template <int MODE, int LAYOUT, bool GLOBAL>
+__global__ void __launch_bounds__(kThreads)
+render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
+                 const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
+                 const PartialDev* __restrict__ parts, int n_parts) {
+    __shared__ float4 tab[256];
+    __shared__ PartialDev part;
+    __shared__ float vals_all[kThreads / 32][32 * kValPitch];
+    __shared__ float4 rays_all[kThreads / 32][64];
+    int fx, fy;                                             // view pixel of this thread's ray
+    bool live;
+    if (GLOBAL) {
+        int tx, ty; tile_pixel(tx, ty);
+        fx = blockIdx.x * kTileW + tx; fy = blockIdx.y * kTileH + ty;
+        live = fx < V.W && fy < V.H;
+    } else {
+        int lx, ly;
+        live = locate_tile(parts, n_parts, part, lx, ly);
+        fx = lx; fy = ly;
+    }
+    if (MODE == VR_MODE_EA) load_tf(tab, T.baked);
+    Ray r; r.k0 = 0; r.k1 = -1;
+    r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
+    if (live) setup_ray(V, c, GLOBAL ? fx : part.x0 + fx, GLOBAL ? fy : part.y0 + fy, r);
+    int ka = r.k0, kb = r.k1;
+    int bid0 = 0, lo0[3] = {0, 0, 0};
+    if (!GLOBAL) {
+        bid0 = part.brick;
+        const int b[3] = {bid0 % c.G[0], (bid0 / c.G[0]) % c.G[1], bid0 / (c.G[0] * c.G[1])};
+        lo0[0] = b[0] * c.B[0]; lo0[1] = b[1] * c.B[1]; lo0[2] = b[2] * c.B[2];
+        brick_interval(c, r, b, lo0, ka, kb);
+    }
+    const BrickRef br0 = brick_ref<LAYOUT>(c, bid0, lo0);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float* vals = vals_all[warp];
+    float4* rays = rays_all[warp];
+    rays[2 * lane] = make_float4(r.o[0], r.o[1], r.o[2], r.d[0]);
+    rays[2 * lane + 1] = make_float4(r.d[1], r.d[2], __int_as_float(ka), __int_as_float(kb));
+    __syncwarp();
+    bool alive = ka <= kb, stopped = false;
+    int K0 = alive ? ka : 0x7fffffff, K1 = alive ? kb : -1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        K0 = min(K0, __shfl_xor_sync(0xffffffffu, K0, o));
+        K1 = max(K1, __shfl_xor_sync(0xffffffffu, K1, o));
+    }
+    Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
+    unsigned long long n_taken = 0, n_skip = 0;
+    const bool cells = A.skip >= 2;
+    for (int kbase = K0; kbase <= K1; kbase += 32) {
+        if (!__ballot_sync(0xffffffffu, alive)) break;
+        const unsigned act = __ballot_sync(0xffffffffu, alive && ka <= kbase + 31 && kb >= kbase);
+        if (!act) continue;
+        // ---- phase 1: lane = sample kbase + lane of ray rr
+        const int k = kbase + lane;
+        const float t = __fmul_rn((float)k, r.step);        // O-3: t_k = k * Delta
+        auto issue = [&](int rr, Lane8& L) {
+            const float4 ra = rays[2 * rr], rb = rays[2 * rr + 1];
+            float m_r = -INFINITY;
+            if (MODE == VR_MODE_MIP) m_r = __shfl_sync(0xffffffffu, acc.m, rr);
+            L.idle = true;
+#pragma unroll
+            for (int e = 0; e < 8; ++e) L.v[e] = 0.f;
+            L.w[0] = L.w[1] = L.w[2] = 0.f;
+            if (k >= __float_as_int(rb.z) && k <= __float_as_int(rb.w)) {
+                float p[3], fl[3];
+                p[0] = __fmaf_rn(t, ra.w, ra.x); p[1] = __fmaf_rn(t, rb.x, ra.y); p[2] = __fmaf_rn(t, rb.y, ra.z);
+                const int iv[3] = {floor_pos(p[0], fl[0]), floor_pos(p[1], fl[1]), floor_pos(p[2], fl[2])};
+                L.w[0] = __fsub_rn(p[0], fl[0]); L.w[1] = __fsub_rn(p[1], fl[1]); L.w[2] = __fsub_rn(p[2], fl[2]);
+                if (GLOBAL) {
+                    int b[3]; brick_of(c, iv, b);
+                    const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
+                    const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
+                    bool idle = false;
+                    if (A.skip) {                           // O-10 (exact), per sample
+                        if (MODE == VR_MODE_MIP) idle = __ldg(&c.brick_mm[bid]).y <= m_r;
+                        else idle = __ldg(&c.brick_active[bid]) == 0;
+                        if (cells && !idle) idle = cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], m_r);
+                    }
+                    L.idle = idle;
+                    if (!idle) { const BrickRef br = brick_ref<LAYOUT>(c, bid, lo); gather8<LAYOUT>(br, iv[0], iv[1], iv[2], L.v); }
+                } else {
+                    L.idle = cells && cell_idle<MODE>(c, bid0, lo0, iv[0], iv[1], iv[2], m_r);
+                    if (!L.idle) gather8<LAYOUT>(br0, iv[0], iv[1], iv[2], L.v);
+                }
+            }
+        };
+        Lane8 cur, nxt;
+        unsigned rest = act;
+        int rc = __ffs(rest) - 1;
+        rest &= rest - 1;
+        issue(rc, cur);
+        for (;;) {
+            int rn = -1;
+            if (rest) { rn = __ffs(rest) - 1; rest &= rest - 1; issue(rn, nxt); }
+            const float val = trilinear(cur.v, cur.w[0], cur.w[1], cur.w[2]);
+            vals[rc * kValPitch + lane] = cur.idle ? -INFINITY : val;
+            if (rn < 0) break;
+            cur = nxt; rc = rn;
+        }
+        __syncwarp();
+        // ---- phase 2: lane = ray
+        if ((act >> lane) & 1u) {
+            const int l0 = max(ka, kbase) - kbase, l1 = min(kb, kbase + 31) - kbase;
+            const float* mine = vals + lane * kValPitch;
+            for (int l = l0; l <= l1; ++l) {
+                const float v = mine[l];
+                if (v == -INFINITY) { ++n_skip; continue; }
+                ++n_taken;
+                if (fold<MODE>(acc, v, tab, T, A.tau)) { stopped = true; alive = false; break; }
+            }
+        }
+        __syncwarp();
+    }
+    if (live) {
+        if (GLOBAL) write_frame_pixel<MODE>(V, T, A, fx, fy, acc, r.k1 >= r.k0);
+        else {
+            const long long px = (long long)fy * part.pitch + fx;
+            if (MODE == VR_MODE_MIP) reinterpret_cast<float*>(part.data)[px] = acc.m;
+            else reinterpret_cast<float4*>(part.data)[px] = make_float4(acc.C[0], acc.C[1], acc.C[2], acc.A);
+        }
+    }
+    if (A.counters) {
+        const unsigned long long nom = kb >= ka ? (unsigned long long)(kb - ka + 1) : 0ULL;
+        if (GLOBAL) count(A.counters, kRays, nom ? 1 : 0);
+        count(A.counters, kNominal, nom);
+        count(A.counters, kTaken, n_taken);
+        count(A.counters, kVisited, nom ? 1 : 0);
+        count(A.counters, kSkipped, n_skip);
+        count(A.counters, kTerminated, stopped ? 1 : 0);
+    }
+}
+
 // O-10 per transfer function: one bit per 8^3 macro-cell, set iff a table entry that the cell's
 // value range [min, max] (halo-inclusive) can touch has non-zero opacity.  `nz` is the running
 // count of entries with non-zero baked opacity, so the range test is one subtraction.
 struct NzPrefix { int v[257]; };
 __global__ void classify_cells_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ NzPrefix nz,
-                                      float vmin, float scale, long long n_slots) {
+                                      float vmin, float scale, long long n_slots,
+                                      unsigned long long* __restrict__ active_count) {
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n_slots;
          e += (long long)gridDim.x * blockDim.x) {
         const long long word = e >> 5;
@@ -641,7 +790,10 @@ __global__ void classify_cells_kernel(const __grid_constant__ CubeDesc c, const 
             }
         }
         const unsigned bits = __ballot_sync(0xffffffffu, active);
-        if ((e & 31) == 0) c.cell_bits[word] = bits;
+        if ((e & 31) == 0) {
+            c.cell_bits[word] = bits;
+            if (bits) atomicAdd(active_count, (unsigned long long)__popc(bits));
+        }
     }
 }
 
@@ -663,9 +815,21 @@ __global__ void upload_half_kernel(float4* dst, const __grid_constant__ HalfTabl
         }                                                                                                \
     } while (0)
 
+#define VR_DISPATCH_LS(GLOBAL, GRID, ...)                                                                \
+    do {                                                                                                 \
+        if (a.mode == VR_MODE_MIP) {                                                                     \
+            if (c.layout == 0) render_ls_kernel<VR_MODE_MIP, 0, GLOBAL><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
+            else render_ls_kernel<VR_MODE_MIP, 1, GLOBAL><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);         \
+        } else {                                                                                         \
+            if (c.layout == 0) render_ls_kernel<VR_MODE_EA, 0, GLOBAL><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
+            else render_ls_kernel<VR_MODE_EA, 1, GLOBAL><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);          \
+        }                                                                                                \
+    } while (0)
+
 cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s) {
     dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
-    if (a.variant == 2) VR_DISPATCH(render_global_sp_kernel, grid, c, v, t, a);
+    if (a.variant == 3) VR_DISPATCH_LS(true, grid, c, v, t, a, nullptr, 0);
+    else if (a.variant == 2) VR_DISPATCH(render_global_sp_kernel, grid, c, v, t, a);
     else VR_DISPATCH(render_global_kernel, grid, c, v, t, a);
     return cudaGetLastError();
 }
@@ -673,18 +837,20 @@ cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFD
 cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a,
                                  const PartialDev* d_partials, int n, int total_tiles, cudaStream_t s) {
     if (n == 0 || total_tiles == 0) return cudaSuccess;
-    if (a.variant == 2) VR_DISPATCH(render_bricks_sp_kernel, total_tiles, c, v, t, a, d_partials, n);
+    if (a.variant == 3) VR_DISPATCH_LS(false, total_tiles, c, v, t, a, d_partials, n);
+    else if (a.variant == 2) VR_DISPATCH(render_bricks_sp_kernel, total_tiles, c, v, t, a, d_partials, n);
     else VR_DISPATCH(render_bricks_kernel, total_tiles, c, v, t, a, d_partials, n);
     return cudaGetLastError();
 }
 
-cudaError_t launch_classify_cells(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale, cudaStream_t s) {
+cudaError_t launch_classify_cells(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale,
+                                  unsigned long long* d_active_count, cudaStream_t s) {
     NzPrefix nz;
     for (int i = 0; i < 257; ++i) nz.v[i] = nz_prefix[i];
     const long long n_slots = (long long)c.nbricks * c.cell_words_per_brick * 32;
     long long blocks = (n_slots + 255) / 256;
     if (blocks > 148LL * 32) blocks = 148LL * 32;
-    classify_cells_kernel<<<(int)blocks, 256, 0, s>>>(c, nz, vmin, scale, n_slots);
+    classify_cells_kernel<<<(int)blocks, 256, 0, s>>>(c, nz, vmin, scale, n_slots, d_active_count);
     return cudaGetLastError();
 }
 

@@ -8,6 +8,10 @@ import numpy as np
 
 TOL_MAX, TOL_RMS = 1e-4, 1e-5
 
+# Options every Scene applies to its context (set by the `marcher` fixture of the GPU tests so that
+# each marcher variant / skipping level is checked, not only the one the library would pick).
+FORCED_OPTIONS = {}
+
 
 def torch_cuda():
     import torch
@@ -28,6 +32,8 @@ class Scene:
         self.d_cube = torch.empty(cb // 4, dtype=torch.float32, device="cuda")
         self.d_meta = torch.empty(mb, dtype=torch.uint8, device="cuda")
         self.ctx = vr.Context(0)
+        for opt, value in FORCED_OPTIONS.items():
+            self.ctx.set_option(opt, value)
         if cube is not None:
             self.ctx.upload_cube(np.ascontiguousarray(cube, dtype=np.float32), dims, brick, self.d_cube, self.d_meta)
         else:

@@ -24,6 +24,19 @@ def H():
     return helpers
 
 
+# Every test below runs once with the library's own choice of marcher variant and macro-cell
+# skipping ("auto") and once per forced variant (0: ray per thread, 2: ray per warp, 3: lockstep),
+# with the macro-cell level of the skipping forced on.
+@pytest.fixture(autouse=True, params=["auto", "v0", "v2", "v3"])
+def marcher(request, H):
+    from paper_1012_2909_b200 import vr
+    H.FORCED_OPTIONS.clear()
+    if request.param != "auto":
+        H.FORCED_OPTIONS.update({vr.OPT_VARIANT: int(request.param[1:]), vr.OPT_CELL_SKIP: 1})
+    yield request.param
+    H.FORCED_OPTIONS.clear()
+
+
 def noise_cube(shape, seed=0, scale=1.0):
     return (np.random.default_rng(seed).normal(size=shape) * scale).astype(np.float32)
 
@@ -360,11 +373,15 @@ def _fullsize_check(H, w, block, n_random, frame_index):
     torch.cuda.empty_cache()
 
 
-def test_config_c2_full_size(H):
+def test_config_c2_full_size(H, marcher):
+    if marcher not in ("auto", "v0"):
+        pytest.skip("full sizes run with the library's choice (what bench.py times) and variant 0")
     _fullsize_check(H, wl.C2, block=16, n_random=200, frame_index=0)
 
 
-def test_config_c3_full_size_64gib(H):
+def test_config_c3_full_size_64gib(H, marcher):
+    if marcher not in ("auto", "v0"):
+        pytest.skip("full sizes run with the library's choice (what bench.py times) and variant 0")
     import torch
     free, total = torch.cuda.mem_get_info()
     if free < 80e9:
