@@ -387,3 +387,102 @@ def test_config_c3_full_size_64gib(H, marcher):
     if free < 80e9:
         pytest.skip("needs ~70 GB of free HBM")
     _fullsize_check(H, wl.C3, block=12, n_random=0, frame_index=37)
+
+
+def _tiled_fullsize_check(H, w, panels, block, mip_frame=None):
+    """Parity at the full size of a tiled-display config (BASELINE.json configs[3], configs[4];
+    PAPER.md line 37: 5 x 5 panels of 1920 x 1080), in the launch configuration bench.py times:
+    every panel is an off-axis frustum of the one camera, rendered sort-last into one pitched
+    frame.  Pixel blocks of the listed panels are compared with the oracle run with the panel's
+    matrix, the cube bytes fetched back brick by brick.  Optionally a whole-cube MIP at `mip_frame` (configs[4])."""
+    import torch
+    from oracle import ovr
+    sc = H.Scene(w.dims, w.brick, gen={"seed": w.seed, "sources": wl.make_sources(w),
+                                       "zero_boxes": wl.make_zero_boxes(w), "continuum": w.continuum})
+    vr = sc.vr
+    W, Hh = w.frame
+    cols, rows = w.panels
+    pw, ph = W // cols, Hh // rows
+    M = wl.config_camera(w, 0)
+    tf = wl.TFS[w.tf]()
+    sc.ctx.set_transfer_function(*tf)
+    frame = torch.full((Hh, W, 4), -7.0, dtype=torch.float32, device="cuda")
+    arena = None
+    n_bricks = 0
+    for r in range(rows):
+        for c in range(cols):
+            sc.ctx.set_view(wl.panel_matrix(M, cols, rows, c, r), pw, ph, w.step)
+            sc.ctx.set_viewport(c * pw, r * ph, W)
+            ids = sc.ctx.sort_bricks(vr.MODE_EA)
+            parts, n, nbytes = sc.ctx.partial_layout(vr.MODE_EA, ids)
+            if arena is None or arena.numel() < nbytes:
+                arena = torch.empty(int(nbytes * 1.3) + 256, dtype=torch.uint8, device="cuda")
+            vr.Context.bind_partials(parts, n, arena)
+            sc.ctx.render_bricks(vr.MODE_EA, parts, n, w.tau)
+            sc.ctx.composite_bricks(vr.MODE_EA, parts, n, frame, BG)
+            n_bricks += n
+    torch.cuda.synchronize()
+    assert n_bricks > 0
+    brick = tuple(min(b, n) for b, n in zip(w.brick, w.dims))
+    cache = {}
+    for (c, r) in panels:
+        # the block in the panel's lower right corner (next to the seams), cast by the oracle with
+        # the panel's own off-axis matrix: same rays, so the float32 oracle must match to the bit
+        Mp = wl.panel_matrix(M, cols, rows, c, r)
+        xs, ys = np.arange(pw - block, pw), np.arange(ph - block, ph)
+        pix = np.stack(np.meshgrid(xs, ys), axis=-1).reshape(-1, 2).astype(np.int32)
+        touched = ovr.bricks_touched(Mp, pw, ph, w.step, w.dims, brick, pix)
+        for b in touched:
+            if int(b) not in cache:
+                cache[int(b)] = sc.download_brick(int(b))
+        vol = ovr.Volume(w.dims, brick, {int(b): cache[int(b)] for b in touched})
+        kw = dict(tf=tf, bg=BG, tau=w.tau, pixels=pix, split=ovr.SPLIT_SORTLAST, partition=brick)
+        o64, fl, _ = ovr.render(vol, Mp, pw, ph, w.step, ovr.EA, ovr.F64, **kw)
+        o32, _, _ = ovr.render(vol, Mp, pw, ph, w.step, ovr.EA, ovr.F32, **kw)
+        got = frame[r * ph + ys[0]:r * ph + ys[-1] + 1, c * pw + xs[0]:c * pw + xs[-1] + 1].cpu().numpy().reshape(-1, 4)
+        H.compare(got, o64, fl, o32, what=f"{w.name} full-size tiled EA, panel {(c, r)}")
+        assert np.array_equal(got, o32)
+    # whole-frame properties: every pixel written, alpha in [0, 1], rows continuous across panel seams
+    lo, hi = torch.aminmax(frame[..., 3])
+    assert float(lo) >= min(0.0, BG[3]) and float(hi) <= 1.0 + 1e-6
+    assert not bool((frame == -7.0).any())
+    for r in range(1, rows):
+        seam = (frame[r * ph] - frame[r * ph - 1]).abs().mean()
+        inner = (frame[r * ph + 1] - frame[r * ph]).abs().mean()
+        assert float(seam) < 4.0 * float(inner) + 1e-3
+    if mip_frame is not None:
+        mw, mh = mip_frame
+        Mm = wl.config_camera(w, 0, frame=mip_frame)
+        mip = sc.render_mip(Mm, mw, mh, w.step, miss=0.0)
+        mip_sl, _, _ = sc.render_sortlast(Mm, mw, mh, w.step, vr.MODE_MIP, bg=(0.0, 0, 0, 0))
+        assert np.array_equal(mip_sl, mip)                      # split == unsplit, bit-exact (O-5)
+        xs, ys = np.arange(mw // 2 - 12, mw // 2 + 12), np.arange(mh // 2 - 12, mh // 2 + 12)
+        pix = np.stack(np.meshgrid(xs, ys), axis=-1).reshape(-1, 2).astype(np.int32)
+        touched = ovr.bricks_touched(Mm, mw, mh, w.step, w.dims, brick, pix)
+        for b in touched:
+            if int(b) not in cache:
+                cache[int(b)] = sc.download_brick(int(b))
+        vol = ovr.Volume(w.dims, brick, {int(b): cache[int(b)] for b in touched})
+        m64, flm, _ = ovr.render(vol, Mm, mw, mh, w.step, ovr.MIP, ovr.F64, miss=0.0, pixels=pix)
+        m32, _, _ = ovr.render(vol, Mm, mw, mh, w.step, ovr.MIP, ovr.F32, miss=0.0, pixels=pix)
+        gm = mip[pix[:, 1], pix[:, 0]]
+        H.compare(gm, m64, flm, m32, mode_mip=True, vmin=tf[1], vmax=tf[2], miss=0.0, what=f"{w.name} full-size MIP")
+        assert np.array_equal(gm, m32)
+    del sc, frame, arena
+    torch.cuda.empty_cache()
+
+
+def test_config_c4_full_size_tiled_9600x5400(H, marcher):
+    if marcher != "auto":
+        pytest.skip("full sizes run with the library's choice (what bench.py times)")
+    _tiled_fullsize_check(H, wl.C4, panels=[(2, 2), (0, 1), (4, 3)], block=8)
+
+
+def test_config_c5_full_size_128gib(H, marcher):
+    if marcher != "auto":
+        pytest.skip("full sizes run with the library's choice (what bench.py times)")
+    import torch
+    free, total = torch.cuda.mem_get_info()
+    if free < 150e9:
+        pytest.skip("needs ~142 GB of free HBM")
+    _tiled_fullsize_check(H, wl.C5, panels=[(2, 2), (1, 3)], block=6, mip_frame=(1920, 1080))
