@@ -150,13 +150,18 @@ int vr_get_counters(vr_ctx* ctx, vr_counters* out, void* stream);
 int vr_reset_counters(vr_ctx* ctx, void* stream);
 /* Options.  None of them changes a frame (tests assert it); they exist for A/B measurements.
  *  VR_OPT_SKIP (default 1): min/max empty-space skipping (O-10) on/off, all levels.
- *  VR_OPT_VARIANT (default 2): 0 = one ray per thread, the 32 lanes of a warp take 8 x 4 pixels;
- *    2 = one ray per warp, the 32 lanes take 32 consecutive samples of it.
- *  VR_OPT_CELL_SKIP (default 0): the 8^3 macro-cell level of the skipping under the configured
- *    bricks on/off (needs VR_OPT_SKIP).
+ *  VR_OPT_VARIANT (default -1): the marcher.  0 = one ray per thread, the 32 lanes of a warp take
+ *    8 x 4 pixels; 3 = lockstep: a warp walks its 32 rays together through chunks of 32 lattice
+ *    indices, the lanes taking the 32 samples of one ray at a time, then each lane folds its own
+ *    ray; -1 = chosen per view from the spacing of neighbouring rays
+ *    (>= 2 voxels: 3, else 0).
+ *  VR_OPT_CELL_SKIP (default -1): the 8^3 macro-cell level of the skipping under the configured
+ *    bricks, 1 on / 0 off (needs VR_OPT_SKIP); -1 = on for emission-absorption if fewer than 3/4
+ *    of the cells are active against the current table, on for MIP in variant 3.
  *  VR_OPT_LAYOUT (default 1): voxel order inside a brick, 0 = rows (x fastest), 1 = 4 x 4 x 2
  *    micro-blocks of one 128-byte line each; read by the next upload / generate / attach call.
- *  VR_OPT_L2_FETCH: cudaLimitMaxL2FetchGranularity of the device (32, 64 or 128 bytes). */
+ *  VR_OPT_L2_FETCH: cudaLimitMaxL2FetchGranularity of the device (32, 64 or 128 bytes; measured
+ *    to have no effect on B200, where HBM is read in whole 128-byte lines). */
 enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETCH = 4, VR_OPT_LAYOUT = 5 };
 int vr_set_option(vr_ctx* ctx, int option, int value);
 

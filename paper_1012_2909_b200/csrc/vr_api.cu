@@ -209,12 +209,13 @@ int resolve_variant(const vr_ctx* ctx) {
 }
 
 // Skipping level: 0 none, 1 configured bricks, 2 bricks and 8^3 macro-cells.  The macro-cell level
-// costs a lookup per run / sample, so by default it is used only for emission-absorption and only
-// if the current table leaves a fair share of the cells idle.
+// costs a lookup per run / sample, so by default emission-absorption uses it only if the current
+// table leaves a fair share of the cells idle, and MIP only in the lockstep marcher (measured).
 int skip_level(const vr_ctx* ctx, int mode) {
     if (!ctx->opt_skip) return 0;
     if (ctx->opt_cell_skip >= 0) return ctx->opt_cell_skip ? 2 : 1;
-    return (mode == VR_MODE_EA && ctx->active_cell_fraction < kCellSkipMaxActive) ? 2 : 1;
+    if (mode == VR_MODE_MIP) return resolve_variant(ctx) == 3 ? 2 : 1;
+    return ctx->active_cell_fraction < kCellSkipMaxActive ? 2 : 1;
 }
 
 TFDesc tf_desc(const vr_ctx* ctx) {
@@ -704,7 +705,7 @@ int vr_set_option(vr_ctx* ctx, int option, int value) {
         return VR_OK;
     }
     if (option == VR_OPT_VARIANT) {
-        if (value != -1 && value != 0 && value != 2 && value != 3) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");
+        if (value != -1 && value != 0 && value != 3) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");
         ctx->opt_variant = value; return VR_OK;
     }
     return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown option");

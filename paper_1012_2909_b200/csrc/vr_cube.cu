@@ -23,7 +23,7 @@ __device__ __forceinline__ Elem decode(const CubeDesc& c, long long brick, long 
         long long blk = rem >> 5;
         const int tx = (int)(blk % c.T[0]); blk /= c.T[0];
         const int ty = (int)(blk % c.T[1]), tz = (int)(blk / c.T[1]);
-        e.l[0] = 4 * tx + (w & 3); e.l[1] = 4 * ty + ((w >> 2) & 3); e.l[2] = 2 * tz + (w >> 4);
+        e.l[0] = 4 * tx + (w & 3); e.l[1] = 4 * ty + 2 * (w >> 4) + ((w >> 2) & 1); e.l[2] = 2 * tz + ((w >> 3) & 1);
         e.stored = tz < c.T[2];                       // padding slots are stored too (as zeros)
     }
     e.in_cube = e.stored;

@@ -18,9 +18,12 @@ constexpr int kTileW = 16, kTileH = 8, kThreads = 128;   // pixel tile of one CT
 // Halo voxels beyond the cube and padding slots are zero.  Two layouts inside a brick:
 //  layout 0 (rows):   offset = lx + P0 (ly + P1 lz), P0 = roundup4(B0 + 1);
 //  layout 1 (blocks): 4 x 4 x 2 micro-blocks of 32 voxels = one 128-byte line each,
-//                     offset = 32 ((lx>>2) + T0 ((ly>>2) + T1 (lz>>1))) + 16 (lz&1) + 4 (ly&3) + (lx&3),
-//                     so that a ray's 2 x 2 x 2 footprints meet about the same number of lines
-//                     whatever its direction.
+//                     offset = 32 ((lx>>2) + T0 ((ly>>2) + T1 (lz>>1)))
+//                              + 16 ((ly>>1)&1) + 8 (lz&1) + 4 (ly&1) + (lx&3),
+//                     i.e. a 32-byte sector is 4 x 2 x 1 voxels and each 64-byte half line (the
+//                     unit HBM is read in) is 4 x 2 x 2, so that a ray's 2 x 2 x 2 footprints
+//                     meet about the same, small number of lines and half lines whatever its
+//                     direction.
 struct CubeDesc {
     int N[3];        // voxels
     int B[3];        // configured brick size
@@ -68,7 +71,7 @@ enum Counter { kRays = 0, kNominal, kTaken, kVisited, kSkipped, kTerminated, kNu
 __host__ __device__ inline long long voxel_slot(const CubeDesc& c, int lx, int ly, int lz) {
     if (c.layout == 0) return lx + (long long)c.P[0] * (ly + (long long)c.P[1] * lz);
     return 32LL * ((lx >> 2) + (long long)c.T[0] * ((ly >> 2) + (long long)c.T[1] * (lz >> 1))) +
-           16 * (lz & 1) + 4 * (ly & 3) + (lx & 3);
+           16 * ((ly >> 1) & 1) + 8 * (lz & 1) + 4 * (ly & 1) + (lx & 3);
 }
 
 size_t align_up(size_t v, size_t a);
@@ -90,7 +93,7 @@ cudaError_t launch_generate(const CubeDesc& c, float* d_cube, const GenDev& g, c
 struct RenderArgs {
     int mode; float tau; float bg[4]; float miss;
     int skip;              // 0: none; 1: configured bricks; 2: bricks and 8^3 macro-cells (O-10)
-    int variant;           // 0: one ray per thread; 2: one ray per warp; 3: lockstep, two phases
+    int variant;           // 0: one ray per thread; 3: lockstep, two phases (ray per warp)
     float* out; float* out_rgba; unsigned long long* counters;
 };
 cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s);

@@ -123,10 +123,10 @@ __device__ __forceinline__ void gather8(const BrickRef& b, int ix, int iy, int i
         q = lx + b.s0 * ly + b.s1 * lz;
         dx = 1u; dy = b.s0; dz = b.s1;
     } else {                              // step to the +1 neighbour: inside the micro-block or into the next one
-        q = ((lx >> 2) << 5) + (lx & 3u) + (ly >> 2) * b.s0 + ((ly & 3u) << 2) + (lz >> 1) * b.s1 + ((lz & 1u) << 4);
+        q = ((lx >> 2) << 5) + (lx & 3u) + (ly >> 2) * b.s0 + ((ly & 2u) << 3) + ((ly & 1u) << 2) + (lz >> 1) * b.s1 + ((lz & 1u) << 3);
         dx = (lx & 3u) == 3u ? 29u : 1u;
-        dy = (ly & 3u) == 3u ? b.s0 - 12u : 4u;
-        dz = (lz & 1u) ? b.s1 - 16u : 16u;
+        dy = (ly & 1u) == 0u ? 4u : ((ly & 2u) == 0u ? 12u : b.s0 - 20u);
+        dz = (lz & 1u) ? b.s1 - 8u : 8u;
     }
     const float* p = b.base + q;
     v[0] = __ldg(p);           v[1] = __ldg(p + dx);
@@ -415,209 +415,7 @@ render_bricks_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
     }
 }
 
-// ================================================================== variant 2: one ray per warp
-// ("sample-parallel").  The 128 threads of a CTA first set up the 128
-// rays of their pixel tile exactly as above (one ray per thread).  Then every warp walks through
-// its own 32 rays one after the other, and the 32 lanes take 32 CONSECUTIVE lattice samples
-// k .. k+31 of that one ray: positions, voxel gathers and trilinear interpolation run in parallel,
-// and the lanes' addresses follow the ray, so the lines the ray needs are fetched once and used at
-// once - nothing has to survive in L1/L2 between iterations, whatever the view direction.  The
-// gathers of the next 32 samples are issued before the current ones are folded.  The
-// front-to-back fold stays sequential in k (O-7): opaque samples are picked out with a ballot
-// and folded in ascending order through shuffles, all lanes keeping the same accumulator;
-// transparent samples (x < x_clear) contribute exact zeros and are not folded.  MIP folds with a
-// warp maximum (exact in any order).
 struct Lane8 { float v[8]; float w[3]; bool idle; };
-
-// Fold the 32 values `val` (lane = sample, `act` = the lane holds a taken, non-skipped sample) of
-// one ray into acc (identical in all lanes).  Returns the number of samples consumed if ERT
-// fired (>= 1), else 0.
-template <int MODE>
-__device__ __forceinline__ int fold32(Accum& acc, float val, bool act, const float4* tab, const TFDesc& T, float tau) {
-    if (MODE == VR_MODE_MIP) {
-        float m = act ? val : -INFINITY;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-        acc.m = fmaxf(acc.m, m);
-        return 0;
-    }
-    const float x = __fmul_rn(__fsub_rn(val, T.vmin), T.scale);
-    const bool opaque = act && !(x < T.x_clear);
-    unsigned bits = __ballot_sync(0xffffffffu, opaque);
-    if (!bits) return 0;
-    float4 col = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (opaque) col = tf_at(tab, x);                        // O-6, one sample per lane
-    while (bits) {                                          // O-7, ascending k
-        const int j = __ffs(bits) - 1;
-        bits &= bits - 1;
-        const float cr = __shfl_sync(0xffffffffu, col.x, j), cg = __shfl_sync(0xffffffffu, col.y, j);
-        const float cb = __shfl_sync(0xffffffffu, col.z, j), ca = __shfl_sync(0xffffffffu, col.w, j);
-        if (over(acc, cr, cg, cb, ca, tau)) return j + 1;
-    }
-    return 0;
-}
-
-template <int MODE, int LAYOUT>
-__global__ void __launch_bounds__(kThreads)
-render_bricks_sp_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
-                        const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
-                        const PartialDev* __restrict__ parts, int n_parts) {
-    __shared__ float4 tab[256];
-    __shared__ PartialDev part;
-    int lx, ly;
-    const bool live = locate_tile(parts, n_parts, part, lx, ly);
-    if (MODE == VR_MODE_EA) load_tf(tab, T.baked);
-    Ray r; r.k0 = 0; r.k1 = -1;
-    r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
-    if (live) setup_ray(V, c, part.x0 + lx, part.y0 + ly, r);
-    const int bid = part.brick;
-    const int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
-    const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
-    int ka = r.k0, kb = r.k1;
-    brick_interval(c, r, b, lo, ka, kb);
-    const BrickRef br = brick_ref<LAYOUT>(c, bid, lo);
-    const int lane = threadIdx.x & 31;
-    const bool cells = A.skip >= 2;
-    Accum mine = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-    unsigned long long n_taken = 0, n_term = 0, n_visit = 0, n_skip = 0;
-    for (unsigned rays = __ballot_sync(0xffffffffu, ka <= kb); rays; rays &= rays - 1) {
-        const int src = __ffs(rays) - 1;
-        Ray q;
-        q.step = r.step;
-#pragma unroll
-        for (int a = 0; a < 3; ++a) { q.o[a] = __shfl_sync(0xffffffffu, r.o[a], src); q.d[a] = __shfl_sync(0xffffffffu, r.d[a], src); }
-        const int qa = __shfl_sync(0xffffffffu, ka, src), qb = __shfl_sync(0xffffffffu, kb, src);
-        Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-        // issue the gathers of samples k0 + lane (idle lanes repeat the ray's last sample)
-        auto issue = [&](int k0, Lane8& L) {
-            float p[3], fx, fy, fz;
-            position(q, (float)min(k0 + lane, qb), p);
-            const int ix = floor_pos(p[0], fx), iy = floor_pos(p[1], fy), iz = floor_pos(p[2], fz);
-            L.w[0] = __fsub_rn(p[0], fx); L.w[1] = __fsub_rn(p[1], fy); L.w[2] = __fsub_rn(p[2], fz);
-            L.idle = cells && cell_idle<MODE>(c, bid, lo, ix, iy, iz, acc.m);
-            if (!L.idle) gather8<LAYOUT>(br, ix, iy, iz, L.v);
-            else {
-#pragma unroll
-                for (int e = 0; e < 8; ++e) L.v[e] = 0.f;
-            }
-        };
-        Lane8 cur, nxt;
-        issue(qa, cur);
-        bool stopped = false;
-        for (int k0 = qa; k0 <= qb; k0 += 32) {
-            const bool more = k0 + 32 <= qb;
-            if (more) issue(k0 + 32, nxt);
-            const bool act = k0 + lane <= qb && !cur.idle;
-            const float val = trilinear(cur.v, cur.w[0], cur.w[1], cur.w[2]);
-            const int n_in = min(qb - k0, 31) + 1;
-            const int hit = fold32<MODE>(acc, val, act, tab, T, A.tau);
-            const unsigned idle_bits = __ballot_sync(0xffffffffu, cur.idle && k0 + lane <= qb);
-            if (lane == 0) {
-                const unsigned upto = hit ? (hit >= 32 ? 0xffffffffu : ((1u << hit) - 1u)) : 0xffffffffu;
-                const int idle_n = __popc(idle_bits & upto);
-                n_taken += (unsigned long long)((hit ? hit : n_in) - idle_n);
-                n_skip += (unsigned long long)idle_n;
-            }
-            if (hit) { stopped = true; break; }
-            cur = nxt;
-        }
-        if (lane == 0) { ++n_visit; n_term += stopped ? 1 : 0; }
-        if (lane == src) mine = acc;
-    }
-    if (live) {
-        const long long px = (long long)ly * part.pitch + lx;
-        if (MODE == VR_MODE_MIP) reinterpret_cast<float*>(part.data)[px] = mine.m;
-        else reinterpret_cast<float4*>(part.data)[px] = make_float4(mine.C[0], mine.C[1], mine.C[2], mine.A);
-    }
-    if (A.counters) {
-        count(A.counters, kNominal, kb >= ka ? (unsigned long long)(kb - ka + 1) : 0ULL);
-        count(A.counters, kTaken, n_taken);
-        count(A.counters, kVisited, n_visit);
-        count(A.counters, kSkipped, n_skip);
-        count(A.counters, kTerminated, n_term);
-    }
-}
-
-// Whole frame, O-8 GLOBAL, one ray per warp: the lanes' 32 consecutive samples may lie in
-// different bricks, so every lane finds its own brick (O-3 membership from its own position); the
-// accumulator is carried along the ray, so ERT and the sample order are those of the unsplit march.
-template <int MODE, int LAYOUT>
-__global__ void __launch_bounds__(kThreads)
-render_global_sp_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
-                        const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A) {
-    __shared__ float4 tab[256];
-    if (MODE == VR_MODE_EA) load_tf(tab, T.baked);
-    int tx, ty; tile_pixel(tx, ty);
-    const int i = blockIdx.x * kTileW + tx, j = blockIdx.y * kTileH + ty;
-    const bool live = i < V.W && j < V.H;
-    Ray r; r.k0 = 0; r.k1 = -1;
-    r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
-    if (live) setup_ray(V, c, i, j, r);
-    const int lane = threadIdx.x & 31;
-    Accum mine = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-    unsigned long long n_taken = 0, n_term = 0, n_visit = 0, n_skip = 0;
-    for (unsigned rays = __ballot_sync(0xffffffffu, r.k0 <= r.k1); rays; rays &= rays - 1) {
-        const int src = __ffs(rays) - 1;
-        Ray q;
-        q.step = r.step;
-#pragma unroll
-        for (int a = 0; a < 3; ++a) { q.o[a] = __shfl_sync(0xffffffffu, r.o[a], src); q.d[a] = __shfl_sync(0xffffffffu, r.d[a], src); }
-        const int qa = __shfl_sync(0xffffffffu, r.k0, src), qb = __shfl_sync(0xffffffffu, r.k1, src);
-        Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-        auto issue = [&](int k0, Lane8& L) {
-            float p[3], fx, fy, fz;
-            position(q, (float)min(k0 + lane, qb), p);
-            const int iv[3] = {floor_pos(p[0], fx), floor_pos(p[1], fy), floor_pos(p[2], fz)};
-            L.w[0] = __fsub_rn(p[0], fx); L.w[1] = __fsub_rn(p[1], fy); L.w[2] = __fsub_rn(p[2], fz);
-            int b[3]; brick_of(c, iv, b);
-            const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
-            const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
-            L.idle = false;
-            if (A.skip) {                                   // O-10 (exact), per sample
-                if (MODE == VR_MODE_MIP) L.idle = __ldg(&c.brick_mm[bid]).y <= acc.m;
-                else L.idle = __ldg(&c.brick_active[bid]) == 0;
-                if (A.skip >= 2 && !L.idle) L.idle = cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], acc.m);
-            }
-            if (!L.idle) { const BrickRef br = brick_ref<LAYOUT>(c, bid, lo); gather8<LAYOUT>(br, iv[0], iv[1], iv[2], L.v); }
-            else {
-#pragma unroll
-                for (int e = 0; e < 8; ++e) L.v[e] = 0.f;
-            }
-        };
-        Lane8 cur, nxt;
-        issue(qa, cur);
-        bool stopped = false;
-        for (int k0 = qa; k0 <= qb; k0 += 32) {
-            const bool more = k0 + 32 <= qb;
-            if (more) issue(k0 + 32, nxt);
-            const bool act = k0 + lane <= qb && !cur.idle;
-            const float val = trilinear(cur.v, cur.w[0], cur.w[1], cur.w[2]);
-            const int n_in = min(qb - k0, 31) + 1;
-            const int hit = fold32<MODE>(acc, val, act, tab, T, A.tau);
-            const unsigned idle_bits = __ballot_sync(0xffffffffu, cur.idle && k0 + lane <= qb);
-            if (lane == 0) {
-                const unsigned upto = hit ? (hit >= 32 ? 0xffffffffu : ((1u << hit) - 1u)) : 0xffffffffu;
-                const int idle_n = __popc(idle_bits & upto);
-                n_taken += (unsigned long long)((hit ? hit : n_in) - idle_n);
-                n_skip += (unsigned long long)idle_n;
-            }
-            if (hit) { stopped = true; break; }
-            cur = nxt;
-        }
-        if (lane == 0) { ++n_visit; n_term += stopped ? 1 : 0; }
-        if (lane == src) mine = acc;
-    }
-    if (live) write_frame_pixel<MODE>(V, T, A, i, j, mine, r.k1 >= r.k0);
-    if (A.counters) {
-        const unsigned long long nom = r.k1 >= r.k0 ? (unsigned long long)(r.k1 - r.k0 + 1) : 0ULL;
-        count(A.counters, kRays, nom ? 1 : 0);
-        count(A.counters, kNominal, nom);
-        count(A.counters, kTaken, n_taken);
-        count(A.counters, kVisited, n_visit);
-        count(A.counters, kSkipped, n_skip);
-        count(A.counters, kTerminated, n_term);
-    }
-}
 
 // ================================================================== variant 3: lockstep, two phases
 // A warp owns the 32 rays of its 8 x 4 pixel tile and walks them TOGETHER through chunks of 32
@@ -726,25 +524,38 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
         int rc = __ffs(rest) - 1;
         rest &= rest - 1;
         issue(rc, cur);
+        unsigned my_fold = 0u, my_done = 0u;                // this lane's ray: samples to fold / interpolated
         for (;;) {
             int rn = -1;
             if (rest) { rn = __ffs(rest) - 1; rest &= rest - 1; issue(rn, nxt); }
             const float val = trilinear(cur.v, cur.w[0], cur.w[1], cur.w[2]);
-            vals[rc * kValPitch + lane] = cur.idle ? -INFINITY : val;
+            vals[rc * kValPitch + lane] = val;
+            // samples whose table coordinate lies below x_clear have weight exactly zero (see fold)
+            bool need = !cur.idle;
+            if (MODE == VR_MODE_EA) need = need && !(__fmul_rn(__fsub_rn(val, T.vmin), T.scale) < T.x_clear);
+            const unsigned fold_bits = __ballot_sync(0xffffffffu, need);
+            const unsigned done_bits = __ballot_sync(0xffffffffu, !cur.idle);
+            if (lane == rc) { my_fold = fold_bits; my_done = done_bits; }
             if (rn < 0) break;
             cur = nxt; rc = rn;
         }
         __syncwarp();
-        // ---- phase 2: lane = ray
+        // ---- phase 2: lane = ray; idle lanes of phase 1 (outside [ka, kb]) carry no bit
         if ((act >> lane) & 1u) {
-            const int l0 = max(ka, kbase) - kbase, l1 = min(kb, kbase + 31) - kbase;
             const float* mine = vals + lane * kValPitch;
-            for (int l = l0; l <= l1; ++l) {
-                const float v = mine[l];
-                if (v == -INFINITY) { ++n_skip; continue; }
-                ++n_taken;
-                if (fold<MODE>(acc, v, tab, T, A.tau)) { stopped = true; alive = false; break; }
+            const int l0 = max(ka, kbase) - kbase, l1 = min(kb, kbase + 31) - kbase;
+            unsigned range = (l1 >= 31 ? 0xffffffffu : ((1u << (l1 + 1)) - 1u)) & ~((1u << l0) - 1u);
+            unsigned upto = 0xffffffffu;
+            for (unsigned bits = my_fold; bits; bits &= bits - 1) {
+                const int l = __ffs(bits) - 1;
+                if (fold<MODE>(acc, mine[l], tab, T, A.tau)) {
+                    stopped = true; alive = false;
+                    upto = l >= 31 ? 0xffffffffu : ((1u << (l + 1)) - 1u);
+                    break;
+                }
             }
+            n_taken += (unsigned long long)__popc(my_done & upto);
+            n_skip += (unsigned long long)__popc(range & ~my_done & upto);
         }
         __syncwarp();
     }
@@ -829,7 +640,6 @@ __global__ void upload_half_kernel(float4* dst, const __grid_constant__ HalfTabl
 cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s) {
     dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
     if (a.variant == 3) VR_DISPATCH_LS(true, grid, c, v, t, a, nullptr, 0);
-    else if (a.variant == 2) VR_DISPATCH(render_global_sp_kernel, grid, c, v, t, a);
     else VR_DISPATCH(render_global_kernel, grid, c, v, t, a);
     return cudaGetLastError();
 }
@@ -838,7 +648,6 @@ cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFD
                                  const PartialDev* d_partials, int n, int total_tiles, cudaStream_t s) {
     if (n == 0 || total_tiles == 0) return cudaSuccess;
     if (a.variant == 3) VR_DISPATCH_LS(false, total_tiles, c, v, t, a, d_partials, n);
-    else if (a.variant == 2) VR_DISPATCH(render_bricks_sp_kernel, total_tiles, c, v, t, a, d_partials, n);
     else VR_DISPATCH(render_bricks_kernel, total_tiles, c, v, t, a, d_partials, n);
     return cudaGetLastError();
 }

@@ -25,9 +25,9 @@ def H():
 
 
 # Every test below runs once with the library's own choice of marcher variant and macro-cell
-# skipping ("auto") and once per forced variant (0: ray per thread, 2: ray per warp, 3: lockstep),
+# skipping ("auto") and once per forced variant (0: ray per thread, 3: lockstep ray per warp),
 # with the macro-cell level of the skipping forced on.
-@pytest.fixture(autouse=True, params=["auto", "v0", "v2", "v3"])
+@pytest.fixture(autouse=True, params=["auto", "v0", "v3"])
 def marcher(request, H):
     from paper_1012_2909_b200 import vr
     H.FORCED_OPTIONS.clear()
