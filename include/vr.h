@@ -161,8 +161,11 @@ int vr_reset_counters(vr_ctx* ctx, void* stream);
  *  VR_OPT_LAYOUT (default 1): voxel order inside a brick, 0 = rows (x fastest), 1 = 4 x 4 x 2
  *    micro-blocks of one 128-byte line each; read by the next upload / generate / attach call.
  *  VR_OPT_L2_FETCH: cudaLimitMaxL2FetchGranularity of the device (32, 64 or 128 bytes; measured
- *    to have no effect on B200, where HBM is read in whole 128-byte lines). */
-enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETCH = 4, VR_OPT_LAYOUT = 5 };
+ *    to have no effect on B200, where HBM is read in whole 128-byte lines).
+ *  VR_OPT_DENSE (default -1): how the lockstep marcher folds emission-absorption samples, 1 =
+ *    through shared memory, all rays of a warp in parallel; 0 = one by one in the lane that owns
+ *    the ray; -1 = 0 if the table starts with transparent entries, else 1. */
+enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETCH = 4, VR_OPT_LAYOUT = 5, VR_OPT_DENSE = 6 };
 int vr_set_option(vr_ctx* ctx, int option, int value);
 
 #ifdef __cplusplus

@@ -37,7 +37,7 @@ struct vr_ctx {
     float* d_stage = nullptr;
     size_t stage_bytes = 0;
     int64_t launches = 0;
-    int opt_skip = 1, opt_cell_skip = -1, opt_variant = -1, opt_layout = 1;   // -1: chosen per view / TF
+    int opt_skip = 1, opt_cell_skip = -1, opt_variant = -1, opt_layout = 1, opt_dense = -1;   // -1: chosen per view / TF
     float x_clear = -INFINITY;
     double active_cell_fraction = 1.0;   // macro-cells active against the current table (EA)
     unsigned long long* d_scratch = nullptr;
@@ -216,6 +216,14 @@ int skip_level(const vr_ctx* ctx, int mode) {
     if (ctx->opt_cell_skip >= 0) return ctx->opt_cell_skip ? 2 : 1;
     if (mode == VR_MODE_MIP) return resolve_variant(ctx) == 3 ? 2 : 1;
     return ctx->active_cell_fraction < kCellSkipMaxActive ? 2 : 1;
+}
+
+// Lockstep emission-absorption: fold through shared memory with all rays in parallel (dense) or
+// hand the few samples above x_clear to the owning lane one by one (sparse).  By default dense
+// unless the table starts with a run of transparent entries (x_clear >= 1).
+int resolve_dense(const vr_ctx* ctx) {
+    if (ctx->opt_dense >= 0) return ctx->opt_dense;
+    return ctx->x_clear >= 1.f ? 0 : 1;
 }
 
 TFDesc tf_desc(const vr_ctx* ctx) {
@@ -572,7 +580,7 @@ int vr_render_ea(vr_ctx* ctx, float* d_out, const float bg[4], float tau, void* 
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
-    a.mode = VR_MODE_EA; a.tau = tau; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx);
+    a.mode = VR_MODE_EA; a.tau = tau; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx); a.dense = resolve_dense(ctx);
     for (int i = 0; i < 4; ++i) a.bg[i] = bg[i];
     a.out = d_out; a.counters = ctx->d_counters;
     VR_CUDA(ctx, launch_render_global(ctx->cube, ctx->view, tf_desc(ctx), a, s));
@@ -653,7 +661,7 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
     int tiles = 0;
     if ((rc = upload_partials(ctx, mode, hp, n, true, &tiles, s))) return rc;
     RenderArgs a{};
-    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx);
+    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx); a.dense = resolve_dense(ctx);
     a.counters = ctx->d_counters;
     VR_CUDA(ctx, launch_render_bricks(ctx->cube, ctx->view, tf_desc(ctx), a, ctx->d_partials, n, tiles, s));
     ctx->launches += (n > 0 && tiles > 0) ? 1 : 0;
@@ -704,6 +712,7 @@ int vr_set_option(vr_ctx* ctx, int option, int value) {
         VR_CUDA(ctx, cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)value));
         return VR_OK;
     }
+    if (option == VR_OPT_DENSE) { ctx->opt_dense = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_VARIANT) {
         if (value != -1 && value != 0 && value != 3) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");
         ctx->opt_variant = value; return VR_OK;

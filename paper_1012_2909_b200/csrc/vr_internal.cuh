@@ -93,7 +93,8 @@ cudaError_t launch_generate(const CubeDesc& c, float* d_cube, const GenDev& g, c
 struct RenderArgs {
     int mode; float tau; float bg[4]; float miss;
     int skip;              // 0: none; 1: configured bricks; 2: bricks and 8^3 macro-cells (O-10)
-    int variant;           // 0: one ray per thread; 3: lockstep, two phases (ray per warp)
+    int variant;           // 0: one ray per thread; 3: lockstep (the lanes of a warp take one ray's samples)
+    int dense;             // lockstep EA: fold through shared memory, all rays in parallel (see vr_march.cu)
     float* out; float* out_rgba; unsigned long long* counters;
 };
 cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s);

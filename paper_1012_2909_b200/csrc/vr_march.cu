@@ -113,12 +113,10 @@ __device__ __forceinline__ BrickRef brick_ref(const CubeDesc& c, int bid, const 
     return b;
 }
 
-// The 8 voxels of the trilinear cell whose lower corner is (ix, iy, iz) (global voxel indices,
-// inside brick b or on its halo), in the order 000 100 010 110 001 101 011 111.
+// Offset q of stored voxel (lx, ly, lz) inside its brick and the steps to its +1 neighbours.
 template <int LAYOUT>
-__device__ __forceinline__ void gather8(const BrickRef& b, int ix, int iy, int iz, float v[8]) {
-    const unsigned lx = (unsigned)(ix - b.lo[0]), ly = (unsigned)(iy - b.lo[1]), lz = (unsigned)(iz - b.lo[2]);
-    unsigned q, dx, dy, dz;
+__device__ __forceinline__ void cell_address(const BrickRef& b, unsigned lx, unsigned ly, unsigned lz, unsigned& q,
+                                             unsigned& dx, unsigned& dy, unsigned& dz) {
     if (LAYOUT == 0) {
         q = lx + b.s0 * ly + b.s1 * lz;
         dx = 1u; dy = b.s0; dz = b.s1;
@@ -128,6 +126,15 @@ __device__ __forceinline__ void gather8(const BrickRef& b, int ix, int iy, int i
         dy = (ly & 1u) == 0u ? 4u : ((ly & 2u) == 0u ? 12u : b.s0 - 20u);
         dz = (lz & 1u) ? b.s1 - 8u : 8u;
     }
+}
+
+// The 8 voxels of the trilinear cell whose lower corner is (ix, iy, iz) (global voxel indices,
+// inside brick b or on its halo), in the order 000 100 010 110 001 101 011 111.
+template <int LAYOUT>
+__device__ __forceinline__ void gather8(const BrickRef& b, int ix, int iy, int iz, float v[8]) {
+    const unsigned lx = (unsigned)(ix - b.lo[0]), ly = (unsigned)(iy - b.lo[1]), lz = (unsigned)(iz - b.lo[2]);
+    unsigned q, dx, dy, dz;
+    cell_address<LAYOUT>(b, lx, ly, lz, q, dx, dy, dz);
     const float* p = b.base + q;
     v[0] = __ldg(p);           v[1] = __ldg(p + dx);
     v[2] = __ldg(p + dy);      v[3] = __ldg(p + dy + dx);
@@ -415,32 +422,68 @@ render_bricks_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
     }
 }
 
-struct Lane8 { float v[8]; float w[3]; bool idle; };
-
-// ================================================================== variant 3: lockstep, two phases
+// ================================================================== variant 3: lockstep
 // A warp owns the 32 rays of its 8 x 4 pixel tile and walks them TOGETHER through chunks of 32
 // lattice indices [kbase, kbase + 31] (k counts from the near plane, so a chunk is a thin shell
 // that all 32 rays cross at about the same place: lines shared by neighbouring rays are fetched
-// once and hit in L1 / L2, not re-read from HBM).  Each chunk has two phases:
-//   phase 1, sample-parallel: for every ray of the warp in turn the 32 lanes take the 32 samples
-//     of that ray in the chunk (positions, gathers, trilinear, O-3 / O-4); the lanes' addresses
-//     follow the ray, and the gathers of the next ray are issued before the current ones are
-//     used.  Interpolated values go to shared memory, vals[ray][sample].
-//   phase 2, ray-parallel: lane r folds the 32 values of ITS ray front to back (O-5 / O-7), the
-//     accumulator never leaves the lane, so dense opaque transfer functions cost the same as
-//     sparse ones and ERT (O-7) is exact per ray.
-// Skipped samples (O-10) are stored as -inf and never folded.
+// once and hit in L1 / L2, not re-read from HBM).  Inside a chunk the rays are taken one after the
+// other, SAMPLE-PARALLEL: the 32 lanes take the 32 samples of that ray in the chunk (positions,
+// O-3; gathers and trilinear interpolation, O-4), so the lanes' addresses follow the ray.
+//
+// The gathers are asynchronous copies (cp.async, 4 bytes each) into a per-lane ring of kDepth
+// slots in shared memory: the 8 voxels of the ray taken kDepth - 1 steps later are requested
+// before the current ones are interpolated, they occupy no register and stall no scoreboard.
+//
+// The values are then folded in ray order (O-5 / O-7) by the lane that owns the ray, whose
+// accumulator never leaves it, so early ray termination (O-7) is exact per ray:
+//   MIP        - max is exact in any order: a warp reduction, then lane r takes the maximum;
+//   EA, SPARSE - the few samples whose table coordinate is not below x_clear (see fold) are
+//                handed to lane r one by one with a shuffle, in lattice order;
+//   EA, DENSE  - the values go to shared memory, vals[ray][sample], and after the last ray of
+//                the chunk every lane folds the 32 values of ITS ray front to back (all 32 rays
+//                in parallel), so opaque transfer functions cost the same as sparse ones.
+// Skipped samples (O-10) are never interpolated or folded.  All three give identical frames.
 constexpr int kValPitch = 33;
+constexpr int kDepth = 3;               // rays in flight per warp (measured: 2 -> 12.1, 3 -> 12.0, 4 -> 13.5 ms on C3)
+constexpr int kBitsWords = 1024;        // shared copy of one brick's macro-cell bits (256^3 bricks: 32^3 cells)
 
-template <int MODE, int LAYOUT, bool GLOBAL>
-__global__ void __launch_bounds__(kThreads)
+__device__ __forceinline__ void cp_async4(unsigned dst, const float* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// Request the 8 voxels of gather8 into dst[e * 32] (floats, e = 0..7; dst is a shared address in bytes).
+template <int LAYOUT>
+__device__ __forceinline__ void gather8_async(const BrickRef& b, int ix, int iy, int iz, unsigned dst) {
+    unsigned q, dx, dy, dz;
+    cell_address<LAYOUT>(b, (unsigned)(ix - b.lo[0]), (unsigned)(iy - b.lo[1]), (unsigned)(iz - b.lo[2]), q, dx, dy, dz);
+    const float* p = b.base + q;
+    cp_async4(dst, p);             cp_async4(dst + 128, p + dx);
+    cp_async4(dst + 256, p + dy);  cp_async4(dst + 384, p + dy + dx);
+    cp_async4(dst + 512, p + dz);  cp_async4(dst + 640, p + dz + dx);
+    cp_async4(dst + 768, p + dz + dy); cp_async4(dst + 896, p + dz + dy + dx);
+}
+
+struct Slot { float w[3]; int rc; bool idle; };   // one ray in flight: weights of this lane's sample
+
+// 7 CTAs per SM: 72 registers; an 8th CTA (64 registers) would shrink L1 to 28 KB and costs 10 % (measured)
+template <int MODE, int LAYOUT, bool GLOBAL, bool DENSE>
+__global__ void __launch_bounds__(kThreads, 7)
 render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                  const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
                  const PartialDev* __restrict__ parts, int n_parts) {
-    __shared__ float4 tab[256];
+    constexpr bool EA = MODE == VR_MODE_EA;
+    constexpr bool VALS = EA && DENSE;
+    constexpr bool SBITS = EA && !GLOBAL;
+    constexpr int kWarps = kThreads / 32;
+    __shared__ float4 tab[EA ? 256 : 1];
     __shared__ PartialDev part;
-    __shared__ float vals_all[kThreads / 32][32 * kValPitch];
-    __shared__ float4 rays_all[kThreads / 32][64];
+    __shared__ float4 rays_all[kWarps][64];
+    __shared__ float stage_all[kWarps][kDepth * 256];
+    __shared__ float vals_all[VALS ? kWarps : 1][VALS ? 32 * kValPitch : 1];
+    __shared__ unsigned sbits[SBITS ? kBitsWords : 1];
     int fx, fy;                                             // view pixel of this thread's ray
     bool live;
     if (GLOBAL) {
@@ -452,26 +495,36 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
         live = locate_tile(parts, n_parts, part, lx, ly);
         fx = lx; fy = ly;
     }
-    if (MODE == VR_MODE_EA) load_tf(tab, T.baked);
+    const bool cells = A.skip >= 2;
+    int bid0 = 0, lo0[3] = {0, 0, 0};
+    if (!GLOBAL) {
+        bid0 = part.brick;
+        lo0[0] = (bid0 % c.G[0]) * c.B[0]; lo0[1] = ((bid0 / c.G[0]) % c.G[1]) * c.B[1]; lo0[2] = (bid0 / (c.G[0] * c.G[1])) * c.B[2];
+    }
+    const bool bits_shared = SBITS && cells && c.cell_words_per_brick <= kBitsWords;
+    if (bits_shared)
+        for (int i = threadIdx.x; i < c.cell_words_per_brick; i += kThreads)
+            sbits[i] = __ldg(&c.cell_bits[(long long)bid0 * c.cell_words_per_brick + i]);
+    if (EA) load_tf(tab, T.baked);                          // ends with __syncthreads()
     Ray r; r.k0 = 0; r.k1 = -1;
     r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
     if (live) setup_ray(V, c, GLOBAL ? fx : part.x0 + fx, GLOBAL ? fy : part.y0 + fy, r);
     int ka = r.k0, kb = r.k1;
-    int bid0 = 0, lo0[3] = {0, 0, 0};
     if (!GLOBAL) {
-        bid0 = part.brick;
         const int b[3] = {bid0 % c.G[0], (bid0 / c.G[0]) % c.G[1], bid0 / (c.G[0] * c.G[1])};
-        lo0[0] = b[0] * c.B[0]; lo0[1] = b[1] * c.B[1]; lo0[2] = b[2] * c.B[2];
         brick_interval(c, r, b, lo0, ka, kb);
     }
     const BrickRef br0 = brick_ref<LAYOUT>(c, bid0, lo0);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float* vals = vals_all[warp];
+    float* vals = vals_all[VALS ? warp : 0];
     float4* rays = rays_all[warp];
+    const float* stage = stage_all[warp] + lane;
+    const unsigned stage_addr = (unsigned)__cvta_generic_to_shared(stage);
     rays[2 * lane] = make_float4(r.o[0], r.o[1], r.o[2], r.d[0]);
     rays[2 * lane + 1] = make_float4(r.d[1], r.d[2], __int_as_float(ka), __int_as_float(kb));
     __syncwarp();
     bool alive = ka <= kb, stopped = false;
+    int k_end = kb;                                         // last lattice index this ray got to (ERT: the stop)
     int K0 = alive ? ka : 0x7fffffff, K1 = alive ? kb : -1;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -479,101 +532,137 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
         K1 = max(K1, __shfl_xor_sync(0xffffffffu, K1, o));
     }
     Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-    unsigned long long n_taken = 0, n_skip = 0;
-    const bool cells = A.skip >= 2;
+    unsigned n_taken = 0;
     for (int kbase = K0; kbase <= K1; kbase += 32) {
         if (!__ballot_sync(0xffffffffu, alive)) break;
         const unsigned act = __ballot_sync(0xffffffffu, alive && ka <= kbase + 31 && kb >= kbase);
         if (!act) continue;
-        // ---- phase 1: lane = sample kbase + lane of ray rr
-        const int k = kbase + lane;
+        const int k = kbase + lane;                         // this lane's sample of every ray of the chunk
         const float t = __fmul_rn((float)k, r.step);        // O-3: t_k = k * Delta
-        auto issue = [&](int rr, Lane8& L) {
-            const float4 ra = rays[2 * rr], rb = rays[2 * rr + 1];
-            float m_r = -INFINITY;
-            if (MODE == VR_MODE_MIP) m_r = __shfl_sync(0xffffffffu, acc.m, rr);
-            L.idle = true;
-#pragma unroll
-            for (int e = 0; e < 8; ++e) L.v[e] = 0.f;
-            L.w[0] = L.w[1] = L.w[2] = 0.f;
-            if (k >= __float_as_int(rb.z) && k <= __float_as_int(rb.w)) {
-                float p[3], fl[3];
-                p[0] = __fmaf_rn(t, ra.w, ra.x); p[1] = __fmaf_rn(t, rb.x, ra.y); p[2] = __fmaf_rn(t, rb.y, ra.z);
-                const int iv[3] = {floor_pos(p[0], fl[0]), floor_pos(p[1], fl[1]), floor_pos(p[2], fl[2])};
-                L.w[0] = __fsub_rn(p[0], fl[0]); L.w[1] = __fsub_rn(p[1], fl[1]); L.w[2] = __fsub_rn(p[2], fl[2]);
-                if (GLOBAL) {
-                    int b[3]; brick_of(c, iv, b);
-                    const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
-                    const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
-                    bool idle = false;
-                    if (A.skip) {                           // O-10 (exact), per sample
-                        if (MODE == VR_MODE_MIP) idle = __ldg(&c.brick_mm[bid]).y <= m_r;
-                        else idle = __ldg(&c.brick_active[bid]) == 0;
-                        if (cells && !idle) idle = cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], m_r);
-                    }
-                    L.idle = idle;
-                    if (!idle) { const BrickRef br = brick_ref<LAYOUT>(c, bid, lo); gather8<LAYOUT>(br, iv[0], iv[1], iv[2], L.v); }
-                } else {
-                    L.idle = cells && cell_idle<MODE>(c, bid0, lo0, iv[0], iv[1], iv[2], m_r);
-                    if (!L.idle) gather8<LAYOUT>(br0, iv[0], iv[1], iv[2], L.v);
-                }
-            }
-        };
-        Lane8 cur, nxt;
         unsigned rest = act;
-        int rc = __ffs(rest) - 1;
-        rest &= rest - 1;
-        issue(rc, cur);
-        unsigned my_fold = 0u, my_done = 0u;                // this lane's ray: samples to fold / interpolated
-        for (;;) {
-            int rn = -1;
-            if (rest) { rn = __ffs(rest) - 1; rest &= rest - 1; issue(rn, nxt); }
-            const float val = trilinear(cur.v, cur.w[0], cur.w[1], cur.w[2]);
-            vals[rc * kValPitch + lane] = val;
-            // samples whose table coordinate lies below x_clear have weight exactly zero (see fold)
-            bool need = !cur.idle;
-            if (MODE == VR_MODE_EA) need = need && !(__fmul_rn(__fsub_rn(val, T.vmin), T.scale) < T.x_clear);
-            const unsigned fold_bits = __ballot_sync(0xffffffffu, need);
-            const unsigned done_bits = __ballot_sync(0xffffffffu, !cur.idle);
-            if (lane == rc) { my_fold = fold_bits; my_done = done_bits; }
-            if (rn < 0) break;
-            cur = nxt; rc = rn;
-        }
-        __syncwarp();
-        // ---- phase 2: lane = ray; idle lanes of phase 1 (outside [ka, kb]) carry no bit
-        if ((act >> lane) & 1u) {
-            const float* mine = vals + lane * kValPitch;
-            const int l0 = max(ka, kbase) - kbase, l1 = min(kb, kbase + 31) - kbase;
-            unsigned range = (l1 >= 31 ? 0xffffffffu : ((1u << (l1 + 1)) - 1u)) & ~((1u << l0) - 1u);
-            unsigned upto = 0xffffffffu;
-            for (unsigned bits = my_fold; bits; bits &= bits - 1) {
-                const int l = __ffs(bits) - 1;
-                if (fold<MODE>(acc, mine[l], tab, T, A.tau)) {
-                    stopped = true; alive = false;
-                    upto = l >= 31 ? 0xffffffffu : ((1u << (l + 1)) - 1u);
-                    break;
+        // request the 8 voxels of this lane's sample of the next ray of the chunk (if any) into slot s
+        auto issue = [&](Slot& S, const int s) {
+            S.rc = -1; S.idle = true;
+            S.w[0] = S.w[1] = S.w[2] = 0.f;
+            if (rest) {
+                const int rr = __ffs(rest) - 1;
+                rest &= rest - 1;
+                S.rc = rr;
+                const float4 ra = rays[2 * rr], rb = rays[2 * rr + 1];
+                float m_r = -INFINITY;
+                if (!EA) m_r = __shfl_sync(0xffffffffu, acc.m, rr);
+                if (k >= __float_as_int(rb.z) && k <= __float_as_int(rb.w)) {
+                    float p[3], fl[3];
+                    p[0] = __fmaf_rn(t, ra.w, ra.x); p[1] = __fmaf_rn(t, rb.x, ra.y); p[2] = __fmaf_rn(t, rb.y, ra.z);
+                    const int iv[3] = {floor_pos(p[0], fl[0]), floor_pos(p[1], fl[1]), floor_pos(p[2], fl[2])};
+                    S.w[0] = __fsub_rn(p[0], fl[0]); S.w[1] = __fsub_rn(p[1], fl[1]); S.w[2] = __fsub_rn(p[2], fl[2]);
+                    if (GLOBAL) {
+                        int b[3]; brick_of(c, iv, b);
+                        const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
+                        const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
+                        bool idle = false;
+                        if (A.skip) {                       // O-10 (exact), per sample
+                            if (!EA) idle = __ldg(&c.brick_mm[bid]).y <= m_r;
+                            else idle = __ldg(&c.brick_active[bid]) == 0;
+                            if (cells && !idle) idle = cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], m_r);
+                        }
+                        S.idle = idle;
+                        if (!idle) gather8_async<LAYOUT>(brick_ref<LAYOUT>(c, bid, lo), iv[0], iv[1], iv[2], stage_addr + 1024u * s);
+                    } else {
+                        bool idle = false;
+                        if (bits_shared) {
+                            const int cidx = ((iv[0] - lo0[0]) >> 3) + c.C[0] * (((iv[1] - lo0[1]) >> 3) + c.C[1] * ((iv[2] - lo0[2]) >> 3));
+                            idle = ((sbits[cidx >> 5] >> (cidx & 31)) & 1u) == 0u;
+                        } else if (cells) idle = cell_idle<MODE>(c, bid0, lo0, iv[0], iv[1], iv[2], m_r);
+                        S.idle = idle;
+                        if (!idle) gather8_async<LAYOUT>(br0, iv[0], iv[1], iv[2], stage_addr + 1024u * s);
+                    }
                 }
             }
-            n_taken += (unsigned long long)__popc(my_done & upto);
-            n_skip += (unsigned long long)__popc(range & ~my_done & upto);
+            cp_async_commit();
+        };
+        unsigned my_fold = 0u, my_done = 0u;                // DENSE: this lane's ray: samples to fold / interpolated
+        // interpolate the samples of the ray in slot s (its copies have landed) and fold them
+        auto consume = [&](const Slot& S, const int s) {
+            const float* st = stage + 256 * s;
+            float v[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) v[e] = st[32 * e];
+            const float val = trilinear(v, S.w[0], S.w[1], S.w[2]);       // idle lanes: stale values, never used
+            const unsigned done_bits = __ballot_sync(0xffffffffu, !S.idle);
+            if (!EA) {
+                float m = S.idle ? -INFINITY : val;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+                if (lane == S.rc) { acc.m = fmaxf(acc.m, m); n_taken += __popc(done_bits); }
+                return;
+            }
+            // samples whose table coordinate lies below x_clear have weight exactly zero (see fold)
+            const bool need = !S.idle && !(__fmul_rn(__fsub_rn(val, T.vmin), T.scale) < T.x_clear);
+            const unsigned fold_bits = __ballot_sync(0xffffffffu, need);
+            if (VALS) {
+                vals[S.rc * kValPitch + lane] = val;
+                if (lane == S.rc) { my_fold = fold_bits; my_done = done_bits; }
+                return;
+            }
+            unsigned upto = 0xffffffffu;
+            for (unsigned bits = fold_bits; bits; bits &= bits - 1) {
+                const int l = __ffs(bits) - 1;
+                const float vl = __shfl_sync(0xffffffffu, val, l);
+                if (lane == S.rc && alive && fold<MODE>(acc, vl, tab, T, A.tau)) {
+                    stopped = true; alive = false; k_end = kbase + l;
+                    upto = l >= 31 ? 0xffffffffu : ((1u << (l + 1)) - 1u);
+                }
+            }
+            if (lane == S.rc) n_taken += __popc(done_bits & upto);
+        };
+        Slot slot[kDepth];
+#pragma unroll
+        for (int s = 0; s < kDepth - 1; ++s) issue(slot[s], s);
+        for (bool more = true; more;) {
+#pragma unroll
+            for (int u = 0; u < kDepth; ++u) {
+                issue(slot[(u + kDepth - 1) % kDepth], (u + kDepth - 1) % kDepth);
+                cp_async_wait<kDepth - 1>();
+                if (slot[u].rc < 0) { more = false; break; }
+                consume(slot[u], u);
+            }
         }
-        __syncwarp();
+        if (VALS) {
+            __syncwarp();
+            // lane = ray: fold its flagged values front to back
+            if ((act >> lane) & 1u) {
+                const float* mine = vals + lane * kValPitch;
+                unsigned upto = 0xffffffffu;
+                for (unsigned bits = my_fold; bits; bits &= bits - 1) {
+                    const int l = __ffs(bits) - 1;
+                    if (fold<MODE>(acc, mine[l], tab, T, A.tau)) {
+                        stopped = true; alive = false; k_end = kbase + l;
+                        upto = l >= 31 ? 0xffffffffu : ((1u << (l + 1)) - 1u);
+                        break;
+                    }
+                }
+                n_taken += __popc(my_done & upto);
+            }
+            __syncwarp();
+        }
     }
     if (live) {
         if (GLOBAL) write_frame_pixel<MODE>(V, T, A, fx, fy, acc, r.k1 >= r.k0);
         else {
             const long long px = (long long)fy * part.pitch + fx;
-            if (MODE == VR_MODE_MIP) reinterpret_cast<float*>(part.data)[px] = acc.m;
+            if (!EA) reinterpret_cast<float*>(part.data)[px] = acc.m;
             else reinterpret_cast<float4*>(part.data)[px] = make_float4(acc.C[0], acc.C[1], acc.C[2], acc.A);
         }
     }
     if (A.counters) {
         const unsigned long long nom = kb >= ka ? (unsigned long long)(kb - ka + 1) : 0ULL;
+        const unsigned long long reached = kb >= ka ? (unsigned long long)(k_end - ka + 1) : 0ULL;
         if (GLOBAL) count(A.counters, kRays, nom ? 1 : 0);
         count(A.counters, kNominal, nom);
         count(A.counters, kTaken, n_taken);
         count(A.counters, kVisited, nom ? 1 : 0);
-        count(A.counters, kSkipped, n_skip);
+        count(A.counters, kSkipped, reached - n_taken);     // lattice samples passed over by O-10
         count(A.counters, kTerminated, stopped ? 1 : 0);
     }
 }
@@ -629,11 +718,14 @@ __global__ void upload_half_kernel(float4* dst, const __grid_constant__ HalfTabl
 #define VR_DISPATCH_LS(GLOBAL, GRID, ...)                                                                \
     do {                                                                                                 \
         if (a.mode == VR_MODE_MIP) {                                                                     \
-            if (c.layout == 0) render_ls_kernel<VR_MODE_MIP, 0, GLOBAL><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
-            else render_ls_kernel<VR_MODE_MIP, 1, GLOBAL><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);         \
+            if (c.layout == 0) render_ls_kernel<VR_MODE_MIP, 0, GLOBAL, false><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
+            else render_ls_kernel<VR_MODE_MIP, 1, GLOBAL, false><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);  \
+        } else if (a.dense) {                                                                            \
+            if (c.layout == 0) render_ls_kernel<VR_MODE_EA, 0, GLOBAL, true><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
+            else render_ls_kernel<VR_MODE_EA, 1, GLOBAL, true><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);    \
         } else {                                                                                         \
-            if (c.layout == 0) render_ls_kernel<VR_MODE_EA, 0, GLOBAL><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
-            else render_ls_kernel<VR_MODE_EA, 1, GLOBAL><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);          \
+            if (c.layout == 0) render_ls_kernel<VR_MODE_EA, 0, GLOBAL, false><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
+            else render_ls_kernel<VR_MODE_EA, 1, GLOBAL, false><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);   \
         }                                                                                                \
     } while (0)
 

@@ -25,14 +25,17 @@ def H():
 
 
 # Every test below runs once with the library's own choice of marcher variant and macro-cell
-# skipping ("auto") and once per forced variant (0: ray per thread, 3: lockstep ray per warp),
-# with the macro-cell level of the skipping forced on.
-@pytest.fixture(autouse=True, params=["auto", "v0", "v3"])
+# skipping ("auto") and once per forced variant (0: ray per thread; 3: lockstep ray per warp, folding
+# emission-absorption samples in the owning lane "v3s" or through shared memory "v3d"), with the
+# macro-cell level of the skipping forced on.
+@pytest.fixture(autouse=True, params=["auto", "v0", "v3s", "v3d"])
 def marcher(request, H):
     from paper_1012_2909_b200 import vr
     H.FORCED_OPTIONS.clear()
     if request.param != "auto":
-        H.FORCED_OPTIONS.update({vr.OPT_VARIANT: int(request.param[1:]), vr.OPT_CELL_SKIP: 1})
+        H.FORCED_OPTIONS.update({vr.OPT_VARIANT: int(request.param[1]), vr.OPT_CELL_SKIP: 1})
+        if request.param[2:]:
+            H.FORCED_OPTIONS[vr.OPT_DENSE] = int(request.param[2] == "d")
     yield request.param
     H.FORCED_OPTIONS.clear()
 
