@@ -54,7 +54,8 @@ const char* vr_status_string(int status);
 /* ---- S0: cube residency (BASELINE.json north_star (2),(4)) -------------- */
 /* Bytes the caller must allocate for the brick-major cube (bricks of bx*by*bz voxels stored with
  * a one-sided +1 halo, x pitch padded to a multiple of 4 floats) and for its metadata (per-brick
- * and per-8^3-cell (min,max) over the halo-inclusive voxel set, plus activity bits). */
+ * and per-8^3-cell (min,max) over the halo-inclusive voxel set, plus activity bits: one per brick,
+ * per macro-cell and per voxel, i.e. 1/32 of the cube). */
 int vr_cube_layout(int nx, int ny, int nz, int bx, int by, int bz, size_t* cube_bytes,
                    size_t* meta_bytes);
 
@@ -164,8 +165,13 @@ int vr_reset_counters(vr_ctx* ctx, void* stream);
  *    to have no effect on B200, where HBM is read in whole 128-byte lines).
  *  VR_OPT_DENSE (default -1): how the lockstep marcher folds emission-absorption samples, 1 =
  *    through shared memory, all rays of a warp in parallel; 0 = one by one in the lane that owns
- *    the ray; -1 = 0 if the table starts with transparent entries, else 1. */
-enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETCH = 4, VR_OPT_LAYOUT = 5, VR_OPT_DENSE = 6 };
+ *    the ray; -1 = 0 if the table starts with transparent entries, else 1.
+ *  VR_OPT_OCCUPANCY (default -1): the finest level of the skipping, one bit per trilinear cell,
+ *    classified on the device when the set of transparent table entries changes (one pass over the
+ *    cube); used by the lockstep marcher for emission-absorption with VR_OPT_DENSE 0 on layout 1.
+ *    1 / -1 = on where it applies, 0 = off. */
+enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETCH = 4, VR_OPT_LAYOUT = 5, VR_OPT_DENSE = 6,
+       VR_OPT_OCCUPANCY = 7 };
 int vr_set_option(vr_ctx* ctx, int option, int value);
 
 #ifdef __cplusplus

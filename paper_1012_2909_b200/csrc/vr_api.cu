@@ -37,10 +37,15 @@ struct vr_ctx {
     float* d_stage = nullptr;
     size_t stage_bytes = 0;
     int64_t launches = 0;
-    int opt_skip = 1, opt_cell_skip = -1, opt_variant = -1, opt_layout = 1, opt_dense = -1;   // -1: chosen per view / TF
+    int opt_skip = 1, opt_cell_skip = -1, opt_variant = -1, opt_layout = 1, opt_dense = -1, opt_occ = -1;   // -1: chosen per view / TF
     float x_clear = -INFINITY;
     double active_cell_fraction = 1.0;   // macro-cells active against the current table (EA)
     unsigned long long* d_scratch = nullptr;
+    // what the activity bits on the device (bricks, macro-cells, occupancy) were classified against:
+    // the zero pattern of the baked opacities and the value -> table mapping
+    bool key_valid = false, occ_valid = false;
+    int key_nz[257];
+    float key_vmin = 0, key_scale = 0;
 };
 
 namespace {
@@ -104,6 +109,7 @@ void bind_meta(CubeDesc& c, const void* d_cube, void* d_meta) {
     c.cell_mm = (float2*)(m + ml.cell_mm);
     c.cell_bits = (unsigned*)(m + ml.cell_bits);
     c.brick_active = (int*)(m + ml.brick_active);
+    c.occ = (unsigned*)(m + ml.occ);
 }
 
 int finish_cube(vr_ctx* ctx, cudaStream_t s) {
@@ -114,7 +120,7 @@ int finish_cube(vr_ctx* ctx, cudaStream_t s) {
     VR_CUDA(ctx, cudaMemcpyAsync(ctx->h_brick_mm.data(), c.brick_mm, sizeof(float2) * c.nbricks, cudaMemcpyDeviceToHost, s));
     VR_CUDA(ctx, cudaStreamSynchronize(s));
     ctx->has_cube = true;
-    ctx->activity_dirty = true;
+    ctx->activity_dirty = true; ctx->key_valid = false; ctx->occ_valid = false;
     return VR_OK;
 }
 
@@ -153,23 +159,30 @@ int ensure_tables(vr_ctx* ctx, cudaStream_t s) {
         ctx->activity_dirty = true;
     }
     if (ctx->activity_dirty && ctx->has_cube) {
-        const int nb = ctx->cube.nbricks;
-        ctx->h_brick_active.resize(nb);
-        for (int b = 0; b < nb; ++b)
-            ctx->h_brick_active[b] = range_active(ctx, ctx->h_brick_mm[b].x, ctx->h_brick_mm[b].y) ? 1 : 0;
-        // pageable source: cudaMemcpyAsync stages it before returning, so the vector may change later
-        VR_CUDA(ctx, cudaMemcpyAsync(ctx->cube.brick_active, ctx->h_brick_active.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, s));
-        // the same test per 8^3 macro-cell, on the device (one bit per cell)
         int nz[257];
         nz[0] = 0;
         for (int j = 0; j < 256; ++j) nz[j + 1] = nz[j] + (ctx->tf_baked[4 * j + 3] != 0.f ? 1 : 0);
-        VR_CUDA(ctx, cudaMemsetAsync(ctx->d_scratch, 0, sizeof(unsigned long long), s));
-        VR_CUDA(ctx, launch_classify_cells(ctx->cube, nz, ctx->vmin, ctx->scale, ctx->d_scratch, s));
-        ctx->launches += 1;
-        unsigned long long n_active = 0;
-        VR_CUDA(ctx, cudaMemcpyAsync(&n_active, ctx->d_scratch, sizeof(n_active), cudaMemcpyDeviceToHost, s));
-        VR_CUDA(ctx, cudaStreamSynchronize(s));
-        ctx->active_cell_fraction = (double)n_active / std::max(1.0, (double)ctx->cube.nbricks * ctx->cube.cells_per_brick);
+        const bool same = ctx->key_valid && ctx->key_vmin == ctx->vmin && ctx->key_scale == ctx->scale &&
+                          std::memcmp(nz, ctx->key_nz, sizeof(nz)) == 0;
+        if (!same) {                                        // else: colours / opacities changed, not what is transparent
+            const int nb = ctx->cube.nbricks;
+            ctx->h_brick_active.resize(nb);
+            for (int b = 0; b < nb; ++b)
+                ctx->h_brick_active[b] = range_active(ctx, ctx->h_brick_mm[b].x, ctx->h_brick_mm[b].y) ? 1 : 0;
+            // pageable source: cudaMemcpyAsync stages it before returning, so the vector may change later
+            VR_CUDA(ctx, cudaMemcpyAsync(ctx->cube.brick_active, ctx->h_brick_active.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, s));
+            // the same test per 8^3 macro-cell, on the device (one bit per cell)
+            VR_CUDA(ctx, cudaMemsetAsync(ctx->d_scratch, 0, sizeof(unsigned long long), s));
+            VR_CUDA(ctx, launch_classify_cells(ctx->cube, nz, ctx->vmin, ctx->scale, ctx->d_scratch, s));
+            ctx->launches += 1;
+            unsigned long long n_active = 0;
+            VR_CUDA(ctx, cudaMemcpyAsync(&n_active, ctx->d_scratch, sizeof(n_active), cudaMemcpyDeviceToHost, s));
+            VR_CUDA(ctx, cudaStreamSynchronize(s));
+            ctx->active_cell_fraction = (double)n_active / std::max(1.0, (double)ctx->cube.nbricks * ctx->cube.cells_per_brick);
+            std::memcpy(ctx->key_nz, nz, sizeof(nz));
+            ctx->key_vmin = ctx->vmin; ctx->key_scale = ctx->scale;
+            ctx->key_valid = true; ctx->occ_valid = false;
+        }
         // samples with table coordinate x < x_clear interpolate two entries of zero opacity
         int i0 = -1;
         while (i0 + 1 < 256 && ctx->tf_baked[4 * (i0 + 1) + 3] == 0.f) ++i0;
@@ -208,14 +221,28 @@ int resolve_variant(const vr_ctx* ctx) {
     return ray_spacing(ctx) >= kSparseRaySpacing ? 3 : 0;
 }
 
-// Skipping level: 0 none, 1 configured bricks, 2 bricks and 8^3 macro-cells.  The macro-cell level
-// costs a lookup per run / sample, so by default emission-absorption uses it only if the current
-// table leaves a fair share of the cells idle, and MIP only in the lockstep marcher (measured).
+int resolve_dense(const vr_ctx* ctx);
+
+// Skipping level: 0 none, 1 configured bricks, 2 + 8^3 macro-cells, 3 + occupancy bits per trilinear
+// cell.  The macro-cell level costs a lookup per run / sample, so by default emission-absorption uses
+// it only if the current table leaves a fair share of the cells idle, and MIP only in the lockstep
+// marcher (measured).  Level 3 is the lockstep marcher's for sparse tables on the micro-block layout.
 int skip_level(const vr_ctx* ctx, int mode) {
     if (!ctx->opt_skip) return 0;
-    if (ctx->opt_cell_skip >= 0) return ctx->opt_cell_skip ? 2 : 1;
+    if (ctx->opt_cell_skip == 0) return 1;
+    if (mode == VR_MODE_EA && ctx->opt_occ != 0 && ctx->cube.layout == 1 && resolve_variant(ctx) == 3 && !resolve_dense(ctx)) return 3;
+    if (ctx->opt_cell_skip > 0) return 2;
     if (mode == VR_MODE_MIP) return resolve_variant(ctx) == 3 ? 2 : 1;
     return ctx->active_cell_fraction < kCellSkipMaxActive ? 2 : 1;
+}
+
+// Occupancy bits are classified when a render first needs them for the current table.
+int ensure_occ(vr_ctx* ctx, int skip, cudaStream_t s) {
+    if (skip < 3 || ctx->occ_valid) return VR_OK;
+    VR_CUDA(ctx, launch_classify_occ(ctx->cube, ctx->key_nz, ctx->key_vmin, ctx->key_scale, s));
+    ctx->launches += 1;
+    ctx->occ_valid = true;
+    return VR_OK;
 }
 
 // Lockstep emission-absorption: fold through shared memory with all rays in parallel (dense) or
@@ -332,6 +359,7 @@ void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz,
     c.nbricks = c.G[0] * c.G[1] * c.G[2];
     c.cells_per_brick = c.C[0] * c.C[1] * c.C[2];
     c.cell_words_per_brick = (c.cells_per_brick + 31) / 32;
+    c.occ_words_per_brick = 32 * c.C[0] * c.C[1] * ((c.C[2] + 1) / 2);
     c.stride = layout == 0 ? (long long)align_up((size_t)c.P[0] * c.P[1] * c.P[2], 32)
                            : 32LL * c.T[0] * c.T[1] * c.T[2];
 }
@@ -345,6 +373,7 @@ MetaLayout meta_layout(const CubeDesc& c) {
     m.cell_mm = off; off = align_up(off + sizeof(float2) * (size_t)c.nbricks * c.cells_per_brick, 256);
     m.cell_bits = off; off = align_up(off + sizeof(unsigned) * (size_t)c.nbricks * c.cell_words_per_brick, 256);
     m.brick_active = off; off = align_up(off + sizeof(int) * c.nbricks, 256);
+    m.occ = off; off = align_up(off + sizeof(unsigned) * (size_t)c.nbricks * c.occ_words_per_brick, 256);
     m.total = off;
     return m;
 }
@@ -416,7 +445,7 @@ int vr_attach_cube(vr_ctx* ctx, int nx, int ny, int nz, int bx, int by, int bz, 
     ctx->h_brick_mm.resize(ctx->cube.nbricks);
     VR_CUDA(ctx, cudaMemcpy(ctx->h_brick_mm.data(), ctx->cube.brick_mm, sizeof(float2) * ctx->cube.nbricks, cudaMemcpyDeviceToHost));
     ctx->has_cube = true;
-    ctx->activity_dirty = true;
+    ctx->activity_dirty = true; ctx->key_valid = false; ctx->occ_valid = false;
     return VR_OK;
 }
 
@@ -583,6 +612,7 @@ int vr_render_ea(vr_ctx* ctx, float* d_out, const float bg[4], float tau, void* 
     a.mode = VR_MODE_EA; a.tau = tau; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx); a.dense = resolve_dense(ctx);
     for (int i = 0; i < 4; ++i) a.bg[i] = bg[i];
     a.out = d_out; a.counters = ctx->d_counters;
+    if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
     VR_CUDA(ctx, launch_render_global(ctx->cube, ctx->view, tf_desc(ctx), a, s));
     ctx->launches += 1;
     return VR_OK;
@@ -663,6 +693,7 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
     RenderArgs a{};
     a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx); a.dense = resolve_dense(ctx);
     a.counters = ctx->d_counters;
+    if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
     VR_CUDA(ctx, launch_render_bricks(ctx->cube, ctx->view, tf_desc(ctx), a, ctx->d_partials, n, tiles, s));
     ctx->launches += (n > 0 && tiles > 0) ? 1 : 0;
     return VR_OK;
@@ -712,6 +743,7 @@ int vr_set_option(vr_ctx* ctx, int option, int value) {
         VR_CUDA(ctx, cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)value));
         return VR_OK;
     }
+    if (option == VR_OPT_OCCUPANCY) { ctx->opt_occ = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_DENSE) { ctx->opt_dense = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_VARIANT) {
         if (value != -1 && value != 0 && value != 3) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");

@@ -42,6 +42,13 @@ struct CubeDesc {
     unsigned* cell_bits;         // EA activity of macro-cells vs the transfer function, 1 bit each
     int* brick_active;           // EA activity of bricks vs the transfer function
     int cell_words_per_brick;
+    // Occupancy bits (layout 1 only): one bit per trilinear cell (lower corner (lx,ly,lz), l < B),
+    // set iff the value range of its 8 corners can touch a table entry of non-zero opacity (O-10 at
+    // the finest level).  One 32-bit word per 4 x 4 x 2 micro-block, bit = the voxel's slot inside
+    // the block; words ordered so that a 128-byte line covers 8 x 8 x 16 voxels:
+    //   word = 32 ((lx>>3) + C0 ((ly>>3) + C1 (lz>>4))) + ((lx>>2)&1) + 2 ((ly>>2)&1) + 4 ((lz>>1)&7)
+    unsigned* occ;
+    int occ_words_per_brick;     // 32 C0 C1 ceil(C2 / 2)
 };
 
 struct ViewDesc {
@@ -77,7 +84,7 @@ __host__ __device__ inline long long voxel_slot(const CubeDesc& c, int lx, int l
 size_t align_up(size_t v, size_t a);
 void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz, int layout);
 size_t cube_bytes(const CubeDesc& c);
-struct MetaLayout { size_t brick_mm, cell_mm, cell_bits, brick_active, total; };
+struct MetaLayout { size_t brick_mm, cell_mm, cell_bits, brick_active, occ, total; };
 MetaLayout meta_layout(const CubeDesc& c);
 
 // kernels' host launchers (vr_cube.cu / vr_march.cu / vr_composite.cu)
@@ -92,7 +99,7 @@ cudaError_t launch_generate(const CubeDesc& c, float* d_cube, const GenDev& g, c
 
 struct RenderArgs {
     int mode; float tau; float bg[4]; float miss;
-    int skip;              // 0: none; 1: configured bricks; 2: bricks and 8^3 macro-cells (O-10)
+    int skip;              // 0: none; 1: configured bricks; 2: + 8^3 macro-cells; 3: + occupancy bits (O-10)
     int variant;           // 0: one ray per thread; 3: lockstep (the lanes of a warp take one ray's samples)
     int dense;             // lockstep EA: fold through shared memory, all rays in parallel (see vr_march.cu)
     float* out; float* out_rgba; unsigned long long* counters;
@@ -104,6 +111,7 @@ cudaError_t launch_composite(const ViewDesc& v, int mode, const PartialDev* d_pa
                              const float bg[4], cudaStream_t s);
 cudaError_t launch_classify_cells(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale,
                                   unsigned long long* d_active_count, cudaStream_t s);
+cudaError_t launch_classify_occ(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale, cudaStream_t s);
 cudaError_t launch_upload_table(float4* d_dst, const float* h_src_1024, cudaStream_t s);
 
 }  // namespace vr

@@ -667,10 +667,275 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
     }
 }
 
+// ================================================================== variant 3 for sparse tables: test, compact, gather, fold
+// Same ownership as render_ls_kernel (a warp walks its 32 rays through chunks of 32 lattice
+// indices, the lanes taking the 32 samples of one ray at a time), but a sample is first TESTED
+// against the occupancy bits (CubeDesc::occ, O-10 at the level of one trilinear cell): only samples
+// whose 8 corners can reach a table entry of non-zero opacity are interpolated.  Per chunk:
+//   test   - for every ray in turn the lanes look up the bit of their sample (macro-cell bit first,
+//            then the occupancy word, requested one ray ahead); the survivors of all rays are
+//            appended to a list in shared memory (ray-major, lattice order inside a ray);
+//   gather - the list is taken 32 entries at a time, one entry per lane (full lanes however few
+//            samples survive): position and weights are recomputed (the same float32 operations),
+//            the 8 voxels come through the cp.async ring, the value goes to vals[list index];
+//   fold   - the lane that owns a ray folds its entries front to back (O-7, exact ERT).
+// When the list is nearly full the rays tested so far are gathered and folded before the test
+// goes on (dense tables use render_ls_kernel<..., DENSE> instead).  Frames are identical to the
+// other marchers': a skipped sample has weight exactly zero.
+constexpr int kListCap = 256;
+
+__device__ __forceinline__ unsigned occ_word_index(const CubeDesc& c, unsigned lx, unsigned ly, unsigned lz) {
+    return 32u * ((lx >> 3) + (unsigned)c.C[0] * ((ly >> 3) + (unsigned)c.C[1] * (lz >> 4))) +
+           ((lx >> 2) & 1u) + 2u * ((ly >> 2) & 1u) + 4u * ((lz >> 1) & 7u);
+}
+__device__ __forceinline__ unsigned occ_bit_index(unsigned lx, unsigned ly, unsigned lz) {      // = slot & 31, layout 1
+    return ((ly & 2u) << 3) + ((lz & 1u) << 3) + ((ly & 1u) << 2) + (lx & 3u);
+}
+
+template <bool GLOBAL>
+__global__ void __launch_bounds__(kThreads, 7)
+render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
+                  const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
+                  const PartialDev* __restrict__ parts, int n_parts) {
+    constexpr int MODE = VR_MODE_EA, LAYOUT = 1;
+    constexpr int kWarps = kThreads / 32;
+    __shared__ PartialDev part;
+    __shared__ float4 rays_all[kWarps][64];
+    __shared__ float stage_all[kWarps][kDepth * 256];
+    __shared__ float vals_all[kWarps][kListCap];
+    __shared__ unsigned short list_all[kWarps][kListCap];
+    __shared__ unsigned sbits[GLOBAL ? 1 : kBitsWords];
+    int fx, fy;
+    bool live;
+    if (GLOBAL) {
+        int tx, ty; tile_pixel(tx, ty);
+        fx = blockIdx.x * kTileW + tx; fy = blockIdx.y * kTileH + ty;
+        live = fx < V.W && fy < V.H;
+    } else {
+        int lx, ly;
+        live = locate_tile(parts, n_parts, part, lx, ly);
+        fx = lx; fy = ly;
+    }
+    int bid0 = 0, lo0[3] = {0, 0, 0};
+    if (!GLOBAL) {
+        bid0 = part.brick;
+        lo0[0] = (bid0 % c.G[0]) * c.B[0]; lo0[1] = ((bid0 / c.G[0]) % c.G[1]) * c.B[1]; lo0[2] = (bid0 / (c.G[0] * c.G[1])) * c.B[2];
+    }
+    const bool bits_shared = !GLOBAL && c.cell_words_per_brick <= kBitsWords;
+    if (bits_shared) {
+        for (int i = threadIdx.x; i < c.cell_words_per_brick; i += kThreads)
+            sbits[i] = __ldg(&c.cell_bits[(long long)bid0 * c.cell_words_per_brick + i]);
+        __syncthreads();
+    }
+    Ray r; r.k0 = 0; r.k1 = -1;
+    r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
+    if (live) setup_ray(V, c, GLOBAL ? fx : part.x0 + fx, GLOBAL ? fy : part.y0 + fy, r);
+    int ka = r.k0, kb = r.k1;
+    if (!GLOBAL) {
+        const int b[3] = {bid0 % c.G[0], (bid0 / c.G[0]) % c.G[1], bid0 / (c.G[0] * c.G[1])};
+        brick_interval(c, r, b, lo0, ka, kb);
+    }
+    const BrickRef br0 = brick_ref<LAYOUT>(c, bid0, lo0);
+    const unsigned* occ0 = c.occ + (long long)bid0 * c.occ_words_per_brick;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float* vals = vals_all[warp];
+    unsigned short* list = list_all[warp];
+    float4* rays = rays_all[warp];
+    const float* stage = stage_all[warp] + lane;
+    const unsigned stage_addr = (unsigned)__cvta_generic_to_shared(stage);
+    rays[2 * lane] = make_float4(r.o[0], r.o[1], r.o[2], r.d[0]);
+    rays[2 * lane + 1] = make_float4(r.d[1], r.d[2], __int_as_float(ka), __int_as_float(kb));
+    __syncwarp();
+    bool alive = ka <= kb, stopped = false;
+    int k_end = kb;
+    int K0 = alive ? ka : 0x7fffffff, K1 = alive ? kb : -1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        K0 = min(K0, __shfl_xor_sync(0xffffffffu, K0, o));
+        K1 = max(K1, __shfl_xor_sync(0xffffffffu, K1, o));
+    }
+    Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
+    unsigned n_taken = 0;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    struct Probe { unsigned word, bit; int rc; };           // this lane's sample of ray rc: occupancy word + bit
+    for (int kbase = K0; kbase <= K1; kbase += 32) {
+        if (!__ballot_sync(0xffffffffu, alive)) break;
+        const unsigned act = __ballot_sync(0xffffffffu, alive && ka <= kbase + 31 && kb >= kbase);
+        if (!act) continue;
+        const int k = kbase + lane;
+        const float t = __fmul_rn((float)k, r.step);        // O-3: t_k = k * Delta
+        unsigned rest = act;
+        // ---- test: request the occupancy word of this lane's sample of the next ray of the chunk
+        auto probe = [&](Probe& P) {
+            P.rc = -1; P.word = 0u; P.bit = 0u;
+            if (!rest) return;
+            const int rr = __ffs(rest) - 1;
+            rest &= rest - 1;
+            P.rc = rr;
+            const float4 ra = rays[2 * rr], rb = rays[2 * rr + 1];
+            if (k >= __float_as_int(rb.z) && k <= __float_as_int(rb.w)) {
+                float fl;
+                const int iv[3] = {floor_pos(__fmaf_rn(t, ra.w, ra.x), fl), floor_pos(__fmaf_rn(t, rb.x, ra.y), fl),
+                                   floor_pos(__fmaf_rn(t, rb.y, ra.z), fl)};
+                if (GLOBAL) {
+                    int b[3]; brick_of(c, iv, b);
+                    const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
+                    const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
+                    if (__ldg(&c.brick_active[bid]) != 0 && !cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], 0.f)) {
+                        const unsigned lx = (unsigned)(iv[0] - lo[0]), ly = (unsigned)(iv[1] - lo[1]), lz = (unsigned)(iv[2] - lo[2]);
+                        P.word = __ldg(c.occ + (long long)bid * c.occ_words_per_brick + occ_word_index(c, lx, ly, lz));
+                        P.bit = occ_bit_index(lx, ly, lz);
+                    }
+                } else {
+                    const unsigned lx = (unsigned)(iv[0] - lo0[0]), ly = (unsigned)(iv[1] - lo0[1]), lz = (unsigned)(iv[2] - lo0[2]);
+                    bool idle;
+                    if (bits_shared) {
+                        const unsigned cidx = (lx >> 3) + (unsigned)c.C[0] * ((ly >> 3) + (unsigned)c.C[1] * (lz >> 3));
+                        idle = ((sbits[cidx >> 5] >> (cidx & 31u)) & 1u) == 0u;
+                    } else idle = cell_idle<MODE>(c, bid0, lo0, iv[0], iv[1], iv[2], 0.f);
+                    if (!idle) {
+                        P.word = __ldg(occ0 + occ_word_index(c, lx, ly, lz));
+                        P.bit = occ_bit_index(lx, ly, lz);
+                    }
+                }
+            }
+        };
+        Probe cur;
+        probe(cur);
+        while (cur.rc >= 0) {                               // one batch: test until the list is nearly full
+            int total = 0, my_start = 0, my_cnt = 0;
+            while (cur.rc >= 0) {
+                Probe nxt;
+                const bool room = total + 64 <= kListCap;   // cur and nxt add at most 32 entries each
+                if (room) probe(nxt);
+                else { nxt.rc = -1; nxt.word = 0u; nxt.bit = 0u; }
+                const bool on = ((cur.word >> cur.bit) & 1u) != 0u;
+                const unsigned m = __ballot_sync(0xffffffffu, on);
+                if (on) list[total + __popc(m & lt_mask)] = (unsigned short)((cur.rc << 5) | lane);
+                if (lane == cur.rc) { my_start = total; my_cnt = __popc(m); }
+                total += __popc(m);
+                cur = nxt;
+            }
+            if (total) {
+                __syncwarp();
+                // ---- gather: one list entry per lane, 32 entries per step, through the cp.async ring
+                const int ngroups = (total + 31) >> 5;
+                auto issue = [&](Slot& S, const int g, const int s) {
+                    S.rc = g < ngroups ? g : -1; S.idle = true;
+                    S.w[0] = S.w[1] = S.w[2] = 0.f;
+                    const int idx = 32 * g + lane;
+                    if (g < ngroups && idx < total) {
+                        const unsigned e = list[idx];
+                        const int rr = (int)(e >> 5);
+                        const float tt = __fmul_rn((float)(kbase + (int)(e & 31u)), r.step);
+                        const float4 ra = rays[2 * rr], rb = rays[2 * rr + 1];
+                        float p[3], fl[3];
+                        p[0] = __fmaf_rn(tt, ra.w, ra.x); p[1] = __fmaf_rn(tt, rb.x, ra.y); p[2] = __fmaf_rn(tt, rb.y, ra.z);
+                        const int iv[3] = {floor_pos(p[0], fl[0]), floor_pos(p[1], fl[1]), floor_pos(p[2], fl[2])};
+                        S.w[0] = __fsub_rn(p[0], fl[0]); S.w[1] = __fsub_rn(p[1], fl[1]); S.w[2] = __fsub_rn(p[2], fl[2]);
+                        S.idle = false;
+                        if (GLOBAL) {
+                            int b[3]; brick_of(c, iv, b);
+                            const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
+                            const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
+                            gather8_async<LAYOUT>(brick_ref<LAYOUT>(c, bid, lo), iv[0], iv[1], iv[2], stage_addr + 1024u * s);
+                        } else gather8_async<LAYOUT>(br0, iv[0], iv[1], iv[2], stage_addr + 1024u * s);
+                    }
+                    cp_async_commit();
+                };
+                auto consume = [&](const Slot& S, const int s) {
+                    if (S.idle) return;
+                    const float* st = stage + 256 * s;
+                    float v[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) v[e] = st[32 * e];
+                    vals[32 * S.rc + lane] = trilinear(v, S.w[0], S.w[1], S.w[2]);
+                };
+                Slot slot[kDepth];
+                int gi = 0;
+#pragma unroll
+                for (int s = 0; s < kDepth - 1; ++s) issue(slot[s], gi++, s);
+                for (bool more = true; more;) {
+#pragma unroll
+                    for (int u = 0; u < kDepth; ++u) {
+                        issue(slot[(u + kDepth - 1) % kDepth], gi++, (u + kDepth - 1) % kDepth);
+                        cp_async_wait<kDepth - 1>();
+                        if (slot[u].rc < 0) { more = false; break; }
+                        consume(slot[u], u);
+                    }
+                }
+                __syncwarp();
+                // ---- fold: lane = ray, its entries front to back (O-7)
+                if (my_cnt) {
+                    int i = 0;
+                    while (i < my_cnt) {
+                        const bool stop = fold<MODE>(acc, vals[my_start + i], T.baked, T, A.tau);
+                        ++i;
+                        if (stop) { stopped = true; alive = false; k_end = kbase + (int)(list[my_start + i - 1] & 31u); break; }
+                    }
+                    n_taken += (unsigned)i;
+                }
+                __syncwarp();
+            }
+            if (cur.rc < 0 && rest) probe(cur);
+        }
+    }
+    if (live) {
+        if (GLOBAL) write_frame_pixel<MODE>(V, T, A, fx, fy, acc, r.k1 >= r.k0);
+        else reinterpret_cast<float4*>(part.data)[(long long)fy * part.pitch + fx] = make_float4(acc.C[0], acc.C[1], acc.C[2], acc.A);
+    }
+    if (A.counters) {
+        const unsigned long long nom = kb >= ka ? (unsigned long long)(kb - ka + 1) : 0ULL;
+        const unsigned long long reached = kb >= ka ? (unsigned long long)(k_end - ka + 1) : 0ULL;
+        if (GLOBAL) count(A.counters, kRays, nom ? 1 : 0);
+        count(A.counters, kNominal, nom);
+        count(A.counters, kTaken, n_taken);
+        count(A.counters, kVisited, nom ? 1 : 0);
+        count(A.counters, kSkipped, reached - n_taken);
+        count(A.counters, kTerminated, stopped ? 1 : 0);
+    }
+}
+
+// O-10 per transfer function at the level of one trilinear cell: one warp per occupancy word, lane =
+// the cell whose lower corner is the lane's voxel of the micro-block; the bit is set iff a table
+// entry that the value range of the cell's 8 corners can touch has non-zero opacity (same test and
+// same float32 operations as classify_cells_kernel; the interpolated value lies inside that range).
+struct NzPrefix { int v[257]; };
+__global__ void __launch_bounds__(256)
+classify_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ NzPrefix nz, float vmin, float scale) {
+    const long long n_words = (long long)c.nbricks * c.occ_words_per_brick;
+    const int lane = threadIdx.x & 31;
+    for (long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; w < n_words;
+         w += ((long long)gridDim.x * blockDim.x) >> 5) {
+        const int brick = (int)(w / c.occ_words_per_brick);
+        unsigned rem = (unsigned)(w % c.occ_words_per_brick);
+        const unsigned within = rem & 31u; rem >>= 5;
+        const unsigned gx = rem % (unsigned)c.C[0], gy = (rem / (unsigned)c.C[0]) % (unsigned)c.C[1], gz = rem / (unsigned)(c.C[0] * c.C[1]);
+        const unsigned bx = 2u * gx + (within & 1u), by = 2u * gy + ((within >> 1) & 1u), bz = 8u * gz + (within >> 2);
+        const int lx = (int)(4u * bx + (lane & 3)), ly = (int)(4u * by + 2u * (lane >> 4) + ((lane >> 2) & 1)), lz = (int)(2u * bz + ((lane >> 3) & 1));
+        const int bi[3] = {brick % c.G[0], (brick / c.G[0]) % c.G[1], brick / (c.G[0] * c.G[1])};
+        const int lo[3] = {bi[0] * c.B[0], bi[1] * c.B[1], bi[2] * c.B[2]};
+        bool active = false;
+        if (lx < c.B[0] && ly < c.B[1] && lz < c.B[2] && lo[0] + lx < c.N[0] && lo[1] + ly < c.N[1] && lo[2] + lz < c.N[2]) {
+            const BrickRef br = brick_ref<1>(c, brick, lo);
+            float v[8];
+            gather8<1>(br, lo[0] + lx, lo[1] + ly, lo[2] + lz, v);
+            float mn = v[0], mx = v[0];
+#pragma unroll
+            for (int e = 1; e < 8; ++e) { mn = fminf(mn, v[e]); mx = fmaxf(mx, v[e]); }
+            const float xa = fminf(fmaxf(__fmul_rn(__fsub_rn(mn, vmin), scale), 0.f), 255.f);
+            const float xb = fminf(fmaxf(__fmul_rn(__fsub_rn(mx, vmin), scale), 0.f), 255.f);
+            const int ia = max(0, min((int)floorf(xa), 255)), ib = max(0, min((int)ceilf(xb), 255));
+            active = nz.v[ib + 1] - nz.v[ia] > 0;
+        }
+        const unsigned bits = __ballot_sync(0xffffffffu, active);
+        if (lane == 0) c.occ[w] = bits;
+    }
+}
+
 // O-10 per transfer function: one bit per 8^3 macro-cell, set iff a table entry that the cell's
 // value range [min, max] (halo-inclusive) can touch has non-zero opacity.  `nz` is the running
 // count of entries with non-zero baked opacity, so the range test is one subtraction.
-struct NzPrefix { int v[257]; };
 __global__ void classify_cells_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ NzPrefix nz,
                                       float vmin, float scale, long long n_slots,
                                       unsigned long long* __restrict__ active_count) {
@@ -729,8 +994,14 @@ __global__ void upload_half_kernel(float4* dst, const __grid_constant__ HalfTabl
         }                                                                                                \
     } while (0)
 
+// the occupancy marcher serves sparse emission-absorption on the micro-block layout
+static bool use_occ_kernel(const CubeDesc& c, const RenderArgs& a) {
+    return a.variant == 3 && a.mode == VR_MODE_EA && a.skip >= 3 && !a.dense && c.layout == 1;
+}
+
 cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s) {
     dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
+    if (use_occ_kernel(c, a)) { render_occ_kernel<true><<<grid, kThreads, 0, s>>>(c, v, t, a, nullptr, 0); return cudaGetLastError(); }
     if (a.variant == 3) VR_DISPATCH_LS(true, grid, c, v, t, a, nullptr, 0);
     else VR_DISPATCH(render_global_kernel, grid, c, v, t, a);
     return cudaGetLastError();
@@ -739,8 +1010,16 @@ cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFD
 cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a,
                                  const PartialDev* d_partials, int n, int total_tiles, cudaStream_t s) {
     if (n == 0 || total_tiles == 0) return cudaSuccess;
+    if (use_occ_kernel(c, a)) { render_occ_kernel<false><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n); return cudaGetLastError(); }
     if (a.variant == 3) VR_DISPATCH_LS(false, total_tiles, c, v, t, a, d_partials, n);
     else VR_DISPATCH(render_bricks_kernel, total_tiles, c, v, t, a, d_partials, n);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_classify_occ(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale, cudaStream_t s) {
+    NzPrefix nz;
+    for (int i = 0; i < 257; ++i) nz.v[i] = nz_prefix[i];
+    classify_occ_kernel<<<148 * 8, 256, 0, s>>>(c, nz, vmin, scale);
     return cudaGetLastError();
 }
 

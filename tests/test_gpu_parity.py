@@ -26,9 +26,10 @@ def H():
 
 # Every test below runs once with the library's own choice of marcher variant and macro-cell
 # skipping ("auto") and once per forced variant (0: ray per thread; 3: lockstep ray per warp, folding
-# emission-absorption samples in the owning lane "v3s" or through shared memory "v3d"), with the
-# macro-cell level of the skipping forced on.
-@pytest.fixture(autouse=True, params=["auto", "v0", "v3s", "v3d"])
+# emission-absorption samples in the owning lane "v3s" or through shared memory "v3d", or testing
+# every sample against the occupancy bits first "v3o"), with the macro-cell level of the skipping
+# forced on.
+@pytest.fixture(autouse=True, params=["auto", "v0", "v3s", "v3d", "v3o"])
 def marcher(request, H):
     from paper_1012_2909_b200 import vr
     H.FORCED_OPTIONS.clear()
@@ -36,6 +37,7 @@ def marcher(request, H):
         H.FORCED_OPTIONS.update({vr.OPT_VARIANT: int(request.param[1]), vr.OPT_CELL_SKIP: 1})
         if request.param[2:]:
             H.FORCED_OPTIONS[vr.OPT_DENSE] = int(request.param[2] == "d")
+            H.FORCED_OPTIONS[vr.OPT_OCCUPANCY] = int(request.param[2] == "o")
     yield request.param
     H.FORCED_OPTIONS.clear()
 
