@@ -44,8 +44,8 @@ struct CubeDesc {
     int cell_words_per_brick;
     // Occupancy bits (layout 1 only): one bit per trilinear cell (lower corner (lx,ly,lz), l < B),
     // set iff the value range of its 8 corners can touch a table entry of non-zero opacity (O-10 at
-    // the finest level).  One 32-bit word per 4 x 4 x 2 micro-block, bit = the voxel's slot inside
-    // the block; words ordered so that a 128-byte line covers 8 x 8 x 16 voxels:
+    // the finest level).  One 32-bit word per 4 x 4 x 2 micro-block, bit = the voxel's place inside
+    // the block, (lx&3) + 4 (ly&3) + 16 (lz&1); words ordered so that a 128-byte line covers 8 x 8 x 16 voxels:
     //   word = 32 ((lx>>3) + C0 ((ly>>3) + C1 (lz>>4))) + ((lx>>2)&1) + 2 ((ly>>2)&1) + 4 ((lz>>1)&7)
     unsigned* occ;
     int occ_words_per_brick;     // 32 C0 C1 ceil(C2 / 2)

@@ -668,28 +668,30 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
 }
 
 // ================================================================== variant 3 for sparse tables: test, compact, gather, fold
-// Same ownership as render_ls_kernel (a warp walks its 32 rays through chunks of 32 lattice
-// indices, the lanes taking the 32 samples of one ray at a time), but a sample is first TESTED
-// against the occupancy bits (CubeDesc::occ, O-10 at the level of one trilinear cell): only samples
-// whose 8 corners can reach a table entry of non-zero opacity are interpolated.  Per chunk:
-//   test   - for every ray in turn the lanes look up the bit of their sample (macro-cell bit first,
-//            then the occupancy word, requested one ray ahead); the survivors of all rays are
-//            appended to a list in shared memory (ray-major, lattice order inside a ray);
-//   gather - the list is taken 32 entries at a time, one entry per lane (full lanes however few
-//            samples survive): position and weights are recomputed (the same float32 operations),
-//            the 8 voxels come through the cp.async ring, the value goes to vals[list index];
-//   fold   - the lane that owns a ray folds its entries front to back (O-7, exact ERT).
-// When the list is nearly full the rays tested so far are gathered and folded before the test
-// goes on (dense tables use render_ls_kernel<..., DENSE> instead).  Frames are identical to the
-// other marchers': a skipped sample has weight exactly zero.
+// Same ownership as render_ls_kernel (a warp walks its 32 rays together through chunks of 32
+// lattice indices), but a sample is first TESTED against the occupancy bits (CubeDesc::occ, O-10
+// at the level of one trilinear cell): only samples whose 8 corners can reach a table entry of
+// non-zero opacity are interpolated.  Per chunk:
+//   test   - lane = ray: every lane walks the 32 lattice indices of the chunk along ITS ray and
+//            looks up the bit of each sample (position and floor only; the occupancy word stays in
+//            a register while the ray stays in its 4 x 4 x 2 cells) -> one 32-bit mask per ray;
+//   list   - the survivors of all rays are written to a list in shared memory, ray-major, lattice
+//            order inside a ray (warp prefix sum of the masks' populations);
+//   gather - lane = list entry, 32 entries per step (full lanes however few samples survive):
+//            position and weights are recomputed (the same float32 operations), the 8 voxels come
+//            through the cp.async ring, the value goes to vals[list index];
+//   fold   - lane = ray: the owner folds its entries front to back (O-7, exact ERT).
+// A list longer than kListCap is taken in batches of whole rays (dense tables use
+// render_ls_kernel<..., DENSE> instead).  Frames are identical to the other marchers': a skipped
+// sample has weight exactly zero.
 constexpr int kListCap = 256;
 
 __device__ __forceinline__ unsigned occ_word_index(const CubeDesc& c, unsigned lx, unsigned ly, unsigned lz) {
     return 32u * ((lx >> 3) + (unsigned)c.C[0] * ((ly >> 3) + (unsigned)c.C[1] * (lz >> 4))) +
            ((lx >> 2) & 1u) + 2u * ((ly >> 2) & 1u) + 4u * ((lz >> 1) & 7u);
 }
-__device__ __forceinline__ unsigned occ_bit_index(unsigned lx, unsigned ly, unsigned lz) {      // = slot & 31, layout 1
-    return ((ly & 2u) << 3) + ((lz & 1u) << 3) + ((ly & 1u) << 2) + (lx & 3u);
+__device__ __forceinline__ unsigned occ_bit_index(unsigned lx, unsigned ly, unsigned lz) {
+    return (lx & 3u) + ((ly & 3u) << 2) + ((lz & 1u) << 4);
 }
 
 template <bool GLOBAL>
@@ -704,7 +706,6 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
     __shared__ float stage_all[kWarps][kDepth * 256];
     __shared__ float vals_all[kWarps][kListCap];
     __shared__ unsigned short list_all[kWarps][kListCap];
-    __shared__ unsigned sbits[GLOBAL ? 1 : kBitsWords];
     int fx, fy;
     bool live;
     if (GLOBAL) {
@@ -721,12 +722,6 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
         bid0 = part.brick;
         lo0[0] = (bid0 % c.G[0]) * c.B[0]; lo0[1] = ((bid0 / c.G[0]) % c.G[1]) * c.B[1]; lo0[2] = (bid0 / (c.G[0] * c.G[1])) * c.B[2];
     }
-    const bool bits_shared = !GLOBAL && c.cell_words_per_brick <= kBitsWords;
-    if (bits_shared) {
-        for (int i = threadIdx.x; i < c.cell_words_per_brick; i += kThreads)
-            sbits[i] = __ldg(&c.cell_bits[(long long)bid0 * c.cell_words_per_brick + i]);
-        __syncthreads();
-    }
     Ray r; r.k0 = 0; r.k1 = -1;
     r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
     if (live) setup_ray(V, c, GLOBAL ? fx : part.x0 + fx, GLOBAL ? fy : part.y0 + fy, r);
@@ -736,7 +731,6 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
         brick_interval(c, r, b, lo0, ka, kb);
     }
     const BrickRef br0 = brick_ref<LAYOUT>(c, bid0, lo0);
-    const unsigned* occ0 = c.occ + (long long)bid0 * c.occ_words_per_brick;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float* vals = vals_all[warp];
     unsigned short* list = list_all[warp];
@@ -756,128 +750,135 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
     }
     Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
     unsigned n_taken = 0;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    struct Probe { unsigned word, bit; int rc; };           // this lane's sample of ray rc: occupancy word + bit
+    // the occupancy word of a sample: index (whole cube) and bit; ~0u if the sample's brick is inactive
+    auto locate = [&](const float tk, unsigned& widx, unsigned& bit) {
+        float fl;
+        const int iv[3] = {floor_pos(__fmaf_rn(tk, r.d[0], r.o[0]), fl), floor_pos(__fmaf_rn(tk, r.d[1], r.o[1]), fl),
+                           floor_pos(__fmaf_rn(tk, r.d[2], r.o[2]), fl)};
+        unsigned lx, ly, lz, base;
+        if (GLOBAL) {
+            int b[3]; brick_of(c, iv, b);
+            const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
+            lx = (unsigned)(iv[0] - b[0] * c.B[0]); ly = (unsigned)(iv[1] - b[1] * c.B[1]); lz = (unsigned)(iv[2] - b[2] * c.B[2]);
+            base = (unsigned)bid * (unsigned)c.occ_words_per_brick;
+            if (__ldg(&c.brick_active[bid]) == 0) { widx = 0xffffffffu; bit = 0u; return; }
+        } else {
+            lx = (unsigned)(iv[0] - lo0[0]); ly = (unsigned)(iv[1] - lo0[1]); lz = (unsigned)(iv[2] - lo0[2]);
+            base = (unsigned)bid0 * (unsigned)c.occ_words_per_brick;
+        }
+        widx = base + occ_word_index(c, lx, ly, lz);
+        bit = occ_bit_index(lx, ly, lz);
+    };
     for (int kbase = K0; kbase <= K1; kbase += 32) {
         if (!__ballot_sync(0xffffffffu, alive)) break;
-        const unsigned act = __ballot_sync(0xffffffffu, alive && ka <= kbase + 31 && kb >= kbase);
+        const bool mine = alive && ka <= kbase + 31 && kb >= kbase;
+        const unsigned act = __ballot_sync(0xffffffffu, mine);
         if (!act) continue;
-        const int k = kbase + lane;
-        const float t = __fmul_rn((float)k, r.step);        // O-3: t_k = k * Delta
-        unsigned rest = act;
-        // ---- test: request the occupancy word of this lane's sample of the next ray of the chunk
-        auto probe = [&](Probe& P) {
-            P.rc = -1; P.word = 0u; P.bit = 0u;
-            if (!rest) return;
-            const int rr = __ffs(rest) - 1;
-            rest &= rest - 1;
-            P.rc = rr;
-            const float4 ra = rays[2 * rr], rb = rays[2 * rr + 1];
-            if (k >= __float_as_int(rb.z) && k <= __float_as_int(rb.w)) {
-                float fl;
-                const int iv[3] = {floor_pos(__fmaf_rn(t, ra.w, ra.x), fl), floor_pos(__fmaf_rn(t, rb.x, ra.y), fl),
-                                   floor_pos(__fmaf_rn(t, rb.y, ra.z), fl)};
-                if (GLOBAL) {
-                    int b[3]; brick_of(c, iv, b);
-                    const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
-                    const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
-                    if (__ldg(&c.brick_active[bid]) != 0 && !cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], 0.f)) {
-                        const unsigned lx = (unsigned)(iv[0] - lo[0]), ly = (unsigned)(iv[1] - lo[1]), lz = (unsigned)(iv[2] - lo[2]);
-                        P.word = __ldg(c.occ + (long long)bid * c.occ_words_per_brick + occ_word_index(c, lx, ly, lz));
-                        P.bit = occ_bit_index(lx, ly, lz);
-                    }
-                } else {
-                    const unsigned lx = (unsigned)(iv[0] - lo0[0]), ly = (unsigned)(iv[1] - lo0[1]), lz = (unsigned)(iv[2] - lo0[2]);
-                    bool idle;
-                    if (bits_shared) {
-                        const unsigned cidx = (lx >> 3) + (unsigned)c.C[0] * ((ly >> 3) + (unsigned)c.C[1] * (lz >> 3));
-                        idle = ((sbits[cidx >> 5] >> (cidx & 31u)) & 1u) == 0u;
-                    } else idle = cell_idle<MODE>(c, bid0, lo0, iv[0], iv[1], iv[2], 0.f);
-                    if (!idle) {
-                        P.word = __ldg(occ0 + occ_word_index(c, lx, ly, lz));
-                        P.bit = occ_bit_index(lx, ly, lz);
-                    }
+        // ---- test, lane = ray: bit j of my_act <=> sample kbase + j of this lane's ray survives.  The
+        // occupancy word stays in a register while the ray stays inside its 4 x 4 x 2 cells, and the
+        // word of the next sample is requested before the current one is tested.
+        unsigned my_act = 0u;
+        {
+            int j0 = mine ? max(ka, kbase) - kbase : 32, j1 = mine ? min(kb, kbase + 31) - kbase : -1;
+            int J0 = j0, J1 = j1;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                J0 = min(J0, __shfl_xor_sync(0xffffffffu, J0, o));
+                J1 = max(J1, __shfl_xor_sync(0xffffffffu, J1, o));
+            }
+            unsigned widx = 0xffffffffu, word = 0u, bit = 0u;        // of sample j
+            if (J0 >= j0 && J0 <= j1) {
+                locate(__fmul_rn((float)(kbase + J0), r.step), widx, bit);
+                if (widx != 0xffffffffu) word = __ldg(c.occ + widx);
+            }
+            for (int j = J0; j <= J1; ++j) {
+                unsigned nidx = 0xffffffffu, nword = 0u, nbit = 0u;  // of sample j + 1
+                if (j + 1 >= j0 && j + 1 <= j1) {
+                    locate(__fmul_rn((float)(kbase + j + 1), r.step), nidx, nbit);
+                    nword = nidx == widx ? word : (nidx != 0xffffffffu ? __ldg(c.occ + nidx) : 0u);
+                }
+                if (j >= j0 && j <= j1 && ((word >> bit) & 1u)) my_act |= 1u << j;
+                widx = nidx; word = nword; bit = nbit;
+            }
+        }
+        // ---- list, ray-major: lane's entries at [off, off + cnt)
+        const int cnt = __popc(my_act);
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int up = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += up;
+        }
+        const int off = incl - cnt, total = __shfl_sync(0xffffffffu, incl, 31);
+        for (int base = 0; base < total;) {                 // batches of whole rays, at most kListCap entries
+            const bool inb = cnt > 0 && off >= base && off + cnt <= base + kListCap;
+            const unsigned bm = __ballot_sync(0xffffffffu, inb);
+            const int bend = __shfl_sync(0xffffffffu, off + cnt, 31 - __clz((int)bm));
+            const int ntot = bend - base, my_start = off - base;
+            if (inb) {
+                int i = my_start;
+                for (unsigned bits = my_act; bits; bits &= bits - 1) list[i++] = (unsigned short)((lane << 5) | (__ffs(bits) - 1));
+            }
+            __syncwarp();
+            // ---- gather: one list entry per lane, 32 entries per step, through the cp.async ring
+            const int ngroups = (ntot + 31) >> 5;
+            auto issue = [&](Slot& S, const int g, const int s) {
+                S.rc = g < ngroups ? g : -1; S.idle = true;
+                S.w[0] = S.w[1] = S.w[2] = 0.f;
+                const int idx = 32 * g + lane;
+                if (g < ngroups && idx < ntot) {
+                    const unsigned e = list[idx];
+                    const int rr = (int)(e >> 5);
+                    const float tt = __fmul_rn((float)(kbase + (int)(e & 31u)), r.step);
+                    const float4 ra = rays[2 * rr], rb = rays[2 * rr + 1];
+                    float p[3], fl[3];
+                    p[0] = __fmaf_rn(tt, ra.w, ra.x); p[1] = __fmaf_rn(tt, rb.x, ra.y); p[2] = __fmaf_rn(tt, rb.y, ra.z);
+                    const int iv[3] = {floor_pos(p[0], fl[0]), floor_pos(p[1], fl[1]), floor_pos(p[2], fl[2])};
+                    S.w[0] = __fsub_rn(p[0], fl[0]); S.w[1] = __fsub_rn(p[1], fl[1]); S.w[2] = __fsub_rn(p[2], fl[2]);
+                    S.idle = false;
+                    if (GLOBAL) {
+                        int b[3]; brick_of(c, iv, b);
+                        const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
+                        const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
+                        gather8_async<LAYOUT>(brick_ref<LAYOUT>(c, bid, lo), iv[0], iv[1], iv[2], stage_addr + 1024u * s);
+                    } else gather8_async<LAYOUT>(br0, iv[0], iv[1], iv[2], stage_addr + 1024u * s);
+                }
+                cp_async_commit();
+            };
+            auto consume = [&](const Slot& S, const int s) {
+                if (S.idle) return;
+                const float* st = stage + 256 * s;
+                float v[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) v[e] = st[32 * e];
+                vals[32 * S.rc + lane] = trilinear(v, S.w[0], S.w[1], S.w[2]);
+            };
+            Slot slot[kDepth];
+            int gi = 0;
+#pragma unroll
+            for (int s = 0; s < kDepth - 1; ++s) issue(slot[s], gi++, s);
+            for (bool more = true; more;) {
+#pragma unroll
+                for (int u = 0; u < kDepth; ++u) {
+                    issue(slot[(u + kDepth - 1) % kDepth], gi++, (u + kDepth - 1) % kDepth);
+                    cp_async_wait<kDepth - 1>();
+                    if (slot[u].rc < 0) { more = false; break; }
+                    consume(slot[u], u);
                 }
             }
-        };
-        Probe cur;
-        probe(cur);
-        while (cur.rc >= 0) {                               // one batch: test until the list is nearly full
-            int total = 0, my_start = 0, my_cnt = 0;
-            while (cur.rc >= 0) {
-                Probe nxt;
-                const bool room = total + 64 <= kListCap;   // cur and nxt add at most 32 entries each
-                if (room) probe(nxt);
-                else { nxt.rc = -1; nxt.word = 0u; nxt.bit = 0u; }
-                const bool on = ((cur.word >> cur.bit) & 1u) != 0u;
-                const unsigned m = __ballot_sync(0xffffffffu, on);
-                if (on) list[total + __popc(m & lt_mask)] = (unsigned short)((cur.rc << 5) | lane);
-                if (lane == cur.rc) { my_start = total; my_cnt = __popc(m); }
-                total += __popc(m);
-                cur = nxt;
-            }
-            if (total) {
-                __syncwarp();
-                // ---- gather: one list entry per lane, 32 entries per step, through the cp.async ring
-                const int ngroups = (total + 31) >> 5;
-                auto issue = [&](Slot& S, const int g, const int s) {
-                    S.rc = g < ngroups ? g : -1; S.idle = true;
-                    S.w[0] = S.w[1] = S.w[2] = 0.f;
-                    const int idx = 32 * g + lane;
-                    if (g < ngroups && idx < total) {
-                        const unsigned e = list[idx];
-                        const int rr = (int)(e >> 5);
-                        const float tt = __fmul_rn((float)(kbase + (int)(e & 31u)), r.step);
-                        const float4 ra = rays[2 * rr], rb = rays[2 * rr + 1];
-                        float p[3], fl[3];
-                        p[0] = __fmaf_rn(tt, ra.w, ra.x); p[1] = __fmaf_rn(tt, rb.x, ra.y); p[2] = __fmaf_rn(tt, rb.y, ra.z);
-                        const int iv[3] = {floor_pos(p[0], fl[0]), floor_pos(p[1], fl[1]), floor_pos(p[2], fl[2])};
-                        S.w[0] = __fsub_rn(p[0], fl[0]); S.w[1] = __fsub_rn(p[1], fl[1]); S.w[2] = __fsub_rn(p[2], fl[2]);
-                        S.idle = false;
-                        if (GLOBAL) {
-                            int b[3]; brick_of(c, iv, b);
-                            const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
-                            const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
-                            gather8_async<LAYOUT>(brick_ref<LAYOUT>(c, bid, lo), iv[0], iv[1], iv[2], stage_addr + 1024u * s);
-                        } else gather8_async<LAYOUT>(br0, iv[0], iv[1], iv[2], stage_addr + 1024u * s);
-                    }
-                    cp_async_commit();
-                };
-                auto consume = [&](const Slot& S, const int s) {
-                    if (S.idle) return;
-                    const float* st = stage + 256 * s;
-                    float v[8];
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) v[e] = st[32 * e];
-                    vals[32 * S.rc + lane] = trilinear(v, S.w[0], S.w[1], S.w[2]);
-                };
-                Slot slot[kDepth];
-                int gi = 0;
-#pragma unroll
-                for (int s = 0; s < kDepth - 1; ++s) issue(slot[s], gi++, s);
-                for (bool more = true; more;) {
-#pragma unroll
-                    for (int u = 0; u < kDepth; ++u) {
-                        issue(slot[(u + kDepth - 1) % kDepth], gi++, (u + kDepth - 1) % kDepth);
-                        cp_async_wait<kDepth - 1>();
-                        if (slot[u].rc < 0) { more = false; break; }
-                        consume(slot[u], u);
-                    }
+            __syncwarp();
+            // ---- fold: lane = ray, its entries front to back (O-7)
+            if (inb) {
+                int i = 0;
+                while (i < cnt) {
+                    const bool stop = fold<MODE>(acc, vals[my_start + i], T.baked, T, A.tau);
+                    ++i;
+                    if (stop) { stopped = true; alive = false; k_end = kbase + (int)(list[my_start + i - 1] & 31u); break; }
                 }
-                __syncwarp();
-                // ---- fold: lane = ray, its entries front to back (O-7)
-                if (my_cnt) {
-                    int i = 0;
-                    while (i < my_cnt) {
-                        const bool stop = fold<MODE>(acc, vals[my_start + i], T.baked, T, A.tau);
-                        ++i;
-                        if (stop) { stopped = true; alive = false; k_end = kbase + (int)(list[my_start + i - 1] & 31u); break; }
-                    }
-                    n_taken += (unsigned)i;
-                }
-                __syncwarp();
+                n_taken += (unsigned)i;
             }
-            if (cur.rc < 0 && rest) probe(cur);
+            __syncwarp();
+            base = bend;
         }
     }
     if (live) {
@@ -900,36 +901,43 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
 // the cell whose lower corner is the lane's voxel of the micro-block; the bit is set iff a table
 // entry that the value range of the cell's 8 corners can touch has non-zero opacity (same test and
 // same float32 operations as classify_cells_kernel; the interpolated value lies inside that range).
+// The 8 warps of a CTA take 4 x 2 micro-blocks in (y, z) and walk along x, so that the lines of
+// the +1 neighbours are found in L1.
 struct NzPrefix { int v[257]; };
 __global__ void __launch_bounds__(256)
 classify_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ NzPrefix nz, float vmin, float scale) {
-    const long long n_words = (long long)c.nbricks * c.occ_words_per_brick;
-    const int lane = threadIdx.x & 31;
-    for (long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; w < n_words;
-         w += ((long long)gridDim.x * blockDim.x) >> 5) {
-        const int brick = (int)(w / c.occ_words_per_brick);
-        unsigned rem = (unsigned)(w % c.occ_words_per_brick);
-        const unsigned within = rem & 31u; rem >>= 5;
-        const unsigned gx = rem % (unsigned)c.C[0], gy = (rem / (unsigned)c.C[0]) % (unsigned)c.C[1], gz = rem / (unsigned)(c.C[0] * c.C[1]);
-        const unsigned bx = 2u * gx + (within & 1u), by = 2u * gy + ((within >> 1) & 1u), bz = 8u * gz + (within >> 2);
-        const int lx = (int)(4u * bx + (lane & 3)), ly = (int)(4u * by + 2u * (lane >> 4) + ((lane >> 2) & 1)), lz = (int)(2u * bz + ((lane >> 3) & 1));
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int nbx = (c.B[0] + 3) >> 2, nby = (c.B[1] + 3) >> 2, nbz = (c.B[2] + 1) >> 1;   // micro-blocks holding lower corners
+    const int ngy = (nby + 3) >> 2, ngz = (nbz + 1) >> 1;
+    const long long n_units = (long long)c.nbricks * ngy * ngz;
+    for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
+        const int brick = (int)(u / (ngy * ngz));
+        const int rem = (int)(u % (ngy * ngz));
+        const int by = 4 * (rem % ngy) + (warp & 3), bz = 2 * (rem / ngy) + (warp >> 2);
+        if (by >= nby || bz >= nbz) continue;
         const int bi[3] = {brick % c.G[0], (brick / c.G[0]) % c.G[1], brick / (c.G[0] * c.G[1])};
         const int lo[3] = {bi[0] * c.B[0], bi[1] * c.B[1], bi[2] * c.B[2]};
-        bool active = false;
-        if (lx < c.B[0] && ly < c.B[1] && lz < c.B[2] && lo[0] + lx < c.N[0] && lo[1] + ly < c.N[1] && lo[2] + lz < c.N[2]) {
-            const BrickRef br = brick_ref<1>(c, brick, lo);
-            float v[8];
-            gather8<1>(br, lo[0] + lx, lo[1] + ly, lo[2] + lz, v);
-            float mn = v[0], mx = v[0];
+        const BrickRef br = brick_ref<1>(c, brick, lo);
+        unsigned* occ = c.occ + (long long)brick * c.occ_words_per_brick;
+        const int ly = 4 * by + ((lane >> 2) & 3), lz = 2 * bz + (lane >> 4);        // lane = occ_bit_index
+        const bool row_ok = ly < c.B[1] && lz < c.B[2] && lo[1] + ly < c.N[1] && lo[2] + lz < c.N[2];
+        for (int bx = 0; bx < nbx; ++bx) {
+            const int lx = 4 * bx + (lane & 3);
+            bool active = false;
+            if (row_ok && lx < c.B[0] && lo[0] + lx < c.N[0]) {
+                float v[8];
+                gather8<1>(br, lo[0] + lx, lo[1] + ly, lo[2] + lz, v);
+                float mn = v[0], mx = v[0];
 #pragma unroll
-            for (int e = 1; e < 8; ++e) { mn = fminf(mn, v[e]); mx = fmaxf(mx, v[e]); }
-            const float xa = fminf(fmaxf(__fmul_rn(__fsub_rn(mn, vmin), scale), 0.f), 255.f);
-            const float xb = fminf(fmaxf(__fmul_rn(__fsub_rn(mx, vmin), scale), 0.f), 255.f);
-            const int ia = max(0, min((int)floorf(xa), 255)), ib = max(0, min((int)ceilf(xb), 255));
-            active = nz.v[ib + 1] - nz.v[ia] > 0;
+                for (int e = 1; e < 8; ++e) { mn = fminf(mn, v[e]); mx = fmaxf(mx, v[e]); }
+                const float xa = fminf(fmaxf(__fmul_rn(__fsub_rn(mn, vmin), scale), 0.f), 255.f);
+                const float xb = fminf(fmaxf(__fmul_rn(__fsub_rn(mx, vmin), scale), 0.f), 255.f);
+                const int ia = max(0, min((int)floorf(xa), 255)), ib = max(0, min((int)ceilf(xb), 255));
+                active = nz.v[ib + 1] - nz.v[ia] > 0;
+            }
+            const unsigned bits = __ballot_sync(0xffffffffu, active);
+            if (lane == 0) occ[occ_word_index(c, 4u * bx, 4u * by, 2u * bz)] = bits;
         }
-        const unsigned bits = __ballot_sync(0xffffffffu, active);
-        if (lane == 0) c.occ[w] = bits;
     }
 }
 
@@ -1019,7 +1027,7 @@ cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFD
 cudaError_t launch_classify_occ(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale, cudaStream_t s) {
     NzPrefix nz;
     for (int i = 0; i < 257; ++i) nz.v[i] = nz_prefix[i];
-    classify_occ_kernel<<<148 * 8, 256, 0, s>>>(c, nz, vmin, scale);
+    classify_occ_kernel<<<148 * 8, 256, 0, s>>>(c, nz, vmin, scale);   // words of the padding beyond the brick are never read
     return cudaGetLastError();
 }
 
