@@ -226,11 +226,13 @@ int resolve_dense(const vr_ctx* ctx);
 // Skipping level: 0 none, 1 configured bricks, 2 + 8^3 macro-cells, 3 + occupancy bits per trilinear
 // cell.  The macro-cell level costs a lookup per run / sample, so by default emission-absorption uses
 // it only if the current table leaves a fair share of the cells idle, and MIP only in the lockstep
-// marcher (measured).  Level 3 is the lockstep marcher's for sparse tables on the micro-block layout.
+// marcher (measured).  Level 3 serves emission-absorption with sparse tables on the micro-block layout
+// (in the lockstep marcher: the test-compact-gather-fold kernel; ray per thread: a bit test per sample
+// inside active macro-cells).
 int skip_level(const vr_ctx* ctx, int mode) {
     if (!ctx->opt_skip) return 0;
     if (ctx->opt_cell_skip == 0) return 1;
-    if (mode == VR_MODE_EA && ctx->opt_occ != 0 && ctx->cube.layout == 1 && resolve_variant(ctx) == 3 && !resolve_dense(ctx)) return 3;
+    if (mode == VR_MODE_EA && ctx->opt_occ != 0 && ctx->cube.layout == 1 && !resolve_dense(ctx)) return 3;
     if (ctx->opt_cell_skip > 0) return 2;
     if (mode == VR_MODE_MIP) return resolve_variant(ctx) == 3 ? 2 : 1;
     return ctx->active_cell_fraction < kCellSkipMaxActive ? 2 : 1;

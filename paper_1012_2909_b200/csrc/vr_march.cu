@@ -285,6 +285,14 @@ __device__ __forceinline__ bool cell_idle(const CubeDesc& c, int bid, const int 
     return ((__ldg(&c.cell_bits[(long long)bid * c.cell_words_per_brick + (cidx >> 5)]) >> (cidx & 31)) & 1u) == 0u;
 }
 
+__device__ __forceinline__ unsigned occ_word_index(const CubeDesc& c, unsigned lx, unsigned ly, unsigned lz) {
+    return 32u * ((lx >> 3) + (unsigned)c.C[0] * ((ly >> 3) + (unsigned)c.C[1] * (lz >> 4))) +
+           ((lx >> 2) & 1u) + 2u * ((ly >> 2) & 1u) + 4u * ((lz >> 1) & 7u);
+}
+__device__ __forceinline__ unsigned occ_bit_index(unsigned lx, unsigned ly, unsigned lz) {
+    return (lx & 3u) + ((ly & 3u) << 2) + ((lz & 1u) << 4);
+}
+
 struct Stats { unsigned long long taken, visit, skip; };
 
 // ================================================================== variant 0: one ray per thread
@@ -296,6 +304,7 @@ __device__ __forceinline__ bool march_interval(const CubeDesc& c, const Ray& r, 
                                                const float4* tab, int bid, const int lo[3], int k, int ke,
                                                Accum& acc, Stats& st) {
     const BrickRef b = brick_ref<LAYOUT>(c, bid, lo);
+    const unsigned* occ = (MODE == VR_MODE_EA && LAYOUT == 1 && A.skip >= 3) ? c.occ + (long long)bid * c.occ_words_per_brick : nullptr;
     const int S8[3] = {kCell, kCell, kCell};
     float kf = (float)k;                                    // exact: k < 2^24
     while (k <= ke) {
@@ -313,6 +322,12 @@ __device__ __forceinline__ bool march_interval(const CubeDesc& c, const Ray& r, 
         for (const int e = k + n; k < e; ++k, kf = __fadd_rn(kf, 1.f)) {
             float p[3];
             position(r, kf, p);
+            if (occ) {                                      // O-10 per trilinear cell: the sample's occupancy bit
+                float fl;
+                const unsigned lx = (unsigned)(floor_pos(p[0], fl) - lo[0]), ly = (unsigned)(floor_pos(p[1], fl) - lo[1]),
+                               lz = (unsigned)(floor_pos(p[2], fl) - lo[2]);
+                if (((__ldg(occ + occ_word_index(c, lx, ly, lz)) >> occ_bit_index(lx, ly, lz)) & 1u) == 0u) continue;
+            }
             const float v = sample<LAYOUT>(b, p);
             ++st.taken;
             if (fold<MODE>(acc, v, tab, T, A.tau)) return true;
@@ -686,14 +701,6 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
 // sample has weight exactly zero.
 constexpr int kListCap = 256;
 
-__device__ __forceinline__ unsigned occ_word_index(const CubeDesc& c, unsigned lx, unsigned ly, unsigned lz) {
-    return 32u * ((lx >> 3) + (unsigned)c.C[0] * ((ly >> 3) + (unsigned)c.C[1] * (lz >> 4))) +
-           ((lx >> 2) & 1u) + 2u * ((ly >> 2) & 1u) + 4u * ((lz >> 1) & 7u);
-}
-__device__ __forceinline__ unsigned occ_bit_index(unsigned lx, unsigned ly, unsigned lz) {
-    return (lx & 3u) + ((ly & 3u) << 2) + ((lz & 1u) << 4);
-}
-
 // 8 CTAs per SM (64 registers): the few gathers leave L1 alone, more warps hide the bit lookups (measured:
 // 7 -> 6.83, 8 -> 6.44, 9 -> 7.27 ms on C3)
 template <bool GLOBAL>
@@ -1006,7 +1013,7 @@ __global__ void upload_half_kernel(float4* dst, const __grid_constant__ HalfTabl
 
 // the occupancy marcher serves sparse emission-absorption on the micro-block layout
 static bool use_occ_kernel(const CubeDesc& c, const RenderArgs& a) {
-    return a.variant == 3 && a.mode == VR_MODE_EA && a.skip >= 3 && !a.dense && c.layout == 1;
+    return a.variant == 3 && a.mode == VR_MODE_EA && a.skip >= 3 && c.layout == 1;
 }
 
 cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s) {
