@@ -29,6 +29,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 from paper_1012_2909_b200 import workloads as wl  # noqa: E402
+from paper_1012_2909_b200.replicas import orbit_frame as _orbit_frame, reduce_run  # noqa: E402
 
 METRIC = "ray samples/s (nominal lattice samples inside the cube; BASELINE.json metric)"
 
@@ -89,10 +90,18 @@ class ClockSampler(threading.Thread):
 
 
 def orbit_frame(w, step_index, n_steps, rank, world):
-    """Frame index of the 360-frame orbit rendered at a given step (evenly spread over the orbit;
-    ranks interleave)."""
-    total = max(1, n_steps * world)
-    return int(round((step_index * world + rank) * 360.0 / total)) % 360
+    """Frame index of the 360-frame orbit rendered at a given step (paper_1012_2909_b200/replicas.py)."""
+    return _orbit_frame(step_index, n_steps, rank, world)
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the marcher, from the committed
+# `ncu --set full` captures (profiles/r1c_c3_render_occ_full.md: orbit frames 0 and 180, 10.28 and 7.26 GB; their mean).  None: not captured.
+NCU_TRAFFIC_BYTES = {"C3": 8.77e9}
+
+MARCHER = {(0, 0): "render_bricks_kernel<EA> (ray per thread)", (0, 1): "render_bricks_kernel<EA> (ray per thread)",
+           (0, 2): "render_bricks_kernel<EA> (ray per thread, macro-cell runs)",
+           (0, 3): "render_bricks_kernel<EA> (ray per thread, macro-cell runs + occupancy bits)",
+           (3, 3): "render_occ_kernel (lockstep: occupancy test, compaction, cp.async gather, fold)"}
 
 
 class Job:
@@ -249,14 +258,8 @@ def main():
     march_ms = sum(a.elapsed_time(b) for a, b in job.march_events)
     n_march = len(job.march_events)
 
-    nominal, taken, launches = cnt["nominal_samples"], cnt["taken_samples"], cnt["kernel_launches"]
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-        s = torch.tensor([nominal, taken, launches], dtype=torch.float64, device="cuda")
-        dist.all_reduce(s, op=dist.ReduceOp.SUM)
-        nominal, taken, launches = (int(v) for v in s.tolist())
+    ms_total, (nominal, taken, launches) = reduce_run(
+        dist, "cuda", ms_total, [cnt["nominal_samples"], cnt["taken_samples"], cnt["kernel_launches"]])
 
     # ---- e2e: the same step through the public API with HOST buffers in the timed region: the
     # view matrix and the transfer-function table go host -> device every step (as kernel
@@ -270,14 +273,7 @@ def main():
         torch.cuda.current_stream().synchronize()
     e2e_s = time.perf_counter() - t0
     cnt2 = job.ctx.get_counters()
-    e2e_nominal = cnt2["nominal_samples"]
-    if dist is not None:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-        s = torch.tensor([e2e_nominal], dtype=torch.float64, device="cuda")
-        dist.all_reduce(s, op=dist.ReduceOp.SUM)
-        e2e_nominal = int(s.item())
+    e2e_s, (e2e_nominal,) = reduce_run(dist, "cuda", e2e_s, [cnt2["nominal_samples"]])
 
     if rank != 0:
         if dist is not None:
@@ -286,6 +282,11 @@ def main():
 
     peaks, peak_src = measured_peaks()
     peak = float(peaks["hbm_gbs"])
+    plan = job.ctx.get_plan(vr.MODE_EA)
+    kernel = MARCHER.get((plan["variant"], plan["skip_level"]),
+                         "render_ls_kernel<EA> (lockstep, cp.async gather)" if plan["variant"] == 3 else "render_bricks_kernel<EA>")
+    traffic = NCU_TRAFFIC_BYTES.get(w.name)
+    launch_s = march_ms / max(n_march, 1) * 1e-3
     achieved = (job.alg_bytes / max(n_march, 1)) / (march_ms / max(n_march, 1) * 1e-3) / 1e9 if march_ms > 0 else 0.0
     cpu = None
     if world == 1:
@@ -314,11 +315,17 @@ def main():
         "e2e": {"value": e2e_nominal / e2e_s, "unit": "samples/s", "ms_per_step": e2e_s * 1e3 / args.steps,
                 "h2d_bytes_per_step": (64 + 4096 + 8) * job.cols * job.rows,
                 "d2h_bytes_per_step": job.H * job.W * 16},
-        "roofline": {"bound": "hbm", "kernel": "render_bricks_kernel<EA>", "achieved": achieved, "peak": peak,
-                     "unit": "GB/s", "frac": achieved / peak if peak else None, "traffic": None,
+        "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak,
+                     "unit": "GB/s", "frac": achieved / peak if peak else None, "traffic": traffic,
                      "peak_source": peak_src, "launch_ms": march_ms / max(n_march, 1),
                      "share_of_step": march_ms / ms_total if ms_total else None,
-                     "algorithmic_bytes_per_launch": job.alg_bytes / max(n_march, 1)},
+                     "algorithmic_bytes_per_launch": job.alg_bytes / max(n_march, 1),
+                     "dram_gbs_from_traffic": traffic / launch_s / 1e9 if traffic and launch_s > 0 else None,
+                     "plan": plan,
+                     "note": "algorithmic bytes = 4 B x voxels of the active in-frustum bricks at the configured brick "
+                             "size + partial images (SURVEY.md 8(d)); skipping below the brick level (macro-cells, "
+                             "occupancy bits) reads fewer bytes than that, so frac can exceed 1: `traffic` is what "
+                             "the launch really moved"},
         "cpu_baseline": cpu,
     }
     print(json.dumps(out))

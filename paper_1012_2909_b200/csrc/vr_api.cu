@@ -732,6 +732,15 @@ int vr_reset_counters(vr_ctx* ctx, void* stream) {
     return VR_OK;
 }
 
+int vr_get_plan(vr_ctx* ctx, int mode, int out[3], void* stream) {
+    int rc = check_render_state(ctx, mode == VR_MODE_EA);
+    if (rc) return rc;
+    if (!out || (mode != VR_MODE_MIP && mode != VR_MODE_EA)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_get_plan: bad argument");
+    if ((rc = ensure_tables(ctx, (cudaStream_t)stream))) return rc;
+    out[0] = resolve_variant(ctx); out[1] = skip_level(ctx, mode); out[2] = mode == VR_MODE_EA ? resolve_dense(ctx) : 0;
+    return VR_OK;
+}
+
 int vr_set_option(vr_ctx* ctx, int option, int value) {
     if (!ctx) return VR_ERR_INVALID_ARG;
     if (option == VR_OPT_SKIP) { ctx->opt_skip = value ? 1 : 0; return VR_OK; }

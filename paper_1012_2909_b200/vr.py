@@ -23,7 +23,7 @@ EXPORTS = [
     "vr_upload_cube", "vr_generate_cube", "vr_attach_cube", "vr_download_brick", "vr_set_view",
     "vr_set_viewport", "vr_set_transfer_function", "vr_render_mip", "vr_render_ea",
     "vr_sort_bricks", "vr_partial_layout", "vr_render_bricks", "vr_composite_bricks",
-    "vr_get_counters", "vr_reset_counters", "vr_set_option",
+    "vr_get_counters", "vr_reset_counters", "vr_set_option", "vr_get_plan",
 ]
 
 
@@ -84,6 +84,7 @@ def load():
     lib.vr_get_counters.argtypes = [vp, C.POINTER(Counters), vp]
     lib.vr_reset_counters.argtypes = [vp, vp]
     lib.vr_set_option.argtypes = [vp, C.c_int, C.c_int]
+    lib.vr_get_plan.argtypes = [vp, C.c_int, C.POINTER(C.c_int), vp]
     _lib = lib
     return lib
 
@@ -231,6 +232,11 @@ class Context:
 
     def reset_counters(self, stream=None):
         self._check(self._lib.vr_reset_counters(self._h, _stream(stream)))
+
+    def get_plan(self, mode, stream=None):
+        out = (C.c_int * 3)()
+        self._check(self._lib.vr_get_plan(self._h, int(mode), out, _stream(stream)))
+        return {"variant": out[0], "skip_level": out[1], "dense": out[2]}
 
     def set_option(self, option, value):
         self._check(self._lib.vr_set_option(self._h, int(option), int(value)))

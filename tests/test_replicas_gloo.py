@@ -1,0 +1,71 @@
+"""The N > 1 path on CPU: two processes over gloo ("replicas only").
+
+The path has no data-path collective (BASELINE.json north_star); what N > 1 adds is the split of
+the orbit's frames over the ranks and the reduction of timing / counters, both host logic."""
+import os
+import socket
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, n_steps, out):
+    import torch
+    import torch.distributed as dist
+    from paper_1012_2909_b200 import replicas
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        mine = replicas.frames_of_rank(n_steps, rank, world)
+        gathered = [None] * world
+        dist.all_gather_object(gathered, mine)
+        # per-rank figures: rank r took (10 + r) ms and counted (100 + r, 7) units
+        ms, sums = replicas.reduce_run(dist, "cpu", 10.0 + rank, [100 + rank, 7])
+        dist.barrier()
+        if rank == 0:
+            out.put((gathered, ms, sums))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("n_steps", [4, 24, 180])
+def test_two_replicas_split_the_orbit_and_reduce(n_steps):
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, n_steps, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    gathered, ms, sums = out.get(timeout=120)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    a, b = gathered
+    assert len(a) == len(b) == n_steps
+    assert not set(a) & set(b), "two replicas rendered the same frame"
+    allf = sorted(a + b)
+    assert len(set(allf)) == 2 * n_steps
+    # evenly spread over the 360-frame orbit, interleaved over the ranks
+    gaps = [y - x for x, y in zip(allf, allf[1:])]
+    assert max(gaps) - min(gaps) <= 1
+    assert ms == 11.0                      # the slowest rank
+    assert sums == [201, 14]               # counters add up
+
+
+def test_single_process_is_the_identity():
+    from paper_1012_2909_b200 import replicas
+    assert replicas.reduce_run(None, "cpu", 3.5, [1, 2]) == (3.5, [1, 2])
+    assert replicas.frames_of_rank(4, 0, 1) == [0, 90, 180, 270]
+    assert replicas.orbit_frame(359, 360) == 359
