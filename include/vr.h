@@ -136,6 +136,25 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* h_partials, int n,
 int vr_composite_bricks(vr_ctx* ctx, int mode, const vr_partial* h_partials, int n, float* d_out,
                         const float bg[4], void* stream);
 
+/* ---- sharding the bricks over several GPUs (PAPER.md line 13 abstract
+ *      and line 19 section 1: "distributed GPUs", sub-volumes rendered where they reside and
+ *      composited) ----------------------------------------------------------------------------- */
+/* Make bricks [first_brick, end_brick) (global ids, x fastest) the only resident ones of this
+ * context: read by the next vr_generate_cube / vr_upload_cube / vr_attach_cube, whose d_cube and
+ * d_meta then hold just these bricks (sizes: vr_window_layout).  All calls keep GLOBAL voxel
+ * coordinates and brick ids; vr_sort_bricks lists resident bricks only; vr_render_mip / vr_render_ea
+ * (one accumulator carried through all bricks) return VR_ERR_STATE.  end_brick < 0: all bricks. */
+int vr_set_brick_window(vr_ctx* ctx, int first_brick, int end_brick);
+int vr_window_layout(int nx, int ny, int nz, int bx, int by, int bz, int first_brick, int end_brick,
+                     size_t* cube_bytes, size_t* meta_bytes);
+/* Front-to-back order (O-9) of n_groups groups of bricks under the current view, group g = bricks
+ * [h_group_first[g], h_group_first[g+1]) (n_groups + 1 ascending entries, whole z-layers of the
+ * brick grid, covering all bricks): along any ray the z index of the bricks moves monotonically
+ * away from the eye's, so slabs are met in the order of their smallest brick key, and slabs with
+ * equal key never share a ray.  Folding the groups' composited partial frames in this order with
+ * vr_composite_bricks equals the fold over all bricks up to float32 reassociation (MIP: exactly). */
+int vr_sort_groups(vr_ctx* ctx, const int* h_group_first, int n_groups, int* h_group_order);
+
 /* ---- counters (SURVEY.md section 5 "metrics") ---------------------------------------------- */
 typedef struct {
     int64_t rays;             /* rays that had at least one lattice sample inside the cube */

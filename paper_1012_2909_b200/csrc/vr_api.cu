@@ -2,6 +2,7 @@
 // (matrix inverse in fp64, opacity-corrected table, brick classification
 // against the table, visibility keys + sort) and the launch plumbing.  No torch types.
 #include <algorithm>
+#include <climits>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -46,6 +47,7 @@ struct vr_ctx {
     bool key_valid = false, occ_valid = false;
     int key_nz[257];
     float key_vmin = 0, key_scale = 0;
+    int win_lo = 0, win_hi = -1;         // vr_set_brick_window (hi < 0: all bricks)
 };
 
 namespace {
@@ -101,24 +103,41 @@ bool valid_dims(int nx, int ny, int nz, int bx, int by, int bz) {
            (long long)nx < (1 << 22) && (long long)ny < (1 << 22) && (long long)nz < (1 << 22);
 }
 
+// Point the descriptor at the caller's buffers.  They hold the bricks of the window only; every
+// pointer is shifted back by the window's first brick so that global brick ids index it.
 void bind_meta(CubeDesc& c, const void* d_cube, void* d_meta) {
     MetaLayout ml = meta_layout(c);
     char* m = (char*)d_meta;
-    c.cube = (const float*)d_cube;
-    c.brick_mm = (float2*)(m + ml.brick_mm);
-    c.cell_mm = (float2*)(m + ml.cell_mm);
-    c.cell_bits = (unsigned*)(m + ml.cell_bits);
-    c.brick_active = (int*)(m + ml.brick_active);
-    c.occ = (unsigned*)(m + ml.occ);
+    const long long lo = c.win_lo;
+    c.cube = (const float*)d_cube - lo * c.stride;
+    c.brick_mm = (float2*)(m + ml.brick_mm) - lo;
+    c.cell_mm = (float2*)(m + ml.cell_mm) - lo * c.cells_per_brick;
+    c.cell_bits = (unsigned*)(m + ml.cell_bits) - lo * c.cell_words_per_brick;
+    c.brick_active = (int*)(m + ml.brick_active) - lo;
+    c.occ = (unsigned*)(m + ml.occ) - lo * c.occ_words_per_brick;
+}
+
+void apply_window(const vr_ctx* ctx, CubeDesc& c) {
+    if (ctx->win_hi >= 0) { c.win_lo = std::min(ctx->win_lo, c.nbricks); c.win_hi = std::min(ctx->win_hi, c.nbricks); }
+}
+
+// (min,max) of the resident bricks to the host; bricks outside the window read as empty
+int fetch_brick_mm(vr_ctx* ctx, cudaStream_t s) {
+    const CubeDesc& c = ctx->cube;
+    ctx->h_brick_mm.assign(c.nbricks, make_float2(INFINITY, -INFINITY));
+    if (c.win_hi > c.win_lo)
+        VR_CUDA(ctx, cudaMemcpyAsync(ctx->h_brick_mm.data() + c.win_lo, c.brick_mm + c.win_lo, sizeof(float2) * (c.win_hi - c.win_lo),
+                                     cudaMemcpyDeviceToHost, s));
+    VR_CUDA(ctx, cudaStreamSynchronize(s));
+    return VR_OK;
 }
 
 int finish_cube(vr_ctx* ctx, cudaStream_t s) {
     CubeDesc& c = ctx->cube;
     VR_CUDA(ctx, launch_minmax(c, s));
     ctx->launches += 2;
-    ctx->h_brick_mm.resize(c.nbricks);
-    VR_CUDA(ctx, cudaMemcpyAsync(ctx->h_brick_mm.data(), c.brick_mm, sizeof(float2) * c.nbricks, cudaMemcpyDeviceToHost, s));
-    VR_CUDA(ctx, cudaStreamSynchronize(s));
+    int rc = fetch_brick_mm(ctx, s);
+    if (rc) return rc;
     ctx->has_cube = true;
     ctx->activity_dirty = true; ctx->key_valid = false; ctx->occ_valid = false;
     return VR_OK;
@@ -170,7 +189,8 @@ int ensure_tables(vr_ctx* ctx, cudaStream_t s) {
             for (int b = 0; b < nb; ++b)
                 ctx->h_brick_active[b] = range_active(ctx, ctx->h_brick_mm[b].x, ctx->h_brick_mm[b].y) ? 1 : 0;
             // pageable source: cudaMemcpyAsync stages it before returning, so the vector may change later
-            VR_CUDA(ctx, cudaMemcpyAsync(ctx->cube.brick_active, ctx->h_brick_active.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, s));
+            const int w0 = ctx->cube.win_lo, wn = ctx->cube.win_hi - ctx->cube.win_lo;
+            if (wn > 0) VR_CUDA(ctx, cudaMemcpyAsync(ctx->cube.brick_active + w0, ctx->h_brick_active.data() + w0, sizeof(int) * wn, cudaMemcpyHostToDevice, s));
             // the same test per 8^3 macro-cell, on the device (one bit per cell)
             VR_CUDA(ctx, cudaMemsetAsync(ctx->d_scratch, 0, sizeof(unsigned long long), s));
             VR_CUDA(ctx, launch_classify_cells(ctx->cube, nz, ctx->vmin, ctx->scale, ctx->d_scratch, s));
@@ -178,7 +198,7 @@ int ensure_tables(vr_ctx* ctx, cudaStream_t s) {
             unsigned long long n_active = 0;
             VR_CUDA(ctx, cudaMemcpyAsync(&n_active, ctx->d_scratch, sizeof(n_active), cudaMemcpyDeviceToHost, s));
             VR_CUDA(ctx, cudaStreamSynchronize(s));
-            ctx->active_cell_fraction = (double)n_active / std::max(1.0, (double)ctx->cube.nbricks * ctx->cube.cells_per_brick);
+            ctx->active_cell_fraction = (double)n_active / std::max(1.0, (double)(ctx->cube.win_hi - ctx->cube.win_lo) * ctx->cube.cells_per_brick);
             std::memcpy(ctx->key_nz, nz, sizeof(nz));
             ctx->key_vmin = ctx->vmin; ctx->key_scale = ctx->scale;
             ctx->key_valid = true; ctx->occ_valid = false;
@@ -324,7 +344,7 @@ int upload_partials(vr_ctx* ctx, int mode, const vr_partial* hp, int n, bool wit
     const int W = ctx->view.W, H = ctx->view.H;
     for (int i = 0; i < n; ++i) {
         const vr_partial& p = hp[i];
-        if (p.brick < 0 || p.brick >= ctx->cube.nbricks || p.w <= 0 || p.h <= 0 || p.x0 < 0 || p.y0 < 0 ||
+        if (p.brick < ctx->cube.win_lo || p.brick >= ctx->cube.win_hi || p.w <= 0 || p.h <= 0 || p.x0 < 0 || p.y0 < 0 ||
             p.x0 + p.w > W || p.y0 + p.h > H || !p.d_data || p.pitch_px < (size_t)p.w)
             return fail(ctx, VR_ERR_INVALID_ARG, "bad vr_partial entry");
         if (((uintptr_t)p.d_data & (mode == VR_MODE_EA ? 15 : 3)) != 0)
@@ -359,6 +379,7 @@ void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz,
     if (layout == 0) c.P[0] = (c.P[0] + 3) / 4 * 4;
     c.T[0] = (c.P[0] + 3) / 4; c.T[1] = (c.P[1] + 3) / 4; c.T[2] = (c.P[2] + 1) / 2;
     c.nbricks = c.G[0] * c.G[1] * c.G[2];
+    c.win_lo = 0; c.win_hi = c.nbricks;
     c.cells_per_brick = c.C[0] * c.C[1] * c.C[2];
     c.cell_words_per_brick = (c.cells_per_brick + 31) / 32;
     c.occ_words_per_brick = 32 * c.C[0] * c.C[1] * ((c.C[2] + 1) / 2);
@@ -366,16 +387,17 @@ void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz,
                            : 32LL * c.T[0] * c.T[1] * c.T[2];
 }
 
-size_t cube_bytes(const CubeDesc& c) { return (size_t)c.nbricks * (size_t)c.stride * sizeof(float); }
+size_t cube_bytes(const CubeDesc& c) { return (size_t)(c.win_hi - c.win_lo) * (size_t)c.stride * sizeof(float); }
 
 MetaLayout meta_layout(const CubeDesc& c) {
     MetaLayout m;
+    const size_t nb = (size_t)(c.win_hi - c.win_lo);
     size_t off = 0;
-    m.brick_mm = off; off = align_up(off + sizeof(float2) * c.nbricks, 256);
-    m.cell_mm = off; off = align_up(off + sizeof(float2) * (size_t)c.nbricks * c.cells_per_brick, 256);
-    m.cell_bits = off; off = align_up(off + sizeof(unsigned) * (size_t)c.nbricks * c.cell_words_per_brick, 256);
-    m.brick_active = off; off = align_up(off + sizeof(int) * c.nbricks, 256);
-    m.occ = off; off = align_up(off + sizeof(unsigned) * (size_t)c.nbricks * c.occ_words_per_brick, 256);
+    m.brick_mm = off; off = align_up(off + sizeof(float2) * nb, 256);
+    m.cell_mm = off; off = align_up(off + sizeof(float2) * nb * c.cells_per_brick, 256);
+    m.cell_bits = off; off = align_up(off + sizeof(unsigned) * nb * c.cell_words_per_brick, 256);
+    m.brick_active = off; off = align_up(off + sizeof(int) * nb, 256);
+    m.occ = off; off = align_up(off + sizeof(unsigned) * nb * c.occ_words_per_brick, 256);
     m.total = off;
     return m;
 }
@@ -443,9 +465,10 @@ int vr_attach_cube(vr_ctx* ctx, int nx, int ny, int nz, int bx, int by, int bz, 
     if (!ctx) return VR_ERR_INVALID_ARG;
     if (!valid_dims(nx, ny, nz, bx, by, bz) || !d_cube || !d_meta) return fail(ctx, VR_ERR_INVALID_ARG, "vr_attach_cube: bad argument");
     fill_cube_desc(ctx->cube, nx, ny, nz, bx, by, bz, ctx->opt_layout);
+    apply_window(ctx, ctx->cube);
     bind_meta(ctx->cube, d_cube, d_meta);
-    ctx->h_brick_mm.resize(ctx->cube.nbricks);
-    VR_CUDA(ctx, cudaMemcpy(ctx->h_brick_mm.data(), ctx->cube.brick_mm, sizeof(float2) * ctx->cube.nbricks, cudaMemcpyDeviceToHost));
+    int rc = fetch_brick_mm(ctx, nullptr);
+    if (rc) return rc;
     ctx->has_cube = true;
     ctx->activity_dirty = true; ctx->key_valid = false; ctx->occ_valid = false;
     return VR_OK;
@@ -459,10 +482,11 @@ int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int
     ctx->has_cube = false;
     CubeDesc& c = ctx->cube;
     fill_cube_desc(c, nx, ny, nz, bx, by, bz, ctx->opt_layout);
+    apply_window(ctx, c);
     bind_meta(c, d_cube, d_meta);
     VR_CUDA(ctx, cudaMemsetAsync(d_cube, 0, cube_bytes(c), s));
     if (src_is_device) {
-        VR_CUDA(ctx, launch_rebrick(c, (float*)d_cube, src, 0, nz, s));
+        VR_CUDA(ctx, launch_rebrick(c, const_cast<float*>(c.cube), src, 0, nz, s));
         ctx->launches += 1;
     } else {
         const size_t plane = (size_t)nx * ny * sizeof(float);
@@ -477,7 +501,7 @@ int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int
         for (int z0 = 0; z0 < nz; z0 += planes) {
             int z1 = std::min(nz, z0 + planes);
             VR_CUDA(ctx, cudaMemcpyAsync(ctx->d_stage, src + (size_t)z0 * nx * ny, plane * (z1 - z0), cudaMemcpyHostToDevice, s));
-            VR_CUDA(ctx, launch_rebrick(c, (float*)d_cube, ctx->d_stage, z0, z1, s));
+            VR_CUDA(ctx, launch_rebrick(c, const_cast<float*>(c.cube), ctx->d_stage, z0, z1, s));
             ctx->launches += 1;
             VR_CUDA(ctx, cudaStreamSynchronize(s));          // the staging slab is reused
         }
@@ -496,6 +520,7 @@ int vr_generate_cube(vr_ctx* ctx, const vr_gen_params* prm, uint64_t seed, int n
     ctx->has_cube = false;
     CubeDesc& c = ctx->cube;
     fill_cube_desc(c, nx, ny, nz, bx, by, bz, ctx->opt_layout);
+    apply_window(ctx, c);
     bind_meta(c, d_cube, d_meta);
     // bin the sources (ascending id) and the zero boxes over 32^3 tiles of the cube
     const int T[3] = {(nx + 31) / 32, (ny + 31) / 32, (nz + 31) / 32};
@@ -538,7 +563,7 @@ int vr_generate_cube(vr_ctx* ctx, const vr_gen_params* prm, uint64_t seed, int n
         g.sources = d_src; g.tile_offsets = d_offs; g.tile_ids = d_ids;
         g.tiles[0] = T[0]; g.tiles[1] = T[1]; g.tiles[2] = T[2];
         g.zero_boxes = d_zb; g.n_zero = prm->n_zero_boxes; g.continuum = prm->continuum; g.seed = seed;
-        e = launch_generate(c, (float*)d_cube, g, s);
+        e = launch_generate(c, const_cast<float*>(c.cube), g, s);
         ctx->launches += 1;
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
@@ -550,7 +575,7 @@ int vr_generate_cube(vr_ctx* ctx, const vr_gen_params* prm, uint64_t seed, int n
 int vr_download_brick(vr_ctx* ctx, int brick_id, float* d_dst, void* stream) {
     if (!ctx) return VR_ERR_INVALID_ARG;
     if (!ctx->has_cube) return fail(ctx, VR_ERR_STATE, "no cube");
-    if (brick_id < 0 || brick_id >= ctx->cube.nbricks || !d_dst) return fail(ctx, VR_ERR_INVALID_ARG, "vr_download_brick: bad argument");
+    if (brick_id < ctx->cube.win_lo || brick_id >= ctx->cube.win_hi || !d_dst) return fail(ctx, VR_ERR_INVALID_ARG, "vr_download_brick: bad argument (brick not resident?)");
     VR_CUDA(ctx, launch_unbrick(ctx->cube, brick_id, d_dst, (cudaStream_t)stream));
     ctx->launches += 1;
     return VR_OK;
@@ -593,6 +618,7 @@ int vr_render_mip(vr_ctx* ctx, float* d_out, float* d_out_rgba, float miss, void
     int rc = check_render_state(ctx, d_out_rgba != nullptr);
     if (rc) return rc;
     if (!d_out) return fail(ctx, VR_ERR_INVALID_ARG, "vr_render_mip: null output");
+    if (ctx->cube.win_hi - ctx->cube.win_lo != ctx->cube.nbricks) return fail(ctx, VR_ERR_STATE, "vr_render_mip needs the whole cube resident (brick window set: use vr_render_bricks)");
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
@@ -608,6 +634,7 @@ int vr_render_ea(vr_ctx* ctx, float* d_out, const float bg[4], float tau, void* 
     if (rc) return rc;
     if (!d_out || !bg || !(tau > 0.f)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_render_ea: bad argument");
     if (((uintptr_t)d_out & 15) != 0) return fail(ctx, VR_ERR_INVALID_ARG, "vr_render_ea: output must be 16-byte aligned");
+    if (ctx->cube.win_hi - ctx->cube.win_lo != ctx->cube.nbricks) return fail(ctx, VR_ERR_STATE, "vr_render_ea needs the whole cube resident (brick window set: use vr_render_bricks)");
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
@@ -620,13 +647,10 @@ int vr_render_ea(vr_ctx* ctx, float* d_out, const float bg[4], float tau, void* 
     return VR_OK;
 }
 
-int vr_sort_bricks(vr_ctx* ctx, int mode, int* h_order, int* n_active) {
-    int rc = check_render_state(ctx, mode == VR_MODE_EA);
-    if (rc) return rc;
-    if (!n_active || (mode != VR_MODE_MIP && mode != VR_MODE_EA)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_sort_bricks: bad argument");
+// O-9 visibility key of every brick under the current view: perspective, eye = h.xyz / h.w with
+// h = Minv (0,0,1,0)^T, key = sum |b_a - E_a|; orthographic: b_a counted along the common direction.
+static void brick_keys(const vr_ctx* ctx, std::vector<int>& key) {
     const CubeDesc& c = ctx->cube;
-    if (mode == VR_MODE_EA && (ctx->tables_dirty || ctx->baked_step != ctx->view.step)) { bake_tf(ctx); ctx->tables_dirty = true; }
-    // O-9: h = Minv (0,0,1,0)^T; perspective eye = h.xyz / h.w, else common direction sign(d)
     const double* Mi = ctx->Minv;
     double h[4] = {Mi[2], Mi[6], Mi[10], Mi[14]};
     double nrm = std::fabs(h[0]) + std::fabs(h[1]) + std::fabs(h[2]);
@@ -644,21 +668,83 @@ int vr_sort_bricks(vr_ctx* ctx, int mode, int* h_order, int* n_active) {
         L = std::sqrt(L);
         for (int a = 0; a < 3; ++a) sg[a] = d[a] / L > 1e-12 ? 1 : (d[a] / L < -1e-12 ? -1 : 0);
     }
-    std::vector<std::pair<int, int>> keyed;
-    keyed.reserve(c.nbricks);
+    key.resize(c.nbricks);
     for (int bid = 0; bid < c.nbricks; ++bid) {
+        int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
+        int k = 0;
+        for (int a = 0; a < 3; ++a)
+            k += persp ? std::abs(b[a] - E[a]) : (sg[a] > 0 ? b[a] : (sg[a] < 0 ? c.G[a] - 1 - b[a] : 0));
+        key[bid] = k;
+    }
+}
+
+int vr_sort_bricks(vr_ctx* ctx, int mode, int* h_order, int* n_active) {
+    int rc = check_render_state(ctx, mode == VR_MODE_EA);
+    if (rc) return rc;
+    if (!n_active || (mode != VR_MODE_MIP && mode != VR_MODE_EA)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_sort_bricks: bad argument");
+    const CubeDesc& c = ctx->cube;
+    if (mode == VR_MODE_EA && (ctx->tables_dirty || ctx->baked_step != ctx->view.step)) { bake_tf(ctx); ctx->tables_dirty = true; }
+    std::vector<int> key;
+    brick_keys(ctx, key);
+    std::vector<std::pair<int, int>> keyed;
+    keyed.reserve(c.win_hi - c.win_lo);
+    for (int bid = c.win_lo; bid < c.win_hi; ++bid) {      // resident bricks only
         int rect[4];
         if (!brick_rect(ctx, bid, rect)) continue;
         if (mode == VR_MODE_EA && ctx->opt_skip && !range_active(ctx, ctx->h_brick_mm[bid].x, ctx->h_brick_mm[bid].y)) continue;
-        int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
-        int key = 0;
-        for (int a = 0; a < 3; ++a)
-            key += persp ? std::abs(b[a] - E[a]) : (sg[a] > 0 ? b[a] : (sg[a] < 0 ? c.G[a] - 1 - b[a] : 0));
-        keyed.emplace_back(key, bid);
+        keyed.emplace_back(key[bid], bid);
     }
     std::stable_sort(keyed.begin(), keyed.end());
     *n_active = (int)keyed.size();
     if (h_order) for (size_t i = 0; i < keyed.size(); ++i) h_order[i] = keyed[i].second;
+    return VR_OK;
+}
+
+int vr_sort_groups(vr_ctx* ctx, const int* h_group_first, int n_groups, int* h_group_order) {
+    int rc = check_render_state(ctx, false);
+    if (rc) return rc;
+    if (!h_group_first || !h_group_order || n_groups <= 0) return fail(ctx, VR_ERR_INVALID_ARG, "vr_sort_groups: bad argument");
+    const CubeDesc& c = ctx->cube;
+    const int layer = c.G[0] * c.G[1];
+    for (int g = 0; g <= n_groups; ++g) {
+        const int f = h_group_first[g];
+        if (f < 0 || f > c.nbricks || f % layer != 0 || (g > 0 && f < h_group_first[g - 1]))
+            return fail(ctx, VR_ERR_INVALID_ARG, "vr_sort_groups: groups must be ascending whole z-layers of bricks");
+    }
+    if (h_group_first[0] != 0 || h_group_first[n_groups] != c.nbricks)
+        return fail(ctx, VR_ERR_INVALID_ARG, "vr_sort_groups: groups must cover all bricks");
+    std::vector<int> key;
+    brick_keys(ctx, key);
+    std::vector<std::pair<int, int>> keyed;
+    for (int g = 0; g < n_groups; ++g) {
+        int k = INT_MAX;
+        for (int bid = h_group_first[g]; bid < h_group_first[g + 1]; ++bid) k = std::min(k, key[bid]);
+        keyed.emplace_back(k, g);                           // an empty group sorts last; it has no partial to fold
+    }
+    std::stable_sort(keyed.begin(), keyed.end());
+    for (int g = 0; g < n_groups; ++g) h_group_order[g] = keyed[g].second;
+    return VR_OK;
+}
+
+int vr_set_brick_window(vr_ctx* ctx, int first_brick, int end_brick) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (end_brick < 0) { ctx->win_lo = 0; ctx->win_hi = -1; return VR_OK; }
+    if (first_brick < 0 || end_brick < first_brick) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_brick_window: bad window");
+    ctx->win_lo = first_brick; ctx->win_hi = end_brick;
+    return VR_OK;
+}
+
+int vr_window_layout(int nx, int ny, int nz, int bx, int by, int bz, int first_brick, int end_brick, size_t* cube_bytes_out,
+                     size_t* meta_bytes_out) {
+    if (!valid_dims(nx, ny, nz, bx, by, bz) || !cube_bytes_out || !meta_bytes_out || first_brick < 0 || end_brick < first_brick)
+        return VR_ERR_INVALID_ARG;
+    CubeDesc c0, c1;
+    fill_cube_desc(c0, nx, ny, nz, bx, by, bz, 0);
+    fill_cube_desc(c1, nx, ny, nz, bx, by, bz, 1);
+    if (end_brick > c0.nbricks) return VR_ERR_INVALID_ARG;
+    c0.win_lo = c1.win_lo = first_brick; c0.win_hi = c1.win_hi = end_brick;
+    *cube_bytes_out = std::max(cube_bytes(c0), cube_bytes(c1));
+    *meta_bytes_out = meta_layout(c0).total;
     return VR_OK;
 }
 

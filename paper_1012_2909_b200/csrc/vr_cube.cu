@@ -45,6 +45,7 @@ __global__ void rebrick_kernel(CubeDesc c, float* __restrict__ cube, const float
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n_elems;
          e += (long long)gridDim.x * blockDim.x) {
         long long brick = brick_lo + e / per, rem = e % per;
+        if (brick < c.win_lo || brick >= c.win_hi) continue;
         Elem el = decode(c, brick, rem);
         if (!el.in_cube || el.g[2] < z0 || el.g[2] >= z1) continue;
         cube[brick * c.stride + rem] =
@@ -65,8 +66,8 @@ __global__ void unbrick_kernel(CubeDesc c, int brick, float* __restrict__ dst, i
 // (min,max) of every macro-cell over its voxels plus the +1 layer (O-10: halo-inclusive), clipped
 // to the cube.  One thread per cell.
 __global__ void cell_minmax_kernel(CubeDesc c) {
-    long long ncell = (long long)c.nbricks * c.cells_per_brick;
-    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ncell;
+    const long long first = (long long)c.win_lo * c.cells_per_brick, ncell = (long long)c.win_hi * c.cells_per_brick;
+    for (long long e = first + (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ncell;
          e += (long long)gridDim.x * blockDim.x) {
         int brick = (int)(e / c.cells_per_brick), cc = (int)(e % c.cells_per_brick);
         int ci[3] = {cc % c.C[0], (cc / c.C[0]) % c.C[1], cc / (c.C[0] * c.C[1])};
@@ -94,7 +95,7 @@ __global__ void cell_minmax_kernel(CubeDesc c) {
 
 __global__ void brick_minmax_kernel(CubeDesc c) {
     __shared__ float smn[256], smx[256];
-    int brick = blockIdx.x;
+    int brick = c.win_lo + blockIdx.x;
     float mn = INFINITY, mx = -INFINITY;
     for (int i = threadIdx.x; i < c.cells_per_brick; i += blockDim.x) {
         float2 v = c.cell_mm[(long long)brick * c.cells_per_brick + i];
@@ -132,7 +133,7 @@ __global__ void generate_kernel(CubeDesc c, float* __restrict__ cube, GenDev g, 
     const long long per = slots_per_brick(c);
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n_elems;
          e += (long long)gridDim.x * blockDim.x) {
-        long long brick = e / per, rem = e % per;
+        long long brick = c.win_lo + e / per, rem = e % per;
         Elem el = decode(c, brick, rem);
         float out = 0.0f;
         if (el.in_cube) {
@@ -198,16 +199,16 @@ cudaError_t launch_unbrick(const CubeDesc& c, int brick, float* d_dst, cudaStrea
 }
 
 cudaError_t launch_minmax(const CubeDesc& c, cudaStream_t s) {
-    long long ncell = (long long)c.nbricks * c.cells_per_brick;
+    long long ncell = (long long)(c.win_hi - c.win_lo) * c.cells_per_brick;
     cell_minmax_kernel<<<grid_for(ncell, 128), 128, 0, s>>>(c);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    brick_minmax_kernel<<<c.nbricks, 256, 0, s>>>(c);
+    brick_minmax_kernel<<<c.win_hi - c.win_lo, 256, 0, s>>>(c);
     return cudaGetLastError();
 }
 
 cudaError_t launch_generate(const CubeDesc& c, float* d_cube, const GenDev& g, cudaStream_t s) {
-    long long n = (long long)c.nbricks * slots_per_brick(c);
+    long long n = (long long)(c.win_hi - c.win_lo) * slots_per_brick(c);
     generate_kernel<<<grid_for(n, 256), 256, 0, s>>>(c, d_cube, g, n);
     return cudaGetLastError();
 }

@@ -34,6 +34,8 @@ struct CubeDesc {
     int sh[3];       // log2(B) if B is a power of two, else -1
     int C[3];        // macro-cells per brick axis = ceil(B / kCell)
     int nbricks;
+    int win_lo, win_hi;          // resident bricks [win_lo, win_hi) (all by default); the pointers below are
+                                 // shifted so that GLOBAL brick ids index them (vr_set_brick_window)
     int cells_per_brick;
     long long stride;            // floats per brick (multiple of 32)
     const float* cube;

@@ -918,9 +918,9 @@ classify_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nbx = (c.B[0] + 3) >> 2, nby = (c.B[1] + 3) >> 2, nbz = (c.B[2] + 1) >> 1;   // micro-blocks holding lower corners
     const int ngy = (nby + 3) >> 2, ngz = (nbz + 1) >> 1;
-    const long long n_units = (long long)c.nbricks * ngy * ngz;
+    const long long n_units = (long long)(c.win_hi - c.win_lo) * ngy * ngz;
     for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
-        const int brick = (int)(u / (ngy * ngz));
+        const int brick = c.win_lo + (int)(u / (ngy * ngz));
         const int rem = (int)(u % (ngy * ngz));
         const int by = 4 * (rem % ngy) + (warp & 3), bz = 2 * (rem / ngy) + (warp >> 2);
         if (by >= nby || bz >= nbz) continue;
@@ -958,7 +958,7 @@ __global__ void classify_cells_kernel(const __grid_constant__ CubeDesc c, const 
                                       unsigned long long* __restrict__ active_count) {
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n_slots;
          e += (long long)gridDim.x * blockDim.x) {
-        const long long word = e >> 5;
+        const long long word = (long long)c.win_lo * c.cell_words_per_brick + (e >> 5);
         const int brick = (int)(word / c.cell_words_per_brick);
         const int cidx = (int)(word % c.cell_words_per_brick) * 32 + (int)(e & 31);
         bool active = false;
@@ -1044,7 +1044,7 @@ cudaError_t launch_classify_cells(const CubeDesc& c, const int nz_prefix[257], f
                                   unsigned long long* d_active_count, cudaStream_t s) {
     NzPrefix nz;
     for (int i = 0; i < 257; ++i) nz.v[i] = nz_prefix[i];
-    const long long n_slots = (long long)c.nbricks * c.cell_words_per_brick * 32;
+    const long long n_slots = (long long)(c.win_hi - c.win_lo) * c.cell_words_per_brick * 32;
     long long blocks = (n_slots + 255) / 256;
     if (blocks > 148LL * 32) blocks = 148LL * 32;
     classify_cells_kernel<<<(int)blocks, 256, 0, s>>>(c, nz, vmin, scale, n_slots, d_active_count);

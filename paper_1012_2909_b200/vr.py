@@ -24,6 +24,7 @@ EXPORTS = [
     "vr_set_viewport", "vr_set_transfer_function", "vr_render_mip", "vr_render_ea",
     "vr_sort_bricks", "vr_partial_layout", "vr_render_bricks", "vr_composite_bricks",
     "vr_get_counters", "vr_reset_counters", "vr_set_option", "vr_get_plan",
+    "vr_set_brick_window", "vr_window_layout", "vr_sort_groups",
 ]
 
 
@@ -85,6 +86,9 @@ def load():
     lib.vr_reset_counters.argtypes = [vp, vp]
     lib.vr_set_option.argtypes = [vp, C.c_int, C.c_int]
     lib.vr_get_plan.argtypes = [vp, C.c_int, C.POINTER(C.c_int), vp]
+    lib.vr_set_brick_window.argtypes = [vp, C.c_int, C.c_int]
+    lib.vr_window_layout.argtypes = [C.c_int] * 8 + [C.POINTER(sz), C.POINTER(sz)]
+    lib.vr_sort_groups.argtypes = [vp, ip, C.c_int, ip]
     _lib = lib
     return lib
 
@@ -108,6 +112,15 @@ def cube_layout(dims, brick):
     rc = load().vr_cube_layout(*(int(v) for v in dims), *(int(v) for v in brick), C.byref(cb), C.byref(mb))
     if rc != OK:
         raise VRError(rc, "vr_cube_layout: invalid argument")
+    return cb.value, mb.value
+
+
+def window_layout(dims, brick, first_brick, end_brick):
+    cb, mb = C.c_size_t(0), C.c_size_t(0)
+    rc = load().vr_window_layout(*(int(v) for v in dims), *(int(v) for v in brick), int(first_brick), int(end_brick),
+                                 C.byref(cb), C.byref(mb))
+    if rc != OK:
+        raise VRError(rc, "vr_window_layout: invalid argument")
     return cb.value, mb.value
 
 
@@ -237,6 +250,16 @@ class Context:
         out = (C.c_int * 3)()
         self._check(self._lib.vr_get_plan(self._h, int(mode), out, _stream(stream)))
         return {"variant": out[0], "skip_level": out[1], "dense": out[2]}
+
+    def set_brick_window(self, first_brick, end_brick):
+        self._check(self._lib.vr_set_brick_window(self._h, int(first_brick), int(end_brick)))
+
+    def sort_groups(self, group_first):
+        g = np.ascontiguousarray(group_first, dtype=np.int32)
+        order = np.zeros(g.size - 1, dtype=np.int32)
+        self._check(self._lib.vr_sort_groups(self._h, g.ctypes.data_as(C.POINTER(C.c_int)), int(g.size - 1),
+                                             order.ctypes.data_as(C.POINTER(C.c_int))))
+        return order
 
     def set_option(self, option, value):
         self._check(self._lib.vr_set_option(self._h, int(option), int(value)))

@@ -1,0 +1,98 @@
+"""NEXT-1: bricks sharded over ranks in z-slabs, partial frames folded in the
+slabs' visibility order.  One GPU: the ranks' contexts render one after the other (nothing waits
+on anything), the exchange is done by slicing.  Reference = the single-context sort-last frame of
+the same cube (itself checked against the oracle in test_gpu_parity.py)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def _render_sharded(torch, vr, wl, sl, w, world, mode, M, tf, bg, tau):
+    W, H = w.frame
+    src = wl.make_sources(w)
+    shards, partials = [], []
+    for r in range(world):
+        ctx = vr.Context(0)
+        sh = sl.Shard(ctx, w.dims, w.brick, r, world)
+        sh.bind()
+        cb, mb = sh.layout()
+        d_cube = torch.empty(max(cb // 4, 1), dtype=torch.float32, device="cuda")
+        d_meta = torch.empty(max(mb, 1), dtype=torch.uint8, device="cuda")
+        ctx.generate_cube(w.seed, w.dims, w.brick, d_cube, d_meta, sources=src, continuum=w.continuum)
+        ctx.set_view(M, W, H, w.step)
+        ctx.set_transfer_function(*tf)
+        partials.append(sh.render_partial(torch, mode, W, H, tau))
+        shards.append((sh, d_cube, d_meta))
+    rows = sl.strip_rows(H, world)
+    strips = []
+    for r in range(world):
+        versions = torch.stack([_strip(torch, p, r, rows) for p in partials])      # what rank r receives
+        strips.append(shards[r][0].fold_strip(torch, mode, versions, W, H, bg))
+    torch.cuda.synchronize()
+    return torch.cat(strips, dim=0)[:H].cpu().numpy(), [s[0] for s in shards]
+
+
+def _strip(torch, p, r, rows):
+    H, W, ch = p.shape
+    out = torch.zeros((rows, W, ch), dtype=p.dtype, device=p.device)
+    h = max(0, min(rows, H - r * rows))
+    out[:h] = p[r * rows:r * rows + h]
+    return out
+
+
+@pytest.mark.parametrize("world", [2, 3])
+@pytest.mark.parametrize("az", [20, 90, 200])
+def test_sharded_slabs_equal_single_context(world, az):
+    import torch
+    from paper_1012_2909_b200 import sortlast as sl, vr, workloads as wl
+    import helpers
+    w = wl.scaled(wl.C3, "shard", (96, 80, 160), (32, 32, 32), (160, 90), n_sources=40)
+    M = wl.perspective_camera(w.dims, w.frame, azimuth_deg=az)
+    tf = wl.tf_fog()
+    bg = (0.05, 0.1, 0.2, 0.0)
+    sc = helpers.Scene(w.dims, w.brick, gen={"seed": w.seed, "sources": wl.make_sources(w), "continuum": w.continuum})
+    W, H = w.frame
+    ref, _, _ = sc.render_sortlast(M, W, H, w.step, vr.MODE_EA, tf=tf, bg=bg, tau=2.0)
+    got, shards = _render_sharded(torch, vr, wl, sl, w, world, vr.MODE_EA, M, tf, bg, 2.0)
+    assert np.abs(got - ref).max() <= 2e-6
+    assert sum(s.end - s.first for s in shards) == 3 * 3 * 5        # every brick resident on exactly one rank
+    ref_m, _, _ = sc.render_sortlast(M, W, H, w.step, vr.MODE_MIP, bg=(-3.0, 0, 0, 0))
+    got_m, _ = _render_sharded(torch, vr, wl, sl, w, world, vr.MODE_MIP, M, tf, (-3.0, 0, 0, 0), 2.0)
+    assert np.array_equal(got_m[..., 0], ref_m)                       # max is exact in any order
+
+
+def test_window_refuses_whole_frame_renders_and_foreign_bricks():
+    import torch
+    from paper_1012_2909_b200 import sortlast as sl, vr, workloads as wl
+    w = wl.scaled(wl.C3, "shard", (64, 64, 128), (32, 32, 32), (64, 36), n_sources=4)
+    ctx = vr.Context(0)
+    sh = sl.Shard(ctx, w.dims, w.brick, 1, 2)
+    sh.bind()
+    cb, mb = sh.layout()
+    full_cb, _ = vr.cube_layout(w.dims, w.brick)
+    assert cb * 2 == full_cb
+    d_cube = torch.empty(cb // 4, dtype=torch.float32, device="cuda")
+    d_meta = torch.empty(mb, dtype=torch.uint8, device="cuda")
+    ctx.generate_cube(w.seed, w.dims, w.brick, d_cube, d_meta, sources=wl.make_sources(w))
+    ctx.set_view(wl.perspective_camera(w.dims, w.frame), 64, 36, 0.5)
+    ctx.set_transfer_function(*wl.tf_fog())
+    out = torch.empty((36, 64, 4), dtype=torch.float32, device="cuda")
+    with pytest.raises(vr.VRError) as e:
+        ctx.render_ea(out)
+    assert e.value.status == vr.ERR_STATE
+    assert set(ctx.sort_bricks(vr.MODE_MIP)) <= set(range(sh.first, sh.end))
+    t = torch.empty(32 ** 3, dtype=torch.float32, device="cuda")
+    with pytest.raises(vr.VRError):
+        ctx.download_brick(0, t)
+    # resident bricks hold the same bytes as in an unsharded context
+    ctx.download_brick(sh.first, t)
+    full = vr.Context(0)
+    fc, fm = vr.cube_layout(w.dims, w.brick)
+    dc = torch.empty(fc // 4, dtype=torch.float32, device="cuda")
+    dm = torch.empty(fm, dtype=torch.uint8, device="cuda")
+    full.generate_cube(w.seed, w.dims, w.brick, dc, dm, sources=wl.make_sources(w))
+    t2 = torch.empty(32 ** 3, dtype=torch.float32, device="cuda")
+    full.download_brick(sh.first, t2)
+    torch.cuda.synchronize()
+    assert torch.equal(t, t2)

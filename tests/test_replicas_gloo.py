@@ -69,3 +69,60 @@ def test_single_process_is_the_identity():
     assert replicas.reduce_run(None, "cpu", 3.5, [1, 2]) == (3.5, [1, 2])
     assert replicas.frames_of_rank(4, 0, 1) == [0, 90, 180, 270]
     assert replicas.orbit_frame(359, 360) == 359
+
+
+# ---- NEXT-1 plumbing (paper_1012_2909_b200/sortlast.py): slab partition and the strip exchange
+def test_slab_groups_cover_the_grid():
+    from paper_1012_2909_b200 import sortlast as sl
+    for grid, world in [((8, 8, 16), 8), ((3, 3, 5), 2), ((3, 3, 5), 3), ((2, 2, 1), 4), ((16, 16, 8), 8)]:
+        first = sl.slab_groups(grid, world)
+        assert len(first) == world + 1 and first[0] == 0 and first[-1] == grid[0] * grid[1] * grid[2]
+        sizes = [b - a for a, b in zip(first, first[1:])]
+        assert all(s >= 0 and s % (grid[0] * grid[1]) == 0 for s in sizes)
+        assert max(sizes) - min(sizes) <= grid[0] * grid[1]
+
+
+def _exchange_worker(rank, world, port, out):
+    import torch
+    import torch.distributed as dist
+    from paper_1012_2909_b200 import sortlast as sl
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        H, W, ch = 7, 5, 4                                   # 7 rows over 2 ranks: a padded last strip
+        partial = (torch.arange(H * W * ch, dtype=torch.float32).view(H, W, ch) + 1000.0 * rank)
+        versions = sl.exchange_strips(dist, partial, world)  # [sender, rows, W, ch]
+        rows = sl.strip_rows(H, world)
+        ok = versions.shape == (world, rows, W, ch)
+        for sender in range(world):
+            want = torch.zeros((rows, W, ch))
+            src = torch.arange(H * W * ch, dtype=torch.float32).view(H, W, ch) + 1000.0 * sender
+            h = max(0, min(rows, H - rank * rows))
+            want[:h] = src[rank * rows:rank * rows + h]
+            ok = ok and torch.equal(versions[sender], want)
+        # "fold" stand-in (the real one is a CUDA kernel): keep the local rank's version
+        frame = sl.gather_strips(dist, versions[rank].clone(), world, H)
+        gathered = [None] * world
+        dist.all_gather_object(gathered, (ok, frame.shape, float(frame.sum())))
+        if rank == 0:
+            out.put(gathered)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_strip_exchange_over_gloo():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_exchange_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = out.get(timeout=120)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert all(r[0] for r in res)
+    assert all(tuple(r[1]) == (7, 5, 4) for r in res)
+    assert res[0][2] == res[1][2]                            # every rank ends with the same frame
