@@ -107,10 +107,12 @@ MARCHER = {(0, 0): "render_bricks_kernel<EA> (ray per thread)", (0, 1): "render_
 class Job:
     """One rank's resident cube + context."""
 
-    def __init__(self, w, device):
+    def __init__(self, w, device, mode="ea"):
         import torch
         from paper_1012_2909_b200 import vr
         self.torch, self.vr, self.w = torch, vr, w
+        self.mode = vr.MODE_EA if mode == "ea" else vr.MODE_MIP
+        self.px_bytes = 16 if mode == "ea" else 4
         torch.cuda.set_device(device)
         cb, mb = vr.cube_layout(w.dims, w.brick)
         self.d_cube = torch.empty(cb // 4, dtype=torch.float32, device="cuda")
@@ -126,9 +128,11 @@ class Job:
         self.W, self.H = w.frame
         self.cols, self.rows = w.panels
         self.pw, self.ph = self.W // self.cols, self.H // self.rows
-        self.frame = torch.zeros((self.H, self.W, 4), dtype=torch.float32, device="cuda")
+        ch = 4 if mode == "ea" else 1
+        self.frame = torch.zeros((self.H, self.W, ch), dtype=torch.float32, device="cuda")
         self.arena = None
-        self.h_frame = torch.empty((self.H, self.W, 4), dtype=torch.float32).pin_memory()
+        self.h_frame = torch.empty((self.H, self.W, ch), dtype=torch.float32).pin_memory()
+        self.step_events = []
         self.bg = (0.0, 0.0, 0.0, 0.0)
         self.march_events = []
         self.alg_bytes = 0
@@ -152,20 +156,24 @@ class Job:
                 Mp = M if (self.cols, self.rows) == (1, 1) else wl.panel_matrix(M, self.cols, self.rows, c, r)
                 ctx.set_view(Mp, self.pw, self.ph, w.step)
                 ctx.set_viewport(c * self.pw, r * self.ph, self.W)
-                ids = ctx.sort_bricks(vr.MODE_EA)
-                parts, n, nbytes = ctx.partial_layout(vr.MODE_EA, ids)
+                ids = ctx.sort_bricks(self.mode)
+                parts, n, nbytes = ctx.partial_layout(self.mode, ids)
                 vr.Context.bind_partials(parts, n, self._arena(nbytes))
                 if timed_events:
                     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                     e0.record()
-                ctx.render_bricks(vr.MODE_EA, parts, n, w.tau)
+                ctx.render_bricks(self.mode, parts, n, w.tau)
                 if timed_events:
                     e1.record()
                     self.march_events.append((e0, e1))
                     # algorithmic bytes of this launch: the active in-frustum bricks
                     # read once + the partial images written once
-                    self.alg_bytes += 4 * brick_vox * n + nbytes
-                ctx.composite_bricks(vr.MODE_EA, parts, n, self.frame, self.bg)
+                    self.alg_bytes += 4 * brick_vox * n + nbytes          # nbytes: the partial images (16 or 4 B per pixel)
+                ctx.composite_bricks(self.mode, parts, n, self.frame, self.bg)
+        if timed_events:
+            e = torch.cuda.Event(enable_timing=True)
+            e.record()
+            self.step_events.append(e)
 
 
 def oracle_sample(job, frame_index, tile, precision_name="F64"):
@@ -191,7 +199,8 @@ def oracle_sample(job, frame_index, tile, precision_name="F64"):
     torch.cuda.synchronize()
     vol = ovr.Volume(w.dims, brick, bricks)
     t0 = time.perf_counter()
-    _, _, cnt = ovr.render(vol, M, job.W, job.H, w.step, ovr.EA, getattr(ovr, precision_name), tf=job.tf,
+    omode = ovr.EA if job.mode == job.vr.MODE_EA else ovr.MIP
+    _, _, cnt = ovr.render(vol, M, job.W, job.H, w.step, omode, getattr(ovr, precision_name), tf=job.tf,
                            split=ovr.SPLIT_SORTLAST, partition=brick, tau=w.tau, bg=job.bg, pixels=pix)
     return time.perf_counter() - t0, cnt, len(touched)
 
@@ -203,6 +212,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="C3", choices=sorted(wl.CONFIGS))
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--mode", default="ea", choices=["ea", "mip"], help="emission-absorption (default) or MIP")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
@@ -223,11 +233,11 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     w = wl.CONFIGS[args.workload]
-    job = Job(w, local_rank)
+    job = Job(w, local_rank, args.mode)
     vr = job.vr
     config = {"workload": f"{w.name}: {w.dims[0]}x{w.dims[1]}x{w.dims[2]} float32 cube, {w.brick[0]}^3 bricks, "
                           f"{w.frame[0]}x{w.frame[1]} frame ({w.panels[0]}x{w.panels[1]} panels), step {w.step}, "
-                          f"EA tf-{w.tf} tau={w.tau}, sort-last path, orbit frames spread over 360 deg",
+                          f"{'EA tf-' + w.tf + ' tau=' + str(w.tau) if args.mode == 'ea' else 'MIP'}, sort-last path, orbit frames spread over 360 deg",
               "cube_gib": round(w.n_voxels * 4 / 2 ** 30, 3), "n_sources": w.n_sources,
               "l2_policy": "inputs larger than L2 (cube >> 126 MB); no explicit flush",
               "replicas": world, "generate_seconds": round(job.gen_seconds, 3)}
@@ -254,6 +264,8 @@ def main():
     barrier()
     clocks = sampler.result()
     ms_total = ev0.elapsed_time(ev1)
+    marks = [ev0] + job.step_events
+    frame_ms = sorted(a.elapsed_time(b) for a, b in zip(marks, marks[1:]))
     cnt = job.ctx.get_counters()
     march_ms = sum(a.elapsed_time(b) for a, b in job.march_events)
     n_march = len(job.march_events)
@@ -282,9 +294,12 @@ def main():
 
     peaks, peak_src = measured_peaks()
     peak = float(peaks["hbm_gbs"])
-    plan = job.ctx.get_plan(vr.MODE_EA)
+    plan = job.ctx.get_plan(job.mode)
     kernel = MARCHER.get((plan["variant"], plan["skip_level"]),
                          "render_ls_kernel<EA> (lockstep, cp.async gather)" if plan["variant"] == 3 else "render_bricks_kernel<EA>")
+    if args.mode == "mip":
+        kernel = ("render_ls_kernel<MIP> (lockstep, cp.async gather, warp-reduced maximum)" if plan["variant"] == 3
+                  else "render_bricks_kernel<MIP> (ray per thread)")
     traffic = NCU_TRAFFIC_BYTES.get(w.name)
     launch_s = march_ms / max(n_march, 1) * 1e-3
     achieved = (job.alg_bytes / max(n_march, 1)) / (march_ms / max(n_march, 1) * 1e-3) / 1e9 if march_ms > 0 else 0.0
@@ -306,6 +321,8 @@ def main():
         "metric": METRIC, "value": nominal / (ms_total * 1e-3), "unit": "samples/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "frames_per_s": args.steps * world / (ms_total * 1e-3),
+        "frame_ms": {"median": frame_ms[len(frame_ms) // 2], "p95": frame_ms[min(len(frame_ms) - 1, int(0.95 * len(frame_ms)))],
+                     "min": frame_ms[0], "max": frame_ms[-1], "note": "rank 0, device time between consecutive frames of the orbit"},
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": config,
         "nominal_samples_per_step": nominal / (args.steps * world),
@@ -314,7 +331,7 @@ def main():
         "clocks": clocks,
         "e2e": {"value": e2e_nominal / e2e_s, "unit": "samples/s", "ms_per_step": e2e_s * 1e3 / args.steps,
                 "h2d_bytes_per_step": (64 + 4096 + 8) * job.cols * job.rows,
-                "d2h_bytes_per_step": job.H * job.W * 16},
+                "d2h_bytes_per_step": job.H * job.W * job.px_bytes},
         "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak,
                      "unit": "GB/s", "frac": achieved / peak if peak else None, "traffic": traffic,
                      "peak_source": peak_src, "launch_ms": march_ms / max(n_march, 1),

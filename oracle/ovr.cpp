@@ -615,4 +615,88 @@ int ovr_generate(uint64_t seed, int nx, int ny, int nz, int x0, int y0, int z0, 
     return OVR_OK;
 }
 
+// ---- O-14 catalogue overlay (section 2), see ovr.h for the rule.
+int ovr_overlay(const ovr_view* view, const int* boxes, int n, const uint8_t* visible, int32_t* pick) {
+    if (!view || !pick || n < 0 || (n > 0 && !boxes) || view->width <= 0 || view->height <= 0) return OVR_ERR_ARG;
+    const int W = view->width, H = view->height;
+    for (long long i = 0; i < (long long)W * H; ++i) pick[i] = 0;
+    double M[16];
+    for (int i = 0; i < 16; ++i) M[i] = (double)view->m[i];
+    for (int b = 0; b < n; ++b) {                            // ascending id: the highest id stays on a pixel
+        if (visible && !visible[b]) continue;
+        const int* B = boxes + 6 * b;
+        for (int a = 0; a < 3; ++a) {                        // the 4 edges parallel to axis a
+            for (int c = 0; c < 4; ++c) {
+                int lo[3], hi[3];
+                const int a1 = (a + 1) % 3, a2 = (a + 2) % 3;
+                lo[a] = B[2 * a]; hi[a] = B[2 * a + 1];
+                lo[a1] = hi[a1] = (c & 1) ? B[2 * a1 + 1] : B[2 * a1];
+                lo[a2] = hi[a2] = (c & 2) ? B[2 * a2 + 1] : B[2 * a2];
+                double P[2][4];                              // clip coordinates of the two ends
+                for (int e = 0; e < 2; ++e) {
+                    const double x = e ? hi[0] : lo[0], y = e ? hi[1] : lo[1], z = e ? hi[2] : lo[2];
+                    for (int r = 0; r < 4; ++r) P[e][r] = ((M[4 * r] * x + M[4 * r + 1] * y) + M[4 * r + 2] * z) + M[4 * r + 3];
+                }
+                double t0 = 0.0, t1 = 1.0;
+                bool out = false;
+                for (int pl = 0; pl < 7 && !out; ++pl) {     // f(P) >= 0 keeps the point
+                    double f[2];
+                    for (int e = 0; e < 2; ++e) {
+                        const double x = P[e][0], y = P[e][1], z = P[e][2], w = P[e][3];
+                        switch (pl) {
+                            case 0: f[e] = w - 1e-9; break;
+                            case 1: f[e] = z + w; break;
+                            case 2: f[e] = w - z; break;
+                            case 3: f[e] = x + 2.0 * w; break;
+                            case 4: f[e] = 2.0 * w - x; break;
+                            case 5: f[e] = y + 2.0 * w; break;
+                            default: f[e] = 2.0 * w - y; break;
+                        }
+                    }
+                    if (f[0] < 0.0 && f[1] < 0.0) { out = true; break; }
+                    if (f[0] < 0.0) t0 = std::fmax(t0, f[0] / (f[0] - f[1]));
+                    if (f[1] < 0.0) t1 = std::fmin(t1, f[0] / (f[0] - f[1]));
+                }
+                if (out || !(t0 <= t1)) continue;
+                double px[2], py[2];
+                for (int e = 0; e < 2; ++e) {
+                    const double t = e ? t1 : t0;
+                    const double x = P[0][0] + (P[1][0] - P[0][0]) * t, y = P[0][1] + (P[1][1] - P[0][1]) * t;
+                    const double w = P[0][3] + (P[1][3] - P[0][3]) * t;
+                    px[e] = ((x / w) + 1.0) * 0.5 * (double)W - 0.5;
+                    py[e] = (1.0 - (y / w)) * 0.5 * (double)H - 0.5;
+                }
+                const double dx = px[1] - px[0], dy = py[1] - py[0];
+                const double len = std::ceil(std::fmax(std::fabs(dx), std::fabs(dy)));
+                if (!(len < 1.0e7)) continue;                // non-finite projection
+                const int ns = len < 1.0 ? 1 : (int)len;
+                for (int s = 0; s <= ns; ++s) {
+                    const double t = (double)s / (double)ns;
+                    const double X = px[0] + dx * t, Y = py[0] + dy * t;
+                    const double fi = std::floor(X + 0.5), fj = std::floor(Y + 0.5);
+                    if (!(fi >= 0.0 && fi < (double)W && fj >= 0.0 && fj < (double)H)) continue;
+                    int32_t& q = pick[(long long)fj * W + (long long)fi];
+                    if (q < b + 1) q = b + 1;
+                }
+            }
+        }
+    }
+    return OVR_OK;
+}
+
+int ovr_overlay_pick(const int32_t* pick, int width, int height, int x, int y, int radius) {
+    long long best_d = -1;
+    int best = -1;
+    for (int dy = -radius; dy <= radius; ++dy)
+        for (int dx = -radius; dx <= radius; ++dx) {
+            const int i = x + dx, j = y + dy;
+            if (i < 0 || j < 0 || i >= width || j >= height) continue;
+            const int id = pick[(long long)j * width + i] - 1;
+            if (id < 0) continue;
+            const long long d = (long long)dx * dx + (long long)dy * dy;
+            if (best_d < 0 || d < best_d || (d == best_d && id > best)) { best_d = d; best = id; }
+        }
+    return best;
+}
+
 }  // extern "C"

@@ -107,6 +107,22 @@ int ovr_generate(uint64_t seed, int nx, int ny, int nz, int x0, int y0, int z0, 
 /* The N(0,1) noise value of linear voxel index idx (fp64). */
 double ovr_noise(uint64_t seed, uint64_t idx);
 
+
+/* O-14 catalogue overlay (section 2: a source finder's catalogue is "a set
+ * of detected astronomical sources represented by their bounding cubes ... superimposed as
+ * wireframe boxes on the volume rendering output", moving with the view, selectable, with groups
+ * shown / hidden).  boxes = n x 6 ints (xlo xhi ylo yhi zlo zhi, voxel coordinates, inclusive);
+ * visible = n bytes or NULL (all shown).  pick = width*height ints, row-major, row 0 on top:
+ * 0 where no edge passes, else 1 + the HIGHEST id of the boxes whose wireframe covers the pixel.
+ * Rule (O-14): the 12 edges of every shown box are projected with M in fp64, clipped in
+ * clip space to w >= 1e-9, |z| <= w and a guard band |x|,|y| <= 2w, mapped to pixel coordinates
+ * px = (xn+1) W/2 - 1/2, py = (1-yn) H/2 - 1/2 and sampled at n+1 equidistant points,
+ * n = max(1, ceil(max(|dpx|,|dpy|))), each rounded to the nearest pixel (floor(v + 1/2)). */
+int ovr_overlay(const ovr_view* view, const int* boxes, int n, const uint8_t* visible, int32_t* pick);
+/* The box to select for a click at pixel (x, y): among the covered pixels of the square window of
+ * half-width `radius` the one at the smallest Euclidean distance (ties: the larger id); -1 if none. */
+int ovr_overlay_pick(const int32_t* pick, int width, int height, int x, int y, int radius);
+
 #ifdef __cplusplus
 }
 #endif

@@ -233,3 +233,30 @@ def generate(seed, dims, region=None, sources=None, zero_boxes=None, continuum=0
                             out.ctypes.data_as(C.POINTER(C.c_float)))
     _check(rc, "generate")
     return out
+
+
+def overlay(M, W, H, boxes, visible=None):
+    """O-14 catalogue overlay: pick image [H, W] int32, 0 = no edge, else 1 + highest box id."""
+    L = lib()
+    B = np.ascontiguousarray(boxes, dtype=np.int32).reshape(-1, 6)
+    vis = None if visible is None else np.ascontiguousarray(visible, dtype=np.uint8)
+    pick = np.zeros((H, W), dtype=np.int32)
+    v = _view(M, W, H, 1.0)
+    _check(L.ovr_overlay(C.byref(v), B.ctypes.data_as(C.c_void_p), int(B.shape[0]),
+                         vis.ctypes.data_as(C.c_void_p) if vis is not None else None,
+                         pick.ctypes.data_as(C.c_void_p)), "ovr_overlay")
+    return pick
+
+
+def overlay_pick(pick, x, y, radius):
+    L = lib()
+    p = np.ascontiguousarray(pick, dtype=np.int32)
+    return int(L.ovr_overlay_pick(p.ctypes.data_as(C.c_void_p), int(p.shape[1]), int(p.shape[0]), int(x), int(y), int(radius)))
+
+
+def overlay_apply(frame, pick, colours):
+    """Opaque wireframe: covered pixels take the colour of their box (numpy, trivial)."""
+    out = np.array(frame, dtype=np.float32, copy=True)
+    m = pick > 0
+    out[m] = np.asarray(colours, dtype=np.float32).reshape(-1, 4)[pick[m] - 1]
+    return out

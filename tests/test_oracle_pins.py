@@ -475,3 +475,111 @@ def test_generator_sources_and_determinism(ovr):
     zb = np.array([[0, 31, 32, 63, 64, 95]], dtype=np.int32)
     z = ovr.generate(w.seed, w.dims, sources=S, zero_boxes=zb)
     assert (z[64:96, 32:64, 0:32] == 0).all() and np.array_equal(z[:64], full[:64])
+
+
+# ------------------------------------------------------------------ O-14 catalogue overlay
+def _brute_edge_points(M, W, H, box, per_edge=6000):
+    """Independent of the oracle's DDA: dense points along the 12 edges of a box in 3-D, kept where
+    the clip-space point is inside near/far, projected to pixel coordinates (numpy fp64)."""
+    M = np.asarray(M, dtype=np.float64).reshape(4, 4)
+    xs, ys, zs = (box[0], box[1]), (box[2], box[3]), (box[4], box[5])
+    pts = []
+    t = np.linspace(0.0, 1.0, per_edge)[:, None]
+    for a in range(3):
+        for c in range(4):
+            lo, hi = [0, 0, 0], [0, 0, 0]
+            a1, a2 = (a + 1) % 3, (a + 2) % 3
+            rng = (xs, ys, zs)
+            lo[a], hi[a] = rng[a]
+            lo[a1] = hi[a1] = rng[a1][c & 1]
+            lo[a2] = hi[a2] = rng[a2][(c >> 1) & 1]
+            p = np.array(lo, float)[None] * (1 - t) + np.array(hi, float)[None] * t
+            clip = np.c_[p, np.ones(len(p))] @ M.T
+            ok = (clip[:, 3] > 1e-9) & (np.abs(clip[:, 2]) <= clip[:, 3])
+            clip = clip[ok]
+            if len(clip):
+                px = (clip[:, 0] / clip[:, 3] + 1) * 0.5 * W - 0.5
+                py = (1 - clip[:, 1] / clip[:, 3]) * 0.5 * H - 0.5
+                pts.append(np.c_[px, py])
+    return np.concatenate(pts) if pts else np.zeros((0, 2))
+
+
+def _check_against_brute(pick, pts, ident):
+    H, W = pick.shape
+    drawn = np.argwhere(pick == ident)[:, ::-1].astype(np.float64)         # (x, y)
+    inside = pts[(pts[:, 0] > -0.49) & (pts[:, 0] < W - 0.51) & (pts[:, 1] > -0.49) & (pts[:, 1] < H - 0.51)]
+    assert len(drawn) > 0 and len(inside) > 0
+    # every drawn pixel hugs an edge: within half a pixel diagonal (+ the brute sampling pitch)
+    d = np.sqrt(((drawn[:, None, :] - inside[None, ::7, :]) ** 2).sum(-1)).min(axis=1)
+    assert d.max() <= 0.5 * np.sqrt(2.0) + 0.2, d.max()
+    # no gaps: the DDA steps the major axis by <= 1, so a point of an edge is within 1/2 (along the
+    # major axis) of a sample, whose pixel is within 1/2 per axis of it: sqrt(1 + 1/4).  Points closer
+    # than a pixel to the viewport border are left out (their sample may round outside).
+    sub = inside[(inside[:, 0] > 0.5) & (inside[:, 0] < W - 1.5) & (inside[:, 1] > 0.5) & (inside[:, 1] < H - 1.5)][::11]
+    d2 = np.sqrt(((sub[:, None, :] - drawn[None, :, :]) ** 2).sum(-1)).min(axis=1)
+    assert d2.max() <= math.sqrt(1.25) + 1e-9, d2.max()
+
+
+def test_overlay_axis_view_draws_exact_rectangles(ovr):
+    dims = (48, 40, 56)
+    M, (W, H) = wl.axis_ortho_camera(dims, axis=2, sign=+1)
+    boxes = np.array([[5, 20, 7, 30, 3, 50], [25, 25, 10, 12, 0, 55]], dtype=np.int32)    # the 2nd is 1 voxel wide
+    pick = ovr.overlay(M, W, H, boxes)
+    want = np.zeros((H, W), dtype=np.int32)
+    for b, (x0, x1, y0, y1, _, _) in enumerate(boxes):
+        want[y0, x0:x1 + 1] = np.maximum(want[y0, x0:x1 + 1], b + 1)
+        want[y1, x0:x1 + 1] = np.maximum(want[y1, x0:x1 + 1], b + 1)
+        want[y0:y1 + 1, x0] = np.maximum(want[y0:y1 + 1, x0], b + 1)
+        want[y0:y1 + 1, x1] = np.maximum(want[y0:y1 + 1, x1], b + 1)
+    assert np.array_equal(pick, want)
+
+
+@pytest.mark.parametrize("az", [10.0, 135.0])
+def test_overlay_perspective_hugs_projected_edges(ovr, az):
+    dims = (96, 80, 160)
+    W, H = 320, 180
+    M = wl.perspective_camera(dims, (W, H), azimuth_deg=az)
+    boxes = np.array([[10, 40, 12, 30, 20, 90], [50, 90, 40, 75, 100, 150]], dtype=np.int32)
+    for b in range(2):
+        vis = np.zeros(2, np.uint8)
+        vis[b] = 1
+        pick = ovr.overlay(M, W, H, boxes, vis)
+        assert set(np.unique(pick)) == {0, b + 1}
+        _check_against_brute(pick, _brute_edge_points(M, W, H, boxes[b]), b + 1)
+
+
+def test_overlay_clips_at_the_near_plane(ovr):
+    dims = (64, 64, 64)
+    W, H = 200, 120
+    # eye inside the cube looking along +z: boxes behind the eye vanish, a box around the eye is clipped
+    eye = np.array([31.5, 31.5, 20.0])
+    V = wl._look_at(eye, eye + np.array([0.0, 0.0, 1.0]), np.array([0.0, 1.0, 0.0]))
+    top = 0.5 * math.tan(math.radians(30.0))
+    M = (wl._frustum(-top * W / H, top * W / H, -top, top, 0.5, 200.0) @ V).astype(np.float32)
+    behind = np.array([[10, 50, 10, 50, 0, 15]], dtype=np.int32)
+    assert not ovr.overlay(M, W, H, behind).any()
+    straddle = np.array([[20, 44, 22, 40, 5, 45]], dtype=np.int32)
+    pick = ovr.overlay(M, W, H, straddle)
+    _check_against_brute(pick, _brute_edge_points(M, W, H, straddle[0], per_edge=40000), 1)
+
+
+def test_overlay_priority_visibility_and_pick(ovr):
+    dims = (64, 64, 64)
+    M, (W, H) = wl.axis_ortho_camera(dims, axis=2, sign=+1)
+    boxes = np.array([[10, 30, 10, 30, 0, 10], [20, 40, 20, 40, 0, 10]], dtype=np.int32)
+    both = ovr.overlay(M, W, H, boxes)
+    assert both[20, 30] == 2 and both[30, 20] == 2          # crossings of the two outlines: the higher id wins
+    only0 = ovr.overlay(M, W, H, boxes, np.array([1, 0], np.uint8))
+    assert only0[20, 30] == 1 and only0[30, 20] == 1 and not (only0 == 2).any()
+    assert not ovr.overlay(M, W, H, boxes, np.zeros(2, np.uint8)).any()
+    assert np.array_equal(ovr.overlay(M, W, H, boxes, np.ones(2, np.uint8)), both)
+    # pick: nearest covered pixel, ties to the larger id, -1 when nothing is near
+    assert ovr.overlay_pick(both, 12, 15, 3) == 0            # 2 px right of box 0's left side
+    assert ovr.overlay_pick(both, 38, 35, 3) == 1
+    assert ovr.overlay_pick(both, 25, 25, 3) == -1           # inside both outlines, 5 px from any edge
+    assert ovr.overlay_pick(both, 25, 25, 5) == 1            # box 0's side x=30 and box 1's side x=20 both at 5: tie
+    assert ovr.overlay_pick(both, 60, 60, 4) == -1
+    colours = np.array([[1, 0, 0, 1], [0, 1, 0, 1]], np.float32)
+    frame = ovr.overlay_apply(np.full((H, W, 4), 0.25, np.float32), both, colours)
+    assert np.array_equal(frame[10, 15], colours[0]) and np.array_equal(frame[20, 30], colours[1])
+    assert np.array_equal(frame[0, 0], np.full(4, 0.25, np.float32))
