@@ -155,6 +155,28 @@ int vr_window_layout(int nx, int ny, int nz, int bx, int by, int bz, int first_b
  * vr_composite_bricks equals the fold over all bricks up to float32 reassociation (MIP: exactly). */
 int vr_sort_groups(vr_ctx* ctx, const int* h_group_first, int n_groups, int* h_group_order);
 
+/* ---- catalogue overlay (section 2: a source finder's
+ *      output, "a set of detected astronomical sources represented by their bounding cubes",
+ *      "superimposed as wireframe boxes on the volume rendering output"; "the user interaction
+ *      with the displayed volume rendering output is automatically applied to the displayed source
+ *      cubes"; a source can be selected; groups can be shown / hidden; catalogues can be told apart
+ *      by colour).  Reading O-14 in DESIGN.md states the rasterisation rule. ------------------- */
+typedef struct {
+    const int* d_boxes;             /* device: n x 6 ints xlo xhi ylo yhi zlo zhi, voxel coordinates, inclusive */
+    const float* d_colours;         /* device: n x 4 floats (r,g,b,a), 16-byte aligned; may be NULL if no frame is painted */
+    const unsigned char* d_visible; /* device: n bytes, 0 = hidden; NULL = all shown */
+    int n;
+} vr_catalogue;
+/* Draw the wireframes of the shown boxes under the current view into the viewport of d_pick
+ * (ints, same pitch and placement as the frame: 0 = no edge, else 1 + the highest id of the boxes
+ * covering the pixel; the viewport is cleared first) and, if d_frame_rgba != NULL, paint the
+ * covered pixels of the frame with their box's colour (opaque, depth-unaware). */
+int vr_overlay_catalogue(vr_ctx* ctx, const vr_catalogue* cat, float* d_frame_rgba, int* d_pick, void* stream);
+/* The box to select for a click at view pixel (x, y): among the covered pixels of the square
+ * window of half-width radius (<= 64) the one at the smallest Euclidean distance, ties to the
+ * larger id; *box = -1 if none.  Synchronises `stream`. */
+int vr_overlay_pick(vr_ctx* ctx, const int* d_pick, int x, int y, int radius, int* box, void* stream);
+
 /* ---- counters (SURVEY.md section 5 "metrics") ---------------------------------------------- */
 typedef struct {
     int64_t rays;             /* rays that had at least one lattice sample inside the cube */

@@ -818,6 +818,31 @@ int vr_reset_counters(vr_ctx* ctx, void* stream) {
     return VR_OK;
 }
 
+int vr_overlay_catalogue(vr_ctx* ctx, const vr_catalogue* cat, float* d_frame_rgba, int* d_pick, void* stream) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (!ctx->has_view) return fail(ctx, VR_ERR_STATE, "no view: call vr_set_view first");
+    if (!cat || !d_pick || cat->n < 0 || (cat->n > 0 && (!cat->d_boxes || (d_frame_rgba && !cat->d_colours))))
+        return fail(ctx, VR_ERR_INVALID_ARG, "vr_overlay_catalogue: bad argument");
+    if (d_frame_rgba && ((uintptr_t)d_frame_rgba & 15) != 0) return fail(ctx, VR_ERR_INVALID_ARG, "vr_overlay_catalogue: frame must be 16-byte aligned");
+    VR_CUDA(ctx, launch_overlay(ctx->view, ctx->M, cat->d_boxes, cat->d_colours, cat->d_visible, cat->n, d_frame_rgba, d_pick,
+                                (cudaStream_t)stream));
+    ctx->launches += cat->n > 0 ? (d_frame_rgba ? 3 : 2) : 1;
+    return VR_OK;
+}
+
+int vr_overlay_pick(vr_ctx* ctx, const int* d_pick, int x, int y, int radius, int* box, void* stream) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (!ctx->has_view) return fail(ctx, VR_ERR_STATE, "no view: call vr_set_view first");
+    if (!d_pick || !box || radius < 0 || radius > 64) return fail(ctx, VR_ERR_INVALID_ARG, "vr_overlay_pick: bad argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    int* d_out = reinterpret_cast<int*>(ctx->d_scratch);
+    VR_CUDA(ctx, launch_overlay_pick(ctx->view, d_pick, x, y, radius, d_out, s));
+    ctx->launches += 1;
+    VR_CUDA(ctx, cudaMemcpyAsync(box, d_out, sizeof(int), cudaMemcpyDeviceToHost, s));
+    VR_CUDA(ctx, cudaStreamSynchronize(s));
+    return VR_OK;
+}
+
 int vr_get_plan(vr_ctx* ctx, int mode, int out[3], void* stream) {
     int rc = check_render_state(ctx, mode == VR_MODE_EA);
     if (rc) return rc;

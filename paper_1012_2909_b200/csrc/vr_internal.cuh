@@ -114,6 +114,9 @@ cudaError_t launch_composite(const ViewDesc& v, int mode, const PartialDev* d_pa
 cudaError_t launch_classify_cells(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale,
                                   unsigned long long* d_active_count, cudaStream_t s);
 cudaError_t launch_classify_occ(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale, cudaStream_t s);
+cudaError_t launch_overlay(const ViewDesc& v, const double M[16], const int* d_boxes, const float* d_colours,
+                           const unsigned char* d_visible, int n, float* d_frame, int* d_pick, cudaStream_t s);
+cudaError_t launch_overlay_pick(const ViewDesc& v, const int* d_pick, int x, int y, int radius, int* d_out, cudaStream_t s);
 cudaError_t launch_upload_table(float4* d_dst, const float* h_src_1024, cudaStream_t s);
 
 }  // namespace vr

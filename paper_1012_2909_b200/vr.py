@@ -24,7 +24,7 @@ EXPORTS = [
     "vr_set_viewport", "vr_set_transfer_function", "vr_render_mip", "vr_render_ea",
     "vr_sort_bricks", "vr_partial_layout", "vr_render_bricks", "vr_composite_bricks",
     "vr_get_counters", "vr_reset_counters", "vr_set_option", "vr_get_plan",
-    "vr_set_brick_window", "vr_window_layout", "vr_sort_groups",
+    "vr_set_brick_window", "vr_window_layout", "vr_sort_groups", "vr_overlay_catalogue", "vr_overlay_pick",
 ]
 
 
@@ -43,6 +43,10 @@ class GenParams(C.Structure):
 class Partial(C.Structure):
     _fields_ = [("brick", C.c_int), ("x0", C.c_int), ("y0", C.c_int), ("w", C.c_int), ("h", C.c_int),
                 ("d_data", C.c_void_p), ("pitch_px", C.c_size_t)]
+
+
+class Catalogue(C.Structure):
+    _fields_ = [("d_boxes", C.c_void_p), ("d_colours", C.c_void_p), ("d_visible", C.c_void_p), ("n", C.c_int)]
 
 
 class Counters(C.Structure):
@@ -89,6 +93,8 @@ def load():
     lib.vr_set_brick_window.argtypes = [vp, C.c_int, C.c_int]
     lib.vr_window_layout.argtypes = [C.c_int] * 8 + [C.POINTER(sz), C.POINTER(sz)]
     lib.vr_sort_groups.argtypes = [vp, ip, C.c_int, ip]
+    lib.vr_overlay_catalogue.argtypes = [vp, C.POINTER(Catalogue), vp, vp, vp]
+    lib.vr_overlay_pick.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, ip, vp]
     _lib = lib
     return lib
 
@@ -260,6 +266,21 @@ class Context:
         self._check(self._lib.vr_sort_groups(self._h, g.ctypes.data_as(C.POINTER(C.c_int)), int(g.size - 1),
                                              order.ctypes.data_as(C.POINTER(C.c_int))))
         return order
+
+    def overlay_catalogue(self, d_boxes, d_colours, d_visible, d_frame, d_pick, stream=None):
+        """d_boxes: int32 CUDA tensor [n, 6]; d_colours: float32 [n, 4] or None; d_visible: uint8 [n] or None."""
+        cat = Catalogue(d_boxes.data_ptr() if d_boxes is not None and d_boxes.numel() else None,
+                        d_colours.data_ptr() if d_colours is not None and d_colours.numel() else None,
+                        d_visible.data_ptr() if d_visible is not None else None,
+                        int(d_boxes.shape[0]) if d_boxes is not None else 0)
+        self._check(self._lib.vr_overlay_catalogue(self._h, C.byref(cat), C.c_void_p(d_frame.data_ptr()) if d_frame is not None else None,
+                                                   C.c_void_p(d_pick.data_ptr()), _stream(stream)))
+
+    def overlay_pick(self, d_pick, x, y, radius, stream=None):
+        box = C.c_int(-1)
+        self._check(self._lib.vr_overlay_pick(self._h, C.c_void_p(d_pick.data_ptr()), int(x), int(y), int(radius), C.byref(box),
+                                              _stream(stream)))
+        return box.value
 
     def set_option(self, option, value):
         self._check(self._lib.vr_set_option(self._h, int(option), int(value)))
