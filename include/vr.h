@@ -177,6 +177,26 @@ int vr_overlay_catalogue(vr_ctx* ctx, const vr_catalogue* cat, float* d_frame_rg
  * larger id; *box = -1 if none.  Synchronises `stream`. */
 int vr_overlay_pick(vr_ctx* ctx, const int* d_pick, int x, int y, int radius, int* box, void* stream);
 
+/* ---- output pyramid (section 3: "The rendering output is
+ *      stored in TIFF format, which is converted to the pyramidal tiled TIFF format").  The TIFF
+ *      container is the client's; this is its pixel content in a device buffer (O-15):
+ *      level 0 = the frame quantised to RGBA8, q = floor(clamp(c,0,1) * 255 + 1/2); level l+1 = 2 x 2
+ *      box reduction (mean of the up to 4 pixels, rounded half up), ceil(w/2) x ceil(h/2); levels
+ *      until one tile holds the image; each level as tile x tile tiles (tile a power of two in
+ *      [16, 4096]), row-major over the tiles, each tile contiguous, edge tiles zero padded. ------ */
+#define VR_PYRAMID_MAX_LEVELS 32
+typedef struct {
+    int width, height;   /* pixels of the level */
+    int tiles_x, tiles_y;
+    size_t offset;       /* bytes from the start of the buffer to the level's first tile */
+} vr_pyramid_level;
+/* Sizes: levels[] needs room for VR_PYRAMID_MAX_LEVELS entries; *bytes = the whole buffer. */
+int vr_pyramid_layout(int width, int height, int tile, int* n_levels, vr_pyramid_level* levels, size_t* bytes);
+/* d_frame_rgba: device, float4 pixels, rows pitch_px apart (e.g. the 9600 x 5400 tiled-display
+ * frame); d_out: device, *bytes of vr_pyramid_layout, caller-owned. */
+int vr_build_pyramid(vr_ctx* ctx, const float* d_frame_rgba, int width, int height, size_t pitch_px, int tile,
+                     void* d_out, void* stream);
+
 /* ---- counters (SURVEY.md section 5 "metrics") ---------------------------------------------- */
 typedef struct {
     int64_t rays;             /* rays that had at least one lattice sample inside the cube */

@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libvr.so")
-SOURCES = ["vr_api.cu", "vr_cube.cu", "vr_march.cu", "vr_composite.cu", "vr_overlay.cu"]
+SOURCES = ["vr_api.cu", "vr_cube.cu", "vr_march.cu", "vr_composite.cu", "vr_overlay.cu", "vr_pyramid.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--fmad=false", "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall", "-shared",
               "-Xptxas", "-v"]

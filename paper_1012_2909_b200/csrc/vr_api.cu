@@ -843,6 +843,26 @@ int vr_overlay_pick(vr_ctx* ctx, const int* d_pick, int x, int y, int radius, in
     return VR_OK;
 }
 
+int vr_pyramid_layout(int width, int height, int tile, int* n_levels, vr_pyramid_level* levels, size_t* bytes) {
+    if (width <= 0 || height <= 0 || tile < 16 || tile > 4096 || (tile & (tile - 1)) != 0 || !n_levels || !levels || !bytes) return VR_ERR_INVALID_ARG;
+    const int n = pyramid_levels(width, height, tile, levels, bytes);
+    if (n < 0) return VR_ERR_INVALID_ARG;
+    *n_levels = n;
+    return VR_OK;
+}
+
+int vr_build_pyramid(vr_ctx* ctx, const float* d_frame_rgba, int width, int height, size_t pitch_px, int tile, void* d_out, void* stream) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    if (!d_frame_rgba || !d_out || width <= 0 || height <= 0 || pitch_px < (size_t)width || tile < 16 || tile > 4096 ||
+        (tile & (tile - 1)) != 0 || ((uintptr_t)d_frame_rgba & 15) != 0 || ((uintptr_t)d_out & 3) != 0)
+        return fail(ctx, VR_ERR_INVALID_ARG, "vr_build_pyramid: bad argument");
+    int launches = 0;
+    cudaError_t e = launch_pyramid(d_frame_rgba, width, height, (long long)pitch_px, tile, d_out, &launches, (cudaStream_t)stream);
+    ctx->launches += launches;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "vr_build_pyramid");
+    return VR_OK;
+}
+
 int vr_get_plan(vr_ctx* ctx, int mode, int out[3], void* stream) {
     int rc = check_render_state(ctx, mode == VR_MODE_EA);
     if (rc) return rc;

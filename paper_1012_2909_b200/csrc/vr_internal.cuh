@@ -117,6 +117,9 @@ cudaError_t launch_classify_occ(const CubeDesc& c, const int nz_prefix[257], flo
 cudaError_t launch_overlay(const ViewDesc& v, const double M[16], const int* d_boxes, const float* d_colours,
                            const unsigned char* d_visible, int n, float* d_frame, int* d_pick, cudaStream_t s);
 cudaError_t launch_overlay_pick(const ViewDesc& v, const int* d_pick, int x, int y, int radius, int* d_out, cudaStream_t s);
+int pyramid_levels(int width, int height, int tile, vr_pyramid_level* lv, size_t* bytes);
+cudaError_t launch_pyramid(const float* d_frame, int width, int height, long long pitch, int tile, void* d_out, int* launches,
+                           cudaStream_t s);
 cudaError_t launch_upload_table(float4* d_dst, const float* h_src_1024, cudaStream_t s);
 
 }  // namespace vr

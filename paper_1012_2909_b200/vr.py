@@ -24,7 +24,7 @@ EXPORTS = [
     "vr_set_viewport", "vr_set_transfer_function", "vr_render_mip", "vr_render_ea",
     "vr_sort_bricks", "vr_partial_layout", "vr_render_bricks", "vr_composite_bricks",
     "vr_get_counters", "vr_reset_counters", "vr_set_option", "vr_get_plan",
-    "vr_set_brick_window", "vr_window_layout", "vr_sort_groups", "vr_overlay_catalogue", "vr_overlay_pick",
+    "vr_set_brick_window", "vr_window_layout", "vr_sort_groups", "vr_overlay_catalogue", "vr_overlay_pick", "vr_pyramid_layout", "vr_build_pyramid",
 ]
 
 
@@ -47,6 +47,10 @@ class Partial(C.Structure):
 
 class Catalogue(C.Structure):
     _fields_ = [("d_boxes", C.c_void_p), ("d_colours", C.c_void_p), ("d_visible", C.c_void_p), ("n", C.c_int)]
+
+
+class PyramidLevel(C.Structure):
+    _fields_ = [("width", C.c_int), ("height", C.c_int), ("tiles_x", C.c_int), ("tiles_y", C.c_int), ("offset", C.c_size_t)]
 
 
 class Counters(C.Structure):
@@ -95,6 +99,8 @@ def load():
     lib.vr_sort_groups.argtypes = [vp, ip, C.c_int, ip]
     lib.vr_overlay_catalogue.argtypes = [vp, C.POINTER(Catalogue), vp, vp, vp]
     lib.vr_overlay_pick.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, ip, vp]
+    lib.vr_pyramid_layout.argtypes = [C.c_int, C.c_int, C.c_int, ip, C.POINTER(PyramidLevel), C.POINTER(sz)]
+    lib.vr_build_pyramid.argtypes = [vp, vp, C.c_int, C.c_int, sz, C.c_int, vp, vp]
     _lib = lib
     return lib
 
@@ -128,6 +134,16 @@ def window_layout(dims, brick, first_brick, end_brick):
     if rc != OK:
         raise VRError(rc, "vr_window_layout: invalid argument")
     return cb.value, mb.value
+
+
+def pyramid_layout(width, height, tile=256):
+    """[(width, height, tiles_x, tiles_y, offset), ...] and the bytes of the whole pyramid buffer."""
+    lv = (PyramidLevel * 32)()
+    n, nbytes = C.c_int(0), C.c_size_t(0)
+    rc = load().vr_pyramid_layout(int(width), int(height), int(tile), C.byref(n), lv, C.byref(nbytes))
+    if rc != OK:
+        raise VRError(rc, "vr_pyramid_layout: invalid argument")
+    return [(lv[i].width, lv[i].height, lv[i].tiles_x, lv[i].tiles_y, lv[i].offset) for i in range(n.value)], nbytes.value
 
 
 class Context:
@@ -281,6 +297,10 @@ class Context:
         self._check(self._lib.vr_overlay_pick(self._h, C.c_void_p(d_pick.data_ptr()), int(x), int(y), int(radius), C.byref(box),
                                               _stream(stream)))
         return box.value
+
+    def build_pyramid(self, d_frame, width, height, pitch_px, d_out, tile=256, stream=None):
+        self._check(self._lib.vr_build_pyramid(self._h, C.c_void_p(d_frame.data_ptr()), int(width), int(height), int(pitch_px),
+                                               int(tile), C.c_void_p(d_out.data_ptr()), _stream(stream)))
 
     def set_option(self, option, value):
         self._check(self._lib.vr_set_option(self._h, int(option), int(value)))
