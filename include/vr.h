@@ -213,10 +213,10 @@ int vr_reset_counters(vr_ctx* ctx, void* stream);
 /* Options.  None of them changes a frame (tests assert it); they exist for A/B measurements.
  *  VR_OPT_SKIP (default 1): min/max empty-space skipping (O-10) on/off, all levels.
  *  VR_OPT_VARIANT (default -1): the marcher.  0 = one ray per thread, the 32 lanes of a warp take
- *    8 x 4 pixels; 3 = lockstep: a warp walks its 32 rays together through chunks of 32 lattice
- *    indices, the lanes taking the 32 samples of one ray at a time, then each lane folds its own
- *    ray; -1 = chosen per view from the spacing of neighbouring rays
- *    (>= 2 voxels: 3, else 0).
+ *    8 x 4 pixels; for partial images one CTA per pixel tile walks all bricks over the tile (ray
+ *    set up once); 1 = the same with one CTA per (brick, tile); 3 = lockstep: a warp walks its 32
+ *    rays together through chunks of 32 lattice indices; -1 = chosen per
+ *    view from the spacing of neighbouring rays (>= 2 voxels: 3, else 0).
  *  VR_OPT_CELL_SKIP (default -1): the 8^3 macro-cell level of the skipping under the configured
  *    bricks, 1 on / 0 off (needs VR_OPT_SKIP); -1 = on for emission-absorption if fewer than 3/4
  *    of the cells are active against the current table, on for MIP in variant 3.

@@ -888,7 +888,7 @@ int vr_set_option(vr_ctx* ctx, int option, int value) {
     if (option == VR_OPT_OCCUPANCY) { ctx->opt_occ = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_DENSE) { ctx->opt_dense = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_VARIANT) {
-        if (value != -1 && value != 0 && value != 3) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");
+        if (value != -1 && value != 0 && value != 1 && value != 3) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");
         ctx->opt_variant = value; return VR_OK;
     }
     return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown option");

@@ -437,6 +437,72 @@ render_bricks_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
     }
 }
 
+// The same partial images, one CTA per PIXEL TILE of the view instead of one per (brick, tile): the
+// ray of a pixel is set up once (fp64) and reused for every brick whose screen rectangle holds
+// the pixel (dense rays cross 10-30 bricks: on C4 the per-brick set-up was a fifth of all
+// instructions).  The CTA culls the partial rectangles against its tile into a shared bitmask
+// (as composite_kernel does) and takes the hits one after the other.
+constexpr int kCullChunk = 2048;
+
+template <int MODE, int LAYOUT>
+__global__ void __launch_bounds__(kThreads)
+render_tiles_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
+                    const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
+                    const PartialDev* __restrict__ parts, int n_parts) {
+    __shared__ float4 tab[256];
+    __shared__ unsigned mask[kCullChunk / 32];
+    if (MODE == VR_MODE_EA) load_tf(tab, T.baked);
+    int tx, ty; tile_pixel(tx, ty);
+    const int x0 = blockIdx.x * kTileW, y0 = blockIdx.y * kTileH;
+    const int i = x0 + tx, j = y0 + ty;
+    const bool live = i < V.W && j < V.H;
+    Ray r; r.k0 = 0; r.k1 = -1;
+    r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
+    r.inv[0] = r.inv[1] = r.inv[2] = 0.f;
+    if (live) setup_ray(V, c, i, j, r);
+    Stats st = {0, 0, 0};
+    unsigned long long nominal = 0, n_stopped = 0;
+    for (int base = 0; base < n_parts; base += kCullChunk) {
+        const int cnt = min(kCullChunk, n_parts - base);
+        __syncthreads();
+        if (threadIdx.x < kCullChunk / 32) mask[threadIdx.x] = 0u;
+        __syncthreads();
+        for (int q = threadIdx.x; q < cnt; q += kThreads) {
+            const PartialDev& P = parts[base + q];
+            if (P.x0 < x0 + kTileW && P.x0 + P.w > x0 && P.y0 < y0 + kTileH && P.y0 + P.h > y0) atomicOr(&mask[q >> 5], 1u << (q & 31));
+        }
+        __syncthreads();
+        for (int w = 0; w < (cnt + 31) / 32; ++w) {
+            for (unsigned bits = mask[w]; bits; bits &= bits - 1) {
+                const PartialDev& P = parts[base + 32 * w + __ffs(bits) - 1];
+                const int lx = i - P.x0, ly = j - P.y0;
+                const bool mine = live && lx >= 0 && ly >= 0 && lx < P.w && ly < P.h;
+                const int bid = P.brick;
+                const int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
+                const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
+                int ka = mine ? r.k0 : 0, kb = mine ? r.k1 : -1;
+                brick_interval(c, r, b, lo, ka, kb);
+                Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
+                const bool stopped = march_interval<MODE, LAYOUT>(c, r, T, A, tab, bid, lo, ka, kb, acc, st);
+                if (mine) {
+                    const long long px = (long long)ly * P.pitch + lx;
+                    if (MODE == VR_MODE_MIP) reinterpret_cast<float*>(P.data)[px] = acc.m;
+                    else reinterpret_cast<float4*>(P.data)[px] = make_float4(acc.C[0], acc.C[1], acc.C[2], acc.A);
+                }
+                if (kb >= ka) nominal += (unsigned long long)(kb - ka + 1);
+                if (stopped) ++n_stopped;
+            }
+        }
+    }
+    if (A.counters) {
+        count(A.counters, kNominal, nominal);
+        count(A.counters, kTaken, st.taken);
+        count(A.counters, kVisited, st.visit);
+        count(A.counters, kSkipped, st.skip);
+        count(A.counters, kTerminated, n_stopped);
+    }
+}
+
 // ================================================================== variant 3: lockstep
 // A warp owns the 32 rays of its 8 x 4 pixel tile and walks them TOGETHER through chunks of 32
 // lattice indices [kbase, kbase + 31] (k counts from the near plane, so a chunk is a thin shell
@@ -1029,7 +1095,11 @@ cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFD
     if (n == 0 || total_tiles == 0) return cudaSuccess;
     if (use_occ_kernel(c, a)) { render_occ_kernel<false><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n); return cudaGetLastError(); }
     if (a.variant == 3) VR_DISPATCH_LS(false, total_tiles, c, v, t, a, d_partials, n);
-    else VR_DISPATCH(render_bricks_kernel, total_tiles, c, v, t, a, d_partials, n);
+    else if (a.variant == 1) VR_DISPATCH(render_bricks_kernel, total_tiles, c, v, t, a, d_partials, n);
+    else {
+        dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
+        VR_DISPATCH(render_tiles_kernel, grid, c, v, t, a, d_partials, n);
+    }
     return cudaGetLastError();
 }
 

@@ -25,11 +25,12 @@ def H():
 
 
 # Every test below runs once with the library's own choice of marcher variant and macro-cell
-# skipping ("auto") and once per forced variant (0: ray per thread; 3: lockstep ray per warp, folding
+# skipping ("auto") and once per forced variant (0 / 1: ray per thread, CTA per pixel tile / per
+# (brick, tile); 3: lockstep ray per warp, folding
 # emission-absorption samples in the owning lane "v3s" or through shared memory "v3d", or testing
 # every sample against the occupancy bits first "v3o"), with the macro-cell level of the skipping
 # forced on.
-@pytest.fixture(autouse=True, params=["auto", "v0", "v3s", "v3d", "v3o"])
+@pytest.fixture(autouse=True, params=["auto", "v0", "v1", "v3s", "v3d", "v3o"])
 def marcher(request, H):
     from paper_1012_2909_b200 import vr
     H.FORCED_OPTIONS.clear()
