@@ -776,36 +776,20 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                   const PartialDev* __restrict__ parts, int n_parts) {
     constexpr int MODE = VR_MODE_EA, LAYOUT = 1;
     constexpr int kWarps = kThreads / 32;
-    __shared__ PartialDev part;
     __shared__ float4 rays_all[kWarps][64];
     __shared__ float stage_all[kWarps][kDepth * 256];
     __shared__ float vals_all[kWarps][kListCap];
     __shared__ unsigned short list_all[kWarps][kListCap];
-    int fx, fy;
-    bool live;
-    if (GLOBAL) {
-        int tx, ty; tile_pixel(tx, ty);
-        fx = blockIdx.x * kTileW + tx; fy = blockIdx.y * kTileH + ty;
-        live = fx < V.W && fy < V.H;
-    } else {
-        int lx, ly;
-        live = locate_tile(parts, n_parts, part, lx, ly);
-        fx = lx; fy = ly;
-    }
-    int bid0 = 0, lo0[3] = {0, 0, 0};
-    if (!GLOBAL) {
-        bid0 = part.brick;
-        lo0[0] = (bid0 % c.G[0]) * c.B[0]; lo0[1] = ((bid0 / c.G[0]) % c.G[1]) * c.B[1]; lo0[2] = (bid0 / (c.G[0] * c.G[1])) * c.B[2];
-    }
+    __shared__ unsigned mask[GLOBAL ? 1 : kCullChunk / 32];
+    // one CTA per pixel tile of the view; for partial images it walks every brick over the tile, so
+    // the ray is set up once (fp64) per pixel, not once per (pixel, brick)
+    int tx, ty; tile_pixel(tx, ty);
+    const int x0 = blockIdx.x * kTileW, y0 = blockIdx.y * kTileH;
+    const int fx = x0 + tx, fy = y0 + ty;
+    const bool live = fx < V.W && fy < V.H;
     Ray r; r.k0 = 0; r.k1 = -1;
     r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
-    if (live) setup_ray(V, c, GLOBAL ? fx : part.x0 + fx, GLOBAL ? fy : part.y0 + fy, r);
-    int ka = r.k0, kb = r.k1;
-    if (!GLOBAL) {
-        const int b[3] = {bid0 % c.G[0], (bid0 / c.G[0]) % c.G[1], bid0 / (c.G[0] * c.G[1])};
-        brick_interval(c, r, b, lo0, ka, kb);
-    }
-    const BrickRef br0 = brick_ref<LAYOUT>(c, bid0, lo0);
+    if (live) setup_ray(V, c, fx, fy, r);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float* vals = vals_all[warp];
     unsigned short* list = list_all[warp];
@@ -813,16 +797,11 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
     const float* stage = stage_all[warp] + lane;
     const unsigned stage_addr = (unsigned)__cvta_generic_to_shared(stage);
     rays[2 * lane] = make_float4(r.o[0], r.o[1], r.o[2], r.d[0]);
-    rays[2 * lane + 1] = make_float4(r.d[1], r.d[2], __int_as_float(ka), __int_as_float(kb));
-    __syncwarp();
-    bool alive = ka <= kb, stopped = false;
-    int k_end = kb;
-    int K0 = alive ? ka : 0x7fffffff, K1 = alive ? kb : -1;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        K0 = min(K0, __shfl_xor_sync(0xffffffffu, K0, o));
-        K1 = max(K1, __shfl_xor_sync(0xffffffffu, K1, o));
-    }
+    // state of the brick being marched (GLOBAL: the whole cube in one go)
+    int bid0 = 0, lo0[3] = {0, 0, 0};
+    BrickRef br0 = brick_ref<LAYOUT>(c, 0, lo0);
+    int ka = r.k0, kb = r.k1, k_end = kb;
+    bool alive = false, stopped = false;
     Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
     unsigned n_taken = 0;
     // the occupancy word of a sample: index (whole cube) and bit; ~0u if the sample's brick is inactive
@@ -844,6 +823,18 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
         widx = base + occ_word_index(c, lx, ly, lz);
         bit = occ_bit_index(lx, ly, lz);
     };
+    // march the taken samples [ka, kb] of every lane's ray (all members of brick bid0 unless GLOBAL) into acc
+    auto march = [&]() {
+    rays[2 * lane + 1] = make_float4(r.d[1], r.d[2], __int_as_float(ka), __int_as_float(kb));
+    __syncwarp();
+    alive = ka <= kb; stopped = false; k_end = kb; n_taken = 0;
+    acc.C[0] = acc.C[1] = acc.C[2] = 0.f; acc.A = 0.f; acc.m = -INFINITY;
+    int K0 = alive ? ka : 0x7fffffff, K1 = alive ? kb : -1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        K0 = min(K0, __shfl_xor_sync(0xffffffffu, K0, o));
+        K1 = max(K1, __shfl_xor_sync(0xffffffffu, K1, o));
+    }
     for (int kbase = K0; kbase <= K1; kbase += 32) {
         if (!__ballot_sync(0xffffffffu, alive)) break;
         const bool mine = alive && ka <= kbase + 31 && kb >= kbase;
@@ -956,19 +947,54 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
             base = bend;
         }
     }
-    if (live) {
-        if (GLOBAL) write_frame_pixel<MODE>(V, T, A, fx, fy, acc, r.k1 >= r.k0);
-        else reinterpret_cast<float4*>(part.data)[(long long)fy * part.pitch + fx] = make_float4(acc.C[0], acc.C[1], acc.C[2], acc.A);
+    __syncwarp();
+    };
+    unsigned long long c_nom = 0, c_reached = 0, c_taken = 0, c_stopped = 0;
+    auto tally = [&]() {
+        if (kb >= ka) { c_nom += (unsigned long long)(kb - ka + 1); c_reached += (unsigned long long)(k_end - ka + 1); }
+        c_taken += n_taken;
+        if (stopped) ++c_stopped;
+    };
+    if (GLOBAL) {
+        march();
+        tally();
+        if (live) write_frame_pixel<MODE>(V, T, A, fx, fy, acc, r.k1 >= r.k0);
+    } else {
+        for (int base = 0; base < n_parts; base += kCullChunk) {
+            const int cnt = min(kCullChunk, n_parts - base);
+            __syncthreads();
+            if (threadIdx.x < kCullChunk / 32) mask[threadIdx.x] = 0u;
+            __syncthreads();
+            for (int q = threadIdx.x; q < cnt; q += kThreads) {
+                const PartialDev& P = parts[base + q];
+                if (P.x0 < x0 + kTileW && P.x0 + P.w > x0 && P.y0 < y0 + kTileH && P.y0 + P.h > y0) atomicOr(&mask[q >> 5], 1u << (q & 31));
+            }
+            __syncthreads();
+            for (int w = 0; w < (cnt + 31) / 32; ++w) {
+                for (unsigned bits = mask[w]; bits; bits &= bits - 1) {
+                    const PartialDev& P = parts[base + 32 * w + __ffs(bits) - 1];
+                    const int lx = fx - P.x0, ly = fy - P.y0;
+                    const bool mine = live && lx >= 0 && ly >= 0 && lx < P.w && ly < P.h;
+                    bid0 = P.brick;
+                    const int b[3] = {bid0 % c.G[0], (bid0 / c.G[0]) % c.G[1], bid0 / (c.G[0] * c.G[1])};
+                    lo0[0] = b[0] * c.B[0]; lo0[1] = b[1] * c.B[1]; lo0[2] = b[2] * c.B[2];
+                    br0 = brick_ref<LAYOUT>(c, bid0, lo0);
+                    ka = mine ? r.k0 : 0; kb = mine ? r.k1 : -1;
+                    brick_interval(c, r, b, lo0, ka, kb);
+                    march();
+                    tally();
+                    if (mine) reinterpret_cast<float4*>(P.data)[(long long)ly * P.pitch + lx] = make_float4(acc.C[0], acc.C[1], acc.C[2], acc.A);
+                }
+            }
+        }
     }
     if (A.counters) {
-        const unsigned long long nom = kb >= ka ? (unsigned long long)(kb - ka + 1) : 0ULL;
-        const unsigned long long reached = kb >= ka ? (unsigned long long)(k_end - ka + 1) : 0ULL;
-        if (GLOBAL) count(A.counters, kRays, nom ? 1 : 0);
-        count(A.counters, kNominal, nom);
-        count(A.counters, kTaken, n_taken);
-        count(A.counters, kVisited, nom ? 1 : 0);
-        count(A.counters, kSkipped, reached - n_taken);
-        count(A.counters, kTerminated, stopped ? 1 : 0);
+        if (GLOBAL) count(A.counters, kRays, c_nom ? 1 : 0);
+        count(A.counters, kNominal, c_nom);
+        count(A.counters, kTaken, c_taken);
+        count(A.counters, kVisited, c_nom ? 1 : 0);
+        count(A.counters, kSkipped, c_reached - c_taken);
+        count(A.counters, kTerminated, c_stopped);
     }
 }
 
@@ -1093,7 +1119,11 @@ cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFD
 cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a,
                                  const PartialDev* d_partials, int n, int total_tiles, cudaStream_t s) {
     if (n == 0 || total_tiles == 0) return cudaSuccess;
-    if (use_occ_kernel(c, a)) { render_occ_kernel<false><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n); return cudaGetLastError(); }
+    if (use_occ_kernel(c, a)) {
+        dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
+        render_occ_kernel<false><<<grid, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
+        return cudaGetLastError();
+    }
     if (a.variant == 3) VR_DISPATCH_LS(false, total_tiles, c, v, t, a, d_partials, n);
     else if (a.variant == 1) VR_DISPATCH(render_bricks_kernel, total_tiles, c, v, t, a, d_partials, n);
     else {
