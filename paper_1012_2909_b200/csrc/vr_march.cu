@@ -766,6 +766,7 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
 // render_ls_kernel<..., DENSE> instead).  Frames are identical to the other marchers': a skipped
 // sample has weight exactly zero.
 constexpr int kListCap = 256;
+constexpr int kOccDepth = 2;             // gathers are few here: a shallower ring leaves more of the SM to L1 (3 -> 6.36, 2 -> 6.26 ms)
 
 // 8 CTAs per SM (64 registers): the few gathers leave L1 alone, more warps hide the bit lookups (measured:
 // 7 -> 6.83, 8 -> 6.44, 9 -> 7.27 ms on C3)
@@ -777,7 +778,7 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
     constexpr int MODE = VR_MODE_EA, LAYOUT = 1;
     constexpr int kWarps = kThreads / 32;
     __shared__ float4 rays_all[kWarps][64];
-    __shared__ float stage_all[kWarps][kDepth * 256];
+    __shared__ float stage_all[kWarps][kOccDepth * 256];
     __shared__ float vals_all[kWarps][kListCap];
     __shared__ unsigned short list_all[kWarps][kListCap];
     __shared__ unsigned mask[GLOBAL ? 1 : kCullChunk / 32];
@@ -919,15 +920,15 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                 for (int e = 0; e < 8; ++e) v[e] = st[32 * e];
                 vals[32 * S.rc + lane] = trilinear(v, S.w[0], S.w[1], S.w[2]);
             };
-            Slot slot[kDepth];
+            Slot slot[kOccDepth];
             int gi = 0;
 #pragma unroll
-            for (int s = 0; s < kDepth - 1; ++s) issue(slot[s], gi++, s);
+            for (int s = 0; s < kOccDepth - 1; ++s) issue(slot[s], gi++, s);
             for (bool more = true; more;) {
 #pragma unroll
-                for (int u = 0; u < kDepth; ++u) {
-                    issue(slot[(u + kDepth - 1) % kDepth], gi++, (u + kDepth - 1) % kDepth);
-                    cp_async_wait<kDepth - 1>();
+                for (int u = 0; u < kOccDepth; ++u) {
+                    issue(slot[(u + kOccDepth - 1) % kOccDepth], gi++, (u + kOccDepth - 1) % kOccDepth);
+                    cp_async_wait<kOccDepth - 1>();
                     if (slot[u].rc < 0) { more = false; break; }
                     consume(slot[u], u);
                 }
