@@ -95,8 +95,8 @@ def orbit_frame(w, step_index, n_steps, rank, world):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the marcher, from the committed
-# `ncu --set full` captures (profiles/r1c_c3_render_occ_full.md: orbit frames 0 and 180, 10.28 and 7.26 GB; their mean).  None: not captured.
-NCU_TRAFFIC_BYTES = {"C3": 8.77e9}
+# `ncu --set full` captures (profiles/r1d_c3_render_occ_full.md: orbit frames 0 and 180, 11.17 and 7.98 GB, their mean; r1d_c3_mip_render_ls_full.md: frame 0).  None: not captured.
+NCU_TRAFFIC_BYTES = {("C3", "ea"): 9.57e9, ("C3", "mip"): 70.8e9}
 
 MARCHER = {(0, 0): "render_bricks_kernel<EA> (ray per thread)", (0, 1): "render_bricks_kernel<EA> (ray per thread)",
            (0, 2): "render_bricks_kernel<EA> (ray per thread, macro-cell runs)",
@@ -213,6 +213,8 @@ def main():
     ap.add_argument("--workload", default="C3", choices=sorted(wl.CONFIGS))
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--mode", default="ea", choices=["ea", "mip"], help="emission-absorption (default) or MIP")
+    ap.add_argument("--frame", default=None, help="WxH: render one frame of this size instead of the workload's "
+                                                   "(BASELINE.json configs[4]: C5's 1920x1080 MIP)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
@@ -233,6 +235,9 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     w = wl.CONFIGS[args.workload]
+    if args.frame:
+        from dataclasses import replace
+        w = replace(w, frame=tuple(int(v) for v in args.frame.lower().split("x")), panels=(1, 1))
     job = Job(w, local_rank, args.mode)
     vr = job.vr
     config = {"workload": f"{w.name}: {w.dims[0]}x{w.dims[1]}x{w.dims[2]} float32 cube, {w.brick[0]}^3 bricks, "
@@ -300,7 +305,7 @@ def main():
     if args.mode == "mip":
         kernel = ("render_ls_kernel<MIP> (lockstep, cp.async gather, warp-reduced maximum)" if plan["variant"] == 3
                   else "render_bricks_kernel<MIP> (ray per thread)")
-    traffic = NCU_TRAFFIC_BYTES.get(w.name)
+    traffic = NCU_TRAFFIC_BYTES.get((w.name, args.mode)) if not args.frame else None
     launch_s = march_ms / max(n_march, 1) * 1e-3
     achieved = (job.alg_bytes / max(n_march, 1)) / (march_ms / max(n_march, 1) * 1e-3) / 1e9 if march_ms > 0 else 0.0
     cpu = None
