@@ -97,6 +97,10 @@ def orbit_frame(w, step_index, n_steps, rank, world):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the marcher, from the committed
 # `ncu --set full` captures (profiles/r1d_c3_render_occ_full.md: orbit frames 0 and 180, 11.17 and 7.98 GB, their mean; r1d_c3_mip_render_ls_full.md: frame 0).  None: not captured.
 NCU_TRAFFIC_BYTES = {("C3", "ea"): 9.57e9, ("C3", "mip"): 70.8e9}
+# smsp__inst_executed.sum (warp instructions) per launch from the same captures, and the issue peak
+# DESIGN.md section 8 derives: 148 SMs x 4 schedulers x 1 warp instruction per clock.
+NCU_WARP_INSTRUCTIONS = {("C3", "ea"): 4.56e9, ("C3", "mip"): 8.25e9}
+ISSUE_SLOTS_PER_CLOCK = 148 * 4
 
 MARCHER = {(0, 0): "render_bricks_kernel<EA> (ray per thread)", (0, 1): "render_bricks_kernel<EA> (ray per thread)",
            (0, 2): "render_bricks_kernel<EA> (ray per thread, macro-cell runs)",
@@ -307,6 +311,14 @@ def main():
                   else "render_bricks_kernel<MIP> (ray per thread)")
     traffic = NCU_TRAFFIC_BYTES.get((w.name, args.mode)) if not args.frame else None
     launch_s = march_ms / max(n_march, 1) * 1e-3
+    winst = NCU_WARP_INSTRUCTIONS.get((w.name, args.mode)) if not args.frame else None
+    issue = None
+    if winst and launch_s > 0 and clocks.get("sm_mhz"):
+        ipeak = ISSUE_SLOTS_PER_CLOCK * clocks["sm_mhz"] * 1e6 / 1e9
+        issue = {"bound": "alu", "achieved": winst / launch_s / 1e9, "peak": ipeak, "unit": "G warp-instructions/s",
+                 "frac": winst / launch_s / 1e9 / ipeak,
+                 "note": "warp instructions per launch from the committed ncu capture / live launch time; peak = 148 SMs x 4 "
+                         "schedulers x the SM clock sampled during the run: what actually bounds the occupancy marcher"}
     achieved = (job.alg_bytes / max(n_march, 1)) / (march_ms / max(n_march, 1) * 1e-3) / 1e9 if march_ms > 0 else 0.0
     cpu = None
     if world == 1:
@@ -343,6 +355,7 @@ def main():
                      "share_of_step": march_ms / ms_total if ms_total else None,
                      "algorithmic_bytes_per_launch": job.alg_bytes / max(n_march, 1),
                      "dram_gbs_from_traffic": traffic / launch_s / 1e9 if traffic and launch_s > 0 else None,
+                     "issue": issue,
                      "plan": plan,
                      "note": "algorithmic bytes = 4 B x voxels of the active in-frustum bricks at the configured brick "
                              "size + partial images (SURVEY.md 8(d)); skipping below the brick level (macro-cells, "
