@@ -199,6 +199,87 @@ def test_bricked_perspective_parity(H, name, dims, brick, frame, step):
         assert c["nominal_samples"] == c32["nominal"]        # integer lattice invariant (O-3)
 
 
+# ------------------------------------------------------------------------------ degenerate and awkward cases
+def _check_both_paths(H, sc, vol, M, W, Hh, step, tf, tau, what, partition):
+    """Whole-frame (GLOBAL) and sort-last EA + MIP of one view against the oracle, bit for bit in float32."""
+    ovr, vr = sc.ovr, sc.vr
+    got = sc.render_ea(M, W, Hh, step, tf, bg=BG, tau=tau)
+    o64, fl, _ = ovr.render(vol, M, W, Hh, step, ovr.EA, ovr.F64, tf=tf, bg=BG, tau=tau)
+    o32, _, _ = ovr.render(vol, M, W, Hh, step, ovr.EA, ovr.F32, tf=tf, bg=BG, tau=tau)
+    H.compare(got, o64, fl, o32, what=what + " EA")
+    assert np.array_equal(got, o32), what + " EA: not bit-identical to the float32 oracle"
+    fr, _, _ = sc.render_sortlast(M, W, Hh, step, vr.MODE_EA, tf=tf, bg=BG, tau=tau)
+    s32, _, _ = ovr.render(vol, M, W, Hh, step, ovr.EA, ovr.F32, tf=tf, bg=BG, tau=tau, split=ovr.SPLIT_SORTLAST, partition=partition)
+    assert np.array_equal(fr, s32), what + " EA sort-last: not bit-identical to the float32 oracle"
+    mip = sc.render_mip(M, W, Hh, step, miss=-1.0)
+    m32, _, _ = ovr.render(vol, M, W, Hh, step, ovr.MIP, ovr.F32, miss=-1.0)
+    assert np.array_equal(mip, m32), what + " MIP"
+    mip_sl, _, _ = sc.render_sortlast(M, W, Hh, step, vr.MODE_MIP, bg=(-1.0, 0, 0, 0))
+    assert np.array_equal(mip_sl, m32), what + " MIP sort-last"
+    return got, mip
+
+
+AWKWARD = [
+    ("flat cube, one voxel thick", (40, 33, 1), (16, 16, 16), (64, 48), 0.5),
+    ("two planes thick", (40, 33, 2), (16, 16, 16), (64, 48), 0.25),
+    ("a single row of voxels", (57, 1, 1), (16, 8, 8), (48, 32), 0.25),
+    ("bricks larger than the cube", (20, 24, 28), (64, 64, 64), (40, 40), 0.5),
+    ("non-cubic bricks, ragged grid", (50, 37, 61), (32, 8, 16), (53, 41), 0.5),
+    ("step longer than a voxel", (48, 48, 48), (16, 16, 16), (40, 40), 1.7),
+    ("one-pixel frame", (32, 32, 32), (16, 16, 16), (1, 1), 0.5),
+]
+
+
+@pytest.mark.parametrize("name,dims,brick,frame,step", AWKWARD)
+def test_awkward_shapes(H, name, dims, brick, frame, step):
+    cube = noise_cube(dims[::-1], seed=11, scale=6.0) + 4.0
+    sc = H.Scene(dims, brick, cube=cube)
+    vol = sc.oracle_volume()
+    W, Hh = frame
+    part = tuple(min(b, n) for b, n in zip(brick, dims))
+    for az, tf, tau in ((40.0, wl.tf_fog(), 0.99), (250.0, wl.tf_src(), 0.5)):
+        M = wl.perspective_camera(dims, frame, azimuth_deg=az) if min(dims) > 1 else wl.perspective_camera(
+            tuple(max(n, 2) for n in dims), frame, azimuth_deg=az)
+        _check_both_paths(H, sc, vol, M, W, Hh, step, tf, tau, f"{name} az={az}", part)
+
+
+def test_camera_inside_the_cube_and_rays_that_miss(H):
+    dims, brick, frame = (64, 64, 64), (16, 16, 16), (72, 54)
+    cube = noise_cube(dims[::-1], seed=3, scale=5.0) + 3.0
+    sc = H.Scene(dims, brick, cube=cube)
+    vol = sc.oracle_volume()
+    W, Hh = frame
+    # eye inside the cube: the near plane cuts the volume, rays start between voxels
+    eye = np.array([30.3, 28.7, 17.2])
+    V = wl._look_at(eye, eye + np.array([0.3, -0.2, 1.0]), np.array([0.0, 1.0, 0.0]))
+    top = 0.75 * math.tan(math.radians(25.0))
+    M = (wl._frustum(-top * W / Hh, top * W / Hh, -top, top, 0.75, 300.0) @ V).astype(np.float32)
+    _check_both_paths(H, sc, vol, M, W, Hh, 0.5, wl.tf_fog(), 0.99, "eye inside", brick)
+    # looking away from the cube: every ray misses, EA = background, MIP = miss value, bit for bit
+    eye = np.array([32.0, 32.0, -80.0])
+    V = wl._look_at(eye, eye + np.array([0.0, 0.0, -1.0]), np.array([0.0, 1.0, 0.0]))
+    M = (wl._frustum(-top * W / Hh, top * W / Hh, -top, top, 0.75, 300.0) @ V).astype(np.float32)
+    ea, mip = _check_both_paths(H, sc, vol, M, W, Hh, 0.5, wl.tf_fog(), 0.99, "all rays miss", brick)
+    assert (ea == np.array(BG, np.float32)).all() and (mip == -1.0).all()
+
+
+def test_extreme_transfer_functions(H):
+    dims, brick, frame = (48, 40, 56), (16, 16, 16), (60, 44)
+    cube = noise_cube(dims[::-1], seed=8, scale=4.0) + 10.0
+    sc = H.Scene(dims, brick, cube=cube)
+    vol = sc.oracle_volume()
+    W, Hh = frame
+    M = wl.perspective_camera(dims, frame, azimuth_deg=120.0)
+    ramp = wl.tf_ramp()[0]
+    clear = ramp.copy(); clear[:, 3] = 0.0                  # nothing is visible: the frame is the background
+    ea, _ = _check_both_paths(H, sc, vol, M, W, Hh, 0.5, (clear, 0.0, 20.0), 0.99, "transparent table", brick)
+    assert (ea == np.array(BG, np.float32)).all()
+    solid = ramp.copy(); solid[:, 3] = 1.0                  # opaque at the first sample: alpha = 1 wherever the cube is hit
+    ea, mip = _check_both_paths(H, sc, vol, M, W, Hh, 0.5, (solid, 0.0, 20.0), 0.99, "opaque table", brick)
+    assert (ea[mip != -1.0][:, 3] == 1.0).all()
+    _check_both_paths(H, sc, vol, M, W, Hh, 0.5, (ramp, 9.0, 9.5), 0.05, "narrow window, tau 0.05", brick)   # nearly everything clamps
+
+
 def test_skipping_never_changes_a_frame(H):
     dims, brick, frame = (96, 96, 96), (16, 16, 16), (120, 90)
     w = wl.scaled(wl.C2, "skip", dims, brick, frame, n_sources=4)
