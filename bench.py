@@ -111,17 +111,25 @@ MARCHER = {(0, 0): "render_bricks_kernel<EA> (ray per thread)", (0, 1): "render_
 class Job:
     """One rank's resident cube + context."""
 
-    def __init__(self, w, device, mode="ea"):
+    def __init__(self, w, device, mode="ea", shard=None, dist=None):
         import torch
         from paper_1012_2909_b200 import vr
         self.torch, self.vr, self.w = torch, vr, w
         self.mode = vr.MODE_EA if mode == "ea" else vr.MODE_MIP
         self.px_bytes = 16 if mode == "ea" else 4
         torch.cuda.set_device(device)
-        cb, mb = vr.cube_layout(w.dims, w.brick)
-        self.d_cube = torch.empty(cb // 4, dtype=torch.float32, device="cuda")
-        self.d_meta = torch.empty(mb, dtype=torch.uint8, device="cuda")
         self.ctx = vr.Context(device)
+        self.shard, self.dist = None, dist
+        if shard is not None:                     # (rank, world): this rank holds one z-slab of the bricks
+            from paper_1012_2909_b200 import sortlast
+            self.sortlast = sortlast
+            self.shard = sortlast.Shard(self.ctx, w.dims, w.brick, shard[0], shard[1])
+            self.shard.bind()
+            cb, mb = self.shard.layout()
+        else:
+            cb, mb = vr.cube_layout(w.dims, w.brick)
+        self.d_cube = torch.empty(max(cb // 4, 1), dtype=torch.float32, device="cuda")
+        self.d_meta = torch.empty(max(mb, 1), dtype=torch.uint8, device="cuda")
         t0 = time.perf_counter()
         self.ctx.generate_cube(w.seed, w.dims, w.brick, self.d_cube, self.d_meta, sources=wl.make_sources(w),
                                zero_boxes=wl.make_zero_boxes(w), continuum=w.continuum)
@@ -155,6 +163,27 @@ class Job:
         brick_vox = 1
         for b, n in zip(w.brick, w.dims):
             brick_vox *= min(b, n)
+        if self.shard is not None:
+            # sharded sort-last (paper_1012_2909_b200/sortlast.py): own bricks -> one partial frame, strips
+            # exchanged, folded in the slabs' visibility order, gathered
+            sh, sl = self.shard, self.sortlast
+            ctx.set_view(M, self.W, self.H, w.step)
+            if timed_events:
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+            part = sh.render_partial(torch, self.mode, self.W, self.H, w.tau)
+            if timed_events:
+                e1.record()
+                self.march_events.append((e0, e1))
+                self.alg_bytes += 4 * brick_vox * (sh.end - sh.first) + self.H * self.W * self.px_bytes
+            versions = sl.exchange_strips(self.dist, part, sh.world)
+            strip = sh.fold_strip(torch, self.mode, versions, self.W, self.H, self.bg)
+            self.frame = sl.gather_strips(self.dist, strip, sh.world, self.H)
+            if timed_events:
+                e = torch.cuda.Event(enable_timing=True)
+                e.record()
+                self.step_events.append(e)
+            return
         for r in range(self.rows):
             for c in range(self.cols):
                 Mp = M if (self.cols, self.rows) == (1, 1) else wl.panel_matrix(M, self.cols, self.rows, c, r)
@@ -217,6 +246,9 @@ def main():
     ap.add_argument("--workload", default="C3", choices=sorted(wl.CONFIGS))
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--mode", default="ea", choices=["ea", "mip"], help="emission-absorption (default) or MIP")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N ranks share ONE cube: bricks sharded in z-slabs, sort-last exchange over NCCL (NEXT-1, "
+                         "strong scaling); default: N independent replicas")
     ap.add_argument("--frame", default=None, help="WxH: render one frame of this size instead of the workload's "
                                                    "(BASELINE.json configs[4]: C5's 1920x1080 MIP)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -242,14 +274,18 @@ def main():
     if args.frame:
         from dataclasses import replace
         w = replace(w, frame=tuple(int(v) for v in args.frame.lower().split("x")), panels=(1, 1))
-    job = Job(w, local_rank, args.mode)
+    if args.sharded and w.panels != (1, 1):
+        raise SystemExit("--sharded renders single-panel frames (use --frame WxH for the tiled workloads)")
+    job = Job(w, local_rank, args.mode, shard=(rank, world) if args.sharded else None, dist=dist)
+    frank, fworld = (0, 1) if args.sharded else (rank, world)          # sharded: every rank renders every frame
     vr = job.vr
     config = {"workload": f"{w.name}: {w.dims[0]}x{w.dims[1]}x{w.dims[2]} float32 cube, {w.brick[0]}^3 bricks, "
                           f"{w.frame[0]}x{w.frame[1]} frame ({w.panels[0]}x{w.panels[1]} panels), step {w.step}, "
                           f"{'EA tf-' + w.tf + ' tau=' + str(w.tau) if args.mode == 'ea' else 'MIP'}, sort-last path, orbit frames spread over 360 deg",
               "cube_gib": round(w.n_voxels * 4 / 2 ** 30, 3), "n_sources": w.n_sources,
               "l2_policy": "inputs larger than L2 (cube >> 126 MB); no explicit flush",
-              "replicas": world, "generate_seconds": round(job.gen_seconds, 3)}
+              "replicas": 1 if args.sharded else world, "shards": world if args.sharded else 1,
+              "generate_seconds": round(job.gen_seconds, 3)}
 
     if args.impl == "reference":
         return run_reference(args, job, config)
@@ -260,7 +296,7 @@ def main():
         torch.cuda.synchronize()
 
     for i in range(args.warmup):
-        job.step(orbit_frame(w, i, args.steps, rank, world))
+        job.step(orbit_frame(w, i, args.steps, frank, fworld))
     job.ctx.reset_counters()
     sampler = ClockSampler(local_rank)
     barrier()
@@ -268,7 +304,7 @@ def main():
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
     for i in range(args.steps):
-        job.step(orbit_frame(w, i, args.steps, rank, world), timed_events=True)
+        job.step(orbit_frame(w, i, args.steps, frank, fworld), timed_events=True)
     ev1.record()
     barrier()
     clocks = sampler.result()
@@ -289,7 +325,7 @@ def main():
     barrier()
     t0 = time.perf_counter()
     for i in range(args.steps):
-        job.step(orbit_frame(w, i, args.steps, rank, world), set_tf=True)
+        job.step(orbit_frame(w, i, args.steps, frank, fworld), set_tf=True)
         job.h_frame.copy_(job.frame, non_blocking=True)
         torch.cuda.current_stream().synchronize()
     e2e_s = time.perf_counter() - t0
@@ -337,12 +373,12 @@ def main():
     out = {
         "metric": METRIC, "value": nominal / (ms_total * 1e-3), "unit": "samples/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_total / args.steps, "frames_per_s": args.steps * world / (ms_total * 1e-3),
+        "ms_per_step": ms_total / args.steps, "frames_per_s": args.steps * fworld / (ms_total * 1e-3),
         "frame_ms": {"median": frame_ms[len(frame_ms) // 2], "p95": frame_ms[min(len(frame_ms) - 1, int(0.95 * len(frame_ms)))],
                      "min": frame_ms[0], "max": frame_ms[-1], "note": "rank 0, device time between consecutive frames of the orbit"},
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": config,
-        "nominal_samples_per_step": nominal / (args.steps * world),
+        "higher_is_better": True, "scaling": "strong" if args.sharded else "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic", "config": config,
+        "nominal_samples_per_step": nominal / (args.steps * fworld),
         "taken_samples_per_s": taken / (ms_total * 1e-3),
         "gpu_launches": launches,
         "clocks": clocks,
