@@ -176,9 +176,12 @@ class Job:
                 e1.record()
                 self.march_events.append((e0, e1))
                 self.alg_bytes += 4 * brick_vox * (sh.end - sh.first) + self.H * self.W * self.px_bytes
-            versions = sl.exchange_strips(self.dist, part, sh.world)
-            strip = sh.fold_strip(torch, self.mode, versions, self.W, self.H, self.bg)
-            self.frame = sl.gather_strips(self.dist, strip, sh.world, self.H)
+            if getattr(self, "slab_only", False):
+                self.frame = part
+            else:
+                versions = sl.exchange_strips(self.dist, part, sh.world)
+                strip = sh.fold_strip(torch, self.mode, versions, self.W, self.H, self.bg)
+                self.frame = sl.gather_strips(self.dist, strip, sh.world, self.H)
             if timed_events:
                 e = torch.cuda.Event(enable_timing=True)
                 e.record()
@@ -249,6 +252,11 @@ def main():
     ap.add_argument("--sharded", action="store_true",
                     help="N ranks share ONE cube: bricks sharded in z-slabs, sort-last exchange over NCCL (NEXT-1, "
                          "strong scaling); default: N independent replicas")
+    ap.add_argument("--slab", default=None, metavar="R/W",
+                    help="render only slab R of a W-way split of the bricks (what rank R of --sharded would render; no "
+                         "exchange): the per-rank cost of NEXT-1 measured on one GPU")
+    ap.add_argument("--next-rows", action="store_true",
+                    help="time the catalogue overlay and the output pyramid (SURVEY.md 8(f) 2 and 3) instead of the marcher")
     ap.add_argument("--frame", default=None, help="WxH: render one frame of this size instead of the workload's "
                                                    "(BASELINE.json configs[4]: C5's 1920x1080 MIP)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -274,9 +282,17 @@ def main():
     if args.frame:
         from dataclasses import replace
         w = replace(w, frame=tuple(int(v) for v in args.frame.lower().split("x")), panels=(1, 1))
-    if args.sharded and w.panels != (1, 1):
+    if args.next_rows:
+        return run_next_rows(args)
+    slab = None
+    if args.slab:
+        slab = tuple(int(v) for v in args.slab.split("/"))
+        if world != 1 or args.sharded or not (0 <= slab[0] < slab[1]):
+            raise SystemExit("--slab R/W runs on one GPU, without --sharded")
+    if (args.sharded or slab) and w.panels != (1, 1):
         raise SystemExit("--sharded renders single-panel frames (use --frame WxH for the tiled workloads)")
-    job = Job(w, local_rank, args.mode, shard=(rank, world) if args.sharded else None, dist=dist)
+    job = Job(w, local_rank, args.mode, shard=slab if slab else ((rank, world) if args.sharded else None), dist=dist)
+    job.slab_only = slab is not None
     frank, fworld = (0, 1) if args.sharded else (rank, world)          # sharded: every rank renders every frame
     vr = job.vr
     config = {"workload": f"{w.name}: {w.dims[0]}x{w.dims[1]}x{w.dims[2]} float32 cube, {w.brick[0]}^3 bricks, "
@@ -284,7 +300,7 @@ def main():
                           f"{'EA tf-' + w.tf + ' tau=' + str(w.tau) if args.mode == 'ea' else 'MIP'}, sort-last path, orbit frames spread over 360 deg",
               "cube_gib": round(w.n_voxels * 4 / 2 ** 30, 3), "n_sources": w.n_sources,
               "l2_policy": "inputs larger than L2 (cube >> 126 MB); no explicit flush",
-              "replicas": 1 if args.sharded else world, "shards": world if args.sharded else 1,
+              "replicas": 1 if args.sharded else world, "shards": world if args.sharded else 1, "slab": args.slab,
               "generate_seconds": round(job.gen_seconds, 3)}
 
     if args.impl == "reference":
@@ -357,7 +373,7 @@ def main():
                          "schedulers x the SM clock sampled during the run: what actually bounds the occupancy marcher"}
     achieved = (job.alg_bytes / max(n_march, 1)) / (march_ms / max(n_march, 1) * 1e-3) / 1e9 if march_ms > 0 else 0.0
     cpu = None
-    if world == 1:
+    if world == 1 and not slab:           # a slab holds only its own bricks: no oracle sample
         tile = 8
         sec, c, nb = oracle_sample(job, orbit_frame(w, 0, args.steps, 0, 1), tile)
         if c["nominal"] > 0 and sec > 0:
@@ -402,6 +418,46 @@ def main():
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
+    return 0
+
+
+def run_next_rows(args):
+    """Timings of vr_overlay_catalogue and vr_build_pyramid (CUDA events, inputs resident in HBM)."""
+    import torch
+    from paper_1012_2909_b200 import vr
+    ctx = vr.Context(0)
+
+    def timeit(fn, n=10):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    out = {"impl": "b200", "what": "NEXT rows: catalogue overlay and output pyramid", "overlay": [], "pyramid": None}
+    W, H = 1920, 1080
+    for name in ("C3", "C5"):
+        w = wl.CONFIGS[name]
+        src = wl.make_sources(w)
+        boxes = torch.from_numpy(src[:, wl.S_XLO:wl.S_ZHI + 1].astype(np.int32)).cuda()
+        col = torch.rand((boxes.shape[0], 4), device="cuda")
+        ctx.set_view(wl.perspective_camera(w.dims, (W, H), azimuth_deg=30.0), W, H, 0.5)
+        frame = torch.zeros((H, W, 4), device="cuda")
+        pick = torch.zeros((H, W), dtype=torch.int32, device="cuda")
+        ms = timeit(lambda: ctx.overlay_catalogue(boxes, col, None, frame, pick))
+        out["overlay"].append({"catalogue": f"{name}: {boxes.shape[0]} source boxes", "frame": f"{W}x{H}", "ms": ms,
+                               "covered_pixels": int((pick > 0).sum().item())})
+    Wp, Hp = 9600, 5400
+    frame = torch.rand((Hp, Wp, 4), device="cuda")
+    levels, nbytes = vr.pyramid_layout(Wp, Hp, 256)
+    buf = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    ms = timeit(lambda: ctx.build_pyramid(frame, Wp, Hp, Wp, buf, 256))
+    out["pyramid"] = {"frame": f"{Wp}x{Hp}", "tile": 256, "levels": len(levels), "bytes_out": nbytes, "ms": ms}
+    print(json.dumps(out))
     return 0
 
 
