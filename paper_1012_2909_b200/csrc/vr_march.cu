@@ -801,27 +801,30 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
     // state of the brick being marched (GLOBAL: the whole cube in one go)
     int bid0 = 0, lo0[3] = {0, 0, 0};
     BrickRef br0 = brick_ref<LAYOUT>(c, 0, lo0);
+    const unsigned* occ0 = c.occ;
     int ka = r.k0, kb = r.k1, k_end = kb;
     bool alive = false, stopped = false;
     Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
     unsigned n_taken = 0;
-    // the occupancy word of a sample: index (whole cube) and bit; ~0u if the sample's brick is inactive
-    auto locate = [&](const float tk, unsigned& widx, unsigned& bit) {
+    // the occupancy word of a sample (0 if its brick is inactive) and the sample's bit in it; 64-bit
+    // brick offsets: a sharded cube's global brick ids times the words per brick can pass 2^32
+    auto locate = [&](const float tk, unsigned& word, unsigned& bit) {
         float fl;
         const int iv[3] = {floor_pos(__fmaf_rn(tk, r.d[0], r.o[0]), fl), floor_pos(__fmaf_rn(tk, r.d[1], r.o[1]), fl),
                            floor_pos(__fmaf_rn(tk, r.d[2], r.o[2]), fl)};
-        unsigned lx, ly, lz, base;
+        unsigned lx, ly, lz;
+        const unsigned* occb;
         if (GLOBAL) {
             int b[3]; brick_of(c, iv, b);
             const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
             lx = (unsigned)(iv[0] - b[0] * c.B[0]); ly = (unsigned)(iv[1] - b[1] * c.B[1]); lz = (unsigned)(iv[2] - b[2] * c.B[2]);
-            base = (unsigned)bid * (unsigned)c.occ_words_per_brick;
-            if (__ldg(&c.brick_active[bid]) == 0) { widx = 0xffffffffu; bit = 0u; return; }
+            occb = c.occ + (long long)bid * c.occ_words_per_brick;
+            if (__ldg(&c.brick_active[bid]) == 0) { word = 0u; bit = 0u; return; }
         } else {
             lx = (unsigned)(iv[0] - lo0[0]); ly = (unsigned)(iv[1] - lo0[1]); lz = (unsigned)(iv[2] - lo0[2]);
-            base = (unsigned)bid0 * (unsigned)c.occ_words_per_brick;
+            occb = occ0;
         }
-        widx = base + occ_word_index(c, lx, ly, lz);
+        word = __ldg(occb + occ_word_index(c, lx, ly, lz));   // an L1 hit while the ray stays in its 4 x 4 x 2 cells
         bit = occ_bit_index(lx, ly, lz);
     };
     // march the taken samples [ka, kb] of every lane's ray (all members of brick bid0 unless GLOBAL) into acc
@@ -853,19 +856,13 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                 J0 = min(J0, __shfl_xor_sync(0xffffffffu, J0, o));
                 J1 = max(J1, __shfl_xor_sync(0xffffffffu, J1, o));
             }
-            unsigned widx = 0xffffffffu, word = 0u, bit = 0u;        // of sample j
-            if (J0 >= j0 && J0 <= j1) {
-                locate(__fmul_rn((float)(kbase + J0), r.step), widx, bit);
-                if (widx != 0xffffffffu) word = __ldg(c.occ + widx);
-            }
+            unsigned word = 0u, bit = 0u;                            // of sample j
+            if (J0 >= j0 && J0 <= j1) locate(__fmul_rn((float)(kbase + J0), r.step), word, bit);
             for (int j = J0; j <= J1; ++j) {
-                unsigned nidx = 0xffffffffu, nword = 0u, nbit = 0u;  // of sample j + 1
-                if (j + 1 >= j0 && j + 1 <= j1) {
-                    locate(__fmul_rn((float)(kbase + j + 1), r.step), nidx, nbit);
-                                        nword = nidx != 0xffffffffu ? __ldg(c.occ + nidx) : 0u;   // an L1 hit while the ray stays in its 4 x 4 x 2 cells
-                }
+                unsigned nword = 0u, nbit = 0u;                      // of sample j + 1
+                if (j + 1 >= j0 && j + 1 <= j1) locate(__fmul_rn((float)(kbase + j + 1), r.step), nword, nbit);
                 if (j >= j0 && j <= j1 && ((word >> bit) & 1u)) my_act |= 1u << j;
-                widx = nidx; word = nword; bit = nbit;
+                word = nword; bit = nbit;
             }
         }
         // ---- list, ray-major: lane's entries at [off, off + cnt)
@@ -980,6 +977,7 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                     const int b[3] = {bid0 % c.G[0], (bid0 / c.G[0]) % c.G[1], bid0 / (c.G[0] * c.G[1])};
                     lo0[0] = b[0] * c.B[0]; lo0[1] = b[1] * c.B[1]; lo0[2] = b[2] * c.B[2];
                     br0 = brick_ref<LAYOUT>(c, bid0, lo0);
+                    occ0 = c.occ + (long long)bid0 * c.occ_words_per_brick;
                     ka = mine ? r.k0 : 0; kb = mine ? r.k1 : -1;
                     brick_interval(c, r, b, lo0, ka, kb);
                     march();
