@@ -300,6 +300,8 @@ def main():
                           f"{'EA tf-' + w.tf + ' tau=' + str(w.tau) if args.mode == 'ea' else 'MIP'}, sort-last path, orbit frames spread over 360 deg",
               "cube_gib": round(w.n_voxels * 4 / 2 ** 30, 3), "n_sources": w.n_sources,
               "l2_policy": "inputs larger than L2 (cube >> 126 MB); no explicit flush",
+              "e2e_policy": "matrix + table host->device and frame device->pinned host every step; two frame buffers, frame "
+                            "i's copy overlaps frame i+1's render, the host waits for frame i-1 before issuing frame i+1",
               "replicas": 1 if args.sharded else world, "shards": world if args.sharded else 1, "slab": args.slab,
               "generate_seconds": round(job.gen_seconds, 3)}
 
@@ -339,12 +341,35 @@ def main():
     # parameters / table upload), the finished frame comes back device -> pinned host memory.
     job.ctx.reset_counters()
     barrier()
+    # Two frame buffers: frame i's device -> host copy runs on a copy stream while frame i + 1 is rendered;
+    # the host takes delivery of frame i - 1 (waits for its copy) before it issues frame i + 1.
+    frames = [job.frame, torch.zeros_like(job.frame)]
+    h_frames = [job.h_frame, torch.empty_like(job.h_frame).pin_memory()]
+    copy_stream = torch.cuda.Stream()
+    copied = [None, None]
+    torch.cuda.synchronize()
     t0 = time.perf_counter()
     for i in range(args.steps):
+        b = i % 2
+        if copied[b] is not None:
+            torch.cuda.current_stream().wait_event(copied[b])      # the buffer's previous frame has left the device
+        job.frame = frames[b]
         job.step(orbit_frame(w, i, args.steps, frank, fworld), set_tf=True)
-        job.h_frame.copy_(job.frame, non_blocking=True)
-        torch.cuda.current_stream().synchronize()
+        src = job.frame                                             # (the sharded path returns a new tensor)
+        rendered = torch.cuda.Event()
+        rendered.record()
+        with torch.cuda.stream(copy_stream):
+            copy_stream.wait_event(rendered)
+            h_frames[b].copy_(src, non_blocking=True)
+            src.record_stream(copy_stream)
+            copied[b] = torch.cuda.Event()
+            copied[b].record()
+        if i > 0:
+            copied[1 - b].synchronize()                             # frame i - 1 is in host memory
+    copied[(args.steps - 1) % 2].synchronize()
+    torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
+    job.frame = frames[0]
     cnt2 = job.ctx.get_counters()
     e2e_s, (e2e_nominal,) = reduce_run(dist, "cuda", e2e_s, [cnt2["nominal_samples"]])
 
