@@ -12,6 +12,18 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
 
 
+def pytest_sessionstart(session):
+    """Build libvr.so / libovr.so in-tree if they are missing or older than their sources (a no-op
+    otherwise).  A failure here is left to the tests that load the libraries to report."""
+    try:
+        from paper_1012_2909_b200 import build as vr_build
+        vr_build.build()
+        from oracle import build as oracle_build
+        oracle_build.build()
+    except Exception as exc:      # e.g. no nvcc on this machine but a built library in the tree
+        print(f"conftest: in-tree build skipped ({exc})")
+
+
 @pytest.fixture(scope="session")
 def ovr():
     from oracle import ovr as _ovr
