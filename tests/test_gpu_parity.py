@@ -589,3 +589,38 @@ def test_config_c5_full_size_128gib(H, marcher):
     if free < 150e9:
         pytest.skip("needs ~142 GB of free HBM")
     _tiled_fullsize_check(H, wl.C5, panels=[(2, 2), (1, 3)], block=6, mip_frame=(1920, 1080))
+
+
+def test_brick_and_macro_cell_minmax_against_numpy(H):
+    """S0 metadata (white box: d_meta starts with (min,max) per brick, then per 8^3 macro-cell, each
+    region 256-byte aligned): min / max over the region's voxels plus the +1 layer, clipped to the
+    cube (O-10: halo-inclusive, so that a trilinear footprint is always covered)."""
+    dims, brick = (45, 38, 29), (16, 24, 8)
+    cube = noise_cube(dims[::-1], seed=21, scale=3.0)
+    sc = H.Scene(dims, brick, cube=cube)
+    sc.torch.cuda.synchronize()
+    meta = sc.d_meta.cpu().numpy()
+    g = sc.grid()
+    nb = g[0] * g[1] * g[2]
+    C = [-(-b // 8) for b in brick]
+    cpb = C[0] * C[1] * C[2]
+    bmm = meta[:8 * nb].view(np.float32).reshape(nb, 2)
+    off = -(-8 * nb // 256) * 256
+    cmm = meta[off:off + 8 * nb * cpb].view(np.float32).reshape(nb, cpb, 2)
+    for bid in range(nb):
+        bi = (bid % g[0], (bid // g[0]) % g[1], bid // (g[0] * g[1]))
+        o = [bi[a] * brick[a] for a in range(3)]
+        hi = [min(o[a] + brick[a], dims[a] - 1) for a in range(3)]               # inclusive, +1 layer, inside the cube
+        reg = cube[o[2]:hi[2] + 1, o[1]:hi[1] + 1, o[0]:hi[0] + 1]
+        assert bmm[bid, 0] == reg.min() and bmm[bid, 1] == reg.max(), bid
+        for cz in range(C[2]):
+            for cy in range(C[1]):
+                for cx in range(C[0]):
+                    lo = [o[0] + 8 * cx, o[1] + 8 * cy, o[2] + 8 * cz]
+                    h2 = [min(lo[a] + 8, o[a] + brick[a], dims[a] - 1) for a in range(3)]
+                    got = cmm[bid, cx + C[0] * (cy + C[1] * cz)]
+                    if any(h2[a] < lo[a] for a in range(3)):
+                        assert got[0] > got[1]                                    # empty cell: (inf, -inf)
+                        continue
+                    r = cube[lo[2]:h2[2] + 1, lo[1]:h2[1] + 1, lo[0]:h2[0] + 1]
+                    assert got[0] == r.min() and got[1] == r.max(), (bid, cx, cy, cz)
