@@ -230,9 +230,12 @@ int vr_reset_counters(vr_ctx* ctx, void* stream);
  *  VR_OPT_OCCUPANCY (default -1): the finest level of the skipping, one bit per trilinear cell,
  *    classified on the device when the set of transparent table entries changes (one pass over the
  *    cube); used by the lockstep marcher for emission-absorption with VR_OPT_DENSE 0 on layout 1.
- *    1 / -1 = on where it applies, 0 = off. */
+ *    1 / -1 = on where it applies, 0 = off.
+ *  VR_OPT_RING (default -1): where the lockstep marcher keeps the gathers in flight, 0 = a ring of
+ *    cp.async slots in shared memory, 1 = registers; -1 = registers iff the central ray runs mostly
+ *    along z, the short axis of the 4 x 4 x 2 micro-blocks (layout 1). */
 enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETCH = 4, VR_OPT_LAYOUT = 5, VR_OPT_DENSE = 6,
-       VR_OPT_OCCUPANCY = 7 };
+       VR_OPT_OCCUPANCY = 7, VR_OPT_RING = 8 };
 int vr_set_option(vr_ctx* ctx, int option, int value);
 /* What a render call of `mode` would launch under the current cube, view and transfer function:
  * out[0] = marcher variant (0 / 3), out[1] = skipping level (0 none, 1 bricks, 2 + macro-cells,

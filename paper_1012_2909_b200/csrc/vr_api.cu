@@ -38,7 +38,7 @@ struct vr_ctx {
     float* d_stage = nullptr;
     size_t stage_bytes = 0;
     int64_t launches = 0;
-    int opt_skip = 1, opt_cell_skip = -1, opt_variant = -1, opt_layout = 1, opt_dense = -1, opt_occ = -1;   // -1: chosen per view / TF
+    int opt_skip = 1, opt_cell_skip = -1, opt_variant = -1, opt_layout = 1, opt_dense = -1, opt_occ = -1, opt_ring = -1;   // -1: chosen per view / TF
     float x_clear = -INFINITY;
     double active_cell_fraction = 1.0;   // macro-cells active against the current table (EA)
     unsigned long long* d_scratch = nullptr;
@@ -273,6 +273,19 @@ int ensure_occ(vr_ctx* ctx, int skip, cudaStream_t s) {
 int resolve_dense(const vr_ctx* ctx) {
     if (ctx->opt_dense >= 0) return ctx->opt_dense;
     return ctx->x_clear >= 1.f ? 0 : 1;
+}
+
+// Lockstep marcher: gathers through registers (1) or through the cp.async ring in shared memory (0).
+// Measured (vr_march.cu, REGS): registers win when the rays run mostly along z, the short axis of the
+// 4 x 4 x 2 micro-blocks, where a request meets the most sectors.
+int resolve_ring(const vr_ctx* ctx) {
+    if (ctx->opt_ring >= 0) return ctx->opt_ring;
+    if (ctx->cube.layout != 1) return 0;
+    const double* Mi = ctx->Minv;
+    double pn[4], pf[4], d[3];
+    for (int r = 0; r < 4; ++r) { pn[r] = -Mi[4 * r + 2] + Mi[4 * r + 3]; pf[r] = Mi[4 * r + 2] + Mi[4 * r + 3]; }   // central pixel, near / far
+    for (int a = 0; a < 3; ++a) d[a] = std::fabs(pf[a] / pf[3] - pn[a] / pn[3]);
+    return (std::isfinite(d[2]) && d[2] > d[0] && d[2] > d[1]) ? 1 : 0;
 }
 
 TFDesc tf_desc(const vr_ctx* ctx) {
@@ -622,7 +635,7 @@ int vr_render_mip(vr_ctx* ctx, float* d_out, float* d_out_rgba, float miss, void
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
-    a.mode = VR_MODE_MIP; a.tau = 2.f; a.miss = miss; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx);
+    a.mode = VR_MODE_MIP; a.tau = 2.f; a.miss = miss; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx); a.ring = resolve_ring(ctx);
     a.out = d_out; a.out_rgba = d_out_rgba; a.counters = ctx->d_counters;
     VR_CUDA(ctx, launch_render_global(ctx->cube, ctx->view, tf_desc(ctx), a, s));
     ctx->launches += 1;
@@ -638,7 +651,7 @@ int vr_render_ea(vr_ctx* ctx, float* d_out, const float bg[4], float tau, void* 
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
-    a.mode = VR_MODE_EA; a.tau = tau; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx); a.dense = resolve_dense(ctx);
+    a.mode = VR_MODE_EA; a.tau = tau; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx); a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
     for (int i = 0; i < 4; ++i) a.bg[i] = bg[i];
     a.out = d_out; a.counters = ctx->d_counters;
     if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
@@ -779,7 +792,7 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
     int tiles = 0;
     if ((rc = upload_partials(ctx, mode, hp, n, true, &tiles, s))) return rc;
     RenderArgs a{};
-    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx); a.dense = resolve_dense(ctx);
+    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx); a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
     a.counters = ctx->d_counters;
     if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
     VR_CUDA(ctx, launch_render_bricks(ctx->cube, ctx->view, tf_desc(ctx), a, ctx->d_partials, n, tiles, s));
@@ -885,6 +898,7 @@ int vr_set_option(vr_ctx* ctx, int option, int value) {
         VR_CUDA(ctx, cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)value));
         return VR_OK;
     }
+    if (option == VR_OPT_RING) { ctx->opt_ring = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_OCCUPANCY) { ctx->opt_occ = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_DENSE) { ctx->opt_dense = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_VARIANT) {

@@ -103,6 +103,7 @@ struct RenderArgs {
     int mode; float tau; float bg[4]; float miss;
     int skip;              // 0: none; 1: configured bricks; 2: + 8^3 macro-cells; 3: + occupancy bits (O-10)
     int variant;           // 0: one ray per thread; 3: lockstep (the lanes of a warp take one ray's samples)
+    int ring;              // lockstep marcher: 0 gathers through the cp.async ring in shared memory, 1 through registers
     int dense;             // lockstep EA: fold through shared memory, all rays in parallel (see vr_march.cu)
     float* out; float* out_rgba; unsigned long long* counters;
 };

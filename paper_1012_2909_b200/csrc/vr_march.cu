@@ -524,6 +524,11 @@ render_tiles_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ 
 //                the chunk every lane folds the 32 values of ITS ray front to back (all 32 rays
 //                in parallel), so opaque transfer functions cost the same as sparse ones.
 // Skipped samples (O-10) are never interpolated or folded.  All three give identical frames.
+//
+// REGS: the same ring in REGISTERS (plain loads, 3 rays ahead, 5 CTAs per SM).  The shared-memory side
+// of a 4-byte cp.async takes one L1 wavefront per arriving sector; rays that run along z (the short
+// axis of the 4 x 4 x 2 micro-blocks) meet the most sectors per request and are faster with plain
+// loads (MIP on C3: 17.3 -> 14.7 ms), rays along x or y with cp.async (12.7 vs 14.1 ms): RenderArgs::ring.
 constexpr int kValPitch = 33;
 constexpr int kDepth = 3;               // rays in flight per warp (measured: 2 -> 12.1, 3 -> 12.0, 4 -> 13.5 ms on C3)
 constexpr int kBitsWords = 1024;        // shared copy of one brick's macro-cell bits (256^3 bricks: 32^3 cells)
@@ -547,11 +552,11 @@ __device__ __forceinline__ void gather8_async(const BrickRef& b, int ix, int iy,
     cp_async4(dst + 768, p + dz + dy); cp_async4(dst + 896, p + dz + dy + dx);
 }
 
-struct Slot { float w[3]; int rc; bool idle; };   // one ray in flight: weights of this lane's sample
+struct Slot { float w[3]; int rc; bool idle; float v[8]; };   // one ray in flight: weights of this lane's sample (v: register ring only)
 
 // 7 CTAs per SM: 72 registers; an 8th CTA (64 registers) would shrink L1 to 28 KB and costs 10 % (measured)
-template <int MODE, int LAYOUT, bool GLOBAL, bool DENSE>
-__global__ void __launch_bounds__(kThreads, 7)
+template <int MODE, int LAYOUT, bool GLOBAL, bool DENSE, bool REGS>
+__global__ void __launch_bounds__(kThreads, REGS ? 5 : 7)
 render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                  const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
                  const PartialDev* __restrict__ parts, int n_parts) {
@@ -562,7 +567,7 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
     __shared__ float4 tab[EA ? 256 : 1];
     __shared__ PartialDev part;
     __shared__ float4 rays_all[kWarps][64];
-    __shared__ float stage_all[kWarps][kDepth * 256];
+    __shared__ float stage_all[REGS ? 1 : kWarps][REGS ? 1 : kDepth * 256];
     __shared__ float vals_all[VALS ? kWarps : 1][VALS ? 32 * kValPitch : 1];
     __shared__ unsigned sbits[SBITS ? kBitsWords : 1];
     int fx, fy;                                             // view pixel of this thread's ray
@@ -599,7 +604,7 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float* vals = vals_all[VALS ? warp : 0];
     float4* rays = rays_all[warp];
-    const float* stage = stage_all[warp] + lane;
+    const float* stage = stage_all[REGS ? 0 : warp] + (REGS ? 0 : lane);
     const unsigned stage_addr = (unsigned)__cvta_generic_to_shared(stage);
     rays[2 * lane] = make_float4(r.o[0], r.o[1], r.o[2], r.d[0]);
     rays[2 * lane + 1] = make_float4(r.d[1], r.d[2], __int_as_float(ka), __int_as_float(kb));
@@ -625,6 +630,10 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
         auto issue = [&](Slot& S, const int s) {
             S.rc = -1; S.idle = true;
             S.w[0] = S.w[1] = S.w[2] = 0.f;
+            if (REGS) {
+#pragma unroll
+                for (int e = 0; e < 8; ++e) S.v[e] = 0.f;
+            }
             if (rest) {
                 const int rr = __ffs(rest) - 1;
                 rest &= rest - 1;
@@ -648,7 +657,10 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
                             if (cells && !idle) idle = cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], m_r);
                         }
                         S.idle = idle;
-                        if (!idle) gather8_async<LAYOUT>(brick_ref<LAYOUT>(c, bid, lo), iv[0], iv[1], iv[2], stage_addr + 1024u * s);
+                        if (!idle) {
+                            if (REGS) gather8<LAYOUT>(brick_ref<LAYOUT>(c, bid, lo), iv[0], iv[1], iv[2], S.v);
+                            else gather8_async<LAYOUT>(brick_ref<LAYOUT>(c, bid, lo), iv[0], iv[1], iv[2], stage_addr + 1024u * s);
+                        }
                     } else {
                         bool idle = false;
                         if (bits_shared) {
@@ -656,7 +668,10 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
                             idle = ((sbits[cidx >> 5] >> (cidx & 31)) & 1u) == 0u;
                         } else if (cells) idle = cell_idle<MODE>(c, bid0, lo0, iv[0], iv[1], iv[2], m_r);
                         S.idle = idle;
-                        if (!idle) gather8_async<LAYOUT>(br0, iv[0], iv[1], iv[2], stage_addr + 1024u * s);
+                        if (!idle) {
+                            if (REGS) gather8<LAYOUT>(br0, iv[0], iv[1], iv[2], S.v);
+                            else gather8_async<LAYOUT>(br0, iv[0], iv[1], iv[2], stage_addr + 1024u * s);
+                        }
                     }
                 }
             }
@@ -665,10 +680,15 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
         unsigned my_fold = 0u, my_done = 0u;                // DENSE: this lane's ray: samples to fold / interpolated
         // interpolate the samples of the ray in slot s (its copies have landed) and fold them
         auto consume = [&](const Slot& S, const int s) {
-            const float* st = stage + 256 * s;
             float v[8];
+            if (REGS) {
 #pragma unroll
-            for (int e = 0; e < 8; ++e) v[e] = st[32 * e];
+                for (int e = 0; e < 8; ++e) v[e] = S.v[e];
+            } else {
+                const float* st = stage + 256 * s;
+#pragma unroll
+                for (int e = 0; e < 8; ++e) v[e] = st[32 * e];
+            }
             const float val = trilinear(v, S.w[0], S.w[1], S.w[2]);       // idle lanes: stale values, never used
             const unsigned done_bits = __ballot_sync(0xffffffffu, !S.idle);
             if (!EA) {
@@ -1088,18 +1108,24 @@ __global__ void upload_half_kernel(float4* dst, const __grid_constant__ HalfTabl
         }                                                                                                \
     } while (0)
 
-#define VR_DISPATCH_LS(GLOBAL, GRID, ...)                                                                \
+#define VR_DISPATCH_LS2(GLOBAL, REGS, GRID, ...)                                                          \
     do {                                                                                                 \
         if (a.mode == VR_MODE_MIP) {                                                                     \
-            if (c.layout == 0) render_ls_kernel<VR_MODE_MIP, 0, GLOBAL, false><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
-            else render_ls_kernel<VR_MODE_MIP, 1, GLOBAL, false><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);  \
+            if (c.layout == 0) render_ls_kernel<VR_MODE_MIP, 0, GLOBAL, false, REGS><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
+            else render_ls_kernel<VR_MODE_MIP, 1, GLOBAL, false, REGS><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);  \
         } else if (a.dense) {                                                                            \
-            if (c.layout == 0) render_ls_kernel<VR_MODE_EA, 0, GLOBAL, true><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
-            else render_ls_kernel<VR_MODE_EA, 1, GLOBAL, true><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);    \
+            if (c.layout == 0) render_ls_kernel<VR_MODE_EA, 0, GLOBAL, true, REGS><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
+            else render_ls_kernel<VR_MODE_EA, 1, GLOBAL, true, REGS><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);    \
         } else {                                                                                         \
-            if (c.layout == 0) render_ls_kernel<VR_MODE_EA, 0, GLOBAL, false><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
-            else render_ls_kernel<VR_MODE_EA, 1, GLOBAL, false><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);   \
+            if (c.layout == 0) render_ls_kernel<VR_MODE_EA, 0, GLOBAL, false, REGS><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
+            else render_ls_kernel<VR_MODE_EA, 1, GLOBAL, false, REGS><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);   \
         }                                                                                                \
+    } while (0)
+
+#define VR_DISPATCH_LS(GLOBAL, GRID, ...)                                                                \
+    do {                                                                                                 \
+        if (a.ring) VR_DISPATCH_LS2(GLOBAL, true, GRID, __VA_ARGS__);                                    \
+        else VR_DISPATCH_LS2(GLOBAL, false, GRID, __VA_ARGS__);                                          \
     } while (0)
 
 // the occupancy marcher serves sparse emission-absorption on the micro-block layout
