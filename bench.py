@@ -96,10 +96,10 @@ def orbit_frame(w, step_index, n_steps, rank, world):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the marcher, from the committed
 # `ncu --set full` captures (profiles/r1d_c3_render_occ_full.md: orbit frames 0 and 180, 11.26 and 8.08 GB read + written, their mean; r1d_c3_mip_render_ls_full.md: frame 0).  None: not captured.
-NCU_TRAFFIC_BYTES = {("C3", "ea"): 9.67e9, ("C3", "mip"): 70.8e9}
+NCU_TRAFFIC_BYTES = {("C3", "ea"): 9.67e9, ("C3", "mip"): 70.3e9}
 # smsp__inst_executed.sum (warp instructions) per launch from the same captures, and the issue peak
 # DESIGN.md section 8 derives: 148 SMs x 4 schedulers x 1 warp instruction per clock.
-NCU_WARP_INSTRUCTIONS = {("C3", "ea"): 4.54e9, ("C3", "mip"): 8.25e9}
+NCU_WARP_INSTRUCTIONS = {("C3", "ea"): 4.54e9, ("C3", "mip"): 8.28e9}
 ISSUE_SLOTS_PER_CLOCK = 148 * 4
 
 MARCHER = {(0, 0): "render_bricks_kernel<EA> (ray per thread)", (0, 1): "render_bricks_kernel<EA> (ray per thread)",
