@@ -107,7 +107,7 @@ struct Vol {
     float at(int i, int j, int k) const {
         int bi = i / v->bx, bj = j / v->by, bk = k / v->bz;
         const float* B = v->bricks[bi + gx * (bj + gy * bk)];
-        if (!B) { missing = true; return std::numeric_limits<float>::quiet_NaN(); }
+        if (!B) { missing = true; return 0.0f; }           // the call then returns OVR_ERR_MISSING; 0 keeps the table index finite
         int ex = std::min(v->bx, v->nx - bi * v->bx), ey = std::min(v->by, v->ny - bj * v->by);
         return B[(int64_t)(i - bi * v->bx) + (int64_t)ex * ((j - bj * v->by) + (int64_t)ey * (k - bk * v->bz))];
     }

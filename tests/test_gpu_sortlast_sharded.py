@@ -96,3 +96,74 @@ def test_window_refuses_whole_frame_renders_and_foreign_bricks():
     full.download_brick(sh.first, t2)
     torch.cuda.synchronize()
     assert torch.equal(t, t2)
+
+
+def test_wallaby_scale_slab_one_rank_of_many():
+    """the WALLABY cube, 6144 x 6144 x 16384 (2.25 TiB at 4 bytes, line 13 "2.2
+    terabyte"), is what the framework is meant to reach.  One B200 holds one rank's share of it: rank
+    20 of a 32-way z-slab split = 2 layers of 24 x 24 bricks of 256^3 (1152 bricks, 77 GB), with GLOBAL
+    voxel coordinates up to 16384 and GLOBAL brick ids (23040...) whose occupancy-word offsets pass
+    2^32.  Its partial images are compared, on sampled pixels, with the oracle's partial image of the
+    same brick (float32 instantiation, bit for bit)."""
+    import torch
+    from paper_1012_2909_b200 import sortlast as sl, vr, workloads as wl
+    from oracle import ovr
+    free, _ = torch.cuda.mem_get_info()
+    if free < 95e9:
+        pytest.skip("needs ~85 GB of free HBM")
+    w = wl.scaled(wl.C3, "WALLABY-shaped", (6144, 6144, 16384), (256, 256, 256), (1920, 1080), n_sources=6000)
+    assert w.brick_grid == (24, 24, 64)
+    world, rank = 32, 20
+    ctx = vr.Context(0)
+    sh = sl.Shard(ctx, w.dims, w.brick, rank, world)
+    assert (sh.first, sh.end) == (24 * 24 * 40, 24 * 24 * 42)
+    assert sh.end * 32 * 32 * 32 * 16 > 2 ** 32                 # occupancy words before the slab's last brick
+    sh.bind()
+    cb, mb = sh.layout()
+    d_cube = torch.empty(cb // 4, dtype=torch.float32, device="cuda")
+    d_meta = torch.empty(mb, dtype=torch.uint8, device="cuda")
+    ctx.generate_cube(w.seed, w.dims, w.brick, d_cube, d_meta, sources=wl.make_sources(w), continuum=w.continuum)
+    W, H = w.frame
+    M = wl.perspective_camera(w.dims, w.frame, azimuth_deg=35.0)
+    tf = wl.tf_src()
+    ctx.set_view(M, W, H, w.step)
+    ctx.set_transfer_function(*tf)
+    for mode, omode in ((vr.MODE_EA, ovr.EA), (vr.MODE_MIP, ovr.MIP)):
+        ids = ctx.sort_bricks(mode)
+        assert len(ids) > 100 and set(ids) <= set(range(sh.first, sh.end))
+        parts, n, nbytes = ctx.partial_layout(mode, ids)
+        arena = torch.zeros(nbytes + 256, dtype=torch.uint8, device="cuda")
+        offs = [(parts[i].d_data or 0) for i in range(n)]
+        vr.Context.bind_partials(parts, n, arena)
+        ctx.render_bricks(mode, parts, n, 0.99)
+        torch.cuda.synchronize()
+        host = arena.cpu().numpy()
+        ch = 4 if mode == vr.MODE_EA else 1
+        # bricks of the slab's lower layer away from the grid's +x / +y faces: the oracle stores plain bricks
+        # (no halo), so it needs the 2 x 2 x 2 neighbourhood, which is resident for these
+        ok = [i for i in range(n) if parts[i].brick // 576 == 40 and parts[i].brick % 24 < 23 and (parts[i].brick // 24) % 24 < 23]
+        assert len(ok) > 20
+        for i in (ok[0], ok[len(ok) // 2], ok[-1]):
+            p = parts[i]
+            img = host[offs[i]:offs[i] + 4 * ch * p.w * p.h].view(np.float32).reshape(p.h, p.w, ch)
+            bricks = {}
+            for dz in (0, 1):
+                for dy in (0, 1):
+                    for dx in (0, 1):
+                        nbid = int(p.brick) + dx + 24 * dy + 576 * dz
+                        t = torch.empty(256 ** 3, dtype=torch.float32, device="cuda")
+                        ctx.download_brick(nbid, t)
+                        bricks[nbid] = t.cpu().numpy().reshape(256, 256, 256)
+                        del t
+            vol = ovr.Volume(w.dims, w.brick, bricks)
+            bw, bh = min(6, p.w), min(6, p.h)
+            rx, ry = p.x0 + (p.w - bw) // 2, p.y0 + (p.h - bh) // 2
+            want = ovr.render_brick(vol, M, W, H, w.step, omode, int(p.brick), (rx, ry, bw, bh), w.brick,
+                                    precision=ovr.F32, tf=tf, tau=0.99)
+            got = img[ry - p.y0:ry - p.y0 + bh, rx - p.x0:rx - p.x0 + bw]
+            got = got if ch == 4 else got[..., 0]
+            assert np.isfinite(want).any()
+            assert np.array_equal(got, want), (mode, int(p.brick))
+    part = sh.render_partial(torch, vr.MODE_EA, W, H, 0.99)
+    torch.cuda.synchronize()
+    assert float(part[..., 3].max()) <= 1.0 + 1e-6 and float(part[..., 3].min()) >= 0.0
