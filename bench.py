@@ -102,9 +102,9 @@ NCU_TRAFFIC_BYTES = {("C3", "ea"): 9.67e9, ("C3", "mip"): 70.3e9}
 NCU_WARP_INSTRUCTIONS = {("C3", "ea"): 4.54e9, ("C3", "mip"): 8.28e9}
 ISSUE_SLOTS_PER_CLOCK = 148 * 4
 
-MARCHER = {(0, 0): "render_bricks_kernel<EA> (ray per thread)", (0, 1): "render_bricks_kernel<EA> (ray per thread)",
-           (0, 2): "render_bricks_kernel<EA> (ray per thread, macro-cell runs)",
-           (0, 3): "render_bricks_kernel<EA> (ray per thread, macro-cell runs + occupancy bits)",
+MARCHER = {(0, 0): "render_tiles_kernel<EA> (ray per thread)", (0, 1): "render_tiles_kernel<EA> (ray per thread)",
+           (0, 2): "render_tiles_kernel<EA> (ray per thread, macro-cell runs)",
+           (0, 3): "render_tiles_kernel<EA> (ray per thread, macro-cell runs + occupancy bits)",
            (3, 3): "render_occ_kernel (lockstep: occupancy test, compaction, cp.async gather, fold)"}
 
 
@@ -382,10 +382,10 @@ def main():
     peak = float(peaks["hbm_gbs"])
     plan = job.ctx.get_plan(job.mode)
     kernel = MARCHER.get((plan["variant"], plan["skip_level"]),
-                         "render_ls_kernel<EA> (lockstep, cp.async gather)" if plan["variant"] == 3 else "render_bricks_kernel<EA>")
+                         "render_ls_kernel<EA> (lockstep, cp.async gather)" if plan["variant"] == 3 else "render_tiles_kernel<EA>")
     if args.mode == "mip":
         kernel = ("render_ls_kernel<MIP> (lockstep, cp.async gather, warp-reduced maximum)" if plan["variant"] == 3
-                  else "render_bricks_kernel<MIP> (ray per thread)")
+                  else "render_tiles_kernel<MIP> (ray per thread)")
     traffic = NCU_TRAFFIC_BYTES.get((w.name, args.mode)) if not args.frame else None
     launch_s = march_ms / max(n_march, 1) * 1e-3
     winst = NCU_WARP_INSTRUCTIONS.get((w.name, args.mode)) if not args.frame else None
