@@ -315,13 +315,21 @@ __device__ __forceinline__ bool march_interval(const CubeDesc& c, const Ray& r, 
     while (k <= ke) {
         int n = ke - k + 1;
         if (A.skip >= 2) {
-            float p[3], fl;
-            position(r, kf, p);
-            const int iv[3] = {floor_pos(p[0], fl), floor_pos(p[1], fl), floor_pos(p[2], fl)};
-            const int clo[3] = {lo[0] + (((iv[0] - lo[0]) >> 3) << 3), lo[1] + (((iv[1] - lo[1]) >> 3) << 3),
-                                lo[2] + (((iv[2] - lo[2]) >> 3) << 3)};
-            n = min(n, run_length(r, p, clo, S8));
-            if (cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], acc.m)) { k += n; kf = __fadd_rn(kf, (float)n); ++st.skip; continue; }
+            // A loop of its own over the idle runs: the lanes of a warp meet again behind it, each at the start
+            // of an ACTIVE run (or at the end of its interval), and take the samples below together.  In one
+            // loop with the samples, a lane in an idle run would wait for the lanes sampling, then sample alone.
+            for (;;) {
+                float p[3], fl;
+                position(r, kf, p);
+                const int iv[3] = {floor_pos(p[0], fl), floor_pos(p[1], fl), floor_pos(p[2], fl)};
+                const int clo[3] = {lo[0] + (((iv[0] - lo[0]) >> 3) << 3), lo[1] + (((iv[1] - lo[1]) >> 3) << 3),
+                                    lo[2] + (((iv[2] - lo[2]) >> 3) << 3)};
+                n = min(ke - k + 1, run_length(r, p, clo, S8));
+                if (!cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], acc.m)) break;
+                k += n; kf = __fadd_rn(kf, (float)n); ++st.skip;
+                if (k > ke) { n = 0; break; }
+            }
+            if (n == 0) break;
         }
         ++st.visit;
         if (JUMP && block_jumps) {
