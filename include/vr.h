@@ -61,7 +61,8 @@ int vr_cube_layout(int nx, int ny, int nz, int bx, int by, int bz, size_t* cube_
 
 /* Rebrick a linear x-fastest float32 cube (host if src_is_device == 0, else device) into d_cube
  * and compute d_meta.  Host sources are streamed slab by slab through a library staging buffer;
- * the call returns after the last slab was enqueued (it synchronises `stream` between slabs). */
+ * the call returns after the last slab was enqueued (it synchronises `stream` between slabs).
+ * Non-finite voxels (NaN, inf) are counted while rebricking: VR_ERR_INVALID_ARG, and no cube is set. */
 int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int ny, int nz,
                    int bx, int by, int bz, void* d_cube, void* d_meta, void* stream);
 

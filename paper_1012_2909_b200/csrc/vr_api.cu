@@ -498,8 +498,9 @@ int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int
     apply_window(ctx, c);
     bind_meta(c, d_cube, d_meta);
     VR_CUDA(ctx, cudaMemsetAsync(d_cube, 0, cube_bytes(c), s));
+    VR_CUDA(ctx, cudaMemsetAsync(ctx->d_scratch, 0, sizeof(unsigned long long), s));
     if (src_is_device) {
-        VR_CUDA(ctx, launch_rebrick(c, const_cast<float*>(c.cube), src, 0, nz, s));
+        VR_CUDA(ctx, launch_rebrick(c, const_cast<float*>(c.cube), src, 0, nz, ctx->d_scratch, s));
         ctx->launches += 1;
     } else {
         const size_t plane = (size_t)nx * ny * sizeof(float);
@@ -514,11 +515,15 @@ int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int
         for (int z0 = 0; z0 < nz; z0 += planes) {
             int z1 = std::min(nz, z0 + planes);
             VR_CUDA(ctx, cudaMemcpyAsync(ctx->d_stage, src + (size_t)z0 * nx * ny, plane * (z1 - z0), cudaMemcpyHostToDevice, s));
-            VR_CUDA(ctx, launch_rebrick(c, const_cast<float*>(c.cube), ctx->d_stage, z0, z1, s));
+            VR_CUDA(ctx, launch_rebrick(c, const_cast<float*>(c.cube), ctx->d_stage, z0, z1, ctx->d_scratch, s));
             ctx->launches += 1;
             VR_CUDA(ctx, cudaStreamSynchronize(s));          // the staging slab is reused
         }
     }
+    unsigned long long n_bad = 0;
+    VR_CUDA(ctx, cudaMemcpyAsync(&n_bad, ctx->d_scratch, sizeof(n_bad), cudaMemcpyDeviceToHost, s));
+    VR_CUDA(ctx, cudaStreamSynchronize(s));
+    if (n_bad) return fail(ctx, VR_ERR_INVALID_ARG, "vr_upload_cube: the cube holds " + std::to_string(n_bad) + " non-finite voxels (NaN / inf)");
     return finish_cube(ctx, s);
 }
 

@@ -40,7 +40,7 @@ __host__ __device__ inline long long slots_per_brick(const CubeDesc& c) {
 }
 
 __global__ void rebrick_kernel(CubeDesc c, float* __restrict__ cube, const float* __restrict__ src,
-                               int z0, int z1, int brick_lo, long long n_elems) {
+                               int z0, int z1, int brick_lo, long long n_elems, unsigned long long* __restrict__ n_bad) {
     const long long per = slots_per_brick(c);
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n_elems;
          e += (long long)gridDim.x * blockDim.x) {
@@ -48,8 +48,9 @@ __global__ void rebrick_kernel(CubeDesc c, float* __restrict__ cube, const float
         if (brick < c.win_lo || brick >= c.win_hi) continue;
         Elem el = decode(c, brick, rem);
         if (!el.in_cube || el.g[2] < z0 || el.g[2] >= z1) continue;
-        cube[brick * c.stride + rem] =
-            src[(size_t)el.g[0] + (size_t)c.N[0] * ((size_t)el.g[1] + (size_t)c.N[1] * (size_t)(el.g[2] - z0))];
+        const float v = src[(size_t)el.g[0] + (size_t)c.N[0] * ((size_t)el.g[1] + (size_t)c.N[1] * (size_t)(el.g[2] - z0))];
+        cube[brick * c.stride + rem] = v;
+        if (!isfinite(v)) atomicAdd(n_bad, 1ULL);         // NaN / inf voxels are refused by vr_upload_cube (never taken: rare path)
     }
 }
 
@@ -176,7 +177,8 @@ int grid_for(long long n, int threads) {
 
 }  // namespace
 
-cudaError_t launch_rebrick(const CubeDesc& c, float* d_cube, const float* d_src, int z0, int z1, cudaStream_t s) {
+cudaError_t launch_rebrick(const CubeDesc& c, float* d_cube, const float* d_src, int z0, int z1, unsigned long long* d_bad,
+                           cudaStream_t s) {
     // bricks whose stored z range [bz*B2, bz*B2 + B2] meets [z0, z1)
     int bz_lo = (z0 - c.B[2] + c.B[2] - 1) / c.B[2];
     if (z0 - c.B[2] <= 0) bz_lo = 0;
@@ -185,7 +187,7 @@ cudaError_t launch_rebrick(const CubeDesc& c, float* d_cube, const float* d_src,
     long long layer = (long long)c.G[0] * c.G[1];
     long long per = slots_per_brick(c);
     long long n = layer * (bz_hi - bz_lo + 1) * per;
-    rebrick_kernel<<<grid_for(n, 256), 256, 0, s>>>(c, d_cube, d_src, z0, z1, (int)(layer * bz_lo), n);
+    rebrick_kernel<<<grid_for(n, 256), 256, 0, s>>>(c, d_cube, d_src, z0, z1, (int)(layer * bz_lo), n, d_bad);
     return cudaGetLastError();
 }
 

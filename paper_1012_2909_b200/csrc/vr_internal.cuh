@@ -90,7 +90,8 @@ struct MetaLayout { size_t brick_mm, cell_mm, cell_bits, brick_active, occ, tota
 MetaLayout meta_layout(const CubeDesc& c);
 
 // kernels' host launchers (vr_cube.cu / vr_march.cu / vr_composite.cu)
-cudaError_t launch_rebrick(const CubeDesc& c, float* d_cube, const float* d_src, int z0, int z1, cudaStream_t s);
+cudaError_t launch_rebrick(const CubeDesc& c, float* d_cube, const float* d_src, int z0, int z1, unsigned long long* d_bad,
+                           cudaStream_t s);
 cudaError_t launch_unbrick(const CubeDesc& c, int brick, float* d_dst, cudaStream_t s);
 cudaError_t launch_minmax(const CubeDesc& c, cudaStream_t s);
 struct GenDev {

@@ -592,6 +592,30 @@ def test_config_c5_full_size_128gib(H, marcher):
     _tiled_fullsize_check(H, wl.C5, panels=[(2, 2), (1, 3)], block=6, mip_frame=(1920, 1080))
 
 
+def test_upload_refuses_non_finite_voxels(H):
+    import torch
+    from paper_1012_2909_b200 import vr
+    dims, brick = (20, 12, 9), (8, 8, 8)
+    for bad in (np.nan, np.inf, -np.inf):
+        cube = noise_cube(dims[::-1], seed=2)
+        cube[4, 7, 13] = bad
+        cb, mb = vr.cube_layout(dims, brick)
+        d_cube = torch.empty(cb // 4, dtype=torch.float32, device="cuda")
+        d_meta = torch.empty(mb, dtype=torch.uint8, device="cuda")
+        ctx = vr.Context(0)
+        with pytest.raises(vr.VRError) as e:
+            ctx.upload_cube(cube, dims, brick, d_cube, d_meta)
+        assert e.value.status == vr.ERR_INVALID_ARG and "non-finite" in str(e.value)
+        with pytest.raises(vr.VRError) as e:                      # and the same from device memory
+            ctx.upload_cube(torch.from_numpy(cube).cuda(), dims, brick, d_cube, d_meta)
+        assert e.value.status == vr.ERR_INVALID_ARG
+        ctx.set_view(np.eye(4, dtype=np.float32), 8, 8, 0.5)
+        out = torch.empty((8, 8), dtype=torch.float32, device="cuda")
+        with pytest.raises(vr.VRError) as e:
+            ctx.render_mip(out)                                     # no cube was set
+        assert e.value.status == vr.ERR_STATE
+
+
 def test_brick_and_macro_cell_minmax_against_numpy(H):
     """S0 metadata (white box: d_meta starts with (min,max) per brick, then per 8^3 macro-cell, each
     region 256-byte aligned): min / max over the region's voxels plus the +1 layer, clipped to the
