@@ -395,7 +395,7 @@ __device__ __forceinline__ void write_frame_pixel(const ViewDesc& V, const TFDes
 }
 
 // ---------------------------------------------------------------- whole frame, O-8 GLOBAL
-template <int MODE, int LAYOUT>
+template <int MODE, int LAYOUT, bool JUMP = false>
 __global__ void __launch_bounds__(kThreads)
 render_global_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                      const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A) {
@@ -425,7 +425,7 @@ render_global_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
             else skip = c.brick_active[bid] == 0;
         }
         if (skip) { k += n; ++st.skip; continue; }
-        if (march_interval<MODE, LAYOUT>(c, r, T, A, tab, bid, lo, k, k + n - 1, acc, st)) { stopped = true; break; }
+        if (march_interval<MODE, LAYOUT, JUMP>(c, r, T, A, tab, bid, lo, k, k + n - 1, acc, st)) { stopped = true; break; }
         k += n;
     }
     if (live) write_frame_pixel<MODE>(V, T, A, i, j, acc, r.k1 >= r.k0);
@@ -1175,6 +1175,8 @@ cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFD
     dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
     if (use_occ_kernel(c, a)) { render_occ_kernel<true><<<grid, kThreads, 0, s>>>(c, v, t, a, nullptr, 0); return cudaGetLastError(); }
     if (a.variant == 3) VR_DISPATCH_LS(true, grid, c, v, t, a, nullptr, 0);
+    else if (a.mode == VR_MODE_EA && c.layout == 1 && a.skip >= 3 && v.step < kJumpStep)     // small steps: jump out of idle micro-blocks
+        render_global_kernel<VR_MODE_EA, 1, true><<<grid, kThreads, 0, s>>>(c, v, t, a);
     else VR_DISPATCH(render_global_kernel, grid, c, v, t, a);
     return cudaGetLastError();
 }
