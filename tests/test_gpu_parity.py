@@ -471,6 +471,7 @@ def test_config_c3_full_size_64gib(H, marcher):
     if marcher not in ("auto", "v0"):
         pytest.skip("full sizes run with the library's choice (what bench.py times) and variant 0")
     import torch
+    torch.cuda.empty_cache()
     free, total = torch.cuda.mem_get_info()
     if free < 80e9:
         pytest.skip("needs ~70 GB of free HBM")
@@ -485,6 +486,7 @@ def test_hipass_shaped_cube_with_partial_edge_bricks(H, marcher):
     if marcher != "auto":
         pytest.skip("run once, with the library's choice")
     import torch
+    torch.cuda.empty_cache()
     free, total = torch.cuda.mem_get_info()
     if free < 20e9:
         pytest.skip("needs ~14 GB of free HBM")
@@ -586,6 +588,7 @@ def test_config_c5_full_size_128gib(H, marcher):
     if marcher != "auto":
         pytest.skip("full sizes run with the library's choice (what bench.py times)")
     import torch
+    torch.cuda.empty_cache()
     free, total = torch.cuda.mem_get_info()
     if free < 150e9:
         pytest.skip("needs ~142 GB of free HBM")

@@ -108,6 +108,7 @@ def test_wallaby_scale_slab_one_rank_of_many():
     import torch
     from paper_1012_2909_b200 import sortlast as sl, vr, workloads as wl
     from oracle import ovr
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < 95e9:
         pytest.skip("needs ~85 GB of free HBM")
