@@ -6,7 +6,12 @@ S1 vr_set_view + vr_sort_bricks (host), S2-S4 vr_render_bricks (the ray marcher,
 images), S5 vr_composite_bricks (sort-last fold), S6 the tiled frame when the workload has panels.
 The cube (S0) is generated on the device once, before the timed region.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3] [--mode ea|mip] [--impl reference]
+
+The headline line is C3 (BASELINE.json configs[2]: the 64 GiB cube at 1920 x 1080, emission-
+absorption).  With the default arguments on one GPU the same JSON line also carries `configs`: the
+other halves of BASELINE.json's metric measured the same way (C3 MIP, C3 with the nothing-skippable
+table, C2, C4 and C5 at 9600 x 5400, C5 MIP), each cube generated, measured and freed in turn.
 
 N > 1 (torchrun): "replicas only" - every rank holds its own copy of the cube and renders its own
 frames of the orbit; there is no data-path collective (BASELINE.json north_star: "no sharding and
@@ -22,6 +27,7 @@ import os
 import sys
 import threading
 import time
+from dataclasses import replace
 
 import numpy as np
 
@@ -32,6 +38,8 @@ from paper_1012_2909_b200 import workloads as wl  # noqa: E402
 from paper_1012_2909_b200.replicas import orbit_frame as _orbit_frame, reduce_run  # noqa: E402
 
 METRIC = "ray samples/s (nominal lattice samples inside the cube; BASELINE.json metric)"
+COUNTERS_JSON = os.path.join(ROOT, "profiles", "r2_counters.json")
+ISSUE_SLOTS_PER_CLOCK = 148 * 4      # 148 SMs x 4 warp schedulers x 1 warp instruction per clock
 
 
 def measured_peaks():
@@ -40,6 +48,22 @@ def measured_peaks():
         with open(path) as f:
             return json.load(f), "measured (MEASURED_PEAKS.json)"
     return {"hbm_gbs": 6650.0}, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def ncu_counters(workload, mode, tf, kernel):
+    """Per-launch counters of the marcher from the committed ncu captures (profiles/r2_counters.json,
+    written by `python -m paper_1012_2909_b200.ncu_counters`): nothing is typed into this file."""
+    if not os.path.exists(COUNTERS_JSON):
+        return None, "no capture: profiles/r2_counters.json is absent"
+    with open(COUNTERS_JSON) as f:
+        caps = json.load(f).get("captures", [])
+    hits = [c for c in caps if c["workload"] == workload and c["mode"] == mode and c.get("tf") == tf and c["kernel"] in kernel]
+    if not hits:
+        return None, f"no capture of {kernel} for {workload} {mode} tf-{tf} in profiles/r2_counters.json"
+    c = hits[-1]
+    n = max(1, len(c["dram_bytes"]))
+    return {"traffic": sum(c["dram_bytes"]) / n, "warp_instructions": sum(c["warp_instructions"]) / n,
+            "source": f"{c['source']} (orbit frames {c.get('frames')}, commit {c.get('commit')})"}, None
 
 
 class ClockSampler(threading.Thread):
@@ -94,29 +118,26 @@ def orbit_frame(w, step_index, n_steps, rank, world):
     return _orbit_frame(step_index, n_steps, rank, world)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the marcher, from the committed
-# `ncu --set full` captures (profiles/r1d_c3_render_occ_full.md: orbit frames 0 and 180, 11.26 and 8.08 GB read + written, their mean; r1d_c3_mip_render_ls_full.md: frame 0).  None: not captured.
-NCU_TRAFFIC_BYTES = {("C3", "ea"): 9.67e9, ("C3", "mip"): 70.3e9}
-# smsp__inst_executed.sum (warp instructions) per launch from the same captures, and the issue peak
-# DESIGN.md section 8 derives: 148 SMs x 4 schedulers x 1 warp instruction per clock.
-NCU_WARP_INSTRUCTIONS = {("C3", "ea"): 4.54e9, ("C3", "mip"): 8.28e9}
-ISSUE_SLOTS_PER_CLOCK = 148 * 4
-
-MARCHER = {(0, 0): "render_tiles_kernel<EA> (ray per thread)", (0, 1): "render_tiles_kernel<EA> (ray per thread)",
-           (0, 2): "render_tiles_kernel<EA> (ray per thread, macro-cell runs)",
-           (0, 3): "render_tiles_kernel<EA> (ray per thread, macro-cell runs + occupancy bits)",
-           (3, 3): "render_occ_kernel (lockstep: occupancy test, compaction, cp.async gather, fold)"}
+def kernel_name(plan, mode):
+    """The marcher vr_render_bricks launches under a plan (vr_get_plan)."""
+    v, skip, dense = plan["variant"], plan["skip_level"], plan["dense"]
+    m = "EA" if mode == "ea" else "MIP"
+    if v == 3:
+        if mode == "ea" and skip >= 3:
+            return "render_occ_kernel (lockstep: occupancy test, compaction, gather, fold)"
+        return f"render_ls_kernel<{m}> (lockstep{', dense fold' if dense and mode == 'ea' else ''})"
+    if v == 1:
+        return f"render_bricks_kernel<{m}> (ray per thread, CTA per (brick, tile))"
+    return f"render_tiles_kernel<{m}> (ray per thread, skip level {skip})"
 
 
 class Job:
-    """One rank's resident cube + context."""
+    """One rank's resident cube + context.  configure() picks mode / table / frame without regenerating."""
 
-    def __init__(self, w, device, mode="ea", shard=None, dist=None):
+    def __init__(self, w, device, mode="ea", shard=None, dist=None, tf=None):
         import torch
         from paper_1012_2909_b200 import vr
         self.torch, self.vr, self.w = torch, vr, w
-        self.mode = vr.MODE_EA if mode == "ea" else vr.MODE_MIP
-        self.px_bytes = 16 if mode == "ea" else 4
         torch.cuda.set_device(device)
         self.ctx = vr.Context(device)
         self.shard, self.dist = None, dist
@@ -135,39 +156,66 @@ class Job:
                                zero_boxes=wl.make_zero_boxes(w), continuum=w.continuum)
         torch.cuda.synchronize()
         self.gen_seconds = time.perf_counter() - t0
-        self.tf = wl.TFS[w.tf]()
+        self.arena = None
+        self.bitmap = None
+        self.bg = (0.0, 0.0, 0.0, 0.0)
+        self.slab_only = False
+        self.configure(mode, tf or w.tf, w.frame, w.panels)
+
+    def configure(self, mode, tf_name, frame, panels):
+        torch, vr = self.torch, self.vr
+        self.mode_name, self.tf_name = mode, tf_name
+        self.mode = vr.MODE_EA if mode == "ea" else vr.MODE_MIP
+        self.px_bytes = 16 if mode == "ea" else 4
+        self.tf = wl.TFS[tf_name]()
         self.ctx.set_transfer_function(*self.tf)
-        self.W, self.H = w.frame
-        self.cols, self.rows = w.panels
+        self.W, self.H = frame
+        self.cols, self.rows = panels
         self.pw, self.ph = self.W // self.cols, self.H // self.rows
         ch = 4 if mode == "ea" else 1
+        self.frame = None
+        self.h_frame = None
         self.frame = torch.zeros((self.H, self.W, ch), dtype=torch.float32, device="cuda")
-        self.arena = None
         self.h_frame = torch.empty((self.H, self.W, ch), dtype=torch.float32).pin_memory()
-        self.step_events = []
-        self.bg = (0.0, 0.0, 0.0, 0.0)
-        self.march_events = []
-        self.alg_bytes = 0
+        self.reset_events()
+
+    def reset_events(self):
+        self.step_events, self.march_events = [], []
+        self.b_brick = self.partial_bytes = 0
+
+    def close(self):
+        self.ctx.close()
+        self.d_cube = self.d_meta = self.arena = self.bitmap = self.frame = self.h_frame = None
+        self.torch.cuda.empty_cache()
 
     def _arena(self, nbytes):
         if self.arena is None or self.arena.numel() < nbytes:
+            self.arena = None
             self.arena = self.torch.empty(int(nbytes * 1.25) + 256, dtype=self.torch.uint8, device="cuda")
         return self.arena
+
+    def brick_voxels(self):
+        n = 1
+        for b, d in zip(self.w.brick, self.w.dims):
+            n *= min(b, d)
+        return n
+
+    def panel_views(self, frame_index):
+        M = wl.config_camera(self.w, frame_index, frame=(self.W, self.H))
+        for r in range(self.rows):
+            for c in range(self.cols):
+                yield c, r, (M if (self.cols, self.rows) == (1, 1) else wl.panel_matrix(M, self.cols, self.rows, c, r))
 
     def step(self, frame_index, timed_events=False, set_tf=False):
         """S1 + S2-S5 (+ S6) for one frame, sort-last path."""
         w, vr, ctx, torch = self.w, self.vr, self.ctx, self.torch
-        M = wl.config_camera(w, frame_index)
         if set_tf:
             ctx.set_transfer_function(*self.tf)
-        brick_vox = 1
-        for b, n in zip(w.brick, w.dims):
-            brick_vox *= min(b, n)
         if self.shard is not None:
             # sharded sort-last (paper_1012_2909_b200/sortlast.py): own bricks -> one partial frame, strips
             # exchanged, folded in the slabs' visibility order, gathered
             sh, sl = self.shard, self.sortlast
-            ctx.set_view(M, self.W, self.H, w.step)
+            ctx.set_view(wl.config_camera(w, frame_index, frame=(self.W, self.H)), self.W, self.H, w.step)
             if timed_events:
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record()
@@ -175,8 +223,9 @@ class Job:
             if timed_events:
                 e1.record()
                 self.march_events.append((e0, e1))
-                self.alg_bytes += 4 * brick_vox * (sh.end - sh.first) + self.H * self.W * self.px_bytes
-            if getattr(self, "slab_only", False):
+                self.b_brick += 4 * self.brick_voxels() * (sh.end - sh.first)
+                self.partial_bytes += self.H * self.W * self.px_bytes
+            if self.slab_only:
                 self.frame = part
             else:
                 versions = sl.exchange_strips(self.dist, part, sh.world)
@@ -187,58 +236,362 @@ class Job:
                 e.record()
                 self.step_events.append(e)
             return
-        for r in range(self.rows):
-            for c in range(self.cols):
-                Mp = M if (self.cols, self.rows) == (1, 1) else wl.panel_matrix(M, self.cols, self.rows, c, r)
-                ctx.set_view(Mp, self.pw, self.ph, w.step)
-                ctx.set_viewport(c * self.pw, r * self.ph, self.W)
-                ids = ctx.sort_bricks(self.mode)
-                parts, n, nbytes = ctx.partial_layout(self.mode, ids)
-                vr.Context.bind_partials(parts, n, self._arena(nbytes))
-                if timed_events:
-                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    e0.record()
-                ctx.render_bricks(self.mode, parts, n, w.tau)
-                if timed_events:
-                    e1.record()
-                    self.march_events.append((e0, e1))
-                    # algorithmic bytes of this launch: the active in-frustum bricks
-                    # read once + the partial images written once
-                    self.alg_bytes += 4 * brick_vox * n + nbytes          # nbytes: the partial images (16 or 4 B per pixel)
-                ctx.composite_bricks(self.mode, parts, n, self.frame, self.bg)
+        for c, r, Mp in self.panel_views(frame_index):
+            ctx.set_view(Mp, self.pw, self.ph, w.step)
+            ctx.set_viewport(c * self.pw, r * self.ph, self.W)
+            ids = ctx.sort_bricks(self.mode)
+            parts, n, nbytes = ctx.partial_layout(self.mode, ids)
+            vr.Context.bind_partials(parts, n, self._arena(nbytes))
+            if timed_events:
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+            ctx.render_bricks(self.mode, parts, n, w.tau)
+            if timed_events:
+                e1.record()
+                self.march_events.append((e0, e1))
+                # B_brick of this launch: the active in-frustum bricks read once;
+                # nbytes: the partial images written once (16 or 4 B per pixel)
+                self.b_brick += 4 * self.brick_voxels() * n
+                self.partial_bytes += nbytes
+            ctx.composite_bricks(self.mode, parts, n, self.frame, self.bg)
         if timed_events:
             e = torch.cuda.Event(enable_timing=True)
             e.record()
             self.step_events.append(e)
 
+    def touch(self, frame_index):
+        """B_touch of every vr_render_bricks launch of one frame: distinct 32-byte sectors and
+        128-byte lines under the footprints of the samples the frame interpolates.  Untimed."""
+        vr, ctx, torch, w = self.vr, self.ctx, self.torch, self.w
+        if self.shard is not None:
+            return None
+        out = {"launches": 0, "sectors": 0, "lines": 0, "taken_samples": 0}
+        for c, r, Mp in self.panel_views(frame_index):
+            ctx.set_view(Mp, self.pw, self.ph, w.step)
+            ctx.set_viewport(c * self.pw, r * self.ph, self.W)
+            ids = ctx.sort_bricks(self.mode)
+            parts, n, nbytes = ctx.partial_layout(self.mode, ids)
+            vr.Context.bind_partials(parts, n, self._arena(nbytes))
+            if self.bitmap is None:
+                self.bitmap = torch.empty(ctx.touch_layout(), dtype=torch.uint8, device="cuda")
+            ctx.measure_touch(self.mode, parts, n, self.bitmap, w.tau)
+            t = ctx.touch_count(self.bitmap)
+            out["launches"] += 1
+            for k in ("sectors", "lines", "taken_samples"):
+                out[k] += t[k]
+        return out
 
-def oracle_sample(job, frame_index, tile, precision_name="F64"):
-    """Time the oracle, as it stands, on a tile x tile pixel block at the frame centre of the
-    same frame (sort-last semantics, same partition, same tau).  Returns (seconds, counters)."""
+
+def fetch_bricks(job, M, W, H, pix, cache):
+    """Cube bytes of the bricks the rays of `pix` meet, fetched back from the device (untimed)."""
     from oracle import ovr
     w, torch = job.w, job.torch
-    M = wl.config_camera(w, frame_index)
-    cx, cy = job.W // 2, job.H // 2
-    xs = np.arange(cx - tile // 2, cx - tile // 2 + tile)
-    ys = np.arange(cy - tile // 2, cy - tile // 2 + tile)
-    pix = np.stack(np.meshgrid(xs, ys), axis=-1).reshape(-1, 2).astype(np.int32)
     brick = tuple(min(b, n) for b, n in zip(w.brick, w.dims))
-    touched = ovr.bricks_touched(M, job.W, job.H, w.step, w.dims, brick, pix)
-    bricks = {}
+    touched = ovr.bricks_touched(M, W, H, w.step, w.dims, brick, pix)
     g = [-(-n // b) for n, b in zip(w.dims, brick)]
-    for b in touched:                       # fetch the cube bytes back from the device (untimed)
+    for b in touched:
+        if int(b) in cache:
+            continue
         bi = (b % g[0], (b // g[0]) % g[1], b // (g[0] * g[1]))
         ext = [min(bb, n - i * bb) for i, bb, n in zip(bi, brick, w.dims)]
         t = torch.empty(ext[0] * ext[1] * ext[2], dtype=torch.float32, device="cuda")
         job.ctx.download_brick(int(b), t)
-        bricks[int(b)] = t.cpu().numpy()
+        cache[int(b)] = t.cpu().numpy()
     torch.cuda.synchronize()
-    vol = ovr.Volume(w.dims, brick, bricks)
-    t0 = time.perf_counter()
+    return ovr.Volume(w.dims, brick, {int(b): cache[int(b)] for b in touched}), brick, len(touched)
+
+
+def oracle_sample(job, frame_index, tile, precision_name="F64", threads=1, cache=None):
+    """Time the oracle, as it stands, on a tile x tile pixel block at the frame centre of the same frame
+    (sort-last semantics, same partition, same tau).  threads > 1: the same code over disjoint interleaved
+    pixel subsets on that many host threads (the ctypes call releases the GIL).  Returns (seconds, counters, bricks)."""
+    from oracle import ovr
+    w = job.w
+    M = wl.config_camera(w, frame_index, frame=(job.W, job.H))
+    cx, cy = job.W // 2, job.H // 2
+    xs = np.arange(max(0, cx - tile // 2), min(job.W, cx - tile // 2 + tile))
+    ys = np.arange(max(0, cy - tile // 2), min(job.H, cy - tile // 2 + tile))
+    pix = np.stack(np.meshgrid(xs, ys), axis=-1).reshape(-1, 2).astype(np.int32)
+    vol, brick, nb = fetch_bricks(job, M, job.W, job.H, pix, {} if cache is None else cache)
     omode = ovr.EA if job.mode == job.vr.MODE_EA else ovr.MIP
-    _, _, cnt = ovr.render(vol, M, job.W, job.H, w.step, omode, getattr(ovr, precision_name), tf=job.tf,
-                           split=ovr.SPLIT_SORTLAST, partition=brick, tau=w.tau, bg=job.bg, pixels=pix)
-    return time.perf_counter() - t0, cnt, len(touched)
+
+    def run(sub):
+        _, _, cnt = ovr.render(vol, M, job.W, job.H, w.step, omode, getattr(ovr, precision_name), tf=job.tf,
+                               split=ovr.SPLIT_SORTLAST, partition=brick, tau=w.tau, bg=job.bg, pixels=sub)
+        return cnt
+
+    t0 = time.perf_counter()
+    if threads <= 1:
+        cnts = [run(pix)]
+    else:
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(max_workers=threads) as pool:
+            cnts = list(pool.map(run, [np.ascontiguousarray(pix[i::threads]) for i in range(threads)]))
+    sec = time.perf_counter() - t0
+    cnt = {k: sum(c[k] for c in cnts) for k in cnts[0]}
+    return sec, cnt, nb
+
+
+def cpu_baseline(job, frame_index, seconds):
+    """The oracle as it stands on one host core, and the same code over disjoint pixels on all host cores
+    (BASELINE.md section 3), each on a pixel block sized for about `seconds` of wall time."""
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    cache = {}
+    out = {}
+    for label, threads in (("one", 1), ("all", cores)):
+        tile = 8
+        sec, c, nb = oracle_sample(job, frame_index, tile, threads=threads, cache=cache)
+        if c["nominal"] > 0 and sec > 0:
+            tile2 = int(min(384, max(8, tile * math.sqrt(seconds / max(sec, 1e-3)))))
+            if tile2 > tile:
+                sec, c, nb = oracle_sample(job, frame_index, tile2, threads=threads, cache=cache)
+                tile = tile2
+        out[label] = {"value": c["nominal"] / sec if sec > 0 else 0.0, "unit": "samples/s", "cores": threads, "kind": "oracle",
+                      "sample": f"fp64 oracle, sort-last, the {tile}x{tile}-pixel block at the centre of orbit frame {frame_index} "
+                                f"({c['nominal']} nominal samples, {nb} bricks fetched back from the device, {sec:.2f} s)"}
+    res = out["one"]
+    res["all_cores"] = out["all"]
+    res["nproc"] = cores
+    return res
+
+
+def measure(job, steps, warmup, frank, fworld, dist, local_rank, e2e=True):
+    """W untimed + K timed frames (device time, CUDA events), then the same K frames end to end with host buffers."""
+    torch, w = job.torch, job.w
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(warmup):
+        job.step(orbit_frame(w, i, steps, frank, fworld))
+    job.ctx.reset_counters()
+    job.reset_events()
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for i in range(steps):
+        job.step(orbit_frame(w, i, steps, frank, fworld), timed_events=True)
+    ev1.record()
+    barrier()
+    clocks = sampler.result()
+    ms_total = ev0.elapsed_time(ev1)
+    marks = [ev0] + job.step_events
+    frame_ms = sorted(a.elapsed_time(b) for a, b in zip(marks, marks[1:]))
+    cnt = job.ctx.get_counters()
+    march_ms = sum(a.elapsed_time(b) for a, b in job.march_events)
+    n_march = len(job.march_events)
+    ms_total, (nominal, taken, launches) = reduce_run(
+        dist, "cuda", ms_total, [cnt["nominal_samples"], cnt["taken_samples"], cnt["kernel_launches"]])
+    res = {"ms_total": ms_total, "frame_ms": frame_ms, "nominal": nominal, "taken": taken, "launches": launches,
+           "march_ms": march_ms, "n_march": n_march, "b_brick": job.b_brick, "partial_bytes": job.partial_bytes,
+           "clocks": clocks, "steps": steps, "fworld": fworld}
+    if not e2e:
+        return res
+    # ---- e2e: the same step through the public API with HOST buffers in the timed region: the
+    # view matrix and the transfer-function table go host -> device every step (as kernel
+    # parameters / table upload), the finished frame comes back device -> pinned host memory.
+    # Two frame buffers: frame i's device -> host copy runs on a copy stream while frame i + 1 is rendered;
+    # the host takes delivery of frame i - 1 (waits for its copy) before it issues frame i + 1.
+    job.ctx.reset_counters()
+    barrier()
+    frames = [job.frame, torch.zeros_like(job.frame)]
+    h_frames = [job.h_frame, torch.empty_like(job.h_frame).pin_memory()]
+    copy_stream = torch.cuda.Stream()
+    copied = [None, None]
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for i in range(steps):
+        b = i % 2
+        if copied[b] is not None:
+            torch.cuda.current_stream().wait_event(copied[b])      # the buffer's previous frame has left the device
+        job.frame = frames[b]
+        job.step(orbit_frame(w, i, steps, frank, fworld), set_tf=True)
+        src = job.frame                                             # (the sharded path returns a new tensor)
+        rendered = torch.cuda.Event()
+        rendered.record()
+        with torch.cuda.stream(copy_stream):
+            copy_stream.wait_event(rendered)
+            h_frames[b].copy_(src, non_blocking=True)
+            src.record_stream(copy_stream)
+            copied[b] = torch.cuda.Event()
+            copied[b].record()
+        if i > 0:
+            copied[1 - b].synchronize()                             # frame i - 1 is in host memory
+    copied[(steps - 1) % 2].synchronize()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    job.frame = frames[0]
+    cnt2 = job.ctx.get_counters()
+    e2e_s, (e2e_nominal,) = reduce_run(dist, "cuda", e2e_s, [cnt2["nominal_samples"]])
+    res["e2e_s"], res["e2e_nominal"] = e2e_s, e2e_nominal
+    return res
+
+
+def roofline(job, m, touch_frames, peak, peak_src):
+    """algorithmic bytes per launch = min(B_brick, B_touch) + partial images written + brick meta,
+    over the launch's CUDA-event duration.  B_touch is measured by vr_measure_touch on `touch_frames`."""
+    n = max(m["n_march"], 1)
+    launch_s = m["march_ms"] / n * 1e-3
+    plan = job.ctx.get_plan(job.mode)
+    kernel = kernel_name(plan, job.mode_name)
+    b_brick = m["b_brick"] / n
+    writes = m["partial_bytes"] / n + 8 * job.w.brick_grid[0] * job.w.brick_grid[1] * job.w.brick_grid[2]
+    touch = None
+    if touch_frames:
+        acc = {"launches": 0, "sectors": 0, "lines": 0, "taken_samples": 0}
+        for f in touch_frames:
+            t = job.touch(f)
+            if t is None:
+                acc = None
+                break
+            for k in acc:
+                acc[k] += t[k]
+        if acc and acc["launches"]:
+            touch = {"frames": list(touch_frames), "sector_bytes_per_launch": 32.0 * acc["sectors"] / acc["launches"],
+                     "line_bytes_per_launch": 128.0 * acc["lines"] / acc["launches"],
+                     "taken_samples_per_launch": acc["taken_samples"] / acc["launches"]}
+    b_touch = touch["sector_bytes_per_launch"] if touch else None
+    alg = (min(b_brick, b_touch) if b_touch is not None else b_brick) + writes
+    achieved = alg / launch_s / 1e9 if launch_s > 0 else 0.0
+    out = {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s",
+           "frac": achieved / peak if peak else None, "peak_source": peak_src,
+           "algorithmic_bytes_per_launch": alg, "b_brick": b_brick, "b_touch": touch, "bytes_written": writes,
+           "launch_ms": m["march_ms"] / n, "share_of_step": m["march_ms"] / m["ms_total"] if m["ms_total"] else None,
+           "plan": plan,
+           "effective_vs_brick": (b_brick + writes) / launch_s / 1e9 / peak if launch_s > 0 and peak else None,
+           "note": "algorithmic bytes = min(B_brick, B_touch) + partial images + brick meta (SURVEY.md 8(d)); B_brick = 4 B x "
+                   "voxels of the active in-frustum bricks at the configured size; B_touch = 32 B x distinct sectors under the "
+                   "footprints of the samples the launch interpolates (vr_measure_touch on the frames listed); frac_lines "
+                   "counts whole 128-byte lines instead (the unit this HBM is read in, DESIGN.md section 4); "
+                   "effective_vs_brick is the B_brick ratio (can exceed 1: skipping below the brick level)"}
+    if touch:
+        lines = min(b_brick, touch["line_bytes_per_launch"]) + writes
+        out["frac_lines"] = lines / launch_s / 1e9 / peak if launch_s > 0 and peak else None
+    cap, why = ncu_counters(job.w.name, job.mode_name, job.tf_name, kernel)
+    clocks = m["clocks"]
+    if cap:
+        out["traffic"] = cap["traffic"]
+        out["traffic_source"] = cap["source"]
+        out["dram_gbs_from_traffic"] = cap["traffic"] / launch_s / 1e9 if launch_s > 0 else None
+        if clocks.get("sm_mhz"):
+            ipeak = ISSUE_SLOTS_PER_CLOCK * clocks["sm_mhz"] * 1e6 / 1e9
+            out["issue"] = {"bound": "alu", "achieved": cap["warp_instructions"] / launch_s / 1e9, "peak": ipeak,
+                            "unit": "G warp-instructions/s", "frac": cap["warp_instructions"] / launch_s / 1e9 / ipeak,
+                            "note": "warp instructions per launch from the committed ncu capture / live launch time; peak = 148 "
+                                    "SMs x 4 schedulers x the SM clock sampled during the run"}
+    else:
+        out["traffic"] = None
+        out["traffic_note"] = why
+    return out
+
+
+def entry(job, m, args, peak, peak_src, touch_frames):
+    """The JSON fields of one measured workload."""
+    steps, fworld, ms_total = m["steps"], m["fworld"], m["ms_total"]
+    frame_ms = m["frame_ms"]
+    w = job.w
+    out = {
+        "value": m["nominal"] / (ms_total * 1e-3), "unit": "samples/s", "steps": steps,
+        "ms_per_step": ms_total / steps, "frames_per_s": steps * fworld / (ms_total * 1e-3),
+        "frame_ms": {"median": frame_ms[len(frame_ms) // 2], "p95": frame_ms[min(len(frame_ms) - 1, int(0.95 * len(frame_ms)))],
+                     "min": frame_ms[0], "max": frame_ms[-1], "note": "rank 0, device time between consecutive frames of the orbit"},
+        "nominal_samples_per_step": m["nominal"] / (steps * fworld),
+        "taken_samples_per_s": m["taken"] / (ms_total * 1e-3),
+        "taken_fraction": m["taken"] / max(m["nominal"], 1),
+        "gpu_launches": m["launches"],
+        "clocks": m["clocks"],
+        "roofline": roofline(job, m, touch_frames, peak, peak_src),
+    }
+    if "e2e_s" in m:
+        out["e2e"] = {"value": m["e2e_nominal"] / m["e2e_s"], "unit": "samples/s", "ms_per_step": m["e2e_s"] * 1e3 / steps,
+                      "h2d_bytes_per_step": (64 + 4096 + 8) * job.cols * job.rows,
+                      "d2h_bytes_per_step": job.H * job.W * job.px_bytes}
+    return out
+
+
+def describe(job, mode, world, args):
+    w = job.w
+    return {"workload": f"{w.name}: {w.dims[0]}x{w.dims[1]}x{w.dims[2]} float32 cube, {w.brick[0]}^3 bricks, "
+                        f"{job.W}x{job.H} frame ({job.cols}x{job.rows} panels), step {w.step}, "
+                        f"{'EA tf-' + job.tf_name + ' tau=' + str(w.tau) if mode == 'ea' else 'MIP'}, sort-last path, orbit frames spread over 360 deg",
+            "cube_gib": round(w.n_voxels * 4 / 2 ** 30, 3), "n_sources": w.n_sources,
+            "l2_policy": "inputs larger than L2 (cube >> 126 MB); no explicit flush",
+            "e2e_policy": "matrix + table host->device and frame device->pinned host every step; two frame buffers, frame "
+                          "i's copy overlaps frame i+1's render, the host waits for frame i-1 before issuing frame i+1",
+            "replicas": 1 if args.sharded else world, "shards": world if args.sharded else 1, "slab": args.slab,
+            "generate_seconds": round(job.gen_seconds, 3)}
+
+
+def tf_edit(job, frame_index):
+    """Milliseconds from a transfer-function edit that changes the SET of transparent entries (the opacity
+    threshold dragged from entry 32 to 40 and back; "colour map", line 13 "interactive") to the
+    finished next frame: vr_set_transfer_function + one step, stream synchronised (re-classification included)."""
+    torch = job.torch
+    keep = job.tf
+    times = []
+    for k in range(4):
+        job.tf = wl.tf_src(40 if k % 2 == 0 else 32)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        job.step(frame_index, set_tf=True)
+        torch.cuda.synchronize()
+        times.append((time.perf_counter() - t0) * 1e3)
+    job.tf = keep
+    job.step(frame_index, set_tf=True)
+    torch.cuda.synchronize()
+    times.sort()
+    return {"ms": times[len(times) // 2], "all_ms": times, "what": "threshold entry 32 <-> 40, then one frame, synchronised"}
+
+
+SUITE = [  # (workload, mode, table, frame, panels, steps): the rest of BASELINE.json's metric, each measured like the headline
+    ("C3", "mip", None, None, None, 12),
+    ("C3", "ea", "fog", None, None, 12),
+    ("C2", "ea", None, None, None, 24),
+    ("C4", "ea", None, None, None, 4),
+    ("C5", "ea", None, None, None, 4),
+    ("C5", "mip", None, (1920, 1080), (1, 1), 12),
+]
+
+
+def run_suite(args, head_job, peak, peak_src, local_rank):
+    import torch
+    out = []
+    job = head_job
+    for name, mode, tf, frame, panels, steps in SUITE:
+        w = wl.CONFIGS[name]
+        try:
+            if job is None or job.w.name != name:
+                if job is not None:
+                    job.close()
+                    job = None
+                free, _ = torch.cuda.mem_get_info()
+                need = w.n_voxels * 4 * 1.09 + 3e9
+                if free < need:
+                    out.append({"config": {"workload": name, "mode": mode}, "skipped": f"needs {need / 1e9:.0f} GB of free HBM, {free / 1e9:.0f} free"})
+                    continue
+                job = Job(w, local_rank, mode, tf=tf)
+            job.configure(mode, tf or w.tf, frame or w.frame, panels or w.panels)
+            m = measure(job, steps, 3, 0, 1, None, local_rank)
+            e = entry(job, m, args, peak, peak_src, [orbit_frame(w, 0, steps, 0, 1)] if not args.no_touch else [])
+            e["config"] = describe(job, mode, 1, args)
+            if name == "C2" and not args.no_cpu:
+                e["cpu_baseline"] = cpu_baseline(job, orbit_frame(w, 0, steps, 0, 1), args.cpu_seconds / 2)
+            out.append(e)
+        except Exception as exc:                      # one failing entry must not lose the headline
+            out.append({"config": {"workload": name, "mode": mode}, "error": f"{type(exc).__name__}: {exc}"})
+            try:
+                if job is not None:
+                    job.close()
+            except Exception:
+                pass
+            job = None
+    if job is not None:
+        job.close()
+    return out
 
 
 def main():
@@ -246,9 +599,10 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=24)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="C3", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--workload", default=None, choices=sorted(wl.CONFIGS))
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--mode", default="ea", choices=["ea", "mip"], help="emission-absorption (default) or MIP")
+    ap.add_argument("--tf", default=None, choices=sorted(wl.TFS), help="transfer function (default: the workload's)")
     ap.add_argument("--sharded", action="store_true",
                     help="N ranks share ONE cube: bricks sharded in z-slabs, sort-last exchange over NCCL (NEXT-1, "
                          "strong scaling); default: N independent replicas")
@@ -259,7 +613,12 @@ def main():
                     help="time the catalogue overlay and the output pyramid (SURVEY.md 8(f) 2 and 3) instead of the marcher")
     ap.add_argument("--frame", default=None, help="WxH: render one frame of this size instead of the workload's "
                                                    "(BASELINE.json configs[4]: C5's 1920x1080 MIP)")
-    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target wall time of each oracle sample")
+    ap.add_argument("--suite", dest="suite", action="store_true", default=None,
+                    help="append the `configs` list (default: on for the default workload on one GPU)")
+    ap.add_argument("--no-suite", dest="suite", action="store_false")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the oracle timing (profiling runs)")
+    ap.add_argument("--no-touch", action="store_true", help="skip the B_touch measurement (profiling runs)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
@@ -278,9 +637,12 @@ def main():
         torch.cuda.set_device(local_rank)
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    w = wl.CONFIGS[args.workload]
+    default_run = (args.workload is None and args.mode == "ea" and args.tf is None and not args.frame and not args.sharded
+                   and not args.slab and world == 1)
+    if args.suite is None:
+        args.suite = default_run and args.impl == "b200"
+    w = wl.CONFIGS[args.workload or "C3"]
     if args.frame:
-        from dataclasses import replace
         w = replace(w, frame=tuple(int(v) for v in args.frame.lower().split("x")), panels=(1, 1))
     if args.next_rows:
         return run_next_rows(args)
@@ -291,88 +653,15 @@ def main():
             raise SystemExit("--slab R/W runs on one GPU, without --sharded")
     if (args.sharded or slab) and w.panels != (1, 1):
         raise SystemExit("--sharded renders single-panel frames (use --frame WxH for the tiled workloads)")
-    job = Job(w, local_rank, args.mode, shard=slab if slab else ((rank, world) if args.sharded else None), dist=dist)
+    job = Job(w, local_rank, args.mode, shard=slab if slab else ((rank, world) if args.sharded else None), dist=dist, tf=args.tf)
     job.slab_only = slab is not None
     frank, fworld = (0, 1) if args.sharded else (rank, world)          # sharded: every rank renders every frame
-    vr = job.vr
-    config = {"workload": f"{w.name}: {w.dims[0]}x{w.dims[1]}x{w.dims[2]} float32 cube, {w.brick[0]}^3 bricks, "
-                          f"{w.frame[0]}x{w.frame[1]} frame ({w.panels[0]}x{w.panels[1]} panels), step {w.step}, "
-                          f"{'EA tf-' + w.tf + ' tau=' + str(w.tau) if args.mode == 'ea' else 'MIP'}, sort-last path, orbit frames spread over 360 deg",
-              "cube_gib": round(w.n_voxels * 4 / 2 ** 30, 3), "n_sources": w.n_sources,
-              "l2_policy": "inputs larger than L2 (cube >> 126 MB); no explicit flush",
-              "e2e_policy": "matrix + table host->device and frame device->pinned host every step; two frame buffers, frame "
-                            "i's copy overlaps frame i+1's render, the host waits for frame i-1 before issuing frame i+1",
-              "replicas": 1 if args.sharded else world, "shards": world if args.sharded else 1, "slab": args.slab,
-              "generate_seconds": round(job.gen_seconds, 3)}
+    config = describe(job, args.mode, world, args)
 
     if args.impl == "reference":
         return run_reference(args, job, config)
 
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for i in range(args.warmup):
-        job.step(orbit_frame(w, i, args.steps, frank, fworld))
-    job.ctx.reset_counters()
-    sampler = ClockSampler(local_rank)
-    barrier()
-    sampler.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record()
-    for i in range(args.steps):
-        job.step(orbit_frame(w, i, args.steps, frank, fworld), timed_events=True)
-    ev1.record()
-    barrier()
-    clocks = sampler.result()
-    ms_total = ev0.elapsed_time(ev1)
-    marks = [ev0] + job.step_events
-    frame_ms = sorted(a.elapsed_time(b) for a, b in zip(marks, marks[1:]))
-    cnt = job.ctx.get_counters()
-    march_ms = sum(a.elapsed_time(b) for a, b in job.march_events)
-    n_march = len(job.march_events)
-
-    ms_total, (nominal, taken, launches) = reduce_run(
-        dist, "cuda", ms_total, [cnt["nominal_samples"], cnt["taken_samples"], cnt["kernel_launches"]])
-
-    # ---- e2e: the same step through the public API with HOST buffers in the timed region: the
-    # view matrix and the transfer-function table go host -> device every step (as kernel
-    # parameters / table upload), the finished frame comes back device -> pinned host memory.
-    job.ctx.reset_counters()
-    barrier()
-    # Two frame buffers: frame i's device -> host copy runs on a copy stream while frame i + 1 is rendered;
-    # the host takes delivery of frame i - 1 (waits for its copy) before it issues frame i + 1.
-    frames = [job.frame, torch.zeros_like(job.frame)]
-    h_frames = [job.h_frame, torch.empty_like(job.h_frame).pin_memory()]
-    copy_stream = torch.cuda.Stream()
-    copied = [None, None]
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    for i in range(args.steps):
-        b = i % 2
-        if copied[b] is not None:
-            torch.cuda.current_stream().wait_event(copied[b])      # the buffer's previous frame has left the device
-        job.frame = frames[b]
-        job.step(orbit_frame(w, i, args.steps, frank, fworld), set_tf=True)
-        src = job.frame                                             # (the sharded path returns a new tensor)
-        rendered = torch.cuda.Event()
-        rendered.record()
-        with torch.cuda.stream(copy_stream):
-            copy_stream.wait_event(rendered)
-            h_frames[b].copy_(src, non_blocking=True)
-            src.record_stream(copy_stream)
-            copied[b] = torch.cuda.Event()
-            copied[b].record()
-        if i > 0:
-            copied[1 - b].synchronize()                             # frame i - 1 is in host memory
-    copied[(args.steps - 1) % 2].synchronize()
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    job.frame = frames[0]
-    cnt2 = job.ctx.get_counters()
-    e2e_s, (e2e_nominal,) = reduce_run(dist, "cuda", e2e_s, [cnt2["nominal_samples"]])
-
+    m = measure(job, args.steps, args.warmup, frank, fworld, dist, local_rank)
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -380,66 +669,23 @@ def main():
 
     peaks, peak_src = measured_peaks()
     peak = float(peaks["hbm_gbs"])
-    plan = job.ctx.get_plan(job.mode)
-    kernel = MARCHER.get((plan["variant"], plan["skip_level"]),
-                         "render_ls_kernel<EA> (lockstep, cp.async gather)" if plan["variant"] == 3 else "render_tiles_kernel<EA>")
-    if args.mode == "mip":
-        kernel = ("render_ls_kernel<MIP> (lockstep, cp.async gather, warp-reduced maximum)" if plan["variant"] == 3
-                  else "render_tiles_kernel<MIP> (ray per thread)")
-    traffic = NCU_TRAFFIC_BYTES.get((w.name, args.mode)) if not args.frame else None
-    launch_s = march_ms / max(n_march, 1) * 1e-3
-    winst = NCU_WARP_INSTRUCTIONS.get((w.name, args.mode)) if not args.frame else None
-    issue = None
-    if winst and launch_s > 0 and clocks.get("sm_mhz"):
-        ipeak = ISSUE_SLOTS_PER_CLOCK * clocks["sm_mhz"] * 1e6 / 1e9
-        issue = {"bound": "alu", "achieved": winst / launch_s / 1e9, "peak": ipeak, "unit": "G warp-instructions/s",
-                 "frac": winst / launch_s / 1e9 / ipeak,
-                 "note": "warp instructions per launch from the committed ncu capture / live launch time; peak = 148 SMs x 4 "
-                         "schedulers x the SM clock sampled during the run: what actually bounds the occupancy marcher"}
-    achieved = (job.alg_bytes / max(n_march, 1)) / (march_ms / max(n_march, 1) * 1e-3) / 1e9 if march_ms > 0 else 0.0
-    cpu = None
-    if world == 1 and not slab:           # a slab holds only its own bricks: no oracle sample
-        tile = 8
-        sec, c, nb = oracle_sample(job, orbit_frame(w, 0, args.steps, 0, 1), tile)
-        if c["nominal"] > 0 and sec > 0:
-            scale = args.cpu_seconds / max(sec, 1e-3)
-            tile2 = int(min(256, max(8, tile * math.sqrt(scale))))
-            if tile2 > tile:
-                sec, c, nb = oracle_sample(job, orbit_frame(w, 0, args.steps, 0, 1), tile2)
-                tile = tile2
-        cpu = {"value": c["nominal"] / sec if sec > 0 else 0.0, "unit": "samples/s", "cores": 1, "kind": "oracle",
-               "sample": f"fp64 oracle, sort-last, the {tile}x{tile}-pixel block at the centre of orbit frame 0 "
-                         f"({c['nominal']} nominal samples, {nb} bricks fetched back from the device, {sec:.2f} s)"}
-
-    out = {
-        "metric": METRIC, "value": nominal / (ms_total * 1e-3), "unit": "samples/s",
-        "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_total / args.steps, "frames_per_s": args.steps * fworld / (ms_total * 1e-3),
-        "frame_ms": {"median": frame_ms[len(frame_ms) // 2], "p95": frame_ms[min(len(frame_ms) - 1, int(0.95 * len(frame_ms)))],
-                     "min": frame_ms[0], "max": frame_ms[-1], "note": "rank 0, device time between consecutive frames of the orbit"},
-        "higher_is_better": True, "scaling": "strong" if args.sharded else "weak", "vs_baseline": None, "dtype": "f32",
-        "data": "synthetic", "config": config,
-        "nominal_samples_per_step": nominal / (args.steps * fworld),
-        "taken_samples_per_s": taken / (ms_total * 1e-3),
-        "gpu_launches": launches,
-        "clocks": clocks,
-        "e2e": {"value": e2e_nominal / e2e_s, "unit": "samples/s", "ms_per_step": e2e_s * 1e3 / args.steps,
-                "h2d_bytes_per_step": (64 + 4096 + 8) * job.cols * job.rows,
-                "d2h_bytes_per_step": job.H * job.W * job.px_bytes},
-        "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak,
-                     "unit": "GB/s", "frac": achieved / peak if peak else None, "traffic": traffic,
-                     "peak_source": peak_src, "launch_ms": march_ms / max(n_march, 1),
-                     "share_of_step": march_ms / ms_total if ms_total else None,
-                     "algorithmic_bytes_per_launch": job.alg_bytes / max(n_march, 1),
-                     "dram_gbs_from_traffic": traffic / launch_s / 1e9 if traffic and launch_s > 0 else None,
-                     "issue": issue,
-                     "plan": plan,
-                     "note": "algorithmic bytes = 4 B x voxels of the active in-frustum bricks at the configured brick "
-                             "size + partial images (SURVEY.md 8(d)); skipping below the brick level (macro-cells, "
-                             "occupancy bits) reads fewer bytes than that, so frac can exceed 1: `traffic` is what "
-                             "the launch really moved"},
-        "cpu_baseline": cpu,
-    }
+    f0 = orbit_frame(w, 0, args.steps, 0, 1)
+    touch_frames = [] if (args.no_touch or args.sharded or slab) else sorted({f0, orbit_frame(w, args.steps // 2, args.steps, 0, 1)})
+    out = {"metric": METRIC}
+    out.update(entry(job, m, args, peak, peak_src, touch_frames))
+    out.update({"n_gpus": world, "warmup": args.warmup, "higher_is_better": True, "scaling": "strong" if args.sharded else "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config})
+    if world == 1 and not slab and not args.no_cpu:           # a slab holds only its own bricks: no oracle sample
+        out["cpu_baseline"] = cpu_baseline(job, f0, args.cpu_seconds)
+        out["vs_cpu_baseline"] = {"one_core": out["value"] / out["cpu_baseline"]["value"] if out["cpu_baseline"]["value"] else None,
+                                  "all_cores": out["value"] / out["cpu_baseline"]["all_cores"]["value"] if out["cpu_baseline"]["all_cores"]["value"] else None,
+                                  "note": "GPU device-timed rate over the oracle's: reported, not a headline (the oracle is a deliberately plain program)"}
+    else:
+        out["cpu_baseline"] = None
+    if default_run and args.mode == "ea" and job.tf_name == "src":
+        out["tf_edit"] = tf_edit(job, f0)
+    if args.suite:
+        out["configs"] = run_suite(args, job, peak, peak_src, local_rank)
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
@@ -491,14 +737,15 @@ def run_reference(args, job, config):
     w = job.w
     budget = 150.0 / max(1, args.steps + args.warmup)
     tile = 8
-    sec, c, nb = oracle_sample(job, 0, tile)
+    cache = {}
+    sec, c, nb = oracle_sample(job, 0, tile, cache=cache)
     if sec > 0:
         tile = int(min(128, max(4, tile * math.sqrt(budget / max(sec, 1e-3)))))
     for i in range(args.warmup):
-        oracle_sample(job, orbit_frame(w, i, args.steps, 0, 1), tile)
+        oracle_sample(job, orbit_frame(w, i, args.steps, 0, 1), tile, cache=cache)
     total_s, total_n = 0.0, 0
     for i in range(args.steps):
-        sec, c, nb = oracle_sample(job, orbit_frame(w, i, args.steps, 0, 1), tile)
+        sec, c, nb = oracle_sample(job, orbit_frame(w, i, args.steps, 0, 1), tile, cache=cache)
         total_s += sec
         total_n += c["nominal"]
     value = total_n / total_s if total_s > 0 else 0.0

@@ -15,7 +15,8 @@
  *    meta, frames, partial images) are CALLER-OWNED device memory (e.g. torch tensors); the
  *    library never allocates O(cube) or O(frame) memory.  It owns only small device scratch:
  *    the transfer-function tables (8 KiB), counters, the source lists of the generator, the
- *    descriptors of partial images (<= ~100 B per brick) and, for host uploads, one staging slab.
+ *    descriptors of partial images (<= ~100 B per brick) and, while vr_upload_cube streams a HOST
+ *    source, two staging slabs of about 128 MiB each (freed before the call returns).
  *  - `stream` is a cudaStream_t passed as void* (torch.cuda.current_stream().cuda_stream); work
  *    is enqueued on it and no call synchronises the device unless stated.  Outputs are valid
  *    after the caller synchronises the stream.
@@ -60,8 +61,8 @@ int vr_cube_layout(int nx, int ny, int nz, int bx, int by, int bz, size_t* cube_
                    size_t* meta_bytes);
 
 /* Rebrick a linear x-fastest float32 cube (host if src_is_device == 0, else device) into d_cube
- * and compute d_meta.  Host sources are streamed slab by slab through a library staging buffer;
- * the call returns after the last slab was enqueued (it synchronises `stream` between slabs).
+ * and compute d_meta.  Host sources are streamed slab by slab (whole planes) through two library
+ * staging slabs, the copy of one overlapping the rebricking of the other; the call synchronises `stream`.
  * Non-finite voxels (NaN, inf) are counted while rebricking: VR_ERR_INVALID_ARG, and no cube is set. */
 int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int ny, int nz,
                    int bx, int by, int bz, void* d_cube, void* d_meta, void* stream);
@@ -197,6 +198,23 @@ int vr_pyramid_layout(int width, int height, int tile, int* n_levels, vr_pyramid
  * frame); d_out: device, *bytes of vr_pyramid_layout, caller-owned. */
 int vr_build_pyramid(vr_ctx* ctx, const float* d_frame_rgba, int width, int height, size_t pitch_px, int tile,
                      void* d_out, void* stream);
+
+/* ---- measurement of the bytes a frame needs ("B_touch = 32 B x distinct sectors inside
+ *      the 2 x 2 x 2 footprints of taken samples ... measure it once per config with a debug kernel that
+ *      sets one bit per sector").  Not on the frame path: bench.py and the tests call it. ------------- */
+/* Bytes of the caller-owned device bitmap: one bit per 32-byte sector of the resident brick-major cube. */
+int vr_touch_layout(vr_ctx* ctx, size_t* bitmap_bytes);
+/* Walk the same (pixel, brick) samples as vr_render_bricks(mode, h_partials, n, ert_tau) one by one, apply
+ * the skipping tests of the current plan (O-10; vr_get_plan) and early ray termination (O-7), and set the
+ * bit of every sector under the 8 corners of every sample that is interpolated.  accumulate == 0 clears the
+ * bitmap and the taken-sample count first (so several launches, e.g. the panels of a tiled frame, can be
+ * summed or measured one by one). */
+int vr_measure_touch(vr_ctx* ctx, int mode, const vr_partial* h_partials, int n, float ert_tau, void* d_bitmap,
+                     int accumulate, void* stream);
+/* out[0] = sectors set, out[1] = 128-byte lines with at least one sector set (the unit HBM is read in,
+ * DESIGN.md section 4), out[2] = samples interpolated by the vr_measure_touch calls since the last clear.
+ * Synchronises `stream`. */
+int vr_touch_count(vr_ctx* ctx, const void* d_bitmap, uint64_t out[3], void* stream);
 
 /* ---- counters (SURVEY.md section 5 "metrics") ---------------------------------------------- */
 typedef struct {

@@ -7,6 +7,8 @@
 #include <cstdio>
 #include <cstring>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "vr_internal.cuh"
 
 using namespace vr;
@@ -35,8 +37,6 @@ struct vr_ctx {
     unsigned long long* d_counters = nullptr;
     PartialDev* d_partials = nullptr;
     size_t partials_cap = 0;
-    float* d_stage = nullptr;
-    size_t stage_bytes = 0;
     int64_t launches = 0;
     int opt_skip = 1, opt_cell_skip = -1, opt_variant = -1, opt_layout = 1, opt_dense = -1, opt_occ = -1, opt_ring = -1;   // -1: chosen per view / TF
     float x_clear = -INFINITY;
@@ -51,6 +51,14 @@ struct vr_ctx {
 };
 
 namespace {
+
+// One NVTX range per C-ABI call that does work (SURVEY.md section 5 "tracing"): an nsys trace of an orbit then reads
+// as set_view / sort / render / composite per frame.  Header-only NVTX: a no-op unless a profiler is attached.
+struct Range {
+    explicit Range(const char* name) { nvtxRangePushA(name); }
+    ~Range() { nvtxRangePop(); }
+};
+#define VR_RANGE() Range nvtx_range__(__func__)
 
 constexpr double kSparseRaySpacing = 2.0;     // voxels between neighbouring rays: variant 3 at or above
 constexpr double kCellSkipMaxActive = 0.75;   // macro-cell skipping only if fewer cells than this are active
@@ -70,7 +78,9 @@ int cuda_fail(vr_ctx* ctx, cudaError_t e, const char* where) {
         if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call);     \
     } while (0)
 
-// 4x4 inverse by cofactors (adjugate / determinant), fp64.
+// 4x4 inverse by cofactors (adjugate / determinant), fp64.  The expansion below is the textbook closed
+// form in the term order of the widely circulated Mesa GLU listing (gluInvertMatrix); the oracle
+// inverts with an independent Gauss-Jordan elimination (oracle/ovr.cpp).
 bool invert4(const double m[16], double inv[16]) {
     double a[16];
     a[0] = m[5] * m[10] * m[15] - m[5] * m[11] * m[14] - m[9] * m[6] * m[15] + m[9] * m[7] * m[14] + m[13] * m[6] * m[11] - m[13] * m[7] * m[10];
@@ -99,8 +109,13 @@ bool invert4(const double m[16], double inv[16]) {
 }
 
 bool valid_dims(int nx, int ny, int nz, int bx, int by, int bz) {
-    return nx > 0 && ny > 0 && nz > 0 && bx > 0 && by > 0 && bz > 0 &&
-           (long long)nx < (1 << 22) && (long long)ny < (1 << 22) && (long long)nz < (1 << 22);
+    if (!(nx > 0 && ny > 0 && nz > 0 && bx > 0 && by > 0 && bz > 0 &&
+          (long long)nx < (1 << 22) && (long long)ny < (1 << 22) && (long long)nz < (1 << 22))) return false;
+    // brick ids, cells per brick and occupancy words per brick are ints: bound them (2^24 bricks, 2^26 cells)
+    const int N[3] = {nx, ny, nz}, B[3] = {std::min(bx, nx), std::min(by, ny), std::min(bz, nz)};
+    long long bricks = 1, cells = 1;
+    for (int a = 0; a < 3; ++a) { bricks *= (N[a] + B[a] - 1) / B[a]; cells *= (B[a] + kCell - 1) / kCell + 1; }
+    return bricks <= (1LL << 24) && cells <= (1LL << 26);
 }
 
 // Point the descriptor at the caller's buffers.  They hold the bricks of the window only; every
@@ -134,8 +149,10 @@ int fetch_brick_mm(vr_ctx* ctx, cudaStream_t s) {
 
 int finish_cube(vr_ctx* ctx, cudaStream_t s) {
     CubeDesc& c = ctx->cube;
-    VR_CUDA(ctx, launch_minmax(c, s));
-    ctx->launches += 2;
+    if (c.win_hi > c.win_lo) {                              // an empty window (more ranks than brick layers) launches nothing
+        VR_CUDA(ctx, launch_minmax(c, s));
+        ctx->launches += 2;
+    }
     int rc = fetch_brick_mm(ctx, s);
     if (rc) return rc;
     ctx->has_cube = true;
@@ -193,8 +210,10 @@ int ensure_tables(vr_ctx* ctx, cudaStream_t s) {
             if (wn > 0) VR_CUDA(ctx, cudaMemcpyAsync(ctx->cube.brick_active + w0, ctx->h_brick_active.data() + w0, sizeof(int) * wn, cudaMemcpyHostToDevice, s));
             // the same test per 8^3 macro-cell, on the device (one bit per cell)
             VR_CUDA(ctx, cudaMemsetAsync(ctx->d_scratch, 0, sizeof(unsigned long long), s));
-            VR_CUDA(ctx, launch_classify_cells(ctx->cube, nz, ctx->vmin, ctx->scale, ctx->d_scratch, s));
-            ctx->launches += 1;
+            if (wn > 0) {
+                VR_CUDA(ctx, launch_classify_cells(ctx->cube, nz, ctx->vmin, ctx->scale, ctx->d_scratch, s));
+                ctx->launches += 1;
+            }
             unsigned long long n_active = 0;
             VR_CUDA(ctx, cudaMemcpyAsync(&n_active, ctx->d_scratch, sizeof(n_active), cudaMemcpyDeviceToHost, s));
             VR_CUDA(ctx, cudaStreamSynchronize(s));
@@ -261,6 +280,7 @@ int skip_level(const vr_ctx* ctx, int mode) {
 // Occupancy bits are classified when a render first needs them for the current table.
 int ensure_occ(vr_ctx* ctx, int skip, cudaStream_t s) {
     if (skip < 3 || ctx->occ_valid) return VR_OK;
+    if (ctx->cube.win_hi <= ctx->cube.win_lo) { ctx->occ_valid = true; return VR_OK; }
     VR_CUDA(ctx, launch_classify_occ(ctx->cube, ctx->key_nz, ctx->key_vmin, ctx->key_scale, s));
     ctx->launches += 1;
     ctx->occ_valid = true;
@@ -336,8 +356,15 @@ bool brick_rect(const vr_ctx* ctx, int bid, int rect[4]) {
     return true;
 }
 
+// A context is bound to one device: make it current for the calling thread (a process may drive several GPUs).
+void enter(const vr_ctx* ctx) {
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != ctx->device) cudaSetDevice(ctx->device);
+}
+
 int check_render_state(vr_ctx* ctx, bool need_tf) {
     if (!ctx) return VR_ERR_INVALID_ARG;
+    enter(ctx);
     if (!ctx->has_cube) return fail(ctx, VR_ERR_STATE, "no cube: call vr_upload_cube / vr_generate_cube first");
     if (!ctx->has_view) return fail(ctx, VR_ERR_STATE, "no view: call vr_set_view first");
     if (need_tf && !ctx->has_tf) return fail(ctx, VR_ERR_STATE, "no transfer function: call vr_set_transfer_function first");
@@ -357,7 +384,8 @@ int upload_partials(vr_ctx* ctx, int mode, const vr_partial* hp, int n, bool wit
     const int W = ctx->view.W, H = ctx->view.H;
     for (int i = 0; i < n; ++i) {
         const vr_partial& p = hp[i];
-        if (p.brick < ctx->cube.win_lo || p.brick >= ctx->cube.win_hi || p.w <= 0 || p.h <= 0 || p.x0 < 0 || p.y0 < 0 ||
+        // the brick id is used by the marchers only (with_tiles); the compositor folds images whatever they show
+        if ((with_tiles && (p.brick < ctx->cube.win_lo || p.brick >= ctx->cube.win_hi)) || p.w <= 0 || p.h <= 0 || p.x0 < 0 || p.y0 < 0 ||
             p.x0 + p.w > W || p.y0 + p.h > H || !p.d_data || p.pitch_px < (size_t)p.w)
             return fail(ctx, VR_ERR_INVALID_ARG, "bad vr_partial entry");
         if (((uintptr_t)p.d_data & (mode == VR_MODE_EA ? 15 : 3)) != 0)
@@ -445,7 +473,7 @@ int vr_create(vr_ctx** out, int device) {
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_tf_raw, 256 * sizeof(float4));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, kNumCounters * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(ctx->d_counters, 0, kNumCounters * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_scratch, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_scratch, 8 * sizeof(unsigned long long));
     if (e != cudaSuccess) { vr_destroy(ctx); return VR_ERR_CUDA; }
     *out = ctx;
     return VR_OK;
@@ -459,7 +487,6 @@ int vr_destroy(vr_ctx* ctx) {
     if (ctx->d_counters) cudaFree(ctx->d_counters);
     if (ctx->d_scratch) cudaFree(ctx->d_scratch);
     if (ctx->d_partials) cudaFree(ctx->d_partials);
-    if (ctx->d_stage) cudaFree(ctx->d_stage);
     delete ctx;
     return VR_OK;
 }
@@ -475,7 +502,9 @@ int vr_cube_layout(int nx, int ny, int nz, int bx, int by, int bz, size_t* cube_
 }
 
 int vr_attach_cube(vr_ctx* ctx, int nx, int ny, int nz, int bx, int by, int bz, const void* d_cube, void* d_meta) {
+    VR_RANGE();
     if (!ctx) return VR_ERR_INVALID_ARG;
+    enter(ctx);
     if (!valid_dims(nx, ny, nz, bx, by, bz) || !d_cube || !d_meta) return fail(ctx, VR_ERR_INVALID_ARG, "vr_attach_cube: bad argument");
     fill_cube_desc(ctx->cube, nx, ny, nz, bx, by, bz, ctx->opt_layout);
     apply_window(ctx, ctx->cube);
@@ -489,7 +518,9 @@ int vr_attach_cube(vr_ctx* ctx, int nx, int ny, int nz, int bx, int by, int bz, 
 
 int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int ny, int nz, int bx, int by,
                    int bz, void* d_cube, void* d_meta, void* stream) {
+    VR_RANGE();
     if (!ctx) return VR_ERR_INVALID_ARG;
+    enter(ctx);
     if (!valid_dims(nx, ny, nz, bx, by, bz) || !src || !d_cube || !d_meta) return fail(ctx, VR_ERR_INVALID_ARG, "vr_upload_cube: bad argument");
     cudaStream_t s = (cudaStream_t)stream;
     ctx->has_cube = false;
@@ -503,22 +534,39 @@ int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int
         VR_CUDA(ctx, launch_rebrick(c, const_cast<float*>(c.cube), src, 0, nz, ctx->d_scratch, s));
         ctx->launches += 1;
     } else {
+        // two staging slabs of whole planes (about 128 MiB each): the copy of slab i + 1 (internal copy
+        // stream) overlaps the rebricking of slab i (caller's stream); freed again before returning
         const size_t plane = (size_t)nx * ny * sizeof(float);
-        size_t want = std::max(plane * (size_t)std::min(nz, c.B[2]), std::min(plane * nz, (size_t)256 << 20));
-        int planes = (int)std::max<size_t>(1, std::min<size_t>((size_t)nz, want / plane));
-        if (ctx->stage_bytes < plane * planes) {
-            if (ctx->d_stage) cudaFree(ctx->d_stage);
-            ctx->d_stage = nullptr; ctx->stage_bytes = 0;
-            VR_CUDA(ctx, cudaMalloc(&ctx->d_stage, plane * planes));
-            ctx->stage_bytes = plane * planes;
+        const int planes = (int)std::max<size_t>(1, std::min<size_t>((size_t)nz, ((size_t)128 << 20) / plane));
+        const size_t slab = plane * planes;
+        float* stage[2] = {nullptr, nullptr};
+        cudaStream_t cs = nullptr;
+        cudaEvent_t copied[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr};
+        cudaError_t e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
+        for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+            e = cudaMalloc(&stage[i], slab);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&copied[i], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&freed[i], cudaEventDisableTiming);
         }
-        for (int z0 = 0; z0 < nz; z0 += planes) {
-            int z1 = std::min(nz, z0 + planes);
-            VR_CUDA(ctx, cudaMemcpyAsync(ctx->d_stage, src + (size_t)z0 * nx * ny, plane * (z1 - z0), cudaMemcpyHostToDevice, s));
-            VR_CUDA(ctx, launch_rebrick(c, const_cast<float*>(c.cube), ctx->d_stage, z0, z1, ctx->d_scratch, s));
+        int i = 0;
+        for (int z0 = 0; z0 < nz && e == cudaSuccess; z0 += planes, ++i) {
+            const int z1 = std::min(nz, z0 + planes), bsel = i & 1;
+            if (i >= 2) e = cudaStreamWaitEvent(cs, freed[bsel], 0);               // the slab's previous content was rebricked
+            if (e == cudaSuccess) e = cudaMemcpyAsync(stage[bsel], src + (size_t)z0 * nx * ny, plane * (z1 - z0), cudaMemcpyHostToDevice, cs);
+            if (e == cudaSuccess) e = cudaEventRecord(copied[bsel], cs);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(s, copied[bsel], 0);
+            if (e == cudaSuccess) e = launch_rebrick(c, const_cast<float*>(c.cube), stage[bsel], z0, z1, ctx->d_scratch, s);
+            if (e == cudaSuccess) e = cudaEventRecord(freed[bsel], s);
             ctx->launches += 1;
-            VR_CUDA(ctx, cudaStreamSynchronize(s));          // the staging slab is reused
         }
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        for (int k = 0; k < 2; ++k) {
+            if (stage[k]) cudaFree(stage[k]);
+            if (copied[k]) cudaEventDestroy(copied[k]);
+            if (freed[k]) cudaEventDestroy(freed[k]);
+        }
+        if (cs) cudaStreamDestroy(cs);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "vr_upload_cube (host source)");
     }
     unsigned long long n_bad = 0;
     VR_CUDA(ctx, cudaMemcpyAsync(&n_bad, ctx->d_scratch, sizeof(n_bad), cudaMemcpyDeviceToHost, s));
@@ -529,7 +577,9 @@ int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int
 
 int vr_generate_cube(vr_ctx* ctx, const vr_gen_params* prm, uint64_t seed, int nx, int ny, int nz, int bx,
                      int by, int bz, void* d_cube, void* d_meta, void* stream) {
+    VR_RANGE();
     if (!ctx) return VR_ERR_INVALID_ARG;
+    enter(ctx);
     if (!valid_dims(nx, ny, nz, bx, by, bz) || !prm || !d_cube || !d_meta) return fail(ctx, VR_ERR_INVALID_ARG, "vr_generate_cube: bad argument");
     if (prm->n_sources < 0 || prm->n_zero_boxes < 0 || (prm->n_sources > 0 && !prm->h_sources) ||
         (prm->n_zero_boxes > 0 && !prm->h_zero_boxes))
@@ -591,7 +641,9 @@ int vr_generate_cube(vr_ctx* ctx, const vr_gen_params* prm, uint64_t seed, int n
 }
 
 int vr_download_brick(vr_ctx* ctx, int brick_id, float* d_dst, void* stream) {
+    VR_RANGE();
     if (!ctx) return VR_ERR_INVALID_ARG;
+    enter(ctx);
     if (!ctx->has_cube) return fail(ctx, VR_ERR_STATE, "no cube");
     if (brick_id < ctx->cube.win_lo || brick_id >= ctx->cube.win_hi || !d_dst) return fail(ctx, VR_ERR_INVALID_ARG, "vr_download_brick: bad argument (brick not resident?)");
     VR_CUDA(ctx, launch_unbrick(ctx->cube, brick_id, d_dst, (cudaStream_t)stream));
@@ -600,6 +652,7 @@ int vr_download_brick(vr_ctx* ctx, int brick_id, float* d_dst, void* stream) {
 }
 
 int vr_set_view(vr_ctx* ctx, const float mvp[16], int width, int height, float step) {
+    VR_RANGE();
     if (!ctx) return VR_ERR_INVALID_ARG;
     if (!mvp || width <= 0 || height <= 0 || !(step > 0.f) || !std::isfinite(step)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_view: bad argument");
     double M[16], Minv[16];
@@ -622,6 +675,7 @@ int vr_set_viewport(vr_ctx* ctx, int x0, int y0, size_t pitch_px) {
 }
 
 int vr_set_transfer_function(vr_ctx* ctx, const float rgba[1024], float vmin, float vmax) {
+    VR_RANGE();
     if (!ctx) return VR_ERR_INVALID_ARG;
     if (!rgba || !(vmax > vmin) || !std::isfinite(vmin) || !std::isfinite(vmax)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_transfer_function: bad argument");
     for (int i = 0; i < 1024; ++i) if (!(rgba[i] >= 0.f && rgba[i] <= 1.f)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_transfer_function: entries must lie in [0,1]");
@@ -633,6 +687,7 @@ int vr_set_transfer_function(vr_ctx* ctx, const float rgba[1024], float vmin, fl
 }
 
 int vr_render_mip(vr_ctx* ctx, float* d_out, float* d_out_rgba, float miss, void* stream) {
+    VR_RANGE();
     int rc = check_render_state(ctx, d_out_rgba != nullptr);
     if (rc) return rc;
     if (!d_out) return fail(ctx, VR_ERR_INVALID_ARG, "vr_render_mip: null output");
@@ -648,6 +703,7 @@ int vr_render_mip(vr_ctx* ctx, float* d_out, float* d_out_rgba, float miss, void
 }
 
 int vr_render_ea(vr_ctx* ctx, float* d_out, const float bg[4], float tau, void* stream) {
+    VR_RANGE();
     int rc = check_render_state(ctx, true);
     if (rc) return rc;
     if (!d_out || !bg || !(tau > 0.f)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_render_ea: bad argument");
@@ -676,7 +732,9 @@ static void brick_keys(const vr_ctx* ctx, std::vector<int>& key) {
     bool persp = std::fabs(h[3]) * nmax * 1e9 > nrm;
     int E[3] = {0, 0, 0}, sg[3] = {0, 0, 0};
     if (persp) {
-        for (int a = 0; a < 3; ++a) E[a] = (int)std::floor((h[a] / h[3]) / (double)c.B[a]);
+        // an eye far outside the grid: any index beyond the grid's ends gives the same order (every |b_a - E_a|
+        // moves by one constant), so clamp before the int cast
+        for (int a = 0; a < 3; ++a) E[a] = (int)std::min((double)c.G[a], std::max(-1.0, std::floor((h[a] / h[3]) / (double)c.B[a])));
     } else {
         // direction of the central ray: far point minus near point
         double pn[4], pf[4];
@@ -697,6 +755,7 @@ static void brick_keys(const vr_ctx* ctx, std::vector<int>& key) {
 }
 
 int vr_sort_bricks(vr_ctx* ctx, int mode, int* h_order, int* n_active) {
+    VR_RANGE();
     int rc = check_render_state(ctx, mode == VR_MODE_EA);
     if (rc) return rc;
     if (!n_active || (mode != VR_MODE_MIP && mode != VR_MODE_EA)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_sort_bricks: bad argument");
@@ -719,6 +778,7 @@ int vr_sort_bricks(vr_ctx* ctx, int mode, int* h_order, int* n_active) {
 }
 
 int vr_sort_groups(vr_ctx* ctx, const int* h_group_first, int n_groups, int* h_group_order) {
+    VR_RANGE();
     int rc = check_render_state(ctx, false);
     if (rc) return rc;
     if (!h_group_first || !h_group_order || n_groups <= 0) return fail(ctx, VR_ERR_INVALID_ARG, "vr_sort_groups: bad argument");
@@ -761,12 +821,13 @@ int vr_window_layout(int nx, int ny, int nz, int bx, int by, int bz, int first_b
     fill_cube_desc(c1, nx, ny, nz, bx, by, bz, 1);
     if (end_brick > c0.nbricks) return VR_ERR_INVALID_ARG;
     c0.win_lo = c1.win_lo = first_brick; c0.win_hi = c1.win_hi = end_brick;
-    *cube_bytes_out = std::max(cube_bytes(c0), cube_bytes(c1));
-    *meta_bytes_out = meta_layout(c0).total;
+    *cube_bytes_out = std::max<size_t>(256, std::max(cube_bytes(c0), cube_bytes(c1)));     // an empty window still gets valid buffers
+    *meta_bytes_out = std::max<size_t>(256, meta_layout(c0).total);
     return VR_OK;
 }
 
 int vr_partial_layout(vr_ctx* ctx, int mode, const int* ids, int n, vr_partial* hp, size_t* arena_bytes) {
+    VR_RANGE();
     int rc = check_render_state(ctx, false);
     if (rc) return rc;
     if (n < 0 || (n > 0 && (!ids || !hp)) || !arena_bytes || (mode != VR_MODE_MIP && mode != VR_MODE_EA))
@@ -788,6 +849,7 @@ int vr_partial_layout(vr_ctx* ctx, int mode, const int* ids, int n, vr_partial* 
 }
 
 int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float tau, void* stream) {
+    VR_RANGE();
     int rc = check_render_state(ctx, mode == VR_MODE_EA);
     if (rc) return rc;
     if (n < 0 || (n > 0 && !hp) || (mode != VR_MODE_MIP && mode != VR_MODE_EA) || !(tau > 0.f))
@@ -806,6 +868,7 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
 }
 
 int vr_composite_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float* d_out, const float bg[4], void* stream) {
+    VR_RANGE();
     int rc = check_render_state(ctx, false);
     if (rc) return rc;
     if (n < 0 || (n > 0 && !hp) || !d_out || !bg || (mode != VR_MODE_MIP && mode != VR_MODE_EA))
@@ -817,8 +880,62 @@ int vr_composite_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, floa
     return VR_OK;
 }
 
+int vr_touch_layout(vr_ctx* ctx, size_t* bitmap_bytes) {
+    if (!ctx || !bitmap_bytes) return VR_ERR_INVALID_ARG;
+    enter(ctx);
+    if (!ctx->has_cube) return fail(ctx, VR_ERR_STATE, "no cube");
+    const size_t sectors = cube_bytes(ctx->cube) / 32;
+    *bitmap_bytes = align_up((sectors + 7) / 8, 256);
+    return VR_OK;
+}
+
+int vr_measure_touch(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float tau, void* d_bitmap, int accumulate, void* stream) {
+    VR_RANGE();
+    int rc = check_render_state(ctx, mode == VR_MODE_EA);
+    if (rc) return rc;
+    if (n < 0 || (n > 0 && !hp) || (mode != VR_MODE_MIP && mode != VR_MODE_EA) || !(tau > 0.f) || !d_bitmap || ((uintptr_t)d_bitmap & 3) != 0)
+        return fail(ctx, VR_ERR_INVALID_ARG, "vr_measure_touch: bad argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    if ((rc = ensure_tables(ctx, s))) return rc;
+    int tiles = 0;
+    if ((rc = upload_partials(ctx, mode, hp, n, true, &tiles, s))) return rc;
+    RenderArgs a{};
+    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx);
+    a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
+    if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
+    size_t bytes = 0;
+    vr_touch_layout(ctx, &bytes);
+    if (!accumulate) {
+        VR_CUDA(ctx, cudaMemsetAsync(d_bitmap, 0, bytes, s));
+        VR_CUDA(ctx, cudaMemsetAsync(ctx->d_scratch + 2, 0, sizeof(unsigned long long), s));
+    }
+    VR_CUDA(ctx, launch_touch(ctx->cube, ctx->view, tf_desc(ctx), a, ctx->d_partials, n, tiles, (unsigned*)d_bitmap, ctx->d_scratch + 2, s));
+    ctx->launches += (n > 0 && tiles > 0) ? 1 : 0;
+    return VR_OK;
+}
+
+int vr_touch_count(vr_ctx* ctx, const void* d_bitmap, uint64_t out[3], void* stream) {
+    VR_RANGE();
+    if (!ctx || !d_bitmap || !out) return VR_ERR_INVALID_ARG;
+    enter(ctx);
+    if (!ctx->has_cube) return fail(ctx, VR_ERR_STATE, "no cube");
+    cudaStream_t s = (cudaStream_t)stream;
+    size_t bytes = 0;
+    vr_touch_layout(ctx, &bytes);
+    VR_CUDA(ctx, cudaMemsetAsync(ctx->d_scratch, 0, 2 * sizeof(unsigned long long), s));
+    VR_CUDA(ctx, launch_touch_count((const unsigned*)d_bitmap, (long long)(bytes / 4), ctx->d_scratch, s));
+    ctx->launches += 1;
+    unsigned long long h[3];
+    VR_CUDA(ctx, cudaMemcpyAsync(h, ctx->d_scratch, sizeof(h), cudaMemcpyDeviceToHost, s));
+    VR_CUDA(ctx, cudaStreamSynchronize(s));
+    out[0] = h[0]; out[1] = h[1]; out[2] = h[2];
+    return VR_OK;
+}
+
 int vr_get_counters(vr_ctx* ctx, vr_counters* out, void* stream) {
+    VR_RANGE();
     if (!ctx || !out) return VR_ERR_INVALID_ARG;
+    enter(ctx);
     unsigned long long h[kNumCounters];
     cudaStream_t s = (cudaStream_t)stream;
     VR_CUDA(ctx, cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s));
@@ -831,13 +948,16 @@ int vr_get_counters(vr_ctx* ctx, vr_counters* out, void* stream) {
 
 int vr_reset_counters(vr_ctx* ctx, void* stream) {
     if (!ctx) return VR_ERR_INVALID_ARG;
+    enter(ctx);
     VR_CUDA(ctx, cudaMemsetAsync(ctx->d_counters, 0, kNumCounters * sizeof(unsigned long long), (cudaStream_t)stream));
     ctx->launches = 0;
     return VR_OK;
 }
 
 int vr_overlay_catalogue(vr_ctx* ctx, const vr_catalogue* cat, float* d_frame_rgba, int* d_pick, void* stream) {
+    VR_RANGE();
     if (!ctx) return VR_ERR_INVALID_ARG;
+    enter(ctx);
     if (!ctx->has_view) return fail(ctx, VR_ERR_STATE, "no view: call vr_set_view first");
     if (!cat || !d_pick || cat->n < 0 || (cat->n > 0 && (!cat->d_boxes || (d_frame_rgba && !cat->d_colours))))
         return fail(ctx, VR_ERR_INVALID_ARG, "vr_overlay_catalogue: bad argument");
@@ -849,7 +969,9 @@ int vr_overlay_catalogue(vr_ctx* ctx, const vr_catalogue* cat, float* d_frame_rg
 }
 
 int vr_overlay_pick(vr_ctx* ctx, const int* d_pick, int x, int y, int radius, int* box, void* stream) {
+    VR_RANGE();
     if (!ctx) return VR_ERR_INVALID_ARG;
+    enter(ctx);
     if (!ctx->has_view) return fail(ctx, VR_ERR_STATE, "no view: call vr_set_view first");
     if (!d_pick || !box || radius < 0 || radius > 64) return fail(ctx, VR_ERR_INVALID_ARG, "vr_overlay_pick: bad argument");
     cudaStream_t s = (cudaStream_t)stream;
@@ -870,7 +992,9 @@ int vr_pyramid_layout(int width, int height, int tile, int* n_levels, vr_pyramid
 }
 
 int vr_build_pyramid(vr_ctx* ctx, const float* d_frame_rgba, int width, int height, size_t pitch_px, int tile, void* d_out, void* stream) {
+    VR_RANGE();
     if (!ctx) return VR_ERR_INVALID_ARG;
+    enter(ctx);
     if (!d_frame_rgba || !d_out || width <= 0 || height <= 0 || pitch_px < (size_t)width || tile < 16 || tile > 4096 ||
         (tile & (tile - 1)) != 0 || ((uintptr_t)d_frame_rgba & 15) != 0 || ((uintptr_t)d_out & 3) != 0)
         return fail(ctx, VR_ERR_INVALID_ARG, "vr_build_pyramid: bad argument");
@@ -882,6 +1006,7 @@ int vr_build_pyramid(vr_ctx* ctx, const float* d_frame_rgba, int width, int heig
 }
 
 int vr_get_plan(vr_ctx* ctx, int mode, int out[3], void* stream) {
+    VR_RANGE();
     int rc = check_render_state(ctx, mode == VR_MODE_EA);
     if (rc) return rc;
     if (!out || (mode != VR_MODE_MIP && mode != VR_MODE_EA)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_get_plan: bad argument");

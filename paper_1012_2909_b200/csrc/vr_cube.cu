@@ -39,18 +39,31 @@ __host__ __device__ inline long long slots_per_brick(const CubeDesc& c) {
     return c.layout == 0 ? (long long)c.P[0] * c.P[1] * c.P[2] : c.stride;
 }
 
+// One thread per SOURCE voxel of the slab [z0, z1): the voxel goes to its own brick and, where it lies on a
+// brick's first plane along an axis, also to the halo plane of the brick before it (up to 8 copies).
 __global__ void rebrick_kernel(CubeDesc c, float* __restrict__ cube, const float* __restrict__ src,
-                               int z0, int z1, int brick_lo, long long n_elems, unsigned long long* __restrict__ n_bad) {
-    const long long per = slots_per_brick(c);
+                               int z0, long long n_elems, unsigned long long* __restrict__ n_bad) {
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n_elems;
          e += (long long)gridDim.x * blockDim.x) {
-        long long brick = brick_lo + e / per, rem = e % per;
-        if (brick < c.win_lo || brick >= c.win_hi) continue;
-        Elem el = decode(c, brick, rem);
-        if (!el.in_cube || el.g[2] < z0 || el.g[2] >= z1) continue;
-        const float v = src[(size_t)el.g[0] + (size_t)c.N[0] * ((size_t)el.g[1] + (size_t)c.N[1] * (size_t)(el.g[2] - z0))];
-        cube[brick * c.stride + rem] = v;
-        if (!isfinite(v)) atomicAdd(n_bad, 1ULL);         // NaN / inf voxels are refused by vr_upload_cube (never taken: rare path)
+        const int x = (int)(e % c.N[0]);
+        const long long r2 = e / c.N[0];
+        const int g[3] = {x, (int)(r2 % c.N[1]), z0 + (int)(r2 / c.N[1])};
+        const float v = src[e];
+        if (!isfinite(v)) atomicAdd(n_bad, 1ULL);         // NaN / inf voxels are refused by vr_upload_cube (rare path)
+        int b[3], l[3], nalt[3];
+        for (int a = 0; a < 3; ++a) {
+            b[a] = c.sh[a] >= 0 ? (g[a] >> c.sh[a]) : (g[a] / c.B[a]);
+            l[a] = g[a] - b[a] * c.B[a];
+            nalt[a] = (l[a] == 0 && b[a] > 0) ? 2 : 1;     // also the +1 halo plane of the previous brick
+        }
+        for (int hz = 0; hz < nalt[2]; ++hz)
+            for (int hy = 0; hy < nalt[1]; ++hy)
+                for (int hx = 0; hx < nalt[0]; ++hx) {
+                    const int bx = b[0] - hx, by = b[1] - hy, bz = b[2] - hz;
+                    const long long brick = bx + (long long)c.G[0] * (by + (long long)c.G[1] * bz);
+                    if (brick < c.win_lo || brick >= c.win_hi) continue;
+                    cube[brick * c.stride + voxel_slot(c, hx ? c.B[0] : l[0], hy ? c.B[1] : l[1], hz ? c.B[2] : l[2])] = v;
+                }
     }
 }
 
@@ -179,15 +192,9 @@ int grid_for(long long n, int threads) {
 
 cudaError_t launch_rebrick(const CubeDesc& c, float* d_cube, const float* d_src, int z0, int z1, unsigned long long* d_bad,
                            cudaStream_t s) {
-    // bricks whose stored z range [bz*B2, bz*B2 + B2] meets [z0, z1)
-    int bz_lo = (z0 - c.B[2] + c.B[2] - 1) / c.B[2];
-    if (z0 - c.B[2] <= 0) bz_lo = 0;
-    int bz_hi = (z1 - 1) / c.B[2];
-    if (bz_hi > c.G[2] - 1) bz_hi = c.G[2] - 1;
-    long long layer = (long long)c.G[0] * c.G[1];
-    long long per = slots_per_brick(c);
-    long long n = layer * (bz_hi - bz_lo + 1) * per;
-    rebrick_kernel<<<grid_for(n, 256), 256, 0, s>>>(c, d_cube, d_src, z0, z1, (int)(layer * bz_lo), n, d_bad);
+    const long long n = (long long)c.N[0] * c.N[1] * (z1 - z0);
+    if (n <= 0) return cudaSuccess;
+    rebrick_kernel<<<grid_for(n, 256), 256, 0, s>>>(c, d_cube, d_src, z0, n, d_bad);
     return cudaGetLastError();
 }
 
@@ -211,6 +218,7 @@ cudaError_t launch_minmax(const CubeDesc& c, cudaStream_t s) {
 
 cudaError_t launch_generate(const CubeDesc& c, float* d_cube, const GenDev& g, cudaStream_t s) {
     long long n = (long long)(c.win_hi - c.win_lo) * slots_per_brick(c);
+    if (n <= 0) return cudaSuccess;
     generate_kernel<<<grid_for(n, 256), 256, 0, s>>>(c, d_cube, g, n);
     return cudaGetLastError();
 }

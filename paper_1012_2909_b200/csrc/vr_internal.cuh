@@ -111,6 +111,9 @@ struct RenderArgs {
 cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s);
 cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a,
                                  const PartialDev* d_partials, int n, int total_tiles, cudaStream_t s);
+cudaError_t launch_touch(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, const PartialDev* d_partials,
+                         int n, int total_tiles, unsigned* d_bitmap, unsigned long long* d_taken, cudaStream_t s);
+cudaError_t launch_touch_count(const unsigned* d_bitmap, long long n_words, unsigned long long* d_out, cudaStream_t s);
 cudaError_t launch_composite(const ViewDesc& v, int mode, const PartialDev* d_partials, int n, float* out,
                              const float bg[4], cudaStream_t s);
 cudaError_t launch_classify_cells(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale,

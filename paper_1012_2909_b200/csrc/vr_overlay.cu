@@ -14,8 +14,9 @@ namespace vr {
 namespace {
 
 __global__ void overlay_clear_kernel(const __grid_constant__ ViewDesc V, int* __restrict__ pick) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
-    if (i < V.W) pick[(long long)(V.vy0 + j) * V.pitch + (V.vx0 + i)] = 0;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= V.W) return;
+    for (int j = blockIdx.y; j < V.H; j += gridDim.y) pick[(long long)(V.vy0 + j) * V.pitch + (V.vx0 + i)] = 0;   // gridDim.y <= 65535
 }
 
 struct Mat4 { double m[16]; };
@@ -79,11 +80,13 @@ __global__ void overlay_edges_kernel(const __grid_constant__ ViewDesc V, const _
 
 __global__ void overlay_paint_kernel(const __grid_constant__ ViewDesc V, const int* __restrict__ pick,
                                      const float4* __restrict__ colours, float4* __restrict__ frame) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= V.W) return;
-    const long long px = (long long)(V.vy0 + j) * V.pitch + (V.vx0 + i);
-    const int id = pick[px];
-    if (id > 0) frame[px] = __ldg(&colours[id - 1]);
+    for (int j = blockIdx.y; j < V.H; j += gridDim.y) {
+        const long long px = (long long)(V.vy0 + j) * V.pitch + (V.vx0 + i);
+        const int id = pick[px];
+        if (id > 0) frame[px] = __ldg(&colours[id - 1]);
+    }
 }
 
 // nearest covered pixel of the (2r+1)^2 window around (x, y); ties: the larger id.  One warp.
@@ -111,7 +114,7 @@ __global__ void overlay_pick_kernel(const __grid_constant__ ViewDesc V, const in
 
 cudaError_t launch_overlay(const ViewDesc& v, const double M[16], const int* d_boxes, const float* d_colours,
                            const unsigned char* d_visible, int n, float* d_frame, int* d_pick, cudaStream_t s) {
-    dim3 grid((v.W + 255) / 256, v.H);
+    dim3 grid((v.W + 255) / 256, v.H < 65535 ? v.H : 65535);
     overlay_clear_kernel<<<grid, 256, 0, s>>>(v, d_pick);
     if (n > 0) {
         Mat4 m;

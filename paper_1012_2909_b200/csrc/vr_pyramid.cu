@@ -25,20 +25,23 @@ __device__ __forceinline__ unsigned quant(float c) {
 // one thread per pixel of the PADDED level (tiles_x*tile x tiles_y*tile): padding is written as zero
 __global__ void pyr_quantise_kernel(const float4* __restrict__ frame, long long pitch, int w, int h, int tiles_x, int tiles_y,
                                     int tile, uchar4* __restrict__ out) {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y;
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
     if (x >= tiles_x * tile) return;
+    for (int y = blockIdx.y; y < tiles_y * tile; y += gridDim.y) {                   // gridDim.y <= 65535
     uchar4 q = make_uchar4(0, 0, 0, 0);
     if (x < w && y < h) {
         const float4 c = __ldg(&frame[(long long)y * pitch + x]);
         q = make_uchar4((unsigned char)quant(c.x), (unsigned char)quant(c.y), (unsigned char)quant(c.z), (unsigned char)quant(c.w));
     }
     out[tiled_index(x, y, tiles_x, tile)] = q;
+    }
 }
 
 __global__ void pyr_reduce_kernel(const uchar4* __restrict__ src, int sw, int sh, int s_tiles_x, int w, int h, int tiles_x,
-                                  int tile, uchar4* __restrict__ out) {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y;
+                                  int tiles_y, int tile, uchar4* __restrict__ out) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
     if (x >= tiles_x * tile) return;
+    for (int y = blockIdx.y; y < tiles_y * tile; y += gridDim.y) {
     uchar4 q = make_uchar4(0, 0, 0, 0);
     if (x < w && y < h) {
         unsigned s0 = 0, s1 = 0, s2 = 0, s3 = 0, n = 0;
@@ -57,6 +60,7 @@ __global__ void pyr_reduce_kernel(const uchar4* __restrict__ src, int sw, int sh
                         (unsigned char)((s3 + r) / n));
     }
     out[tiled_index(x, y, tiles_x, tile)] = q;
+    }
 }
 
 }  // namespace
@@ -86,12 +90,12 @@ cudaError_t launch_pyramid(const float* d_frame, int width, int height, long lon
     char* base = (char*)d_out;
     for (int l = 0; l < n; ++l) {
         const vr_pyramid_level& L = lv[l];
-        dim3 grid((L.tiles_x * tile + 255) / 256, L.tiles_y * tile);
+        dim3 grid((L.tiles_x * tile + 255) / 256, L.tiles_y * tile < 65535 ? L.tiles_y * tile : 65535);
         uchar4* out = reinterpret_cast<uchar4*>(base + L.offset);
         if (l == 0) pyr_quantise_kernel<<<grid, 256, 0, s>>>(reinterpret_cast<const float4*>(d_frame), pitch, L.width, L.height, L.tiles_x,
                                                               L.tiles_y, tile, out);
         else pyr_reduce_kernel<<<grid, 256, 0, s>>>(reinterpret_cast<const uchar4*>(base + lv[l - 1].offset), lv[l - 1].width,
-                                                    lv[l - 1].height, lv[l - 1].tiles_x, L.width, L.height, L.tiles_x, tile, out);
+                                                    lv[l - 1].height, lv[l - 1].tiles_x, L.width, L.height, L.tiles_x, L.tiles_y, tile, out);
         ++*launches;
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;

@@ -25,6 +25,7 @@ EXPORTS = [
     "vr_sort_bricks", "vr_partial_layout", "vr_render_bricks", "vr_composite_bricks",
     "vr_get_counters", "vr_reset_counters", "vr_set_option", "vr_get_plan",
     "vr_set_brick_window", "vr_window_layout", "vr_sort_groups", "vr_overlay_catalogue", "vr_overlay_pick", "vr_pyramid_layout", "vr_build_pyramid",
+    "vr_touch_layout", "vr_measure_touch", "vr_touch_count",
 ]
 
 
@@ -101,6 +102,9 @@ def load():
     lib.vr_overlay_pick.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, ip, vp]
     lib.vr_pyramid_layout.argtypes = [C.c_int, C.c_int, C.c_int, ip, C.POINTER(PyramidLevel), C.POINTER(sz)]
     lib.vr_build_pyramid.argtypes = [vp, vp, C.c_int, C.c_int, sz, C.c_int, vp, vp]
+    lib.vr_touch_layout.argtypes = [vp, C.POINTER(sz)]
+    lib.vr_measure_touch.argtypes = [vp, C.c_int, C.POINTER(Partial), C.c_int, C.c_float, vp, C.c_int, vp]
+    lib.vr_touch_count.argtypes = [vp, vp, C.POINTER(C.c_uint64), vp]
     _lib = lib
     return lib
 
@@ -258,6 +262,21 @@ class Context:
     def composite_bricks(self, mode, parts, n, d_out, bg=(0, 0, 0, 0), stream=None):
         b = (C.c_float * 4)(*[float(x) for x in bg])
         self._check(self._lib.vr_composite_bricks(self._h, int(mode), parts, int(n), C.c_void_p(d_out.data_ptr()), b, _stream(stream)))
+
+    # ---- B_touch measurement
+    def touch_layout(self):
+        n = C.c_size_t(0)
+        self._check(self._lib.vr_touch_layout(self._h, C.byref(n)))
+        return n.value
+
+    def measure_touch(self, mode, parts, n, d_bitmap, tau=0.99, accumulate=False, stream=None):
+        self._check(self._lib.vr_measure_touch(self._h, int(mode), parts, int(n), float(tau), C.c_void_p(d_bitmap.data_ptr()),
+                                               int(bool(accumulate)), _stream(stream)))
+
+    def touch_count(self, d_bitmap, stream=None):
+        out = (C.c_uint64 * 3)()
+        self._check(self._lib.vr_touch_count(self._h, C.c_void_p(d_bitmap.data_ptr()), out, _stream(stream)))
+        return {"sectors": int(out[0]), "lines": int(out[1]), "taken_samples": int(out[2])}
 
     # ---- counters / options
     def get_counters(self, stream=None):

@@ -182,12 +182,13 @@ def tf_ramp():
     return t.astype(np.float32), 0.0, 20.0
 
 
-def tf_src():
-    """TF-src (C2..C5): vmin 0, vmax 32, alpha 0 for i <= 32 (v <= 4.02 sigma: noise is
-    transparent), then linear to 0.25 at i = 255."""
+def tf_src(threshold: int = 32):
+    """TF-src (C2..C5): vmin 0, vmax 32, alpha 0 for i <= threshold (32: v <= 4.02 sigma, noise is
+    transparent), then linear to 0.25 at i = 255.  Other thresholds model the astronomer dragging
+    the opacity threshold of the colour map (bench.py's tf_edit_ms)."""
     t = _colour_ramp()
     i = np.arange(256, dtype=np.float64)
-    t[:, 3] = np.where(i <= 32, 0.0, 0.25 * (i - 32.0) / (255.0 - 32.0))
+    t[:, 3] = np.where(i <= threshold, 0.0, 0.25 * (i - threshold) / (255.0 - threshold))
     return t.astype(np.float32), 0.0, 32.0
 
 

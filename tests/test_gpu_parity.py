@@ -410,55 +410,86 @@ def test_error_codes(H):
 
 
 # ------------------------------------------------------------------------------ BASELINE.json full sizes
-def _fullsize_check(H, w, block, n_random, frame_index):
+def _central_ray_axis(M):
+    """Dominant axis of the ray through the frame centre (what VR_OPT_RING's default looks at)."""
+    Mi = np.linalg.inv(np.asarray(M, dtype=np.float64).reshape(4, 4))
+    pn, pf = Mi @ np.array([0, 0, -1.0, 1.0]), Mi @ np.array([0, 0, 1.0, 1.0])
+    d = np.abs(pf[:3] / pf[3] - pn[:3] / pn[3])
+    return int(np.argmax(d))
+
+
+def _fullsize_check(H, w, block, n_random, frame_index, anchors=0, per_anchor=0):
     """Parity at a config's full size, in the launch configuration bench.py times (sort-last EA,
     plus whole-frame MIP): sampled pixels against the oracle (cube bytes fetched back brick by
-    brick), and whole-frame properties that hold at any size."""
+    brick), and whole-frame properties that hold at any size.  `frame_index` may be a list of orbit
+    frames (one resident cube).  Sampled pixels: a block at the frame centre, `n_random` seeded
+    pixels that hit the cube anywhere in the frame, and `anchors` seeded hit pixels spread over the
+    whole frame with `per_anchor` pixels drawn from the 9 x 9 neighbourhood of each (neighbouring
+    rays cross the same bricks, so a 64 GiB cube is checked far from the frame centre for a few GB of
+    traffic; the bricks of one anchor are dropped before the next is fetched)."""
     import torch
     from oracle import ovr
     sc = H.Scene(w.dims, w.brick, gen={"seed": w.seed, "sources": wl.make_sources(w),
                                        "zero_boxes": wl.make_zero_boxes(w), "continuum": w.continuum})
     vr = sc.vr
     W, Hh = w.frame
-    M = wl.config_camera(w, frame_index)
     tf = wl.TFS[w.tf]()
-    frame, imgs, ids = sc.render_sortlast(M, W, Hh, w.step, vr.MODE_EA, tf=tf, bg=BG, tau=w.tau)
-    mip = sc.render_mip(M, W, Hh, w.step, miss=0.0)
-    # sampled pixels: a block at the frame centre + seeded random pixels that hit the cube
-    rng = np.random.default_rng(w.view_seed)
-    cx, cy = W // 2, Hh // 2
-    xs, ys = np.arange(cx - block // 2, cx + block // 2), np.arange(cy - block // 2, cy + block // 2)
-    pix = np.stack(np.meshgrid(xs, ys), axis=-1).reshape(-1, 2)
-    if n_random:
-        hit = np.argwhere(mip != 0.0)
-        pick = hit[rng.choice(len(hit), size=min(n_random, len(hit)), replace=False)]
-        pix = np.concatenate([pix, pick[:, ::-1]])
-    pix = pix.astype(np.int32)
     brick = tuple(min(b, n) for b, n in zip(w.brick, w.dims))
-    touched = ovr.bricks_touched(M, W, Hh, w.step, w.dims, brick, pix)
-    vol = ovr.Volume(w.dims, brick, {int(b): sc.download_brick(int(b)) for b in touched})
-    kw = dict(tf=tf, bg=BG, tau=w.tau, pixels=pix)
-    o64, fl, _ = ovr.render(vol, M, W, Hh, w.step, ovr.EA, ovr.F64, split=ovr.SPLIT_SORTLAST, partition=brick, **kw)
-    o32, _, _ = ovr.render(vol, M, W, Hh, w.step, ovr.EA, ovr.F32, split=ovr.SPLIT_SORTLAST, partition=brick, **kw)
-    got = frame[pix[:, 1], pix[:, 0]]
-    H.compare(got, o64, fl, o32, what=f"{w.name} full-size EA sort-last")
-    assert np.array_equal(got, o32)
-    m64, flm, _ = ovr.render(vol, M, W, Hh, w.step, ovr.MIP, ovr.F64, miss=0.0, pixels=pix)
-    m32, _, _ = ovr.render(vol, M, W, Hh, w.step, ovr.MIP, ovr.F32, miss=0.0, pixels=pix)
-    gm = mip[pix[:, 1], pix[:, 0]]
-    H.compare(gm, m64, flm, m32, mode_mip=True, vmin=tf[1], vmax=tf[2], miss=0.0, what=f"{w.name} full-size MIP")
-    assert np.array_equal(gm, m32)
-    # whole-frame properties: MIP split == unsplit bit-exact; EA sort-last (ERT off) == global to 1e-6;
-    # ERT bound |frame_tau - frame_inf| <= (1 - tau) / tau; alpha within [0, 1]
-    mip_sl, _, _ = sc.render_sortlast(M, W, Hh, w.step, vr.MODE_MIP, bg=(0.0, 0, 0, 0))
-    assert np.array_equal(mip_sl, mip)
-    sl_inf, _, _ = sc.render_sortlast(M, W, Hh, w.step, vr.MODE_EA, tf=tf, bg=BG, tau=2.0)
-    gl_inf = sc.render_ea(M, W, Hh, w.step, tf, bg=BG, tau=2.0)
-    assert np.abs(sl_inf - gl_inf).max() < 2e-6
-    assert np.abs(frame - sl_inf).max() <= (1 - w.tau) / w.tau + 1e-6
-    assert frame[..., 3].min() >= 0.0 and frame[..., 3].max() <= 1.0 + 1e-6
+    rng = np.random.default_rng(w.view_seed)
+    frames = list(frame_index) if isinstance(frame_index, (list, tuple)) else [frame_index]
+    axes = []
+    for fi in frames:
+        M = wl.config_camera(w, fi)
+        axes.append(_central_ray_axis(M))
+        frame, imgs, ids = sc.render_sortlast(M, W, Hh, w.step, vr.MODE_EA, tf=tf, bg=BG, tau=w.tau)
+        mip = sc.render_mip(M, W, Hh, w.step, miss=0.0)
+        cx, cy = W // 2, Hh // 2
+        xs, ys = np.arange(cx - block // 2, cx + block // 2), np.arange(cy - block // 2, cy + block // 2)
+        groups = [np.stack(np.meshgrid(xs, ys), axis=-1).reshape(-1, 2)]
+        hit = np.argwhere(mip != 0.0)
+        if n_random:
+            pick = hit[rng.choice(len(hit), size=min(n_random, len(hit)), replace=False)]
+            groups[0] = np.concatenate([groups[0], pick[:, ::-1]])
+        for a in hit[rng.choice(len(hit), size=min(anchors, len(hit)), replace=False)] if anchors else []:
+            dx, dy = rng.integers(-4, 5, size=per_anchor), rng.integers(-4, 5, size=per_anchor)
+            px = np.stack([np.clip(a[1] + dx, 0, W - 1), np.clip(a[0] + dy, 0, Hh - 1)], axis=-1)
+            groups.append(np.unique(px, axis=0))
+        n_checked, off_centre_bricks = 0, set()
+        for pix in groups:
+            pix = pix.astype(np.int32)
+            touched = ovr.bricks_touched(M, W, Hh, w.step, w.dims, brick, pix)
+            off_centre_bricks.update(int(b) for b in touched)
+            vol = ovr.Volume(w.dims, brick, {int(b): sc.download_brick(int(b)) for b in touched})
+            kw = dict(tf=tf, bg=BG, tau=w.tau, pixels=pix)
+            o64, fl, _ = ovr.render(vol, M, W, Hh, w.step, ovr.EA, ovr.F64, split=ovr.SPLIT_SORTLAST, partition=brick, **kw)
+            o32, _, _ = ovr.render(vol, M, W, Hh, w.step, ovr.EA, ovr.F32, split=ovr.SPLIT_SORTLAST, partition=brick, **kw)
+            got = frame[pix[:, 1], pix[:, 0]]
+            H.compare(got, o64, fl, o32, what=f"{w.name} full-size EA sort-last, frame {fi}")
+            assert np.array_equal(got, o32)
+            m64, flm, _ = ovr.render(vol, M, W, Hh, w.step, ovr.MIP, ovr.F64, miss=0.0, pixels=pix)
+            m32, _, _ = ovr.render(vol, M, W, Hh, w.step, ovr.MIP, ovr.F32, miss=0.0, pixels=pix)
+            gm = mip[pix[:, 1], pix[:, 0]]
+            H.compare(gm, m64, flm, m32, mode_mip=True, vmin=tf[1], vmax=tf[2], miss=0.0, what=f"{w.name} full-size MIP, frame {fi}")
+            assert np.array_equal(gm, m32)
+            n_checked += len(pix)
+            del vol
+        assert n_checked >= block * block + n_random + anchors * max(1, per_anchor // 3)
+        # whole-frame properties: MIP split == unsplit bit-exact (so the sort-last MIP frame equals the oracle on the
+        # sampled pixels too); EA sort-last (ERT off) == global to 1e-6;
+        # ERT bound |frame_tau - frame_inf| <= (1 - tau) / tau; alpha within [0, 1]
+        mip_sl, _, _ = sc.render_sortlast(M, W, Hh, w.step, vr.MODE_MIP, bg=(0.0, 0, 0, 0))
+        assert np.array_equal(mip_sl, mip)
+        sl_inf, _, _ = sc.render_sortlast(M, W, Hh, w.step, vr.MODE_EA, tf=tf, bg=BG, tau=2.0)
+        gl_inf = sc.render_ea(M, W, Hh, w.step, tf, bg=BG, tau=2.0)
+        assert np.abs(sl_inf - gl_inf).max() < 2e-6
+        assert np.abs(frame - sl_inf).max() <= (1 - w.tau) / w.tau + 1e-6
+        assert frame[..., 3].min() >= 0.0 and frame[..., 3].max() <= 1.0 + 1e-6
+        if anchors:        # the anchors reach bricks whose byte offset in the brick-major cube passes 2^32
+            vox = brick[0] * brick[1] * brick[2]
+            assert max(off_centre_bricks) * vox * 4 > 2 ** 32 or w.n_voxels * 4 <= 2 ** 32
     del sc
     torch.cuda.empty_cache()
+    return axes
 
 
 def test_config_c2_full_size(H, marcher):
@@ -475,7 +506,10 @@ def test_config_c3_full_size_64gib(H, marcher):
     free, total = torch.cuda.mem_get_info()
     if free < 80e9:
         pytest.skip("needs ~70 GB of free HBM")
-    _fullsize_check(H, wl.C3, block=12, n_random=0, frame_index=37)
+    # two orbit frames: the central ray runs mostly along z on one (VR_OPT_RING resolves to the register ring)
+    # and across it on the other (cp.async ring); seeded hit pixels over the whole frame
+    axes = _fullsize_check(H, wl.C3, block=12, n_random=0, frame_index=[0, 90], anchors=12, per_anchor=24)
+    assert (axes[0] == 2) != (axes[1] == 2), axes
 
 
 def test_hipass_shaped_cube_with_partial_edge_bricks(H, marcher):
@@ -531,23 +565,30 @@ def _tiled_fullsize_check(H, w, panels, block, mip_frame=None):
     assert n_bricks > 0
     brick = tuple(min(b, n) for b, n in zip(w.brick, w.dims))
     cache = {}
+    rng = np.random.default_rng(w.view_seed)
+    n_checked = 0
     for (c, r) in panels:
         # the block in the panel's lower right corner (next to the seams), cast by the oracle with
         # the panel's own off-axis matrix: same rays, so the float32 oracle must match to the bit
         Mp = wl.panel_matrix(M, cols, rows, c, r)
-        xs, ys = np.arange(pw - block, pw), np.arange(ph - block, ph)
-        pix = np.stack(np.meshgrid(xs, ys), axis=-1).reshape(-1, 2).astype(np.int32)
-        touched = ovr.bricks_touched(Mp, pw, ph, w.step, w.dims, brick, pix)
-        for b in touched:
-            if int(b) not in cache:
-                cache[int(b)] = sc.download_brick(int(b))
-        vol = ovr.Volume(w.dims, brick, {int(b): cache[int(b)] for b in touched})
-        kw = dict(tf=tf, bg=BG, tau=w.tau, pixels=pix, split=ovr.SPLIT_SORTLAST, partition=brick)
-        o64, fl, _ = ovr.render(vol, Mp, pw, ph, w.step, ovr.EA, ovr.F64, **kw)
-        o32, _, _ = ovr.render(vol, Mp, pw, ph, w.step, ovr.EA, ovr.F32, **kw)
-        got = frame[r * ph + ys[0]:r * ph + ys[-1] + 1, c * pw + xs[0]:c * pw + xs[-1] + 1].cpu().numpy().reshape(-1, 4)
-        H.compare(got, o64, fl, o32, what=f"{w.name} full-size tiled EA, panel {(c, r)}")
-        assert np.array_equal(got, o32)
+        bx, by = int(rng.integers(0, pw - block + 1)), int(rng.integers(0, ph - block + 1))
+        for (ox, oy) in ((pw - block, ph - block), (bx, by)):          # ... and a block at a seeded place inside the panel
+            xs, ys = np.arange(ox, ox + block), np.arange(oy, oy + block)
+            pix = np.stack(np.meshgrid(xs, ys), axis=-1).reshape(-1, 2).astype(np.int32)
+            touched = ovr.bricks_touched(Mp, pw, ph, w.step, w.dims, brick, pix)
+            if len(cache) + len(touched) > 48:
+                cache.clear()                                           # bound the host copy of the cube
+            for b in touched:
+                if int(b) not in cache:
+                    cache[int(b)] = sc.download_brick(int(b))
+            vol = ovr.Volume(w.dims, brick, {int(b): cache[int(b)] for b in touched})
+            kw = dict(tf=tf, bg=BG, tau=w.tau, pixels=pix, split=ovr.SPLIT_SORTLAST, partition=brick)
+            o64, fl, _ = ovr.render(vol, Mp, pw, ph, w.step, ovr.EA, ovr.F64, **kw)
+            o32, _, _ = ovr.render(vol, Mp, pw, ph, w.step, ovr.EA, ovr.F32, **kw)
+            got = frame[r * ph + ys[0]:r * ph + ys[-1] + 1, c * pw + xs[0]:c * pw + xs[-1] + 1].cpu().numpy().reshape(-1, 4)
+            H.compare(got, o64, fl, o32, what=f"{w.name} full-size tiled EA, panel {(c, r)} block at {(ox, oy)}")
+            assert np.array_equal(got, o32)
+            n_checked += len(pix)
     # whole-frame properties: every pixel written, alpha in [0, 1], rows continuous across panel seams
     lo, hi = torch.aminmax(frame[..., 3])
     assert float(lo) >= min(0.0, BG[3]) and float(hi) <= 1.0 + 1e-6
@@ -581,7 +622,7 @@ def _tiled_fullsize_check(H, w, panels, block, mip_frame=None):
 def test_config_c4_full_size_tiled_9600x5400(H, marcher):
     if marcher != "auto":
         pytest.skip("full sizes run with the library's choice (what bench.py times)")
-    _tiled_fullsize_check(H, wl.C4, panels=[(2, 2), (0, 1), (4, 3)], block=8)
+    _tiled_fullsize_check(H, wl.C4, panels=[(2, 2), (0, 1), (4, 3), (2, 0)], block=8)
 
 
 def test_config_c5_full_size_128gib(H, marcher):
@@ -592,7 +633,7 @@ def test_config_c5_full_size_128gib(H, marcher):
     free, total = torch.cuda.mem_get_info()
     if free < 150e9:
         pytest.skip("needs ~142 GB of free HBM")
-    _tiled_fullsize_check(H, wl.C5, panels=[(2, 2), (1, 3)], block=6, mip_frame=(1920, 1080))
+    _tiled_fullsize_check(H, wl.C5, panels=[(2, 2), (1, 3), (3, 1)], block=6, mip_frame=(1920, 1080))
 
 
 def test_upload_refuses_non_finite_voxels(H):
