@@ -56,7 +56,7 @@ const char* vr_status_string(int status);
 /* Bytes the caller must allocate for the brick-major cube (bricks of bx*by*bz voxels stored with
  * a one-sided +1 halo, x pitch padded to a multiple of 4 floats) and for its metadata (per-brick
  * and per-8^3-cell (min,max) over the halo-inclusive voxel set, plus activity bits: one per brick,
- * per macro-cell and per voxel, i.e. 1/32 of the cube). */
+ * per macro-cell and per voxel, and a scratch bit per voxel for their classification: 2/32 of the cube). */
 int vr_cube_layout(int nx, int ny, int nz, int bx, int by, int bz, size_t* cube_bytes,
                    size_t* meta_bytes);
 

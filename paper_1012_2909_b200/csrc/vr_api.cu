@@ -130,6 +130,7 @@ void bind_meta(CubeDesc& c, const void* d_cube, void* d_meta) {
     c.cell_bits = (unsigned*)(m + ml.cell_bits) - lo * c.cell_words_per_brick;
     c.brick_active = (int*)(m + ml.brick_active) - lo;
     c.occ = (unsigned*)(m + ml.occ) - lo * c.occ_words_per_brick;
+    c.hot = (unsigned*)(m + ml.hot) - lo * c.occ_words_per_brick;
 }
 
 void apply_window(const vr_ctx* ctx, CubeDesc& c) {
@@ -281,8 +282,11 @@ int skip_level(const vr_ctx* ctx, int mode) {
 int ensure_occ(vr_ctx* ctx, int skip, cudaStream_t s) {
     if (skip < 3 || ctx->occ_valid) return VR_OK;
     if (ctx->cube.win_hi <= ctx->cube.win_lo) { ctx->occ_valid = true; return VR_OK; }
-    VR_CUDA(ctx, launch_classify_occ(ctx->cube, ctx->key_nz, ctx->key_vmin, ctx->key_scale, s));
-    ctx->launches += 1;
+    // the table's transparent prefix 0 .. t: a cell whose 8 corners all map to x <= t only meets entries of zero opacity
+    int t = -1;
+    while (t + 1 < 256 && ctx->key_nz[t + 2] == 0) ++t;
+    VR_CUDA(ctx, launch_classify_occ(ctx->cube, ctx->key_vmin, ctx->key_scale, (float)t, s));
+    ctx->launches += 2;
     ctx->occ_valid = true;
     return VR_OK;
 }
@@ -423,7 +427,7 @@ void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz,
     c.win_lo = 0; c.win_hi = c.nbricks;
     c.cells_per_brick = c.C[0] * c.C[1] * c.C[2];
     c.cell_words_per_brick = (c.cells_per_brick + 31) / 32;
-    c.occ_words_per_brick = 32 * c.C[0] * c.C[1] * ((c.C[2] + 1) / 2);
+    c.occ_words_per_brick = c.T[0] * c.T[1] * c.T[2];
     c.stride = layout == 0 ? (long long)align_up((size_t)c.P[0] * c.P[1] * c.P[2], 32)
                            : 32LL * c.T[0] * c.T[1] * c.T[2];
 }
@@ -439,6 +443,7 @@ MetaLayout meta_layout(const CubeDesc& c) {
     m.cell_bits = off; off = align_up(off + sizeof(unsigned) * nb * c.cell_words_per_brick, 256);
     m.brick_active = off; off = align_up(off + sizeof(int) * nb, 256);
     m.occ = off; off = align_up(off + sizeof(unsigned) * nb * c.occ_words_per_brick, 256);
+    m.hot = off; off = align_up(off + sizeof(unsigned) * nb * c.occ_words_per_brick, 256);
     m.total = off;
     return m;
 }
@@ -497,7 +502,7 @@ int vr_cube_layout(int nx, int ny, int nz, int bx, int by, int bz, size_t* cube_
     fill_cube_desc(c0, nx, ny, nz, bx, by, bz, 0);
     fill_cube_desc(c1, nx, ny, nz, bx, by, bz, 1);
     *cube_bytes_out = std::max(cube_bytes(c0), cube_bytes(c1));
-    *meta_bytes_out = meta_layout(c0).total;
+    *meta_bytes_out = std::max(meta_layout(c0).total, meta_layout(c1).total);
     return VR_OK;
 }
 
@@ -822,7 +827,7 @@ int vr_window_layout(int nx, int ny, int nz, int bx, int by, int bz, int first_b
     if (end_brick > c0.nbricks) return VR_ERR_INVALID_ARG;
     c0.win_lo = c1.win_lo = first_brick; c0.win_hi = c1.win_hi = end_brick;
     *cube_bytes_out = std::max<size_t>(256, std::max(cube_bytes(c0), cube_bytes(c1)));     // an empty window still gets valid buffers
-    *meta_bytes_out = std::max<size_t>(256, meta_layout(c0).total);
+    *meta_bytes_out = std::max<size_t>(256, std::max(meta_layout(c0).total, meta_layout(c1).total));
     return VR_OK;
 }
 

@@ -209,8 +209,9 @@ cudaError_t launch_unbrick(const CubeDesc& c, int brick, float* d_dst, cudaStrea
 
 cudaError_t launch_minmax(const CubeDesc& c, cudaStream_t s) {
     long long ncell = (long long)(c.win_hi - c.win_lo) * c.cells_per_brick;
-    cell_minmax_kernel<<<grid_for(ncell, 128), 128, 0, s>>>(c);
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e;
+    if (c.layout == 1) e = launch_cell_minmax_lines(c, s);          // vr_setup.cu: whole lines, coalesced
+    else { cell_minmax_kernel<<<grid_for(ncell, 128), 128, 0, s>>>(c); e = cudaGetLastError(); }
     if (e != cudaSuccess) return e;
     brick_minmax_kernel<<<c.win_hi - c.win_lo, 256, 0, s>>>(c);
     return cudaGetLastError();

@@ -44,13 +44,13 @@ struct CubeDesc {
     unsigned* cell_bits;         // EA activity of macro-cells vs the transfer function, 1 bit each
     int* brick_active;           // EA activity of bricks vs the transfer function
     int cell_words_per_brick;
-    // Occupancy bits (layout 1 only): one bit per trilinear cell (lower corner (lx,ly,lz), l < B),
-    // set iff the value range of its 8 corners can touch a table entry of non-zero opacity (O-10 at
-    // the finest level).  One 32-bit word per 4 x 4 x 2 micro-block, bit = the voxel's place inside
-    // the block, (lx&3) + 4 (ly&3) + 16 (lz&1); words ordered so that a 128-byte line covers 8 x 8 x 16 voxels:
-    //   word = 32 ((lx>>3) + C0 ((ly>>3) + C1 (lz>>4))) + ((lx>>2)&1) + 2 ((ly>>2)&1) + 4 ((lz>>1)&7)
+    // Occupancy bits (layout 1 only): one bit per trilinear cell (lower corner (lx,ly,lz), l < B), set iff one of
+    // its 8 corners maps above the transparent prefix of the table (O-10 at the finest level).  One 32-bit word per
+    // 4 x 4 x 2 micro-block, in the order of the block's 128-byte line in the brick (word = line index), bit = the
+    // slot of the lower corner inside the line, (lx&3) + 4 (ly&1) + 8 (lz&1) + 16 ((ly>>1)&1).
     unsigned* occ;
-    int occ_words_per_brick;     // 32 C0 C1 ceil(C2 / 2)
+    unsigned* hot;               // scratch of the same shape: one bit per VOXEL ("maps above the transparent prefix")
+    int occ_words_per_brick;     // T0 T1 T2
 };
 
 struct ViewDesc {
@@ -86,7 +86,7 @@ __host__ __device__ inline long long voxel_slot(const CubeDesc& c, int lx, int l
 size_t align_up(size_t v, size_t a);
 void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz, int layout);
 size_t cube_bytes(const CubeDesc& c);
-struct MetaLayout { size_t brick_mm, cell_mm, cell_bits, brick_active, occ, total; };
+struct MetaLayout { size_t brick_mm, cell_mm, cell_bits, brick_active, occ, hot, total; };
 MetaLayout meta_layout(const CubeDesc& c);
 
 // kernels' host launchers (vr_cube.cu / vr_march.cu / vr_composite.cu)
@@ -118,7 +118,8 @@ cudaError_t launch_composite(const ViewDesc& v, int mode, const PartialDev* d_pa
                              const float bg[4], cudaStream_t s);
 cudaError_t launch_classify_cells(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale,
                                   unsigned long long* d_active_count, cudaStream_t s);
-cudaError_t launch_classify_occ(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale, cudaStream_t s);
+cudaError_t launch_classify_occ(const CubeDesc& c, float vmin, float scale, float thr, cudaStream_t s);
+cudaError_t launch_cell_minmax_lines(const CubeDesc& c, cudaStream_t s);
 cudaError_t launch_overlay(const ViewDesc& v, const double M[16], const int* d_boxes, const float* d_colours,
                            const unsigned char* d_visible, int n, float* d_frame, int* d_pick, cudaStream_t s);
 cudaError_t launch_overlay_pick(const ViewDesc& v, const int* d_pick, int x, int y, int radius, int* d_out, cudaStream_t s);

@@ -772,84 +772,6 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
     }
 }
 
-// O-10 per transfer function at the level of one trilinear cell: one warp per occupancy word, lane =
-// the cell whose lower corner is the lane's voxel of the micro-block; the bit is set iff a table
-// entry that the value range of the cell's 8 corners can touch has non-zero opacity (same test and
-// same float32 operations as classify_cells_kernel; the interpolated value lies inside that range).
-// The 8 warps of a CTA take 4 x 2 micro-blocks in (y, z) and walk along x, so that the lines of
-// the +1 neighbours are found in L1.
-struct NzPrefix { int v[257]; };
-__global__ void __launch_bounds__(256)
-classify_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ NzPrefix nz, float vmin, float scale) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int nbx = (c.B[0] + 3) >> 2, nby = (c.B[1] + 3) >> 2, nbz = (c.B[2] + 1) >> 1;   // micro-blocks holding lower corners
-    const int ngy = (nby + 3) >> 2, ngz = (nbz + 1) >> 1;
-    const long long n_units = (long long)(c.win_hi - c.win_lo) * ngy * ngz;
-    for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
-        const int brick = c.win_lo + (int)(u / (ngy * ngz));
-        const int rem = (int)(u % (ngy * ngz));
-        const int by = 4 * (rem % ngy) + (warp & 3), bz = 2 * (rem / ngy) + (warp >> 2);
-        if (by >= nby || bz >= nbz) continue;
-        const int bi[3] = {brick % c.G[0], (brick / c.G[0]) % c.G[1], brick / (c.G[0] * c.G[1])};
-        const int lo[3] = {bi[0] * c.B[0], bi[1] * c.B[1], bi[2] * c.B[2]};
-        const BrickRef br = brick_ref<1>(c, brick, lo);
-        unsigned* occ = c.occ + (long long)brick * c.occ_words_per_brick;
-        const int ly = 4 * by + ((lane >> 2) & 3), lz = 2 * bz + (lane >> 4);        // lane = occ_bit_index
-        const bool row_ok = ly < c.B[1] && lz < c.B[2] && lo[1] + ly < c.N[1] && lo[2] + lz < c.N[2];
-        for (int bx = 0; bx < nbx; ++bx) {
-            const int lx = 4 * bx + (lane & 3);
-            bool active = false;
-            if (row_ok && lx < c.B[0] && lo[0] + lx < c.N[0]) {
-                float v[8];
-                gather8<1>(br, lo[0] + lx, lo[1] + ly, lo[2] + lz, v);
-                float mn = v[0], mx = v[0];
-#pragma unroll
-                for (int e = 1; e < 8; ++e) { mn = fminf(mn, v[e]); mx = fmaxf(mx, v[e]); }
-                const float xa = fminf(fmaxf(__fmul_rn(__fsub_rn(mn, vmin), scale), 0.f), 255.f);
-                const float xb = fminf(fmaxf(__fmul_rn(__fsub_rn(mx, vmin), scale), 0.f), 255.f);
-                const int ia = max(0, min((int)floorf(xa), 255)), ib = max(0, min((int)ceilf(xb), 255));
-                active = nz.v[ib + 1] - nz.v[ia] > 0;
-            }
-            const unsigned bits = __ballot_sync(0xffffffffu, active);
-            if (lane == 0) occ[occ_word_index(c, 4u * bx, 4u * by, 2u * bz)] = bits;
-        }
-    }
-}
-
-// O-10 per transfer function: one bit per 8^3 macro-cell, set iff a table entry that the cell's
-// value range [min, max] (halo-inclusive) can touch has non-zero opacity.  `nz` is the running
-// count of entries with non-zero baked opacity, so the range test is one subtraction.
-__global__ void classify_cells_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ NzPrefix nz,
-                                      float vmin, float scale, long long n_slots,
-                                      unsigned long long* __restrict__ active_count) {
-    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n_slots;
-         e += (long long)gridDim.x * blockDim.x) {
-        const long long word = (long long)c.win_lo * c.cell_words_per_brick + (e >> 5);
-        const int brick = (int)(word / c.cell_words_per_brick);
-        const int cidx = (int)(word % c.cell_words_per_brick) * 32 + (int)(e & 31);
-        bool active = false;
-        if (cidx < c.cells_per_brick) {
-            const float2 mm = c.cell_mm[(long long)brick * c.cells_per_brick + cidx];
-            if (mm.x <= mm.y) {
-                float xa = fminf(fmaxf(__fmul_rn(__fsub_rn(mm.x, vmin), scale), 0.f), 255.f);
-                float xb = fminf(fmaxf(__fmul_rn(__fsub_rn(mm.y, vmin), scale), 0.f), 255.f);
-                const int lo = max(0, min((int)floorf(xa), 255)), hi = max(0, min((int)ceilf(xb), 255));
-                active = nz.v[hi + 1] - nz.v[lo] > 0;
-            }
-        }
-        const unsigned bits = __ballot_sync(0xffffffffu, active);
-        if ((e & 31) == 0) {
-            c.cell_bits[word] = bits;
-            if (bits) atomicAdd(active_count, (unsigned long long)__popc(bits));
-        }
-    }
-}
-
-struct HalfTable { float4 v[128]; };
-__global__ void upload_half_kernel(float4* dst, const __grid_constant__ HalfTable h, int offset) {
-    if (threadIdx.x < 128) dst[offset + threadIdx.x] = h.v[threadIdx.x];
-}
-
 }  // namespace
 
 #define VR_DISPATCH(KERNEL, GRID, ...)                                                                   \
@@ -921,40 +843,6 @@ cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFD
         }
     }
     return cudaGetLastError();
-}
-
-cudaError_t launch_classify_occ(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale, cudaStream_t s) {
-    NzPrefix nz;
-    for (int i = 0; i < 257; ++i) nz.v[i] = nz_prefix[i];
-    classify_occ_kernel<<<148 * 8, 256, 0, s>>>(c, nz, vmin, scale);   // words of the padding beyond the brick are never read
-    return cudaGetLastError();
-}
-
-cudaError_t launch_classify_cells(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale,
-                                  unsigned long long* d_active_count, cudaStream_t s) {
-    NzPrefix nz;
-    for (int i = 0; i < 257; ++i) nz.v[i] = nz_prefix[i];
-    const long long n_slots = (long long)(c.win_hi - c.win_lo) * c.cell_words_per_brick * 32;
-    long long blocks = (n_slots + 255) / 256;
-    if (blocks > 148LL * 32) blocks = 148LL * 32;
-    classify_cells_kernel<<<(int)blocks, 256, 0, s>>>(c, nz, vmin, scale, n_slots, d_active_count);
-    return cudaGetLastError();
-}
-
-// The 4 KiB table travels in kernel parameter space (copied at launch), so the host buffer can be
-// reused immediately and no pinned staging or stream synchronisation is needed.
-cudaError_t launch_upload_table(float4* d_dst, const float* h_src_1024, cudaStream_t s) {
-    for (int half = 0; half < 2; ++half) {
-        HalfTable h;
-        for (int i = 0; i < 128; ++i) {
-            const float* p = h_src_1024 + 4 * (128 * half + i);
-            h.v[i] = make_float4(p[0], p[1], p[2], p[3]);
-        }
-        upload_half_kernel<<<1, 128, 0, s>>>(d_dst, h, 128 * half);
-        cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-    }
-    return cudaSuccess;
 }
 
 }  // namespace vr

@@ -284,12 +284,13 @@ __device__ __forceinline__ bool cell_idle(const CubeDesc& c, int bid, const int 
     return ((__ldg(&c.cell_bits[(long long)bid * c.cell_words_per_brick + (cidx >> 5)]) >> (cidx & 31)) & 1u) == 0u;
 }
 
+// Occupancy word and bit (CubeDesc::occ) of the trilinear cell whose lower corner is stored voxel (lx, ly, lz) of a
+// brick: the word of its micro-block (= the index of the block's line in the brick), the voxel's slot in the line.
 __device__ __forceinline__ unsigned occ_word_index(const CubeDesc& c, unsigned lx, unsigned ly, unsigned lz) {
-    return 32u * ((lx >> 3) + (unsigned)c.C[0] * ((ly >> 3) + (unsigned)c.C[1] * (lz >> 4))) +
-           ((lx >> 2) & 1u) + 2u * ((ly >> 2) & 1u) + 4u * ((lz >> 1) & 7u);
+    return (lx >> 2) + (unsigned)c.T[0] * ((ly >> 2) + (unsigned)c.T[1] * (lz >> 1));
 }
 __device__ __forceinline__ unsigned occ_bit_index(unsigned lx, unsigned ly, unsigned lz) {
-    return (lx & 3u) + ((ly & 3u) << 2) + ((lz & 1u) << 4);
+    return (lx & 3u) + ((ly & 1u) << 2) + ((lz & 1u) << 3) + ((ly & 2u) << 3);
 }
 
 constexpr float kJumpStep = 0.4f;

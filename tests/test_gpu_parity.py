@@ -455,6 +455,7 @@ def _fullsize_check(H, w, block, n_random, frame_index, anchors=0, per_anchor=0)
             px = np.stack([np.clip(a[1] + dx, 0, W - 1), np.clip(a[0] + dy, 0, Hh - 1)], axis=-1)
             groups.append(np.unique(px, axis=0))
         n_checked, off_centre_bricks = 0, set()
+        pool = {"ea": [], "mip": []}
         for pix in groups:
             pix = pix.astype(np.int32)
             touched = ovr.bricks_touched(M, W, Hh, w.step, w.dims, brick, pix)
@@ -464,15 +465,21 @@ def _fullsize_check(H, w, block, n_random, frame_index, anchors=0, per_anchor=0)
             o64, fl, _ = ovr.render(vol, M, W, Hh, w.step, ovr.EA, ovr.F64, split=ovr.SPLIT_SORTLAST, partition=brick, **kw)
             o32, _, _ = ovr.render(vol, M, W, Hh, w.step, ovr.EA, ovr.F32, split=ovr.SPLIT_SORTLAST, partition=brick, **kw)
             got = frame[pix[:, 1], pix[:, 0]]
-            H.compare(got, o64, fl, o32, what=f"{w.name} full-size EA sort-last, frame {fi}")
-            assert np.array_equal(got, o32)
+            assert np.array_equal(got, o32)                   # the kernels implement the float32 reading to the bit
+            pool["ea"].append((got, o64, fl, o32))
             m64, flm, _ = ovr.render(vol, M, W, Hh, w.step, ovr.MIP, ovr.F64, miss=0.0, pixels=pix)
             m32, _, _ = ovr.render(vol, M, W, Hh, w.step, ovr.MIP, ovr.F32, miss=0.0, pixels=pix)
             gm = mip[pix[:, 1], pix[:, 0]]
-            H.compare(gm, m64, flm, m32, mode_mip=True, vmin=tf[1], vmax=tf[2], miss=0.0, what=f"{w.name} full-size MIP, frame {fi}")
             assert np.array_equal(gm, m32)
+            pool["mip"].append((gm, m64, flm, m32))
             n_checked += len(pix)
             del vol
+        # BASELINE.json's tolerances are per frame and channel: all sampled pixels of the frame pooled
+        ea, mp = ([np.concatenate(v) for v in zip(*pool[k])] for k in ("ea", "mip"))
+        st_ea = H.compare(*ea, what=f"{w.name} full-size EA sort-last, frame {fi}")
+        st_mip = H.compare(*mp, mode_mip=True, vmin=tf[1], vmax=tf[2], miss=0.0, what=f"{w.name} full-size MIP, frame {fi}")
+        print(f"[parity] {w.name} frame {fi}: {n_checked} pixels, {len(off_centre_bricks)} bricks; EA max {st_ea['max'].max():.2e} rms "
+              f"{st_ea['rms'].max():.2e}; MIP max {st_mip['max'].max():.2e} rms {st_mip['rms'].max():.2e} (of 1e-4 / 1e-5)")
         assert n_checked >= block * block + n_random + anchors * max(1, per_anchor // 3)
         # whole-frame properties: MIP split == unsplit bit-exact (so the sort-last MIP frame equals the oracle on the
         # sampled pixels too); EA sort-last (ERT off) == global to 1e-6;
@@ -693,3 +700,55 @@ def test_brick_and_macro_cell_minmax_against_numpy(H):
                         continue
                     r = cube[lo[2]:h2[2] + 1, lo[1]:h2[1] + 1, lo[0]:h2[0] + 1]
                     assert got[0] == r.min() and got[1] == r.max(), (bid, cx, cy, cz)
+
+
+def test_occupancy_bits_against_numpy(H):
+    """S1 classification at the finest level (white box: d_meta holds (min,max) per brick and per macro-cell, the
+    macro-cell bits, the brick flags, then one occupancy word per 128-byte line of the cube, each region 256-byte
+    aligned): the bit of the trilinear cell with lower corner (lx, ly, lz), slot (lx&3) + 4 (ly&1) + 8 (lz&1) +
+    16 ((ly>>1)&1) of micro-block (lx>>2, ly>>2, lz>>1), is set iff one of the cell's 8 corners (zeros beyond the
+    cube) maps above the table's transparent prefix, (v - vmin) * scale > t in float32 (O-10)."""
+    dims, brick = (45, 38, 29), (16, 24, 8)
+    cube = noise_cube(dims[::-1], seed=33, scale=2.0)
+    sc = H.Scene(dims, brick, cube=cube)
+    vr = sc.vr
+    sc.ctx.set_option(vr.OPT_VARIANT, 0)
+    tfs = wl.tf_src(24)
+    M = wl.perspective_camera(dims, (64, 48), azimuth_deg=20.0)
+    sc.render_ea(M, 64, 48, 0.5, tfs, tau=0.99)                    # classifies against the table
+    assert sc.ctx.get_plan(vr.MODE_EA)["skip_level"] == 3
+    meta = sc.d_meta.cpu().numpy()
+    g = sc.grid()
+    nb = g[0] * g[1] * g[2]
+    C = [-(-b // 8) for b in brick]
+    cpb = C[0] * C[1] * C[2]
+    T = [(brick[0] + 4) // 4, (brick[1] + 4) // 4, (brick[2] + 2) // 2]
+    per = T[0] * T[1] * T[2]
+    up = lambda v: -(-v // 256) * 256
+    off = up(8 * nb)
+    off = up(off + 8 * nb * cpb)
+    off = up(off + 4 * nb * ((cpb + 31) // 32))
+    off = up(off + 4 * nb)
+    occ = meta[off:off + 4 * nb * per].view(np.uint32).reshape(nb, per)
+    pad = np.zeros((dims[2] + 1, dims[1] + 1, dims[0] + 1), dtype=np.float32)
+    pad[:-1, :-1, :-1] = cube
+    scale = np.float32(255.0 / (tfs[2] - tfs[1]))
+    hot = ((pad - np.float32(tfs[1])) * scale) > np.float32(24.0)
+    want = np.zeros_like(hot[:-1, :-1, :-1])
+    for dz in (0, 1):
+        for dy in (0, 1):
+            for dx in (0, 1):
+                want |= hot[dz:dz + dims[2], dy:dy + dims[1], dx:dx + dims[0]]
+    n_set = 0
+    for bid in range(nb):
+        bi = (bid % g[0], (bid // g[0]) % g[1], bid // (g[0] * g[1]))
+        o = [bi[a] * brick[a] for a in range(3)]
+        ext = [min(brick[a], dims[a] - o[a]) for a in range(3)]
+        lx, ly, lz = np.meshgrid(np.arange(ext[0]), np.arange(ext[1]), np.arange(ext[2]), indexing="ij")
+        word = (lx >> 2) + T[0] * ((ly >> 2) + T[1] * (lz >> 1))
+        bit = (lx & 3) + 4 * (ly & 1) + 8 * (lz & 1) + 16 * ((ly >> 1) & 1)
+        got = (occ[bid][word] >> bit.astype(np.uint32)) & 1
+        ref = want[o[2] + lz, o[1] + ly, o[0] + lx]
+        assert np.array_equal(got.astype(bool), ref), bid
+        n_set += int(ref.sum())
+    assert 0 < n_set < want.size // 2
