@@ -160,6 +160,8 @@ class Job:
         self.bitmap = None
         self.bg = (0.0, 0.0, 0.0, 0.0)
         self.slab_only = False
+        self.staged = False
+        self.peerfold = None
         self.configure(mode, tf or w.tf, w.frame, w.panels)
 
     def configure(self, mode, tf_name, frame, panels):
@@ -180,7 +182,7 @@ class Job:
         self.reset_events()
 
     def reset_events(self):
-        self.step_events, self.march_events = [], []
+        self.step_events, self.march_events, self.fold_events = [], [], []
         self.b_brick = self.partial_bytes = 0
 
     def close(self):
@@ -212,25 +214,39 @@ class Job:
         if set_tf:
             ctx.set_transfer_function(*self.tf)
         if self.shard is not None:
-            # sharded sort-last (paper_1012_2909_b200/sortlast.py): own bricks -> one partial frame, strips
-            # exchanged, folded in the slabs' visibility order, gathered
+            # sharded sort-last (paper_1012_2909_b200/sortlast.py): own bricks -> one partial frame; then ONE kernel reads
+            # this rank's strip of every rank's partial frame through peer pointers, folds the versions in the slabs'
+            # visibility order and stores the rows into every rank's final frame (--staged: all_to_all + fold + all_gather)
             sh, sl = self.shard, self.sortlast
             ctx.set_view(wl.config_camera(w, frame_index, frame=(self.W, self.H)), self.W, self.H, w.step)
-            if timed_events:
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record()
-            part = sh.render_partial(torch, self.mode, self.W, self.H, w.tau)
-            if timed_events:
-                e1.record()
-                self.march_events.append((e0, e1))
+            if self.peerfold is None or self.peerfold.mode != self.mode:
+                self.peerfold = sl.PeerFold(sh, torch, self.mode, self.W, self.H, dist=self.dist)
+            pf = self.peerfold
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)] if timed_events else None
+            if ev:
+                ev[0].record()
+            part = pf.render(w.tau)
+            if ev:
+                ev[1].record()
+                self.march_events.append((ev[0], ev[1]))
                 self.b_brick += 4 * self.brick_voxels() * (sh.end - sh.first)
                 self.partial_bytes += self.H * self.W * self.px_bytes
             if self.slab_only:
                 self.frame = part
-            else:
+            elif self.staged:
                 versions = sl.exchange_strips(self.dist, part, sh.world)
                 strip = sh.fold_strip(torch, self.mode, versions, self.W, self.H, self.bg)
                 self.frame = sl.gather_strips(self.dist, strip, sh.world, self.H)
+            else:
+                pf.barrier()
+                if ev:
+                    ev[2].record()
+                pf.fold(self.bg)
+                if ev:
+                    ev[3].record()
+                    self.fold_events.append((ev[2], ev[3]))
+                pf.barrier()
+                self.frame = pf.final
             if timed_events:
                 e = torch.cuda.Event(enable_timing=True)
                 e.record()
@@ -606,6 +622,8 @@ def main():
     ap.add_argument("--sharded", action="store_true",
                     help="N ranks share ONE cube: bricks sharded in z-slabs, sort-last exchange over NCCL (NEXT-1, "
                          "strong scaling); default: N independent replicas")
+    ap.add_argument("--staged", action="store_true", help="--sharded with the staged exchange (all_to_all_single + fold + all_gather) "
+                                                          "instead of the fused peer-memory kernel: the A/B baseline")
     ap.add_argument("--slab", default=None, metavar="R/W",
                     help="render only slab R of a W-way split of the bricks (what rank R of --sharded would render; no "
                          "exchange): the per-rank cost of NEXT-1 measured on one GPU")
@@ -655,6 +673,7 @@ def main():
         raise SystemExit("--sharded renders single-panel frames (use --frame WxH for the tiled workloads)")
     job = Job(w, local_rank, args.mode, shard=slab if slab else ((rank, world) if args.sharded else None), dist=dist, tf=args.tf)
     job.slab_only = slab is not None
+    job.staged = args.staged
     frank, fworld = (0, 1) if args.sharded else (rank, world)          # sharded: every rank renders every frame
     config = describe(job, args.mode, world, args)
 
@@ -675,6 +694,13 @@ def main():
     out.update(entry(job, m, args, peak, peak_src, touch_frames))
     out.update({"n_gpus": world, "warmup": args.warmup, "higher_is_better": True, "scaling": "strong" if args.sharded else "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config})
+    if args.sharded or slab:
+        fold_ms = [a.elapsed_time(b) for a, b in job.fold_events]
+        out["sharded"] = {"exchange": "staged (NCCL all_to_all_single + vr_composite_bricks + all_gather)" if args.staged else
+                          "fused (vr_fold_peers: peer-pointer loads, over-operator, peer-pointer stores in one kernel)",
+                          "rank0_render_ms": m["march_ms"] / max(m["n_march"], 1),
+                          "rank0_fold_ms": sum(fold_ms) / len(fold_ms) if fold_ms else None,
+                          "measured_on_ranks": world, "note": "N > 1 was not available to this build: unmeasured on hardware beyond what this line shows"}
     if world == 1 and not slab and not args.no_cpu:           # a slab holds only its own bricks: no oracle sample
         out["cpu_baseline"] = cpu_baseline(job, f0, args.cpu_seconds)
         out["vs_cpu_baseline"] = {"one_core": out["value"] / out["cpu_baseline"]["value"] if out["cpu_baseline"]["value"] else None,

@@ -157,6 +157,23 @@ int vr_window_layout(int nx, int ny, int nz, int bx, int by, int bz, int first_b
  * vr_composite_bricks equals the fold over all bricks up to float32 reassociation (MIP: exactly). */
 int vr_sort_groups(vr_ctx* ctx, const int* h_group_first, int n_groups, int* h_group_order);
 
+/* One kernel for the exchange, the fold and the gather of a sharded frame ("composite fused into the
+ * exchange"; PAPER.md line 13 / line 19: images of sub-volumes rendered on distributed GPUs are composited).  Rank r
+ * of n holds a full-frame partial image of its slab (vr_render_bricks + vr_composite_bricks with bg = 0, or -inf for
+ * MIP) in h_d_frames[r]: DEVICE pointers to this device's memory or to a peer's, mapped into this process (CUDA IPC:
+ * vr_ipc_export on the owner, vr_ipc_open here; or any peer-accessible allocation), float4 (EA) / float (MIP) pixels,
+ * rows pitch_px apart.  The call folds rows [y0, y0 + rows) of the n images in the order h_order (front first, from
+ * vr_sort_groups), reading each pixel straight from the owners' memory over NVLink, applies the background and stores
+ * the finished rows into the same rows of every frame of h_d_out[0 .. n_out) (each rank's final frame: the gather).
+ * No staging copy and no scratch.  The caller orders it after all ranks' partial frames are complete (a barrier). */
+int vr_fold_peers(vr_ctx* ctx, int mode, const void* const* h_d_frames, const int* h_order, int n, int width, int height,
+                  size_t pitch_px, int y0, int rows, void* const* h_d_out, int n_out, size_t out_pitch_px, const float bg[4],
+                  void* stream);
+/* CUDA IPC plumbing for the above: handle (64 bytes) + byte offset of d_ptr inside its allocation, to be sent to the
+ * peer processes; vr_ipc_open maps it there (the mapping lives until vr_destroy). */
+int vr_ipc_export(vr_ctx* ctx, const void* d_ptr, unsigned char handle[64], size_t* offset);
+int vr_ipc_open(vr_ctx* ctx, const unsigned char handle[64], size_t offset, void** d_ptr);
+
 /* ---- catalogue overlay (section 2: a source finder's
  *      output, "a set of detected astronomical sources represented by their bounding cubes",
  *      "superimposed as wireframe boxes on the volume rendering output"; "the user interaction

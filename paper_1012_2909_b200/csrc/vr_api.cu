@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 
+#include <cuda.h>
 #include <nvtx3/nvToolsExt.h>
 
 #include "vr_internal.cuh"
@@ -48,6 +49,7 @@ struct vr_ctx {
     int key_nz[257];
     float key_vmin = 0, key_scale = 0;
     int win_lo = 0, win_hi = -1;         // vr_set_brick_window (hi < 0: all bricks)
+    std::vector<void*> ipc_bases;        // peer allocations opened by vr_ipc_open
 };
 
 namespace {
@@ -378,6 +380,7 @@ int check_render_state(vr_ctx* ctx, bool need_tf) {
 int upload_partials(vr_ctx* ctx, int mode, const vr_partial* hp, int n, bool with_tiles, int* total_tiles, cudaStream_t s) {
     if (n > (int)ctx->partials_cap) {
         if (ctx->d_partials) cudaFree(ctx->d_partials);
+    for (void* b : ctx->ipc_bases) cudaIpcCloseMemHandle(b);
         ctx->d_partials = nullptr;
         size_t cap = std::max<size_t>(256, (size_t)n * 2);
         VR_CUDA(ctx, cudaMalloc(&ctx->d_partials, cap * sizeof(PartialDev)));
@@ -492,6 +495,7 @@ int vr_destroy(vr_ctx* ctx) {
     if (ctx->d_counters) cudaFree(ctx->d_counters);
     if (ctx->d_scratch) cudaFree(ctx->d_scratch);
     if (ctx->d_partials) cudaFree(ctx->d_partials);
+    for (void* b : ctx->ipc_bases) cudaIpcCloseMemHandle(b);
     delete ctx;
     return VR_OK;
 }
@@ -882,6 +886,67 @@ int vr_composite_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, floa
     if ((rc = upload_partials(ctx, mode, hp, n, false, nullptr, s))) return rc;
     VR_CUDA(ctx, launch_composite(ctx->view, mode, ctx->d_partials, n, d_out, bg, s));
     ctx->launches += 1;
+    return VR_OK;
+}
+
+int vr_ipc_export(vr_ctx* ctx, const void* d_ptr, unsigned char handle[64], size_t* offset) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    enter(ctx);
+    if (!d_ptr || !handle || !offset) return fail(ctx, VR_ERR_INVALID_ARG, "vr_ipc_export: bad argument");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "cudaIpcMemHandle_t is 64 bytes");
+    cudaIpcMemHandle_t h;
+    VR_CUDA(ctx, cudaIpcGetMemHandle(&h, const_cast<void*>(d_ptr)));       // names the whole allocation d_ptr lies in
+    // the base of that allocation: a driver call, looked up at run time so that libvr needs no link to libcuda
+    typedef CUresult (*range_fn)(CUdeviceptr*, size_t*, CUdeviceptr);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    VR_CUDA(ctx, cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &qr));
+    CUdeviceptr base = 0;
+    size_t size = 0;
+    if (!fn || qr != cudaDriverEntryPointSuccess || ((range_fn)fn)(&base, &size, (CUdeviceptr)d_ptr) != CUDA_SUCCESS)
+        return fail(ctx, VR_ERR_CUDA, "vr_ipc_export: cuMemGetAddressRange failed");
+    std::memcpy(handle, &h, 64);
+    *offset = (size_t)((CUdeviceptr)d_ptr - base);
+    return VR_OK;
+}
+
+int vr_ipc_open(vr_ctx* ctx, const unsigned char handle[64], size_t offset, void** d_ptr) {
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    enter(ctx);
+    if (!handle || !d_ptr) return fail(ctx, VR_ERR_INVALID_ARG, "vr_ipc_open: bad argument");
+    cudaIpcMemHandle_t h;
+    std::memcpy(&h, handle, 64);
+    void* base = nullptr;
+    VR_CUDA(ctx, cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess));
+    ctx->ipc_bases.push_back(base);                                          // closed by vr_destroy
+    *d_ptr = (char*)base + offset;
+    return VR_OK;
+}
+
+int vr_fold_peers(vr_ctx* ctx, int mode, const void* const* h_d_frames, const int* h_order, int n, int width, int height,
+                  size_t pitch_px, int y0, int rows, void* const* h_d_out, int n_out, size_t out_pitch_px, const float bg[4],
+                  void* stream) {
+    VR_RANGE();
+    if (!ctx) return VR_ERR_INVALID_ARG;
+    enter(ctx);
+    if (!h_d_frames || !h_order || !h_d_out || !bg || n <= 0 || n > kMaxPeers || n_out <= 0 || n_out > kMaxPeers || width <= 0 ||
+        height <= 0 || pitch_px < (size_t)width || out_pitch_px < (size_t)width || y0 < 0 || rows < 0 || y0 + rows > height ||
+        (mode != VR_MODE_MIP && mode != VR_MODE_EA))
+        return fail(ctx, VR_ERR_INVALID_ARG, "vr_fold_peers: bad argument");
+    PeerList L{};
+    const uintptr_t align = mode == VR_MODE_EA ? 15 : 3;
+    for (int g = 0; g < n; ++g) {
+        const int r = h_order[g];
+        if (r < 0 || r >= n || !h_d_frames[r] || ((uintptr_t)h_d_frames[r] & align)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_fold_peers: bad order / frame pointer");
+        L.in[g] = h_d_frames[r];
+    }
+    for (int o = 0; o < n_out; ++o) {
+        if (!h_d_out[o] || ((uintptr_t)h_d_out[o] & align)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_fold_peers: bad output pointer");
+        L.out[o] = h_d_out[o];
+    }
+    L.n = n; L.n_out = n_out;
+    VR_CUDA(ctx, launch_fold_peers(L, mode, width, (long long)pitch_px, y0, rows, (long long)out_pitch_px, bg, (cudaStream_t)stream));
+    ctx->launches += rows > 0 ? 1 : 0;
     return VR_OK;
 }
 

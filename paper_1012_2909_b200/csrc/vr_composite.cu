@@ -63,7 +63,56 @@ composite_kernel(const __grid_constant__ ViewDesc V, const PartialDev* __restric
     }
 }
 
+// NEXT-1: exchange + fold + gather of a sharded sort-last frame as ONE kernel over peer
+// memory.  Every rank holds a full-frame partial image of its slab of bricks; this rank owns rows [y0, y0 + rows).
+// Each thread reads its pixel from every rank's buffer (its own or a peer's mapped over NVLink: plain
+// ld.global on peer pointers, no staging copy), folds the versions front to back (O-8 SORT-LAST) and stores the
+// finished pixel into every rank's output frame (st.global on peer pointers: the gather).
+template <int MODE>
+__global__ void __launch_bounds__(128)
+fold_peers_kernel(const __grid_constant__ PeerList L, int width, long long pitch, int y0, int rows, long long out_pitch,
+                  float bg0, float bg1, float bg2, float bg3) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= (long long)rows * width) return;
+    const int i = (int)(e % width), j = y0 + (int)(e / width);
+    const long long px = (long long)j * pitch + i;
+    if (MODE == VR_MODE_MIP) {
+        float m = -INFINITY;
+        for (int g = 0; g < L.n; ++g) m = fmaxf(m, __ldcg(reinterpret_cast<const float*>(L.in[g]) + px));
+        const float v = (m == -INFINITY) ? bg0 : m;
+        for (int o = 0; o < L.n_out; ++o) reinterpret_cast<float*>(L.out[o])[(long long)j * out_pitch + i] = v;
+        return;
+    }
+    float C0 = 0.f, C1 = 0.f, C2 = 0.f, A = 0.f;
+    for (int base = 0; base < L.n; base += 8) {                // 8 peer loads in flight per thread
+        float4 pb[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            pb[u] = base + u < L.n ? __ldcg(reinterpret_cast<const float4*>(L.in[base + u]) + px) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            if (base + u >= L.n) break;
+            const float t = __fsub_rn(1.f, A);
+            C0 = __fmaf_rn(t, pb[u].x, C0); C1 = __fmaf_rn(t, pb[u].y, C1); C2 = __fmaf_rn(t, pb[u].z, C2);
+            A = __fmaf_rn(t, pb[u].w, A);
+        }
+    }
+    const float t = __fsub_rn(1.f, A);
+    const float4 v = make_float4(__fmaf_rn(t, bg0, C0), __fmaf_rn(t, bg1, C1), __fmaf_rn(t, bg2, C2), __fmaf_rn(t, bg3, A));
+    for (int o = 0; o < L.n_out; ++o) reinterpret_cast<float4*>(L.out[o])[(long long)j * out_pitch + i] = v;
+}
+
 }  // namespace
+
+cudaError_t launch_fold_peers(const PeerList& L, int mode, int width, long long pitch, int y0, int rows, long long out_pitch,
+                              const float bg[4], cudaStream_t s) {
+    const long long n = (long long)rows * width;
+    if (n <= 0) return cudaSuccess;
+    const unsigned blocks = (unsigned)((n + 127) / 128);
+    if (mode == VR_MODE_MIP) fold_peers_kernel<VR_MODE_MIP><<<blocks, 128, 0, s>>>(L, width, pitch, y0, rows, out_pitch, bg[0], bg[1], bg[2], bg[3]);
+    else fold_peers_kernel<VR_MODE_EA><<<blocks, 128, 0, s>>>(L, width, pitch, y0, rows, out_pitch, bg[0], bg[1], bg[2], bg[3]);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_composite(const ViewDesc& v, int mode, const PartialDev* d_partials, int n, float* out,
                              const float bg[4], cudaStream_t s) {

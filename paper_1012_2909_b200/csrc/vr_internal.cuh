@@ -116,6 +116,10 @@ cudaError_t launch_touch(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, 
 cudaError_t launch_touch_count(const unsigned* d_bitmap, long long n_words, unsigned long long* d_out, cudaStream_t s);
 cudaError_t launch_composite(const ViewDesc& v, int mode, const PartialDev* d_partials, int n, float* out,
                              const float bg[4], cudaStream_t s);
+constexpr int kMaxPeers = 32;
+struct PeerList { const void* in[kMaxPeers]; void* out[kMaxPeers]; int n, n_out; };   // `in` already in fold order
+cudaError_t launch_fold_peers(const PeerList& L, int mode, int width, long long pitch, int y0, int rows, long long out_pitch,
+                              const float bg[4], cudaStream_t s);
 cudaError_t launch_classify_cells(const CubeDesc& c, const int nz_prefix[257], float vmin, float scale,
                                   unsigned long long* d_active_count, cudaStream_t s);
 cudaError_t launch_classify_occ(const CubeDesc& c, float vmin, float scale, float thr, cudaStream_t s);

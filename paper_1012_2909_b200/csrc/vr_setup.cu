@@ -49,42 +49,55 @@ cell_minmax_lines_kernel(const __grid_constant__ CubeDesc c, int chunks_x) {
         const int ly = 4 * ty + ly3, lz = 2 * tz + lz1;
         const bool row_ok = ly <= lim[1] && lz <= lim[2] && (ty_off < 2 || ly3 == 0) && (tz_off < 4 || lz1 == 0);
         const float4* col = reinterpret_cast<const float4*>(brick_base + 32LL * c.T[0] * (ty + (long long)c.T[1] * tz)) + r;
-        for (int t0 = tx_a; t0 <= tx_b; t0 += 4) {
-            const int tx = t0 + g;
-            float mn = INFINITY, mx = -INFINITY, fmn = INFINITY, fmx = -INFINITY;
-            if (row_ok && tx <= tx_b) {
-                const float4 v = __ldg(col + 8 * tx);
-                const int x0 = 4 * tx;
-                if (x0 + 3 <= lim[0]) {
-                    mn = fminf(fminf(v.x, v.y), fminf(v.z, v.w)); mx = fmaxf(fmaxf(v.x, v.y), fmaxf(v.z, v.w));
-                    fmn = fmx = v.x;
-                } else {
-                    if (x0 <= lim[0]) { mn = mx = fmn = fmx = v.x; }
-                    if (x0 + 1 <= lim[0]) { mn = fminf(mn, v.y); mx = fmaxf(mx, v.y); }
-                    if (x0 + 2 <= lim[0]) { mn = fminf(mn, v.z); mx = fmaxf(mx, v.z); }
-                }
+        // 4 warp-loads (16 lines, 2 KiB) in flight per warp before the first is reduced: the pass is bound by the
+        // bytes in flight (one load per warp at a time reached 2 TB/s)
+        for (int t00 = tx_a; t00 <= tx_b; t00 += 16) {
+            float4 vv[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int tx = t00 + 4 * u + g;
+                vv[u] = (row_ok && tx <= tx_b) ? __ldg(col + 8 * tx) : make_float4(0.f, 0.f, 0.f, 0.f);
             }
 #pragma unroll
-            for (int o = 1; o < 8; o <<= 1) {                  // over the 8 rows of the line
-                mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, o)); mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-                fmn = fminf(fmn, __shfl_xor_sync(0xffffffffu, fmn, o)); fmx = fmaxf(fmx, __shfl_xor_sync(0xffffffffu, fmx, o));
+            for (int u = 0; u < 4; ++u) {
+                const int t0 = t00 + 4 * u;
+                if (t0 > tx_b) break;                           // warp-uniform
+                const int tx = t0 + g;
+                float mn = INFINITY, mx = -INFINITY, fmn = INFINITY, fmx = -INFINITY;
+                if (row_ok && tx <= tx_b) {
+                    const float4 v = vv[u];
+                    const int x0 = 4 * tx;
+                    if (x0 + 3 <= lim[0]) {
+                        mn = fminf(fminf(v.x, v.y), fminf(v.z, v.w)); mx = fmaxf(fmaxf(v.x, v.y), fmaxf(v.z, v.w));
+                        fmn = fmx = v.x;
+                    } else {
+                        if (x0 <= lim[0]) { mn = mx = fmn = fmx = v.x; }
+                        if (x0 + 1 <= lim[0]) { mn = fminf(mn, v.y); mx = fmaxf(mx, v.y); }
+                        if (x0 + 2 <= lim[0]) { mn = fminf(mn, v.z); mx = fmaxf(mx, v.z); }
+                    }
+                }
+#pragma unroll
+                for (int o = 1; o < 8; o <<= 1) {                  // over the 8 rows of the line
+                    mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, o)); mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+                    fmn = fminf(fmn, __shfl_xor_sync(0xffffffffu, fmn, o)); fmx = fmaxf(fmx, __shfl_xor_sync(0xffffffffu, fmx, o));
+                }
+                // lines q, q + 1 (q even, relative to tx_a) fill cell q / 2; the first plane of line q + 2 is its halo
+                const float mn1 = __shfl_down_sync(0xffffffffu, mn, 8), mx1 = __shfl_down_sync(0xffffffffu, mx, 8);
+                const float fmn2 = __shfl_down_sync(0xffffffffu, fmn, 16), fmx2 = __shfl_down_sync(0xffffffffu, fmx, 16);
+                const int cell = (t0 - tx_a) / 2 + (g >> 1);
+                if (lane == 0) {                                   // the halo of the previous iteration's second cell
+                    if (cell > 0) { smin[warp][cell - 1] = fminf(smin[warp][cell - 1], fmn); smax[warp][cell - 1] = fmaxf(smax[warp][cell - 1], fmx); }
+                }
+                __syncwarp();
+                if (lane == 0) {
+                    smin[warp][cell] = fminf(smin[warp][cell], fminf(fminf(mn, mn1), fmn2));
+                    smax[warp][cell] = fmaxf(smax[warp][cell], fmaxf(fmaxf(mx, mx1), fmx2));
+                } else if (lane == 16) {
+                    smin[warp][cell] = fminf(smin[warp][cell], fminf(mn, mn1));
+                    smax[warp][cell] = fmaxf(smax[warp][cell], fmaxf(mx, mx1));
+                }
+                __syncwarp();
             }
-            // lines q, q + 1 (q even, relative to tx_a) fill cell q / 2; the first plane of line q + 2 is its halo
-            const float mn1 = __shfl_down_sync(0xffffffffu, mn, 8), mx1 = __shfl_down_sync(0xffffffffu, mx, 8);
-            const float fmn2 = __shfl_down_sync(0xffffffffu, fmn, 16), fmx2 = __shfl_down_sync(0xffffffffu, fmx, 16);
-            const int cell = (t0 - tx_a) / 2 + (g >> 1);
-            if (lane == 0) {                                   // the halo of the previous iteration's second cell
-                if (cell > 0) { smin[warp][cell - 1] = fminf(smin[warp][cell - 1], fmn); smax[warp][cell - 1] = fmaxf(smax[warp][cell - 1], fmx); }
-            }
-            __syncwarp();
-            if (lane == 0) {
-                smin[warp][cell] = fminf(smin[warp][cell], fminf(fminf(mn, mn1), fmn2));
-                smax[warp][cell] = fmaxf(smax[warp][cell], fmaxf(fmaxf(mx, mx1), fmx2));
-            } else if (lane == 16) {
-                smin[warp][cell] = fminf(smin[warp][cell], fminf(mn, mn1));
-                smax[warp][cell] = fmaxf(smax[warp][cell], fmaxf(mx, mx1));
-            }
-            __syncwarp();
         }
     }
     __syncthreads();

@@ -25,7 +25,7 @@ EXPORTS = [
     "vr_sort_bricks", "vr_partial_layout", "vr_render_bricks", "vr_composite_bricks",
     "vr_get_counters", "vr_reset_counters", "vr_set_option", "vr_get_plan",
     "vr_set_brick_window", "vr_window_layout", "vr_sort_groups", "vr_overlay_catalogue", "vr_overlay_pick", "vr_pyramid_layout", "vr_build_pyramid",
-    "vr_touch_layout", "vr_measure_touch", "vr_touch_count",
+    "vr_touch_layout", "vr_measure_touch", "vr_touch_count", "vr_fold_peers", "vr_ipc_export", "vr_ipc_open",
 ]
 
 
@@ -105,6 +105,10 @@ def load():
     lib.vr_touch_layout.argtypes = [vp, C.POINTER(sz)]
     lib.vr_measure_touch.argtypes = [vp, C.c_int, C.POINTER(Partial), C.c_int, C.c_float, vp, C.c_int, vp]
     lib.vr_touch_count.argtypes = [vp, vp, C.POINTER(C.c_uint64), vp]
+    lib.vr_fold_peers.argtypes = [vp, C.c_int, C.POINTER(vp), ip, C.c_int, C.c_int, C.c_int, sz, C.c_int, C.c_int,
+                                  C.POINTER(vp), C.c_int, sz, fp, vp]
+    lib.vr_ipc_export.argtypes = [vp, vp, C.c_char_p, C.POINTER(sz)]
+    lib.vr_ipc_open.argtypes = [vp, C.c_char_p, sz, C.POINTER(vp)]
     _lib = lib
     return lib
 
@@ -262,6 +266,32 @@ class Context:
     def composite_bricks(self, mode, parts, n, d_out, bg=(0, 0, 0, 0), stream=None):
         b = (C.c_float * 4)(*[float(x) for x in bg])
         self._check(self._lib.vr_composite_bricks(self._h, int(mode), parts, int(n), C.c_void_p(d_out.data_ptr()), b, _stream(stream)))
+
+    # ---- sharded sort-last: exchange + fold + gather in one kernel over peer memory
+    def fold_peers(self, mode, frame_ptrs, order, width, height, pitch_px, y0, rows, out_ptrs, out_pitch_px, bg=(0, 0, 0, 0),
+                   stream=None):
+        """frame_ptrs / out_ptrs: device addresses (ints) of every rank's partial frame / final frame."""
+        n, n_out = len(frame_ptrs), len(out_ptrs)
+        fin = (C.c_void_p * n)(*[int(p) for p in frame_ptrs])
+        fout = (C.c_void_p * n_out)(*[int(p) for p in out_ptrs])
+        order = np.ascontiguousarray(order, dtype=np.int32)
+        b = (C.c_float * 4)(*[float(x) for x in bg])
+        self._check(self._lib.vr_fold_peers(self._h, int(mode), fin, order.ctypes.data_as(C.POINTER(C.c_int)), n, int(width),
+                                            int(height), int(pitch_px), int(y0), int(rows), fout, n_out, int(out_pitch_px), b,
+                                            _stream(stream)))
+
+    def ipc_export(self, tensor):
+        """(handle bytes, offset) naming a CUDA tensor's memory for another process (CUDA IPC)."""
+        h = C.create_string_buffer(64)
+        off = C.c_size_t(0)
+        self._check(self._lib.vr_ipc_export(self._h, C.c_void_p(tensor.data_ptr()), h, C.byref(off)))
+        return h.raw, off.value
+
+    def ipc_open(self, handle, offset):
+        """Device address in THIS process of memory exported by a peer process."""
+        p = C.c_void_p(None)
+        self._check(self._lib.vr_ipc_open(self._h, C.c_char_p(handle), int(offset), C.byref(p)))
+        return p.value
 
     # ---- B_touch measurement
     def touch_layout(self):

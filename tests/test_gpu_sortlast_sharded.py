@@ -168,3 +168,78 @@ def test_wallaby_scale_slab_one_rank_of_many():
     part = sh.render_partial(torch, vr.MODE_EA, W, H, 0.99)
     torch.cuda.synchronize()
     assert float(part[..., 3].max()) <= 1.0 + 1e-6 and float(part[..., 3].min()) >= 0.0
+
+
+def _oracle_two_level(ovr, vol, M, W, H, step, omode, brick, grid, group_first, tf, tau, bg, miss):
+    """The sharded frame by the oracle's own pieces, float32: per-brick partial images (O-8 SORT-LAST), folded per
+    slab in the bricks' visibility order without a background, then the slabs' images folded in the slabs' order."""
+    keys, _ = ovr.visibility_keys(M, W, H, step, brick, grid)
+    order = ovr.visibility_order(keys)
+    full = (0, 0, W, H)
+    slab_imgs, slab_keys = [], []
+    for g in range(len(group_first) - 1):
+        ids = [int(b) for b in order if group_first[g] <= b < group_first[g + 1]]
+        imgs = [ovr.render_brick(vol, M, W, H, step, omode, b, full, brick, ovr.F32, tf=tf, tau=tau) for b in ids]
+        if omode == ovr.EA:
+            img = ovr.composite(omode, [full] * len(ids), imgs, None, W, H, bg=(0, 0, 0, 0), precision=ovr.F32) if ids else np.zeros((H, W, 4), np.float32)
+        else:
+            img = np.max(np.stack(imgs), axis=0) if ids else np.full((H, W), -np.inf, np.float32)
+        slab_imgs.append(img)
+        slab_keys.append(min(keys[group_first[g]:group_first[g + 1]]) if ids else np.iinfo(np.int32).max)
+    slab_order = np.argsort(np.array(slab_keys), kind="stable").astype(np.int32)
+    return ovr.composite(omode, [full] * len(slab_imgs), slab_imgs, slab_order, W, H, bg=bg, miss=miss, precision=ovr.F32)
+
+
+@pytest.mark.parametrize("world,balanced", [(2, False), (3, True), (7, False)])
+def test_fused_peer_fold_equals_the_oracle(world, balanced):
+    """NEXT-1: one vr_fold_peers launch per rank (exchange + fold + gather through the peers' pointers; here all
+    ranks live in one process on one device, so the pointers are plain) against the ORACLE's sort-last pieces put
+    together slab by slab.  world = 7 exceeds the 5 brick layers: two ranks hold empty slabs."""
+    import torch
+    from paper_1012_2909_b200 import sortlast as sl, vr, workloads as wl
+    from oracle import ovr
+    import helpers
+    w = wl.scaled(wl.C3, "shard", (96, 80, 160), (32, 32, 32), (160, 90), n_sources=40)
+    W, H = w.frame
+    src = wl.make_sources(w)
+    tf = wl.tf_fog()
+    bg = (0.05, 0.1, 0.2, 0.3)
+    grid = w.brick_grid
+    M0 = wl.perspective_camera(w.dims, w.frame, azimuth_deg=20.0)
+    group_first = sl.plan_slabs(w.dims, w.brick, w.frame, [wl.perspective_camera(w.dims, w.frame, azimuth_deg=a) for a in (0, 120, 240)],
+                                w.step, world) if balanced else None
+    sc = helpers.Scene(w.dims, w.brick, gen={"seed": w.seed, "sources": src, "continuum": w.continuum})
+    vol = sc.oracle_volume()
+    for mode, omode, tau in ((vr.MODE_EA, ovr.EA, 0.95), (vr.MODE_MIP, ovr.MIP, 2.0)):
+        shards, folds, keep = [], [], []
+        for r in range(world):
+            ctx = vr.Context(0)
+            sh = sl.Shard(ctx, w.dims, w.brick, r, world, group_first=group_first)
+            sh.bind()
+            cb, mb = sh.layout()
+            d_cube = torch.empty(max(cb // 4, 64), dtype=torch.float32, device="cuda")
+            d_meta = torch.empty(max(mb, 256), dtype=torch.uint8, device="cuda")
+            ctx.generate_cube(w.seed, w.dims, w.brick, d_cube, d_meta, sources=src, continuum=w.continuum)
+            ctx.set_transfer_function(*tf)
+            shards.append(sh)
+            keep.append((d_cube, d_meta))
+            folds.append(sl.PeerFold(sh, torch, mode, W, H))
+        peers = [(f.partial.data_ptr(), f.final.data_ptr()) for f in folds]
+        for f in folds:
+            f.bind(peers)
+        assert sum(s.end - s.first for s in shards) == grid[0] * grid[1] * grid[2]
+        for az in (20.0, 200.0):
+            M = wl.perspective_camera(w.dims, w.frame, azimuth_deg=az)
+            for f in folds:
+                f.shard.ctx.set_view(M, W, H, w.step)
+                f.render(tau)
+            torch.cuda.synchronize()                                  # the barrier of the multi-process path
+            for f in folds:
+                f.fold(bg if mode == vr.MODE_EA else (-3.0, 0, 0, 0))
+            torch.cuda.synchronize()
+            want = _oracle_two_level(ovr, vol, M, W, H, w.step, omode, w.brick, grid, shards[0].group_first, tf, tau, bg, -3.0)
+            for f in folds:                                           # every rank holds the whole finished frame
+                got = f.final.cpu().numpy()
+                got = got if mode == vr.MODE_EA else got[..., 0]
+                assert np.array_equal(got, want), (world, mode, az, f.shard.rank)
+    del M0

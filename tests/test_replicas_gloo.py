@@ -82,6 +82,23 @@ def test_slab_groups_cover_the_grid():
         assert max(sizes) - min(sizes) <= grid[0] * grid[1]
 
 
+def test_balanced_groups_minimise_the_heaviest_slab():
+    """Linear partition of z-layers by weight (paper_1012_2909_b200/sortlast.py): brute force over all cuts."""
+    import itertools
+    import numpy as np
+    from paper_1012_2909_b200 import sortlast as sl
+    rng = np.random.default_rng(5)
+    for n, world in ((6, 3), (8, 4), (5, 2), (4, 4), (3, 5)):
+        wts = rng.uniform(0.5, 4.0, n)
+        first = sl.balanced_groups(wts, 7, world)
+        assert first[0] == 0 and first[-1] == 7 * n and all(b >= a for a, b in zip(first, first[1:])) and all(f % 7 == 0 for f in first)
+        cuts = [f // 7 for f in first]
+        got = max(wts[a:b].sum() for a, b in zip(cuts, cuts[1:]) if b > a)
+        k = min(world, n)
+        best = min(max(wts[a:b].sum() for a, b in zip((0,) + c, c + (n,))) for c in itertools.combinations(range(1, n), k - 1))
+        assert abs(got - best) < 1e-12
+
+
 def _exchange_worker(rank, world, port, out):
     import torch
     import torch.distributed as dist
