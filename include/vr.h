@@ -60,6 +60,11 @@ const char* vr_status_string(int status);
 int vr_cube_layout(int nx, int ny, int nz, int bx, int by, int bz, size_t* cube_bytes,
                    size_t* meta_bytes);
 
+/* The same for the micro-block layout (VR_OPT_LAYOUT 1, the default) with a stored voxel type (VR_OPT_VOXEL_TYPE:
+ * 0 = float32, 1 = float16, half the bytes) and a window of resident bricks (end_brick < 0: all bricks). */
+int vr_cube_layout_typed(int nx, int ny, int nz, int bx, int by, int bz, int voxel_type, int first_brick, int end_brick,
+                         size_t* cube_bytes, size_t* meta_bytes);
+
 /* Rebrick a linear x-fastest float32 cube (host if src_is_device == 0, else device) into d_cube
  * and compute d_meta.  Host sources are streamed slab by slab (whole planes) through two library
  * staging slabs, the copy of one overlapping the rebricking of the other; the call synchronises `stream`.
@@ -246,7 +251,7 @@ typedef struct {
 /* Synchronises `stream`, then copies the device counters. */
 int vr_get_counters(vr_ctx* ctx, vr_counters* out, void* stream);
 int vr_reset_counters(vr_ctx* ctx, void* stream);
-/* Options.  None of them changes a frame (tests assert it); they exist for A/B measurements.
+/* Options.  None of them but VR_OPT_VOXEL_TYPE changes a frame (tests assert it); they exist for A/B measurements.
  *  VR_OPT_SKIP (default 1): min/max empty-space skipping (O-10) on/off, all levels.
  *  VR_OPT_VARIANT (default -1): the marcher.  0 = one ray per thread, the 32 lanes of a warp take
  *    8 x 4 pixels; for partial images one CTA per pixel tile walks all bricks over the tile (ray
@@ -269,9 +274,16 @@ int vr_reset_counters(vr_ctx* ctx, void* stream);
  *    1 / -1 = on where it applies, 0 = off.
  *  VR_OPT_RING (default -1): where the lockstep marcher keeps the gathers in flight, 0 = a ring of
  *    cp.async slots in shared memory, 1 = registers; -1 = registers iff the central ray runs mostly
- *    along z, the short axis of the 4 x 4 x 2 micro-blocks (layout 1). */
+ *    along z, the short axis of the 4 x 4 x 2 micro-blocks (layout 1).
+ *  VR_OPT_VOXEL_TYPE (default 0): how voxels are stored in HBM (SURVEY.md 8(f)-4 "reduced-precision bricks"; PAPER.md
+ *    line 19: cubes "larger than a single machine memory limit"): 0 = float32; 1 = float16, IEEE half precision,
+ *    each voxel rounded to nearest even when the cube is uploaded / generated and converted back (exactly) when it is
+ *    read, so the renderer computes on the cube Q(v) = float32(float16(v)) with the same float32 arithmetic (DESIGN.md
+ *    O-16): half the bytes per voxel, a 256 GiB-class cube fits one B200.  Needs VR_OPT_LAYOUT 1; read by the next
+ *    upload / generate / attach call; |v| beyond the float16 range (65504) is refused like a non-finite voxel.
+ *    THIS option changes frames (by the quantisation of the cube, nothing else). */
 enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETCH = 4, VR_OPT_LAYOUT = 5, VR_OPT_DENSE = 6,
-       VR_OPT_OCCUPANCY = 7, VR_OPT_RING = 8 };
+       VR_OPT_OCCUPANCY = 7, VR_OPT_RING = 8, VR_OPT_VOXEL_TYPE = 9 };
 int vr_set_option(vr_ctx* ctx, int option, int value);
 /* What a render call of `mode` would launch under the current cube, view and transfer function:
  * out[0] = marcher variant (0 / 3), out[1] = skipping level (0 none, 1 bricks, 2 + macro-cells,

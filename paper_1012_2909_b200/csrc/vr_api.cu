@@ -40,6 +40,7 @@ struct vr_ctx {
     size_t partials_cap = 0;
     int64_t launches = 0;
     int opt_skip = 1, opt_cell_skip = -1, opt_variant = -1, opt_layout = 1, opt_dense = -1, opt_occ = -1, opt_ring = -1;   // -1: chosen per view / TF
+    int opt_vtype = 0;                   // VR_OPT_VOXEL_TYPE: 0 float32, 1 float16
     float x_clear = -INFINITY;
     double active_cell_fraction = 1.0;   // macro-cells active against the current table (EA)
     unsigned long long* d_scratch = nullptr;
@@ -126,7 +127,7 @@ void bind_meta(CubeDesc& c, const void* d_cube, void* d_meta) {
     MetaLayout ml = meta_layout(c);
     char* m = (char*)d_meta;
     const long long lo = c.win_lo;
-    c.cube = (const float*)d_cube - lo * c.stride;
+    c.cube = c.vtype == 1 ? (const float*)((const unsigned short*)d_cube - lo * c.stride) : (const float*)d_cube - lo * c.stride;
     c.brick_mm = (float2*)(m + ml.brick_mm) - lo;
     c.cell_mm = (float2*)(m + ml.cell_mm) - lo * c.cells_per_brick;
     c.cell_bits = (unsigned*)(m + ml.cell_bits) - lo * c.cell_words_per_brick;
@@ -305,6 +306,7 @@ int resolve_dense(const vr_ctx* ctx) {
 // Measured (vr_march.cu, REGS): registers win when the rays run mostly along z, the short axis of the
 // 4 x 4 x 2 micro-blocks, where a request meets the most sectors.
 int resolve_ring(const vr_ctx* ctx) {
+    if (ctx->cube.vtype == 1) return 1;                      // float16 voxels: plain loads only (vr_march_h.cu)
     if (ctx->opt_ring >= 0) return ctx->opt_ring;
     if (ctx->cube.layout != 1) return 0;
     const double* Mi = ctx->Minv;
@@ -412,9 +414,10 @@ namespace vr {
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz, int layout) {
+void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz, int layout, int vtype) {
     std::memset(&c, 0, sizeof(c));
     c.layout = layout;
+    c.vtype = vtype;
     int N[3] = {nx, ny, nz}, B[3] = {bx, by, bz};
     for (int a = 0; a < 3; ++a) {
         c.N[a] = N[a]; c.B[a] = std::min(B[a], N[a]);
@@ -435,7 +438,7 @@ void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz,
                            : 32LL * c.T[0] * c.T[1] * c.T[2];
 }
 
-size_t cube_bytes(const CubeDesc& c) { return (size_t)(c.win_hi - c.win_lo) * (size_t)c.stride * sizeof(float); }
+size_t cube_bytes(const CubeDesc& c) { return (size_t)(c.win_hi - c.win_lo) * (size_t)c.stride * (c.vtype == 1 ? 2 : sizeof(float)); }
 
 MetaLayout meta_layout(const CubeDesc& c) {
     MetaLayout m;
@@ -510,12 +513,26 @@ int vr_cube_layout(int nx, int ny, int nz, int bx, int by, int bz, size_t* cube_
     return VR_OK;
 }
 
+int vr_cube_layout_typed(int nx, int ny, int nz, int bx, int by, int bz, int voxel_type, int first_brick, int end_brick,
+                         size_t* cube_bytes_out, size_t* meta_bytes_out) {
+    if (!valid_dims(nx, ny, nz, bx, by, bz) || !cube_bytes_out || !meta_bytes_out || (voxel_type != 0 && voxel_type != 1)) return VR_ERR_INVALID_ARG;
+    CubeDesc c;
+    fill_cube_desc(c, nx, ny, nz, bx, by, bz, 1, voxel_type);
+    if (end_brick >= 0) {
+        if (first_brick < 0 || end_brick < first_brick || end_brick > c.nbricks) return VR_ERR_INVALID_ARG;
+        c.win_lo = first_brick; c.win_hi = end_brick;
+    }
+    *cube_bytes_out = std::max<size_t>(256, cube_bytes(c));
+    *meta_bytes_out = std::max<size_t>(256, meta_layout(c).total);
+    return VR_OK;
+}
+
 int vr_attach_cube(vr_ctx* ctx, int nx, int ny, int nz, int bx, int by, int bz, const void* d_cube, void* d_meta) {
     VR_RANGE();
     if (!ctx) return VR_ERR_INVALID_ARG;
     enter(ctx);
     if (!valid_dims(nx, ny, nz, bx, by, bz) || !d_cube || !d_meta) return fail(ctx, VR_ERR_INVALID_ARG, "vr_attach_cube: bad argument");
-    fill_cube_desc(ctx->cube, nx, ny, nz, bx, by, bz, ctx->opt_layout);
+    fill_cube_desc(ctx->cube, nx, ny, nz, bx, by, bz, ctx->opt_layout, ctx->opt_vtype);
     apply_window(ctx, ctx->cube);
     bind_meta(ctx->cube, d_cube, d_meta);
     int rc = fetch_brick_mm(ctx, nullptr);
@@ -534,7 +551,7 @@ int vr_upload_cube(vr_ctx* ctx, const float* src, int src_is_device, int nx, int
     cudaStream_t s = (cudaStream_t)stream;
     ctx->has_cube = false;
     CubeDesc& c = ctx->cube;
-    fill_cube_desc(c, nx, ny, nz, bx, by, bz, ctx->opt_layout);
+    fill_cube_desc(c, nx, ny, nz, bx, by, bz, ctx->opt_layout, ctx->opt_vtype);
     apply_window(ctx, c);
     bind_meta(c, d_cube, d_meta);
     VR_CUDA(ctx, cudaMemsetAsync(d_cube, 0, cube_bytes(c), s));
@@ -596,7 +613,7 @@ int vr_generate_cube(vr_ctx* ctx, const vr_gen_params* prm, uint64_t seed, int n
     cudaStream_t s = (cudaStream_t)stream;
     ctx->has_cube = false;
     CubeDesc& c = ctx->cube;
-    fill_cube_desc(c, nx, ny, nz, bx, by, bz, ctx->opt_layout);
+    fill_cube_desc(c, nx, ny, nz, bx, by, bz, ctx->opt_layout, ctx->opt_vtype);
     apply_window(ctx, c);
     bind_meta(c, d_cube, d_meta);
     // bin the sources (ascending id) and the zero boxes over 32^3 tiles of the cube
@@ -1091,12 +1108,18 @@ int vr_set_option(vr_ctx* ctx, int option, int value) {
     if (option == VR_OPT_CELL_SKIP) { ctx->opt_cell_skip = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_LAYOUT) {
         if (value != 0 && value != 1) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: layout must be 0 (rows) or 1 (4x4x2 blocks)");
+        if (value == 0 && ctx->opt_vtype == 1) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: float16 voxels need the micro-block layout");
         ctx->opt_layout = value; return VR_OK;                  // takes effect at the next upload / generate / attach
     }
     if (option == VR_OPT_L2_FETCH) {
         if (value != 32 && value != 64 && value != 128) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: L2 fetch granularity must be 32, 64 or 128");
         VR_CUDA(ctx, cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)value));
         return VR_OK;
+    }
+    if (option == VR_OPT_VOXEL_TYPE) {
+        if (value != 0 && value != 1) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: voxel type must be 0 (float32) or 1 (float16)");
+        if (value == 1 && ctx->opt_layout != 1) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: float16 voxels need the micro-block layout (VR_OPT_LAYOUT 1)");
+        ctx->opt_vtype = value; return VR_OK;                   // takes effect at the next upload / generate / attach
     }
     if (option == VR_OPT_RING) { ctx->opt_ring = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_OCCUPANCY) { ctx->opt_occ = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }

@@ -1,6 +1,8 @@
 // S0 "cube residency" kernels (BASELINE.json north_star (2) "brick-major voxel
 // layout, per-brick min/max" and (4) "a device-side generator for the synthetic cubes"):
 // rebrick a linear cube, generate the synthetic cube in place, per-cell / per-brick min-max.
+#include <cuda_fp16.h>
+
 #include "vr_internal.cuh"
 
 namespace vr {
@@ -8,6 +10,16 @@ namespace vr {
 namespace {
 
 struct Elem { int b[3]; int l[3]; int g[3]; bool stored; bool in_cube; };
+
+// Stored voxel i of the brick-major cube: float32, or float16 rounded to nearest even (CubeDesc::vtype).
+__device__ __forceinline__ float put_voxel(const CubeDesc& c, void* cube, long long i, float v) {
+    if (c.vtype == 1) { const __half h = __float2half_rn(v); reinterpret_cast<__half*>(cube)[i] = h; return __half2float(h); }
+    reinterpret_cast<float*>(cube)[i] = v;
+    return v;
+}
+__device__ __forceinline__ float get_voxel(const CubeDesc& c, long long i) {
+    return c.vtype == 1 ? __half2float(__ldg(reinterpret_cast<const __half*>(c.cube) + i)) : __ldg(c.cube + i);
+}
 
 // Decompose a storage slot (brick, offset inside the brick) of the brick-major cube.
 __device__ __forceinline__ Elem decode(const CubeDesc& c, long long brick, long long rem) {
@@ -49,7 +61,8 @@ __global__ void rebrick_kernel(CubeDesc c, float* __restrict__ cube, const float
         const long long r2 = e / c.N[0];
         const int g[3] = {x, (int)(r2 % c.N[1]), z0 + (int)(r2 / c.N[1])};
         const float v = src[e];
-        if (!isfinite(v)) atomicAdd(n_bad, 1ULL);         // NaN / inf voxels are refused by vr_upload_cube (rare path)
+        // NaN / inf voxels (also: beyond the float16 range when stored as such) are refused by vr_upload_cube (rare path)
+        if (!isfinite(v) || (c.vtype == 1 && !isfinite(__half2float(__float2half_rn(v))))) atomicAdd(n_bad, 1ULL);
         int b[3], l[3], nalt[3];
         for (int a = 0; a < 3; ++a) {
             b[a] = c.sh[a] >= 0 ? (g[a] >> c.sh[a]) : (g[a] / c.B[a]);
@@ -62,18 +75,18 @@ __global__ void rebrick_kernel(CubeDesc c, float* __restrict__ cube, const float
                     const int bx = b[0] - hx, by = b[1] - hy, bz = b[2] - hz;
                     const long long brick = bx + (long long)c.G[0] * (by + (long long)c.G[1] * bz);
                     if (brick < c.win_lo || brick >= c.win_hi) continue;
-                    cube[brick * c.stride + voxel_slot(c, hx ? c.B[0] : l[0], hy ? c.B[1] : l[1], hz ? c.B[2] : l[2])] = v;
+                    put_voxel(c, cube, brick * c.stride + voxel_slot(c, hx ? c.B[0] : l[0], hy ? c.B[1] : l[1], hz ? c.B[2] : l[2]), v);
                 }
     }
 }
 
 __global__ void unbrick_kernel(CubeDesc c, int brick, float* __restrict__ dst, int ex, int ey, int ez) {
     long long n = (long long)ex * ey * ez;
-    const float* B = c.cube + (long long)brick * c.stride;
+    const long long B0 = (long long)brick * c.stride;
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n;
          e += (long long)gridDim.x * blockDim.x) {
         int x = (int)(e % ex), y = (int)((e / ex) % ey), z = (int)(e / ((long long)ex * ey));
-        dst[e] = B[voxel_slot(c, x, y, z)];
+        dst[e] = get_voxel(c, B0 + voxel_slot(c, x, y, z));
     }
 }
 
@@ -178,7 +191,7 @@ __global__ void generate_kernel(CubeDesc c, float* __restrict__ cube, GenDev g, 
                 out = (float)v;
             }
         }
-        if (el.stored) cube[brick * c.stride + rem] = out;
+        if (el.stored) put_voxel(c, cube, brick * c.stride + rem, out);
     }
 }
 

@@ -30,6 +30,7 @@ struct CubeDesc {
     int G[3];        // brick grid
     int P[3];        // stored brick extents: B + 1 (layout 0: P0 rounded up to a multiple of 4)
     int layout;      // 0: rows, 1: 4x4x2 micro-blocks
+    int vtype;       // stored voxel type: 0 float32, 1 float16 (IEEE half, layout 1 only); `stride` counts voxels
     int T[3];        // layout 1: micro-blocks per axis = ceil(P0/4), ceil(P1/4), ceil(P2/2)
     int sh[3];       // log2(B) if B is a power of two, else -1
     int C[3];        // macro-cells per brick axis = ceil(B / kCell)
@@ -37,7 +38,7 @@ struct CubeDesc {
     int win_lo, win_hi;          // resident bricks [win_lo, win_hi) (all by default); the pointers below are
                                  // shifted so that GLOBAL brick ids index them (vr_set_brick_window)
     int cells_per_brick;
-    long long stride;            // floats per brick (multiple of 32)
+    long long stride;            // voxels per brick (multiple of 32)
     const float* cube;
     float2* brick_mm;            // (min,max) per brick, halo-inclusive
     float2* cell_mm;             // (min,max) per macro-cell, halo-inclusive, brick-major
@@ -84,7 +85,7 @@ __host__ __device__ inline long long voxel_slot(const CubeDesc& c, int lx, int l
 }
 
 size_t align_up(size_t v, size_t a);
-void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz, int layout);
+void fill_cube_desc(CubeDesc& c, int nx, int ny, int nz, int bx, int by, int bz, int layout, int vtype = 0);
 size_t cube_bytes(const CubeDesc& c);
 struct MetaLayout { size_t brick_mm, cell_mm, cell_bits, brick_active, occ, hot, total; };
 MetaLayout meta_layout(const CubeDesc& c);

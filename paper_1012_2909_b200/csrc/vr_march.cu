@@ -1,848 +1,20 @@
-// The ray marcher (BASELINE.json north_star (2)): per-pixel rays through the
-// brick-major cube, fixed step, trilinear interpolation, MIP or front-to-back emission-absorption
-// through the 256-entry transfer function with early ray termination, min/max brick skipping.
-//
-// Arithmetic contract (readings O-2...O-7, O-11): the
-// ray is set up in fp64 and rounded once to float32; every per-sample operation is an explicit
-// IEEE float32 + - * fma floor min max compare (no fast-math, built with --fmad=false), so frames
-// agree with the float32 instantiation of the oracle to the bit and with its fp64 instantiation
-// within BASELINE.json's tolerances.
-#include "vr_sample.cuh"
+// The float32-voxel instantiation of the ray marchers (vr_march.cuh) and the entry points the C ABI calls.
+#include "vr_march.cuh"
 
 namespace vr {
 
-namespace {
-
-// ================================================================== variant 0: one ray per thread
-// March the lattice samples k .. ke (all of them members of brick `bid`, O-3) into `acc`.  With
-// A.skip >= 2 the interval is cut into runs inside 8^3 macro-cells and idle runs are jumped.
-// Returns true if early ray termination fired.
-template <int MODE, int LAYOUT, bool JUMP = false>
-__device__ __forceinline__ bool march_interval(const CubeDesc& c, const Ray& r, const TFDesc& T, const RenderArgs& A,
-                                               const float4* tab, int bid, const int lo[3], int k, int ke,
-                                               Accum& acc, Stats& st) {
-    const BrickRef b = brick_ref<LAYOUT>(c, bid, lo);
-    const unsigned* occ = (MODE == VR_MODE_EA && LAYOUT == 1 && A.skip >= 3) ? c.occ + (long long)bid * c.occ_words_per_brick : nullptr;
-    const int S8[3] = {kCell, kCell, kCell};
-    // a jump out of an idle micro-block costs about as much as testing 3 samples one by one: worth it when
-    // the block holds more than that (measured: step 0.25 -> C4 29.6 to 26.2 ms; step 0.5 -> C2 0.70 to 0.76 ms),
-    // and a separate instantiation, because the extra path costs the other one registers
-    const bool block_jumps = JUMP && occ != nullptr;        // JUMP kernels are launched for steps < kJumpStep only
-    float kf = (float)k;                                    // exact: k < 2^24
-    while (k <= ke) {
-        int n = ke - k + 1;
-        if (A.skip >= 2) {
-            // A loop of its own over the idle runs: the lanes of a warp meet again behind it, each at the start
-            // of an ACTIVE run (or at the end of its interval), and take the samples below together.  In one
-            // loop with the samples, a lane in an idle run would wait for the lanes sampling, then sample alone.
-            for (;;) {
-                float p[3], fl;
-                position(r, kf, p);
-                const int iv[3] = {floor_pos(p[0], fl), floor_pos(p[1], fl), floor_pos(p[2], fl)};
-                const int clo[3] = {lo[0] + (((iv[0] - lo[0]) >> 3) << 3), lo[1] + (((iv[1] - lo[1]) >> 3) << 3),
-                                    lo[2] + (((iv[2] - lo[2]) >> 3) << 3)};
-                n = min(ke - k + 1, run_length(r, p, clo, S8));
-                if (!cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], acc.m)) break;
-                k += n; kf = __fadd_rn(kf, (float)n); ++st.skip;
-                if (k > ke) { n = 0; break; }
-            }
-            if (n == 0) break;
-        }
-        ++st.visit;
-        if (JUMP && block_jumps) {
-            // small steps: inside an active macro-cell the ray leaves every idle 4 x 4 x 2 block of cells (occupancy
-            // word == 0) in one jump instead of testing its samples one by one
-            for (const int e = k + n; k < e;) {
-                float p[3], fl;
-                position(r, kf, p);
-                const unsigned lx = (unsigned)(floor_pos(p[0], fl) - lo[0]), ly = (unsigned)(floor_pos(p[1], fl) - lo[1]),
-                               lz = (unsigned)(floor_pos(p[2], fl) - lo[2]);
-                const unsigned word = __ldg(occ + occ_word_index(c, lx, ly, lz));
-                if (word == 0u) {
-                    const int blo[3] = {lo[0] + (int)(lx & ~3u), lo[1] + (int)(ly & ~3u), lo[2] + (int)(lz & ~1u)};
-                    const int S4[3] = {4, 4, 2};
-                    const int m = min(run_length(r, p, blo, S4), e - k);
-                    k += m; kf = __fadd_rn(kf, (float)m);
-                    continue;
-                }
-                if ((word >> occ_bit_index(lx, ly, lz)) & 1u) {
-                    const float v = sample<LAYOUT>(b, p);
-                    ++st.taken;
-                    if (fold<MODE>(acc, v, tab, T, A.tau)) return true;
-                }
-                ++k; kf = __fadd_rn(kf, 1.f);
-            }
-            continue;
-        }
-        for (const int e = k + n; k < e; ++k, kf = __fadd_rn(kf, 1.f)) {
-            float p[3];
-            position(r, kf, p);
-            if (occ) {                                      // O-10 per trilinear cell: the sample's occupancy bit
-                float fl;
-                const unsigned lx = (unsigned)(floor_pos(p[0], fl) - lo[0]), ly = (unsigned)(floor_pos(p[1], fl) - lo[1]),
-                               lz = (unsigned)(floor_pos(p[2], fl) - lo[2]);
-                if (((__ldg(occ + occ_word_index(c, lx, ly, lz)) >> occ_bit_index(lx, ly, lz)) & 1u) == 0u) continue;
-            }
-            const float v = sample<LAYOUT>(b, p);
-            ++st.taken;
-            if (fold<MODE>(acc, v, tab, T, A.tau)) return true;
-        }
-    }
-    return false;
-}
-
-__device__ __forceinline__ float4 raw_tf_at(const TFDesc& T, float m) {
-    float x = __fmul_rn(__fsub_rn(m, T.vmin), T.scale);
-    return tf_at(T.raw, x);
-}
-
-template <int MODE>
-__device__ __forceinline__ void write_frame_pixel(const ViewDesc& V, const TFDesc& T, const RenderArgs& A, int i, int j,
-                                                  const Accum& acc, bool any) {
-    const long long px = (long long)(V.vy0 + j) * V.pitch + (V.vx0 + i);
-    if (MODE == VR_MODE_MIP) {
-        A.out[px] = any ? acc.m : A.miss;
-        if (A.out_rgba)
-            reinterpret_cast<float4*>(A.out_rgba)[px] = any ? raw_tf_at(T, acc.m) : make_float4(0.f, 0.f, 0.f, 0.f);
-    } else {                                               // O-7: premultiplied colour over bg
-        const float t = __fsub_rn(1.f, acc.A);
-        reinterpret_cast<float4*>(A.out)[px] = make_float4(__fmaf_rn(t, A.bg[0], acc.C[0]), __fmaf_rn(t, A.bg[1], acc.C[1]),
-                                                           __fmaf_rn(t, A.bg[2], acc.C[2]), __fmaf_rn(t, A.bg[3], acc.A));
-    }
-}
-
-// ---------------------------------------------------------------- whole frame, O-8 GLOBAL
-template <int MODE, int LAYOUT, bool JUMP = false>
-__global__ void __launch_bounds__(kThreads)
-render_global_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
-                     const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A) {
-    __shared__ float4 tab[256];
-    if (MODE == VR_MODE_EA) load_tf(tab, T.baked);
-    int tx, ty; tile_pixel(tx, ty);
-    const int i = blockIdx.x * kTileW + tx, j = blockIdx.y * kTileH + ty;
-    const bool live = i < V.W && j < V.H;
-    Ray r; r.k0 = 0; r.k1 = -1;
-    if (live) setup_ray(V, c, i, j, r);
-    Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-    Stats st = {0, 0, 0};
-    bool stopped = false;
-    int k = r.k0;
-    while (k <= r.k1) {
-        float p[3];
-        position(r, (float)k, p);
-        float fl;
-        int iv[3] = {floor_pos(p[0], fl), floor_pos(p[1], fl), floor_pos(p[2], fl)};
-        int b[3]; brick_of(c, iv, b);
-        int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
-        int n = min(run_length(r, p, lo, c.B), r.k1 - k + 1);
-        const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
-        bool skip = false;
-        if (A.skip) {
-            if (MODE == VR_MODE_MIP) skip = c.brick_mm[bid].y <= acc.m;       // O-10 (exact)
-            else skip = c.brick_active[bid] == 0;
-        }
-        if (skip) { k += n; ++st.skip; continue; }
-        if (march_interval<MODE, LAYOUT, JUMP>(c, r, T, A, tab, bid, lo, k, k + n - 1, acc, st)) { stopped = true; break; }
-        k += n;
-    }
-    if (live) write_frame_pixel<MODE>(V, T, A, i, j, acc, r.k1 >= r.k0);
-    if (A.counters) {
-        const unsigned long long nom = r.k1 >= r.k0 ? (unsigned long long)(r.k1 - r.k0 + 1) : 0ULL;
-        count(A.counters, kRays, nom ? 1 : 0);
-        count(A.counters, kNominal, nom);
-        count(A.counters, kTaken, st.taken);
-        count(A.counters, kVisited, st.visit);
-        count(A.counters, kSkipped, st.skip);
-        count(A.counters, kTerminated, stopped ? 1 : 0);
-    }
-}
-
-// ---------------------------------------------------------------- per-brick partial images (O-8 SORT-LAST)
-template <int MODE, int LAYOUT>
-__global__ void __launch_bounds__(kThreads)
-render_bricks_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
-                     const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
-                     const PartialDev* __restrict__ parts, int n_parts) {
-    __shared__ float4 tab[256];
-    __shared__ PartialDev part;
-    int lx, ly;
-    const bool live = locate_tile(parts, n_parts, part, lx, ly);
-    if (MODE == VR_MODE_EA) load_tf(tab, T.baked);
-    Ray r; r.k0 = 0; r.k1 = -1;
-    if (live) setup_ray(V, c, part.x0 + lx, part.y0 + ly, r);
-    const int bid = part.brick;
-    const int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
-    const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
-    int ka = r.k0, kb = r.k1;
-    brick_interval(c, r, b, lo, ka, kb);
-    Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-    Stats st = {0, 0, 0};
-    const bool stopped = march_interval<MODE, LAYOUT>(c, r, T, A, tab, bid, lo, ka, kb, acc, st);
-    if (live) {
-        const long long px = (long long)ly * part.pitch + lx;
-        if (MODE == VR_MODE_MIP) reinterpret_cast<float*>(part.data)[px] = acc.m;
-        else reinterpret_cast<float4*>(part.data)[px] = make_float4(acc.C[0], acc.C[1], acc.C[2], acc.A);
-    }
-    if (A.counters) {
-        count(A.counters, kNominal, kb >= ka ? (unsigned long long)(kb - ka + 1) : 0ULL);
-        count(A.counters, kTaken, st.taken);
-        count(A.counters, kVisited, st.visit);
-        count(A.counters, kSkipped, st.skip);
-        count(A.counters, kTerminated, stopped ? 1 : 0);
-    }
-}
-
-// The same partial images, one CTA per PIXEL TILE of the view instead of one per (brick, tile): the
-// ray of a pixel is set up once (fp64) and reused for every brick whose screen rectangle holds
-// the pixel (dense rays cross 10-30 bricks: on C4 the per-brick set-up was a fifth of all
-// instructions).  The CTA culls the partial rectangles against its tile into a shared bitmask
-// (as composite_kernel does) and takes the hits one after the other.
-constexpr int kCullChunk = 2048;
-
-template <int MODE, int LAYOUT, bool JUMP>
-__global__ void __launch_bounds__(kThreads)
-render_tiles_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
-                    const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
-                    const PartialDev* __restrict__ parts, int n_parts) {
-    __shared__ float4 tab[256];
-    __shared__ unsigned mask[kCullChunk / 32];
-    if (MODE == VR_MODE_EA) load_tf(tab, T.baked);
-    int tx, ty; tile_pixel(tx, ty);
-    const int x0 = blockIdx.x * kTileW, y0 = blockIdx.y * kTileH;
-    const int i = x0 + tx, j = y0 + ty;
-    const bool live = i < V.W && j < V.H;
-    Ray r; r.k0 = 0; r.k1 = -1;
-    r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
-    r.inv[0] = r.inv[1] = r.inv[2] = 0.f;
-    if (live) setup_ray(V, c, i, j, r);
-    Stats st = {0, 0, 0};
-    unsigned long long nominal = 0, n_stopped = 0;
-    for (int base = 0; base < n_parts; base += kCullChunk) {
-        const int cnt = min(kCullChunk, n_parts - base);
-        __syncthreads();
-        if (threadIdx.x < kCullChunk / 32) mask[threadIdx.x] = 0u;
-        __syncthreads();
-        for (int q = threadIdx.x; q < cnt; q += kThreads) {
-            const PartialDev& P = parts[base + q];
-            if (P.x0 < x0 + kTileW && P.x0 + P.w > x0 && P.y0 < y0 + kTileH && P.y0 + P.h > y0) atomicOr(&mask[q >> 5], 1u << (q & 31));
-        }
-        __syncthreads();
-        for (int w = 0; w < (cnt + 31) / 32; ++w) {
-            for (unsigned bits = mask[w]; bits; bits &= bits - 1) {
-                const PartialDev& P = parts[base + 32 * w + __ffs(bits) - 1];
-                const int lx = i - P.x0, ly = j - P.y0;
-                const bool mine = live && lx >= 0 && ly >= 0 && lx < P.w && ly < P.h;
-                const int bid = P.brick;
-                const int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
-                const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
-                int ka = mine ? r.k0 : 0, kb = mine ? r.k1 : -1;
-                brick_interval(c, r, b, lo, ka, kb);
-                Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-                const bool stopped = march_interval<MODE, LAYOUT, JUMP>(c, r, T, A, tab, bid, lo, ka, kb, acc, st);
-                if (mine) {
-                    const long long px = (long long)ly * P.pitch + lx;
-                    if (MODE == VR_MODE_MIP) reinterpret_cast<float*>(P.data)[px] = acc.m;
-                    else reinterpret_cast<float4*>(P.data)[px] = make_float4(acc.C[0], acc.C[1], acc.C[2], acc.A);
-                }
-                if (kb >= ka) nominal += (unsigned long long)(kb - ka + 1);
-                if (stopped) ++n_stopped;
-            }
-        }
-    }
-    if (A.counters) {
-        count(A.counters, kNominal, nominal);
-        count(A.counters, kTaken, st.taken);
-        count(A.counters, kVisited, st.visit);
-        count(A.counters, kSkipped, st.skip);
-        count(A.counters, kTerminated, n_stopped);
-    }
-}
-
-// ================================================================== variant 3: lockstep
-// A warp owns the 32 rays of its 8 x 4 pixel tile and walks them TOGETHER through chunks of 32
-// lattice indices [kbase, kbase + 31] (k counts from the near plane, so a chunk is a thin shell
-// that all 32 rays cross at about the same place: lines shared by neighbouring rays are fetched
-// once and hit in L1 / L2, not re-read from HBM).  Inside a chunk the rays are taken one after the
-// other, SAMPLE-PARALLEL: the 32 lanes take the 32 samples of that ray in the chunk (positions,
-// O-3; gathers and trilinear interpolation, O-4), so the lanes' addresses follow the ray.
-//
-// The gathers are asynchronous copies (cp.async, 4 bytes each) into a per-lane ring of kDepth
-// slots in shared memory: the 8 voxels of the ray taken kDepth - 1 steps later are requested
-// before the current ones are interpolated, they occupy no register and stall no scoreboard.
-//
-// The values are then folded in ray order (O-5 / O-7) by the lane that owns the ray, whose
-// accumulator never leaves it, so early ray termination (O-7) is exact per ray:
-//   MIP        - max is exact in any order: a warp reduction, then lane r takes the maximum;
-//   EA, SPARSE - the few samples whose table coordinate is not below x_clear (see fold) are
-//                handed to lane r one by one with a shuffle, in lattice order;
-//   EA, DENSE  - the values go to shared memory, vals[ray][sample], and after the last ray of
-//                the chunk every lane folds the 32 values of ITS ray front to back (all 32 rays
-//                in parallel), so opaque transfer functions cost the same as sparse ones.
-// Skipped samples (O-10) are never interpolated or folded.  All three give identical frames.
-//
-// REGS: the same ring in REGISTERS (plain loads, 3 rays ahead, 5 CTAs per SM).  The shared-memory side
-// of a 4-byte cp.async takes one L1 wavefront per arriving sector; rays that run along z (the short
-// axis of the 4 x 4 x 2 micro-blocks) meet the most sectors per request and are faster with plain
-// loads (MIP on C3: 17.3 -> 14.7 ms), rays along x or y with cp.async (12.7 vs 14.1 ms): RenderArgs::ring.
-constexpr int kValPitch = 33;
-constexpr int kDepth = 3;               // rays in flight per warp (measured: 2 -> 12.1, 3 -> 12.0, 4 -> 13.5 ms on C3)
-constexpr int kBitsWords = 1024;        // shared copy of one brick's macro-cell bits (256^3 bricks: 32^3 cells)
-
-__device__ __forceinline__ void cp_async4(unsigned dst, const float* src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-// Request the 8 voxels of gather8 into dst[e * 32] (floats, e = 0..7; dst is a shared address in bytes).
-template <int LAYOUT>
-__device__ __forceinline__ void gather8_async(const BrickRef& b, int ix, int iy, int iz, unsigned dst) {
-    unsigned q, dx, dy, dz;
-    cell_address<LAYOUT>(b, (unsigned)(ix - b.lo[0]), (unsigned)(iy - b.lo[1]), (unsigned)(iz - b.lo[2]), q, dx, dy, dz);
-    const float* p = b.base + q;
-    cp_async4(dst, p);             cp_async4(dst + 128, p + dx);
-    cp_async4(dst + 256, p + dy);  cp_async4(dst + 384, p + dy + dx);
-    cp_async4(dst + 512, p + dz);  cp_async4(dst + 640, p + dz + dx);
-    cp_async4(dst + 768, p + dz + dy); cp_async4(dst + 896, p + dz + dy + dx);
-}
-
-struct Slot { float w[3]; int rc; bool idle; float v[8]; };   // one ray in flight: weights of this lane's sample (v: register ring only)
-
-// 7 CTAs per SM: 72 registers; an 8th CTA (64 registers) would shrink L1 to 28 KB and costs 10 % (measured)
-template <int MODE, int LAYOUT, bool GLOBAL, bool DENSE, bool REGS>
-__global__ void __launch_bounds__(kThreads, REGS ? 5 : 7)
-render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
-                 const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
-                 const PartialDev* __restrict__ parts, int n_parts) {
-    constexpr bool EA = MODE == VR_MODE_EA;
-    constexpr bool VALS = EA && DENSE;
-    constexpr bool SBITS = EA && !GLOBAL;
-    constexpr int kWarps = kThreads / 32;
-    __shared__ float4 tab[EA ? 256 : 1];
-    __shared__ PartialDev part;
-    __shared__ float4 rays_all[kWarps][64];
-    __shared__ float stage_all[REGS ? 1 : kWarps][REGS ? 1 : kDepth * 256];
-    __shared__ float vals_all[VALS ? kWarps : 1][VALS ? 32 * kValPitch : 1];
-    __shared__ unsigned sbits[SBITS ? kBitsWords : 1];
-    int fx, fy;                                             // view pixel of this thread's ray
-    bool live;
-    if (GLOBAL) {
-        int tx, ty; tile_pixel(tx, ty);
-        fx = blockIdx.x * kTileW + tx; fy = blockIdx.y * kTileH + ty;
-        live = fx < V.W && fy < V.H;
-    } else {
-        int lx, ly;
-        live = locate_tile(parts, n_parts, part, lx, ly);
-        fx = lx; fy = ly;
-    }
-    const bool cells = A.skip >= 2;
-    int bid0 = 0, lo0[3] = {0, 0, 0};
-    if (!GLOBAL) {
-        bid0 = part.brick;
-        lo0[0] = (bid0 % c.G[0]) * c.B[0]; lo0[1] = ((bid0 / c.G[0]) % c.G[1]) * c.B[1]; lo0[2] = (bid0 / (c.G[0] * c.G[1])) * c.B[2];
-    }
-    const bool bits_shared = SBITS && cells && c.cell_words_per_brick <= kBitsWords;
-    if (bits_shared)
-        for (int i = threadIdx.x; i < c.cell_words_per_brick; i += kThreads)
-            sbits[i] = __ldg(&c.cell_bits[(long long)bid0 * c.cell_words_per_brick + i]);
-    if (EA) load_tf(tab, T.baked);                          // ends with __syncthreads()
-    Ray r; r.k0 = 0; r.k1 = -1;
-    r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
-    if (live) setup_ray(V, c, GLOBAL ? fx : part.x0 + fx, GLOBAL ? fy : part.y0 + fy, r);
-    int ka = r.k0, kb = r.k1;
-    if (!GLOBAL) {
-        const int b[3] = {bid0 % c.G[0], (bid0 / c.G[0]) % c.G[1], bid0 / (c.G[0] * c.G[1])};
-        brick_interval(c, r, b, lo0, ka, kb);
-    }
-    const BrickRef br0 = brick_ref<LAYOUT>(c, bid0, lo0);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float* vals = vals_all[VALS ? warp : 0];
-    float4* rays = rays_all[warp];
-    const float* stage = stage_all[REGS ? 0 : warp] + (REGS ? 0 : lane);
-    const unsigned stage_addr = (unsigned)__cvta_generic_to_shared(stage);
-    rays[2 * lane] = make_float4(r.o[0], r.o[1], r.o[2], r.d[0]);
-    rays[2 * lane + 1] = make_float4(r.d[1], r.d[2], __int_as_float(ka), __int_as_float(kb));
-    __syncwarp();
-    bool alive = ka <= kb, stopped = false;
-    int k_end = kb;                                         // last lattice index this ray got to (ERT: the stop)
-    int K0 = alive ? ka : 0x7fffffff, K1 = alive ? kb : -1;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        K0 = min(K0, __shfl_xor_sync(0xffffffffu, K0, o));
-        K1 = max(K1, __shfl_xor_sync(0xffffffffu, K1, o));
-    }
-    Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-    unsigned n_taken = 0;
-    for (int kbase = K0; kbase <= K1; kbase += 32) {
-        if (!__ballot_sync(0xffffffffu, alive)) break;
-        const unsigned act = __ballot_sync(0xffffffffu, alive && ka <= kbase + 31 && kb >= kbase);
-        if (!act) continue;
-        const int k = kbase + lane;                         // this lane's sample of every ray of the chunk
-        const float t = __fmul_rn((float)k, r.step);        // O-3: t_k = k * Delta
-        unsigned rest = act;
-        // request the 8 voxels of this lane's sample of the next ray of the chunk (if any) into slot s
-        auto issue = [&](Slot& S, const int s) {
-            S.rc = -1; S.idle = true;
-            S.w[0] = S.w[1] = S.w[2] = 0.f;
-            if (REGS) {
-#pragma unroll
-                for (int e = 0; e < 8; ++e) S.v[e] = 0.f;
-            }
-            if (rest) {
-                const int rr = __ffs(rest) - 1;
-                rest &= rest - 1;
-                S.rc = rr;
-                const float4 ra = rays[2 * rr], rb = rays[2 * rr + 1];
-                float m_r = -INFINITY;
-                if (!EA) m_r = __shfl_sync(0xffffffffu, acc.m, rr);
-                if (k >= __float_as_int(rb.z) && k <= __float_as_int(rb.w)) {
-                    float p[3], fl[3];
-                    p[0] = __fmaf_rn(t, ra.w, ra.x); p[1] = __fmaf_rn(t, rb.x, ra.y); p[2] = __fmaf_rn(t, rb.y, ra.z);
-                    const int iv[3] = {floor_pos(p[0], fl[0]), floor_pos(p[1], fl[1]), floor_pos(p[2], fl[2])};
-                    S.w[0] = __fsub_rn(p[0], fl[0]); S.w[1] = __fsub_rn(p[1], fl[1]); S.w[2] = __fsub_rn(p[2], fl[2]);
-                    if (GLOBAL) {
-                        int b[3]; brick_of(c, iv, b);
-                        const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
-                        const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
-                        bool idle = false;
-                        if (A.skip) {                       // O-10 (exact), per sample
-                            if (!EA) idle = __ldg(&c.brick_mm[bid]).y <= m_r;
-                            else idle = __ldg(&c.brick_active[bid]) == 0;
-                            if (cells && !idle) idle = cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], m_r);
-                        }
-                        S.idle = idle;
-                        if (!idle) {
-                            if (REGS) gather8<LAYOUT>(brick_ref<LAYOUT>(c, bid, lo), iv[0], iv[1], iv[2], S.v);
-                            else gather8_async<LAYOUT>(brick_ref<LAYOUT>(c, bid, lo), iv[0], iv[1], iv[2], stage_addr + 1024u * s);
-                        }
-                    } else {
-                        bool idle = false;
-                        if (bits_shared) {
-                            const int cidx = ((iv[0] - lo0[0]) >> 3) + c.C[0] * (((iv[1] - lo0[1]) >> 3) + c.C[1] * ((iv[2] - lo0[2]) >> 3));
-                            idle = ((sbits[cidx >> 5] >> (cidx & 31)) & 1u) == 0u;
-                        } else if (cells) idle = cell_idle<MODE>(c, bid0, lo0, iv[0], iv[1], iv[2], m_r);
-                        S.idle = idle;
-                        if (!idle) {
-                            if (REGS) gather8<LAYOUT>(br0, iv[0], iv[1], iv[2], S.v);
-                            else gather8_async<LAYOUT>(br0, iv[0], iv[1], iv[2], stage_addr + 1024u * s);
-                        }
-                    }
-                }
-            }
-            cp_async_commit();
-        };
-        unsigned my_fold = 0u, my_done = 0u;                // DENSE: this lane's ray: samples to fold / interpolated
-        // interpolate the samples of the ray in slot s (its copies have landed) and fold them
-        auto consume = [&](const Slot& S, const int s) {
-            float v[8];
-            if (REGS) {
-#pragma unroll
-                for (int e = 0; e < 8; ++e) v[e] = S.v[e];
-            } else {
-                const float* st = stage + 256 * s;
-#pragma unroll
-                for (int e = 0; e < 8; ++e) v[e] = st[32 * e];
-            }
-            const float val = trilinear(v, S.w[0], S.w[1], S.w[2]);       // idle lanes: stale values, never used
-            const unsigned done_bits = __ballot_sync(0xffffffffu, !S.idle);
-            if (!EA) {
-                float m = S.idle ? -INFINITY : val;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-                if (lane == S.rc) { acc.m = fmaxf(acc.m, m); n_taken += __popc(done_bits); }
-                return;
-            }
-            // samples whose table coordinate lies below x_clear have weight exactly zero (see fold)
-            const bool need = !S.idle && !(__fmul_rn(__fsub_rn(val, T.vmin), T.scale) < T.x_clear);
-            const unsigned fold_bits = __ballot_sync(0xffffffffu, need);
-            if (VALS) {
-                vals[S.rc * kValPitch + lane] = val;
-                if (lane == S.rc) { my_fold = fold_bits; my_done = done_bits; }
-                return;
-            }
-            unsigned upto = 0xffffffffu;
-            for (unsigned bits = fold_bits; bits; bits &= bits - 1) {
-                const int l = __ffs(bits) - 1;
-                const float vl = __shfl_sync(0xffffffffu, val, l);
-                if (lane == S.rc && alive && fold<MODE>(acc, vl, tab, T, A.tau)) {
-                    stopped = true; alive = false; k_end = kbase + l;
-                    upto = l >= 31 ? 0xffffffffu : ((1u << (l + 1)) - 1u);
-                }
-            }
-            if (lane == S.rc) n_taken += __popc(done_bits & upto);
-        };
-        Slot slot[kDepth];
-#pragma unroll
-        for (int s = 0; s < kDepth - 1; ++s) issue(slot[s], s);
-        for (bool more = true; more;) {
-#pragma unroll
-            for (int u = 0; u < kDepth; ++u) {
-                issue(slot[(u + kDepth - 1) % kDepth], (u + kDepth - 1) % kDepth);
-                cp_async_wait<kDepth - 1>();
-                if (slot[u].rc < 0) { more = false; break; }
-                consume(slot[u], u);
-            }
-        }
-        if (VALS) {
-            __syncwarp();
-            // lane = ray: fold its flagged values front to back
-            if ((act >> lane) & 1u) {
-                const float* mine = vals + lane * kValPitch;
-                unsigned upto = 0xffffffffu;
-                for (unsigned bits = my_fold; bits; bits &= bits - 1) {
-                    const int l = __ffs(bits) - 1;
-                    if (fold<MODE>(acc, mine[l], tab, T, A.tau)) {
-                        stopped = true; alive = false; k_end = kbase + l;
-                        upto = l >= 31 ? 0xffffffffu : ((1u << (l + 1)) - 1u);
-                        break;
-                    }
-                }
-                n_taken += __popc(my_done & upto);
-            }
-            __syncwarp();
-        }
-    }
-    if (live) {
-        if (GLOBAL) write_frame_pixel<MODE>(V, T, A, fx, fy, acc, r.k1 >= r.k0);
-        else {
-            const long long px = (long long)fy * part.pitch + fx;
-            if (!EA) reinterpret_cast<float*>(part.data)[px] = acc.m;
-            else reinterpret_cast<float4*>(part.data)[px] = make_float4(acc.C[0], acc.C[1], acc.C[2], acc.A);
-        }
-    }
-    if (A.counters) {
-        const unsigned long long nom = kb >= ka ? (unsigned long long)(kb - ka + 1) : 0ULL;
-        const unsigned long long reached = kb >= ka ? (unsigned long long)(k_end - ka + 1) : 0ULL;
-        if (GLOBAL) count(A.counters, kRays, nom ? 1 : 0);
-        count(A.counters, kNominal, nom);
-        count(A.counters, kTaken, n_taken);
-        count(A.counters, kVisited, nom ? 1 : 0);
-        count(A.counters, kSkipped, reached - n_taken);     // lattice samples passed over by O-10
-        count(A.counters, kTerminated, stopped ? 1 : 0);
-    }
-}
-
-// ================================================================== variant 3 for sparse tables: test, compact, gather, fold
-// Same ownership as render_ls_kernel (a warp walks its 32 rays together through chunks of 32
-// lattice indices), but a sample is first TESTED against the occupancy bits (CubeDesc::occ, O-10
-// at the level of one trilinear cell): only samples whose 8 corners can reach a table entry of
-// non-zero opacity are interpolated.  Per chunk:
-//   test   - lane = ray: every lane walks the 32 lattice indices of the chunk along ITS ray and
-//            looks up the bit of each sample (position and floor only; the next sample's word is
-//            requested before the current one is tested) -> one 32-bit mask per ray;
-//   list   - the survivors of all rays are written to a list in shared memory, ray-major, lattice
-//            order inside a ray (warp prefix sum of the masks' populations);
-//   gather - lane = list entry, 32 entries per step (full lanes however few samples survive):
-//            position and weights are recomputed (the same float32 operations), the 8 voxels come
-//            through the cp.async ring, the value goes to vals[list index];
-//   fold   - lane = ray: the owner folds its entries front to back (O-7, exact ERT).
-// A list longer than kListCap is taken in batches of whole rays (dense tables use
-// render_ls_kernel<..., DENSE> instead).  Frames are identical to the other marchers': a skipped
-// sample has weight exactly zero.
-constexpr int kListCap = 256;
-constexpr int kOccDepth = 2;             // gathers are few here: a shallower ring leaves more of the SM to L1 (3 -> 6.36, 2 -> 6.26 ms)
-
-// 8 CTAs per SM (64 registers): the few gathers leave L1 alone, more warps hide the bit lookups (measured:
-// 7 -> 6.83, 8 -> 6.44, 9 -> 7.27 ms on C3)
-template <bool GLOBAL>
-__global__ void __launch_bounds__(kThreads, 8)
-render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
-                  const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
-                  const PartialDev* __restrict__ parts, int n_parts) {
-    constexpr int MODE = VR_MODE_EA, LAYOUT = 1;
-    constexpr int kWarps = kThreads / 32;
-    __shared__ float4 rays_all[kWarps][64];
-    __shared__ float stage_all[kWarps][kOccDepth * 256];
-    __shared__ float vals_all[kWarps][kListCap];
-    __shared__ unsigned short list_all[kWarps][kListCap];
-    __shared__ unsigned mask[GLOBAL ? 1 : kCullChunk / 32];
-    // one CTA per pixel tile of the view; for partial images it walks every brick over the tile, so
-    // the ray is set up once (fp64) per pixel, not once per (pixel, brick)
-    int tx, ty; tile_pixel(tx, ty);
-    const int x0 = blockIdx.x * kTileW, y0 = blockIdx.y * kTileH;
-    const int fx = x0 + tx, fy = y0 + ty;
-    const bool live = fx < V.W && fy < V.H;
-    Ray r; r.k0 = 0; r.k1 = -1;
-    r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
-    if (live) setup_ray(V, c, fx, fy, r);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float* vals = vals_all[warp];
-    unsigned short* list = list_all[warp];
-    float4* rays = rays_all[warp];
-    const float* stage = stage_all[warp] + lane;
-    const unsigned stage_addr = (unsigned)__cvta_generic_to_shared(stage);
-    rays[2 * lane] = make_float4(r.o[0], r.o[1], r.o[2], r.d[0]);
-    // state of the brick being marched (GLOBAL: the whole cube in one go)
-    int bid0 = 0, lo0[3] = {0, 0, 0};
-    BrickRef br0 = brick_ref<LAYOUT>(c, 0, lo0);
-    const unsigned* occ0 = c.occ;
-    int ka = r.k0, kb = r.k1, k_end = kb;
-    bool alive = false, stopped = false;
-    Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
-    unsigned n_taken = 0;
-    // the occupancy word of a sample (0 if its brick is inactive) and the sample's bit in it; 64-bit
-    // brick offsets: a sharded cube's global brick ids times the words per brick can pass 2^32
-    auto locate = [&](const float tk, unsigned& word, unsigned& bit) {
-        float fl;
-        const int iv[3] = {floor_pos(__fmaf_rn(tk, r.d[0], r.o[0]), fl), floor_pos(__fmaf_rn(tk, r.d[1], r.o[1]), fl),
-                           floor_pos(__fmaf_rn(tk, r.d[2], r.o[2]), fl)};
-        unsigned lx, ly, lz;
-        const unsigned* occb;
-        if (GLOBAL) {
-            int b[3]; brick_of(c, iv, b);
-            const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
-            lx = (unsigned)(iv[0] - b[0] * c.B[0]); ly = (unsigned)(iv[1] - b[1] * c.B[1]); lz = (unsigned)(iv[2] - b[2] * c.B[2]);
-            occb = c.occ + (long long)bid * c.occ_words_per_brick;
-            if (__ldg(&c.brick_active[bid]) == 0) { word = 0u; bit = 0u; return; }
-        } else {
-            lx = (unsigned)(iv[0] - lo0[0]); ly = (unsigned)(iv[1] - lo0[1]); lz = (unsigned)(iv[2] - lo0[2]);
-            occb = occ0;
-        }
-        word = __ldg(occb + occ_word_index(c, lx, ly, lz));   // an L1 hit while the ray stays in its 4 x 4 x 2 cells
-        bit = occ_bit_index(lx, ly, lz);
-    };
-    // march the taken samples [ka, kb] of every lane's ray (all members of brick bid0 unless GLOBAL) into acc
-    auto march = [&]() {
-    rays[2 * lane + 1] = make_float4(r.d[1], r.d[2], __int_as_float(ka), __int_as_float(kb));
-    __syncwarp();
-    alive = ka <= kb; stopped = false; k_end = kb; n_taken = 0;
-    acc.C[0] = acc.C[1] = acc.C[2] = 0.f; acc.A = 0.f; acc.m = -INFINITY;
-    int K0 = alive ? ka : 0x7fffffff, K1 = alive ? kb : -1;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        K0 = min(K0, __shfl_xor_sync(0xffffffffu, K0, o));
-        K1 = max(K1, __shfl_xor_sync(0xffffffffu, K1, o));
-    }
-    for (int kbase = K0; kbase <= K1; kbase += 32) {
-        if (!__ballot_sync(0xffffffffu, alive)) break;
-        const bool mine = alive && ka <= kbase + 31 && kb >= kbase;
-        const unsigned act = __ballot_sync(0xffffffffu, mine);
-        if (!act) continue;
-        // ---- test, lane = ray: bit j of my_act <=> sample kbase + j of this lane's ray survives.  The
-        // word of the next sample is requested before the current one is tested (reloading it every
-        // time measured faster than keeping it in a register while the ray stays in its cells).
-        unsigned my_act = 0u;
-        {
-            int j0 = mine ? max(ka, kbase) - kbase : 32, j1 = mine ? min(kb, kbase + 31) - kbase : -1;
-            int J0 = j0, J1 = j1;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                J0 = min(J0, __shfl_xor_sync(0xffffffffu, J0, o));
-                J1 = max(J1, __shfl_xor_sync(0xffffffffu, J1, o));
-            }
-            unsigned word = 0u, bit = 0u;                            // of sample j
-            if (J0 >= j0 && J0 <= j1) locate(__fmul_rn((float)(kbase + J0), r.step), word, bit);
-            for (int j = J0; j <= J1; ++j) {
-                unsigned nword = 0u, nbit = 0u;                      // of sample j + 1
-                if (j + 1 >= j0 && j + 1 <= j1) locate(__fmul_rn((float)(kbase + j + 1), r.step), nword, nbit);
-                if (j >= j0 && j <= j1 && ((word >> bit) & 1u)) my_act |= 1u << j;
-                word = nword; bit = nbit;
-            }
-        }
-        // ---- list, ray-major: lane's entries at [off, off + cnt)
-        const int cnt = __popc(my_act);
-        int incl = cnt;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int up = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += up;
-        }
-        const int off = incl - cnt, total = __shfl_sync(0xffffffffu, incl, 31);
-        for (int base = 0; base < total;) {                 // batches of whole rays, at most kListCap entries
-            const bool inb = cnt > 0 && off >= base && off + cnt <= base + kListCap;
-            const unsigned bm = __ballot_sync(0xffffffffu, inb);
-            const int bend = __shfl_sync(0xffffffffu, off + cnt, 31 - __clz((int)bm));
-            const int ntot = bend - base, my_start = off - base;
-            if (inb) {
-                int i = my_start;
-                for (unsigned bits = my_act; bits; bits &= bits - 1) list[i++] = (unsigned short)((lane << 5) | (__ffs(bits) - 1));
-            }
-            __syncwarp();
-            // ---- gather: one list entry per lane, 32 entries per step, through the cp.async ring
-            const int ngroups = (ntot + 31) >> 5;
-            auto issue = [&](Slot& S, const int g, const int s) {
-                S.rc = g < ngroups ? g : -1; S.idle = true;
-                S.w[0] = S.w[1] = S.w[2] = 0.f;
-                const int idx = 32 * g + lane;
-                if (g < ngroups && idx < ntot) {
-                    const unsigned e = list[idx];
-                    const int rr = (int)(e >> 5);
-                    const float tt = __fmul_rn((float)(kbase + (int)(e & 31u)), r.step);
-                    const float4 ra = rays[2 * rr], rb = rays[2 * rr + 1];
-                    float p[3], fl[3];
-                    p[0] = __fmaf_rn(tt, ra.w, ra.x); p[1] = __fmaf_rn(tt, rb.x, ra.y); p[2] = __fmaf_rn(tt, rb.y, ra.z);
-                    const int iv[3] = {floor_pos(p[0], fl[0]), floor_pos(p[1], fl[1]), floor_pos(p[2], fl[2])};
-                    S.w[0] = __fsub_rn(p[0], fl[0]); S.w[1] = __fsub_rn(p[1], fl[1]); S.w[2] = __fsub_rn(p[2], fl[2]);
-                    S.idle = false;
-                    if (GLOBAL) {
-                        int b[3]; brick_of(c, iv, b);
-                        const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
-                        const int bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
-                        gather8_async<LAYOUT>(brick_ref<LAYOUT>(c, bid, lo), iv[0], iv[1], iv[2], stage_addr + 1024u * s);
-                    } else gather8_async<LAYOUT>(br0, iv[0], iv[1], iv[2], stage_addr + 1024u * s);
-                }
-                cp_async_commit();
-            };
-            auto consume = [&](const Slot& S, const int s) {
-                if (S.idle) return;
-                const float* st = stage + 256 * s;
-                float v[8];
-#pragma unroll
-                for (int e = 0; e < 8; ++e) v[e] = st[32 * e];
-                vals[32 * S.rc + lane] = trilinear(v, S.w[0], S.w[1], S.w[2]);
-            };
-            Slot slot[kOccDepth];
-            int gi = 0;
-#pragma unroll
-            for (int s = 0; s < kOccDepth - 1; ++s) issue(slot[s], gi++, s);
-            for (bool more = true; more;) {
-#pragma unroll
-                for (int u = 0; u < kOccDepth; ++u) {
-                    issue(slot[(u + kOccDepth - 1) % kOccDepth], gi++, (u + kOccDepth - 1) % kOccDepth);
-                    cp_async_wait<kOccDepth - 1>();
-                    if (slot[u].rc < 0) { more = false; break; }
-                    consume(slot[u], u);
-                }
-            }
-            __syncwarp();
-            // ---- fold: lane = ray, its entries front to back (O-7)
-            if (inb) {
-                int i = 0;
-                while (i < cnt) {
-                    const bool stop = fold<MODE>(acc, vals[my_start + i], T.baked, T, A.tau);
-                    ++i;
-                    if (stop) { stopped = true; alive = false; k_end = kbase + (int)(list[my_start + i - 1] & 31u); break; }
-                }
-                n_taken += (unsigned)i;
-            }
-            __syncwarp();
-            base = bend;
-        }
-    }
-    __syncwarp();
-    };
-    unsigned long long c_nom = 0, c_reached = 0, c_taken = 0, c_stopped = 0;
-    auto tally = [&]() {
-        if (kb >= ka) { c_nom += (unsigned long long)(kb - ka + 1); c_reached += (unsigned long long)(k_end - ka + 1); }
-        c_taken += n_taken;
-        if (stopped) ++c_stopped;
-    };
-    if (GLOBAL) {
-        march();
-        tally();
-        if (live) write_frame_pixel<MODE>(V, T, A, fx, fy, acc, r.k1 >= r.k0);
-    } else {
-        for (int base = 0; base < n_parts; base += kCullChunk) {
-            const int cnt = min(kCullChunk, n_parts - base);
-            __syncthreads();
-            if (threadIdx.x < kCullChunk / 32) mask[threadIdx.x] = 0u;
-            __syncthreads();
-            for (int q = threadIdx.x; q < cnt; q += kThreads) {
-                const PartialDev& P = parts[base + q];
-                if (P.x0 < x0 + kTileW && P.x0 + P.w > x0 && P.y0 < y0 + kTileH && P.y0 + P.h > y0) atomicOr(&mask[q >> 5], 1u << (q & 31));
-            }
-            __syncthreads();
-            for (int w = 0; w < (cnt + 31) / 32; ++w) {
-                for (unsigned bits = mask[w]; bits; bits &= bits - 1) {
-                    const PartialDev& P = parts[base + 32 * w + __ffs(bits) - 1];
-                    const int lx = fx - P.x0, ly = fy - P.y0;
-                    const bool mine = live && lx >= 0 && ly >= 0 && lx < P.w && ly < P.h;
-                    bid0 = P.brick;
-                    const int b[3] = {bid0 % c.G[0], (bid0 / c.G[0]) % c.G[1], bid0 / (c.G[0] * c.G[1])};
-                    lo0[0] = b[0] * c.B[0]; lo0[1] = b[1] * c.B[1]; lo0[2] = b[2] * c.B[2];
-                    br0 = brick_ref<LAYOUT>(c, bid0, lo0);
-                    occ0 = c.occ + (long long)bid0 * c.occ_words_per_brick;
-                    ka = mine ? r.k0 : 0; kb = mine ? r.k1 : -1;
-                    brick_interval(c, r, b, lo0, ka, kb);
-                    march();
-                    tally();
-                    if (mine) reinterpret_cast<float4*>(P.data)[(long long)ly * P.pitch + lx] = make_float4(acc.C[0], acc.C[1], acc.C[2], acc.A);
-                }
-            }
-        }
-    }
-    if (A.counters) {
-        if (GLOBAL) count(A.counters, kRays, c_nom ? 1 : 0);
-        count(A.counters, kNominal, c_nom);
-        count(A.counters, kTaken, c_taken);
-        count(A.counters, kVisited, c_nom ? 1 : 0);
-        count(A.counters, kSkipped, c_reached - c_taken);
-        count(A.counters, kTerminated, c_stopped);
-    }
-}
-
-}  // namespace
-
-#define VR_DISPATCH(KERNEL, GRID, ...)                                                                   \
-    do {                                                                                                 \
-        if (a.mode == VR_MODE_MIP) {                                                                     \
-            if (c.layout == 0) KERNEL<VR_MODE_MIP, 0><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);            \
-            else KERNEL<VR_MODE_MIP, 1><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);                          \
-        } else {                                                                                         \
-            if (c.layout == 0) KERNEL<VR_MODE_EA, 0><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);             \
-            else KERNEL<VR_MODE_EA, 1><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);                           \
-        }                                                                                                \
-    } while (0)
-
-#define VR_DISPATCH_LS2(GLOBAL, REGS, GRID, ...)                                                          \
-    do {                                                                                                 \
-        if (a.mode == VR_MODE_MIP) {                                                                     \
-            if (c.layout == 0) render_ls_kernel<VR_MODE_MIP, 0, GLOBAL, false, REGS><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
-            else render_ls_kernel<VR_MODE_MIP, 1, GLOBAL, false, REGS><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);  \
-        } else if (a.dense) {                                                                            \
-            if (c.layout == 0) render_ls_kernel<VR_MODE_EA, 0, GLOBAL, true, REGS><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
-            else render_ls_kernel<VR_MODE_EA, 1, GLOBAL, true, REGS><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);    \
-        } else {                                                                                         \
-            if (c.layout == 0) render_ls_kernel<VR_MODE_EA, 0, GLOBAL, false, REGS><<<GRID, kThreads, 0, s>>>(__VA_ARGS__); \
-            else render_ls_kernel<VR_MODE_EA, 1, GLOBAL, false, REGS><<<GRID, kThreads, 0, s>>>(__VA_ARGS__);   \
-        }                                                                                                \
-    } while (0)
-
-#define VR_DISPATCH_LS(GLOBAL, GRID, ...)                                                                \
-    do {                                                                                                 \
-        if (a.ring) VR_DISPATCH_LS2(GLOBAL, true, GRID, __VA_ARGS__);                                    \
-        else VR_DISPATCH_LS2(GLOBAL, false, GRID, __VA_ARGS__);                                          \
-    } while (0)
-
-// the occupancy marcher serves sparse emission-absorption on the micro-block layout
-static bool use_occ_kernel(const CubeDesc& c, const RenderArgs& a) {
-    return a.variant == 3 && a.mode == VR_MODE_EA && a.skip >= 3 && c.layout == 1;
-}
+cudaError_t launch_render_global_f16(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s);
+cudaError_t launch_render_bricks_f16(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a,
+                                     const PartialDev* d_partials, int n, int total_tiles, cudaStream_t s);
 
 cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s) {
-    dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
-    if (use_occ_kernel(c, a)) { render_occ_kernel<true><<<grid, kThreads, 0, s>>>(c, v, t, a, nullptr, 0); return cudaGetLastError(); }
-    if (a.variant == 3) VR_DISPATCH_LS(true, grid, c, v, t, a, nullptr, 0);
-    else if (a.mode == VR_MODE_EA && c.layout == 1 && a.skip >= 3 && v.step < kJumpStep)     // small steps: jump out of idle micro-blocks
-        render_global_kernel<VR_MODE_EA, 1, true><<<grid, kThreads, 0, s>>>(c, v, t, a);
-    else VR_DISPATCH(render_global_kernel, grid, c, v, t, a);
-    return cudaGetLastError();
+    return c.vtype == 1 ? launch_render_global_f16(c, v, t, a, s) : launch_render_global_t<float>(c, v, t, a, s);
 }
 
 cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a,
                                  const PartialDev* d_partials, int n, int total_tiles, cudaStream_t s) {
-    if (n == 0 || total_tiles == 0) return cudaSuccess;
-    if (use_occ_kernel(c, a)) {
-        dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
-        render_occ_kernel<false><<<grid, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-        return cudaGetLastError();
-    }
-    if (a.variant == 3) VR_DISPATCH_LS(false, total_tiles, c, v, t, a, d_partials, n);
-    else if (a.variant == 1) VR_DISPATCH(render_bricks_kernel, total_tiles, c, v, t, a, d_partials, n);
-    else {
-        dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
-        if (a.mode == VR_MODE_EA && c.layout == 1 && a.skip >= 3 && v.step < kJumpStep)      // small steps: jump out of idle micro-blocks
-            render_tiles_kernel<VR_MODE_EA, 1, true><<<grid, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-        else if (a.mode == VR_MODE_MIP) {
-            if (c.layout == 0) render_tiles_kernel<VR_MODE_MIP, 0, false><<<grid, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-            else render_tiles_kernel<VR_MODE_MIP, 1, false><<<grid, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-        } else {
-            if (c.layout == 0) render_tiles_kernel<VR_MODE_EA, 0, false><<<grid, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-            else render_tiles_kernel<VR_MODE_EA, 1, false><<<grid, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
-        }
-    }
-    return cudaGetLastError();
+    return c.vtype == 1 ? launch_render_bricks_f16(c, v, t, a, d_partials, n, total_tiles, s)
+                        : launch_render_bricks_t<float>(c, v, t, a, d_partials, n, total_tiles, s);
 }
 
 }  // namespace vr

@@ -6,6 +6,8 @@
 // ray is set up in fp64 and rounded once to float32; every per-sample operation is an explicit
 // IEEE float32 + - * fma floor min max compare (no fast-math, built with --fmad=false).
 #pragma once
+#include <cuda_fp16.h>
+
 #include "vr_internal.cuh"
 
 namespace vr {
@@ -95,26 +97,33 @@ __device__ __forceinline__ int floor_pos(float p, float& fl) {
 __device__ __forceinline__ float lerp(float a, float b, float w) { return __fmaf_rn(w, __fsub_rn(b, a), a); }   // O-4
 
 // One brick as the sampler sees it.  s0 / s1: layout 0 - row pitch P0 and plane pitch P0 P1;
-// layout 1 - floats per row of micro-blocks (32 T0) and per plane of micro-blocks (32 T0 T1).
-struct BrickRef {
-    const float* base;
+// layout 1 - elements per row of micro-blocks (32 T0) and per plane of micro-blocks (32 T0 T1).
+// V: the stored voxel type, float or __half (CubeDesc::vtype; VR_OPT_VOXEL_TYPE).  A __half voxel is converted to
+// float32 when it is read (exact), everything after that is the same float32 arithmetic.
+template <typename V>
+struct BrickRefT {
+    const V* base;
     int lo[3];
     unsigned s0, s1;
 };
+using BrickRef = BrickRefT<float>;
 
-template <int LAYOUT>
-__device__ __forceinline__ BrickRef brick_ref(const CubeDesc& c, int bid, const int lo[3]) {
-    BrickRef b;
-    b.base = c.cube + (long long)bid * c.stride;
+template <int LAYOUT, typename V = float>
+__device__ __forceinline__ BrickRefT<V> brick_ref(const CubeDesc& c, int bid, const int lo[3]) {
+    BrickRefT<V> b;
+    b.base = reinterpret_cast<const V*>(c.cube) + (long long)bid * c.stride;
     b.lo[0] = lo[0]; b.lo[1] = lo[1]; b.lo[2] = lo[2];
     if (LAYOUT == 0) { b.s0 = (unsigned)c.P[0]; b.s1 = (unsigned)(c.P[0] * c.P[1]); }
     else { b.s0 = 32u * (unsigned)c.T[0]; b.s1 = 32u * (unsigned)(c.T[0] * c.T[1]); }
     return b;
 }
 
+__device__ __forceinline__ float load_voxel(const float* p) { return __ldg(p); }
+__device__ __forceinline__ float load_voxel(const __half* p) { return __half2float(__ldg(p)); }
+
 // Offset q of stored voxel (lx, ly, lz) inside its brick and the steps to its +1 neighbours.
-template <int LAYOUT>
-__device__ __forceinline__ void cell_address(const BrickRef& b, unsigned lx, unsigned ly, unsigned lz, unsigned& q,
+template <int LAYOUT, typename V>
+__device__ __forceinline__ void cell_address(const BrickRefT<V>& b, unsigned lx, unsigned ly, unsigned lz, unsigned& q,
                                              unsigned& dx, unsigned& dy, unsigned& dz) {
     if (LAYOUT == 0) {
         q = lx + b.s0 * ly + b.s1 * lz;
@@ -129,16 +138,16 @@ __device__ __forceinline__ void cell_address(const BrickRef& b, unsigned lx, uns
 
 // The 8 voxels of the trilinear cell whose lower corner is (ix, iy, iz) (global voxel indices,
 // inside brick b or on its halo), in the order 000 100 010 110 001 101 011 111.
-template <int LAYOUT>
-__device__ __forceinline__ void gather8(const BrickRef& b, int ix, int iy, int iz, float v[8]) {
+template <int LAYOUT, typename V>
+__device__ __forceinline__ void gather8(const BrickRefT<V>& b, int ix, int iy, int iz, float v[8]) {
     const unsigned lx = (unsigned)(ix - b.lo[0]), ly = (unsigned)(iy - b.lo[1]), lz = (unsigned)(iz - b.lo[2]);
     unsigned q, dx, dy, dz;
     cell_address<LAYOUT>(b, lx, ly, lz, q, dx, dy, dz);
-    const float* p = b.base + q;
-    v[0] = __ldg(p);           v[1] = __ldg(p + dx);
-    v[2] = __ldg(p + dy);      v[3] = __ldg(p + dy + dx);
-    v[4] = __ldg(p + dz);      v[5] = __ldg(p + dz + dx);
-    v[6] = __ldg(p + dz + dy); v[7] = __ldg(p + dz + dy + dx);
+    const V* p = b.base + q;
+    v[0] = load_voxel(p);           v[1] = load_voxel(p + dx);
+    v[2] = load_voxel(p + dy);      v[3] = load_voxel(p + dy + dx);
+    v[4] = load_voxel(p + dz);      v[5] = load_voxel(p + dz + dx);
+    v[6] = load_voxel(p + dz + dy); v[7] = load_voxel(p + dz + dy + dx);
 }
 
 __device__ __forceinline__ float trilinear(const float v[8], float wx, float wy, float wz) {   // O-4: x, then y, then z
@@ -147,8 +156,8 @@ __device__ __forceinline__ float trilinear(const float v[8], float wx, float wy,
     return lerp(lerp(c00, c10, wy), lerp(c01, c11, wy), wz);
 }
 
-template <int LAYOUT>
-__device__ __forceinline__ float sample(const BrickRef& b, const float p[3]) {
+template <int LAYOUT, typename V>
+__device__ __forceinline__ float sample(const BrickRefT<V>& b, const float p[3]) {
     float fx, fy, fz, v[8];
     const int ix = floor_pos(p[0], fx), iy = floor_pos(p[1], fy), iz = floor_pos(p[2], fz);
     gather8<LAYOUT>(b, ix, iy, iz, v);

@@ -22,6 +22,15 @@ constexpr int kMMCells = 64;       // cells of one row handled per CTA (256^3 br
 
 // Column j of the 3 x 5 columns of micro-blocks (rows of lines along x) that a row of cells (cy, cz) needs:
 // ty = 2 cy + j % 3, tz = 4 cz + j / 3; the third column in y and the fifth in z are the +1 halo planes.
+// a row of 4 x-voxels of a line as float32
+__device__ __forceinline__ float4 load_row(const float* rows, long long i) { return __ldg(reinterpret_cast<const float4*>(rows) + i); }
+__device__ __forceinline__ float4 load_row(const __half* rows, long long i) {
+    const uint2 u = __ldg(reinterpret_cast<const uint2*>(rows) + i);
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&u.x)), b = __half22float2(*reinterpret_cast<const __half2*>(&u.y));
+    return make_float4(a.x, a.y, b.x, b.y);
+}
+
+template <typename V>
 __global__ void __launch_bounds__(kMMWarps * 32)
 cell_minmax_lines_kernel(const __grid_constant__ CubeDesc c, int chunks_x) {
     __shared__ float smin[kMMWarps][kMMCells + 1], smax[kMMWarps][kMMCells + 1];
@@ -38,7 +47,7 @@ cell_minmax_lines_kernel(const __grid_constant__ CubeDesc c, int chunks_x) {
     const int cx0 = xc * kMMCells, ncell = min(kMMCells, c.C[0] - cx0);
     for (int i = lane; i <= kMMCells; i += 32) { smin[warp][i] = INFINITY; smax[warp][i] = -INFINITY; }
     __syncwarp();
-    const float* brick_base = c.cube + (long long)brick * c.stride;
+    const V* brick_base = reinterpret_cast<const V*>(c.cube) + (long long)brick * c.stride;
     const int tx_a = 2 * cx0, tx_b = min(c.T[0] - 1, 2 * (cx0 + ncell));     // last line: the halo plane lx = 8 (cx0 + ncell)
     const int r = lane & 7, g = lane >> 3;
     const int ly3 = 2 * (r >> 2) + (r & 1), lz1 = (r >> 1) & 1;                // this lane's row of 4 x-voxels inside a line
@@ -48,57 +57,48 @@ cell_minmax_lines_kernel(const __grid_constant__ CubeDesc c, int chunks_x) {
         if (ty >= c.T[1] || tz >= c.T[2]) continue;
         const int ly = 4 * ty + ly3, lz = 2 * tz + lz1;
         const bool row_ok = ly <= lim[1] && lz <= lim[2] && (ty_off < 2 || ly3 == 0) && (tz_off < 4 || lz1 == 0);
-        const float4* col = reinterpret_cast<const float4*>(brick_base + 32LL * c.T[0] * (ty + (long long)c.T[1] * tz)) + r;
-        // 4 warp-loads (16 lines, 2 KiB) in flight per warp before the first is reduced: the pass is bound by the
-        // bytes in flight (one load per warp at a time reached 2 TB/s)
-        for (int t00 = tx_a; t00 <= tx_b; t00 += 16) {
-            float4 vv[4];
+        const V* col = brick_base + 32LL * c.T[0] * (ty + (long long)c.T[1] * tz) + 4 * r;   // rows of 4 voxels, 8 per line
+        // group g of 8 lanes takes cell c0 + g: its two lines and the first plane of the next line are reduced inside
+        // the lane, so only one reduction over the 8 rows (6 shuffles) is paid per cell; 8 cells (2 KiB) in flight per warp
+        auto fold4 = [&](const float4 v, const int x0, float& mn, float& mx) {
+            if (x0 + 3 <= lim[0]) {
+                mn = fminf(mn, fminf(fminf(v.x, v.y), fminf(v.z, v.w))); mx = fmaxf(mx, fmaxf(fmaxf(v.x, v.y), fmaxf(v.z, v.w)));
+            } else {
+                if (x0 <= lim[0]) { mn = fminf(mn, v.x); mx = fmaxf(mx, v.x); }
+                if (x0 + 1 <= lim[0]) { mn = fminf(mn, v.y); mx = fmaxf(mx, v.y); }
+                if (x0 + 2 <= lim[0]) { mn = fminf(mn, v.z); mx = fmaxf(mx, v.z); }
+            }
+        };
+        for (int c0 = 0; c0 < ncell; c0 += 8) {
+            float4 va[2], vb[2];
+            float vh[2];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int tx = t00 + 4 * u + g;
-                vv[u] = (row_ok && tx <= tx_b) ? __ldg(col + 8 * tx) : make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int u = 0; u < 2; ++u) {
+                const int tx = tx_a + 2 * (c0 + 4 * u + g);
+                const bool ok = row_ok && c0 + 4 * u + g < ncell;
+                va[u] = (ok && tx <= tx_b) ? load_row(col, 8LL * tx) : make_float4(0.f, 0.f, 0.f, 0.f);
+                vb[u] = (ok && tx + 1 <= tx_b) ? load_row(col, 8LL * (tx + 1)) : make_float4(0.f, 0.f, 0.f, 0.f);
+                vh[u] = (ok && tx + 2 <= tx_b) ? load_voxel(col + 32LL * (tx + 2)) : 0.f;
             }
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int t0 = t00 + 4 * u;
-                if (t0 > tx_b) break;                           // warp-uniform
-                const int tx = t0 + g;
-                float mn = INFINITY, mx = -INFINITY, fmn = INFINITY, fmx = -INFINITY;
-                if (row_ok && tx <= tx_b) {
-                    const float4 v = vv[u];
-                    const int x0 = 4 * tx;
-                    if (x0 + 3 <= lim[0]) {
-                        mn = fminf(fminf(v.x, v.y), fminf(v.z, v.w)); mx = fmaxf(fmaxf(v.x, v.y), fmaxf(v.z, v.w));
-                        fmn = fmx = v.x;
-                    } else {
-                        if (x0 <= lim[0]) { mn = mx = fmn = fmx = v.x; }
-                        if (x0 + 1 <= lim[0]) { mn = fminf(mn, v.y); mx = fmaxf(mx, v.y); }
-                        if (x0 + 2 <= lim[0]) { mn = fminf(mn, v.z); mx = fmaxf(mx, v.z); }
-                    }
+            for (int u = 0; u < 2; ++u) {
+                const int cell = c0 + 4 * u + g, tx = tx_a + 2 * cell;
+                float mn = INFINITY, mx = -INFINITY;
+                if (row_ok && cell < ncell) {
+                    if (tx <= tx_b) fold4(va[u], 4 * tx, mn, mx);
+                    if (tx + 1 <= tx_b) fold4(vb[u], 4 * tx + 4, mn, mx);
+                    if (tx + 2 <= tx_b && 4 * tx + 8 <= lim[0]) { mn = fminf(mn, vh[u]); mx = fmaxf(mx, vh[u]); }
                 }
 #pragma unroll
-                for (int o = 1; o < 8; o <<= 1) {                  // over the 8 rows of the line
+                for (int o = 1; o < 8; o <<= 1) {                  // over the 8 rows of the lines
                     mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, o)); mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-                    fmn = fminf(fmn, __shfl_xor_sync(0xffffffffu, fmn, o)); fmx = fmaxf(fmx, __shfl_xor_sync(0xffffffffu, fmx, o));
                 }
-                // lines q, q + 1 (q even, relative to tx_a) fill cell q / 2; the first plane of line q + 2 is its halo
-                const float mn1 = __shfl_down_sync(0xffffffffu, mn, 8), mx1 = __shfl_down_sync(0xffffffffu, mx, 8);
-                const float fmn2 = __shfl_down_sync(0xffffffffu, fmn, 16), fmx2 = __shfl_down_sync(0xffffffffu, fmx, 16);
-                const int cell = (t0 - tx_a) / 2 + (g >> 1);
-                if (lane == 0) {                                   // the halo of the previous iteration's second cell
-                    if (cell > 0) { smin[warp][cell - 1] = fminf(smin[warp][cell - 1], fmn); smax[warp][cell - 1] = fmaxf(smax[warp][cell - 1], fmx); }
+                if (r == 0 && cell < ncell) {                      // one lane per cell: no two lanes meet in a slot
+                    smin[warp][cell] = fminf(smin[warp][cell], mn); smax[warp][cell] = fmaxf(smax[warp][cell], mx);
                 }
-                __syncwarp();
-                if (lane == 0) {
-                    smin[warp][cell] = fminf(smin[warp][cell], fminf(fminf(mn, mn1), fmn2));
-                    smax[warp][cell] = fmaxf(smax[warp][cell], fmaxf(fmaxf(mx, mx1), fmx2));
-                } else if (lane == 16) {
-                    smin[warp][cell] = fminf(smin[warp][cell], fminf(mn, mn1));
-                    smax[warp][cell] = fmaxf(smax[warp][cell], fmaxf(mx, mx1));
-                }
-                __syncwarp();
             }
         }
+        __syncwarp();
     }
     __syncthreads();
     for (int i = threadIdx.x; i < ncell; i += kMMWarps * 32) {
@@ -139,9 +139,10 @@ __device__ __forceinline__ void bulk_load(unsigned dst, const void* src, unsigne
 
 // hot[line] bit s = voxel in slot s of the line maps above the transparent prefix: (v - vmin) * scale > thr.
 // Persistent CTAs; chunk k of a CTA is chunk blockIdx.x + k * gridDim.x of the window's lines.
+template <typename V>
 __global__ void __launch_bounds__(kHotThreads)
-hot_kernel(const float* __restrict__ lines, unsigned* __restrict__ hot, long long n_lines, float vmin, float scale, float thr) {
-    __shared__ __align__(128) float buf[kHotStages][kHotLines * 32];
+hot_kernel(const V* __restrict__ lines, unsigned* __restrict__ hot, long long n_lines, float vmin, float scale, float thr) {
+    __shared__ __align__(128) V buf[kHotStages][kHotLines * 32];
     __shared__ __align__(8) unsigned long long full[kHotStages];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long n_chunks = (n_lines + kHotLines - 1) / kHotLines;
@@ -152,8 +153,8 @@ hot_kernel(const float* __restrict__ lines, unsigned* __restrict__ hot, long lon
         const int s = (int)(k % kHotStages);
         const unsigned nl = (unsigned)min((long long)kHotLines, n_lines - chunk * kHotLines);
         const unsigned bar = (unsigned)__cvta_generic_to_shared(&full[s]);
-        mbar_expect_tx(bar, nl * 128u);
-        bulk_load((unsigned)__cvta_generic_to_shared(&buf[s][0]), lines + chunk * kHotLines * 32, nl * 128u, bar);
+        mbar_expect_tx(bar, nl * 32u * (unsigned)sizeof(V));
+        bulk_load((unsigned)__cvta_generic_to_shared(&buf[s][0]), lines + chunk * kHotLines * 32, nl * 32u * (unsigned)sizeof(V), bar);
     };
     if (threadIdx.x == 0) {
         for (int s = 0; s < kHotStages; ++s) mbar_init((unsigned)__cvta_generic_to_shared(&full[s]), 1u);
@@ -171,7 +172,7 @@ hot_kernel(const float* __restrict__ lines, unsigned* __restrict__ hot, long lon
 #pragma unroll
         for (int j = 0; j < kPerWarp; ++j) {
             const int line = warp * kPerWarp + j;
-            const float v = line < nl ? buf[s][line * 32 + lane] : 0.f;
+            const float v = line < nl ? (float)buf[s][line * 32 + lane] : 0.f;
             const unsigned b = __ballot_sync(0xffffffffu, line < nl && __fmul_rn(__fsub_rn(v, vmin), scale) > thr);
             if (lane == j) word = b;
         }
@@ -252,7 +253,8 @@ cudaError_t launch_cell_minmax_lines(const CubeDesc& c, cudaStream_t s) {
     const long long ctas = (long long)(c.win_hi - c.win_lo) * c.C[2] * c.C[1] * chunks_x;
     if (ctas <= 0) return cudaSuccess;
     if (ctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    cell_minmax_lines_kernel<<<(unsigned)ctas, kMMWarps * 32, 0, s>>>(c, chunks_x);
+    if (c.vtype == 1) cell_minmax_lines_kernel<__half><<<(unsigned)ctas, kMMWarps * 32, 0, s>>>(c, chunks_x);
+    else cell_minmax_lines_kernel<float><<<(unsigned)ctas, kMMWarps * 32, 0, s>>>(c, chunks_x);
     return cudaGetLastError();
 }
 
@@ -260,9 +262,9 @@ cudaError_t launch_cell_minmax_lines(const CubeDesc& c, cudaStream_t s) {
 cudaError_t launch_classify_occ(const CubeDesc& c, float vmin, float scale, float thr, cudaStream_t s) {
     const long long n_lines = (long long)(c.win_hi - c.win_lo) * c.occ_words_per_brick;
     if (n_lines <= 0) return cudaSuccess;
-    const float* lines = c.cube + (long long)c.win_lo * c.stride;
     unsigned* hot = c.hot + (long long)c.win_lo * c.occ_words_per_brick;
-    hot_kernel<<<148 * 4, kHotThreads, 0, s>>>(lines, hot, n_lines, vmin, scale, thr);
+    if (c.vtype == 1) hot_kernel<__half><<<148 * 4, kHotThreads, 0, s>>>(reinterpret_cast<const __half*>(c.cube) + (long long)c.win_lo * c.stride, hot, n_lines, vmin, scale, thr);
+    else hot_kernel<float><<<148 * 4, kHotThreads, 0, s>>>(c.cube + (long long)c.win_lo * c.stride, hot, n_lines, vmin, scale, thr);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     dilate_kernel<<<148 * 16, 256, 0, s>>>(c, hot, n_lines);

@@ -17,7 +17,7 @@ __device__ __forceinline__ void mark(unsigned* __restrict__ bitmap, long long se
     if ((*(volatile unsigned*)w & bit) == 0u) atomicOr(w, bit);
 }
 
-template <int MODE, int LAYOUT>
+template <int MODE, int LAYOUT, typename VT>
 __global__ void __launch_bounds__(kThreads)
 touch_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V, const __grid_constant__ TFDesc T,
              const __grid_constant__ RenderArgs A, const PartialDev* __restrict__ parts, int n_parts,
@@ -33,9 +33,10 @@ touch_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDes
     const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
     int ka = r.k0, kb = r.k1;
     brick_interval(c, r, b, lo, ka, kb);
-    const BrickRef br = brick_ref<LAYOUT>(c, bid, lo);
+    const BrickRefT<VT> br = brick_ref<LAYOUT, VT>(c, bid, lo);
     const unsigned* occ = (MODE == VR_MODE_EA && LAYOUT == 1 && A.skip >= 3) ? c.occ + (long long)bid * c.occ_words_per_brick : nullptr;
-    const long long brick_sector0 = ((long long)(bid - c.win_lo) * c.stride) >> 3;      // stride is a multiple of 32 floats
+    constexpr int kShift = sizeof(VT) == 4 ? 3 : 4;                                       // voxels per 32-byte sector: 8 or 16
+    const long long brick_sector0 = ((long long)(bid - c.win_lo) * c.stride) >> kShift;  // stride is a multiple of 32 voxels
     Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
     unsigned long long taken = 0;
     bool skip_brick = false;
@@ -55,8 +56,8 @@ touch_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDes
             float v[8];
 #pragma unroll
             for (int e = 0; e < 8; ++e) {
-                mark(bitmap, brick_sector0 + (off[e] >> 3));
-                v[e] = __ldg(br.base + off[e]);
+                mark(bitmap, brick_sector0 + (off[e] >> kShift));
+                v[e] = load_voxel(br.base + off[e]);
             }
             ++taken;
             const float val = trilinear(v, __fsub_rn(p[0], fl[0]), __fsub_rn(p[1], fl[1]), __fsub_rn(p[2], fl[2]));
@@ -83,12 +84,15 @@ __global__ void touch_count_kernel(const unsigned* __restrict__ bitmap, long lon
 cudaError_t launch_touch(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, const PartialDev* d_partials,
                          int n, int total_tiles, unsigned* d_bitmap, unsigned long long* d_taken, cudaStream_t s) {
     if (n == 0 || total_tiles == 0) return cudaSuccess;
-    if (a.mode == VR_MODE_MIP) {
-        if (c.layout == 0) touch_kernel<VR_MODE_MIP, 0><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n, d_bitmap, d_taken);
-        else touch_kernel<VR_MODE_MIP, 1><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n, d_bitmap, d_taken);
+    if (c.vtype == 1) {
+        if (a.mode == VR_MODE_MIP) touch_kernel<VR_MODE_MIP, 1, __half><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n, d_bitmap, d_taken);
+        else touch_kernel<VR_MODE_EA, 1, __half><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n, d_bitmap, d_taken);
+    } else if (a.mode == VR_MODE_MIP) {
+        if (c.layout == 0) touch_kernel<VR_MODE_MIP, 0, float><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n, d_bitmap, d_taken);
+        else touch_kernel<VR_MODE_MIP, 1, float><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n, d_bitmap, d_taken);
     } else {
-        if (c.layout == 0) touch_kernel<VR_MODE_EA, 0><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n, d_bitmap, d_taken);
-        else touch_kernel<VR_MODE_EA, 1><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n, d_bitmap, d_taken);
+        if (c.layout == 0) touch_kernel<VR_MODE_EA, 0, float><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n, d_bitmap, d_taken);
+        else touch_kernel<VR_MODE_EA, 1, float><<<total_tiles, kThreads, 0, s>>>(c, v, t, a, d_partials, n, d_bitmap, d_taken);
     }
     return cudaGetLastError();
 }

@@ -16,7 +16,8 @@ LIB_PATH = os.path.join(_HERE, "libvr.so")
 
 OK, ERR_INVALID_ARG, ERR_BUFFER, ERR_CUDA, ERR_STATE, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 MODE_MIP, MODE_EA = 0, 1
-OPT_SKIP, OPT_VARIANT, OPT_CELL_SKIP, OPT_L2_FETCH, OPT_LAYOUT, OPT_DENSE, OPT_OCCUPANCY, OPT_RING = 1, 2, 3, 4, 5, 6, 7, 8
+OPT_SKIP, OPT_VARIANT, OPT_CELL_SKIP, OPT_L2_FETCH, OPT_LAYOUT, OPT_DENSE, OPT_OCCUPANCY, OPT_RING, OPT_VOXEL_TYPE = 1, 2, 3, 4, 5, 6, 7, 8, 9
+VOXEL_F32, VOXEL_F16 = 0, 1
 
 EXPORTS = [
     "vr_create", "vr_destroy", "vr_last_error", "vr_status_string", "vr_cube_layout",
@@ -26,6 +27,7 @@ EXPORTS = [
     "vr_get_counters", "vr_reset_counters", "vr_set_option", "vr_get_plan",
     "vr_set_brick_window", "vr_window_layout", "vr_sort_groups", "vr_overlay_catalogue", "vr_overlay_pick", "vr_pyramid_layout", "vr_build_pyramid",
     "vr_touch_layout", "vr_measure_touch", "vr_touch_count", "vr_fold_peers", "vr_ipc_export", "vr_ipc_open",
+    "vr_cube_layout_typed",
 ]
 
 
@@ -105,6 +107,7 @@ def load():
     lib.vr_touch_layout.argtypes = [vp, C.POINTER(sz)]
     lib.vr_measure_touch.argtypes = [vp, C.c_int, C.POINTER(Partial), C.c_int, C.c_float, vp, C.c_int, vp]
     lib.vr_touch_count.argtypes = [vp, vp, C.POINTER(C.c_uint64), vp]
+    lib.vr_cube_layout_typed.argtypes = [C.c_int] * 9 + [C.POINTER(sz), C.POINTER(sz)]
     lib.vr_fold_peers.argtypes = [vp, C.c_int, C.POINTER(vp), ip, C.c_int, C.c_int, C.c_int, sz, C.c_int, C.c_int,
                                   C.POINTER(vp), C.c_int, sz, fp, vp]
     lib.vr_ipc_export.argtypes = [vp, vp, C.c_char_p, C.POINTER(sz)]
@@ -132,6 +135,16 @@ def cube_layout(dims, brick):
     rc = load().vr_cube_layout(*(int(v) for v in dims), *(int(v) for v in brick), C.byref(cb), C.byref(mb))
     if rc != OK:
         raise VRError(rc, "vr_cube_layout: invalid argument")
+    return cb.value, mb.value
+
+
+def cube_layout_typed(dims, brick, voxel_type=VOXEL_F32, first_brick=0, end_brick=-1):
+    """Bytes of the cube and meta buffers for the micro-block layout with a stored voxel type (and a brick window)."""
+    cb, mb = C.c_size_t(0), C.c_size_t(0)
+    rc = load().vr_cube_layout_typed(*(int(v) for v in dims), *(int(v) for v in brick), int(voxel_type), int(first_brick),
+                                     int(end_brick), C.byref(cb), C.byref(mb))
+    if rc != OK:
+        raise VRError(rc, "vr_cube_layout_typed: invalid argument")
     return cb.value, mb.value
 
 
