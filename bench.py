@@ -134,21 +134,23 @@ def kernel_name(plan, mode):
 class Job:
     """One rank's resident cube + context.  configure() picks mode / table / frame without regenerating."""
 
-    def __init__(self, w, device, mode="ea", shard=None, dist=None, tf=None):
+    def __init__(self, w, device, mode="ea", shard=None, dist=None, tf=None, voxel="f32"):
         import torch
         from paper_1012_2909_b200 import vr
-        self.torch, self.vr, self.w = torch, vr, w
+        self.torch, self.vr, self.w, self.voxel = torch, vr, w, voxel
         torch.cuda.set_device(device)
         self.ctx = vr.Context(device)
+        vt = vr.VOXEL_F16 if voxel == "f16" else vr.VOXEL_F32
+        self.ctx.set_option(vr.OPT_VOXEL_TYPE, vt)
         self.shard, self.dist = None, dist
         if shard is not None:                     # (rank, world): this rank holds one z-slab of the bricks
             from paper_1012_2909_b200 import sortlast
             self.sortlast = sortlast
             self.shard = sortlast.Shard(self.ctx, w.dims, w.brick, shard[0], shard[1])
             self.shard.bind()
-            cb, mb = self.shard.layout()
+            cb, mb = vr.cube_layout_typed(w.dims, w.brick, vt, self.shard.first, self.shard.end)
         else:
-            cb, mb = vr.cube_layout(w.dims, w.brick)
+            cb, mb = vr.cube_layout_typed(w.dims, w.brick, vt)
         self.d_cube = torch.empty(max(cb // 4, 1), dtype=torch.float32, device="cuda")
         self.d_meta = torch.empty(max(mb, 1), dtype=torch.uint8, device="cuda")
         t0 = time.perf_counter()
@@ -531,10 +533,10 @@ def entry(job, m, args, peak, peak_src, touch_frames):
 
 def describe(job, mode, world, args):
     w = job.w
-    return {"workload": f"{w.name}: {w.dims[0]}x{w.dims[1]}x{w.dims[2]} float32 cube, {w.brick[0]}^3 bricks, "
+    return {"workload": f"{w.name}: {w.dims[0]}x{w.dims[1]}x{w.dims[2]} cube stored as {'float16' if job.voxel == 'f16' else 'float32'}, {w.brick[0]}^3 bricks, "
                         f"{job.W}x{job.H} frame ({job.cols}x{job.rows} panels), step {w.step}, "
                         f"{'EA tf-' + job.tf_name + ' tau=' + str(w.tau) if mode == 'ea' else 'MIP'}, sort-last path, orbit frames spread over 360 deg",
-            "cube_gib": round(w.n_voxels * 4 / 2 ** 30, 3), "n_sources": w.n_sources,
+            "cube_gib": round(w.n_voxels * (2 if job.voxel == "f16" else 4) / 2 ** 30, 3), "n_sources": w.n_sources,
             "l2_policy": "inputs larger than L2 (cube >> 126 MB); no explicit flush",
             "e2e_policy": "matrix + table host->device and frame device->pinned host every step; two frame buffers, frame "
                           "i's copy overlaps frame i+1's render, the host waits for frame i-1 before issuing frame i+1",
@@ -563,13 +565,17 @@ def tf_edit(job, frame_index):
     return {"ms": times[len(times) // 2], "all_ms": times, "what": "threshold entry 32 <-> 40, then one frame, synchronised"}
 
 
-SUITE = [  # (workload, mode, table, frame, panels, steps): the rest of BASELINE.json's metric, each measured like the headline
-    ("C3", "mip", None, None, None, 12),
-    ("C3", "ea", "fog", None, None, 12),
-    ("C2", "ea", None, None, None, 24),
-    ("C4", "ea", None, None, None, 4),
-    ("C5", "ea", None, None, None, 4),
-    ("C5", "mip", None, (1920, 1080), (1, 1), 12),
+SUITE = [  # (workload, mode, table, frame, panels, steps, voxels): the rest of BASELINE.json's metric, each measured like the headline
+    ("C3", "mip", None, None, None, 12, "f32"),
+    ("C3", "ea", "fog", None, None, 12, "f32"),
+    ("C2", "ea", None, None, None, 24, "f32"),
+    ("C4", "ea", None, None, None, 4, "f32"),
+    ("C5", "ea", None, None, None, 4, "f32"),
+    ("C5", "mip", None, (1920, 1080), (1, 1), 12, "f32"),
+    # the paper's HIPASS shape, and a 256 GiB-class cube resident as float16
+    ("HIPASS", "ea", None, None, None, 8, "f32"),
+    ("W256", "ea", None, None, None, 8, "f16"),
+    ("W256", "mip", None, None, None, 8, "f16"),
 ]
 
 
@@ -577,19 +583,19 @@ def run_suite(args, head_job, peak, peak_src, local_rank):
     import torch
     out = []
     job = head_job
-    for name, mode, tf, frame, panels, steps in SUITE:
+    for name, mode, tf, frame, panels, steps, voxel in SUITE:
         w = wl.CONFIGS[name]
         try:
-            if job is None or job.w.name != name:
+            if job is None or job.w.name != name or job.voxel != voxel:
                 if job is not None:
                     job.close()
                     job = None
                 free, _ = torch.cuda.mem_get_info()
-                need = w.n_voxels * 4 * 1.09 + 3e9
+                need = w.n_voxels * (2 if voxel == "f16" else 4) * (1.16 if voxel == "f16" else 1.10) + 3e9
                 if free < need:
                     out.append({"config": {"workload": name, "mode": mode}, "skipped": f"needs {need / 1e9:.0f} GB of free HBM, {free / 1e9:.0f} free"})
                     continue
-                job = Job(w, local_rank, mode, tf=tf)
+                job = Job(w, local_rank, mode, tf=tf, voxel=voxel)
             job.configure(mode, tf or w.tf, frame or w.frame, panels or w.panels)
             m = measure(job, steps, 3, 0, 1, None, local_rank)
             e = entry(job, m, args, peak, peak_src, [orbit_frame(w, 0, steps, 0, 1)] if not args.no_touch else [])
@@ -619,6 +625,7 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--mode", default="ea", choices=["ea", "mip"], help="emission-absorption (default) or MIP")
     ap.add_argument("--tf", default=None, choices=sorted(wl.TFS), help="transfer function (default: the workload's)")
+    ap.add_argument("--voxel", default="f32", choices=["f32", "f16"], help="stored voxel type (VR_OPT_VOXEL_TYPE)")
     ap.add_argument("--sharded", action="store_true",
                     help="N ranks share ONE cube: bricks sharded in z-slabs, sort-last exchange over NCCL (NEXT-1, "
                          "strong scaling); default: N independent replicas")
@@ -656,7 +663,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     default_run = (args.workload is None and args.mode == "ea" and args.tf is None and not args.frame and not args.sharded
-                   and not args.slab and world == 1)
+                   and not args.slab and world == 1 and args.voxel == "f32")
     if args.suite is None:
         args.suite = default_run and args.impl == "b200"
     w = wl.CONFIGS[args.workload or "C3"]
@@ -671,7 +678,8 @@ def main():
             raise SystemExit("--slab R/W runs on one GPU, without --sharded")
     if (args.sharded or slab) and w.panels != (1, 1):
         raise SystemExit("--sharded renders single-panel frames (use --frame WxH for the tiled workloads)")
-    job = Job(w, local_rank, args.mode, shard=slab if slab else ((rank, world) if args.sharded else None), dist=dist, tf=args.tf)
+    job = Job(w, local_rank, args.mode, shard=slab if slab else ((rank, world) if args.sharded else None), dist=dist, tf=args.tf,
+              voxel=args.voxel)
     job.slab_only = slab is not None
     job.staged = args.staged
     frank, fworld = (0, 1) if args.sharded else (rank, world)          # sharded: every rank renders every frame

@@ -75,7 +75,15 @@ C4 = Workload("C4", 3, (1024, 1024, 2048), (128, 128, 128), (9600, 5400), 0.25, 
               panels=(5, 5))
 C5 = Workload("C5", 4, (4096, 4096, 2048), (256, 256, 256), (9600, 5400), 0.5, 80000,
               zero_fraction=0.1, panels=(5, 5))
-CONFIGS = {w.name: w for w in (C1, C2, C3, C4, C5)}
+# Beyond BASELINE.json's five: the shape of the paper's largest rendered cube (HIPASS:
+# 1721 x 1721 x 1025, "12 GB", shown at 3000 x 3000 and 8000 x 8000, line 61; partial edge bricks on every face), and a
+# 256 GiB-class cube (as float32; "larger than a single machine memory limit", line 47 towards WALLABY)
+# that fits one B200 only with float16 voxels.  Same recipe as C3.
+HIPASS = Workload("HIPASS", 5, (1721, 1721, 1025), (256, 256, 256), (3000, 3000), 0.5, 3000, continuum=2.0,
+                  notes="PAPER.md line 57 shape, synthetic content")
+W256 = Workload("W256", 6, (4096, 4096, 4096), (256, 256, 256), (1920, 1080), 0.5, 160000, continuum=2.0,
+                notes="256 GiB as float32: resident as float16 only")
+CONFIGS = {w.name: w for w in (C1, C2, C3, C4, C5, HIPASS, W256)}
 
 
 def scaled(w: Workload, name: str, dims, brick, frame, n_sources=None, panels=None) -> Workload:
@@ -322,5 +330,5 @@ def config_camera(w: Workload, frame_index: int = 0, frame=None) -> np.ndarray:
     if w.projection == "orthographic":
         d = seeded_directions(w.view_seed, 3)[frame_index % 3]
         return ortho_camera(w.dims, frame, d)
-    az = float(frame_index) if w.name.startswith("C3") else 30.0 + float(frame_index)
+    az = float(frame_index) if w.name.startswith(("C3", "W256")) else 30.0 + float(frame_index)
     return perspective_camera(w.dims, frame, azimuth_deg=az)
