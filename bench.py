@@ -210,7 +210,7 @@ class Job:
             for c in range(self.cols):
                 yield c, r, (M if (self.cols, self.rows) == (1, 1) else wl.panel_matrix(M, self.cols, self.rows, c, r))
 
-    def step(self, frame_index, timed_events=False, set_tf=False):
+    def step(self, frame_index, timed_events=False, set_tf=False, one_call=False):
         """S1 + S2-S5 (+ S6) for one frame, sort-last path."""
         w, vr, ctx, torch = self.w, self.vr, self.ctx, self.torch
         if set_tf:
@@ -253,6 +253,17 @@ class Job:
                 e = torch.cuda.Event(enable_timing=True)
                 e.record()
                 self.step_events.append(e)
+            return
+        if one_call:
+            # the same frame through vr_render_sortlast: sort, layout, march and fold of a panel in ONE call (the e2e loop)
+            for c, r, Mp in self.panel_views(frame_index):
+                ctx.set_view(Mp, self.pw, self.ph, w.step)
+                ctx.set_viewport(c * self.pw, r * self.ph, self.W)
+                ok, need = ctx.render_sortlast(self.mode, self.arena, self.frame, self.bg, w.tau)
+                if not ok:
+                    self._arena(need)
+                    ok, need = ctx.render_sortlast(self.mode, self.arena, self.frame, self.bg, w.tau)
+                    assert ok
             return
         for c, r, Mp in self.panel_views(frame_index):
             ctx.set_view(Mp, self.pw, self.ph, w.step)
@@ -427,7 +438,7 @@ def measure(job, steps, warmup, frank, fworld, dist, local_rank, e2e=True):
         if copied[b] is not None:
             torch.cuda.current_stream().wait_event(copied[b])      # the buffer's previous frame has left the device
         job.frame = frames[b]
-        job.step(orbit_frame(w, i, steps, frank, fworld), set_tf=True)
+        job.step(orbit_frame(w, i, steps, frank, fworld), set_tf=True, one_call=True)
         src = job.frame                                             # (the sharded path returns a new tensor)
         rendered = torch.cuda.Event()
         rendered.record()
@@ -538,7 +549,7 @@ def describe(job, mode, world, args):
                         f"{'EA tf-' + job.tf_name + ' tau=' + str(w.tau) if mode == 'ea' else 'MIP'}, sort-last path, orbit frames spread over 360 deg",
             "cube_gib": round(w.n_voxels * (2 if job.voxel == "f16" else 4) / 2 ** 30, 3), "n_sources": w.n_sources,
             "l2_policy": "inputs larger than L2 (cube >> 126 MB); no explicit flush",
-            "e2e_policy": "matrix + table host->device and frame device->pinned host every step; two frame buffers, frame "
+            "e2e_policy": "through vr_set_view + vr_render_sortlast (one call per panel); matrix + table host->device and frame device->pinned host every step; two frame buffers, frame "
                           "i's copy overlaps frame i+1's render, the host waits for frame i-1 before issuing frame i+1",
             "replicas": 1 if args.sharded else world, "shards": world if args.sharded else 1, "slab": args.slab,
             "generate_seconds": round(job.gen_seconds, 3)}

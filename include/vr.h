@@ -143,6 +143,14 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* h_partials, int n,
 int vr_composite_bricks(vr_ctx* ctx, int mode, const vr_partial* h_partials, int n, float* d_out,
                         const float bg[4], void* stream);
 
+/* The four calls above for the current view in one: the resident bricks that can contribute are sorted front to back
+ * (O-9), their partial images are packed into d_arena (device, 256-byte aligned, arena_bytes; *needed_bytes receives
+ * what this view needs: VR_ERR_BUFFER and nothing launched if that is more), rendered (S2-S4) and folded into the
+ * viewport of d_out (S5).  Same kernels and the same frame as the four calls; the descriptors travel once, through a
+ * pinned staging ring of the library, so a frame (or one panel of a tiled frame) costs one call and no host allocation. */
+int vr_render_sortlast(vr_ctx* ctx, int mode, float ert_tau, void* d_arena, size_t arena_bytes, size_t* needed_bytes,
+                       float* d_out, const float bg[4], void* stream);
+
 /* ---- sharding the bricks over several GPUs (PAPER.md line 13 abstract
  *      and line 19 section 1: "distributed GPUs", sub-volumes rendered where they reside and
  *      composited) ----------------------------------------------------------------------------- */

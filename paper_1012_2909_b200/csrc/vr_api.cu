@@ -51,6 +51,14 @@ struct vr_ctx {
     float key_vmin = 0, key_scale = 0;
     int win_lo = 0, win_hi = -1;         // vr_set_brick_window (hi < 0: all bricks)
     std::vector<void*> ipc_bases;        // peer allocations opened by vr_ipc_open
+    // vr_render_sortlast: descriptors staged through a small ring of pinned slots (no allocation, no pageable copy per frame)
+    static constexpr int kPinSlots = 4;
+    PartialDev* h_pin = nullptr;
+    size_t pin_cap = 0;                  // descriptors per slot
+    cudaEvent_t pin_done[kPinSlots] = {nullptr, nullptr, nullptr, nullptr};
+    int pin_next = 0;
+    std::vector<std::pair<int, int>> keyed;   // scratch: (visibility key, brick)
+    std::vector<int> keys;
 };
 
 namespace {
@@ -382,7 +390,6 @@ int check_render_state(vr_ctx* ctx, bool need_tf) {
 int upload_partials(vr_ctx* ctx, int mode, const vr_partial* hp, int n, bool with_tiles, int* total_tiles, cudaStream_t s) {
     if (n > (int)ctx->partials_cap) {
         if (ctx->d_partials) cudaFree(ctx->d_partials);
-    for (void* b : ctx->ipc_bases) cudaIpcCloseMemHandle(b);
         ctx->d_partials = nullptr;
         size_t cap = std::max<size_t>(256, (size_t)n * 2);
         VR_CUDA(ctx, cudaMalloc(&ctx->d_partials, cap * sizeof(PartialDev)));
@@ -499,6 +506,8 @@ int vr_destroy(vr_ctx* ctx) {
     if (ctx->d_scratch) cudaFree(ctx->d_scratch);
     if (ctx->d_partials) cudaFree(ctx->d_partials);
     for (void* b : ctx->ipc_bases) cudaIpcCloseMemHandle(b);
+    if (ctx->h_pin) cudaFreeHost(ctx->h_pin);
+    for (cudaEvent_t e : ctx->pin_done) if (e) cudaEventDestroy(e);
     delete ctx;
     return VR_OK;
 }
@@ -890,6 +899,74 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
     if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
     VR_CUDA(ctx, launch_render_bricks(ctx->cube, ctx->view, tf_desc(ctx), a, ctx->d_partials, n, tiles, s));
     ctx->launches += (n > 0 && tiles > 0) ? 1 : 0;
+    return VR_OK;
+}
+
+int vr_render_sortlast(vr_ctx* ctx, int mode, float tau, void* d_arena, size_t arena_bytes, size_t* needed_bytes, float* d_out,
+                       const float bg[4], void* stream) {
+    VR_RANGE();
+    int rc = check_render_state(ctx, mode == VR_MODE_EA);
+    if (rc) return rc;
+    if ((mode != VR_MODE_MIP && mode != VR_MODE_EA) || !(tau > 0.f) || !d_out || !bg || !needed_bytes || (arena_bytes > 0 && !d_arena) ||
+        ((uintptr_t)d_arena & 255) != 0)
+        return fail(ctx, VR_ERR_INVALID_ARG, "vr_render_sortlast: bad argument (the arena must be 256-byte aligned)");
+    cudaStream_t s = (cudaStream_t)stream;
+    if ((rc = ensure_tables(ctx, s))) return rc;
+    const CubeDesc& c = ctx->cube;
+    // S1: front-to-back list of the resident bricks that can contribute, with their screen rectangles (computed once)
+    brick_keys(ctx, ctx->keys);
+    ctx->keyed.clear();
+    for (int bid = c.win_lo; bid < c.win_hi; ++bid) {
+        if (mode == VR_MODE_EA && ctx->opt_skip && !ctx->h_brick_active[bid]) continue;
+        ctx->keyed.emplace_back(ctx->keys[bid], bid);
+    }
+    std::stable_sort(ctx->keyed.begin(), ctx->keyed.end());
+    // pinned slot
+    const size_t cap_needed = ctx->keyed.size() + 1;
+    if (ctx->pin_cap < cap_needed) {
+        for (cudaEvent_t e : ctx->pin_done) if (e) cudaEventSynchronize(e);
+        if (ctx->h_pin) cudaFreeHost(ctx->h_pin);
+        ctx->h_pin = nullptr; ctx->pin_cap = 0;
+        const size_t cap = std::max<size_t>(1024, 2 * cap_needed);
+        VR_CUDA(ctx, cudaHostAlloc(&ctx->h_pin, sizeof(PartialDev) * cap * vr_ctx::kPinSlots, cudaHostAllocDefault));
+        ctx->pin_cap = cap;
+        for (cudaEvent_t& e : ctx->pin_done) if (!e) VR_CUDA(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    const int slot = ctx->pin_next;
+    ctx->pin_next = (slot + 1) % vr_ctx::kPinSlots;
+    VR_CUDA(ctx, cudaEventSynchronize(ctx->pin_done[slot]));                 // the copy that last used this slot has left it
+    PartialDev* v = ctx->h_pin + (size_t)slot * ctx->pin_cap;
+    const size_t px_bytes = mode == VR_MODE_EA ? 16 : 4;
+    size_t off = 0;
+    int n = 0, tiles = 0;
+    for (const auto& kb : ctx->keyed) {
+        int rect[4];
+        if (!brick_rect(ctx, kb.second, rect)) continue;                      // outside the frustum
+        PartialDev& d = v[n++];
+        d.brick = kb.second; d.x0 = rect[0]; d.y0 = rect[1]; d.w = rect[2]; d.h = rect[3]; d.tile0 = tiles;
+        d.pitch = rect[2]; d.data = (char*)d_arena + off;
+        tiles += ((rect[2] + kTileW - 1) / kTileW) * ((rect[3] + kTileH - 1) / kTileH);
+        off = align_up(off + px_bytes * (size_t)rect[2] * rect[3], 256);
+    }
+    *needed_bytes = off;
+    if (off > arena_bytes) return fail(ctx, VR_ERR_BUFFER, "vr_render_sortlast: the arena is too small (see *needed_bytes)");
+    if (n > (int)ctx->partials_cap) {
+        if (ctx->d_partials) cudaFree(ctx->d_partials);
+        ctx->d_partials = nullptr;
+        const size_t cap = std::max<size_t>(256, (size_t)n * 2);
+        VR_CUDA(ctx, cudaMalloc(&ctx->d_partials, cap * sizeof(PartialDev)));
+        ctx->partials_cap = cap;
+    }
+    if (n > 0) VR_CUDA(ctx, cudaMemcpyAsync(ctx->d_partials, v, sizeof(PartialDev) * n, cudaMemcpyHostToDevice, s));
+    VR_CUDA(ctx, cudaEventRecord(ctx->pin_done[slot], s));
+    RenderArgs a{};
+    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx);
+    a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
+    a.counters = ctx->d_counters;
+    if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
+    VR_CUDA(ctx, launch_render_bricks(c, ctx->view, tf_desc(ctx), a, ctx->d_partials, n, tiles, s));
+    VR_CUDA(ctx, launch_composite(ctx->view, mode, ctx->d_partials, n, d_out, bg, s));
+    ctx->launches += (n > 0 && tiles > 0) ? 2 : 1;
     return VR_OK;
 }
 

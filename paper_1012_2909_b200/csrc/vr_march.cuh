@@ -288,7 +288,14 @@ render_tiles_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ 
 // axis of the 4 x 4 x 2 micro-blocks) meet the most sectors per request and are faster with plain
 // loads (MIP on C3: 17.3 -> 14.7 ms), rays along x or y with cp.async (12.7 vs 14.1 ms): RenderArgs::ring.
 constexpr int kValPitch = 33;
+#ifndef VR_DEPTH_REGS
+#define VR_DEPTH_REGS 3
+#endif
+#ifndef VR_REGS_CTAS
+#define VR_REGS_CTAS 5
+#endif
 constexpr int kDepth = 3;               // rays in flight per warp (measured: 2 -> 12.1, 3 -> 12.0, 4 -> 13.5 ms on C3)
+constexpr int kDepthRegs = VR_DEPTH_REGS;   // the same for the register ring
 constexpr int kBitsWords = 1024;        // shared copy of one brick's macro-cell bits (256^3 bricks: 32^3 cells)
 
 __device__ __forceinline__ void cp_async4(unsigned dst, const float* src) {
@@ -314,7 +321,7 @@ struct Slot { float w[3]; int rc; bool idle; float v[8]; };   // one ray in flig
 
 // 7 CTAs per SM: 72 registers; an 8th CTA (64 registers) would shrink L1 to 28 KB and costs 10 % (measured)
 template <int MODE, int LAYOUT, bool GLOBAL, bool DENSE, bool REGS, typename VT = float>
-__global__ void __launch_bounds__(kThreads, REGS ? 5 : 7)
+__global__ void __launch_bounds__(kThreads, REGS ? VR_REGS_CTAS : 7)
 render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                  const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
                  const PartialDev* __restrict__ parts, int n_parts) {
@@ -325,6 +332,7 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
     __shared__ float4 tab[EA ? 256 : 1];
     __shared__ PartialDev part;
     __shared__ float4 rays_all[kWarps][64];
+    constexpr int D = REGS ? kDepthRegs : kDepth;
     __shared__ float stage_all[REGS ? 1 : kWarps][REGS ? 1 : kDepth * 256];
     __shared__ float vals_all[VALS ? kWarps : 1][VALS ? 32 * kValPitch : 1];
     __shared__ unsigned sbits[SBITS ? kBitsWords : 1];
@@ -475,14 +483,14 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
             }
             if (lane == S.rc) n_taken += __popc(done_bits & upto);
         };
-        Slot slot[kDepth];
+        Slot slot[D];
 #pragma unroll
-        for (int s = 0; s < kDepth - 1; ++s) issue(slot[s], s);
+        for (int s = 0; s < D - 1; ++s) issue(slot[s], s);
         for (bool more = true; more;) {
 #pragma unroll
-            for (int u = 0; u < kDepth; ++u) {
-                issue(slot[(u + kDepth - 1) % kDepth], (u + kDepth - 1) % kDepth);
-                cp_async_wait<kDepth - 1>();
+            for (int u = 0; u < D; ++u) {
+                issue(slot[(u + D - 1) % D], (u + D - 1) % D);
+                cp_async_wait<D - 1>();
                 if (slot[u].rc < 0) { more = false; break; }
                 consume(slot[u], u);
             }

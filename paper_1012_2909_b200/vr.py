@@ -27,7 +27,7 @@ EXPORTS = [
     "vr_get_counters", "vr_reset_counters", "vr_set_option", "vr_get_plan",
     "vr_set_brick_window", "vr_window_layout", "vr_sort_groups", "vr_overlay_catalogue", "vr_overlay_pick", "vr_pyramid_layout", "vr_build_pyramid",
     "vr_touch_layout", "vr_measure_touch", "vr_touch_count", "vr_fold_peers", "vr_ipc_export", "vr_ipc_open",
-    "vr_cube_layout_typed",
+    "vr_cube_layout_typed", "vr_render_sortlast",
 ]
 
 
@@ -107,6 +107,7 @@ def load():
     lib.vr_touch_layout.argtypes = [vp, C.POINTER(sz)]
     lib.vr_measure_touch.argtypes = [vp, C.c_int, C.POINTER(Partial), C.c_int, C.c_float, vp, C.c_int, vp]
     lib.vr_touch_count.argtypes = [vp, vp, C.POINTER(C.c_uint64), vp]
+    lib.vr_render_sortlast.argtypes = [vp, C.c_int, C.c_float, vp, sz, C.POINTER(sz), vp, fp, vp]
     lib.vr_cube_layout_typed.argtypes = [C.c_int] * 9 + [C.POINTER(sz), C.POINTER(sz)]
     lib.vr_fold_peers.argtypes = [vp, C.c_int, C.POINTER(vp), ip, C.c_int, C.c_int, C.c_int, sz, C.c_int, C.c_int,
                                   C.POINTER(vp), C.c_int, sz, fp, vp]
@@ -279,6 +280,19 @@ class Context:
     def composite_bricks(self, mode, parts, n, d_out, bg=(0, 0, 0, 0), stream=None):
         b = (C.c_float * 4)(*[float(x) for x in bg])
         self._check(self._lib.vr_composite_bricks(self._h, int(mode), parts, int(n), C.c_void_p(d_out.data_ptr()), b, _stream(stream)))
+
+    def render_sortlast(self, mode, d_arena, d_out, bg=(0, 0, 0, 0), tau=0.99, stream=None):
+        """One sort-last frame / panel in one call.  Returns (ok, needed_bytes): ok is False if d_arena (a uint8 CUDA tensor
+        or None) is smaller than needed_bytes and nothing was rendered."""
+        b = (C.c_float * 4)(*[float(x) for x in bg])
+        need = C.c_size_t(0)
+        ptr = C.c_void_p(d_arena.data_ptr()) if d_arena is not None else None
+        rc = self._lib.vr_render_sortlast(self._h, int(mode), float(tau), ptr, int(d_arena.numel()) if d_arena is not None else 0,
+                                          C.byref(need), C.c_void_p(d_out.data_ptr()), b, _stream(stream))
+        if rc == ERR_BUFFER:
+            return False, need.value
+        self._check(rc)
+        return True, need.value
 
     # ---- sharded sort-last: exchange + fold + gather in one kernel over peer memory
     def fold_peers(self, mode, frame_ptrs, order, width, height, pitch_px, y0, rows, out_ptrs, out_pitch_px, bg=(0, 0, 0, 0),

@@ -754,3 +754,31 @@ def test_occupancy_bits_against_numpy(H, marcher):
         assert np.array_equal(got.astype(bool), ref), bid
         n_set += int(ref.sum())
     assert 0 < n_set < want.size // 2
+
+
+@pytest.mark.parametrize("mode_name", ["ea", "mip"])
+def test_render_sortlast_one_call_equals_the_four_calls(H, marcher, mode_name):
+    """vr_render_sortlast = vr_sort_bricks + vr_partial_layout + vr_render_bricks + vr_composite_bricks: same frame, bit
+    for bit; an arena that is too small is refused with the size it needs and nothing is rendered."""
+    import torch
+    w = wl.scaled(wl.C2, "one", (96, 80, 112), (32, 32, 32), (160, 100), n_sources=10)
+    sc = H.Scene(w.dims, w.brick, gen={"seed": w.seed, "sources": wl.make_sources(w)})
+    vr = sc.vr
+    mode = vr.MODE_EA if mode_name == "ea" else vr.MODE_MIP
+    W, Hh = w.frame
+    tf = wl.tf_src(20)
+    bg = BG if mode == vr.MODE_EA else (-2.0, 0, 0, 0)
+    for az in (15.0, 140.0):
+        M = wl.perspective_camera(w.dims, w.frame, azimuth_deg=az)
+        ref, _, ids = sc.render_sortlast(M, W, Hh, 0.5, mode, tf=tf, bg=bg, tau=0.9)
+        ch = 4 if mode == vr.MODE_EA else 1
+        out = torch.full((Hh, W, ch), -7.0, dtype=torch.float32, device="cuda")
+        ok, need = sc.ctx.render_sortlast(mode, None, out, bg, 0.9)
+        assert not ok and need > 0 and float(out.min()) == -7.0
+        small = torch.empty(need - 256, dtype=torch.uint8, device="cuda")
+        assert sc.ctx.render_sortlast(mode, small, out, bg, 0.9) == (False, need)
+        arena = torch.empty(need, dtype=torch.uint8, device="cuda")
+        assert sc.ctx.render_sortlast(mode, arena, out, bg, 0.9) == (True, need)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy()
+        assert np.array_equal(got if ch == 4 else got[..., 0], ref)
