@@ -294,8 +294,10 @@ enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETC
        VR_OPT_OCCUPANCY = 7, VR_OPT_RING = 8, VR_OPT_VOXEL_TYPE = 9 };
 int vr_set_option(vr_ctx* ctx, int option, int value);
 /* What a render call of `mode` would launch under the current cube, view and transfer function:
- * out[0] = marcher variant (0 / 3), out[1] = skipping level (0 none, 1 bricks, 2 + macro-cells,
- * 3 + occupancy bits), out[2] = VR_OPT_DENSE as resolved (0 / 1).  May classify the cube against
+ * out[0] = marcher variant (0 / 3), out[1] = skipping level of the sort-last path, vr_render_bricks / vr_render_sortlast
+ * (0 none, 1 bricks, 2 + macro-cells, 3 + occupancy bits; the whole-frame vr_render_mip, which carries one maximum
+ * through all bricks, also uses the macro-cells where the sort-last MIP stops at the brick level),
+ * out[2] = VR_OPT_DENSE as resolved (0 / 1).  May classify the cube against
  * the table (as the render call would) and then synchronises `stream`. */
 int vr_get_plan(vr_ctx* ctx, int mode, int out[3], void* stream);
 

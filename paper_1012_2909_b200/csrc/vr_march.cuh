@@ -288,6 +288,12 @@ render_tiles_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ 
 // axis of the 4 x 4 x 2 micro-blocks) meet the most sectors per request and are faster with plain
 // loads (MIP on C3: 17.3 -> 14.7 ms), rays along x or y with cp.async (12.7 vs 14.1 ms): RenderArgs::ring.
 constexpr int kValPitch = 33;
+#ifndef VR_OCC_GROUP
+#define VR_OCC_GROUP 8
+#endif
+#ifndef VR_OCC_CTAS
+#define VR_OCC_CTAS 8
+#endif
 #ifndef VR_DEPTH_REGS
 #define VR_DEPTH_REGS 3
 #endif
@@ -385,7 +391,11 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
     }
     Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
     unsigned n_taken = 0;
+    // sort-last MIP: once a ray's maximum has reached the brick's maximum nothing in the brick can raise it (O-10 at the
+    // brick level, exact; an all-zero brick of flagged channels is left after its first chunk)
+    const float brick_max = (!EA && !GLOBAL && A.skip >= 1) ? __ldg(&c.brick_mm[bid0]).y : INFINITY;
     for (int kbase = K0; kbase <= K1; kbase += 32) {
+        if (!EA && !GLOBAL && brick_max <= acc.m) alive = false;
         if (!__ballot_sync(0xffffffffu, alive)) break;
         const unsigned act = __ballot_sync(0xffffffffu, alive && ka <= kbase + 31 && kb >= kbase);
         if (!act) continue;
@@ -557,7 +567,7 @@ constexpr int kOccDepth = 2;             // gathers are few here: a shallower ri
 // 8 CTAs per SM (64 registers): the few gathers leave L1 alone, more warps hide the bit lookups (measured:
 // 7 -> 6.83, 8 -> 6.44, 9 -> 7.27 ms on C3)
 template <bool GLOBAL, typename VT = float, bool ASYNC = true>
-__global__ void __launch_bounds__(kThreads, ASYNC ? 8 : 6)      // gathers held in registers: 80 instead of 64
+__global__ void __launch_bounds__(kThreads, ASYNC ? VR_OCC_CTAS : 6)      // gathers held in registers: 80 instead of 64
 render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                   const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
                   const PartialDev* __restrict__ parts, int n_parts) {
@@ -642,6 +652,7 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                 J0 = min(J0, __shfl_xor_sync(0xffffffffu, J0, o));
                 J1 = max(J1, __shfl_xor_sync(0xffffffffu, J1, o));
             }
+#if VR_OCC_GROUP <= 1
             unsigned word = 0u, bit = 0u;                            // of sample j
             if (J0 >= j0 && J0 <= j1) locate(__fmul_rn((float)(kbase + J0), r.step), word, bit);
             for (int j = J0; j <= J1; ++j) {
@@ -650,6 +661,20 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                 if (j >= j0 && j <= j1 && ((word >> bit) & 1u)) my_act |= 1u << j;
                 word = nword; bit = nbit;
             }
+#else
+            // VR_OCC_GROUP words are requested before the first of them is tested: with one request ahead the warp
+            // waited on the word at its use (ncu: 45 % of the kernel's stall samples on that one shift)
+            for (int j = J0; j <= J1; j += VR_OCC_GROUP) {
+                unsigned word[VR_OCC_GROUP], bit[VR_OCC_GROUP];
+#pragma unroll
+                for (int u = 0; u < VR_OCC_GROUP; ++u) {
+                    word[u] = 0u; bit[u] = 0u;                       // out of this ray's range: reads as idle
+                    if (j + u >= j0 && j + u <= j1) locate(__fmul_rn((float)(kbase + j + u), r.step), word[u], bit[u]);
+                }
+#pragma unroll
+                for (int u = 0; u < VR_OCC_GROUP; ++u) my_act |= ((word[u] >> bit[u]) & 1u) << ((j + u) & 31);
+            }
+#endif
         }
         // ---- list, ray-major: lane's entries at [off, off + cnt)
         const int cnt = __popc(my_act);
