@@ -164,6 +164,7 @@ class Job:
         self.slab_only = False
         self.staged = False
         self.peerfold = None
+        self.streams = self.arenas = None
         self.configure(mode, tf or w.tf, w.frame, w.panels)
 
     def configure(self, mode, tf_name, frame, panels):
@@ -189,7 +190,7 @@ class Job:
 
     def close(self):
         self.ctx.close()
-        self.d_cube = self.d_meta = self.arena = self.bitmap = self.frame = self.h_frame = None
+        self.d_cube = self.d_meta = self.arena = self.arenas = self.bitmap = self.frame = self.h_frame = None
         self.torch.cuda.empty_cache()
 
     def _arena(self, nbytes):
@@ -255,15 +256,45 @@ class Job:
                 self.step_events.append(e)
             return
         if one_call:
-            # the same frame through vr_render_sortlast: sort, layout, march and fold of a panel in ONE call (the e2e loop)
-            for c, r, Mp in self.panel_views(frame_index):
+            # the frame through vr_render_sortlast: sort, layout, march and fold of a panel in ONE call.  The panels of a
+            # tiled frame write disjoint viewports: they go round-robin over 3 streams (each with its own arena), so the tail
+            # of one panel's launch overlaps the next panel's; the first panel runs on the caller's stream and the others
+            # start after it (it enqueues whatever a new table needs)
+            main = torch.cuda.current_stream()
+            multi = self.cols * self.rows > 1
+            if multi and self.streams is None:
+                self.streams = [torch.cuda.Stream() for _ in range(3)]
+                self.arenas = [None, None, None]
+            first = None
+            for i, (c, r, Mp) in enumerate(self.panel_views(frame_index)):
                 ctx.set_view(Mp, self.pw, self.ph, w.step)
                 ctx.set_viewport(c * self.pw, r * self.ph, self.W)
-                ok, need = ctx.render_sortlast(self.mode, self.arena, self.frame, self.bg, w.tau)
+                if not multi or i == 0:
+                    st, slot = main, None
+                else:
+                    slot = i % 3
+                    st = self.streams[slot]
+                    st.wait_event(first)
+                arena = self.arena if slot is None else self.arenas[slot]
+                ok, need = ctx.render_sortlast(self.mode, arena, self.frame, self.bg, w.tau, stream=st.cuda_stream)
                 if not ok:
-                    self._arena(need)
-                    ok, need = ctx.render_sortlast(self.mode, self.arena, self.frame, self.bg, w.tau)
+                    arena = torch.empty(int(need * 1.25) + 256, dtype=torch.uint8, device="cuda")
+                    if slot is None:
+                        self.arena = arena
+                    else:
+                        self.arenas[slot] = arena
+                    ok, need = ctx.render_sortlast(self.mode, arena, self.frame, self.bg, w.tau, stream=st.cuda_stream)
                     assert ok
+                if multi and i == 0:
+                    first = torch.cuda.Event()
+                    first.record(main)
+            if multi:
+                for st in self.streams:
+                    main.wait_stream(st)
+            if timed_events:
+                e = torch.cuda.Event(enable_timing=True)
+                e.record()
+                self.step_events.append(e)
             return
         for c, r, Mp in self.panel_views(frame_index):
             ctx.set_view(Mp, self.pw, self.ph, w.step)
@@ -393,8 +424,9 @@ def measure(job, steps, warmup, frank, fworld, dist, local_rank, e2e=True):
             dist.barrier()
         torch.cuda.synchronize()
 
+    one = job.shard is None            # frames through vr_render_sortlast (the sharded path has its own calls)
     for i in range(warmup):
-        job.step(orbit_frame(w, i, steps, frank, fworld))
+        job.step(orbit_frame(w, i, steps, frank, fworld), one_call=one)
     job.ctx.reset_counters()
     job.reset_events()
     sampler = ClockSampler(local_rank)
@@ -403,7 +435,7 @@ def measure(job, steps, warmup, frank, fworld, dist, local_rank, e2e=True):
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
     for i in range(steps):
-        job.step(orbit_frame(w, i, steps, frank, fworld), timed_events=True)
+        job.step(orbit_frame(w, i, steps, frank, fworld), timed_events=True, one_call=one)
     ev1.record()
     barrier()
     clocks = sampler.result()
@@ -411,11 +443,20 @@ def measure(job, steps, warmup, frank, fworld, dist, local_rank, e2e=True):
     marks = [ev0] + job.step_events
     frame_ms = sorted(a.elapsed_time(b) for a, b in zip(marks, marks[1:]))
     cnt = job.ctx.get_counters()
+    if one:
+        # the marcher timed alone (roofline.launch_ms): the same frames through the separate calls, one launch after
+        # the other on one stream, CUDA events around every vr_render_bricks
+        job.reset_events()
+        for i in range(min(steps, 6)):
+            job.step(orbit_frame(w, i, steps, frank, fworld), timed_events=True)
+        torch.cuda.synchronize()
+        job.ctx.reset_counters()
     march_ms = sum(a.elapsed_time(b) for a, b in job.march_events)
     n_march = len(job.march_events)
     ms_total, (nominal, taken, launches) = reduce_run(
         dist, "cuda", ms_total, [cnt["nominal_samples"], cnt["taken_samples"], cnt["kernel_launches"]])
     res = {"ms_total": ms_total, "frame_ms": frame_ms, "nominal": nominal, "taken": taken, "launches": launches,
+           "launches_per_step": n_march / max(1, min(steps, 6) if one else steps),
            "march_ms": march_ms, "n_march": n_march, "b_brick": job.b_brick, "partial_bytes": job.partial_bytes,
            "clocks": clocks, "steps": steps, "fworld": fworld}
     if not e2e:
@@ -489,7 +530,8 @@ def roofline(job, m, touch_frames, peak, peak_src):
     out = {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s",
            "frac": achieved / peak if peak else None, "peak_source": peak_src,
            "algorithmic_bytes_per_launch": alg, "b_brick": b_brick, "b_touch": touch, "bytes_written": writes,
-           "launch_ms": m["march_ms"] / n, "share_of_step": m["march_ms"] / m["ms_total"] if m["ms_total"] else None,
+           "launch_ms": m["march_ms"] / n, "launches_per_step": m["launches_per_step"],
+           "share_of_step": min(1.0, m["march_ms"] / n * m["launches_per_step"] / (m["ms_total"] / m["steps"])) if m["ms_total"] else None,
            "plan": plan,
            "effective_vs_brick": (b_brick + writes) / launch_s / 1e9 / peak if launch_s > 0 and peak else None,
            "note": "algorithmic bytes = min(B_brick, B_touch) + partial images + brick meta (SURVEY.md 8(d)); B_brick = 4 B x "
@@ -566,7 +608,7 @@ def tf_edit(job, frame_index):
         job.tf = wl.tf_src(40 if k % 2 == 0 else 32)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        job.step(frame_index, set_tf=True)
+        job.step(frame_index, set_tf=True, one_call=True)
         torch.cuda.synchronize()
         times.append((time.perf_counter() - t0) * 1e3)
     job.tf = keep

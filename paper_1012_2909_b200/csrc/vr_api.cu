@@ -54,6 +54,7 @@ struct vr_ctx {
     // vr_render_sortlast: descriptors staged through a small ring of pinned slots (no allocation, no pageable copy per frame)
     static constexpr int kPinSlots = 4;
     PartialDev* h_pin = nullptr;
+    PartialDev* d_pin = nullptr;         // the same slots on the device: calls on different streams do not share descriptors
     size_t pin_cap = 0;                  // descriptors per slot
     cudaEvent_t pin_done[kPinSlots] = {nullptr, nullptr, nullptr, nullptr};
     int pin_next = 0;
@@ -510,6 +511,7 @@ int vr_destroy(vr_ctx* ctx) {
     if (ctx->d_partials) cudaFree(ctx->d_partials);
     for (void* b : ctx->ipc_bases) cudaIpcCloseMemHandle(b);
     if (ctx->h_pin) cudaFreeHost(ctx->h_pin);
+    if (ctx->d_pin) cudaFree(ctx->d_pin);
     for (cudaEvent_t e : ctx->pin_done) if (e) cudaEventDestroy(e);
     delete ctx;
     return VR_OK;
@@ -929,16 +931,19 @@ int vr_render_sortlast(vr_ctx* ctx, int mode, float tau, void* d_arena, size_t a
     if (ctx->pin_cap < cap_needed) {
         for (cudaEvent_t e : ctx->pin_done) if (e) cudaEventSynchronize(e);
         if (ctx->h_pin) cudaFreeHost(ctx->h_pin);
-        ctx->h_pin = nullptr; ctx->pin_cap = 0;
+        if (ctx->d_pin) cudaFree(ctx->d_pin);
+        ctx->h_pin = nullptr; ctx->d_pin = nullptr; ctx->pin_cap = 0;
         const size_t cap = std::max<size_t>(1024, 2 * cap_needed);
         VR_CUDA(ctx, cudaHostAlloc(&ctx->h_pin, sizeof(PartialDev) * cap * vr_ctx::kPinSlots, cudaHostAllocDefault));
+        VR_CUDA(ctx, cudaMalloc(&ctx->d_pin, sizeof(PartialDev) * cap * vr_ctx::kPinSlots));
         ctx->pin_cap = cap;
         for (cudaEvent_t& e : ctx->pin_done) if (!e) VR_CUDA(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
     const int slot = ctx->pin_next;
     ctx->pin_next = (slot + 1) % vr_ctx::kPinSlots;
-    VR_CUDA(ctx, cudaEventSynchronize(ctx->pin_done[slot]));                 // the copy that last used this slot has left it
+    VR_CUDA(ctx, cudaEventSynchronize(ctx->pin_done[slot]));                 // the call that last used this slot is done with it
     PartialDev* v = ctx->h_pin + (size_t)slot * ctx->pin_cap;
+    PartialDev* dv = ctx->d_pin + (size_t)slot * ctx->pin_cap;
     const size_t px_bytes = mode == VR_MODE_EA ? 16 : 4;
     size_t off = 0;
     int n = 0, tiles = 0;
@@ -953,22 +958,15 @@ int vr_render_sortlast(vr_ctx* ctx, int mode, float tau, void* d_arena, size_t a
     }
     *needed_bytes = off;
     if (off > arena_bytes) return fail(ctx, VR_ERR_BUFFER, "vr_render_sortlast: the arena is too small (see *needed_bytes)");
-    if (n > (int)ctx->partials_cap) {
-        if (ctx->d_partials) cudaFree(ctx->d_partials);
-        ctx->d_partials = nullptr;
-        const size_t cap = std::max<size_t>(256, (size_t)n * 2);
-        VR_CUDA(ctx, cudaMalloc(&ctx->d_partials, cap * sizeof(PartialDev)));
-        ctx->partials_cap = cap;
-    }
-    if (n > 0) VR_CUDA(ctx, cudaMemcpyAsync(ctx->d_partials, v, sizeof(PartialDev) * n, cudaMemcpyHostToDevice, s));
-    VR_CUDA(ctx, cudaEventRecord(ctx->pin_done[slot], s));
+    if (n > 0) VR_CUDA(ctx, cudaMemcpyAsync(dv, v, sizeof(PartialDev) * n, cudaMemcpyHostToDevice, s));
     RenderArgs a{};
     a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = resolve_variant(ctx);
     a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
     a.counters = ctx->d_counters;
     if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
-    VR_CUDA(ctx, launch_render_bricks(c, ctx->view, tf_desc(ctx), a, ctx->d_partials, n, tiles, s));
-    VR_CUDA(ctx, launch_composite(ctx->view, mode, ctx->d_partials, n, d_out, bg, s));
+    VR_CUDA(ctx, launch_render_bricks(c, ctx->view, tf_desc(ctx), a, dv, n, tiles, s));
+    VR_CUDA(ctx, launch_composite(ctx->view, mode, dv, n, d_out, bg, s));
+    VR_CUDA(ctx, cudaEventRecord(ctx->pin_done[slot], s));                   // both kernels have read the slot
     ctx->launches += (n > 0 && tiles > 0) ? 2 : 1;
     return VR_OK;
 }
