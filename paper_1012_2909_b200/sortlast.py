@@ -185,9 +185,14 @@ class PeerFold:
         self.in_ptrs, self.out_ptrs = [p[0] for p in peers], [p[1] for p in peers]
 
     def barrier(self):
-        """Stream-ordered: kernels enqueued after it start only when every rank's earlier kernels are done."""
+        """Kernels enqueued after it start only when every rank's earlier kernels are done.  NCCL: a one-float
+        all-reduce on the stream (no host wait); other backends (gloo in the tests): synchronise, then a host barrier."""
         if self.dist is not None and self.shard.world > 1 and hasattr(self, "flag"):
-            self.dist.all_reduce(self.flag)
+            if self.dist.get_backend() == "nccl":
+                self.dist.all_reduce(self.flag)
+            else:
+                self.torch.cuda.synchronize()
+                self.dist.barrier()
 
     def render(self, tau=0.99):
         return self.shard.render_partial(self.torch, self.mode, self.W, self.H, tau, out=self.partial)

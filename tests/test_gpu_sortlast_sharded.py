@@ -243,3 +243,71 @@ def test_fused_peer_fold_equals_the_oracle(world, balanced):
                 got = got if mode == vr.MODE_EA else got[..., 0]
                 assert np.array_equal(got, want), (world, mode, az, f.shard.rank)
     del M0
+
+
+def _ipc_worker(rank, world, port, out_dir):
+    """One rank of the multi-process path: its own CUDA context on the one device, the peers' frames mapped with CUDA
+    IPC (vr_ipc_export / vr_ipc_open), vr_fold_peers reading and writing through the mapped pointers."""
+    import os
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1012_2909_b200 import sortlast as sl, vr, workloads as wl
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    torch.cuda.set_device(0)
+    w = wl.scaled(wl.C3, "shard", (96, 80, 160), (32, 32, 32), (160, 90), n_sources=40)
+    W, H = w.frame
+    ctx = vr.Context(0)
+    sh = sl.Shard(ctx, w.dims, w.brick, rank, world)
+    sh.bind()
+    cb, mb = sh.layout()
+    d_cube = torch.empty(max(cb // 4, 64), dtype=torch.float32, device="cuda")
+    d_meta = torch.empty(max(mb, 256), dtype=torch.uint8, device="cuda")
+    ctx.generate_cube(w.seed, w.dims, w.brick, d_cube, d_meta, sources=wl.make_sources(w), continuum=w.continuum)
+    ctx.set_transfer_function(*wl.tf_fog())
+    pf = sl.PeerFold(sh, torch, vr.MODE_EA, W, H, dist=dist)
+    assert len(pf.in_ptrs) == world and pf.in_ptrs[rank] == pf.partial.data_ptr()
+    frames = []
+    for az in (20.0, 200.0):
+        ctx.set_view(wl.perspective_camera(w.dims, w.frame, azimuth_deg=az), W, H, w.step)
+        frames.append(pf.frame((0.05, 0.1, 0.2, 0.3), tau=0.95).clone())
+    torch.cuda.synchronize()
+    np.save(os.path.join(out_dir, f"rank{rank}.npy"), torch.stack(frames).cpu().numpy())
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_fused_fold_across_two_processes_over_cuda_ipc(tmp_path):
+    """The multi-process form of NEXT-1 on the one GPU this run has: two processes, each holding a slab, exchange
+    CUDA IPC handles over gloo; every rank's kernel reads the other's partial frame and writes the other's final frame
+    through the mapped pointers.  No kernel waits on another (host barriers only).  Both ranks must end with the frame
+    the oracle's pieces give."""
+    import socket
+    import torch
+    import torch.multiprocessing as mp
+    from paper_1012_2909_b200 import sortlast as sl, vr, workloads as wl
+    from oracle import ovr
+    import helpers
+    with socket.socket() as sck:
+        sck.bind(("127.0.0.1", 0))
+        port = sck.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    procs = [ctx.Process(target=_ipc_worker, args=(r, 2, port, str(tmp_path))) for r in range(2)]
+    for p in procs:
+        p.start()
+    for p in procs:
+        p.join(timeout=600)
+        assert p.exitcode == 0, "a rank failed or hung"
+    w = wl.scaled(wl.C3, "shard", (96, 80, 160), (32, 32, 32), (160, 90), n_sources=40)
+    W, H = w.frame
+    sc = helpers.Scene(w.dims, w.brick, gen={"seed": w.seed, "sources": wl.make_sources(w), "continuum": w.continuum})
+    vol = sc.oracle_volume()
+    group_first = sl.slab_groups(w.brick_grid, 2)
+    got = [np.load(tmp_path / f"rank{r}.npy") for r in range(2)]
+    assert np.array_equal(got[0], got[1])
+    for i, az in enumerate((20.0, 200.0)):
+        M = wl.perspective_camera(w.dims, w.frame, azimuth_deg=az)
+        want = _oracle_two_level(ovr, vol, M, W, H, w.step, ovr.EA, w.brick, w.brick_grid, group_first, wl.tf_fog(), 0.95,
+                                 (0.05, 0.1, 0.2, 0.3), 0.0)
+        assert np.array_equal(got[0][i], want), az
