@@ -267,8 +267,11 @@ int vr_reset_counters(vr_ctx* ctx, void* stream);
  *  VR_OPT_VARIANT (default -1): the marcher.  0 = one ray per thread, the 32 lanes of a warp take
  *    8 x 4 pixels; for partial images one CTA per pixel tile walks all bricks over the tile (ray
  *    set up once); 1 = the same with one CTA per (brick, tile); 3 = lockstep: a warp walks its 32
- *    rays together through chunks of 32 lattice indices; -1 = chosen per
- *    view from the spacing of neighbouring rays (>= 2 voxels: 3, else 0).
+ *    rays together through chunks of 32 lattice indices; 4 = for dense rays,
+ *    emission-absorption with occupancy bits: per chunk every lane cuts its ray into macro-cell runs, the
+ *    warp then tests the samples of active runs in step, compacts, gathers and folds (any other
+ *    mode / skipping level under 4 runs as 0); -1 = chosen per view from the spacing of neighbouring
+ *    rays (>= 2 voxels: 3, else 4 where it applies, else 0).
  *  VR_OPT_CELL_SKIP (default -1): the 8^3 macro-cell level of the skipping under the configured
  *    bricks, 1 on / 0 off (needs VR_OPT_SKIP); -1 = on for emission-absorption if fewer than 3/4
  *    of the cells are active against the current table, on for MIP in variant 3.
@@ -297,7 +300,7 @@ enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETC
        VR_OPT_OCCUPANCY = 7, VR_OPT_RING = 8, VR_OPT_VOXEL_TYPE = 9 };
 int vr_set_option(vr_ctx* ctx, int option, int value);
 /* What a render call of `mode` would launch under the current cube, view and transfer function:
- * out[0] = marcher variant (0 / 3), out[1] = skipping level of the sort-last path, vr_render_bricks / vr_render_sortlast
+ * out[0] = marcher variant (0 / 3 / 4), out[1] = skipping level of the sort-last path, vr_render_bricks / vr_render_sortlast
  * (0 none, 1 bricks, 2 + macro-cells, 3 + occupancy bits; the whole-frame vr_render_mip, which carries one maximum
  * through all bricks, also uses the macro-cells where the sort-last MIP stops at the brick level),
  * out[2] = VR_OPT_DENSE as resolved (0 / 1).  May classify the cube against

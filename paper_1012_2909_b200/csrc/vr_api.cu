@@ -293,6 +293,15 @@ int skip_level(const vr_ctx* ctx, int mode, bool sortlast = false) {
     return ctx->active_cell_fraction < kCellSkipMaxActive ? 2 : 1;
 }
 
+// The marcher of a render call of `mode` at skipping level `skip`: with dense rays, emission-absorption through
+// a sparse table on the micro-block layout goes to variant 4 (macro-cell runs first, then the occupancy test in step
+// over the warp, compaction, gather, fold), everything else of variant 0 stays a ray per thread.
+int pick_variant(const vr_ctx* ctx, int mode, int skip) {
+    const int v = resolve_variant(ctx);
+    if (v == 0 && ctx->opt_variant < 0 && mode == VR_MODE_EA && skip >= 3 && ctx->cube.layout == 1) return 4;
+    return v;
+}
+
 // Occupancy bits are classified when a render first needs them for the current table.
 int ensure_occ(vr_ctx* ctx, int skip, cudaStream_t s) {
     if (skip < 3 || ctx->occ_valid) return VR_OK;
@@ -410,7 +419,7 @@ int upload_partials(vr_ctx* ctx, int mode, const vr_partial* hp, int n, bool wit
             return fail(ctx, VR_ERR_INVALID_ARG, "bad vr_partial entry");
         if (((uintptr_t)p.d_data & (mode == VR_MODE_EA ? 15 : 3)) != 0)
             return fail(ctx, VR_ERR_INVALID_ARG, "vr_partial.d_data misaligned");
-        v[i].brick = p.brick; v[i].x0 = p.x0; v[i].y0 = p.y0; v[i].w = p.w; v[i].h = p.h;
+        set_brick(v[i], ctx->cube, p.brick); v[i].x0 = p.x0; v[i].y0 = p.y0; v[i].w = p.w; v[i].h = p.h;
         v[i].pitch = (long long)p.pitch_px; v[i].data = p.d_data; v[i].tile0 = tiles;
         if (with_tiles) tiles += ((p.w + kTileW - 1) / kTileW) * ((p.h + kTileH - 1) / kTileH);
     }
@@ -735,7 +744,7 @@ int vr_render_mip(vr_ctx* ctx, float* d_out, float* d_out_rgba, float miss, void
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
-    a.mode = VR_MODE_MIP; a.tau = 2.f; a.miss = miss; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx); a.ring = resolve_ring(ctx);
+    a.mode = VR_MODE_MIP; a.tau = 2.f; a.miss = miss; a.skip = skip_level(ctx, a.mode); a.variant = pick_variant(ctx, a.mode, a.skip); a.ring = resolve_ring(ctx);
     a.out = d_out; a.out_rgba = d_out_rgba; a.counters = ctx->d_counters;
     VR_CUDA(ctx, launch_render_global(ctx->cube, ctx->view, tf_desc(ctx), a, s));
     ctx->launches += 1;
@@ -752,7 +761,7 @@ int vr_render_ea(vr_ctx* ctx, float* d_out, const float bg[4], float tau, void* 
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
-    a.mode = VR_MODE_EA; a.tau = tau; a.skip = skip_level(ctx, a.mode); a.variant = resolve_variant(ctx); a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
+    a.mode = VR_MODE_EA; a.tau = tau; a.skip = skip_level(ctx, a.mode); a.variant = pick_variant(ctx, a.mode, a.skip); a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
     for (int i = 0; i < 4; ++i) a.bg[i] = bg[i];
     a.out = d_out; a.counters = ctx->d_counters;
     if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
@@ -899,7 +908,7 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
     int tiles = 0;
     if ((rc = upload_partials(ctx, mode, hp, n, true, &tiles, s))) return rc;
     RenderArgs a{};
-    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = resolve_variant(ctx); a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
+    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = pick_variant(ctx, a.mode, a.skip); a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
     a.counters = ctx->d_counters;
     if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
     VR_CUDA(ctx, launch_render_bricks(ctx->cube, ctx->view, tf_desc(ctx), a, ctx->d_partials, n, tiles, s));
@@ -951,7 +960,7 @@ int vr_render_sortlast(vr_ctx* ctx, int mode, float tau, void* d_arena, size_t a
         int rect[4];
         if (!brick_rect(ctx, kb.second, rect)) continue;                      // outside the frustum
         PartialDev& d = v[n++];
-        d.brick = kb.second; d.x0 = rect[0]; d.y0 = rect[1]; d.w = rect[2]; d.h = rect[3]; d.tile0 = tiles;
+        set_brick(d, ctx->cube, kb.second); d.x0 = rect[0]; d.y0 = rect[1]; d.w = rect[2]; d.h = rect[3]; d.tile0 = tiles;
         d.pitch = rect[2]; d.data = (char*)d_arena + off;
         tiles += ((rect[2] + kTileW - 1) / kTileW) * ((rect[3] + kTileH - 1) / kTileH);
         off = align_up(off + px_bytes * (size_t)rect[2] * rect[3], 256);
@@ -960,7 +969,7 @@ int vr_render_sortlast(vr_ctx* ctx, int mode, float tau, void* d_arena, size_t a
     if (off > arena_bytes) return fail(ctx, VR_ERR_BUFFER, "vr_render_sortlast: the arena is too small (see *needed_bytes)");
     if (n > 0) VR_CUDA(ctx, cudaMemcpyAsync(dv, v, sizeof(PartialDev) * n, cudaMemcpyHostToDevice, s));
     RenderArgs a{};
-    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = resolve_variant(ctx);
+    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = pick_variant(ctx, a.mode, a.skip);
     a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
     a.counters = ctx->d_counters;
     if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
@@ -1065,7 +1074,7 @@ int vr_measure_touch(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
     int tiles = 0;
     if ((rc = upload_partials(ctx, mode, hp, n, true, &tiles, s))) return rc;
     RenderArgs a{};
-    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = resolve_variant(ctx);
+    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = pick_variant(ctx, a.mode, a.skip);
     a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
     if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
     size_t bytes = 0;
@@ -1176,7 +1185,7 @@ int vr_get_plan(vr_ctx* ctx, int mode, int out[3], void* stream) {
     if (rc) return rc;
     if (!out || (mode != VR_MODE_MIP && mode != VR_MODE_EA)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_get_plan: bad argument");
     if ((rc = ensure_tables(ctx, (cudaStream_t)stream))) return rc;
-    out[0] = resolve_variant(ctx); out[1] = skip_level(ctx, mode, true); out[2] = mode == VR_MODE_EA ? resolve_dense(ctx) : 0;
+    out[1] = skip_level(ctx, mode, true); out[0] = pick_variant(ctx, mode, out[1]); out[2] = mode == VR_MODE_EA ? resolve_dense(ctx) : 0;
     return VR_OK;
 }
 
@@ -1203,7 +1212,7 @@ int vr_set_option(vr_ctx* ctx, int option, int value) {
     if (option == VR_OPT_OCCUPANCY) { ctx->opt_occ = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_DENSE) { ctx->opt_dense = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_VARIANT) {
-        if (value != -1 && value != 0 && value != 1 && value != 3) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");
+        if (value != -1 && value != 0 && value != 1 && value != 3 && value != 4) return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown marcher variant");
         ctx->opt_variant = value; return VR_OK;
     }
     return fail(ctx, VR_ERR_INVALID_ARG, "vr_set_option: unknown option");

@@ -73,7 +73,14 @@ struct PartialDev {        // device descriptor of one partial image
     int brick, x0, y0, w, h, tile0;   // tile0: first CTA tile of this partial in the launch
     long long pitch;
     void* data;
+    int b[3];                         // the brick's grid coordinates (brick = b0 + G0 (b1 + G1 b2)), so that no kernel divides
+    int pad;
 };
+inline void set_brick(PartialDev& d, const CubeDesc& c, int brick) {
+    d.brick = brick; d.pad = 0;
+    if (brick >= 0 && c.G[0] > 0 && c.G[1] > 0) { d.b[0] = brick % c.G[0]; d.b[1] = (brick / c.G[0]) % c.G[1]; d.b[2] = brick / (c.G[0] * c.G[1]); }
+    else d.b[0] = d.b[1] = d.b[2] = 0;
+}
 
 enum Counter { kRays = 0, kNominal, kTaken, kVisited, kSkipped, kTerminated, kNumCounters };
 

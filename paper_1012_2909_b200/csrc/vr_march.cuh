@@ -174,7 +174,7 @@ render_bricks_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__
     Ray r; r.k0 = 0; r.k1 = -1;
     if (live) setup_ray(V, c, part.x0 + lx, part.y0 + ly, r);
     const int bid = part.brick;
-    const int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
+    const int b[3] = {part.b[0], part.b[1], part.b[2]};
     const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
     int ka = r.k0, kb = r.k1;
     brick_interval(c, r, b, lo, ka, kb);
@@ -236,7 +236,7 @@ render_tiles_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ 
                 const int lx = i - P.x0, ly = j - P.y0;
                 const bool mine = live && lx >= 0 && ly >= 0 && lx < P.w && ly < P.h;
                 const int bid = P.brick;
-                const int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
+                const int b[3] = {P.b[0], P.b[1], P.b[2]};
                 const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
                 int ka = mine ? r.k0 : 0, kb = mine ? r.k1 : -1;
                 brick_interval(c, r, b, lo, ka, kb);
@@ -296,6 +296,12 @@ constexpr int kValPitch = 33;
 #endif
 #ifndef VR_DEPTH_REGS
 #define VR_DEPTH_REGS 3
+#endif
+#ifndef VR_DENSE_TEST
+#define VR_DENSE_TEST 2
+#endif
+#ifndef VR_RUNS_GROUP
+#define VR_RUNS_GROUP 4
 #endif
 #ifndef VR_REGS_CTAS
 #define VR_REGS_CTAS 5
@@ -357,7 +363,7 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
     int bid0 = 0, lo0[3] = {0, 0, 0};
     if (!GLOBAL) {
         bid0 = part.brick;
-        lo0[0] = (bid0 % c.G[0]) * c.B[0]; lo0[1] = ((bid0 / c.G[0]) % c.G[1]) * c.B[1]; lo0[2] = (bid0 / (c.G[0] * c.G[1])) * c.B[2];
+        lo0[0] = part.b[0] * c.B[0]; lo0[1] = part.b[1] * c.B[1]; lo0[2] = part.b[2] * c.B[2];
     }
     const bool bits_shared = SBITS && cells && c.cell_words_per_brick <= kBitsWords;
     if (bits_shared)
@@ -369,7 +375,7 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
     if (live) setup_ray(V, c, GLOBAL ? fx : part.x0 + fx, GLOBAL ? fy : part.y0 + fy, r);
     int ka = r.k0, kb = r.k1;
     if (!GLOBAL) {
-        const int b[3] = {bid0 % c.G[0], (bid0 / c.G[0]) % c.G[1], bid0 / (c.G[0] * c.G[1])};
+        const int b[3] = {part.b[0], part.b[1], part.b[2]};
         brick_interval(c, r, b, lo0, ka, kb);
     }
     const BrickRefT<VT> br0 = brick_ref<LAYOUT, VT>(c, bid0, lo0);
@@ -566,7 +572,7 @@ constexpr int kOccDepth = 2;             // gathers are few here: a shallower ri
 
 // 8 CTAs per SM (64 registers): the few gathers leave L1 alone, more warps hide the bit lookups (measured:
 // 7 -> 6.83, 8 -> 6.44, 9 -> 7.27 ms on C3)
-template <bool GLOBAL, typename VT = float, bool ASYNC = true>
+template <bool GLOBAL, typename VT = float, bool ASYNC = true, int TEST = 0>
 __global__ void __launch_bounds__(kThreads, ASYNC ? VR_OCC_CTAS : 6)      // gathers held in registers: 80 instead of 64
 render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                   const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
@@ -635,7 +641,66 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
         K0 = min(K0, __shfl_xor_sync(0xffffffffu, K0, o));
         K1 = max(K1, __shfl_xor_sync(0xffffffffu, K1, o));
     }
+    int cur = ka, run_left = 0;                             // TEST 1: next lattice index to classify, rest of its macro-cell run
+    bool run_on = false;
+    unsigned beam_flags = 0u;                               // TEST 2: chunks of the current group of 4 whose beam meets a non-zero word
+    // TEST 2: local voxel coordinates of the trilinear cell of this lane's sample k, k clipped to [klo, khi]
+    auto cell_of = [&](int k, int klo, int khi, int l[3]) {
+        const float tk = __fmul_rn((float)min(max(k, klo), khi), r.step);
+        float fl;
+        l[0] = floor_pos(__fmaf_rn(tk, r.d[0], r.o[0]), fl) - lo0[0];
+        l[1] = floor_pos(__fmaf_rn(tk, r.d[1], r.o[1]), fl) - lo0[1];
+        l[2] = floor_pos(__fmaf_rn(tk, r.d[2], r.o[2]), fl) - lo0[2];
+    };
+    // TEST 2: the beam against the occupancy words over four consecutive stretches of `stride` lattice indices from k0.
+    // Stretch i holds every lane's samples k0 + i stride .. k0 + (i + 1) stride (one more than its share: conservative),
+    // clipped to the lane's interval; positions are monotone along a ray, so the box of the two end samples holds the ones
+    // between, and the box over the lanes (redux) holds the whole beam.  The 4 x 4 x 2 blocks of cells that meet box i are
+    // shared out among lanes 8 i .. 8 i + 7, one occupancy word each per round, so the four stretches' loads are in flight
+    // together.  Returns bit i = some word of stretch i is non-zero (warp-uniform).  One small loop: this is all a warp
+    // runs while its beam crosses empty space.
+    auto test4 = [&](const int k0, const int stride) {
+        const int grp = lane >> 3;
+        int bl[3] = {0, 0, 0}, bh[3] = {-1, -1, -1}, ca[3], cb[3];
+        cell_of(k0, ka, kb, ca);
+#pragma unroll 1                                            // rolled: the loop a warp runs through empty space has to stay in the L0 instruction cache
+        for (int i = 0; i < 4; ++i) {
+            cell_of(k0 + stride * (i + 1), ka, kb, cb);
+            const bool part = alive && ka <= k0 + stride * (i + 1) - 1 && kb >= k0 + stride * i;
+#pragma unroll
+            for (int x = 0; x < 3; ++x) {
+                const int lo = __reduce_min_sync(0xffffffffu, part ? min(ca[x], cb[x]) : 0x7fffffff);
+                const int hi = __reduce_max_sync(0xffffffffu, part ? max(ca[x], cb[x]) : -1);
+                if (grp == i) { bl[x] = lo; bh[x] = hi; }
+                ca[x] = cb[x];
+            }
+        }
+        // (testing the 8^3 macro-cells of the box first, one activity bit each, did not pay: C4 19.8 -> 20.1, C5 56.1 -> 57.6 ms)
+        const int bx0 = bl[0] >> 2, by0 = bl[1] >> 2, bz0 = bl[2] >> 1;
+        const int nx = (bh[0] >> 2) - bx0 + 1, ny = (bh[1] >> 2) - by0 + 1, nz = (bh[2] >> 1) - bz0 + 1;
+        const int nxy = nx * ny, total = (nx > 0 && ny > 0 && nz > 0) ? nxy * nz : 0;
+        bool any = total > 2048;                            // an absurd box: not tested, taken as met
+        if (!any) {
+            const float rx = __frcp_rn((float)nx), rxy = __frcp_rn((float)nxy);
+            for (int e = lane & 7; e < total; e += 8) {     // e -> (ex, ey, ez): (e + 1/2) / n floors exactly for these small integers
+                const int ez = __float2int_rz(__fmul_rn((float)e + 0.5f, rxy)), rem = e - ez * nxy;
+                const int ey = __float2int_rz(__fmul_rn((float)rem + 0.5f, rx)), ex = rem - ey * nx;
+                any |= __ldg(occ0 + ((unsigned)(bx0 + ex) + (unsigned)c.T[0] * ((unsigned)(by0 + ey) + (unsigned)c.T[1] * (unsigned)(bz0 + ez)))) != 0u;
+            }
+        }
+        const unsigned v = __ballot_sync(0xffffffffu, any);
+        return ((v & 0xffu) ? 1u : 0u) | ((v & 0xff00u) ? 2u : 0u) | ((v & 0xff0000u) ? 4u : 0u) | ((v & 0xff000000u) ? 8u : 0u);
+    };
     for (int kbase = K0; kbase <= K1; kbase += 32) {
+        if constexpr (TEST == 2) {
+            const int sub = ((kbase - K0) >> 5) & 3;
+            if (sub == 0) {                                 // four chunks at a time
+                if (!__ballot_sync(0xffffffffu, alive)) break;
+                beam_flags = test4(kbase, 32);
+                if (beam_flags == 0u) { kbase += 96; continue; }
+            }
+            if (((beam_flags >> sub) & 1u) == 0u) continue;
+        }
         if (!__ballot_sync(0xffffffffu, alive)) break;
         const bool mine = alive && ka <= kbase + 31 && kb >= kbase;
         const unsigned act = __ballot_sync(0xffffffffu, mine);
@@ -644,7 +709,74 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
         // word of the next sample is requested before the current one is tested (reloading it every
         // time measured faster than keeping it in a register while the ray stays in its cells).
         unsigned my_act = 0u;
-        {
+        if constexpr (TEST != 0) {
+            // DENSE RAYS (neighbouring rays closer than a voxel).  The warp's 32 rays form a thin beam; `cand` = the samples
+            // that go to the per-sample occupancy test, found per chunk in one of two ways:
+            //  TEST 2 (partial images): the beam is tested as a whole against the occupancy WORDS (one per 4 x 4 x 2 block
+            //   of cells): the bounding box of all 32 rays' samples of the chunk (positions are monotone along a ray, so
+            //   the box of the samples at the two ends of every lane's part of the chunk), one block per lane; if every word
+            //   is zero the chunk is left by the whole warp.  Otherwise the same test per quarter of the chunk (8 lattice
+            //   indices); the samples of the quarters with a non-zero word are the candidates.  No per-ray traversal.
+            //  TEST 1 (whole frame, O-8 GLOBAL): every lane cuts ITS part of the chunk into runs inside 8^3 macro-cells
+            //   (one position, one run length and one activity bit per run; a run that leaves the chunk is carried into
+            //   the next); the candidates are the samples of active runs.
+            // Then the warp walks the candidate indices together, each lane looking up the occupancy bit of its own
+            // sample at that index: the loop is uniform, so the lanes stay together whatever their rays skip (a ray
+            // per thread that tests and samples on its own ran at a quarter of the lanes inside active cells).
+            unsigned cand = 0u;
+            if constexpr (TEST == 2) {
+                // the chunk's beam met a non-zero word: the same test per quarter of the chunk; the samples of the quarters
+                // that meet one are the candidates
+                const unsigned q4 = test4(kbase, 8);
+                const unsigned quarters = ((q4 & 1u) ? 0xffu : 0u) | ((q4 & 2u) ? 0xff00u : 0u) | ((q4 & 4u) ? 0xff0000u : 0u) | ((q4 & 8u) ? 0xff000000u : 0u);
+                if (mine) cand = quarters & (0xffffffffu << (max(ka, kbase) - kbase)) & (0xffffffffu >> (31 - (min(kb, kbase + 31) - kbase)));
+            } else if (mine) {
+                const int kend = min(kb, kbase + 31);
+                const int S8[3] = {kCell, kCell, kCell};
+                while (cur <= kend) {
+                    if (run_left == 0) {
+                        float p[3], fl;
+                        position(r, (float)cur, p);
+                        const int iv[3] = {floor_pos(p[0], fl), floor_pos(p[1], fl), floor_pos(p[2], fl)};
+                        int bid = bid0, lo[3] = {lo0[0], lo0[1], lo0[2]};
+                        bool brick_on = true;
+                        if (GLOBAL) {
+                            int b[3]; brick_of(c, iv, b);
+                            lo[0] = b[0] * c.B[0]; lo[1] = b[1] * c.B[1]; lo[2] = b[2] * c.B[2];
+                            bid = b[0] + c.G[0] * (b[1] + c.G[1] * b[2]);
+                            brick_on = __ldg(&c.brick_active[bid]) != 0;
+                        }
+                        if (brick_on) {
+                            const int clo[3] = {lo[0] + (((iv[0] - lo[0]) >> 3) << 3), lo[1] + (((iv[1] - lo[1]) >> 3) << 3),
+                                                lo[2] + (((iv[2] - lo[2]) >> 3) << 3)};
+                            run_left = min(kb - cur + 1, run_length(r, p, clo, S8));
+                            run_on = !cell_idle<MODE>(c, bid, lo, iv[0], iv[1], iv[2], 0.f);
+                        } else {
+                            run_left = min(kb - cur + 1, run_length(r, p, lo, c.B));
+                            run_on = false;
+                        }
+                    }
+                    const int take = min(run_left, kend - cur + 1);
+                    if (run_on) cand |= (take >= 32 ? 0xffffffffu : ((1u << take) - 1u)) << (cur - kbase);
+                    cur += take; run_left -= take;
+                }
+            }
+            const unsigned all = __reduce_or_sync(0xffffffffu, cand);
+            if (all == 0u) continue;
+            for (unsigned bits = all; bits;) {
+                int jj[VR_RUNS_GROUP];
+                unsigned word[VR_RUNS_GROUP], bit[VR_RUNS_GROUP];
+#pragma unroll
+                for (int u = 0; u < VR_RUNS_GROUP; ++u) { jj[u] = bits ? __ffs(bits) - 1 : -1; bits &= bits - 1; }
+#pragma unroll
+                for (int u = 0; u < VR_RUNS_GROUP; ++u) {
+                    word[u] = 0u; bit[u] = 0u;
+                    if (jj[u] >= 0 && ((cand >> jj[u]) & 1u)) locate(__fmul_rn((float)(kbase + jj[u]), r.step), word[u], bit[u]);
+                }
+#pragma unroll
+                for (int u = 0; u < VR_RUNS_GROUP; ++u) my_act |= ((word[u] >> bit[u]) & 1u) << (jj[u] & 31);
+            }
+        } else {
             int j0 = mine ? max(ka, kbase) - kbase : 32, j1 = mine ? min(kb, kbase + 31) - kbase : -1;
             int J0 = j0, J1 = j1;
 #pragma unroll
@@ -794,7 +926,7 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                     const int lx = fx - P.x0, ly = fy - P.y0;
                     const bool mine = live && lx >= 0 && ly >= 0 && lx < P.w && ly < P.h;
                     bid0 = P.brick;
-                    const int b[3] = {bid0 % c.G[0], (bid0 / c.G[0]) % c.G[1], bid0 / (c.G[0] * c.G[1])};
+                    const int b[3] = {P.b[0], P.b[1], P.b[2]};
                     lo0[0] = b[0] * c.B[0]; lo0[1] = b[1] * c.B[1]; lo0[2] = b[2] * c.B[2];
                     br0 = brick_ref<LAYOUT, VT>(c, bid0, lo0);
                     occ0 = c.occ + (long long)bid0 * c.occ_words_per_brick;
@@ -829,6 +961,11 @@ static bool use_occ_kernel(const CubeDesc& c, const RenderArgs& a) {
     return a.variant == 3 && a.mode == VR_MODE_EA && a.skip >= 3 && c.layout == 1;
 }
 
+// the same kernel with the macro-cell runs walked first and the occupancy test in step over the warp: dense rays
+static bool use_runs_kernel(const CubeDesc& c, const RenderArgs& a) {
+    return a.variant == 4 && a.mode == VR_MODE_EA && a.skip >= 3 && c.layout == 1;
+}
+
 template <typename V, bool GLOBAL, bool REGS, typename... Args>
 static void launch_ls(const CubeDesc& c, const RenderArgs& a, dim3 grid, cudaStream_t s, Args... args) {
     if (a.mode == VR_MODE_MIP) {
@@ -857,6 +994,7 @@ static cudaError_t launch_render_global_t(const CubeDesc& c, const ViewDesc& v, 
     dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
     const PartialDev* none = nullptr;
     if (use_occ_kernel(c, a)) { render_occ_kernel<true, V, !kHalf<V>><<<grid, kThreads, 0, s>>>(c, v, t, a, none, 0); return cudaGetLastError(); }
+    if (use_runs_kernel(c, a)) { render_occ_kernel<true, V, !kHalf<V>, 1><<<grid, kThreads, 0, s>>>(c, v, t, a, none, 0); return cudaGetLastError(); }
     if (a.variant == 3) launch_ls_ring<V, true>(c, a, grid, s, c, v, t, a, none, 0);
     else if (a.mode == VR_MODE_EA && c.layout == 1 && a.skip >= 3 && v.step < kJumpStep)     // small steps: jump out of idle micro-blocks
         render_global_kernel<VR_MODE_EA, 1, true, V><<<grid, kThreads, 0, s>>>(c, v, t, a);
@@ -877,6 +1015,10 @@ static cudaError_t launch_render_bricks_t(const CubeDesc& c, const ViewDesc& v, 
     dim3 grid((v.W + kTileW - 1) / kTileW, (v.H + kTileH - 1) / kTileH);
     if (use_occ_kernel(c, a)) {
         render_occ_kernel<false, V, !kHalf<V>><<<grid, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
+        return cudaGetLastError();
+    }
+    if (use_runs_kernel(c, a)) {
+        render_occ_kernel<false, V, !kHalf<V>, VR_DENSE_TEST><<<grid, kThreads, 0, s>>>(c, v, t, a, d_partials, n);
         return cudaGetLastError();
     }
     if (a.variant == 3) launch_ls_ring<V, false>(c, a, dim3(total_tiles), s, c, v, t, a, d_partials, n);

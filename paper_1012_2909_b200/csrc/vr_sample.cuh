@@ -236,32 +236,32 @@ __device__ __forceinline__ void tile_pixel(int& tx, int& ty) {     // warp = 8 x
 // floor(p_a) / B_a == b_a, which is monotone per axis.
 __device__ __forceinline__ void brick_interval(const CubeDesc& c, const Ray& r, const int b[3], const int lo[3], int& ka, int& kb) {
     if (ka > kb) return;
+    // in units of the lattice index: r.inv = 1 / (step |d|), no division
     float t0 = 0.f, t1 = 3.0e38f;
     bool empty = false;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         float flo = (float)lo[a] - r.margin, fhi = (float)(lo[a] + c.B[a]) + r.margin;
         if (r.d[a] == 0.f) { if (r.o[a] < flo || r.o[a] > fhi) empty = true; continue; }
-        float ta = (flo - r.o[a]) / r.d[a], tb = (fhi - r.o[a]) / r.d[a];
+        const float si = r.d[a] > 0.f ? r.inv[a] : -r.inv[a];
+        float ta = __fmul_rn(flo - r.o[a], si), tb = __fmul_rn(fhi - r.o[a], si);
         t0 = fmaxf(t0, fminf(ta, tb)); t1 = fminf(t1, fmaxf(ta, tb));
     }
     if (empty || !(t0 <= t1)) { ka = 0; kb = -1; return; }
-    float qa = floorf(t0 / r.step) - 2.f, qb = ceilf(t1 / r.step) + 2.f;
+    float qa = floorf(t0) - 2.f, qb = ceilf(t1) + 2.f;
     ka = max(ka, (int)fminf(fmaxf(qa, 0.f), 1.0e9f));
     kb = min(kb, (int)fminf(fmaxf(qb, -1.f), 1.0e9f));
     float p[3], fl;
     while (ka <= kb) {
-        position(r, (float)ka, p);
-        int iv[3] = {floor_pos(p[0], fl), floor_pos(p[1], fl), floor_pos(p[2], fl)};
-        int bb[3]; brick_of(c, iv, bb);
-        if (bb[0] == b[0] && bb[1] == b[1] && bb[2] == b[2]) break;
+        position(r, (float)ka, p);                          // floor(p_a) / B_a == b_a  <=>  lo_a <= floor(p_a) < lo_a + B_a
+        if ((unsigned)(floor_pos(p[0], fl) - lo[0]) < (unsigned)c.B[0] && (unsigned)(floor_pos(p[1], fl) - lo[1]) < (unsigned)c.B[1] &&
+            (unsigned)(floor_pos(p[2], fl) - lo[2]) < (unsigned)c.B[2]) break;
         ++ka;
     }
     while (kb >= ka) {
         position(r, (float)kb, p);
-        int iv[3] = {floor_pos(p[0], fl), floor_pos(p[1], fl), floor_pos(p[2], fl)};
-        int bb[3]; brick_of(c, iv, bb);
-        if (bb[0] == b[0] && bb[1] == b[1] && bb[2] == b[2]) break;
+        if ((unsigned)(floor_pos(p[0], fl) - lo[0]) < (unsigned)c.B[0] && (unsigned)(floor_pos(p[1], fl) - lo[1]) < (unsigned)c.B[1] &&
+            (unsigned)(floor_pos(p[2], fl) - lo[2]) < (unsigned)c.B[2]) break;
         --kb;
     }
 }

@@ -29,7 +29,7 @@ touch_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDes
     r.o[0] = r.o[1] = r.o[2] = 0.f; r.d[0] = r.d[1] = r.d[2] = 0.f; r.step = V.step; r.margin = 0.f;
     if (live) setup_ray(V, c, part.x0 + lx, part.y0 + ly, r);
     const int bid = part.brick;
-    const int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
+    const int b[3] = {part.b[0], part.b[1], part.b[2]};
     const int lo[3] = {b[0] * c.B[0], b[1] * c.B[1], b[2] * c.B[2]};
     int ka = r.k0, kb = r.k1;
     brick_interval(c, r, b, lo, ka, kb);

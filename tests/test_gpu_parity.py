@@ -28,9 +28,9 @@ def H():
 # skipping ("auto") and once per forced variant (0 / 1: ray per thread, CTA per pixel tile / per
 # (brick, tile); 3: lockstep ray per warp, folding
 # emission-absorption samples in the owning lane "v3s" or through shared memory "v3d", or testing
-# every sample against the occupancy bits first "v3o", or with the gathers in a register ring "v3r"), with the macro-cell level of the skipping
-# forced on.
-@pytest.fixture(autouse=True, params=["auto", "v0", "v1", "v3s", "v3d", "v3o", "v3r"])
+# every sample against the occupancy bits first "v3o", or with the gathers in a register ring "v3r"; 4: the occupancy marcher for
+# dense rays, macro-cell runs first "v4o"), with the macro-cell level of the skipping forced on.
+@pytest.fixture(autouse=True, params=["auto", "v0", "v1", "v3s", "v3d", "v3o", "v3r", "v4o"])
 def marcher(request, H):
     from paper_1012_2909_b200 import vr
     H.FORCED_OPTIONS.clear()

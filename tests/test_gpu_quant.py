@@ -20,7 +20,7 @@ def H():
     return helpers
 
 
-@pytest.fixture(params=["auto", "v0", "v1", "v3s", "v3d", "v3o"])
+@pytest.fixture(params=["auto", "v0", "v1", "v3s", "v3d", "v3o", "v4o"])
 def plan(request, H):
     from paper_1012_2909_b200 import vr
     H.FORCED_OPTIONS.clear()
