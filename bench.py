@@ -127,7 +127,7 @@ def kernel_name(plan, mode):
             return "render_occ_kernel (lockstep: occupancy test, compaction, gather, fold)"
         return f"render_ls_kernel<{m}> (lockstep{', dense fold' if dense and mode == 'ea' else ''})"
     if v == 4 and mode == "ea" and skip >= 3:
-        return "render_occ_kernel<RUNS> (dense rays: macro-cell runs, occupancy test in step, compaction, gather, fold)"
+        return "render_occ_kernel<BEAM> (dense rays: beam test against the occupancy words, occupancy test in step, compaction, gather, fold)"
     if v == 1:
         return f"render_bricks_kernel<{m}> (ray per thread, CTA per (brick, tile))"
     return f"render_tiles_kernel<{m}> (ray per thread, skip level {skip})"

@@ -17,12 +17,17 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "_obj")
 LIB = os.path.join(HERE, "libvr.so")
-SOURCES = ["vr_api.cu", "vr_cube.cu", "vr_march.cu", "vr_march_h.cu", "vr_dense.cu", "vr_setup.cu", "vr_touch.cu", "vr_quant.cu",
+SOURCES = ["vr_api.cu", "vr_cube.cu", "vr_march.cu", "vr_march_h.cu", "vr_setup.cu", "vr_touch.cu",
            "vr_composite.cu", "vr_overlay.cu", "vr_pyramid.cu"]
 HEADERS = [os.path.join(CSRC, "vr_internal.cuh"), os.path.join(CSRC, "vr_sample.cuh"), os.path.join(CSRC, "vr_march.cuh"),
            os.path.join(os.path.dirname(HERE), "include", "vr.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--fmad=false", "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall", "-Xptxas", "-v"]
+
+
+def _flags():
+    """NVCC_FLAGS plus VR_NVCC_EXTRA from the environment (-D switches of A/B builds, e.g. "-DVR_LIST_CAP=128")."""
+    return NVCC_FLAGS + os.environ.get("VR_NVCC_EXTRA", "").split()
 
 
 def _nvcc() -> str:
@@ -54,7 +59,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     def compile_one(job):
         src, obj = job
         tmp = obj + f".tmp{os.getpid()}"
-        res = subprocess.run([nvcc, *NVCC_FLAGS, "-c", src, "-o", tmp], capture_output=True, text=True)
+        res = subprocess.run([nvcc, *_flags(), "-c", src, "-o", tmp], capture_output=True, text=True)
         if res.returncode == 0:
             os.replace(tmp, obj)
             with open(obj[:-2] + ".log", "w") as f:        # ptxas -v: registers, spills, shared memory

@@ -298,7 +298,10 @@ int skip_level(const vr_ctx* ctx, int mode, bool sortlast = false) {
 // over the warp, compaction, gather, fold), everything else of variant 0 stays a ray per thread.
 int pick_variant(const vr_ctx* ctx, int mode, int skip) {
     const int v = resolve_variant(ctx);
-    if (v == 0 && ctx->opt_variant < 0 && mode == VR_MODE_EA && skip >= 3 && ctx->cube.layout == 1) return 4;
+    // small bricks: a ray spends one or two groups of chunks in a brick, the per-(tile, brick) set-up of the warp-wide
+    // marcher then outweighs what it saves (C2, 64^3 bricks: 0.73 ms as variant 0, 0.80 as 4)
+    const int bmin = std::min(ctx->cube.B[0], std::min(ctx->cube.B[1], ctx->cube.B[2]));
+    if (v == 0 && ctx->opt_variant < 0 && mode == VR_MODE_EA && skip >= 3 && ctx->cube.layout == 1 && bmin >= 128) return 4;
     return v;
 }
 

@@ -300,6 +300,9 @@ constexpr int kValPitch = 33;
 #ifndef VR_DENSE_TEST
 #define VR_DENSE_TEST 2
 #endif
+#ifndef VR_BEAM_COARSE
+#define VR_BEAM_COARSE true
+#endif
 #ifndef VR_RUNS_GROUP
 #define VR_RUNS_GROUP 4
 #endif
@@ -567,7 +570,16 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
 // A list longer than kListCap is taken in batches of whole rays (dense tables use
 // render_ls_kernel<..., DENSE> instead).  Frames are identical to the other marchers': a skipped
 // sample has weight exactly zero.
-constexpr int kListCap = 256;
+#ifndef VR_LIST_CAP
+#define VR_LIST_CAP 256
+#endif
+#ifndef VR_DENSE_LIST_CAP
+#define VR_DENSE_LIST_CAP 512
+#endif
+// entries per batch.  Sparse rays (C3) live on L1: more shared memory per CTA costs more than the batches save (256 -> 512:
+// 5.4 -> 13.7 ms); dense rays meet whole sources, where every sample survives, and gain from longer batches (C4 19.6 ->
+// 18.8, C5 52.9 -> 50.3 ms)
+template <int TEST> constexpr int kListCapOf = TEST == 0 ? VR_LIST_CAP : VR_DENSE_LIST_CAP;
 constexpr int kOccDepth = 2;             // gathers are few here: a shallower ring leaves more of the SM to L1 (3 -> 6.36, 2 -> 6.26 ms)
 
 // 8 CTAs per SM (64 registers): the few gathers leave L1 alone, more warps hide the bit lookups (measured:
@@ -579,6 +591,7 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                   const PartialDev* __restrict__ parts, int n_parts) {
     constexpr int MODE = VR_MODE_EA, LAYOUT = 1;
     constexpr int kWarps = kThreads / 32;
+    constexpr int kListCap = kListCapOf<TEST>;
     __shared__ float4 rays_all[kWarps][64];
     __shared__ float stage_all[ASYNC ? kWarps : 1][ASYNC ? kOccDepth * 256 : 1];
     __shared__ float vals_all[kWarps][kListCap];
@@ -604,6 +617,7 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
     int bid0 = 0, lo0[3] = {0, 0, 0};
     BrickRefT<VT> br0 = brick_ref<LAYOUT, VT>(c, 0, lo0);
     const unsigned* occ0 = c.occ;
+    const unsigned* cbits0 = c.cell_bits;
     int ka = r.k0, kb = r.k1, k_end = kb;
     bool alive = false, stopped = false;
     Accum acc = {{0.f, 0.f, 0.f}, 0.f, -INFINITY};
@@ -659,7 +673,7 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
     // shared out among lanes 8 i .. 8 i + 7, one occupancy word each per round, so the four stretches' loads are in flight
     // together.  Returns bit i = some word of stretch i is non-zero (warp-uniform).  One small loop: this is all a warp
     // runs while its beam crosses empty space.
-    auto test4 = [&](const int k0, const int stride) {
+    auto test4 = [&](const int k0, const int stride, const bool coarse) {
         const int grp = lane >> 3;
         int bl[3] = {0, 0, 0}, bh[3] = {-1, -1, -1}, ca[3], cb[3];
         cell_of(k0, ka, kb, ca);
@@ -675,17 +689,21 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                 ca[x] = cb[x];
             }
         }
-        // (testing the 8^3 macro-cells of the box first, one activity bit each, did not pay: C4 19.8 -> 20.1, C5 56.1 -> 57.6 ms)
-        const int bx0 = bl[0] >> 2, by0 = bl[1] >> 2, bz0 = bl[2] >> 1;
-        const int nx = (bh[0] >> 2) - bx0 + 1, ny = (bh[1] >> 2) - by0 + 1, nz = (bh[2] >> 1) - bz0 + 1;
+        // coarse: the 8^3 macro-cells that meet the box (one activity bit each); else its 4 x 4 x 2 blocks (one word each)
+        const int sx = coarse ? 3 : 2, sz = coarse ? 3 : 1;
+        const int bx0 = bl[0] >> sx, by0 = bl[1] >> sx, bz0 = bl[2] >> sz;
+        const int nx = (bh[0] >> sx) - bx0 + 1, ny = (bh[1] >> sx) - by0 + 1, nz = (bh[2] >> sz) - bz0 + 1;
         const int nxy = nx * ny, total = (nx > 0 && ny > 0 && nz > 0) ? nxy * nz : 0;
+        const unsigned s0 = coarse ? (unsigned)c.C[0] : (unsigned)c.T[0], s1 = coarse ? (unsigned)c.C[1] : (unsigned)c.T[1];
         bool any = total > 2048;                            // an absurd box: not tested, taken as met
         if (!any) {
             const float rx = __frcp_rn((float)nx), rxy = __frcp_rn((float)nxy);
             for (int e = lane & 7; e < total; e += 8) {     // e -> (ex, ey, ez): (e + 1/2) / n floors exactly for these small integers
                 const int ez = __float2int_rz(__fmul_rn((float)e + 0.5f, rxy)), rem = e - ez * nxy;
                 const int ey = __float2int_rz(__fmul_rn((float)rem + 0.5f, rx)), ex = rem - ey * nx;
-                any |= __ldg(occ0 + ((unsigned)(bx0 + ex) + (unsigned)c.T[0] * ((unsigned)(by0 + ey) + (unsigned)c.T[1] * (unsigned)(bz0 + ez)))) != 0u;
+                const unsigned idx = (unsigned)(bx0 + ex) + s0 * ((unsigned)(by0 + ey) + s1 * (unsigned)(bz0 + ez));
+                if (coarse) any |= ((__ldg(cbits0 + (idx >> 5)) >> (idx & 31u)) & 1u) != 0u;
+                else any |= __ldg(occ0 + idx) != 0u;
             }
         }
         const unsigned v = __ballot_sync(0xffffffffu, any);
@@ -696,7 +714,7 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
             const int sub = ((kbase - K0) >> 5) & 3;
             if (sub == 0) {                                 // four chunks at a time
                 if (!__ballot_sync(0xffffffffu, alive)) break;
-                beam_flags = test4(kbase, 32);
+                beam_flags = test4(kbase, 32, VR_BEAM_COARSE);
                 if (beam_flags == 0u) { kbase += 96; continue; }
             }
             if (((beam_flags >> sub) & 1u) == 0u) continue;
@@ -727,7 +745,7 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
             if constexpr (TEST == 2) {
                 // the chunk's beam met a non-zero word: the same test per quarter of the chunk; the samples of the quarters
                 // that meet one are the candidates
-                const unsigned q4 = test4(kbase, 8);
+                const unsigned q4 = test4(kbase, 8, false);
                 const unsigned quarters = ((q4 & 1u) ? 0xffu : 0u) | ((q4 & 2u) ? 0xff00u : 0u) | ((q4 & 4u) ? 0xff0000u : 0u) | ((q4 & 8u) ? 0xff000000u : 0u);
                 if (mine) cand = quarters & (0xffffffffu << (max(ka, kbase) - kbase)) & (0xffffffffu >> (31 - (min(kb, kbase + 31) - kbase)));
             } else if (mine) {
@@ -883,7 +901,8 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                 }
             }
             __syncwarp();
-            // ---- fold: lane = ray, its entries front to back (O-7)
+            // ---- fold: lane = ray, its entries front to back (O-7).  (Looking the colours up first, with lane = list entry
+            // and full lanes, and folding (r, g, b, a') from shared memory cost more shared memory than it saved: -3 %.)
             if (inb) {
                 int i = 0;
                 while (i < cnt) {
@@ -930,6 +949,7 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                     lo0[0] = b[0] * c.B[0]; lo0[1] = b[1] * c.B[1]; lo0[2] = b[2] * c.B[2];
                     br0 = brick_ref<LAYOUT, VT>(c, bid0, lo0);
                     occ0 = c.occ + (long long)bid0 * c.occ_words_per_brick;
+                    cbits0 = c.cell_bits + (long long)bid0 * c.cell_words_per_brick;
                     ka = mine ? r.k0 : 0; kb = mine ? r.k1 : -1;
                     brick_interval(c, r, b, lo0, ka, kb);
                     march();

@@ -1,4 +1,4 @@
-// Device-side building blocks of the ray marchers, shared by the kernels of vr_march.cu, vr_dense.cu and
+// Device-side building blocks of the ray marchers, shared by the kernels of vr_march.cu and
 // vr_touch.cu (not part of the C ABI): O-2 ray set-up, O-3 lattice positions and brick membership, O-4
 // trilinear gather, O-6 table lookup, O-7 front-to-back fold, run lengths and the O-10 activity tests.
 //
