@@ -668,6 +668,10 @@ def run_suite(args, head_job, peak, peak_src, local_rank):
             job = None
     if job is not None:
         job.close()
+    try:                                              # the HIPASS-shaped cube streamed from pinned host memory
+        out.append(run_streamed(wl.CONFIGS["HIPASS"], "ea", 2, 6, 2, local_rank))
+    except Exception as exc:
+        out.append({"config": {"workload": "HIPASS streamed"}, "error": f"{type(exc).__name__}: {exc}"})
     return out
 
 
@@ -699,6 +703,9 @@ def main():
     ap.add_argument("--no-suite", dest="suite", action="store_false")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle timing (profiling runs)")
     ap.add_argument("--no-touch", action="store_true", help="skip the B_touch measurement (profiling runs)")
+    ap.add_argument("--streamed", type=int, default=0, metavar="SLOTS",
+                    help="out-of-core run: the cube in pinned host memory, streamed through SLOTS device slots of one slab each "
+                         "(SURVEY.md 8(f)-4; paper_1012_2909_b200/outofcore.py)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
@@ -726,6 +733,9 @@ def main():
         w = replace(w, frame=tuple(int(v) for v in args.frame.lower().split("x")), panels=(1, 1))
     if args.next_rows:
         return run_next_rows(args)
+    if args.streamed:
+        print(json.dumps(run_streamed(w, args.mode, args.streamed, args.steps, args.warmup, local_rank, args.tf)))
+        return 0
     slab = None
     if args.slab:
         slab = tuple(int(v) for v in args.slab.split("/"))
@@ -779,6 +789,48 @@ def main():
     if dist is not None:
         dist.destroy_process_group()
     return 0
+
+
+def run_streamed(w, mode_name, n_slots, steps, warmup, local_rank, tf_name=None):
+    """SURVEY.md 8(f)-4 / PAPER.md line 19 (cubes "larger than a single machine memory limit"): the cube kept brick-major in
+    pinned host memory, streamed per frame through `n_slots` device slots of one slab (whole z-layers of bricks) each
+    (paper_1012_2909_b200/outofcore.py): host -> device copy of the next slab overlapping the render of the current one, one
+    vr_fold_peers launch per frame.  Wall-clock per frame, synchronised (the copies are part of the frame)."""
+    import torch
+    from paper_1012_2909_b200 import outofcore, vr
+    torch.cuda.set_device(local_rank)
+    grid_z = -(-w.dims[2] // w.brick[2])
+    t0 = time.perf_counter()
+    cube = outofcore.StreamedCube(w.dims, w.brick, n_slabs=min(grid_z, 32), n_slots=n_slots, device=local_rank)
+    cube.ingest_generated(w.seed, sources=wl.make_sources(w), zero_boxes=wl.make_zero_boxes(w), continuum=w.continuum)
+    ingest_s = time.perf_counter() - t0
+    mode = vr.MODE_EA if mode_name == "ea" else vr.MODE_MIP
+    cube.set_transfer_function(*wl.TFS[tf_name or w.tf]())
+    W, H = w.frame if w.panels == (1, 1) else (w.frame[0] // w.panels[0], w.frame[1] // w.panels[1])
+    times = []
+    for i in range(warmup + steps):
+        M = wl.config_camera(w, orbit_frame(w, max(i - warmup, 0), steps, 0, 1), frame=(W, H))
+        torch.cuda.synchronize()
+        before = dict(cube.stats)
+        t0 = time.perf_counter()
+        cube.render(mode, M, W, H, w.step, tau=w.tau)
+        torch.cuda.synchronize()
+        if i >= warmup:
+            times.append((time.perf_counter() - t0, cube.stats["h2d_bytes"] - before["h2d_bytes"], cube.stats["slabs_copied"] - before["slabs_copied"]))
+    total_s = sum(t[0] for t in times)
+    out = {"config": {"workload": f"{w.name} streamed: {w.dims[0]}x{w.dims[1]}x{w.dims[2]} float32 cube in pinned host memory, "
+                                  f"{cube.n_slabs} slabs of whole brick layers through {cube.n_slots} device slots, {W}x{H} frame, "
+                                  f"{'EA tf-' + (tf_name or w.tf) if mode_name == 'ea' else 'MIP'}, step {w.step}",
+                      "host_gib": round(cube.host_bytes() / 2 ** 30, 2),
+                      "device_pool_gib": round(sum(s["d_cube"].numel() * 4 for s in cube.slots) / 2 ** 30, 2)},
+           "ms_per_step": total_s * 1e3 / len(times), "frames_per_s": len(times) / total_s, "steps": len(times),
+           "slabs_copied_per_frame": sum(t[2] for t in times) / len(times),
+           "h2d_gb_per_frame": sum(t[1] for t in times) / len(times) / 1e9,
+           "h2d_gbs": sum(t[1] for t in times) / total_s / 1e9,
+           "ingest_seconds": round(ingest_s, 2),
+           "note": "wall clock, synchronised per frame: the frame time is the host -> device traffic of the slabs that are not resident"}
+    cube.close()
+    return out
 
 
 def run_next_rows(args):

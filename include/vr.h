@@ -65,6 +65,14 @@ int vr_cube_layout(int nx, int ny, int nz, int bx, int by, int bz, size_t* cube_
 int vr_cube_layout_typed(int nx, int ny, int nz, int bx, int by, int bz, int voxel_type, int first_brick, int end_brick,
                          size_t* cube_bytes, size_t* meta_bytes);
 
+/* Bytes at the START of d_meta that depend on the cube alone ((min,max) per brick and per macro-cell); the rest is
+ * classification against the current transfer function, which the library recomputes on the device when a render
+ * needs it.  A caller that keeps (a window of) a cube outside HBM and brings it back later (PAPER.md
+ * line 19: cubes "larger than a single machine memory limit"; paper_1012_2909_b200/outofcore.py) saves and restores the cube
+ * bytes and these leading meta bytes, then calls vr_attach_cube. */
+int vr_meta_static_bytes(int nx, int ny, int nz, int bx, int by, int bz, int voxel_type, int first_brick, int end_brick,
+                         size_t* static_bytes);
+
 /* Rebrick a linear x-fastest float32 cube (host if src_is_device == 0, else device) into d_cube
  * and compute d_meta.  Host sources are streamed slab by slab (whole planes) through two library
  * staging slabs, the copy of one overlapping the rebricking of the other; the call synchronises `stream`.

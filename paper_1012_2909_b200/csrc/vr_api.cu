@@ -553,6 +553,19 @@ int vr_cube_layout_typed(int nx, int ny, int nz, int bx, int by, int bz, int vox
     return VR_OK;
 }
 
+int vr_meta_static_bytes(int nx, int ny, int nz, int bx, int by, int bz, int voxel_type, int first_brick, int end_brick,
+                         size_t* static_bytes_out) {
+    if (!valid_dims(nx, ny, nz, bx, by, bz) || !static_bytes_out || (voxel_type != 0 && voxel_type != 1)) return VR_ERR_INVALID_ARG;
+    CubeDesc c;
+    fill_cube_desc(c, nx, ny, nz, bx, by, bz, 1, voxel_type);
+    if (end_brick >= 0) {
+        if (first_brick < 0 || end_brick < first_brick || end_brick > c.nbricks) return VR_ERR_INVALID_ARG;
+        c.win_lo = first_brick; c.win_hi = end_brick;
+    }
+    *static_bytes_out = meta_layout(c).cell_bits;           // (min,max) per brick and per macro-cell lead the meta buffer
+    return VR_OK;
+}
+
 int vr_attach_cube(vr_ctx* ctx, int nx, int ny, int nz, int bx, int by, int bz, const void* d_cube, void* d_meta) {
     VR_RANGE();
     if (!ctx) return VR_ERR_INVALID_ARG;

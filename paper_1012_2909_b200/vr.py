@@ -27,7 +27,7 @@ EXPORTS = [
     "vr_get_counters", "vr_reset_counters", "vr_set_option", "vr_get_plan",
     "vr_set_brick_window", "vr_window_layout", "vr_sort_groups", "vr_overlay_catalogue", "vr_overlay_pick", "vr_pyramid_layout", "vr_build_pyramid",
     "vr_touch_layout", "vr_measure_touch", "vr_touch_count", "vr_fold_peers", "vr_ipc_export", "vr_ipc_open",
-    "vr_cube_layout_typed", "vr_render_sortlast",
+    "vr_cube_layout_typed", "vr_render_sortlast", "vr_meta_static_bytes",
 ]
 
 
@@ -109,6 +109,7 @@ def load():
     lib.vr_touch_count.argtypes = [vp, vp, C.POINTER(C.c_uint64), vp]
     lib.vr_render_sortlast.argtypes = [vp, C.c_int, C.c_float, vp, sz, C.POINTER(sz), vp, fp, vp]
     lib.vr_cube_layout_typed.argtypes = [C.c_int] * 9 + [C.POINTER(sz), C.POINTER(sz)]
+    lib.vr_meta_static_bytes.argtypes = [C.c_int] * 9 + [C.POINTER(sz)]
     lib.vr_fold_peers.argtypes = [vp, C.c_int, C.POINTER(vp), ip, C.c_int, C.c_int, C.c_int, sz, C.c_int, C.c_int,
                                   C.POINTER(vp), C.c_int, sz, fp, vp]
     lib.vr_ipc_export.argtypes = [vp, vp, C.c_char_p, C.POINTER(sz)]
@@ -147,6 +148,16 @@ def cube_layout_typed(dims, brick, voxel_type=VOXEL_F32, first_brick=0, end_bric
     if rc != OK:
         raise VRError(rc, "vr_cube_layout_typed: invalid argument")
     return cb.value, mb.value
+
+
+def meta_static_bytes(dims, brick, voxel_type=VOXEL_F32, first_brick=0, end_brick=-1):
+    """Leading bytes of the meta buffer that depend on the cube alone (vr_meta_static_bytes)."""
+    nb = C.c_size_t(0)
+    rc = load().vr_meta_static_bytes(*(int(v) for v in dims), *(int(v) for v in brick), int(voxel_type), int(first_brick),
+                                     int(end_brick), C.byref(nb))
+    if rc != OK:
+        raise VRError(rc, "vr_meta_static_bytes: invalid argument")
+    return nb.value
 
 
 def window_layout(dims, brick, first_brick, end_brick):
