@@ -122,6 +122,8 @@ def kernel_name(plan, mode):
     """The marcher vr_render_bricks launches under a plan (vr_get_plan)."""
     v, skip, dense = plan["variant"], plan["skip_level"], plan["dense"]
     m = "EA" if mode == "ea" else "MIP"
+    if v == 5:
+        return "mip_tiles_kernel (object order: tiles of 32x32x16 cells staged in shared memory by bulk asynchronous copies)"
     if v == 3:
         if mode == "ea" and skip >= 3:
             return "render_occ_kernel (lockstep: occupancy test, compaction, gather, fold)"

@@ -303,12 +303,18 @@ int vr_reset_counters(vr_ctx* ctx, void* stream);
  *    read, so the renderer computes on the cube Q(v) = float32(float16(v)) with the same float32 arithmetic (DESIGN.md
  *    O-16): half the bytes per voxel, a 256 GiB-class cube fits one B200.  Needs VR_OPT_LAYOUT 1; read by the next
  *    upload / generate / attach call; |v| beyond the float16 range (65504) is refused like a non-finite voxel.
- *    THIS option changes frames (by the quantisation of the cube, nothing else). */
+ *    THIS option changes frames (by the quantisation of the cube, nothing else).
+ *  VR_OPT_MIP_TILES (default -1): per-brick partial images by maximum intensity (vr_render_bricks / vr_render_sortlast, MIP)
+ *    in OBJECT order: the bricks are cut into tiles of 32 x 32 x 16 cells that stream through shared memory (bulk
+ *    asynchronous copies), every tile samples the rays that cross it and merges with an atomic maximum (MIP is order
+ *    independent, the partial images are the same to the bit).  1 = on, 0 / -1 = off (the image-order marchers measured
+ *    faster on every workload of bench.py: DESIGN.md section 5); float32 voxels on layout 1.  The library keeps one ray record (48 bytes)
+ *    per view pixel for it, allocated at first use. */
 enum { VR_OPT_SKIP = 1, VR_OPT_VARIANT = 2, VR_OPT_CELL_SKIP = 3, VR_OPT_L2_FETCH = 4, VR_OPT_LAYOUT = 5, VR_OPT_DENSE = 6,
-       VR_OPT_OCCUPANCY = 7, VR_OPT_RING = 8, VR_OPT_VOXEL_TYPE = 9 };
+       VR_OPT_OCCUPANCY = 7, VR_OPT_RING = 8, VR_OPT_VOXEL_TYPE = 9, VR_OPT_MIP_TILES = 10 };
 int vr_set_option(vr_ctx* ctx, int option, int value);
 /* What a render call of `mode` would launch under the current cube, view and transfer function:
- * out[0] = marcher variant (0 / 3 / 4), out[1] = skipping level of the sort-last path, vr_render_bricks / vr_render_sortlast
+ * out[0] = marcher variant (0 / 3 / 4; 5 = the object-order MIP of VR_OPT_MIP_TILES), out[1] = skipping level of the sort-last path, vr_render_bricks / vr_render_sortlast
  * (0 none, 1 bricks, 2 + macro-cells, 3 + occupancy bits; the whole-frame vr_render_mip, which carries one maximum
  * through all bricks, also uses the macro-cells where the sort-last MIP stops at the brick level),
  * out[2] = VR_OPT_DENSE as resolved (0 / 1).  May classify the cube against

@@ -40,6 +40,11 @@ struct vr_ctx {
     size_t partials_cap = 0;
     int64_t launches = 0;
     int opt_skip = 1, opt_cell_skip = -1, opt_variant = -1, opt_layout = 1, opt_dense = -1, opt_occ = -1, opt_ring = -1;   // -1: chosen per view / TF
+    int opt_mip_tiles = -1;
+    // object-order MIP (vr_mip_tiles.cu): one ray record per view pixel, one buffer per descriptor slot of
+    // vr_render_sortlast (calls in flight on different streams) plus one for vr_render_bricks; grown on demand
+    float4* d_rays[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    size_t rays_bytes[5] = {0, 0, 0, 0, 0};
     int opt_vtype = 0;                   // VR_OPT_VOXEL_TYPE: 0 float32, 1 float16
     float x_clear = -INFINITY;
     double active_cell_fraction = 1.0;   // macro-cells active against the current table (EA)
@@ -403,7 +408,33 @@ int check_render_state(vr_ctx* ctx, bool need_tf) {
     return VR_OK;
 }
 
-int upload_partials(vr_ctx* ctx, int mode, const vr_partial* hp, int n, bool with_tiles, int* total_tiles, cudaStream_t s) {
+// Per-brick partial images by maximum intensity in object order (vr_mip_tiles.cu: the bricks' tiles stream through
+// shared memory); float32 voxels on the micro-block layout.
+bool use_mip_tiles(const vr_ctx* ctx, int mode) {
+    if (mode != VR_MODE_MIP || ctx->cube.layout != 1 || ctx->cube.vtype != 0 || ctx->opt_mip_tiles == 0) return false;
+    // measured on C3 (64 GiB, rays 3.5 - 7 voxels apart): 30.7 ms per frame against 14.7 ms of the image-order lockstep
+    // marcher: on request only
+    return ctx->opt_mip_tiles > 0;
+}
+
+// Object-tile prefix of the descriptors (PartialDev::otile0); returns the total.
+int number_object_tiles(const vr_ctx* ctx, PartialDev* v, int n) {
+    int total = 0;
+    for (int i = 0; i < n; ++i) { v[i].otile0 = total; total += object_tiles_of_brick(ctx->cube, v[i].b); }
+    return total;
+}
+
+int ensure_rays(vr_ctx* ctx, int slot) {
+    const size_t need = ray_buffer_bytes(ctx->view.W, ctx->view.H);
+    if (ctx->rays_bytes[slot] >= need) return VR_OK;
+    if (ctx->d_rays[slot]) { VR_CUDA(ctx, cudaDeviceSynchronize()); cudaFree(ctx->d_rays[slot]); }
+    ctx->d_rays[slot] = nullptr; ctx->rays_bytes[slot] = 0;
+    VR_CUDA(ctx, cudaMalloc(&ctx->d_rays[slot], need));
+    ctx->rays_bytes[slot] = need;
+    return VR_OK;
+}
+
+int upload_partials(vr_ctx* ctx, int mode, const vr_partial* hp, int n, bool with_tiles, int* total_tiles, cudaStream_t s, int* object_tiles = nullptr) {
     if (n > (int)ctx->partials_cap) {
         if (ctx->d_partials) cudaFree(ctx->d_partials);
         ctx->d_partials = nullptr;
@@ -427,6 +458,7 @@ int upload_partials(vr_ctx* ctx, int mode, const vr_partial* hp, int n, bool wit
         if (with_tiles) tiles += ((p.w + kTileW - 1) / kTileW) * ((p.h + kTileH - 1) / kTileH);
     }
     if (total_tiles) *total_tiles = tiles;
+    if (object_tiles) *object_tiles = number_object_tiles(ctx, v.data(), n);
     if (n > 0) VR_CUDA(ctx, cudaMemcpyAsync(ctx->d_partials, v.data(), sizeof(PartialDev) * n, cudaMemcpyHostToDevice, s));
     return VR_OK;
 }
@@ -521,6 +553,7 @@ int vr_destroy(vr_ctx* ctx) {
     if (ctx->d_counters) cudaFree(ctx->d_counters);
     if (ctx->d_scratch) cudaFree(ctx->d_scratch);
     if (ctx->d_partials) cudaFree(ctx->d_partials);
+    for (float4* r : ctx->d_rays) if (r) cudaFree(r);
     for (void* b : ctx->ipc_bases) cudaIpcCloseMemHandle(b);
     if (ctx->h_pin) cudaFreeHost(ctx->h_pin);
     if (ctx->d_pin) cudaFree(ctx->d_pin);
@@ -921,11 +954,18 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
         return fail(ctx, VR_ERR_INVALID_ARG, "vr_render_bricks: bad argument");
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
-    int tiles = 0;
-    if ((rc = upload_partials(ctx, mode, hp, n, true, &tiles, s))) return rc;
+    int tiles = 0, otiles = 0;
+    const bool by_tiles = use_mip_tiles(ctx, mode);
+    if ((rc = upload_partials(ctx, mode, hp, n, true, &tiles, s, by_tiles ? &otiles : nullptr))) return rc;
     RenderArgs a{};
     a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = pick_variant(ctx, a.mode, a.skip); a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
     a.counters = ctx->d_counters;
+    if (by_tiles) {
+        if ((rc = ensure_rays(ctx, 4))) return rc;
+        VR_CUDA(ctx, launch_mip_tiles(ctx->cube, ctx->view, ctx->M, a, ctx->d_partials, n, tiles, otiles, ctx->d_rays[4], s));
+        ctx->launches += (n > 0 && tiles > 0) ? 3 : 0;
+        return VR_OK;
+    }
     if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
     VR_CUDA(ctx, launch_render_bricks(ctx->cube, ctx->view, tf_desc(ctx), a, ctx->d_partials, n, tiles, s));
     ctx->launches += (n > 0 && tiles > 0) ? 1 : 0;
@@ -983,13 +1023,21 @@ int vr_render_sortlast(vr_ctx* ctx, int mode, float tau, void* d_arena, size_t a
     }
     *needed_bytes = off;
     if (off > arena_bytes) return fail(ctx, VR_ERR_BUFFER, "vr_render_sortlast: the arena is too small (see *needed_bytes)");
+    const bool by_tiles = use_mip_tiles(ctx, mode);
+    const int otiles = by_tiles ? number_object_tiles(ctx, v, n) : 0;
     if (n > 0) VR_CUDA(ctx, cudaMemcpyAsync(dv, v, sizeof(PartialDev) * n, cudaMemcpyHostToDevice, s));
     RenderArgs a{};
     a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = pick_variant(ctx, a.mode, a.skip);
     a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
     a.counters = ctx->d_counters;
-    if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
-    VR_CUDA(ctx, launch_render_bricks(c, ctx->view, tf_desc(ctx), a, dv, n, tiles, s));
+    if (by_tiles) {
+        if ((rc = ensure_rays(ctx, slot))) return rc;
+        VR_CUDA(ctx, launch_mip_tiles(c, ctx->view, ctx->M, a, dv, n, tiles, otiles, ctx->d_rays[slot], s));
+        ctx->launches += (n > 0 && tiles > 0) ? 2 : 0;
+    } else {
+        if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
+        VR_CUDA(ctx, launch_render_bricks(c, ctx->view, tf_desc(ctx), a, dv, n, tiles, s));
+    }
     VR_CUDA(ctx, launch_composite(ctx->view, mode, dv, n, d_out, bg, s));
     VR_CUDA(ctx, cudaEventRecord(ctx->pin_done[slot], s));                   // both kernels have read the slot
     ctx->launches += (n > 0 && tiles > 0) ? 2 : 1;
@@ -1201,7 +1249,7 @@ int vr_get_plan(vr_ctx* ctx, int mode, int out[3], void* stream) {
     if (rc) return rc;
     if (!out || (mode != VR_MODE_MIP && mode != VR_MODE_EA)) return fail(ctx, VR_ERR_INVALID_ARG, "vr_get_plan: bad argument");
     if ((rc = ensure_tables(ctx, (cudaStream_t)stream))) return rc;
-    out[1] = skip_level(ctx, mode, true); out[0] = pick_variant(ctx, mode, out[1]); out[2] = mode == VR_MODE_EA ? resolve_dense(ctx) : 0;
+    out[1] = skip_level(ctx, mode, true); out[0] = use_mip_tiles(ctx, mode) ? 5 : pick_variant(ctx, mode, out[1]); out[2] = mode == VR_MODE_EA ? resolve_dense(ctx) : 0;
     return VR_OK;
 }
 
@@ -1225,6 +1273,7 @@ int vr_set_option(vr_ctx* ctx, int option, int value) {
         ctx->opt_vtype = value; return VR_OK;                   // takes effect at the next upload / generate / attach
     }
     if (option == VR_OPT_RING) { ctx->opt_ring = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
+    if (option == VR_OPT_MIP_TILES) { ctx->opt_mip_tiles = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_OCCUPANCY) { ctx->opt_occ = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_DENSE) { ctx->opt_dense = value < 0 ? -1 : (value ? 1 : 0); return VR_OK; }
     if (option == VR_OPT_VARIANT) {

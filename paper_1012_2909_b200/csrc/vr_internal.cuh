@@ -74,10 +74,10 @@ struct PartialDev {        // device descriptor of one partial image
     long long pitch;
     void* data;
     int b[3];                         // the brick's grid coordinates (brick = b0 + G0 (b1 + G1 b2)), so that no kernel divides
-    int pad;
+    int otile0;                       // first object tile of this brick in a mip_tiles_kernel launch (vr_mip_tiles.cu)
 };
 inline void set_brick(PartialDev& d, const CubeDesc& c, int brick) {
-    d.brick = brick; d.pad = 0;
+    d.brick = brick; d.otile0 = 0;
     if (brick >= 0 && c.G[0] > 0 && c.G[1] > 0) { d.b[0] = brick % c.G[0]; d.b[1] = (brick / c.G[0]) % c.G[1]; d.b[2] = brick / (c.G[0] * c.G[1]); }
     else d.b[0] = d.b[1] = d.b[2] = 0;
 }
@@ -119,6 +119,11 @@ struct RenderArgs {
 cudaError_t launch_render_global(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, cudaStream_t s);
 cudaError_t launch_render_bricks(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a,
                                  const PartialDev* d_partials, int n, int total_tiles, cudaStream_t s);
+// object-order MIP of per-brick partial images (vr_mip_tiles.cu)
+int object_tiles_of_brick(const CubeDesc& c, const int b[3]);
+size_t ray_buffer_bytes(int W, int H);
+cudaError_t launch_mip_tiles(const CubeDesc& c, const ViewDesc& v, const double M[16], const RenderArgs& a, const PartialDev* d_partials,
+                             int n, int total_pixel_tiles, int total_object_tiles, float4* d_rays, cudaStream_t s);
 cudaError_t launch_touch(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, const RenderArgs& a, const PartialDev* d_partials,
                          int n, int total_tiles, unsigned* d_bitmap, unsigned long long* d_taken, cudaStream_t s);
 cudaError_t launch_touch_count(const unsigned* d_bitmap, long long n_words, unsigned long long* d_out, cudaStream_t s);

@@ -300,6 +300,9 @@ constexpr int kValPitch = 33;
 #ifndef VR_DENSE_TEST
 #define VR_DENSE_TEST 2
 #endif
+#ifndef VR_DENSE_CTAS
+#define VR_DENSE_CTAS 8
+#endif
 #ifndef VR_BEAM_COARSE
 #define VR_BEAM_COARSE true
 #endif
@@ -585,7 +588,7 @@ constexpr int kOccDepth = 2;             // gathers are few here: a shallower ri
 // 8 CTAs per SM (64 registers): the few gathers leave L1 alone, more warps hide the bit lookups (measured:
 // 7 -> 6.83, 8 -> 6.44, 9 -> 7.27 ms on C3)
 template <bool GLOBAL, typename VT = float, bool ASYNC = true, int TEST = 0>
-__global__ void __launch_bounds__(kThreads, ASYNC ? VR_OCC_CTAS : 6)      // gathers held in registers: 80 instead of 64
+__global__ void __launch_bounds__(kThreads, ASYNC ? (TEST == 2 ? VR_DENSE_CTAS : VR_OCC_CTAS) : 6)      // gathers held in registers: 80 instead of 64
 render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                   const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
                   const PartialDev* __restrict__ parts, int n_parts) {

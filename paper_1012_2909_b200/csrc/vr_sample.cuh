@@ -231,17 +231,17 @@ __device__ __forceinline__ void tile_pixel(int& tx, int& ty) {     // warp = 8 x
     ty = (warp >> 1) * 4 + (lane >> 3);
 }
 
-// Shrink the taken interval [ka, kb] of ray r to its members of brick b (O-3): conservative float32
-// bracket of the brick's slab interval, then exact shrink with the membership predicate
-// floor(p_a) / B_a == b_a, which is monotone per axis.
-__device__ __forceinline__ void brick_interval(const CubeDesc& c, const Ray& r, const int b[3], const int lo[3], int& ka, int& kb) {
+// Shrink the taken interval [ka, kb] of ray r to its members of the box of cells [lo, lo + ext), i.e. the samples
+// with lo_a <= floor(p_a) < lo_a + ext_a (O-3: for a brick, floor(p_a) / B_a == b_a): conservative float32
+// bracket of the box's slab interval, then exact shrink with the membership predicate, which is monotone per axis.
+__device__ __forceinline__ void box_interval(const Ray& r, const int lo[3], const int ext[3], int& ka, int& kb) {
     if (ka > kb) return;
     // in units of the lattice index: r.inv = 1 / (step |d|), no division
     float t0 = 0.f, t1 = 3.0e38f;
     bool empty = false;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        float flo = (float)lo[a] - r.margin, fhi = (float)(lo[a] + c.B[a]) + r.margin;
+        float flo = (float)lo[a] - r.margin, fhi = (float)(lo[a] + ext[a]) + r.margin;
         if (r.d[a] == 0.f) { if (r.o[a] < flo || r.o[a] > fhi) empty = true; continue; }
         const float si = r.d[a] > 0.f ? r.inv[a] : -r.inv[a];
         float ta = __fmul_rn(flo - r.o[a], si), tb = __fmul_rn(fhi - r.o[a], si);
@@ -254,16 +254,21 @@ __device__ __forceinline__ void brick_interval(const CubeDesc& c, const Ray& r, 
     float p[3], fl;
     while (ka <= kb) {
         position(r, (float)ka, p);                          // floor(p_a) / B_a == b_a  <=>  lo_a <= floor(p_a) < lo_a + B_a
-        if ((unsigned)(floor_pos(p[0], fl) - lo[0]) < (unsigned)c.B[0] && (unsigned)(floor_pos(p[1], fl) - lo[1]) < (unsigned)c.B[1] &&
-            (unsigned)(floor_pos(p[2], fl) - lo[2]) < (unsigned)c.B[2]) break;
+        if ((unsigned)(floor_pos(p[0], fl) - lo[0]) < (unsigned)ext[0] && (unsigned)(floor_pos(p[1], fl) - lo[1]) < (unsigned)ext[1] &&
+            (unsigned)(floor_pos(p[2], fl) - lo[2]) < (unsigned)ext[2]) break;
         ++ka;
     }
     while (kb >= ka) {
         position(r, (float)kb, p);
-        if ((unsigned)(floor_pos(p[0], fl) - lo[0]) < (unsigned)c.B[0] && (unsigned)(floor_pos(p[1], fl) - lo[1]) < (unsigned)c.B[1] &&
-            (unsigned)(floor_pos(p[2], fl) - lo[2]) < (unsigned)c.B[2]) break;
+        if ((unsigned)(floor_pos(p[0], fl) - lo[0]) < (unsigned)ext[0] && (unsigned)(floor_pos(p[1], fl) - lo[1]) < (unsigned)ext[1] &&
+            (unsigned)(floor_pos(p[2], fl) - lo[2]) < (unsigned)ext[2]) break;
         --kb;
     }
+}
+
+__device__ __forceinline__ void brick_interval(const CubeDesc& c, const Ray& r, const int b[3], const int lo[3], int& ka, int& kb) {
+    (void)b;
+    box_interval(r, lo, c.B, ka, kb);
 }
 
 // Which partial does this CTA's tile belong to, and which pixel of it is this thread's.

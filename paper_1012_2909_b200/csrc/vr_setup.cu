@@ -10,6 +10,7 @@
 //  dilate_kernel             occupancy bit of a trilinear cell = OR of the hot bits of its 8 corners: pure bit
 //                            operations on the hot words of the 8 neighbouring micro-blocks.
 //  classify_cells_kernel     the same O-10 test per macro-cell from its (min,max).
+#include "vr_async.cuh"
 #include "vr_sample.cuh"
 
 namespace vr {
@@ -113,29 +114,6 @@ cell_minmax_lines_kernel(const __grid_constant__ CubeDesc c, int chunks_x) {
 constexpr int kHotLines = 64;      // lines per stage (8 KiB)
 constexpr int kHotStages = 4;
 constexpr int kHotThreads = 256;
-
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-// 1-D bulk asynchronous copy global -> shared (the TMA engine's linear mode; SASS: UBLKCP), completing on an mbarrier
-__device__ __forceinline__ void bulk_load(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
 
 // hot[line] bit s = voxel in slot s of the line maps above the transparent prefix: (v - vmin) * scale > thr.
 // Persistent CTAs; chunk k of a CTA is chunk blockIdx.x + k * gridDim.x of the window's lines.

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libvr.so")
 
 OK, ERR_INVALID_ARG, ERR_BUFFER, ERR_CUDA, ERR_STATE, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 MODE_MIP, MODE_EA = 0, 1
-OPT_SKIP, OPT_VARIANT, OPT_CELL_SKIP, OPT_L2_FETCH, OPT_LAYOUT, OPT_DENSE, OPT_OCCUPANCY, OPT_RING, OPT_VOXEL_TYPE = 1, 2, 3, 4, 5, 6, 7, 8, 9
+OPT_SKIP, OPT_VARIANT, OPT_CELL_SKIP, OPT_L2_FETCH, OPT_LAYOUT, OPT_DENSE, OPT_OCCUPANCY, OPT_RING, OPT_VOXEL_TYPE, OPT_MIP_TILES = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 VOXEL_F32, VOXEL_F16 = 0, 1
 
 EXPORTS = [

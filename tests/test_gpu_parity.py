@@ -29,8 +29,8 @@ def H():
 # (brick, tile); 3: lockstep ray per warp, folding
 # emission-absorption samples in the owning lane "v3s" or through shared memory "v3d", or testing
 # every sample against the occupancy bits first "v3o", or with the gathers in a register ring "v3r"; 4: the occupancy marcher for
-# dense rays, macro-cell runs first "v4o"), with the macro-cell level of the skipping forced on.
-@pytest.fixture(autouse=True, params=["auto", "v0", "v1", "v3s", "v3d", "v3o", "v3r", "v4o"])
+# dense rays, macro-cell runs first "v4o"; "v3t": the per-brick MIP images in object order), with the macro-cell level of the skipping forced on.
+@pytest.fixture(autouse=True, params=["auto", "v0", "v1", "v3s", "v3d", "v3o", "v3r", "v4o", "v3t"])
 def marcher(request, H):
     from paper_1012_2909_b200 import vr
     H.FORCED_OPTIONS.clear()
@@ -40,6 +40,7 @@ def marcher(request, H):
             H.FORCED_OPTIONS[vr.OPT_DENSE] = int(request.param[2] == "d")
             H.FORCED_OPTIONS[vr.OPT_OCCUPANCY] = int(request.param[2] == "o")
             H.FORCED_OPTIONS[vr.OPT_RING] = int(request.param[2] == "r")     # "v3r": sparse fold, gathers through registers
+            H.FORCED_OPTIONS[vr.OPT_MIP_TILES] = int(request.param[2] == "t")  # "v3t": per-brick MIP in object order (vr_mip_tiles.cu); else off
     yield request.param
     H.FORCED_OPTIONS.clear()
 
@@ -506,8 +507,8 @@ def test_config_c2_full_size(H, marcher):
 
 
 def test_config_c3_full_size_64gib(H, marcher):
-    if marcher not in ("auto", "v0"):
-        pytest.skip("full sizes run with the library's choice (what bench.py times) and variant 0")
+    if marcher not in ("auto", "v0", "v3t"):
+        pytest.skip("full sizes run with the library's choice (what bench.py times), variant 0 and the object-order MIP")
     import torch
     torch.cuda.empty_cache()
     free, total = torch.cuda.mem_get_info()
