@@ -62,8 +62,18 @@ def ncu_counters(workload, mode, tf, kernel):
         return None, f"no capture of {kernel} for {workload} {mode} tf-{tf} in profiles/r2_counters.json"
     c = hits[-1]
     n = max(1, len(c["dram_bytes"]))
-    return {"traffic": sum(c["dram_bytes"]) / n, "warp_instructions": sum(c["warp_instructions"]) / n,
-            "source": f"{c['source']} (orbit frames {c.get('frames')}, commit {c.get('commit')})"}, None
+    return {"traffic": sum(c["dram_bytes"]) / n, "warp_instructions": sum(c["warp_instructions"]) / n, "frames": list(c.get("frames", [])),
+            "launches": n, "source": f"{c['source']} (orbit frames {c.get('frames')}, {n} launches, commit {c.get('commit')})"}, None
+
+
+def captured_frames(workload, mode, tf):
+    """Orbit frames of the committed ncu captures of a workload (any kernel): the marcher is timed on them too, so that
+    counters per launch and seconds per launch describe the same launches."""
+    if not os.path.exists(COUNTERS_JSON):
+        return []
+    with open(COUNTERS_JSON) as f:
+        caps = json.load(f).get("captures", [])
+    return sorted({int(fr) for c in caps if c["workload"] == workload and c["mode"] == mode and c.get("tf") == tf for fr in c.get("frames", [])})
 
 
 class ClockSampler(threading.Thread):
@@ -235,7 +245,7 @@ class Job:
             part = pf.render(w.tau)
             if ev:
                 ev[1].record()
-                self.march_events.append((ev[0], ev[1]))
+                self.march_events.append((ev[0], ev[1], frame_index))
                 self.b_brick += 4 * self.brick_voxels() * (sh.end - sh.first)
                 self.partial_bytes += self.H * self.W * self.px_bytes
             if self.slab_only:
@@ -312,7 +322,7 @@ class Job:
             ctx.render_bricks(self.mode, parts, n, w.tau)
             if timed_events:
                 e1.record()
-                self.march_events.append((e0, e1))
+                self.march_events.append((e0, e1, frame_index))
                 # B_brick of this launch: the active in-frustum bricks read once;
                 # nbytes: the partial images written once (16 or 4 B per pixel)
                 self.b_brick += 4 * self.brick_voxels() * n
@@ -439,7 +449,9 @@ def measure(job, steps, warmup, frank, fworld, dist, local_rank, e2e=True):
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
     for i in range(steps):
+        torch.cuda.nvtx.range_push(f"timed_frame_{i}")       # ncu --nvtx --nvtx-include "timed_frame_0/": the launches of one whole frame
         job.step(orbit_frame(w, i, steps, frank, fworld), timed_events=True, one_call=one)
+        torch.cuda.nvtx.range_pop()
     ev1.record()
     barrier()
     clocks = sampler.result()
@@ -455,14 +467,27 @@ def measure(job, steps, warmup, frank, fworld, dist, local_rank, e2e=True):
             job.step(orbit_frame(w, i, steps, frank, fworld), timed_events=True)
         torch.cuda.synchronize()
         job.ctx.reset_counters()
-    march_ms = sum(a.elapsed_time(b) for a, b in job.march_events)
+    march_ms = sum(a.elapsed_time(b) for a, b, _ in job.march_events)
     n_march = len(job.march_events)
+    by_frame = {}
+    if one:
+        # ... and on the orbit frames of the committed ncu captures (roofline.traffic / roofline.issue divide counters of
+        # those launches by seconds of the same launches); kept apart from the means above
+        keep = (job.march_events, job.b_brick, job.partial_bytes)
+        job.reset_events()
+        for f in captured_frames(w.name, job.mode_name, job.tf_name):
+            job.step(f, timed_events=True)
+        torch.cuda.synchronize()
+        for a, b, f in job.march_events:
+            by_frame.setdefault(f, []).append(a.elapsed_time(b))
+        job.march_events, job.b_brick, job.partial_bytes = keep
+        job.ctx.reset_counters()
     ms_total, (nominal, taken, launches) = reduce_run(
         dist, "cuda", ms_total, [cnt["nominal_samples"], cnt["taken_samples"], cnt["kernel_launches"]])
     res = {"ms_total": ms_total, "frame_ms": frame_ms, "nominal": nominal, "taken": taken, "launches": launches,
            "launches_per_step": n_march / max(1, min(steps, 6) if one else steps),
            "march_ms": march_ms, "n_march": n_march, "b_brick": job.b_brick, "partial_bytes": job.partial_bytes,
-           "clocks": clocks, "steps": steps, "fworld": fworld}
+           "march_by_frame": by_frame, "clocks": clocks, "steps": steps, "fworld": fworld}
     if not e2e:
         return res
     # ---- e2e: the same step through the public API with HOST buffers in the timed region: the
@@ -549,15 +574,26 @@ def roofline(job, m, touch_frames, peak, peak_src):
     cap, why = ncu_counters(job.w.name, job.mode_name, job.tf_name, kernel)
     clocks = m["clocks"]
     if cap:
+        # seconds per launch of the very launches that were captured: the same orbit frames, timed alone in this run (a tiled
+        # frame: the first `launches` panels of the frame if fewer than all were captured - named in the capture's title)
+        # (a panel that no brick meets launches nothing: the captured launches of a frame are fewer than its panels, so the
+        # frames' summed marcher time is divided by the number of CAPTURED launches, which are whole frames)
+        by = m.get("march_by_frame", {})
+        have = all(f in by for f in cap["frames"]) and cap["frames"]
+        cap_s = sum(t for f in cap["frames"] for t in by[f]) / cap["launches"] * 1e-3 if have else None
         out["traffic"] = cap["traffic"]
         out["traffic_source"] = cap["source"]
-        out["dram_gbs_from_traffic"] = cap["traffic"] / launch_s / 1e9 if launch_s > 0 else None
-        if clocks.get("sm_mhz"):
-            ipeak = ISSUE_SLOTS_PER_CLOCK * clocks["sm_mhz"] * 1e6 / 1e9
-            out["issue"] = {"bound": "alu", "achieved": cap["warp_instructions"] / launch_s / 1e9, "peak": ipeak,
-                            "unit": "G warp-instructions/s", "frac": cap["warp_instructions"] / launch_s / 1e9 / ipeak,
-                            "note": "warp instructions per launch from the committed ncu capture / live launch time; peak = 148 "
-                                    "SMs x 4 schedulers x the SM clock sampled during the run"}
+        out["captured_launch_ms"] = cap_s * 1e3 if cap_s else None
+        if cap_s:
+            out["dram_gbs_from_traffic"] = cap["traffic"] / cap_s / 1e9
+            if clocks.get("sm_mhz"):
+                ipeak = ISSUE_SLOTS_PER_CLOCK * clocks["sm_mhz"] * 1e6 / 1e9
+                out["issue"] = {"bound": "alu", "achieved": cap["warp_instructions"] / cap_s / 1e9, "peak": ipeak,
+                                "unit": "G warp-instructions/s", "frac": cap["warp_instructions"] / cap_s / 1e9 / ipeak,
+                                "note": "warp instructions per launch from the committed ncu capture / seconds per launch of the same orbit "
+                                        "frames timed alone in this run; peak = 148 SMs x 4 schedulers x the SM clock sampled during the run"}
+        else:
+            out["traffic_note"] = "the captured orbit frames were not timed in this run (sharded / slab runs): no rate derived from the capture"
     else:
         out["traffic"] = None
         out["traffic_note"] = why

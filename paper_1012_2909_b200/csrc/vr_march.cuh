@@ -300,6 +300,9 @@ constexpr int kValPitch = 33;
 #ifndef VR_DENSE_TEST
 #define VR_DENSE_TEST 2
 #endif
+#ifndef VR_PIN_OCC0
+#define VR_PIN_OCC0 1
+#endif
 #ifndef VR_DENSE_CTAS
 #define VR_DENSE_CTAS 8
 #endif
@@ -627,7 +630,9 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
     unsigned n_taken = 0;
     // the occupancy word of a sample (0 if its brick is inactive) and the sample's bit in it; 64-bit
     // brick offsets: a sharded cube's global brick ids times the words per brick can pass 2^32
-    auto locate = [&](const float tk, unsigned& word, unsigned& bit) {
+    // `valid` false: the sample lies outside this lane's interval - the address arithmetic runs anyway (it cannot fault),
+    // only the load is predicated: no branch around the ~25 instructions of a test (non-GLOBAL; 5 of ~30 were the branch)
+    auto locate = [&](const float tk, unsigned& word, unsigned& bit, const bool valid = true) {
         float fl;
         const int iv[3] = {floor_pos(__fmaf_rn(tk, r.d[0], r.o[0]), fl), floor_pos(__fmaf_rn(tk, r.d[1], r.o[1]), fl),
                            floor_pos(__fmaf_rn(tk, r.d[2], r.o[2]), fl)};
@@ -643,7 +648,8 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
             lx = (unsigned)(iv[0] - lo0[0]); ly = (unsigned)(iv[1] - lo0[1]); lz = (unsigned)(iv[2] - lo0[2]);
             occb = occ0;
         }
-        word = __ldg(occb + occ_word_index(c, lx, ly, lz));   // an L1 hit while the ray stays in its 4 x 4 x 2 cells
+        word = 0u;
+        if (valid) word = __ldg(occb + occ_word_index(c, lx, ly, lz));   // an L1 hit while the ray stays in its 4 x 4 x 2 cells
         bit = occ_bit_index(lx, ly, lz);
     };
     // march the taken samples [ka, kb] of every lane's ray (all members of brick bid0 unless GLOBAL) into acc
@@ -791,8 +797,10 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                 for (int u = 0; u < VR_RUNS_GROUP; ++u) { jj[u] = bits ? __ffs(bits) - 1 : -1; bits &= bits - 1; }
 #pragma unroll
                 for (int u = 0; u < VR_RUNS_GROUP; ++u) {
-                    word[u] = 0u; bit[u] = 0u;
-                    if (jj[u] >= 0 && ((cand >> jj[u]) & 1u)) locate(__fmul_rn((float)(kbase + jj[u]), r.step), word[u], bit[u]);
+                    if constexpr (GLOBAL) {
+                        word[u] = 0u; bit[u] = 0u;
+                        if (jj[u] >= 0 && ((cand >> jj[u]) & 1u)) locate(__fmul_rn((float)(kbase + jj[u]), r.step), word[u], bit[u]);
+                    } else locate(__fmul_rn((float)(kbase + max(jj[u], 0)), r.step), word[u], bit[u], jj[u] >= 0 && ((cand >> (jj[u] & 31)) & 1u));
                 }
 #pragma unroll
                 for (int u = 0; u < VR_RUNS_GROUP; ++u) my_act |= ((word[u] >> bit[u]) & 1u) << (jj[u] & 31);
@@ -821,8 +829,10 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                 unsigned word[VR_OCC_GROUP], bit[VR_OCC_GROUP];
 #pragma unroll
                 for (int u = 0; u < VR_OCC_GROUP; ++u) {
-                    word[u] = 0u; bit[u] = 0u;                       // out of this ray's range: reads as idle
-                    if (j + u >= j0 && j + u <= j1) locate(__fmul_rn((float)(kbase + j + u), r.step), word[u], bit[u]);
+                    if constexpr (GLOBAL) {
+                        word[u] = 0u; bit[u] = 0u;                   // out of this ray's range: reads as idle
+                        if (j + u >= j0 && j + u <= j1) locate(__fmul_rn((float)(kbase + j + u), r.step), word[u], bit[u]);
+                    } else locate(__fmul_rn((float)(kbase + j + u), r.step), word[u], bit[u], j + u >= j0 && j + u <= j1);
                 }
 #pragma unroll
                 for (int u = 0; u < VR_OCC_GROUP; ++u) my_act |= ((word[u] >> bit[u]) & 1u) << ((j + u) & 31);
@@ -952,7 +962,13 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                     lo0[0] = b[0] * c.B[0]; lo0[1] = b[1] * c.B[1]; lo0[2] = b[2] * c.B[2];
                     br0 = brick_ref<LAYOUT, VT>(c, bid0, lo0);
                     occ0 = c.occ + (long long)bid0 * c.occ_words_per_brick;
+#if VR_PIN_OCC0
+                    asm volatile("" : "+l"(occ0));          // kept in two registers: otherwise re-derived from the brick id at every sample (3 instructions of ~33)
+#endif
                     cbits0 = c.cell_bits + (long long)bid0 * c.cell_words_per_brick;
+#if VR_PIN_OCC0
+                    if constexpr (TEST == 2) asm volatile("" : "+l"(cbits0));
+#endif
                     ka = mine ? r.k0 : 0; kb = mine ? r.k1 : -1;
                     brick_interval(c, r, b, lo0, ka, kb);
                     march();
