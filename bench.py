@@ -586,6 +586,7 @@ def roofline(job, m, touch_frames, peak, peak_src):
         out["captured_launch_ms"] = cap_s * 1e3 if cap_s else None
         if cap_s:
             out["dram_gbs_from_traffic"] = cap["traffic"] / cap_s / 1e9
+            out["traffic_frac"] = out["dram_gbs_from_traffic"] / peak if peak else None      # what ncu saw the launch move, over the HBM peak
             if clocks.get("sm_mhz"):
                 ipeak = ISSUE_SLOTS_PER_CLOCK * clocks["sm_mhz"] * 1e6 / 1e9
                 out["issue"] = {"bound": "alu", "achieved": cap["warp_instructions"] / cap_s / 1e9, "peak": ipeak,
