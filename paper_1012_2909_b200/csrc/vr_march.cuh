@@ -658,12 +658,7 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
     __syncwarp();
     alive = ka <= kb; stopped = false; k_end = kb; n_taken = 0;
     acc.C[0] = acc.C[1] = acc.C[2] = 0.f; acc.A = 0.f; acc.m = -INFINITY;
-    int K0 = alive ? ka : 0x7fffffff, K1 = alive ? kb : -1;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        K0 = min(K0, __shfl_xor_sync(0xffffffffu, K0, o));
-        K1 = max(K1, __shfl_xor_sync(0xffffffffu, K1, o));
-    }
+    const int K0 = __reduce_min_sync(0xffffffffu, alive ? ka : 0x7fffffff), K1 = __reduce_max_sync(0xffffffffu, alive ? kb : -1);
     int cur = ka, run_left = 0;                             // TEST 1: next lattice index to classify, rest of its macro-cell run
     bool run_on = false;
     unsigned beam_flags = 0u;                               // TEST 2: chunks of the current group of 4 whose beam meets a non-zero word
@@ -807,12 +802,7 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
             }
         } else {
             int j0 = mine ? max(ka, kbase) - kbase : 32, j1 = mine ? min(kb, kbase + 31) - kbase : -1;
-            int J0 = j0, J1 = j1;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                J0 = min(J0, __shfl_xor_sync(0xffffffffu, J0, o));
-                J1 = max(J1, __shfl_xor_sync(0xffffffffu, J1, o));
-            }
+            const int J0 = __reduce_min_sync(0xffffffffu, j0), J1 = __reduce_max_sync(0xffffffffu, j1);
 #if VR_OCC_GROUP <= 1
             unsigned word = 0u, bit = 0u;                            // of sample j
             if (J0 >= j0 && J0 <= j1) locate(__fmul_rn((float)(kbase + J0), r.step), word, bit);
