@@ -483,9 +483,10 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
             const float val = trilinear(v, S.w[0], S.w[1], S.w[2]);       // idle lanes: stale values, never used
             const unsigned done_bits = __ballot_sync(0xffffffffu, !S.idle);
             if (!EA) {
-                float m = S.idle ? -INFINITY : val;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+                // warp maximum by one redux.sync on a key that orders floats as integers (no NaN here: refused at upload)
+                const int bits = __float_as_int(S.idle ? -INFINITY : val);
+                const int top = __reduce_max_sync(0xffffffffu, bits ^ ((bits >> 31) & 0x7fffffff));
+                const float m = __int_as_float(top ^ ((top >> 31) & 0x7fffffff));
                 if (lane == S.rc) { acc.m = fmaxf(acc.m, m); n_taken += __popc(done_bits); }
                 return;
             }
