@@ -387,7 +387,8 @@ render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vie
         const int b[3] = {part.b[0], part.b[1], part.b[2]};
         brick_interval(c, r, b, lo0, ka, kb);
     }
-    const BrickRefT<VT> br0 = brick_ref<LAYOUT, VT>(c, bid0, lo0);
+    BrickRefT<VT> br0 = brick_ref<LAYOUT, VT>(c, bid0, lo0);
+    if (!GLOBAL) asm volatile("" : "+l"(br0.base));         // the brick's base stays in two registers (else re-derived from the brick id per sample)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float* vals = vals_all[VALS ? warp : 0];
     float4* rays = rays_all[warp];
