@@ -24,8 +24,9 @@ template <int MODE, int LAYOUT, bool JUMP = false, typename VT = float>
 __device__ __forceinline__ bool march_interval(const CubeDesc& c, const Ray& r, const TFDesc& T, const RenderArgs& A,
                                                const float4* tab, int bid, const int lo[3], int k, int ke,
                                                Accum& acc, Stats& st) {
-    const BrickRefT<VT> b = brick_ref<LAYOUT, VT>(c, bid, lo);
+    BrickRefT<VT> b = brick_ref<LAYOUT, VT>(c, bid, lo);
     const unsigned* occ = (MODE == VR_MODE_EA && LAYOUT == 1 && A.skip >= 3) ? c.occ + (long long)bid * c.occ_words_per_brick : nullptr;
+    asm volatile("" : "+l"(b.base), "+l"(occ));             // both stay in registers (else re-derived from the brick id per sample)
     const int S8[3] = {kCell, kCell, kCell};
     // a jump out of an idle micro-block costs about as much as testing 3 samples one by one: worth it when
     // the block holds more than that (measured: step 0.25 -> C4 29.6 to 26.2 ms; step 0.5 -> C2 0.70 to 0.76 ms),
