@@ -954,6 +954,9 @@ render_occ_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ Vi
                     const int b[3] = {P.b[0], P.b[1], P.b[2]};
                     lo0[0] = b[0] * c.B[0]; lo0[1] = b[1] * c.B[1]; lo0[2] = b[2] * c.B[2];
                     br0 = brick_ref<LAYOUT, VT>(c, bid0, lo0);
+#if VR_PIN_OCC0
+                    asm volatile("" : "+l"(br0.base));
+#endif
                     occ0 = c.occ + (long long)bid0 * c.occ_words_per_brick;
 #if VR_PIN_OCC0
                     asm volatile("" : "+l"(occ0));          // kept in two registers: otherwise re-derived from the brick id at every sample (3 instructions of ~33)
