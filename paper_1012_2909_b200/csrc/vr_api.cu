@@ -332,17 +332,20 @@ int resolve_dense(const vr_ctx* ctx) {
 }
 
 // Lockstep marcher: gathers through registers (1) or through the cp.async ring in shared memory (0).
-// Measured (vr_march.cu, REGS): registers win when the rays run mostly along z, the short axis of the
-// 4 x 4 x 2 micro-blocks, where a request meets the most sectors.
-int resolve_ring(const vr_ctx* ctx) {
+// Measured over the C3 orbit with the final build (vr_march.cuh, REGS): MIP is faster with registers whatever the view
+// (12.9 vs 15.2 ms, mean of 12 azimuths); emission-absorption with a dense table is faster with the cp.async ring only
+// where the rays run mostly along x, the axis along which consecutive lines are contiguous (16.0 vs 17.0 ms), and with
+// registers elsewhere (18.6 vs 22.5 ms).
+int resolve_ring(const vr_ctx* ctx, int mode) {
     if (ctx->cube.vtype == 1) return 1;                      // float16 voxels: plain loads only (vr_march_h.cu)
     if (ctx->opt_ring >= 0) return ctx->opt_ring;
     if (ctx->cube.layout != 1) return 0;
+    if (mode == VR_MODE_MIP) return 1;
     const double* Mi = ctx->Minv;
     double pn[4], pf[4], d[3];
     for (int r = 0; r < 4; ++r) { pn[r] = -Mi[4 * r + 2] + Mi[4 * r + 3]; pf[r] = Mi[4 * r + 2] + Mi[4 * r + 3]; }   // central pixel, near / far
     for (int a = 0; a < 3; ++a) d[a] = std::fabs(pf[a] / pf[3] - pn[a] / pn[3]);
-    return (std::isfinite(d[2]) && d[2] > d[0] && d[2] > d[1]) ? 1 : 0;
+    return (std::isfinite(d[0]) && d[0] > d[1] && d[0] > d[2]) ? 0 : 1;
 }
 
 TFDesc tf_desc(const vr_ctx* ctx) {
@@ -793,7 +796,7 @@ int vr_render_mip(vr_ctx* ctx, float* d_out, float* d_out_rgba, float miss, void
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
-    a.mode = VR_MODE_MIP; a.tau = 2.f; a.miss = miss; a.skip = skip_level(ctx, a.mode); a.variant = pick_variant(ctx, a.mode, a.skip); a.ring = resolve_ring(ctx);
+    a.mode = VR_MODE_MIP; a.tau = 2.f; a.miss = miss; a.skip = skip_level(ctx, a.mode); a.variant = pick_variant(ctx, a.mode, a.skip); a.ring = resolve_ring(ctx, a.mode);
     a.out = d_out; a.out_rgba = d_out_rgba; a.counters = ctx->d_counters;
     VR_CUDA(ctx, launch_render_global(ctx->cube, ctx->view, tf_desc(ctx), a, s));
     ctx->launches += 1;
@@ -810,7 +813,7 @@ int vr_render_ea(vr_ctx* ctx, float* d_out, const float bg[4], float tau, void* 
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = ensure_tables(ctx, s))) return rc;
     RenderArgs a{};
-    a.mode = VR_MODE_EA; a.tau = tau; a.skip = skip_level(ctx, a.mode); a.variant = pick_variant(ctx, a.mode, a.skip); a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
+    a.mode = VR_MODE_EA; a.tau = tau; a.skip = skip_level(ctx, a.mode); a.variant = pick_variant(ctx, a.mode, a.skip); a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx, a.mode);
     for (int i = 0; i < 4; ++i) a.bg[i] = bg[i];
     a.out = d_out; a.counters = ctx->d_counters;
     if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
@@ -958,7 +961,7 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
     const bool by_tiles = use_mip_tiles(ctx, mode);
     if ((rc = upload_partials(ctx, mode, hp, n, true, &tiles, s, by_tiles ? &otiles : nullptr))) return rc;
     RenderArgs a{};
-    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = pick_variant(ctx, a.mode, a.skip); a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
+    a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = pick_variant(ctx, a.mode, a.skip); a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx, a.mode);
     a.counters = ctx->d_counters;
     if (by_tiles) {
         if ((rc = ensure_rays(ctx, 4))) return rc;
@@ -1028,7 +1031,7 @@ int vr_render_sortlast(vr_ctx* ctx, int mode, float tau, void* d_arena, size_t a
     if (n > 0) VR_CUDA(ctx, cudaMemcpyAsync(dv, v, sizeof(PartialDev) * n, cudaMemcpyHostToDevice, s));
     RenderArgs a{};
     a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = pick_variant(ctx, a.mode, a.skip);
-    a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
+    a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx, a.mode);
     a.counters = ctx->d_counters;
     if (by_tiles) {
         if ((rc = ensure_rays(ctx, slot))) return rc;
@@ -1139,7 +1142,7 @@ int vr_measure_touch(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
     if ((rc = upload_partials(ctx, mode, hp, n, true, &tiles, s))) return rc;
     RenderArgs a{};
     a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = pick_variant(ctx, a.mode, a.skip);
-    a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx);
+    a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx, a.mode);
     if ((rc = ensure_occ(ctx, a.skip, s))) return rc;
     size_t bytes = 0;
     vr_touch_layout(ctx, &bytes);
