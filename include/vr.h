@@ -150,6 +150,18 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* h_partials, int n,
  * max then miss value bg[0] (MIP), into the viewport of d_out. */
 int vr_composite_bricks(vr_ctx* ctx, int mode, const vr_partial* h_partials, int n, float* d_out,
                         const float bg[4], void* stream);
+/* The same fold for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): vr_composite_bricks keeps the device copy of the descriptors in a buffer it cudaMallocs on its first
+ * call and whenever n grows; this variant keeps it in a static __device__ array of the library instead (224 KiB, held by
+ * every GPU that loads libvr until the process exits) and calls no cudaMalloc, cudaFree or other allocating routine, on
+ * the device or on the host.  Arguments, result (bit for bit) and error behaviour as vr_composite_bricks, plus: n above
+ * VR_STATIC_MAX_PARTIALS is refused with VR_ERR_BUFFER (vr_last_error says so) and nothing is launched.  All calls on a
+ * device share the one array: a call rewrites entries [0, n) before its kernel reads them and reads no others, so nothing
+ * needs clearing between calls; calls that overlap on the GPU (different streams without an event between them, or
+ * different contexts of one device) race on it - order them. */
+#define VR_STATIC_MAX_PARTIALS 4096
+int vr_composite_bricks_static(vr_ctx* ctx, int mode, const vr_partial* h_partials, int n, float* d_out,
+                               const float bg[4], void* stream);
 
 /* The four calls above for the current view in one: the resident bricks that can contribute are sorted front to back
  * (O-9), their partial images are packed into d_arena (device, 256-byte aligned, arena_bytes; *needed_bytes receives

@@ -18,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "_obj")
 LIB = os.path.join(HERE, "libvr.so")
 SOURCES = ["vr_api.cu", "vr_cube.cu", "vr_march.cu", "vr_march_h.cu", "vr_setup.cu", "vr_touch.cu", "vr_mip_tiles.cu",
-           "vr_composite.cu", "vr_overlay.cu", "vr_pyramid.cu"]
+           "vr_composite.cu", "vr_composite_static.cu", "vr_overlay.cu", "vr_pyramid.cu"]
 HEADERS = [os.path.join(CSRC, "vr_internal.cuh"), os.path.join(CSRC, "vr_sample.cuh"), os.path.join(CSRC, "vr_march.cuh"), os.path.join(CSRC, "vr_async.cuh"),
            os.path.join(os.path.dirname(HERE), "include", "vr.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

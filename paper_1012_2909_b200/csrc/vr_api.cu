@@ -1060,6 +1060,42 @@ int vr_composite_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, floa
     return VR_OK;
 }
 
+int vr_composite_bricks_static(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float* d_out, const float bg[4], void* stream) {
+    VR_RANGE();
+    int rc = check_render_state(ctx, false);                 // makes the context's device current
+    if (rc) return rc;
+    if (n < 0 || (n > 0 && !hp) || !d_out || !bg || (mode != VR_MODE_MIP && mode != VR_MODE_EA))
+        return fail(ctx, VR_ERR_INVALID_ARG, "vr_composite_bricks_static: bad argument");
+    if (n > kStaticMaxPartials)
+        return fail(ctx, VR_ERR_BUFFER, "vr_composite_bricks_static: " + std::to_string(n) + " partial images exceed the static maximum of " +
+                                        std::to_string(kStaticMaxPartials) + " (VR_STATIC_MAX_PARTIALS): use vr_composite_bricks");
+    cudaStream_t s = (cudaStream_t)stream;
+    const int W = ctx->view.W, H = ctx->view.H;
+    for (int i = 0; i < n; ++i) {                            // every entry is checked before anything is enqueued
+        const vr_partial& p = hp[i];
+        if (p.w <= 0 || p.h <= 0 || p.x0 < 0 || p.y0 < 0 || p.x0 + p.w > W || p.y0 + p.h > H || !p.d_data || p.pitch_px < (size_t)p.w)
+            return fail(ctx, VR_ERR_INVALID_ARG, "bad vr_partial entry");
+        if (((uintptr_t)p.d_data & (mode == VR_MODE_EA ? 15 : 3)) != 0)
+            return fail(ctx, VR_ERR_INVALID_ARG, "vr_partial.d_data misaligned");
+    }
+    constexpr int kStage = 128;                              // descriptors converted per copy, on the stack: no host allocation
+    PartialDev stage[kStage];
+    for (int first = 0; first < n; first += kStage) {
+        const int cnt = std::min(kStage, n - first);
+        for (int i = 0; i < cnt; ++i) {
+            const vr_partial& p = hp[first + i];
+            PartialDev& d = stage[i];
+            d.brick = p.brick; d.b[0] = d.b[1] = d.b[2] = 0; d.otile0 = 0;   // the fold reads rectangles and pixels only
+            d.x0 = p.x0; d.y0 = p.y0; d.w = p.w; d.h = p.h; d.tile0 = 0;
+            d.pitch = (long long)p.pitch_px; d.data = p.d_data;
+        }
+        VR_CUDA(ctx, static_partials_store(first, stage, cnt, s));
+    }
+    VR_CUDA(ctx, launch_composite_static(ctx->view, mode, n, d_out, bg, s));
+    ctx->launches += 1;
+    return VR_OK;
+}
+
 int vr_ipc_export(vr_ctx* ctx, const void* d_ptr, unsigned char handle[64], size_t* offset) {
     if (!ctx) return VR_ERR_INVALID_ARG;
     enter(ctx);

@@ -129,6 +129,10 @@ cudaError_t launch_touch(const CubeDesc& c, const ViewDesc& v, const TFDesc& t, 
 cudaError_t launch_touch_count(const unsigned* d_bitmap, long long n_words, unsigned long long* d_out, cudaStream_t s);
 cudaError_t launch_composite(const ViewDesc& v, int mode, const PartialDev* d_partials, int n, float* out,
                              const float bg[4], cudaStream_t s);
+// vr_composite_bricks_static (vr_composite_static.cu): the descriptors live in a static __device__ array of the library
+constexpr int kStaticMaxPartials = VR_STATIC_MAX_PARTIALS;
+cudaError_t static_partials_store(int first, const PartialDev* h, int count, cudaStream_t s);
+cudaError_t launch_composite_static(const ViewDesc& v, int mode, int n, float* out, const float bg[4], cudaStream_t s);
 constexpr int kMaxPeers = 32;
 struct PeerList { const void* in[kMaxPeers]; void* out[kMaxPeers]; int n, n_out; };   // `in` already in fold order
 cudaError_t launch_fold_peers(const PeerList& L, int mode, int width, long long pitch, int y0, int rows, long long out_pitch,

@@ -18,6 +18,7 @@ OK, ERR_INVALID_ARG, ERR_BUFFER, ERR_CUDA, ERR_STATE, ERR_UNSUPPORTED = 0, -1, -
 MODE_MIP, MODE_EA = 0, 1
 OPT_SKIP, OPT_VARIANT, OPT_CELL_SKIP, OPT_L2_FETCH, OPT_LAYOUT, OPT_DENSE, OPT_OCCUPANCY, OPT_RING, OPT_VOXEL_TYPE, OPT_MIP_TILES = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 VOXEL_F32, VOXEL_F16 = 0, 1
+STATIC_MAX_PARTIALS = 4096          # VR_STATIC_MAX_PARTIALS: partial images vr_composite_bricks_static folds per call
 
 EXPORTS = [
     "vr_create", "vr_destroy", "vr_last_error", "vr_status_string", "vr_cube_layout",
@@ -27,7 +28,7 @@ EXPORTS = [
     "vr_get_counters", "vr_reset_counters", "vr_set_option", "vr_get_plan",
     "vr_set_brick_window", "vr_window_layout", "vr_sort_groups", "vr_overlay_catalogue", "vr_overlay_pick", "vr_pyramid_layout", "vr_build_pyramid",
     "vr_touch_layout", "vr_measure_touch", "vr_touch_count", "vr_fold_peers", "vr_ipc_export", "vr_ipc_open",
-    "vr_cube_layout_typed", "vr_render_sortlast", "vr_meta_static_bytes",
+    "vr_cube_layout_typed", "vr_render_sortlast", "vr_meta_static_bytes", "vr_composite_bricks_static",
 ]
 
 
@@ -93,6 +94,7 @@ def load():
     lib.vr_partial_layout.argtypes = [vp, C.c_int, ip, C.c_int, C.POINTER(Partial), C.POINTER(sz)]
     lib.vr_render_bricks.argtypes = [vp, C.c_int, C.POINTER(Partial), C.c_int, C.c_float, vp]
     lib.vr_composite_bricks.argtypes = [vp, C.c_int, C.POINTER(Partial), C.c_int, vp, fp, vp]
+    lib.vr_composite_bricks_static.argtypes = [vp, C.c_int, C.POINTER(Partial), C.c_int, vp, fp, vp]
     lib.vr_get_counters.argtypes = [vp, C.POINTER(Counters), vp]
     lib.vr_reset_counters.argtypes = [vp, vp]
     lib.vr_set_option.argtypes = [vp, C.c_int, C.c_int]
@@ -291,6 +293,11 @@ class Context:
     def composite_bricks(self, mode, parts, n, d_out, bg=(0, 0, 0, 0), stream=None):
         b = (C.c_float * 4)(*[float(x) for x in bg])
         self._check(self._lib.vr_composite_bricks(self._h, int(mode), parts, int(n), C.c_void_p(d_out.data_ptr()), b, _stream(stream)))
+
+    def composite_bricks_static(self, mode, parts, n, d_out, bg=(0, 0, 0, 0), stream=None):
+        """vr_composite_bricks without any allocation: descriptors in the library's static device array (n <= STATIC_MAX_PARTIALS)."""
+        b = (C.c_float * 4)(*[float(x) for x in bg])
+        self._check(self._lib.vr_composite_bricks_static(self._h, int(mode), parts, int(n), C.c_void_p(d_out.data_ptr()), b, _stream(stream)))
 
     def render_sortlast(self, mode, d_arena, d_out, bg=(0, 0, 0, 0), tau=0.99, stream=None):
         """One sort-last frame / panel in one call.  Returns (ok, needed_bytes): ok is False if d_arena (a uint8 CUDA tensor
