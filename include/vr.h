@@ -168,7 +168,7 @@ int vr_composite_bricks_static(vr_ctx* ctx, int mode, const vr_partial* h_partia
  * what this view needs: VR_ERR_BUFFER and nothing launched if that is more), rendered (S2-S4) and folded into the
  * viewport of d_out (S5).  Same kernels and the same frame as the four calls; the descriptors travel once, through a
  * pinned staging ring of the library, so a frame (or one panel of a tiled frame) costs one call and no host allocation.
- * Up to 4 calls may be in flight on DIFFERENT streams (e.g. the panels of a tiled frame, each with its own arena
+ * Up to 32 calls may be in flight on DIFFERENT streams (e.g. the panels of a tiled frame, each with its own arena
  * and viewport): each call has its own descriptor slot; the classification a new table needs is enqueued by the
  * first call that sees it, so order that call before the others (one event). */
 int vr_render_sortlast(vr_ctx* ctx, int mode, float ert_tau, void* d_arena, size_t arena_bytes, size_t* needed_bytes,

@@ -1,6 +1,9 @@
 // Host side of libvr: the C ABI of include/vr.h.  Per-view / per-transfer-function setup
 // (matrix inverse in fp64, opacity-corrected table, brick classification
 // against the table, visibility keys + sort) and the launch plumbing.  No torch types.
+#ifndef VR_PIN_SLOTS
+#define VR_PIN_SLOTS 32   // descriptor slots of vr_render_sortlast (calls the host may have in flight)
+#endif
 #include <algorithm>
 #include <climits>
 #include <cmath>
@@ -13,6 +16,9 @@
 #include "vr_internal.cuh"
 
 using namespace vr;
+
+// One corner of a brick under the current view: NDC coordinates, or `behind` (w <= 0: no projection).
+struct Corner { double xn, yn, zn; bool behind; };
 
 struct vr_ctx {
     int device = 0;
@@ -43,8 +49,9 @@ struct vr_ctx {
     int opt_mip_tiles = -1;
     // object-order MIP (vr_mip_tiles.cu): one ray record per view pixel, one buffer per descriptor slot of
     // vr_render_sortlast (calls in flight on different streams) plus one for vr_render_bricks; grown on demand
-    float4* d_rays[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
-    size_t rays_bytes[5] = {0, 0, 0, 0, 0};
+    static constexpr int kPinSlots = VR_PIN_SLOTS;
+    float4* d_rays[kPinSlots + 1] = {};
+    size_t rays_bytes[kPinSlots + 1] = {};
     int opt_vtype = 0;                   // VR_OPT_VOXEL_TYPE: 0 float32, 1 float16
     float x_clear = -INFINITY;
     double active_cell_fraction = 1.0;   // macro-cells active against the current table (EA)
@@ -57,13 +64,16 @@ struct vr_ctx {
     int win_lo = 0, win_hi = -1;         // vr_set_brick_window (hi < 0: all bricks)
     std::vector<void*> ipc_bases;        // peer allocations opened by vr_ipc_open
     // vr_render_sortlast: descriptors staged through a small ring of pinned slots (no allocation, no pageable copy per frame)
-    static constexpr int kPinSlots = 4;
+    // (32 slots: the host may run a whole tiled frame of 25 panels ahead of the GPU; with 4 it stalled at every frame start
+    // until the GPU had finished the last panels of the frame before: C4 end to end 19.9 ms against 17.5 on the device)
     PartialDev* h_pin = nullptr;
     PartialDev* d_pin = nullptr;         // the same slots on the device: calls on different streams do not share descriptors
     size_t pin_cap = 0;                  // descriptors per slot
-    cudaEvent_t pin_done[kPinSlots] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t pin_done[kPinSlots] = {};
     int pin_next = 0;
     std::vector<std::pair<int, int>> keyed;   // scratch: (visibility key, brick)
+    std::vector<int> key_count;               // scratch of the counting sort in vr_render_sortlast
+    std::vector<Corner> corner_grid;          // scratch: the brick grid's corners under the current view
     std::vector<int> keys;
 };
 
@@ -355,32 +365,27 @@ TFDesc tf_desc(const vr_ctx* ctx) {
     return t;
 }
 
-// Screen rectangle (view pixels, clipped) that holds every pixel whose ray can meet brick b.
+inline Corner project_corner(const double* M, double x, double y, double z) {
+    Corner k{0.0, 0.0, 0.0, false};
+    const double X = M[0] * x + M[1] * y + M[2] * z + M[3];
+    const double Y = M[4] * x + M[5] * y + M[6] * z + M[7];
+    const double Z = M[8] * x + M[9] * y + M[10] * z + M[11];
+    const double Wc = M[12] * x + M[13] * y + M[14] * z + M[15];
+    if (!(Wc > 1e-9)) { k.behind = true; return k; }
+    k.xn = X / Wc; k.yn = Y / Wc; k.zn = Z / Wc;
+    return k;
+}
+
+// Screen rectangle (view pixels, clipped) that holds every pixel whose ray can meet a brick with these 8 corners.
 // Returns false if the brick is outside the frustum.
-bool brick_rect(const vr_ctx* ctx, int bid, int rect[4]) {
-    const CubeDesc& c = ctx->cube;
-    const int W = ctx->view.W, H = ctx->view.H;
-    int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
-    double lo[3], hi[3];
-    for (int a = 0; a < 3; ++a) {
-        lo[a] = (double)b[a] * c.B[a];
-        hi[a] = std::min((double)(b[a] + 1) * c.B[a], (double)(c.N[a] - 1));
-        if (hi[a] < lo[a]) return false;
-    }
+inline bool rect_of_corners(int W, int H, const Corner* const k[8], int rect[4]) {
     double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300, zmin = 1e300, zmax = -1e300;
     bool behind = false;
-    for (int k = 0; k < 8; ++k) {
-        double p[3] = {(k & 1) ? hi[0] : lo[0], (k & 2) ? hi[1] : lo[1], (k & 4) ? hi[2] : lo[2]};
-        const double* M = ctx->M;
-        double X = M[0] * p[0] + M[1] * p[1] + M[2] * p[2] + M[3];
-        double Y = M[4] * p[0] + M[5] * p[1] + M[6] * p[2] + M[7];
-        double Z = M[8] * p[0] + M[9] * p[1] + M[10] * p[2] + M[11];
-        double Wc = M[12] * p[0] + M[13] * p[1] + M[14] * p[2] + M[15];
-        if (!(Wc > 1e-9)) { behind = true; continue; }
-        double xn = X / Wc, yn = Y / Wc, zn = Z / Wc;
-        xmin = std::min(xmin, xn); xmax = std::max(xmax, xn);
-        ymin = std::min(ymin, yn); ymax = std::max(ymax, yn);
-        zmin = std::min(zmin, zn); zmax = std::max(zmax, zn);
+    for (int i = 0; i < 8; ++i) {
+        if (k[i]->behind) { behind = true; continue; }
+        xmin = std::min(xmin, k[i]->xn); xmax = std::max(xmax, k[i]->xn);
+        ymin = std::min(ymin, k[i]->yn); ymax = std::max(ymax, k[i]->yn);
+        zmin = std::min(zmin, k[i]->zn); zmax = std::max(zmax, k[i]->zn);
     }
     int x0 = 0, x1 = W - 1, y0 = 0, y1 = H - 1;
     if (!behind) {
@@ -394,6 +399,50 @@ bool brick_rect(const vr_ctx* ctx, int bid, int rect[4]) {
     if (x1 < x0 || y1 < y0) return false;
     rect[0] = x0; rect[1] = y0; rect[2] = x1 - x0 + 1; rect[3] = y1 - y0 + 1;
     return true;
+}
+
+// Screen rectangle (view pixels, clipped) that holds every pixel whose ray can meet brick b.
+// Returns false if the brick is outside the frustum.
+bool brick_rect(const vr_ctx* ctx, int bid, int rect[4]) {
+    const CubeDesc& c = ctx->cube;
+    int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
+    double lo[3], hi[3];
+    for (int a = 0; a < 3; ++a) {
+        lo[a] = (double)b[a] * c.B[a];
+        hi[a] = std::min((double)(b[a] + 1) * c.B[a], (double)(c.N[a] - 1));
+        if (hi[a] < lo[a]) return false;
+    }
+    Corner k[8];
+    const Corner* kp[8];
+    for (int i = 0; i < 8; ++i) {
+        k[i] = project_corner(ctx->M, (i & 1) ? hi[0] : lo[0], (i & 2) ? hi[1] : lo[1], (i & 4) ? hi[2] : lo[2]);
+        kp[i] = &k[i];
+    }
+    return rect_of_corners(ctx->view.W, ctx->view.H, kp, rect);
+}
+
+// The same rectangles for many bricks of one view: neighbouring bricks share their corners (the upper face of brick b
+// is the lower face of brick b + 1, the last brick ends at N - 1), so the (G0+1)(G1+1)(G2+1) grid corners are projected
+// once (vr_render_sortlast: 1024 bricks of a C4 panel cost 8192 projections per call, 25 calls per frame).
+void project_corner_grid(const vr_ctx* ctx, std::vector<Corner>& grid) {
+    const CubeDesc& c = ctx->cube;
+    const int n0 = c.G[0] + 1, n1 = c.G[1] + 1, n2 = c.G[2] + 1;
+    grid.resize((size_t)n0 * n1 * n2);
+    auto at = [&](int a, int i) { return i < c.G[a] ? (double)i * c.B[a] : (double)(c.N[a] - 1); };   // = lo of brick i = hi of brick i - 1
+    size_t e = 0;
+    for (int iz = 0; iz < n2; ++iz)
+        for (int iy = 0; iy < n1; ++iy)
+            for (int ix = 0; ix < n0; ++ix) grid[e++] = project_corner(ctx->M, at(0, ix), at(1, iy), at(2, iz));
+}
+
+bool brick_rect_grid(const vr_ctx* ctx, const std::vector<Corner>& grid, int bid, int rect[4]) {
+    const CubeDesc& c = ctx->cube;
+    const int n0 = c.G[0] + 1, n1 = c.G[1] + 1;
+    const int b[3] = {bid % c.G[0], (bid / c.G[0]) % c.G[1], bid / (c.G[0] * c.G[1])};
+    const Corner* kp[8];
+    for (int i = 0; i < 8; ++i)
+        kp[i] = &grid[(size_t)(b[0] + (i & 1)) + (size_t)n0 * ((b[1] + ((i >> 1) & 1)) + (size_t)n1 * (b[2] + ((i >> 2) & 1)))];
+    return rect_of_corners(ctx->view.W, ctx->view.H, kp, rect);
 }
 
 // A context is bound to one device: make it current for the calling thread (a process may drive several GPUs).
@@ -964,8 +1013,8 @@ int vr_render_bricks(vr_ctx* ctx, int mode, const vr_partial* hp, int n, float t
     a.mode = mode; a.tau = mode == VR_MODE_EA ? tau : 2.f; a.skip = skip_level(ctx, a.mode, true); a.variant = pick_variant(ctx, a.mode, a.skip); a.dense = resolve_dense(ctx); a.ring = resolve_ring(ctx, a.mode);
     a.counters = ctx->d_counters;
     if (by_tiles) {
-        if ((rc = ensure_rays(ctx, 4))) return rc;
-        VR_CUDA(ctx, launch_mip_tiles(ctx->cube, ctx->view, ctx->M, a, ctx->d_partials, n, tiles, otiles, ctx->d_rays[4], s));
+        if ((rc = ensure_rays(ctx, vr_ctx::kPinSlots))) return rc;
+        VR_CUDA(ctx, launch_mip_tiles(ctx->cube, ctx->view, ctx->M, a, ctx->d_partials, n, tiles, otiles, ctx->d_rays[vr_ctx::kPinSlots], s));
         ctx->launches += (n > 0 && tiles > 0) ? 3 : 0;
         return VR_OK;
     }
@@ -988,12 +1037,18 @@ int vr_render_sortlast(vr_ctx* ctx, int mode, float tau, void* d_arena, size_t a
     const CubeDesc& c = ctx->cube;
     // S1: front-to-back list of the resident bricks that can contribute, with their screen rectangles (computed once)
     brick_keys(ctx, ctx->keys);
-    ctx->keyed.clear();
-    for (int bid = c.win_lo; bid < c.win_hi; ++bid) {
-        if (mode == VR_MODE_EA && ctx->opt_skip && !ctx->h_brick_active[bid]) continue;
-        ctx->keyed.emplace_back(ctx->keys[bid], bid);
+    {   // counting sort by key, bricks of equal key in ascending id (= the stable sort of vr_sort_bricks; keys are small
+        // non-negative integers, at most G0 + G1 + G2 + 3; no allocation once the scratch vectors have grown)
+        int kmax = 0;
+        for (int bid = c.win_lo; bid < c.win_hi; ++bid) kmax = std::max(kmax, ctx->keys[bid]);
+        ctx->key_count.assign((size_t)kmax + 2, 0);
+        auto live = [&](int bid) { return !(mode == VR_MODE_EA && ctx->opt_skip && !ctx->h_brick_active[bid]); };
+        for (int bid = c.win_lo; bid < c.win_hi; ++bid) if (live(bid)) ++ctx->key_count[ctx->keys[bid] + 1];
+        for (int k = 0; k <= kmax; ++k) ctx->key_count[k + 1] += ctx->key_count[k];
+        ctx->keyed.resize((size_t)ctx->key_count[kmax + 1]);
+        for (int bid = c.win_lo; bid < c.win_hi; ++bid) if (live(bid)) ctx->keyed[ctx->key_count[ctx->keys[bid]]++] = {ctx->keys[bid], bid};
     }
-    std::stable_sort(ctx->keyed.begin(), ctx->keyed.end());
+    project_corner_grid(ctx, ctx->corner_grid);
     // pinned slot
     const size_t cap_needed = ctx->keyed.size() + 1;
     if (ctx->pin_cap < cap_needed) {
@@ -1017,7 +1072,7 @@ int vr_render_sortlast(vr_ctx* ctx, int mode, float tau, void* d_arena, size_t a
     int n = 0, tiles = 0;
     for (const auto& kb : ctx->keyed) {
         int rect[4];
-        if (!brick_rect(ctx, kb.second, rect)) continue;                      // outside the frustum
+        if (!brick_rect_grid(ctx, ctx->corner_grid, kb.second, rect)) continue;   // outside the frustum
         PartialDev& d = v[n++];
         set_brick(d, ctx->cube, kb.second); d.x0 = rect[0]; d.y0 = rect[1]; d.w = rect[2]; d.h = rect[3]; d.tile0 = tiles;
         d.pitch = rect[2]; d.data = (char*)d_arena + off;
