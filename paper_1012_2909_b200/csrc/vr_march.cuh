@@ -343,7 +343,9 @@ struct Slot { float w[3]; int rc; bool idle; float v[8]; };   // one ray in flig
 
 // 7 CTAs per SM: 72 registers; an 8th CTA (64 registers) would shrink L1 to 28 KB and costs 10 % (measured)
 template <int MODE, int LAYOUT, bool GLOBAL, bool DENSE, bool REGS, typename VT = float>
-__global__ void __launch_bounds__(kThreads, REGS ? VR_REGS_CTAS : 7)
+// register ring: 5 CTAs per SM for MIP; emission-absorption has its fold phase, in which a warp keeps no load in flight, and
+// gains from a sixth CTA to cover it (C3 with a dense table 18.6 -> 17.5 ms; MIP is indifferent: 12.7 - 13.1 either way)
+__global__ void __launch_bounds__(kThreads, REGS ? (MODE == VR_MODE_EA ? VR_REGS_CTAS + 1 : VR_REGS_CTAS) : 7)
 render_ls_kernel(const __grid_constant__ CubeDesc c, const __grid_constant__ ViewDesc V,
                  const __grid_constant__ TFDesc T, const __grid_constant__ RenderArgs A,
                  const PartialDev* __restrict__ parts, int n_parts) {
