@@ -86,3 +86,39 @@ def test_streamed_host_cube_and_view_that_misses():
     assert np.array_equal(got, np.broadcast_to(np.array(bg, dtype=np.float32), got.shape))
     torch.cuda.synchronize()
     cube.close()
+
+
+def test_streamed_float16_cube_equals_the_oracle_on_the_dequantised_cube():
+    """Both halves of NEXT-4 together (O-16 + O-17): a cube stored as float16, kept in pinned host memory and
+    streamed through 2 of 5 slots, renders the oracle's two-level composite of the DEquantised cube, bit for bit."""
+    import torch
+    from paper_1012_2909_b200 import outofcore, vr, workloads as wl
+    from oracle import ovr
+    import helpers
+    from test_gpu_sortlast_sharded import _oracle_two_level
+    helpers.torch_cuda()
+    w, src = _scene()
+    W, H = w.frame
+    helpers.FORCED_OPTIONS.clear()
+    helpers.FORCED_OPTIONS[vr.OPT_VOXEL_TYPE] = vr.VOXEL_F16
+    try:
+        sc = helpers.Scene(w.dims, w.brick, gen={"seed": w.seed, "sources": src, "continuum": w.continuum})
+    finally:
+        helpers.FORCED_OPTIONS.clear()
+    vol = sc.oracle_volume()                                          # the values the device holds: float32(float16(v))
+    cube = outofcore.StreamedCube(w.dims, w.brick, n_slabs=5, n_slots=2, voxel_type=vr.VOXEL_F16)
+    cube.ingest_generated(w.seed, sources=src, continuum=w.continuum)
+    cb32, _ = vr.cube_layout_typed(w.dims, w.brick, vr.VOXEL_F32)
+    assert cube.host_bytes() < 0.6 * cb32                             # half the bytes on the host, too
+    bg = (0.05, 0.1, 0.2, 0.3)
+    for mode, omode, tau, tf in ((vr.MODE_EA, ovr.EA, 0.95, wl.tf_fog()), (vr.MODE_EA, ovr.EA, 0.99, wl.tf_src()),
+                                 (vr.MODE_MIP, ovr.MIP, 2.0, wl.tf_src())):
+        cube.set_transfer_function(*tf)
+        M = wl.perspective_camera(w.dims, w.frame, azimuth_deg=140.0)
+        got = cube.render(mode, M, W, H, w.step, bg=bg if mode == vr.MODE_EA else (-3.0, 0, 0, 0), tau=tau)
+        torch.cuda.synchronize()
+        got = got.cpu().numpy()
+        got = got if mode == vr.MODE_EA else got[..., 0]
+        want = _oracle_two_level(ovr, vol, M, W, H, w.step, omode, w.brick, w.brick_grid, cube.group_first, tf, tau, bg, -3.0)
+        assert np.array_equal(got, want), mode
+    cube.close()
