@@ -775,7 +775,7 @@ def main():
     if args.next_rows:
         return run_next_rows(args)
     if args.streamed:
-        print(json.dumps(run_streamed(w, args.mode, args.streamed, args.steps, args.warmup, local_rank, args.tf)))
+        print(json.dumps(run_streamed(w, args.mode, args.streamed, args.steps, args.warmup, local_rank, args.tf, args.voxel)))
         return 0
     slab = None
     if args.slab:
@@ -832,7 +832,7 @@ def main():
     return 0
 
 
-def run_streamed(w, mode_name, n_slots, steps, warmup, local_rank, tf_name=None):
+def run_streamed(w, mode_name, n_slots, steps, warmup, local_rank, tf_name=None, voxel="f32"):
     """SURVEY.md 8(f)-4 / PAPER.md line 19 (cubes "larger than a single machine memory limit"): the cube kept brick-major in
     pinned host memory, streamed per frame through `n_slots` device slots of one slab (whole z-layers of bricks) each
     (paper_1012_2909_b200/outofcore.py): host -> device copy of the next slab overlapping the render of the current one, one
@@ -842,7 +842,8 @@ def run_streamed(w, mode_name, n_slots, steps, warmup, local_rank, tf_name=None)
     torch.cuda.set_device(local_rank)
     grid_z = -(-w.dims[2] // w.brick[2])
     t0 = time.perf_counter()
-    cube = outofcore.StreamedCube(w.dims, w.brick, n_slabs=min(grid_z, 32), n_slots=n_slots, device=local_rank)
+    cube = outofcore.StreamedCube(w.dims, w.brick, n_slabs=min(grid_z, 32), n_slots=n_slots, device=local_rank,
+                                  voxel_type=vr.VOXEL_F16 if voxel == "f16" else vr.VOXEL_F32)
     cube.ingest_generated(w.seed, sources=wl.make_sources(w), zero_boxes=wl.make_zero_boxes(w), continuum=w.continuum)
     ingest_s = time.perf_counter() - t0
     mode = vr.MODE_EA if mode_name == "ea" else vr.MODE_MIP
@@ -859,7 +860,7 @@ def run_streamed(w, mode_name, n_slots, steps, warmup, local_rank, tf_name=None)
         if i >= warmup:
             times.append((time.perf_counter() - t0, cube.stats["h2d_bytes"] - before["h2d_bytes"], cube.stats["slabs_copied"] - before["slabs_copied"]))
     total_s = sum(t[0] for t in times)
-    out = {"config": {"workload": f"{w.name} streamed: {w.dims[0]}x{w.dims[1]}x{w.dims[2]} float32 cube in pinned host memory, "
+    out = {"config": {"workload": f"{w.name} streamed: {w.dims[0]}x{w.dims[1]}x{w.dims[2]} {'float16' if voxel == 'f16' else 'float32'} cube in pinned host memory, "
                                   f"{cube.n_slabs} slabs of whole brick layers through {cube.n_slots} device slots, {W}x{H} frame, "
                                   f"{'EA tf-' + (tf_name or w.tf) if mode_name == 'ea' else 'MIP'}, step {w.step}",
                       "host_gib": round(cube.host_bytes() / 2 ** 30, 2),
