@@ -4,7 +4,8 @@ rendering image cubes larger than a single machine memory limit", line 47: the W
 The paper spreads the sub-volumes over the memories of several GPUs and composites their images; one B200 can do
 the same IN TIME instead of in space.  The cube lives brick-major in pinned host memory, cut into slabs of whole
 z-layers of bricks (the slabs of paper_1012_2909_b200/sortlast.py); a small pool of device slots holds a few slabs at a time.
-Per frame the slabs that meet the frustum are taken in visibility order: the next slab is copied host -> device on
+Per frame the slabs that meet the frustum are visited one after the other (in alternating direction from frame to frame,
+so that the slabs the last frame left resident come first): the next slab is copied host -> device on
 a copy stream while the current one is rendered into its own premultiplied partial frame (`vr_render_bricks` +
 `vr_composite_bricks` on the resident window, `vr_set_brick_window`), and ONE `vr_fold_peers` launch folds the
 slabs' partial frames in the slabs' visibility order (`vr_sort_groups`) and adds the background - the very fold of
@@ -151,10 +152,16 @@ class StreamedCube:
             self.partials = {}
         main = torch.cuda.current_stream()
         needed, order = self._needed(mode, M, W, H, step)
-        for i, g in enumerate(needed):
-            window = needed[i:i + self.n_slots]                              # slabs that must not be evicted now
+        # The fold at the end takes the partial frames in visibility order whatever order they were rendered in, so the
+        # slabs are VISITED in the direction that meets the resident ones first: front to back on one frame, back to
+        # front on the next (visiting them the same way round every frame evicts each slab just before it is wanted again).
+        resident = {s["slab"] for s in self.slots}
+        back = needed[::-1]
+        seq = needed if sum(g in resident for g in needed[:self.n_slots]) >= sum(g in resident for g in back[:self.n_slots]) else back
+        for i, g in enumerate(seq):
+            window = seq[i:i + self.n_slots]                                 # slabs that must not be evicted now
             slot = self._prefetch(g, window)
-            for nxt in needed[i + 1:i + self.n_slots]:                       # copies of the next slabs overlap this render
+            for nxt in seq[i + 1:i + self.n_slots]:                          # copies of the next slabs overlap this render
                 self._prefetch(nxt, window)
             main.wait_event(slot["copied"])
             ctx = slot["ctx"]
