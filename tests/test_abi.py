@@ -56,3 +56,14 @@ def test_no_oracle_in_product_path():
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(import|from)\s+paper_1012_2909_b200", src, flags=re.M), f
             assert not re.search(r"#include\s+\"[^\"]*(?<!o)vr[_a-z]*\.(h|cuh)\"", src), f
+
+
+def test_binding_constants_match_the_header():
+    """Constants the binding repeats (ctypes cannot read macros) are the header's."""
+    from paper_1012_2909_b200 import vr
+    text = open(os.path.join(ROOT, "include", "vr.h")).read()
+    m = re.search(r"#define\s+VR_STATIC_MAX_PARTIALS\s+(\d+)", text)
+    assert m and int(m.group(1)) == vr.STATIC_MAX_PARTIALS
+    opts = dict(re.findall(r"(VR_OPT_[A-Z0-9_]+)\s*=\s*(\d+)", text))
+    for name, value in opts.items():
+        assert getattr(vr, name[3:]) == int(value), name
