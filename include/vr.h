@@ -307,8 +307,8 @@ int vr_reset_counters(vr_ctx* ctx, void* stream);
  *    cube); used by the lockstep marcher for emission-absorption with VR_OPT_DENSE 0 on layout 1.
  *    1 / -1 = on where it applies, 0 = off.
  *  VR_OPT_RING (default -1): where the lockstep marcher keeps the gathers in flight, 0 = a ring of
- *    cp.async slots in shared memory, 1 = registers; -1 = registers for MIP, and for emission-absorption
- *    unless the central ray runs mostly along x (layout 1; measured).
+ *    cp.async slots in shared memory, 1 = registers; -1 = registers on layout 1 (measured faster at every
+ *    view), the cp.async ring on layout 0.
  *  VR_OPT_VOXEL_TYPE (default 0): how voxels are stored in HBM (SURVEY.md 8(f)-4 "reduced-precision bricks"; PAPER.md
  *    line 19: cubes "larger than a single machine memory limit"): 0 = float32; 1 = float16, IEEE half precision,
  *    each voxel rounded to nearest even when the cube is uploaded / generated and converted back (exactly) when it is

@@ -342,20 +342,15 @@ int resolve_dense(const vr_ctx* ctx) {
 }
 
 // Lockstep marcher: gathers through registers (1) or through the cp.async ring in shared memory (0).
-// Measured over the C3 orbit with the final build (vr_march.cuh, REGS): MIP is faster with registers whatever the view
-// (12.9 vs 15.2 ms, mean of 12 azimuths); emission-absorption with a dense table is faster with the cp.async ring only
-// where the rays run mostly along x, the axis along which consecutive lines are contiguous (16.0 vs 17.0 ms), and with
-// registers elsewhere (18.6 vs 22.5 ms).
+// Measured over the C3 orbit with the final build (vr_march.cuh, REGS): the register ring is faster whatever the view, for
+// MIP (12.9 vs 15.2 ms, mean of 12 azimuths) and, since its emission-absorption instantiations take six CTAs per SM, for
+// emission-absorption with a dense table too (along x, where the cp.async ring used to win: 15.1 vs 16.0 ms; at 60 degrees
+// from x 16.6 vs 19.9).  The cp.async ring serves the row layout and VR_OPT_RING 0.
 int resolve_ring(const vr_ctx* ctx, int mode) {
+    (void)mode;
     if (ctx->cube.vtype == 1) return 1;                      // float16 voxels: plain loads only (vr_march_h.cu)
     if (ctx->opt_ring >= 0) return ctx->opt_ring;
-    if (ctx->cube.layout != 1) return 0;
-    if (mode == VR_MODE_MIP) return 1;
-    const double* Mi = ctx->Minv;
-    double pn[4], pf[4], d[3];
-    for (int r = 0; r < 4; ++r) { pn[r] = -Mi[4 * r + 2] + Mi[4 * r + 3]; pf[r] = Mi[4 * r + 2] + Mi[4 * r + 3]; }   // central pixel, near / far
-    for (int a = 0; a < 3; ++a) d[a] = std::fabs(pf[a] / pf[3] - pn[a] / pn[3]);
-    return (std::isfinite(d[0]) && d[0] > d[1] && d[0] > d[2]) ? 0 : 1;
+    return ctx->cube.layout == 1 ? 1 : 0;
 }
 
 TFDesc tf_desc(const vr_ctx* ctx) {

@@ -514,8 +514,9 @@ def test_config_c3_full_size_64gib(H, marcher):
     free, total = torch.cuda.mem_get_info()
     if free < 80e9:
         pytest.skip("needs ~70 GB of free HBM")
-    # two orbit frames: the central ray runs mostly along z on one (VR_OPT_RING resolves to the register ring)
-    # and across it on the other (cp.async ring); seeded hit pixels over the whole frame
+    # two orbit frames: the central ray runs mostly along z, the short axis of the micro-blocks, on one and along x on
+    # the other (the two extremes of the gather pattern; the library's ring form, registers on this layout, serves both -
+    # the cp.async form is compared with the oracle under the forced "v3s" / "v3d" plans); seeded hit pixels over the frame
     axes = _fullsize_check(H, wl.C3, block=12, n_random=0, frame_index=[0, 90], anchors=12, per_anchor=24)
     assert (axes[0] == 2) != (axes[1] == 2), axes
 
